@@ -1,0 +1,197 @@
+/*
+ * kc.h — C-ABI of the B200 (sm_100a) kinetic 2-NN certificate library (libkc.so).
+ *
+ * What it computes: the per-step exact 2-nearest-neighbour certificate maintenance of
+ * "Repair Entropy in Dynamic Geometric Nearest-Neighbour Structures" (arxiv/paper_2606_18314):
+ * for N moving points in d = 2 or 3 the certificate (nn_i, d1_i <= d2_i), the clearance
+ * c_i = d2_i - d1_i (Definition 1), the candidate repair frontier
+ * F = {i : c_i <= 4 eps} (Lemma 1; Algorithm 1 line 2), the
+ * normalised frontier entropy H(F) over the index cells (Definition 2), and the
+ * frontier-only repair against a resident uniform grid (Algorithm 1 lines 3-7).
+ *
+ * Conventions (all entry points):
+ *  - Pointers are DEVICE pointers owned by the caller unless the comment says "host".
+ *    The library never frees or keeps a caller pointer beyond the call's stream work.
+ *  - Positions are contiguous row-major float32 [N][d] (d = 2 or 3).  Indices are int32.
+ *    Outputs are indexed by the ORIGINAL point id.  nn2 (runner-up index) may be NULL.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call is
+ *    asynchronous on that stream; no call synchronises the host except kc_grid_info and
+ *    kc_fp32_probe, which say so.  Counts that one call produces and the next consumes
+ *    (|F|, eps_t) stay on the device.
+ *  - Arithmetic (north_star): squared distance
+ *    s = ((dx*dx)+(dy*dy))+(dz*dz) with separately rounded binary32 ops (no FMA, no FTZ);
+ *    the two smallest keys under the total order (s, j) (equal s: smaller index first);
+ *    d1 = sqrtf(s1), d2 = sqrtf(s2) correctly rounded, c = d2 - d1.  Only j = i is excluded;
+ *    coincident points are neighbours at distance 0.  N = 2 gives d2 = c = +inf, nn2 = -1.
+ *  - Errors: every function returns a kc_status.  KC_EINVAL for a bad argument (d not in {2,3},
+ *    N < 2, a required pointer NULL or misaligned, workspace too small ...); KC_ENOMEM when a
+ *    device allocation fails; KC_ECUDA when the CUDA runtime reports an error (text in
+ *    kc_last_error()); KC_EREBUILD when the resident grid cannot serve the call (not built yet,
+ *    N differs from the build, or a whole-set search is asked of an incrementally updated
+ *    grid) and the caller must call kc_grid_build / kc_cert_grid_rebuild first.
+ *    Non-finite coordinates are a precondition violation: no crash, unspecified certificates.
+ *  - There is no CPU fallback anywhere in this library.
+ */
+#ifndef KC_H_
+#define KC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    KC_OK = 0,
+    KC_EINVAL = -1,
+    KC_ENOMEM = -2,
+    KC_ECUDA = -3,
+    KC_EREBUILD = -4
+} kc_status;
+
+/* Uniform-grid geometry ("a uniform grid whose resolution is chosen so the mean
+ * cell occupancy is a small constant").  Cubic cells of width h; cell of x on axis a is
+ * clamp(floorf(fl(fl(x - lo[a]) * inv_h)), 0, G[a]-1); linear id = (kz*G[1] + ky)*G[0] + kx.
+ * Points outside the box are filed in the nearest boundary cell (the search stays exact). */
+typedef struct {
+    int32_t d;          /* 2 or 3 */
+    int32_t G[3];       /* cells per axis; G[2] = 1 when d = 2 */
+    float lo[3];        /* grid origin */
+    float h;            /* cell width */
+    float inv_h;        /* binary32 nearest to 1/h */
+} kc_geom;
+
+/* Opaque resident grid: library-owned device buffers sized at creation. */
+typedef struct kc_grid kc_grid;
+
+/* Host-side snapshot of the grid's device counters (kc_grid_info). */
+typedef struct {
+    int64_t n_points;    /* N of the last build */
+    int64_t n_cells;     /* G[0]*G[1]*G[2] */
+    int32_t c_occ;       /* C: cells holding >= 1 point at the current filing */
+    int32_t max_occ;     /* largest cell occupancy seen by the last build */
+    int32_t n_misfiled;  /* points re-filed into overflow chains since the last build */
+    int32_t built;       /* 1 once kc_grid_build has run */
+    int32_t dirty;       /* 1 once kc_frontier_repair has updated the grid since the build */
+    int32_t n_stragglers;/* queries of the last search that needed more than the solo rings */
+} kc_grid_info_t;
+
+/* ---- host utilities -------------------------------------------------------------------- */
+
+const char *kc_version(void);
+/* host; thread-local text of the last KC_ECUDA / KC_EINVAL raised on this thread. */
+const char *kc_last_error(void);
+
+/* host.  Geometry for a bounding box [lo, hi] (host float[3] each; entries beyond d ignored):
+ * the same G on every axis, the smallest integer with G^d >= ceil(N/occ) (occ = target mean
+ * occupancy, 2.0 in BASELINE.json's configs); h = max_a(hi[a]-lo[a])/G*(1+2^-20) evaluated in
+ * double and rounded once; inv_h = 1/h from the rounded h (reading A6 of PAPER.md:27).
+ * A degenerate box (all extents 0) gets h = 1. */
+kc_status kc_geom_from_bbox(int64_t N, int d, const float *lo, const float *hi, double occ,
+                            kc_geom *out);
+
+/* device.  Exact per-axis min / max of p: lo_hi[0..2] = min, lo_hi[3..5] = max (device float[6];
+ * unused axes 0).  For callers that refit the geometry to moved points. */
+kc_status kc_bbox(const float *p, int64_t N, int d, float *lo_hi, void *stream);
+
+/* ---- A0: Algorithm 1 line 1, eps_t = max_i ||p'_i - p_i|| ----------------- */
+/* eps_out: device float[1].  Each norm is sqrtf of the squared distance defined above. */
+kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d, float *eps_out,
+                              void *stream);
+
+/* ---- A1: exact all-pairs certificates ("exact N x N pass", Table 2) ---------- */
+/* Workspace the tiled kernel needs for (N, d), in bytes (host; 0 is possible). */
+size_t kc_cert_allpairs_workspace(int64_t N, int d);
+/* nn,d1,d2,c: device [N]; nn2 device [N] or NULL; workspace: device, >= the size above
+ * (may be NULL when that size is 0). */
+kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t *nn, int32_t *nn2, float *d1,
+                           float *d2, float *c, void *workspace, size_t workspace_bytes,
+                           void *stream);
+
+/* ---- NEXT #1: frontier oracle (PAPER.md:69 rtx_frontier_oracle) -------------------------- */
+/* Relabel the queries q[0..*nq) (device int32, distinct ids; *nq read on the device, at most
+ * nq_max) against ALL N points by tiled brute force, O(|q| N).  Results are written in place at
+ * the query ids (nn[q[k]] ...), other entries are untouched.  workspace: device scratch of at
+ * least kc_frontier_oracle_workspace(N, d, nq_max) bytes (NULL allowed when that is 0). */
+size_t kc_frontier_oracle_workspace(int64_t N, int d, int64_t nq_max);
+kc_status kc_frontier_oracle(const float *p, int64_t N, int d, const int32_t *q, const int32_t *nq,
+                             int64_t nq_max, int32_t *nn, int32_t *nn2, float *d1, float *d2,
+                             float *c, void *workspace, size_t workspace_bytes, void *stream);
+
+/* ---- A2/A3: uniform grid build and whole-set search (PAPER.md:27, :69 rtx_grid_rebuild) --- */
+/* Allocates every device buffer for up to N_max points on geometry *geom (host pointer,
+ * copied).  *out receives the handle.  Uses the current CUDA device. */
+kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom *geom);
+kc_status kc_grid_destroy(kc_grid *g);
+/* Bytes of device memory the grid holds (host). */
+size_t kc_grid_bytes(const kc_grid *g);
+
+/* A2: cell id per point, per-cell histogram, exclusive scan, scatter into cell-sorted arrays.
+ * After it the grid is resident at positions p (copied; p may be freed afterwards). */
+kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream);
+/* A3: certificates of all N points of a freshly built grid by the ring-expanding search
+ * (3^d block first, then wider Chebyshev rings; a query stops only when the distance to the
+ * nearest unscanned cell face, shrunk by a rounding slack, exceeds d2 — Corollary 1,
+ * PAPER.md:171-173; never a search cap).  KC_EREBUILD if the grid is not freshly built. */
+kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
+                              void *stream);
+/* A2 + A3 in one call: the O(N) rebuild strategy. */
+kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *nn, int32_t *nn2,
+                               float *d1, float *d2, float *c, void *stream);
+
+/* ---- A4: Algorithm 1 line 2, F = { i : c_i <= 4 eps } ----------------------- */
+/* eps: device float[1] (e.g. kc_max_displacement's output).  flags: device uint8[N] or NULL.
+ * F: device int32[N] (capacity N), filled with the frontier ids, ascending inside each block of
+ * 1024 ids, blocks in arbitrary order.  nF: device int32[1], set to |F|. */
+kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps, uint8_t *flags,
+                               int32_t *F, int32_t *nF, void *stream);
+
+/* ---- A5: Definition 2, H(F) over the grid's cells ------------------------ */
+/* F: device int32 list of DISTINCT point ids, *nF entries (device int32[1]), at most nF_max
+ * (host upper bound used only to size launches; pass N if unknown).  Cells are the grid's
+ * current filing; C counts cells occupied by any point.  Outputs (device): H double[1]
+ * (0 when |F| = 0 or C <= 1), m_cells int32[1] (cells the frontier meets, Theorem 3
+ * PAPER.md:187), C_occ int32[1]; m_cells / C_occ may be NULL. */
+kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF, int64_t nF_max,
+                              double *H, int32_t *m_cells, int32_t *C_occ, void *stream);
+
+/* ---- A6 + A7: Algorithm 1 lines 3-7 -------------------------------------- */
+/* Incremental update of the resident grid to positions p_new, then exact re-search of the
+ * frontier only.
+ *  movers: device int32 list of DISTINCT ids whose position differs from what the grid holds
+ *          (*n_movers on the device, at most n_movers_max), or NULL = every point may have
+ *          moved.  Movers keep their slot if their cell is unchanged; otherwise they are
+ *          tombstoned and re-filed into their new cell's overflow chain (line 3).
+ *  F, nF, nF_max: as for kc_frontier_entropy; the queries to recompute (lines 4-7).
+ *  nn, nn2, d1, d2, c: certificates, updated IN PLACE at the ids in F, untouched elsewhere.
+ * The search is the same unbounded ring search as A3, over sorted ranges and chains. */
+kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
+                             const int32_t *n_movers, int64_t n_movers_max, const int32_t *F,
+                             const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
+                             float *d1, float *d2, float *c, void *stream);
+
+/* ---- inspection (tests, reports) ---------------------------------------------------------- */
+/* Synchronises `stream`, copies the device counters to *out (host). */
+kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream);
+/* Copies one of the grid's int32 arrays into dst (device int32[capacity], caller-owned),
+ * asynchronously on `stream`; *count (host) receives the array length (KC_EINVAL if it exceeds
+ * capacity; dst may be NULL to query the length only).
+ *  what = 0: cell id of point i, int32[N]      (current filing)
+ *         1: cell_start, int32[n_cells+1]      (exclusive scan of the last build's histogram)
+ *         2: sorted_idx, int32[N]              (point id in each sorted slot; -1 = tombstone)
+ *         3: slot, int32[N]                    (sorted slot of point i; -1 = in an overflow chain)
+ *         4: counts, int32[n_cells]            (live occupancy per cell) */
+kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, int64_t capacity, int64_t *count,
+                         void *stream);
+
+/* ---- measurement helper ------------------------------------------------------------------- */
+/* Empirical FP32 lane-op rate: `blocks` x 256 threads each run `iters` rounds of 16
+ * independent non-fused FADD/FMUL chains; returns separately-rounded FP32 ops/s in *ops_per_s
+ * (host double).  Synchronises the stream.  Used only to report the A1 roofline peak. */
+kc_status kc_fp32_probe(int blocks, int iters, double *ops_per_s, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KC_H_ */

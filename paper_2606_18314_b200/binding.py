@@ -1,0 +1,334 @@
+"""Thin Python binding of libkc.so: same names as include/kc.h, argument marshalling only.
+
+Every function takes torch CUDA tensors (device memory) and passes ``data_ptr()`` plus the
+current torch stream through the C-ABI; every step of the path runs in the library's own CUDA
+kernels.  There is no CPU fallback: if libkc.so is missing or fails to load, importing any
+entry point raises ``RuntimeError``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+KC_OK, KC_EINVAL, KC_ENOMEM, KC_ECUDA, KC_EREBUILD = 0, -1, -2, -3, -4
+_STATUS = {0: "KC_OK", -1: "KC_EINVAL", -2: "KC_ENOMEM", -3: "KC_ECUDA", -4: "KC_EREBUILD"}
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libkc.so")
+
+EXPORTS = (
+    "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_max_displacement",
+    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_frontier_oracle_workspace",
+    "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
+    "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
+    "kc_frontier_repair", "kc_grid_info", "kc_grid_export", "kc_fp32_probe",
+)
+
+
+class KcError(RuntimeError):
+    def __init__(self, status, where, msg):
+        super().__init__(f"{where}: {_STATUS.get(status, status)} {msg}")
+        self.status = status
+
+
+class RebuildRequired(KcError):
+    pass
+
+
+class kc_geom(C.Structure):
+    _fields_ = [("d", C.c_int32), ("G", C.c_int32 * 3), ("lo", C.c_float * 3),
+                ("h", C.c_float), ("inv_h", C.c_float)]
+
+    @property
+    def n_cells(self):
+        return int(self.G[0]) * int(self.G[1]) * int(self.G[2])
+
+
+class kc_grid_info_t(C.Structure):
+    _fields_ = [("n_points", C.c_int64), ("n_cells", C.c_int64), ("c_occ", C.c_int32),
+                ("max_occ", C.c_int32), ("n_misfiled", C.c_int32), ("built", C.c_int32),
+                ("dirty", C.c_int32), ("n_stragglers", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libkc.so (fails loudly; never falls back to anything)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_18314_b200._build` "
+                           "(nvcc, sm_100a). There is no CPU fallback.")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, sz, ci = C.c_void_p, C.c_int64, C.c_size_t, C.c_int
+    L.kc_version.restype = C.c_char_p
+    L.kc_last_error.restype = C.c_char_p
+    L.kc_geom_from_bbox.argtypes = [i64, ci, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_double,
+                                    C.POINTER(kc_geom)]
+    L.kc_bbox.argtypes = [vp, i64, ci, vp, vp]
+    L.kc_max_displacement.argtypes = [vp, vp, i64, ci, vp, vp]
+    L.kc_cert_allpairs_workspace.restype = sz
+    L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
+    L.kc_cert_allpairs.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.kc_frontier_oracle_workspace.restype = sz
+    L.kc_frontier_oracle_workspace.argtypes = [i64, ci, i64]
+    L.kc_frontier_oracle.argtypes = [vp, i64, ci, vp, vp, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.kc_grid_create.argtypes = [C.POINTER(vp), i64, C.POINTER(kc_geom)]
+    L.kc_grid_destroy.argtypes = [vp]
+    L.kc_grid_bytes.restype = sz
+    L.kc_grid_bytes.argtypes = [vp]
+    L.kc_grid_build.argtypes = [vp, vp, i64, vp]
+    L.kc_cert_grid_search.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.kc_cert_grid_rebuild.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    L.kc_frontier_classify.argtypes = [vp, i64, vp, vp, vp, vp, vp]
+    L.kc_frontier_entropy.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
+    L.kc_frontier_repair.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
+    L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
+    L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
+    for name in EXPORTS:
+        fn = getattr(L, name)
+        if fn.restype is C.c_int:      # default restype: all kc_status functions
+            fn.restype = C.c_int
+    _lib = L
+    return L
+
+
+def _check(status, where):
+    if status != KC_OK:
+        msg = lib().kc_last_error().decode()
+        raise (RebuildRequired if status == KC_EREBUILD else KcError)(status, where, msg)
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _ptr(t, dtype=None, name="tensor"):
+    if t is None:
+        return C.c_void_p(0)
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name} must have dtype {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+def _pos(p, name="p"):
+    if p.dim() != 2 or p.shape[1] not in (2, 3):
+        raise ValueError(f"{name} must be (N, 2) or (N, 3)")
+    return _ptr(p, torch.float32, name), int(p.shape[0]), int(p.shape[1])
+
+
+@dataclass
+class Certs:
+    """Device certificate arrays of Definition 1, indexed by point id."""
+    nn: torch.Tensor
+    nn2: torch.Tensor
+    d1: torch.Tensor
+    d2: torch.Tensor
+    c: torch.Tensor
+
+    @staticmethod
+    def empty(N, device="cuda"):
+        return Certs(torch.empty(N, dtype=torch.int32, device=device),
+                     torch.empty(N, dtype=torch.int32, device=device),
+                     torch.empty(N, dtype=torch.float32, device=device),
+                     torch.empty(N, dtype=torch.float32, device=device),
+                     torch.empty(N, dtype=torch.float32, device=device))
+
+    def clone(self):
+        return Certs(self.nn.clone(), self.nn2.clone(), self.d1.clone(), self.d2.clone(), self.c.clone())
+
+    def _ptrs(self):
+        return (_ptr(self.nn, torch.int32, "nn"), _ptr(self.nn2, torch.int32, "nn2"),
+                _ptr(self.d1, torch.float32, "d1"), _ptr(self.d2, torch.float32, "d2"),
+                _ptr(self.c, torch.float32, "c"))
+
+
+# ------------------------------------------------------------------------------------------
+def kc_version() -> str:
+    return lib().kc_version().decode()
+
+
+def kc_geom_from_bbox(N, d, lo, hi, occ=2.0) -> kc_geom:
+    """Host: grid geometry of reading A6."""
+    lo3 = (C.c_float * 3)(*[float(x) for x in list(lo)[:3]] + [0.0] * (3 - len(list(lo)[:3])))
+    hi3 = (C.c_float * 3)(*[float(x) for x in list(hi)[:3]] + [0.0] * (3 - len(list(hi)[:3])))
+    g = kc_geom()
+    _check(lib().kc_geom_from_bbox(int(N), int(d), lo3, hi3, float(occ), C.byref(g)), "kc_geom_from_bbox")
+    return g
+
+
+def kc_bbox(p, out=None):
+    """Device bbox: returns a float32[6] CUDA tensor (min xyz, max xyz)."""
+    pp, N, d = _pos(p)
+    out = out if out is not None else torch.empty(6, dtype=torch.float32, device=p.device)
+    _check(lib().kc_bbox(pp, N, d, _ptr(out, torch.float32), _stream()), "kc_bbox")
+    return out
+
+
+def kc_geom_for(p, occ=2.0) -> kc_geom:
+    """Convenience: device bbox (one sync) then kc_geom_from_bbox."""
+    b = kc_bbox(p).cpu().numpy()
+    return kc_geom_from_bbox(p.shape[0], p.shape[1], b[:3], b[3:], occ)
+
+
+def kc_max_displacement(p, p2, eps_out=None):
+    """A0, Algorithm 1 line 1.  Returns the device float32[1] tensor eps_t."""
+    pp, N, d = _pos(p)
+    pq, N2, d2 = _pos(p2, "p2")
+    if (N, d) != (N2, d2):
+        raise ValueError("p and p2 must have the same shape")
+    eps_out = eps_out if eps_out is not None else torch.empty(1, dtype=torch.float32, device=p.device)
+    _check(lib().kc_max_displacement(pp, pq, N, d, _ptr(eps_out, torch.float32), _stream()),
+           "kc_max_displacement")
+    return eps_out
+
+
+_ws_cache = {}
+
+
+def _workspace(nbytes, device):
+    if nbytes == 0:
+        return None
+    key = str(device)
+    w = _ws_cache.get(key)
+    if w is None or w.numel() < nbytes:
+        w = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        _ws_cache[key] = w
+    return w
+
+
+def kc_cert_allpairs(p, out: Certs | None = None, workspace=None) -> Certs:
+    """A1: exact all-pairs certificates (Table 2)."""
+    pp, N, d = _pos(p)
+    out = out or Certs.empty(N, p.device)
+    need = lib().kc_cert_allpairs_workspace(N, d)
+    ws = workspace if workspace is not None else _workspace(need, p.device)
+    _check(lib().kc_cert_allpairs(pp, N, d, *out._ptrs(), _ptr(ws), ws.numel() if ws is not None else 0,
+                                  _stream()), "kc_cert_allpairs")
+    return out
+
+
+def kc_frontier_oracle(p, q, nq, certs: Certs, nq_max=None, workspace=None) -> Certs:
+    """NEXT #1 (PAPER.md:69 rtx_frontier_oracle): brute-force relabel of the ids in q."""
+    pp, N, d = _pos(p)
+    nq_max = int(q.numel() if nq_max is None else nq_max)
+    need = lib().kc_frontier_oracle_workspace(N, d, nq_max)
+    ws = workspace if workspace is not None else _workspace(need, p.device)
+    _check(lib().kc_frontier_oracle(pp, N, d, _ptr(q, torch.int32, "q"), _ptr(nq, torch.int32, "nq"),
+                                    nq_max, *certs._ptrs(), _ptr(ws),
+                                    ws.numel() if ws is not None else 0, _stream()), "kc_frontier_oracle")
+    return certs
+
+
+class Grid:
+    """Resident uniform grid (kc_grid handle).  Owns only the handle; arrays are the library's."""
+
+    def __init__(self, N_max: int, geom: kc_geom):
+        self.geom = geom
+        self.N_max = int(N_max)
+        h = C.c_void_p()
+        _check(lib().kc_grid_create(C.byref(h), self.N_max, C.byref(geom)), "kc_grid_create")
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().kc_grid_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    @property
+    def bytes(self) -> int:
+        return int(lib().kc_grid_bytes(self._h))
+
+    def info(self) -> kc_grid_info_t:
+        out = kc_grid_info_t()
+        _check(lib().kc_grid_info(self._h, C.byref(out), _stream()), "kc_grid_info")
+        return out
+
+    def export(self, what: int) -> torch.Tensor:
+        """One of the grid's int32 arrays (see kc_grid_export) copied into a new CUDA tensor."""
+        cnt = C.c_int64()
+        _check(lib().kc_grid_export(self._h, what, C.c_void_p(0), 0, C.byref(cnt), _stream()), "kc_grid_export")
+        out = torch.empty(cnt.value, dtype=torch.int32, device="cuda")
+        _check(lib().kc_grid_export(self._h, what, _ptr(out), cnt.value, C.byref(cnt), _stream()), "kc_grid_export")
+        return out
+
+
+def kc_grid_build(grid: Grid, p):
+    """A2: cell ids, histogram, scan, scatter."""
+    pp, N, d = _pos(p)
+    _check(lib().kc_grid_build(grid._h, pp, N, _stream()), "kc_grid_build")
+
+
+def kc_cert_grid_search(grid: Grid, out: Certs | None = None, N=None) -> Certs:
+    """A3 (Corollary 1): certificates of all points of a fresh grid."""
+    out = out or Certs.empty(N if N is not None else grid.N_max)
+    _check(lib().kc_cert_grid_search(grid._h, *out._ptrs(), _stream()), "kc_cert_grid_search")
+    return out
+
+
+def kc_cert_grid_rebuild(grid: Grid, p, out: Certs | None = None) -> Certs:
+    """A2 + A3: the O(N) rebuild strategy (PAPER.md:69 rtx_grid_rebuild)."""
+    pp, N, d = _pos(p)
+    out = out or Certs.empty(N, p.device)
+    _check(lib().kc_cert_grid_rebuild(grid._h, pp, N, *out._ptrs(), _stream()), "kc_cert_grid_rebuild")
+    return out
+
+
+def kc_frontier_classify(c, eps, flags=None, F=None, nF=None):
+    """A4, Algorithm 1 line 2.  eps: device float32[1].  Returns (flags, F, nF)."""
+    N = c.numel()
+    flags = flags if flags is not None else torch.empty(N, dtype=torch.uint8, device=c.device)
+    F = F if F is not None else torch.empty(N, dtype=torch.int32, device=c.device)
+    nF = nF if nF is not None else torch.empty(1, dtype=torch.int32, device=c.device)
+    _check(lib().kc_frontier_classify(_ptr(c, torch.float32, "c"), N, _ptr(eps, torch.float32, "eps"),
+                                      _ptr(flags, torch.uint8, "flags"), _ptr(F, torch.int32, "F"),
+                                      _ptr(nF, torch.int32, "nF"), _stream()), "kc_frontier_classify")
+    return flags, F, nF
+
+
+def kc_frontier_entropy(grid: Grid, F, nF, nF_max=None, out=None):
+    """A5, Definition 2.  Returns device tensors (H float64[1], m int32[1], C int32[1])."""
+    nF_max = int(F.numel() if nF_max is None else nF_max)
+    if out is None:
+        out = (torch.empty(1, dtype=torch.float64, device=F.device),
+               torch.empty(1, dtype=torch.int32, device=F.device),
+               torch.empty(1, dtype=torch.int32, device=F.device))
+    H, m, Cc = out
+    _check(lib().kc_frontier_entropy(grid._h, _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
+                                     _ptr(H, torch.float64, "H"), _ptr(m, torch.int32), _ptr(Cc, torch.int32),
+                                     _stream()), "kc_frontier_entropy")
+    return H, m, Cc
+
+
+def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_movers=None,
+                       nF_max=None, n_movers_max=None) -> Certs:
+    """A6 + A7, Algorithm 1 lines 3-7: update the grid, re-search F in place."""
+    pp, N, d = _pos(p_new, "p_new")
+    nF_max = int(F.numel() if nF_max is None else nF_max)
+    if movers is not None:
+        n_movers_max = int(movers.numel() if n_movers_max is None else n_movers_max)
+        if n_movers is None:
+            n_movers = torch.tensor([movers.numel()], dtype=torch.int32, device=p_new.device)
+    else:
+        n_movers_max = 0
+    _check(lib().kc_frontier_repair(grid._h, pp, N, _ptr(movers, torch.int32, "movers"),
+                                    _ptr(n_movers, torch.int32, "n_movers"), n_movers_max,
+                                    _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
+                                    *certs._ptrs(), _stream()), "kc_frontier_repair")
+    return certs
+
+
+def kc_fp32_probe(blocks=148 * 8, iters=20000) -> float:
+    out = C.c_double()
+    _check(lib().kc_fp32_probe(int(blocks), int(iters), C.byref(out), _stream()), "kc_fp32_probe")
+    return float(out.value)

@@ -1,0 +1,85 @@
+// kc_common.cuh — shared device helpers of libkc (CUDA side only; the CPU oracle shares nothing
+// with this file).  Arithmetic contract: include/kc.h ("Arithmetic"), north_star.
+#pragma once
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+
+#include "../../include/kc.h"
+
+#define KC_NOIDX 0x7fffffff
+
+namespace kc {
+
+void set_error(const char *fmt, ...);
+kc_status cuda_fail(cudaError_t e, const char *where);
+
+#define KC_CUDA(call)                                              \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return kc::cuda_fail(e_, #call);    \
+    } while (0)
+#define KC_LAUNCH_CHECK(name)                                      \
+    do {                                                           \
+        cudaError_t e_ = cudaGetLastError();                       \
+        if (e_ != cudaSuccess) return kc::cuda_fail(e_, name);     \
+    } while (0)
+
+// Squared distance, separately rounded binary32 ops in the fixed order ((dx*dx)+(dy*dy))+(dz*dz).
+// __f*_rn intrinsics are never contracted into FMA by nvcc (and the library is built -fmad=false).
+__device__ __forceinline__ float sqd2(float ax, float ay, float bx, float by)
+{
+    float dx = __fsub_rn(ax, bx), dy = __fsub_rn(ay, by);
+    return __fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy));
+}
+__device__ __forceinline__ float sqd3(float ax, float ay, float az, float bx, float by, float bz)
+{
+    float dx = __fsub_rn(ax, bx), dy = __fsub_rn(ay, by), dz = __fsub_rn(az, bz);
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
+// Running two smallest keys under the total order (s, j): equal s -> smaller index first.
+struct Top2 {
+    float s1, s2;
+    int j1, j2;
+    __device__ __forceinline__ void init()
+    {
+        s1 = CUDART_INF_F; s2 = CUDART_INF_F; j1 = KC_NOIDX; j2 = KC_NOIDX;
+    }
+    __device__ __forceinline__ void offer(float s, int j)
+    {
+        if (s < s1 || (s == s1 && j < j1)) {
+            s2 = s1; j2 = j1; s1 = s; j1 = j;
+        } else if (s < s2 || (s == s2 && j < j2)) {
+            s2 = s; j2 = j;
+        }
+    }
+    __device__ __forceinline__ void merge(const Top2 &o)
+    {
+        offer(o.s1, o.j1);
+        offer(o.s2, o.j2);
+    }
+};
+
+// Definition 1: d1 = sqrtf(s1), d2 = sqrtf(s2), c = d2 - d1.
+__device__ __forceinline__ void store_cert(const Top2 &t, int i, int32_t *nn, int32_t *nn2,
+                                           float *d1, float *d2, float *c)
+{
+    float a = __fsqrt_rn(t.s1), b = __fsqrt_rn(t.s2);
+    nn[i] = t.j1 == KC_NOIDX ? -1 : t.j1;
+    if (nn2) nn2[i] = t.j2 == KC_NOIDX ? -1 : t.j2;
+    d1[i] = a;
+    d2[i] = b;
+    c[i] = __fsub_rn(b, a);
+}
+
+// Cell coordinate on one axis (kc_geom comment): clamp(floorf(fl(fl(x - lo) * inv_h)), 0, G-1).
+__device__ __forceinline__ int cell_axis(float x, float lo, float inv_h, int G)
+{
+    float t = __fmul_rn(__fsub_rn(x, lo), inv_h);
+    float f = floorf(t);
+    int k = f < 0.0f ? 0 : (f > (float)(G - 1) ? G - 1 : (int)f);
+    return k;
+}
+
+}  // namespace kc

@@ -1,0 +1,741 @@
+// kc_grid.cu — the resident uniform grid: A2 build, A3 whole-set ring search, A5 frontier
+// entropy, A6 incremental cell update, A7 frontier-only repair.  Contract: include/kc.h.
+//
+// Layout in HBM (N points, C_tot cells):
+//   cell[N]        int32   current filing cell of point i
+//   rank[N]        int32   arrival rank inside its cell at build time (scratch of the build)
+//   counts[C_tot]  int32   live occupancy per cell (histogram, kept current by A6)
+//   cell_start[C_tot+1] int32  exclusive scan of the build histogram
+//   spos2[N] float2 (d=2) / spos4[N] float4 = (x,y,z,bits(idx)) (d=3)   cell-sorted positions
+//   sidx[N]        int32   point id per sorted slot (-1 = tombstone)
+//   slot[N]        int32   sorted slot of point i (-1 = lives in an overflow chain)
+//   head[C_tot], next[N], opos[N] float4, mlist[N]   overflow chains of re-filed points (A6)
+//   fcount[C_tot], mhist[]  scratch of A5 (always left zeroed)
+// Rows of cells along x are contiguous in the sorted arrays (linear id has x fastest), so a
+// (2r+1)-cell row segment is ONE contiguous candidate range: two cell_start reads per row.
+#include <new>
+
+#include "kc_common.cuh"
+
+using namespace kc;
+
+namespace {
+
+constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
+
+struct Counters {
+    int n_misfiled;
+    int c_occ;
+    int max_occ;
+    int n_stragglers;
+    int m_cells;
+    int pad[3];
+    double big;               // sum k ln k over cells with k >= MHIST (rare)
+};
+
+struct View {
+    int G0, G1, G2;
+    float lo0, lo1, lo2, h, inv_h, shrink;
+    const int32_t *cell_start;
+    const float2 *spos2;
+    const float4 *spos4;
+    const int32_t *sidx;
+    const int32_t *head;
+    const int32_t *next;
+    const float4 *opos;
+};
+
+}  // namespace
+
+struct kc_grid {
+    kc_geom geom;
+    int64_t N_max, n_cells, N;
+    int built, dirty;
+    size_t bytes;
+    int32_t *cell, *rank, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
+    int32_t *blocksums;
+    float2 *spos2;
+    float4 *spos4, *opos;
+    Counters *ctr;
+    int n_scan_blocks;
+};
+
+namespace {
+
+constexpr int SCAN_CHUNK = 2048;   // cells per scan block (256 threads x 8)
+
+View make_view(const kc_grid *g)
+{
+    View v;
+    v.G0 = g->geom.G[0]; v.G1 = g->geom.G[1]; v.G2 = g->geom.G[2];
+    v.lo0 = g->geom.lo[0]; v.lo1 = g->geom.lo[1]; v.lo2 = g->geom.lo[2];
+    v.h = g->geom.h; v.inv_h = g->geom.inv_h;
+    int Gm = v.G0 > v.G1 ? v.G0 : v.G1;
+    if (v.G2 > Gm) Gm = v.G2;
+    // rounding slack of the ring bound: computed cell faces are off by O(u*G) cell widths
+    v.shrink = 1.0f - (1.0f / 512.0f + (float)Gm * (1.0f / 524288.0f));
+    v.cell_start = g->cell_start;
+    v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
+    v.head = g->head; v.next = g->next; v.opos = g->opos;
+    return v;
+}
+
+// ------------------------------------------------------------------ A2 build
+__global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
+                                    int32_t *head, const Counters *ctr)
+{
+    int n = ctr->n_misfiled;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
+        head[cell[mlist[e]]] = -1;
+}
+__global__ void reset_counters_kernel(Counters *ctr, int full)
+{
+    ctr->n_misfiled = 0;
+    if (full) { ctr->c_occ = 0; ctr->max_occ = 0; }
+    ctr->n_stragglers = 0;
+}
+
+template <int D>
+__device__ __forceinline__ int cell_of(const View &v, float x, float y, float z)
+{
+    int kx = cell_axis(x, v.lo0, v.inv_h, v.G0);
+    int ky = cell_axis(y, v.lo1, v.inv_h, v.G1);
+    int kz = D == 3 ? cell_axis(z, v.lo2, v.inv_h, v.G2) : 0;
+    return (kz * v.G1 + ky) * v.G0 + kx;
+}
+
+template <int D>
+__global__ void __launch_bounds__(256)
+cellid_rank_kernel(View v, const float *__restrict__ p, int N, int32_t *__restrict__ cell,
+                   int32_t *__restrict__ rank, int32_t *counts)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float x, y, z = 0.f;
+    if (D == 2) {
+        float2 t = reinterpret_cast<const float2 *>(p)[i];
+        x = t.x; y = t.y;
+    } else {
+        x = p[3 * (int64_t)i]; y = p[3 * (int64_t)i + 1]; z = p[3 * (int64_t)i + 2];
+    }
+    int cidx = cell_of<D>(v, x, y, z);
+    cell[i] = cidx;
+    rank[i] = atomicAdd(&counts[cidx], 1);
+}
+
+__global__ void __launch_bounds__(256)
+scan_reduce_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *blocksums, Counters *ctr)
+{
+    int base = blockIdx.x * SCAN_CHUNK;
+    int sum = 0, occ = 0, mx = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        int idx = base + k * 256 + threadIdx.x;
+        int cnt = idx < n_cells ? counts[idx] : 0;
+        sum += cnt; occ += cnt > 0; mx = max(mx, cnt);
+    }
+    sum = __reduce_add_sync(0xffffffffu, sum);
+    occ = __reduce_add_sync(0xffffffffu, occ);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    __shared__ int s_sum[8], s_occ[8], s_mx[8];
+    int w = threadIdx.x >> 5;
+    if ((threadIdx.x & 31) == 0) { s_sum[w] = sum; s_occ[w] = occ; s_mx[w] = mx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int a = 0, b = 0, c = 0;
+        for (int k = 0; k < 8; ++k) { a += s_sum[k]; b += s_occ[k]; c = max(c, s_mx[k]); }
+        blocksums[blockIdx.x] = a;
+        if (b) atomicAdd(&ctr->c_occ, b);
+        atomicMax(&ctr->max_occ, c);
+    }
+}
+// exclusive scan of blocksums[0..nb) in place, one CTA of 1024 threads, carry across segments
+__global__ void __launch_bounds__(1024) scan_blocksums_kernel(int32_t *blocksums, int nb)
+{
+    __shared__ int wsum[32];
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < nb; base += 1024) {
+        int idx = base + threadIdx.x;
+        int v = idx < nb ? blocksums[idx] : 0;
+        int incl = v;
+        int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) wsum[w] = incl;
+        __syncthreads();
+        if (w == 0) {
+            int x = wsum[lane], xi = x;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                int t = __shfl_up_sync(0xffffffffu, xi, o);
+                if (lane >= o) xi += t;
+            }
+            wsum[lane] = xi - x;   // exclusive warp offsets
+        }
+        __syncthreads();
+        int carry = carry_s;
+        int excl = carry + wsum[w] + incl - v;
+        if (idx < nb) blocksums[idx] = excl;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = excl + v;
+        __syncthreads();
+    }
+}
+__global__ void __launch_bounds__(256)
+scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, const int32_t *__restrict__ blocksums,
+                  int32_t *__restrict__ cell_start, int N)
+{
+    // thread t owns 8 consecutive cells
+    int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
+    int v[8];
+    int tsum = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        v[k] = base + k < n_cells ? counts[base + k] : 0;
+        tsum += v[k];
+    }
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int incl = tsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __shared__ int wsum[8];
+    if (lane == 31) wsum[w] = incl;
+    __syncthreads();
+    int off = blocksums[blockIdx.x];
+    for (int k = 0; k < w; ++k) off += wsum[k];
+    int run = off + incl - tsum;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        if (base + k < n_cells) cell_start[base + k] = run;
+        run += v[k];
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[n_cells] = N;
+}
+
+template <int D>
+__global__ void __launch_bounds__(256)
+scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ cell,
+               const int32_t *__restrict__ rank, const int32_t *__restrict__ cell_start,
+               float2 *__restrict__ spos2, float4 *__restrict__ spos4, int32_t *__restrict__ sidx,
+               int32_t *__restrict__ slot)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    int s = cell_start[cell[i]] + rank[i];
+    if (D == 2) {
+        spos2[s] = reinterpret_cast<const float2 *>(p)[i];
+    } else {
+        spos4[s] = make_float4(p[3 * (int64_t)i], p[3 * (int64_t)i + 1], p[3 * (int64_t)i + 2],
+                               __int_as_float(i));
+    }
+    sidx[s] = i;
+    slot[i] = s;
+}
+
+// ------------------------------------------------------------------ A3 / A7 ring search
+// Exact top-2 of query (qx,qy,qz), excluding point id `self`, over the grid's sorted ranges and
+// (if chains) its overflow chains.  Corollary 1: the block is widened until
+// the second neighbour is provably enclosed.  After the Chebyshev-radius-r block around the
+// query's cell (cx,cy,cz) has been scanned, every unscanned point lies beyond one of the
+// block's faces that are interior to the grid (points outside the box are filed in boundary
+// cells, and clamping is non-expansive), so its distance is >= bound = min over those faces of
+// the query's distance to the face.  Stop only when s2 < (bound*shrink)^2, strictly; shrink
+// absorbs the O(u*G) error of computed faces.  No face left = whole grid scanned = stop.
+template <int D>
+__device__ __forceinline__ void scan_range(const View &v, int b, int e, float qx, float qy, float qz,
+                                           int self, Top2 &best)
+{
+    for (int t = b; t < e; ++t) {
+        if (D == 2) {
+            float2 c = v.spos2[t];
+            float s = sqd2(qx, qy, c.x, c.y);
+            if (s <= best.s2) {
+                int j = v.sidx[t];
+                if (j != self && j >= 0) best.offer(s, j);
+            }
+        } else {
+            float4 c = v.spos4[t];
+            float s = sqd3(qx, qy, qz, c.x, c.y, c.z);
+            if (s <= best.s2) {
+                int j = __float_as_int(c.w);
+                if (j != self && j >= 0) best.offer(s, j);
+            }
+        }
+    }
+}
+template <int D>
+__device__ __forceinline__ void scan_chain(const View &v, int cidx, float qx, float qy, float qz,
+                                           int self, Top2 &best)
+{
+    for (int e = v.head[cidx]; e >= 0; e = v.next[e]) {
+        float4 c = v.opos[e];
+        float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
+        if (s <= best.s2 && e != self) best.offer(s, e);
+    }
+}
+template <int D>
+__device__ __forceinline__ void scan_row(const View &v, bool chains, int rowbase, int x0, int x1,
+                                         float qx, float qy, float qz, int self, Top2 &best)
+{
+    int b = v.cell_start[rowbase + x0], e = v.cell_start[rowbase + x1 + 1];
+    scan_range<D>(v, b, e, qx, qy, qz, self, best);
+    if (chains)
+        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
+}
+
+template <int D>
+__device__ int ring_search(const View &v, bool chains, float qx, float qy, float qz, int self,
+                           Top2 &best)
+{
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    int r = 1;
+    // radius-1 block: all rows, full segments
+    {
+        int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
+        int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
+        int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y)
+                scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, x0, x1, qx, qy, qz, self, best);
+    }
+    for (;;) {
+        float bound = CUDART_INF_F;
+        if (cx - r >= 1) bound = fminf(bound, __fsub_rn(qx, __fadd_rn(v.lo0, __fmul_rn((float)(cx - r), v.h))));
+        if (cx + r < v.G0 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo0, __fmul_rn((float)(cx + r + 1), v.h)), qx));
+        if (cy - r >= 1) bound = fminf(bound, __fsub_rn(qy, __fadd_rn(v.lo1, __fmul_rn((float)(cy - r), v.h))));
+        if (cy + r < v.G1 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo1, __fmul_rn((float)(cy + r + 1), v.h)), qy));
+        if (D == 3) {
+            if (cz - r >= 1) bound = fminf(bound, __fsub_rn(qz, __fadd_rn(v.lo2, __fmul_rn((float)(cz - r), v.h))));
+            if (cz + r < v.G2 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo2, __fmul_rn((float)(cz + r + 1), v.h)), qz));
+        }
+        if (bound == CUDART_INF_F) break;                 // the block covers the whole grid
+        float bs = __fmul_rn(bound, v.shrink);
+        if (bs > 0.0f && best.s2 < __fmul_rn(bs, bs)) break;
+        ++r;
+        // ring r: shell rows get the full segment, inner rows only the two end cells
+        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
+        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y) {
+                int rowbase = (z * v.G1 + y) * v.G0;
+                bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
+                if (shell) {
+                    scan_row<D>(v, chains, rowbase, x0, x1, qx, qy, qz, self, best);
+                } else {
+                    if (cx - r >= 0) scan_row<D>(v, chains, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
+                    if (cx + r <= v.G0 - 1) scan_row<D>(v, chains, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                }
+            }
+    }
+    return r;
+}
+
+template <int D>
+__global__ void __launch_bounds__(128)
+search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
+{
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    float qx, qy, qz = 0.f;
+    int self;
+    if (D == 2) {
+        float2 q = v.spos2[s];
+        qx = q.x; qy = q.y; self = v.sidx[s];
+    } else {
+        float4 q = v.spos4[s];
+        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
+    }
+    Top2 best;
+    best.init();
+    int r = ring_search<D>(v, false, qx, qy, qz, self, best);
+    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    store_cert(best, self, nn, nn2, d1, d2, c);
+}
+
+template <int D>
+__global__ void __launch_bounds__(128)
+search_frontier_kernel(View v, const float *__restrict__ p_new, const int32_t *__restrict__ F,
+                       const int32_t *__restrict__ nF, Counters *ctr, int32_t *nn, int32_t *nn2,
+                       float *d1, float *d2, float *c)
+{
+    const int n = *nF;
+    const bool chains = ctr->n_misfiled > 0;
+    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
+        int i = F[f];
+        float qx = p_new[(int64_t)i * D], qy = p_new[(int64_t)i * D + 1];
+        float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
+        Top2 best;
+        best.init();
+        int r = ring_search<D>(v, chains, qx, qy, qz, i, best);
+        if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+        store_cert(best, i, nn, nn2, d1, d2, c);
+    }
+}
+
+// ------------------------------------------------------------------ A6 incremental update
+// Algorithm 1 line 3: "update cell_i in G for points that changed cell".
+// A mover whose cell is unchanged is overwritten in its sorted slot; one whose cell changed is
+// tombstoned (NaN coordinates: every comparison with NaN is false, so it is never selected) and
+// appended once to the misfiled list; misfiled points live in per-cell overflow chains that are
+// cleared and re-linked every call, O(#misfiled).
+template <int D>
+__global__ void __launch_bounds__(256)
+refresh_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__restrict__ movers,
+               const int32_t *__restrict__ n_movers, int32_t *cell, int32_t *slot, int32_t *sidx,
+               float2 *spos2, float4 *spos4, float4 *opos, int32_t *mlist, int32_t *counts,
+               Counters *ctr)
+{
+    const int n = movers ? *n_movers : N;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
+        int i = movers ? movers[k] : k;
+        float x = p_new[(int64_t)i * D], y = p_new[(int64_t)i * D + 1];
+        float z = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
+        int cnew = cell_of<D>(v, x, y, z);
+        int cold = cell[i];
+        int sl = slot[i];
+        if (sl >= 0) {
+            if (cnew == cold) {
+                if (D == 2) spos2[sl] = make_float2(x, y);
+                else spos4[sl] = make_float4(x, y, z, __int_as_float(i));
+                continue;
+            }
+            const float qnan = __int_as_float(0x7fc00000);
+            if (D == 2) spos2[sl] = make_float2(qnan, qnan);
+            else spos4[sl] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+            sidx[sl] = -1;
+            slot[i] = -1;
+            mlist[atomicAdd(&ctr->n_misfiled, 1)] = i;
+        }
+        opos[i] = make_float4(x, y, z, 0.f);
+        if (cnew != cold) {
+            cell[i] = cnew;
+            if (atomicSub(&counts[cold], 1) == 1) atomicSub(&ctr->c_occ, 1);
+            if (atomicAdd(&counts[cnew], 1) == 0) atomicAdd(&ctr->c_occ, 1);
+        }
+    }
+}
+__global__ void link_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
+                                   int32_t *head, int32_t *next, const Counters *ctr)
+{
+    int n = ctr->n_misfiled;
+    for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+        int i = mlist[e];
+        next[i] = atomicExch(&head[cell[i]], i);
+    }
+}
+
+// ------------------------------------------------------------------ A5 frontier entropy
+// Definition 2 with n = |F|, k = frontier points per cell:
+//   H = ( ln n - (1/n) sum_cells k ln k ) / ln C.
+// Counts are integers (atomics), the sum is taken over the histogram-of-counts M[k] in a fixed
+// order in double, so the result does not depend on atomic ordering.
+__global__ void __launch_bounds__(256)
+entropy_count_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF,
+                     const int32_t *__restrict__ cell, int32_t *fcount)
+{
+    int n = *nF;
+    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x)
+        atomicAdd(&fcount[cell[F[f]]], 1);
+}
+__global__ void __launch_bounds__(256)
+entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF,
+                       const int32_t *__restrict__ cell, int32_t *fcount, int32_t *mhist, Counters *ctr)
+{
+    int n = *nF;
+    int m_local = 0;
+    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
+        int k = atomicExch(&fcount[cell[F[f]]], 0);     // first visitor collects and re-zeroes
+        if (k > 0) {
+            ++m_local;
+            if (k < MHIST) atomicAdd(&mhist[k], 1);
+            else atomicAdd(&ctr->big, (double)k * log((double)k));
+        }
+    }
+    m_local = __reduce_add_sync(0xffffffffu, m_local);
+    if ((threadIdx.x & 31) == 0 && m_local) atomicAdd(&ctr->m_cells, m_local);
+}
+__global__ void __launch_bounds__(1024)
+entropy_finish_kernel(const int32_t *__restrict__ nF, int32_t *mhist, Counters *ctr, double *H,
+                      int32_t *m_cells, int32_t *C_occ)
+{
+    __shared__ double part[32];
+    double acc = 0.0;
+    for (int k = threadIdx.x; k < MHIST; k += 1024) {
+        int M = mhist[k];
+        if (M) {
+            if (k > 1) acc += (double)M * ((double)k * log((double)k));
+            mhist[k] = 0;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double S = ctr->big;
+        for (int w = 0; w < 32; ++w) S += part[w];
+        int n = *nF, C = ctr->c_occ;
+        double h = 0.0;
+        if (n > 0 && C > 1) h = (log((double)n) - S / (double)n) / log((double)C);
+        *H = h;
+        if (m_cells) *m_cells = ctr->m_cells;
+        if (C_occ) *C_occ = C;
+        ctr->m_cells = 0;
+        ctr->big = 0.0;
+    }
+}
+
+inline int blocks_for(int64_t n, int threads, int cap = 148 * 16)
+{
+    int64_t b = (n + threads - 1) / threads;
+    if (b < 1) b = 1;
+    return (int)(b < cap ? b : cap);
+}
+
+kc_status check_certs(const int32_t *nn, const float *d1, const float *d2, const float *c, const char *who)
+{
+    if (!nn || !d1 || !d2 || !c) {
+        set_error("%s: nn, d1, d2, c must be non-NULL", who);
+        return KC_EINVAL;
+    }
+    return KC_OK;
+}
+
+}  // namespace
+
+// ====================================================================== C-ABI
+extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom *geom)
+{
+    if (!out || !geom || N_max < 2 || N_max > 0x7ffffff0 || (geom->d != 2 && geom->d != 3) ||
+        geom->G[0] < 1 || geom->G[1] < 1 || geom->G[2] < 1 || !(geom->h > 0.f) || !(geom->inv_h > 0.f) ||
+        (geom->d == 2 && geom->G[2] != 1)) {
+        set_error("kc_grid_create: bad argument");
+        return KC_EINVAL;
+    }
+    int64_t n_cells = (int64_t)geom->G[0] * geom->G[1] * geom->G[2];
+    int Gm = geom->G[0] > geom->G[1] ? geom->G[0] : geom->G[1];
+    if (geom->G[2] > Gm) Gm = geom->G[2];
+    if (n_cells > 0x7ffffff0 || Gm > 131072) {
+        set_error("kc_grid_create: grid too large");
+        return KC_EINVAL;
+    }
+    kc_grid *g = new (std::nothrow) kc_grid();
+    if (!g) return KC_ENOMEM;
+    g->geom = *geom;
+    g->N_max = N_max; g->n_cells = n_cells; g->N = 0; g->built = 0; g->dirty = 0; g->bytes = 0;
+    g->n_scan_blocks = (int)((n_cells + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    bool ok = true;
+    auto alloc = [&](void **p, size_t bytes) {
+        *p = nullptr;
+        if (!ok) return;
+        if (cudaMalloc(p, bytes) != cudaSuccess) { ok = false; *p = nullptr; cudaGetLastError(); return; }
+        g->bytes += bytes;
+    };
+    size_t n = (size_t)N_max, nc = (size_t)n_cells;
+    alloc((void **)&g->cell, n * 4); alloc((void **)&g->rank, n * 4);
+    alloc((void **)&g->counts, nc * 4); alloc((void **)&g->cell_start, (nc + 1) * 4);
+    alloc((void **)&g->sidx, n * 4); alloc((void **)&g->slot, n * 4);
+    alloc((void **)&g->head, nc * 4); alloc((void **)&g->next, n * 4);
+    alloc((void **)&g->mlist, n * 4); alloc((void **)&g->fcount, nc * 4);
+    alloc((void **)&g->mhist, MHIST * 4);
+    alloc((void **)&g->blocksums, (size_t)g->n_scan_blocks * 4 + 4);
+    g->spos2 = nullptr; g->spos4 = nullptr;
+    if (geom->d == 2) alloc((void **)&g->spos2, n * sizeof(float2));
+    else alloc((void **)&g->spos4, n * sizeof(float4));
+    alloc((void **)&g->opos, n * sizeof(float4));
+    alloc((void **)&g->ctr, sizeof(Counters));
+    if (!ok) {
+        kc_grid_destroy(g);
+        set_error("kc_grid_create: device allocation failed");
+        return KC_ENOMEM;
+    }
+    // one-time initialisation (default stream, synchronous): chains empty, scratch zeroed
+    bool e = cudaMemset(g->head, 0xff, nc * 4) != cudaSuccess ||
+             cudaMemset(g->fcount, 0, nc * 4) != cudaSuccess ||
+             cudaMemset(g->mhist, 0, MHIST * 4) != cudaSuccess ||
+             cudaMemset(g->ctr, 0, sizeof(Counters)) != cudaSuccess ||
+             cudaDeviceSynchronize() != cudaSuccess;
+    if (e) {
+        kc_status s = cuda_fail(cudaGetLastError(), "kc_grid_create init");
+        kc_grid_destroy(g);
+        return s;
+    }
+    *out = g;
+    return KC_OK;
+}
+
+extern "C" kc_status kc_grid_destroy(kc_grid *g)
+{
+    if (!g) return KC_OK;
+    void *ptrs[] = {g->cell, g->rank, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
+                    g->mlist, g->fcount, g->mhist, g->blocksums, g->spos2, g->spos4, g->opos, g->ctr};
+    for (void *p : ptrs)
+        if (p) cudaFree(p);
+    delete g;
+    return KC_OK;
+}
+
+extern "C" size_t kc_grid_bytes(const kc_grid *g) { return g ? g->bytes : 0; }
+
+extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream)
+{
+    if (!g || !p || N < 2 || N > g->N_max || (reinterpret_cast<uintptr_t>(p) & 7)) {
+        set_error("kc_grid_build: bad argument (N must be in [2, N_max], p 8-byte aligned)");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    View v = make_view(g);
+    const int n = (int)N, nc = (int)g->n_cells;
+    // drop the overflow chains of the previous residency, then start from an empty histogram
+    clear_chains_kernel<<<blocks_for(g->N, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
+    reset_counters_kernel<<<1, 1, 0, st>>>(g->ctr, 1);
+    KC_CUDA(cudaMemsetAsync(g->counts, 0, (size_t)nc * 4, st));
+    if (g->geom.d == 2) cellid_rank_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->rank, g->counts);
+    else cellid_rank_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->rank, g->counts);
+    scan_reduce_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->ctr);
+    scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, g->n_scan_blocks);
+    scan_write_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->cell_start, n);
+    if (g->geom.d == 2)
+        scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+    else
+        scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+    KC_LAUNCH_CHECK("kc_grid_build");
+    g->N = N; g->built = 1; g->dirty = 0;
+    return KC_OK;
+}
+
+extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2,
+                                         float *c, void *stream)
+{
+    if (!g) { set_error("kc_cert_grid_search: NULL grid"); return KC_EINVAL; }
+    kc_status s = check_certs(nn, d1, d2, c, "kc_cert_grid_search");
+    if (s != KC_OK) return s;
+    if (!g->built || g->dirty) {
+        set_error("kc_cert_grid_search: grid is not freshly built");
+        return KC_EREBUILD;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    View v = make_view(g);
+    const int n = (int)g->N;
+    if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    KC_LAUNCH_CHECK("kc_cert_grid_search");
+    return KC_OK;
+}
+
+extern "C" kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *nn,
+                                          int32_t *nn2, float *d1, float *d2, float *c, void *stream)
+{
+    kc_status s = check_certs(nn, d1, d2, c, "kc_cert_grid_rebuild");
+    if (s != KC_OK) return s;
+    s = kc_grid_build(g, p, N, stream);
+    if (s != KC_OK) return s;
+    return kc_cert_grid_search(g, nn, nn2, d1, d2, c, stream);
+}
+
+extern "C" kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF,
+                                         int64_t nF_max, double *H, int32_t *m_cells, int32_t *C_occ,
+                                         void *stream)
+{
+    if (!g || !F || !nF || !H || nF_max < 0) {
+        set_error("kc_frontier_entropy: bad argument");
+        return KC_EINVAL;
+    }
+    if (!g->built) { set_error("kc_frontier_entropy: grid not built"); return KC_EREBUILD; }
+    cudaStream_t st = (cudaStream_t)stream;
+    int blocks = blocks_for(nF_max, 256, 148 * 8);
+    entropy_count_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount);
+    entropy_collect_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount, g->mhist, g->ctr);
+    entropy_finish_kernel<<<1, 1024, 0, st>>>(nF, g->mhist, g->ctr, H, m_cells, C_occ);
+    KC_LAUNCH_CHECK("kc_frontier_entropy");
+    return KC_OK;
+}
+
+extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
+                                        const int32_t *n_movers, int64_t n_movers_max, const int32_t *F,
+                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
+                                        float *d1, float *d2, float *c, void *stream)
+{
+    if (!g || !p_new || !F || !nF || nF_max < 0 || (movers && (!n_movers || n_movers_max < 0))) {
+        set_error("kc_frontier_repair: bad argument");
+        return KC_EINVAL;
+    }
+    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_repair");
+    if (s != KC_OK) return s;
+    if (!g->built || N != g->N) {
+        set_error("kc_frontier_repair: grid not built for this N");
+        return KC_EREBUILD;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    View v = make_view(g);
+    const int n = (int)N;
+    const int64_t nm = movers ? n_movers_max : N;
+    const int chain_blocks = blocks_for(g->dirty ? N : 1, 256, 148 * 4);
+    // line 3: unlink every chain, refresh positions / re-file cell changers, link again
+    if (g->dirty) clear_chains_kernel<<<chain_blocks, 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
+    if (nm > 0) {
+        int blocks = blocks_for(nm, 256, 148 * 16);
+        if (g->geom.d == 2)
+            refresh_kernel<2><<<blocks, 256, 0, st>>>(v, p_new, n, movers, n_movers, g->cell, g->slot, g->sidx,
+                                                      g->spos2, g->spos4, g->opos, g->mlist, g->counts, g->ctr);
+        else
+            refresh_kernel<3><<<blocks, 256, 0, st>>>(v, p_new, n, movers, n_movers, g->cell, g->slot, g->sidx,
+                                                      g->spos2, g->spos4, g->opos, g->mlist, g->counts, g->ctr);
+    }
+    link_chains_kernel<<<blocks_for(nm > 0 || g->dirty ? N : 1, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->next, g->ctr);
+    g->dirty = 1;
+    // lines 4-7: re-search the frontier only
+    if (nF_max > 0) {
+        int blocks = blocks_for(nF_max, 128, 148 * 32);
+        if (g->geom.d == 2)
+            search_frontier_kernel<2><<<blocks, 128, 0, st>>>(v, p_new, F, nF, g->ctr, nn, nn2, d1, d2, c);
+        else
+            search_frontier_kernel<3><<<blocks, 128, 0, st>>>(v, p_new, F, nF, g->ctr, nn, nn2, d1, d2, c);
+    }
+    KC_LAUNCH_CHECK("kc_frontier_repair");
+    return KC_OK;
+}
+
+extern "C" kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream)
+{
+    if (!g || !out) { set_error("kc_grid_info: bad argument"); return KC_EINVAL; }
+    Counters h;
+    KC_CUDA(cudaMemcpyAsync(&h, g->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    KC_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    out->n_points = g->N; out->n_cells = g->n_cells;
+    out->c_occ = h.c_occ; out->max_occ = h.max_occ; out->n_misfiled = h.n_misfiled;
+    out->built = g->built; out->dirty = g->dirty; out->n_stragglers = h.n_stragglers;
+    return KC_OK;
+}
+
+extern "C" kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, int64_t capacity,
+                                    int64_t *count, void *stream)
+{
+    if (!g || !count) { set_error("kc_grid_export: bad argument"); return KC_EINVAL; }
+    const int32_t *src = nullptr;
+    int64_t n = 0;
+    switch (what) {
+    case 0: src = g->cell; n = g->N; break;
+    case 1: src = g->cell_start; n = g->n_cells + 1; break;
+    case 2: src = g->sidx; n = g->N; break;
+    case 3: src = g->slot; n = g->N; break;
+    case 4: src = g->counts; n = g->n_cells; break;
+    default: set_error("kc_grid_export: unknown array %d", what); return KC_EINVAL;
+    }
+    *count = n;
+    if (!dst) return KC_OK;
+    if (capacity < n) { set_error("kc_grid_export: capacity %lld < %lld", (long long)capacity, (long long)n); return KC_EINVAL; }
+    KC_CUDA(cudaMemcpyAsync(dst, src, (size_t)n * 4, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return KC_OK;
+}

@@ -1,0 +1,309 @@
+// kc_misc.cu — host utilities, A0 max displacement, A4 frontier classify + compaction, bbox,
+// FP32 probe.  See include/kc.h for the contract of each entry point.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+
+#include "kc_common.cuh"
+
+namespace kc {
+
+static thread_local char g_err[512] = "";
+
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+kc_status cuda_fail(cudaError_t e, const char *where)
+{
+    set_error("CUDA error %d (%s) at %s", (int)e, cudaGetErrorString(e), where);
+    return KC_ECUDA;
+}
+
+}  // namespace kc
+
+using namespace kc;
+
+extern "C" const char *kc_version(void) { return "libkc 0.1 (sm_100a)"; }
+extern "C" const char *kc_last_error(void) { return g_err; }
+
+// ------------------------------------------------------------------ geometry (host, reading A6)
+extern "C" kc_status kc_geom_from_bbox(int64_t N, int d, const float *lo, const float *hi,
+                                       double occ, kc_geom *out)
+{
+    if (!out || !lo || !hi || N < 1 || (d != 2 && d != 3) || !(occ > 0.0)) {
+        set_error("kc_geom_from_bbox: bad argument");
+        return KC_EINVAL;
+    }
+    int64_t target = (int64_t)ceil((double)N / occ);
+    if (target < 1) target = 1;
+    int64_t G = 1;
+    for (;; ++G) {
+        int64_t v = G * G * (d == 3 ? G : 1);
+        if (v >= target) break;
+    }
+    if (G * G * (d == 3 ? G : 1) > (int64_t)0x7ffffff0) {
+        set_error("kc_geom_from_bbox: grid too large for int32 cell ids");
+        return KC_EINVAL;
+    }
+    double ext = 0.0;
+    for (int a = 0; a < d; ++a) ext = fmax(ext, (double)hi[a] - (double)lo[a]);
+    double hd = ext > 0.0 ? ext / (double)G * (1.0 + 1.0 / 1048576.0) : 1.0;
+    out->d = d;
+    out->G[0] = out->G[1] = (int32_t)G;
+    out->G[2] = d == 3 ? (int32_t)G : 1;
+    for (int a = 0; a < 3; ++a) out->lo[a] = a < d ? lo[a] : 0.0f;
+    out->h = (float)hd;
+    out->inv_h = (float)(1.0 / (double)out->h);
+    return KC_OK;
+}
+
+// ------------------------------------------------------------------ bbox
+// Non-negative-agnostic float min/max through order-preserving integer keys.
+__device__ __forceinline__ unsigned fkey(float f)
+{
+    unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float funkey(unsigned k)
+{
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+__global__ void bbox_init_kernel(unsigned *keys)
+{
+    int t = threadIdx.x;
+    if (t < 3) keys[t] = 0xffffffffu;      // running min key
+    else if (t < 6) keys[t] = 0u;          // running max key
+}
+template <int D>
+__global__ void __launch_bounds__(256) bbox_kernel(const float *__restrict__ p, int64_t N,
+                                                   unsigned *keys)
+{
+    unsigned mn[D], mx[D];
+#pragma unroll
+    for (int a = 0; a < D; ++a) { mn[a] = 0xffffffffu; mx[a] = 0u; }
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N;
+         i += (int64_t)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            unsigned k = fkey(p[i * D + a]);
+            mn[a] = min(mn[a], k);
+            mx[a] = max(mx[a], k);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+        mn[a] = __reduce_min_sync(0xffffffffu, mn[a]);
+        mx[a] = __reduce_max_sync(0xffffffffu, mx[a]);
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int a = 0; a < D; ++a) {
+            atomicMin(&keys[a], mn[a]);
+            atomicMax(&keys[3 + a], mx[a]);
+        }
+    }
+}
+__global__ void bbox_finish_kernel(unsigned *keys, int d)
+{
+    int t = threadIdx.x;
+    if (t < 6) {
+        float v = (t % 3) < d ? funkey(keys[t]) : 0.0f;
+        reinterpret_cast<float *>(keys)[t] = v;
+    }
+}
+
+extern "C" kc_status kc_bbox(const float *p, int64_t N, int d, float *lo_hi, void *stream)
+{
+    if (!p || !lo_hi || N < 1 || (d != 2 && d != 3)) {
+        set_error("kc_bbox: bad argument");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned *keys = reinterpret_cast<unsigned *>(lo_hi);
+    bbox_init_kernel<<<1, 32, 0, st>>>(keys);
+    int blocks = (int)((N + 255) / 256 < 148 * 8 ? (N + 255) / 256 : 148 * 8);
+    if (d == 2) bbox_kernel<2><<<blocks, 256, 0, st>>>(p, N, keys);
+    else bbox_kernel<3><<<blocks, 256, 0, st>>>(p, N, keys);
+    bbox_finish_kernel<<<1, 32, 0, st>>>(keys, d);
+    KC_LAUNCH_CHECK("kc_bbox");
+    return KC_OK;
+}
+
+// ------------------------------------------------------------------ A0 max displacement
+// eps_t = max_i sqrtf(s(p_i, p'_i)) (Algorithm 1 line 1).  sqrt is monotone and the
+// squared norms are non-negative, so the max is taken on the raw bits of s and one sqrt of the
+// winner is bit-identical to the max of the sqrts.
+__global__ void zero_u32_kernel(unsigned *x) { *x = 0u; }
+
+template <int D>
+__global__ void __launch_bounds__(256) maxdisp_kernel(const float *__restrict__ p,
+                                                      const float *__restrict__ p2, int64_t N,
+                                                      unsigned *out)
+{
+    // flat float4 view when the buffers allow it: consecutive floats, D-agnostic loads
+    float m = 0.0f;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        float s;
+        if (D == 2) {
+            float2 a = reinterpret_cast<const float2 *>(p)[i];
+            float2 b = reinterpret_cast<const float2 *>(p2)[i];
+            s = sqd2(b.x, b.y, a.x, a.y);
+        } else {
+            const float *a = p + i * 3, *b = p2 + i * 3;
+            s = sqd3(b[0], b[1], b[2], a[0], a[1], a[2]);
+        }
+        m = fmaxf(m, s);
+    }
+    unsigned k = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+    __shared__ unsigned sm[8];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = k;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        k = sm[threadIdx.x];
+        k = __reduce_max_sync(0xffu, k);
+        if (threadIdx.x == 0) atomicMax(out, k);
+    }
+}
+__global__ void sqrt_inplace_kernel(float *x) { *x = __fsqrt_rn(*x); }
+
+extern "C" kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d,
+                                         float *eps_out, void *stream)
+{
+    if (!p || !p2 || !eps_out || N < 1 || (d != 2 && d != 3) ||
+        (d == 2 && ((reinterpret_cast<uintptr_t>(p) | reinterpret_cast<uintptr_t>(p2)) & 7))) {
+        set_error("kc_max_displacement: bad argument (d=2 positions must be 8-byte aligned)");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned *out = reinterpret_cast<unsigned *>(eps_out);
+    zero_u32_kernel<<<1, 1, 0, st>>>(out);
+    int blocks = (int)((N + 255) / 256 < 148 * 8 ? (N + 255) / 256 : 148 * 8);
+    if (d == 2) maxdisp_kernel<2><<<blocks, 256, 0, st>>>(p, p2, N, out);
+    else maxdisp_kernel<3><<<blocks, 256, 0, st>>>(p, p2, N, out);
+    sqrt_inplace_kernel<<<1, 1, 0, st>>>(eps_out);
+    KC_LAUNCH_CHECK("kc_max_displacement");
+    return KC_OK;
+}
+
+// ------------------------------------------------------------------ A4 classify + compaction
+// F = { i : c_i <= 4 eps } (Algorithm 1 line 2); thr = fl(4*eps) is exact.
+// One block handles 1024 consecutive ids (4 per thread); ids are written ascending inside the
+// block's reserved range; blocks reserve ranges with one atomicAdd each.
+__global__ void __launch_bounds__(256) classify_kernel(const float *__restrict__ c, int64_t N,
+                                                       const float *__restrict__ eps,
+                                                       uint8_t *__restrict__ flags,
+                                                       int32_t *__restrict__ F, int32_t *nF)
+{
+    const float thr = __fmul_rn(4.0f, *eps);
+    const int64_t base = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) * 4;
+    unsigned bits = 0;
+    if (base + 3 < N) {
+        float4 v = *reinterpret_cast<const float4 *>(c + base);
+        bits = (v.x <= thr) | ((v.y <= thr) << 1) | ((v.z <= thr) << 2) | ((v.w <= thr) << 3);
+        if (flags)
+            *reinterpret_cast<uchar4 *>(flags + base) =
+                make_uchar4(bits & 1, (bits >> 1) & 1, (bits >> 2) & 1, (bits >> 3) & 1);
+    } else {
+        for (int k = 0; k < 4; ++k)
+            if (base + k < N) {
+                unsigned f = c[base + k] <= thr;
+                bits |= f << k;
+                if (flags) flags[base + k] = (uint8_t)f;
+            }
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int cnt = __popc(bits);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __shared__ int wsum[8];
+    __shared__ int bbase;
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
+        bbase = tot ? atomicAdd(nF, tot) : 0;
+    }
+    __syncthreads();
+    int pos = bbase + wsum[warp] + incl - cnt;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (bits & (1u << k)) F[pos++] = (int32_t)(base + k);
+}
+
+extern "C" kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps,
+                                          uint8_t *flags, int32_t *F, int32_t *nF, void *stream)
+{
+    if (!c || !eps || !F || !nF || N < 1 || N > 0x7fffffff) {
+        set_error("kc_frontier_classify: bad argument");
+        return KC_EINVAL;
+    }
+    if ((reinterpret_cast<uintptr_t>(c) & 15) || (flags && (reinterpret_cast<uintptr_t>(flags) & 3))) {
+        set_error("kc_frontier_classify: c must be 16-byte aligned, flags 4-byte aligned");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    zero_u32_kernel<<<1, 1, 0, st>>>(reinterpret_cast<unsigned *>(nF));
+    int64_t blocks = (N + 1023) / 1024;
+    classify_kernel<<<(unsigned)blocks, 256, 0, st>>>(c, N, eps, flags, F, nF);
+    KC_LAUNCH_CHECK("kc_frontier_classify");
+    return KC_OK;
+}
+
+// ------------------------------------------------------------------ FP32 probe
+// 16 independent dependent-chains per thread of alternating non-fused FMUL / FADD: the empirical
+// separately-rounded FP32 lane-op rate the A1 roofline is quoted against.
+__global__ void __launch_bounds__(256) fp32_probe_kernel(int iters, float *sink)
+{
+    float v[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = 1.0f + 1e-3f * (float)(threadIdx.x + k);
+    const float a = 1.0000001f, b = 1e-7f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = __fmul_rn(v[k], a);
+#pragma unroll
+        for (int k = 0; k < 16; ++k) v[k] = __fadd_rn(v[k], b);
+    }
+    float s = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) s += v[k];
+    if (s == 12345.678f) *sink = s;
+}
+
+extern "C" kc_status kc_fp32_probe(int blocks, int iters, double *ops_per_s, void *stream)
+{
+    if (!ops_per_s || blocks < 1 || iters < 1) {
+        set_error("kc_fp32_probe: bad argument");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    float *sink = nullptr;
+    KC_CUDA(cudaMalloc(&sink, sizeof(float)));
+    cudaEvent_t e0, e1;
+    KC_CUDA(cudaEventCreate(&e0));
+    KC_CUDA(cudaEventCreate(&e1));
+    fp32_probe_kernel<<<blocks, 256, 0, st>>>(iters, sink);   // warm-up
+    KC_CUDA(cudaEventRecord(e0, st));
+    fp32_probe_kernel<<<blocks, 256, 0, st>>>(iters, sink);
+    KC_CUDA(cudaEventRecord(e1, st));
+    KC_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    KC_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    *ops_per_s = (double)blocks * 256.0 * (double)iters * 32.0 / ((double)ms * 1e-3);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    return KC_OK;
+}

@@ -1,0 +1,281 @@
+"""GPU parity (B200): every C-ABI entry point against the CPU oracle, element by element,
+bit-exact for indices / flags / fp32 certificates, 1e-6 absolute for H (north_star)."""
+import json
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_18314_b200 import binding as kc
+from paper_2606_18314_b200 import workloads as wl
+
+from _util import assert_same, dev, geoms, host, ref_certs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    kc.lib()
+
+
+def scenes_small():
+    rng = np.random.default_rng(7)
+    out = {}
+    for n in (2, 3, 4, 5, 31, 32, 33, 127, 129):
+        for d in (2, 3):
+            out[f"rand{n}_d{d}"] = rng.random((n, d)).astype(np.float32)
+            out[f"lat{n}_d{d}"] = (rng.integers(0, 8, (n, d)) / 8.0).astype(np.float32)   # ties + duplicates
+    out["lattice2"] = wl.lattice_points(33, 2)
+    out["lattice3"] = wl.lattice_points(9, 3)
+    out["dups"] = np.repeat(rng.random((50, 3)).astype(np.float32), 3, axis=0)
+    out["onepoint"] = np.full((300, 2), 0.375, np.float32)
+    pts = (0.5 + 0.01 * rng.standard_normal((3000, 2))).astype(np.float32)
+    pts[1234] = (9.0, -7.0)
+    out["outlier2"] = pts
+    pts = (0.5 + 0.01 * rng.standard_normal((3000, 3))).astype(np.float32)
+    pts[17] = (3.0, 2.0, -4.0)
+    out["outlier3"] = pts
+    out["cfg1"] = wl.make_points("cfg1")
+    out["ragged5003_d2"] = wl.uniform_points(5003, 2, 21)
+    out["ragged4099_d3"] = wl.uniform_points(4099, 3, 22)
+    out["clusters3b"] = wl.cluster_points(6000, 3, 23, 32, 0.02)[0]
+    out["mix_d2"] = wl.mixture_points(9000, 2, 24, 16, 0.005)
+    out["mix_d3"] = wl.mixture_points(9000, 3, 25, 16, 0.005)
+    return out
+
+
+SMALL = scenes_small()
+
+
+@pytest.mark.parametrize("name", ["p1_scene2d.json", "p2_tie_scene.json", "p2b_scene3d.json"])
+def test_golden_scenes_on_gpu(golden_dir, name):
+    g = json.load(open(os.path.join(golden_dir, name)))
+    p = np.array(g["points"], np.float32)
+    for got in (kc.kc_cert_allpairs(dev(p)), kc.kc_cert_grid_rebuild(kc.Grid(len(p), geoms(p)[1]), dev(p))):
+        h = host(got)
+        assert h.nn.tolist() == g["nn"] and h.nn2.tolist() == g["nn2"]
+        assert ["%08x" % v for v in h.c.view(np.uint32)] == g["c_bits"]
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_allpairs_small(name):
+    p = SMALL[name]
+    assert_same(kc.kc_cert_allpairs(dev(p)), oracle.bruteforce_top2(p), what=name)
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_grid_rebuild_small(name):
+    p = SMALL[name]
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(p.shape[0], g_kc)
+    got = kc.kc_cert_grid_rebuild(grid, dev(p))
+    assert_same(got, oracle.bruteforce_top2(p), what=name)
+    # A2 index work, bit-exact: cell ids, histogram scan, permutation
+    cid = oracle.cell_ids(p, g_or)
+    assert np.array_equal(grid.export(0).cpu().numpy(), cid)
+    counts = np.bincount(cid, minlength=g_or.n_cells)
+    assert np.array_equal(grid.export(4).cpu().numpy(), counts)
+    start = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    assert np.array_equal(grid.export(1).cpu().numpy(), start)
+    sidx = grid.export(2).cpu().numpy()
+    slot = grid.export(3).cpu().numpy()
+    assert np.array_equal(np.sort(sidx), np.arange(p.shape[0]))
+    assert np.array_equal(sidx[slot], np.arange(p.shape[0]))
+    assert np.all(np.diff(cid[sidx]) >= 0)                      # slots are cell-sorted
+    info = grid.info()
+    assert info.c_occ == np.count_nonzero(counts) and info.max_occ == counts.max()
+
+
+@pytest.mark.parametrize("cfg,N", [("cfg2", 16000), ("cfg3", 16000), ("cfg4", 80000), ("cfg4", 262144),
+                                   ("cfg5_d2", 310000), ("cfg5_d3", 310000)])
+def test_allpairs_and_rebuild_configs(cfg, N):
+    p = wl.make_points(cfg, N=N)
+    want = ref_certs(p)
+    P = dev(p)
+    assert_same(kc.kc_cert_allpairs(P), want, what=f"allpairs {cfg} {N}")
+    grid = kc.Grid(N, geoms(p)[1])
+    assert_same(kc.kc_cert_grid_rebuild(grid, P), want, what=f"rebuild {cfg} {N}")
+
+
+def test_grid_with_points_outside_the_box():
+    # geometry fitted to the central half of the points: the rest is clamped into boundary cells
+    p = wl.uniform_points(20000, 3, 31)
+    g_or, g_kc = geoms(p, lo=np.full(3, 0.25, np.float32), hi=np.full(3, 0.75, np.float32))
+    grid = kc.Grid(p.shape[0], g_kc)
+    assert_same(kc.kc_cert_grid_rebuild(grid, dev(p)), oracle.bruteforce_top2(p), what="clamped")
+    assert np.array_equal(grid.export(0).cpu().numpy(), oracle.cell_ids(p, g_or))
+    p2 = wl.uniform_points(20000, 2, 32)
+    g_or, g_kc = geoms(p2, occ=0.5, lo=np.full(2, 0.4, np.float32), hi=np.full(2, 0.6, np.float32))
+    assert_same(kc.kc_cert_grid_rebuild(kc.Grid(p2.shape[0], g_kc), dev(p2)), oracle.bruteforce_top2(p2),
+                what="clamped2")
+
+
+@pytest.mark.parametrize("occ", [0.25, 1.0, 8.0, 64.0])
+def test_grid_any_occupancy(occ):
+    for d in (2, 3):
+        p = wl.mixture_points(12000, d, 40 + d, 8, 0.01)
+        grid = kc.Grid(p.shape[0], geoms(p, occ=occ)[1])
+        assert_same(kc.kc_cert_grid_rebuild(grid, dev(p)), oracle.bruteforce_top2(p), what=f"occ{occ} d{d}")
+
+
+def test_frontier_oracle_subset():
+    for cfg in ("cfg2", "cfg3"):
+        p = wl.make_points(cfg)
+        want = oracle.bruteforce_top2(p)
+        for nq in (1, 77, 5000):
+            q = np.sort(np.random.default_rng(nq).choice(p.shape[0], nq, replace=False)).astype(np.int32)
+            certs = kc.Certs.empty(p.shape[0])
+            for t in (certs.nn, certs.nn2):
+                t.fill_(-7)
+            for t in (certs.d1, certs.d2, certs.c):
+                t.fill_(-7.0)
+            kc.kc_frontier_oracle(dev(p), dev(q), dev(np.array([nq], np.int32)), certs)
+            assert_same(certs, want, idx=q, what=f"oracle {cfg} {nq}")
+            rest = np.setdiff1d(np.arange(p.shape[0]), q)
+            assert np.all(host(certs).nn[rest] == -7) and np.all(host(certs).c[rest] == -7.0)
+
+
+def test_max_displacement_and_classify():
+    for cfg in ("cfg1", "cfg2", "cfg3"):
+        for fam in wl.CONFIGS[cfg]["families"]:
+            p, mot = wl.make_scene(cfg, fam)
+            q, _ = mot.step(p)
+            eps = kc.kc_max_displacement(dev(p), dev(q))
+            want_eps = oracle.max_displacement(p, q)
+            assert eps.cpu().numpy().view(np.uint32)[0] == np.array([want_eps]).view(np.uint32)[0]
+            c = oracle.kdtree_top2(p).c
+            flags, F, nF = kc.kc_frontier_classify(dev(c), eps)
+            wf, wF = oracle.frontier(c, want_eps)
+            assert np.array_equal(flags.cpu().numpy(), wf)
+            n = int(nF.item())
+            assert n == wF.size
+            assert np.array_equal(np.sort(F[:n].cpu().numpy()), wF)
+    # ragged sizes and the inclusive threshold
+    for N in (1, 3, 4, 5, 1023, 1024, 1025, 4097):
+        c = np.random.default_rng(N).random(N).astype(np.float32)
+        e = np.float32(0.125)
+        c[0] = 0.5                                                # == 4*eps exactly: in F
+        flags, F, nF = kc.kc_frontier_classify(dev(c), dev(np.array([e])))
+        wf, wF = oracle.frontier(c, e)
+        assert np.array_equal(flags.cpu().numpy(), wf) and int(nF.item()) == wF.size
+        assert np.array_equal(np.sort(F[:wF.size].cpu().numpy()), wF)
+    z = kc.kc_max_displacement(dev(p), dev(p))
+    assert float(z.item()) == 0.0
+
+
+def test_entropy_matches_oracle():
+    rng = np.random.default_rng(5)
+    for cfg, N in (("cfg1", 1000), ("cfg2", 16000), ("cfg3", 16000), ("cfg5_d3", 50000)):
+        p = wl.make_points(cfg, N=N)
+        g_or, g_kc = geoms(p)
+        grid = kc.Grid(N, g_kc)
+        kc.kc_grid_build(grid, dev(p))
+        cid = oracle.cell_ids(p, g_or)
+        lists = [np.arange(N), np.zeros(0, np.int64), np.flatnonzero(cid == cid[0]),
+                 rng.choice(N, N // 10, replace=False), np.unique(cid, return_index=True)[1]]
+        for F in lists:
+            F = np.sort(F).astype(np.int32)
+            Fd = dev(F) if F.size else torch.zeros(1, dtype=torch.int32, device="cuda")
+            for rep in range(2):                                  # scratch must be left clean
+                H, m, C = kc.kc_frontier_entropy(grid, Fd, dev(np.array([F.size], np.int32)), nF_max=max(F.size, 1))
+                wH, wm, wC = oracle.entropy(cid, F, g_or.n_cells)
+                assert abs(float(H.item()) - wH) <= 1e-6, (cfg, F.size, float(H.item()), wH)
+                assert int(m.item()) == wm and int(C.item()) == wC
+                assert wm >= wC ** wH * (1 - 1e-9)                # Theorem 3
+
+
+def run_repair_steps(cfg, fam, N, steps, use_movers, frontier="lemma", **kw):
+    p, mot = wl.make_scene(cfg, fam, N=N, **kw)
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+    pre = ref_certs(p)
+    assert_same(certs, pre, what="pre")
+    for t in range(steps):
+        q, movers = mot.step(p)
+        Q = dev(q)
+        eps = kc.kc_max_displacement(dev(p), Q)
+        if frontier == "lemma":
+            flags, F, nF = kc.kc_frontier_classify(certs.c, eps)
+        elif frontier == "all":
+            F, nF = dev(np.arange(N, dtype=np.int32)), dev(np.array([N], np.int32))
+        else:                                                     # the mover list as the frontier (A12)
+            mv = movers if movers is not None else np.arange(N, dtype=np.int32)
+            F, nF = dev(mv), dev(np.array([mv.size], np.int32))
+        mv_d = dev(movers) if (use_movers and movers is not None and movers.size) else None
+        if use_movers and movers is not None and movers.size == 0:
+            mv_d, nmv = torch.zeros(1, dtype=torch.int32, device="cuda"), dev(np.array([0], np.int32))
+            kc.kc_frontier_repair(grid, Q, F, nF, certs, movers=mv_d, n_movers=nmv, n_movers_max=0)
+        else:
+            kc.kc_frontier_repair(grid, Q, F, nF, certs, movers=mv_d)
+        post = ref_certs(q)
+        n = int(nF.item())
+        Fh = np.sort(F[:n].cpu().numpy())
+        got = host(certs)
+        # O8: repaired entries equal the exact post-step certificates, bit for bit
+        assert_same(got, post, idx=Fh, what=f"{cfg}/{fam} step {t} repaired")
+        rest = np.setdiff1d(np.arange(N), Fh)
+        if frontier == "lemma":
+            # Lemma 1: nn of every skipped point is still exact; d1,d2,c keep pre-step values
+            assert np.array_equal(got.nn[rest], post.nn[rest])
+            assert_same(got, pre, idx=rest, what=f"{cfg}/{fam} step {t} untouched", nn2=False)
+        # entropy and cells on the updated filing
+        cid = oracle.cell_ids(q, g_or)
+        assert np.array_equal(grid.export(0).cpu().numpy(), cid)
+        H, m, C = kc.kc_frontier_entropy(grid, F, nF)
+        wH, wm, wC = oracle.entropy(cid, Fh.astype(np.int32), g_or.n_cells)
+        assert abs(float(H.item()) - wH) <= 1e-6 and int(m.item()) == wm and int(C.item()) == wC
+        # per-transition protocol (A13): next step starts from exact certificates
+        certs = kc.Certs(*(dev(x) for x in (post.nn, post.nn2, post.d1, post.d2, post.c)))
+        p, pre = q, post
+    info = grid.info()
+    return info
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", f) for f in wl.CONFIGS["cfg2"]["families"]] +
+                         [("cfg3", f) for f in wl.CONFIGS["cfg3"]["families"]])
+def test_repair_per_family(cfg, fam):
+    info = run_repair_steps(cfg, fam, 16000, 4, use_movers=True)
+    assert info.dirty == 1
+
+
+@pytest.mark.parametrize("d_cfg", ["cfg2", "cfg3"])
+def test_repair_long_run_chains_accumulate(d_cfg):
+    # 12 steps without a rebuild in between: misfiled points accumulate and move again
+    info = run_repair_steps(d_cfg, "walk", 6000, 12, use_movers=False, frontier="all")
+    assert info.n_misfiled > 500
+
+
+def test_repair_mover_list_as_frontier_cfg4_style():
+    for ball in (False, True):
+        for f in (0.001, 0.03, 1.0):
+            run_repair_steps("cfg4", "fraction", 40000, 2, use_movers=True, frontier="movers", fraction=f, ball=ball)
+
+
+def test_search_refused_on_dirty_grid():
+    p, mot = wl.make_scene("cfg1")
+    grid = kc.Grid(p.shape[0], geoms(p)[1])
+    with pytest.raises(kc.RebuildRequired):
+        kc.kc_cert_grid_search(grid, kc.Certs.empty(p.shape[0]))
+    certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+    q, _ = mot.step(p)
+    F = dev(np.arange(p.shape[0], dtype=np.int32))
+    kc.kc_frontier_repair(grid, dev(q), F, dev(np.array([p.shape[0]], np.int32)), certs)
+    assert_same(certs, oracle.bruteforce_top2(q), what="cfg1 full-frontier repair")
+    with pytest.raises(kc.RebuildRequired):
+        kc.kc_cert_grid_search(grid, certs)
+    with pytest.raises(kc.RebuildRequired):
+        kc.kc_frontier_repair(grid, dev(q[:500]), F, dev(np.array([10], np.int32)), certs)
+    assert_same(kc.kc_cert_grid_rebuild(grid, dev(q)), oracle.bruteforce_top2(q), what="rebuild after repair")
+
+
+def test_bbox_device():
+    p = (np.random.default_rng(1).standard_normal((10007, 3)) * 5).astype(np.float32)
+    b = kc.kc_bbox(dev(p)).cpu().numpy()
+    assert np.array_equal(b[:3], p.min(0)) and np.array_equal(b[3:], p.max(0))
+    lo, hi = oracle.bbox(p)
+    assert np.array_equal(b[:3], lo) and np.array_equal(b[3:], hi)
