@@ -1,0 +1,516 @@
+#!/usr/bin/env python
+"""bench.py — certified points/s of the whole hot path.
+
+    python bench.py --gpus 1 --steps K --warmup W            # this repo's CUDA path
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands
+
+A "step" is one maintenance transition p -> p' through every row of the hot path (max
+displacement, Lemma-1 classify, incremental repair, frontier entropy, O(N) grid rebuild, all-pairs
+certification) on BASELINE.json configs[1] (N=16,000, d=2, five motion families, eps=1e-3).
+Prints ONE JSON line (rank 0).  Details of every field: DESIGN.md §measurement.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_18314_b200 import workloads as wl  # noqa: E402
+
+METRIC = "certified_points_per_s"
+UNIT = "points/s"
+L2_FLUSH_BYTES = 256 << 20
+FP32_LANES = 148 * 128          # B200: 148 SMs x 128 FP32 lanes, one non-fused op / lane / clk
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def build_trajectories(cfg, n_per_family, seed_shift=0):
+    """Host-side positions for every family: {family: (list of (N,d) float32, list of movers)}."""
+    c = wl.CONFIGS[cfg]
+    out = {}
+    for fam in c["families"]:
+        p, mot = wl.make_scene(cfg, fam, seed=c["seed"] + 7919 * seed_shift)
+        ps, mv = [p], [None]
+        for _ in range(n_per_family):
+            q, movers = mot.step(ps[-1])
+            ps.append(q)
+            mv.append(movers)
+        out[fam] = (ps, mv)
+    return out
+
+
+def schedule(cfg, K):
+    """K steps split evenly (round-robin remainder) over the config's families, family by family."""
+    fams = wl.CONFIGS[cfg]["families"]
+    per = [K // len(fams) + (1 if i < K % len(fams) else 0) for i in range(len(fams))]
+    return fams, per
+
+
+# ------------------------------------------------------------------------------------------
+# CPU oracle arm (cpu_baseline and --impl reference): the oracle as it stands, never tuned.
+def oracle_step(oracle, p, q, pre_c, geom, brute_queries=None):
+    """The oracle's restatement of one step: O3, O4, O5+O6, and the certificates by definition
+    (brute force; a bounded query sample when asked)."""
+    eps = oracle.max_displacement(p, q)
+    flags, F = oracle.frontier(pre_c, eps)
+    cid = oracle.cell_ids(q, geom)
+    H, m, C = oracle.entropy(cid, F, geom.n_cells)
+    post = oracle.kdtree_top2(q)                                   # the O(N log N) exact relabel
+    bf = oracle.bruteforce_top2(q, queries=brute_queries)          # the O(N^2) definition
+    return post, bf, (float(eps), F.size, H)
+
+
+def run_oracle_arm(cfg, K, W, time_budget_s=None, pair_budget=1.5e11):
+    import oracle
+    oracle.build()
+    c = wl.CONFIGS[cfg]
+    N = c["N"]
+    fams, per = schedule(cfg, K)
+    nq = int(min(N, max(64, pair_budget // max(1, K * N))))
+    queries = None if nq >= N else np.sort(np.random.default_rng(0).choice(N, nq, replace=False)).astype(np.int32)
+    traj = build_trajectories(cfg, max(per) + W)
+    p0 = traj[fams[0]][0][0]
+    geom = oracle.geom_for(p0)
+    done, t_total = 0, 0.0
+    for fi, fam in enumerate(fams):
+        ps, _ = traj[fam]
+        pre = oracle.kdtree_top2(ps[0])
+        n_warm = W if fi == 0 else 0
+        for t in range(per[fi] + n_warm):
+            t0 = time.perf_counter()
+            post, bf, _ = oracle_step(oracle, ps[t], ps[t + 1], pre.c, geom, queries)
+            dt = time.perf_counter() - t0
+            pre = post
+            if t >= n_warm:
+                t_total += dt
+                done += 1
+            if time_budget_s is not None and t_total > time_budget_s:
+                break
+        if time_budget_s is not None and t_total > time_budget_s:
+            break
+    frac = 1.0 if queries is None else nq / N
+    sample = (f"{done} full steps of {cfg} (families {','.join(fams)} in order); per step: max displacement, "
+              f"Lemma-1 frontier, cell ids + entropy, k-d tree relabel of all {N} points, brute-force "
+              f"definition for {nq if queries is not None else N} of {N} query points")
+    # points certified per step by the O(N^2) definition, as in the GPU arm's all-pairs row
+    value = (N * frac) * done / t_total
+    return dict(value=value, steps=done, seconds=t_total, cores=oracle.num_procs(), sample=sample,
+                ms_per_step=1e3 * t_total / max(done, 1))
+
+
+# ------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        os.unlink(self.f.name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["no samples"])
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                    samples=len(sm), reasons=sorted(reasons))
+
+
+# ------------------------------------------------------------------------------------------
+def run_gpu_arm(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_18314_b200 import binding as kc
+    from paper_2606_18314_b200.driver import Maintainer, crossover_fraction
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    kc.lib()
+    dev = torch.device("cuda", local)
+    cfg, K, W = args.workload, args.steps, args.warmup
+    c = wl.CONFIGS[cfg]
+    N, d = c["N"], c["d"]
+    fams, per = schedule(cfg, K)
+    # replicas only: every rank runs its own seeded copy of the workload
+    traj = build_trajectories(cfg, 2 * max(per) + W, seed_shift=rank)
+    flush = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # device-resident inputs for `value`: every position array uploaded before the timed region
+    dev_traj = {f: [torch.from_numpy(p).to(dev) for p in traj[f][0][: per[i] + W + 1]] for i, f in enumerate(fams)}
+    dev_mv = {f: [None if m is None else torch.from_numpy(m).to(dev) for m in traj[f][1][: per[i] + W + 1]]
+              for i, f in enumerate(fams)}
+    maint = {f: Maintainer(dev_traj[f][0]) for f in fams}
+    torch.cuda.synchronize()
+
+    phase_sum = {ph: 0.0 for ph in ("maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs")}
+    fam_stats = {f: dict(steps=0, repair_ms=0.0, rebuild_ms=0.0, frontier=0, H=0.0) for f in fams}
+    step_events, phase_events = [], []
+    # warm-up (first family), untimed
+    for t in range(W):
+        maint[fams[0]].step(dev_traj[fams[0]][t + 1], movers=dev_mv[fams[0]][t + 1])
+    barrier()
+    sampler = ClockSampler(local)
+    launches0 = kc.kc_launch_count()
+    t_wall0 = time.perf_counter()
+    for fi, f in enumerate(fams):
+        off = W if fi == 0 else 0
+        for t in range(per[fi]):
+            flush.zero_()                                            # L2 flush between timed steps
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            res = maint[f].step(dev_traj[f][off + t + 1], movers=dev_mv[f][off + t + 1], time_phases=True)
+            e1.record()
+            step_events.append((e0, e1))
+            phase_events.append((f, res.phase_ms, res.nF.clone(), res.H.clone()))
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = kc.kc_launch_count() - launches0
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in step_events)
+    for f, ev, nF, H in phase_events:
+        pt = Maintainer.phase_times(ev)
+        for ph in phase_sum:
+            phase_sum[ph] += pt[ph]
+        s = fam_stats[f]
+        s["steps"] += 1; s["repair_ms"] += pt["repair"] + pt["classify"] + pt["maxdisp"]
+        s["rebuild_ms"] += pt["rebuild"]; s["frontier"] += int(nF.item()); s["H"] += float(H.item())
+    tmax = torch.tensor([dev_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    dev_ms_max = float(tmax.item())
+    value = N * K * world / (dev_ms_max * 1e-3)
+
+    # ---- end to end through the public API: pinned host inputs, H2D + step + D2H per step ----
+    host_next = {f: [torch.from_numpy(p).pin_memory() for p in traj[f][0]] for f in fams}
+    host_out = dict(nn=torch.empty(N, dtype=torch.int32).pin_memory(), d1=torch.empty(N).pin_memory(),
+                    d2=torch.empty(N).pin_memory(), c=torch.empty(N).pin_memory(),
+                    eps=torch.empty(1).pin_memory(), nF=torch.empty(1, dtype=torch.int32).pin_memory(),
+                    H=torch.empty(1, dtype=torch.float64).pin_memory())
+    bufs = [torch.empty(N, d, device=dev), torch.empty(N, d, device=dev)]
+    h2d = N * d * 4
+    d2h = 4 * N * 4 + 4 + 4 + 8
+    e2e_events = []
+    barrier()
+    k = 0
+    for fi, f in enumerate(fams):
+        base = per[fi] + (W if fi == 0 else 0)        # continue each family's trajectory
+        m = maint[f]
+        for t in range(per[fi]):
+            flush.zero_()
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            buf = bufs[k & 1]
+            k += 1
+            buf.copy_(host_next[f][base + t + 1], non_blocking=True)
+            mv = traj[f][1][base + t + 1]
+            mvd = None if mv is None else torch.from_numpy(mv).to(dev, non_blocking=True)
+            res = m.step(buf, movers=mvd)
+            host_out["nn"].copy_(res.rebuilt.nn, non_blocking=True)
+            host_out["d1"].copy_(res.rebuilt.d1, non_blocking=True)
+            host_out["d2"].copy_(res.rebuilt.d2, non_blocking=True)
+            host_out["c"].copy_(res.rebuilt.c, non_blocking=True)
+            host_out["eps"].copy_(res.eps, non_blocking=True)
+            host_out["nF"].copy_(res.nF, non_blocking=True)
+            host_out["H"].copy_(res.H, non_blocking=True)
+            e1.record()
+            e1.synchronize()                                         # the user reads the result here
+            e2e_events.append((e0, e1))
+    barrier()
+    e2e_ms = sum(a.elapsed_time(b) for a, b in e2e_events)
+    tmax = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    e2e_value = N * K * world / (float(tmax.item()) * 1e-3)
+
+    out = None
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        # ---- parity of the timed outputs against the CPU oracle (outside the timed region) ----
+        certified = verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams)
+        # ---- roofline of the dominant kernel (all-pairs; FP32 ALU bound) ----
+        ops_per_pair = 5 if d == 2 else 8
+        ap_ms = phase_sum["allpairs"] / K
+        achieved = N * (N - 1) * ops_per_pair / (ap_ms * 1e-3) / 1e12
+        sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        peak = FP32_LANES * sm_max * 1e6 / 1e12
+        probe = kc.kc_fp32_probe() / 1e12
+        roofline = dict(bound="alu", kernel="allpairs_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
+                        frac=achieved / peak, traffic=None,
+                        note=(f"{ops_per_pair} separately rounded FP32 ops per ordered pair (no FMA by contract); peak = "
+                              f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md); measured non-fused "
+                              f"FADD/FMUL chain rate {probe:.2f} Top/s; kernel share of step = "
+                              f"{phase_sum['allpairs'] / sum(phase_sum.values()):.2f}"),
+                        pairs_per_s=N * (N - 1) / (ap_ms * 1e-3), ms_per_launch=ap_ms, fp32_probe_tops=probe)
+        cpu = run_oracle_arm(cfg, K=30, W=0, time_budget_s=25.0)
+        cpu_baseline = dict(value=cpu["value"], unit=UNIT, cores=cpu["cores"], kind="oracle", sample=cpu["sample"],
+                            ms_per_step=cpu["ms_per_step"])
+        extras = {}
+        if not args.no_extras:
+            extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks)
+        families = {f: dict(steps=s["steps"], frontier_frac=s["frontier"] / max(1, s["steps"]) / N,
+                            H=s["H"] / max(1, s["steps"]),
+                            repair_path_ms=s["repair_ms"] / max(1, s["steps"]),
+                            rebuild_path_ms=s["rebuild_ms"] / max(1, s["steps"]),
+                            repair_over_rebuild=s["repair_ms"] / max(s["rebuild_ms"], 1e-12))
+                    for f, s in fam_stats.items()}
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": dev_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{cfg}: N={N}, d={d}, eps={c['eps']}, families {','.join(fams)} "
+                                   f"({'/'.join(map(str, per))} steps), grid occupancy 2, every step = A0,A4,A6+A7,A5,A2+A3,A1",
+                       "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
+                       "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
+                       "certified": certified},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+            "phases_ms_per_step": {ph: v / K for ph, v in phase_sum.items()},
+            "paths_points_per_s": {"allpairs": N / (phase_sum["allpairs"] / K * 1e-3),
+                                   "grid_rebuild": N / (phase_sum["rebuild"] / K * 1e-3),
+                                   "frontier_repair": N / ((phase_sum["repair"] + phase_sum["classify"] + phase_sum["maxdisp"]) / K * 1e-3)},
+            "families": families,
+            "wall_s_timed_region": t_wall,
+            "extras": extras,
+        }
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return out
+
+
+def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per_family=2):
+    """'Certified' = the outputs of the timed configuration equal the CPU oracle's bit for bit
+    (H within 1e-6).  Checked outside the timed region on the first transitions of every family;
+    raises on any mismatch."""
+    import oracle
+    N = wl.CONFIGS[cfg]["N"]
+    checked = 0
+    for f in fams:
+        ps, mvs = traj[f]
+        m = Maintainer(torch.from_numpy(ps[0]).to(dev))
+        g = oracle.geom_for(ps[0])
+        pre = oracle.bruteforce_top2(ps[0])
+        for t in range(steps_per_family):
+            q = ps[t + 1]
+            mv = None if mvs[t + 1] is None else torch.from_numpy(mvs[t + 1]).to(dev)
+            res = m.step(torch.from_numpy(q).to(dev), movers=mv)
+            torch.cuda.synchronize()
+            post = oracle.bruteforce_top2(q)
+            eps = oracle.max_displacement(ps[t], q)
+            flags, F = oracle.frontier(pre.c, eps)
+            ok = res.eps.cpu().numpy().view(np.uint32)[0] == np.array([eps]).view(np.uint32)[0]
+            ok &= int(res.nF.item()) == F.size
+            for name in ("nn", "nn2", "d1", "d2", "c"):
+                want = getattr(post, name)
+                for got in (res.rebuilt, res.certified):
+                    ok &= bool(np.array_equal(getattr(got, name).cpu().numpy().view(np.uint32), want.view(np.uint32)))
+                ok &= bool(np.array_equal(getattr(res.repaired, name).cpu().numpy().view(np.uint32)[F], want.view(np.uint32)[F]))
+            H, mm, C = oracle.entropy(oracle.cell_ids(q, g), F, g.n_cells)
+            ok &= abs(float(res.H.item()) - H) <= 1e-6 and int(res.m_cells.item()) == mm and int(res.C_occ.item()) == C
+            if not ok:
+                raise RuntimeError(f"parity failure against the CPU oracle: {cfg}/{f} step {t}")
+            pre = post
+            checked += 1
+    return f"{checked} transitions ({steps_per_family} per family) bit-exact vs CPU oracle, H within 1e-6"
+
+
+def _median_ms(torch, fn, reps, setup=None, flush=None):
+    ts = []
+    for _ in range(reps):
+        if setup is not None:
+            setup()
+        if flush is not None:
+            flush.zero_()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        fn()
+        e1.record()
+        e1.synchronize()
+        ts.append(e0.elapsed_time(e1))
+    return float(np.median(ts))
+
+
+def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
+    """Other configs, reported beside the headline (not part of `value`):
+    config 4 repair-vs-rebuild sweep (crossover per entropy class) and config 5 at scale."""
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    flush = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+    ex = {"hbm_peak_gbs": hbm, "hbm_peak_source": "measured" if "hbm_gbs" in peaks else "fallback"}
+    # ---------------- config 4: N=262,144, d=3, mover fraction sweep, scattered vs one ball
+    c4 = wl.CONFIGS["cfg4"]
+    N = c4["N"]
+    sweep = {}
+    for ball in (False, True):
+        rows = []
+        for f in wl.CFG4_FRACTIONS:
+            p, mot = wl.make_scene("cfg4", "fraction", fraction=f, ball=ball)
+            q, movers = mot.step(p)
+            P, Q, MV = (torch.from_numpy(x).to(dev) for x in (p, q, movers))
+            nMV = torch.tensor([movers.size], dtype=torch.int32, device=dev)
+            m = Maintainer(P, allpairs=False)
+            certs = m.certs.clone()
+            eps = torch.zeros(1, device=dev)
+            H = torch.zeros(1, dtype=torch.float64, device=dev)
+            mc = torch.zeros(1, dtype=torch.int32, device=dev)
+            Cc = torch.zeros(1, dtype=torch.int32, device=dev)
+
+            def reset():
+                kc.kc_grid_build(m.grid, P)
+
+            def repair():
+                kc.kc_max_displacement(P, Q, eps)
+                kc.kc_frontier_classify(certs.c, eps, m.flags, m.F, m.nF)
+                kc.kc_frontier_repair(m.grid, Q, MV, nMV, certs, movers=MV, n_movers=nMV)
+
+            def rebuild():
+                kc.kc_cert_grid_rebuild(m.grid, Q, m.other)
+
+            t_rep = _median_ms(torch, repair, 7, setup=reset, flush=flush)
+            t_reb = _median_ms(torch, rebuild, 7, flush=flush)
+            kc.kc_frontier_entropy(m.grid, MV, nMV, out=(H, mc, Cc))
+            lemma = int(m.nF.item())
+            rows.append(dict(f=f, movers=int(movers.size), repair_ms=t_rep, rebuild_ms=t_reb, H=float(H.item()),
+                             m_cells=int(mc.item()), lemma1_frontier_frac=lemma / N))
+            del m
+        fs = [r["f"] for r in rows]
+        sweep["ball" if ball else "scattered"] = dict(
+            rows=rows, crossover_f=crossover_fraction(fs, [r["repair_ms"] for r in rows], [r["rebuild_ms"] for r in rows]))
+    ex["cfg4_sweep"] = sweep
+    # ---------------- config 5: 4,194,304 points, rebuild + Lemma-1 repair; all-pairs at 2^20
+    for cfg in ("cfg5_d2", "cfg5_d3"):
+        c5 = wl.CONFIGS[cfg]
+        N, d = c5["N"], c5["d"]
+        p, mot = wl.make_scene(cfg)
+        q, _ = mot.step(p)
+        P, Q = torch.from_numpy(p).to(dev), torch.from_numpy(q).to(dev)
+        m = Maintainer(P, allpairs=False)
+        t_build = _median_ms(torch, lambda: kc.kc_grid_build(m.grid, Q), 5, flush=flush)
+        t_reb = _median_ms(torch, lambda: kc.kc_cert_grid_rebuild(m.grid, Q, m.other), 5, flush=flush)
+        info = m.grid.info()
+        kc.kc_cert_grid_rebuild(m.grid, P, m.certs)
+        eps = kc.kc_max_displacement(P, Q)
+        kc.kc_frontier_classify(m.certs.c, eps, m.flags, m.F, m.nF)
+        nF = int(m.nF.item())
+        certs = m.certs.clone()
+        t_rep = _median_ms(torch, lambda: kc.kc_frontier_repair(m.grid, Q, m.F, m.nF, certs), 3,
+                           setup=lambda: kc.kc_grid_build(m.grid, P), flush=flush)
+        # algorithmic bytes per point of the rebuild: positions read twice,
+        # cell+rank written and read, histogram + scan, sorted records, idx, slot, certificates
+        pos = 4 * d
+        rec = 8 if d == 2 else 16
+        cells_per_pt = m.grid.geom.n_cells / N
+        bpp = (pos + 8) + cells_per_pt * (4 + 4 + 4 + 4) + (pos + 8 + 4 + rec + 4 + 4) + (rec + (4 if d == 2 else 0) + 8 + 20)
+        n_ap = 1 << 20
+        PA = P[:n_ap].contiguous()
+        ap = kc.Certs.empty(n_ap, dev)
+        ws = torch.empty(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
+        t_ap = _median_ms(torch, lambda: kc.kc_cert_allpairs(PA, ap, ws), 2, flush=flush)
+        ops = 5 if d == 2 else 8
+        ex[cfg] = dict(N=N, grid_build_ms=t_build, rebuild_ms=t_reb, rebuild_points_per_s=N / (t_reb * 1e-3),
+                       rebuild_alg_bytes_per_point=bpp, rebuild_gbs=N * bpp / (t_reb * 1e-3) / 1e9,
+                       rebuild_frac_of_hbm=N * bpp / (t_reb * 1e-3) / 1e9 / hbm,
+                       max_cell_occupancy=int(info.max_occ), occupied_cells=int(info.c_occ),
+                       lemma1_frontier_frac=nF / N, repair_ms=t_rep, repair_points_per_s=nF / (t_rep * 1e-3),
+                       allpairs_N=n_ap, allpairs_ms=t_ap, allpairs_pairs_per_s=n_ap * (n_ap - 1) / (t_ap * 1e-3),
+                       allpairs_points_per_s=n_ap / (t_ap * 1e-3),
+                       allpairs_tflops=n_ap * (n_ap - 1) * ops / (t_ap * 1e-3) / 1e12)
+        del m
+    return ex
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the config 4 / config 5 side measurements")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    rank = int(os.environ.get("RANK", "0"))
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        r = run_oracle_arm(args.workload, args.steps, args.warmup)
+        c = wl.CONFIGS[args.workload]
+        line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT,
+                "n_gpus": args.gpus, "steps": r["steps"], "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": f"{args.workload}: N={c['N']}, d={c['d']}, eps={c['eps']} (CPU oracle arm)"},
+                "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                                 "sample": r["sample"]},
+                "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line), flush=True)
+        return
+    out = run_gpu_arm(args)
+    if out is not None:
+        print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

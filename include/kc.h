@@ -185,7 +185,10 @@ kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream);
 kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, int64_t capacity, int64_t *count,
                          void *stream);
 
-/* ---- measurement helper ------------------------------------------------------------------- */
+/* ---- measurement helpers ------------------------------------------------------------------ */
+/* host.  Number of CUDA kernels this library has launched in this process so far (bench.py
+ * reports the difference over its timed region as gpu_launches). */
+uint64_t kc_launch_count(void);
 /* Empirical FP32 lane-op rate: `blocks` x 256 threads each run `iters` rounds of 16
  * independent non-fused FADD/FMUL chains; returns separately-rounded FP32 ops/s in *ops_per_s
  * (host double).  Synchronises the stream.  Used only to report the A1 roofline peak. */

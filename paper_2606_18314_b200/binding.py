@@ -24,7 +24,7 @@ EXPORTS = (
     "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_grid_info", "kc_grid_export", "kc_fp32_probe",
+    "kc_frontier_repair", "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
 
@@ -91,6 +91,8 @@ def lib():
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
+    L.kc_launch_count.restype = C.c_uint64
+    L.kc_launch_count.argtypes = []
     for name in EXPORTS:
         fn = getattr(L, name)
         if fn.restype is C.c_int:      # default restype: all kc_status functions
@@ -326,6 +328,10 @@ def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_mo
                                     _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
                                     *certs._ptrs(), _stream()), "kc_frontier_repair")
     return certs
+
+
+def kc_launch_count() -> int:
+    return int(lib().kc_launch_count())
 
 
 def kc_fp32_probe(blocks=148 * 8, iters=20000) -> float:

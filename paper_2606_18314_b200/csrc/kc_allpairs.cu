@@ -186,6 +186,7 @@ kc_status launch(const float *p, int64_t N, const int32_t *q, const int32_t *nq_
         allpairs_kernel<D, 1><<<grid, AP_THREADS, 0, st>>>(p, N, q, nq_dev, nq, jchunk, part, nn, nn2, d1, d2, c);
     if (js > 1)
         allpairs_merge_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(part, nq, js, q, nq_dev, nn, nn2, d1, d2, c);
+    count_launches(js > 1 ? 2 : 1);
     KC_LAUNCH_CHECK("kc_cert_allpairs");
     return KC_OK;
 }

@@ -12,6 +12,7 @@
 namespace kc {
 
 void set_error(const char *fmt, ...);
+void count_launches(int n);   // host-side tally of kernel launches issued by the library
 kc_status cuda_fail(cudaError_t e, const char *where);
 
 #define KC_CUDA(call)                                              \

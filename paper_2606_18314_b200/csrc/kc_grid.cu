@@ -610,6 +610,7 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
         scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
     else
         scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+    count_launches(7);   // + one memset node
     KC_LAUNCH_CHECK("kc_grid_build");
     g->N = N; g->built = 1; g->dirty = 0;
     return KC_OK;
@@ -630,6 +631,7 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     const int n = (int)g->N;
     if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
     else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
     return KC_OK;
 }
@@ -658,6 +660,7 @@ extern "C" kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int
     entropy_count_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount);
     entropy_collect_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount, g->mhist, g->ctr);
     entropy_finish_kernel<<<1, 1024, 0, st>>>(nF, g->mhist, g->ctr, H, m_cells, C_occ);
+    count_launches(3);
     KC_LAUNCH_CHECK("kc_frontier_entropy");
     return KC_OK;
 }
@@ -684,6 +687,7 @@ extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t 
     const int chain_blocks = blocks_for(g->dirty ? N : 1, 256, 148 * 4);
     // line 3: unlink every chain, refresh positions / re-file cell changers, link again
     if (g->dirty) clear_chains_kernel<<<chain_blocks, 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
+    count_launches((g->dirty ? 1 : 0) + (nm > 0 ? 1 : 0) + 1 + (nF_max > 0 ? 1 : 0));
     if (nm > 0) {
         int blocks = blocks_for(nm, 256, 148 * 16);
         if (g->geom.d == 2)

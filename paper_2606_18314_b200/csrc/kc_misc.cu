@@ -1,5 +1,6 @@
 // kc_misc.cu — host utilities, A0 max displacement, A4 frontier classify + compaction, bbox,
 // FP32 probe.  See include/kc.h for the contract of each entry point.
+#include <atomic>
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
@@ -9,6 +10,9 @@
 namespace kc {
 
 static thread_local char g_err[512] = "";
+static std::atomic<unsigned long long> g_launches{0};
+
+void count_launches(int n) { g_launches.fetch_add((unsigned long long)n, std::memory_order_relaxed); }
 
 void set_error(const char *fmt, ...)
 {
@@ -29,6 +33,7 @@ using namespace kc;
 
 extern "C" const char *kc_version(void) { return "libkc 0.1 (sm_100a)"; }
 extern "C" const char *kc_last_error(void) { return g_err; }
+extern "C" uint64_t kc_launch_count(void) { return (uint64_t)g_launches.load(); }
 
 // ------------------------------------------------------------------ geometry (host, reading A6)
 extern "C" kc_status kc_geom_from_bbox(int64_t N, int d, const float *lo, const float *hi,
@@ -130,6 +135,7 @@ extern "C" kc_status kc_bbox(const float *p, int64_t N, int d, float *lo_hi, voi
     if (d == 2) bbox_kernel<2><<<blocks, 256, 0, st>>>(p, N, keys);
     else bbox_kernel<3><<<blocks, 256, 0, st>>>(p, N, keys);
     bbox_finish_kernel<<<1, 32, 0, st>>>(keys, d);
+    count_launches(3);
     KC_LAUNCH_CHECK("kc_bbox");
     return KC_OK;
 }
@@ -187,6 +193,7 @@ extern "C" kc_status kc_max_displacement(const float *p, const float *p2, int64_
     if (d == 2) maxdisp_kernel<2><<<blocks, 256, 0, st>>>(p, p2, N, out);
     else maxdisp_kernel<3><<<blocks, 256, 0, st>>>(p, p2, N, out);
     sqrt_inplace_kernel<<<1, 1, 0, st>>>(eps_out);
+    count_launches(3);
     KC_LAUNCH_CHECK("kc_max_displacement");
     return KC_OK;
 }
@@ -257,6 +264,7 @@ extern "C" kc_status kc_frontier_classify(const float *c, int64_t N, const float
     zero_u32_kernel<<<1, 1, 0, st>>>(reinterpret_cast<unsigned *>(nF));
     int64_t blocks = (N + 1023) / 1024;
     classify_kernel<<<(unsigned)blocks, 256, 0, st>>>(c, N, eps, flags, F, nF);
+    count_launches(2);
     KC_LAUNCH_CHECK("kc_frontier_classify");
     return KC_OK;
 }

@@ -1,0 +1,140 @@
+"""A8 step driver: one maintenance step of Algorithm 1 on the GPU, both ways.
+
+Per transition p -> p' (the per-transition protocol of reading A13: every step starts from exact
+certificates and a grid resident at p, like the paper's independently labelled transitions,
+PAPER.md:69-73):
+
+    A0  eps_t = max_i ||p'_i - p_i||                         kc_max_displacement   (Alg. 1 l.1)
+    A4  F = {i : c_i <= 4 eps_t}                             kc_frontier_classify  (Alg. 1 l.2)
+    A6+A7  REPAIR path: incremental cell update + search of F  kc_frontier_repair  (Alg. 1 l.3-7)
+    A5  H(F), m, C on the updated filing                     kc_frontier_entropy   (Def. 2)
+    A2+A3  REBUILD path: O(N) grid rebuild at p'             kc_cert_grid_rebuild
+    A1  all-pairs certification at p'                        kc_cert_allpairs
+
+This module is host orchestration only: every arithmetic step runs in libkc's kernels.  It owns
+the device buffers (torch tensors) and hands pointers to the C-ABI through :mod:`.binding`.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+
+import numpy as np
+import torch
+
+from . import binding as kc
+
+PHASES = ("maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs")
+
+
+@dataclass
+class StepResult:
+    """Device-side results of one step (no host sync was made to produce them)."""
+    eps: torch.Tensor          # float32[1]
+    nF: torch.Tensor           # int32[1]
+    H: torch.Tensor            # float64[1]
+    m_cells: torch.Tensor      # int32[1]
+    C_occ: torch.Tensor        # int32[1]
+    repaired: kc.Certs         # pre-step certificates with F re-searched (repair path); this buffer
+                               # is reused by the NEXT step's rebuild
+    rebuilt: kc.Certs          # exact certificates at p' from the grid rebuild
+    certified: kc.Certs | None # exact certificates at p' from the all-pairs pass
+    phase_ms: dict = field(default_factory=dict)
+
+
+class Maintainer:
+    """Resident state for N points: grid, certificates, frontier buffers."""
+
+    def __init__(self, p0: torch.Tensor, occ: float = 2.0, geom: kc.kc_geom | None = None,
+                 allpairs: bool = True):
+        assert p0.is_cuda and p0.dtype == torch.float32 and p0.dim() == 2
+        self.N, self.d = int(p0.shape[0]), int(p0.shape[1])
+        self.geom = geom if geom is not None else kc.kc_geom_for(p0, occ)
+        self.grid = kc.Grid(self.N, self.geom)
+        dev = p0.device
+        N = self.N
+        self.certs = kc.Certs.empty(N, dev)        # current exact certificates (pre-step)
+        self.other = kc.Certs.empty(N, dev)        # ping-pong partner: the rebuild writes here
+        self.ap = kc.Certs.empty(N, dev) if allpairs else None
+        self.flags = torch.empty(N, dtype=torch.uint8, device=dev)
+        self.F = torch.empty(N, dtype=torch.int32, device=dev)
+        self.nF = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.eps = torch.zeros(1, dtype=torch.float32, device=dev)
+        self.H = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.m = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.C = torch.zeros(1, dtype=torch.int32, device=dev)
+        need = kc.lib().kc_cert_allpairs_workspace(N, self.d) if allpairs else 0
+        self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+        self.p = p0
+        kc.kc_cert_grid_rebuild(self.grid, p0, self.certs)
+
+    def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None,
+             frontier: torch.Tensor | None = None, time_phases: bool = False,
+             do_allpairs: bool = True) -> StepResult:
+        """One transition p -> p_next through every row of the hot path.
+
+        ``movers``: optional int32 id list of the points that moved (None = all may have moved).
+        ``frontier``: optional int32 id list to repair instead of the Lemma-1 set (reading A12:
+        the sweep's controlled frontier is the mover list)."""
+        ev = {}
+
+        def mark(name):
+            if time_phases:
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                ev[name] = e
+
+        mark("t0")
+        kc.kc_max_displacement(self.p, p_next, self.eps)
+        mark("maxdisp")
+        if frontier is None:
+            kc.kc_frontier_classify(self.certs.c, self.eps, self.flags, self.F, self.nF)
+            F, nF, nF_max = self.F, self.nF, self.N
+        else:
+            kc.kc_frontier_classify(self.certs.c, self.eps, self.flags, self.F, self.nF)
+            F, nF_max = frontier, int(frontier.numel())
+            nF = torch.full((1,), nF_max, dtype=torch.int32, device=F.device)
+        mark("classify")
+        # repair path: in place on the pre-step certificates (Alg. 1 returns "updated certificates");
+        # the rebuild path writes the ping-pong partner, so neither strategy sees the other's output
+        repaired = self.certs
+        kc.kc_frontier_repair(self.grid, p_next, F, nF, repaired, movers=movers, nF_max=nF_max)
+        mark("repair")
+        kc.kc_frontier_entropy(self.grid, F, nF, nF_max=nF_max, out=(self.H, self.m, self.C))
+        mark("entropy")
+        kc.kc_cert_grid_rebuild(self.grid, p_next, self.other)
+        self.certs, self.other = self.other, self.certs
+        mark("rebuild")
+        if do_allpairs and self.ap is not None:
+            kc.kc_cert_allpairs(p_next, self.ap, self.ws)
+        mark("allpairs")
+        self.p = p_next
+        res = StepResult(self.eps, nF, self.H, self.m, self.C, repaired, self.certs,
+                         self.ap if do_allpairs else None)
+        if time_phases:
+            res.phase_ms = ev
+        return res
+
+    @staticmethod
+    def phase_times(ev: dict) -> dict:
+        """Milliseconds per phase from the events of a finished step (call after a sync)."""
+        order = ["t0", "maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs"]
+        out = {}
+        for a, b in zip(order[:-1], order[1:]):
+            out[b] = ev[a].elapsed_time(ev[b])
+        return out
+
+
+def crossover_fraction(fracs, t_repair, t_rebuild):
+    """Smallest mover fraction f* with t_repair(f*) >= t_rebuild, by linear interpolation in log f
+    between the bracketing sweep points (Proposition 1).  None if repair always wins
+    inside the sweep, 0.0 if it never does."""
+    fracs = np.asarray(fracs, float)
+    r = np.asarray(t_repair, float) / np.asarray(t_rebuild, float)
+    if r[0] >= 1.0:
+        return 0.0
+    for k in range(1, len(fracs)):
+        if r[k] >= 1.0:
+            a, b = np.log(fracs[k - 1]), np.log(fracs[k])
+            w = (1.0 - r[k - 1]) / (r[k] - r[k - 1])
+            return float(np.exp(a + w * (b - a)))
+    return None
