@@ -3,9 +3,9 @@
 //
 // Layout in HBM (N points, C_tot cells):
 //   cell[N]        int32   current filing cell of point i
-//   rank[N]        int32   arrival rank inside its cell at build time (scratch of the build)
 //   counts[C_tot]  int32   live occupancy per cell (histogram, kept current by A6)
-//   cell_start[C_tot+1] int32  exclusive scan of the build histogram
+//   cell_start[C_tot+1] int32  exclusive scan of the build histogram (entry c+1 doubles as the
+//                           scatter cursor of cell c during the build)
 //   spos2[N] float2 (d=2) / spos4[N] float4 = (x,y,z,bits(idx)) (d=3)   cell-sorted positions
 //   sidx[N]        int32   point id per sorted slot (-1 = tombstone)
 //   slot[N]        int32   sorted slot of point i (-1 = lives in an overflow chain)
@@ -13,6 +13,8 @@
 //   fcount[C_tot], mhist[]  scratch of A5 (always left zeroed)
 // Rows of cells along x are contiguous in the sorted arrays (linear id has x fastest), so a
 // (2r+1)-cell row segment is ONE contiguous candidate range: two cell_start reads per row.
+#include <stdlib.h>
+
 #include <new>
 
 #include "kc_common.cuh"
@@ -52,7 +54,7 @@ struct kc_grid {
     int64_t N_max, n_cells, N;
     int built, dirty;
     size_t bytes;
-    int32_t *cell, *rank, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
+    int32_t *cell, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
     int32_t *blocksums;
     float2 *spos2;
     float4 *spos4, *opos;
@@ -106,8 +108,8 @@ __device__ __forceinline__ int cell_of(const View &v, float x, float y, float z)
 
 template <int D>
 __global__ void __launch_bounds__(256)
-cellid_rank_kernel(View v, const float *__restrict__ p, int N, int32_t *__restrict__ cell,
-                   int32_t *__restrict__ rank, int32_t *counts)
+cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restrict__ cell,
+                   int32_t *counts)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
@@ -120,7 +122,7 @@ cellid_rank_kernel(View v, const float *__restrict__ p, int N, int32_t *__restri
     }
     int cidx = cell_of<D>(v, x, y, z);
     cell[i] = cidx;
-    rank[i] = atomicAdd(&counts[cidx], 1);
+    atomicAdd(&counts[cidx], 1);                  // result unused: compiles to a RED
 }
 
 __global__ void __launch_bounds__(256)
@@ -214,22 +216,29 @@ scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, const int32_t
     int run = off + incl - tsum;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        if (base + k < n_cells) cell_start[base + k] = run;
+        // stored one slot to the right: cell_start[c+1] is the scatter cursor of cell c and ends
+        // up as start[c] + count[c] = start[c+1], i.e. the array becomes the exclusive scan itself
+        if (base + k < n_cells) cell_start[base + k + 1] = run;
         run += v[k];
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[n_cells] = N;
+    if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[0] = 0;
 }
 
 template <int D>
 __global__ void __launch_bounds__(256)
 scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ cell,
-               const int32_t *__restrict__ rank, const int32_t *__restrict__ cell_start,
-               float2 *__restrict__ spos2, float4 *__restrict__ spos4, int32_t *__restrict__ sidx,
+               int32_t *cell_start, float2 *__restrict__ spos2, float4 *__restrict__ spos4, int32_t *__restrict__ sidx,
                int32_t *__restrict__ slot)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < 8) {                                  // inert padding behind the last slot
+        const float qnan = __int_as_float(0x7fc00000);
+        if (D == 2) spos2[N + i] = make_float2(qnan, qnan);
+        else spos4[N + i] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        sidx[N + i] = -1;
+    }
     if (i >= N) return;
-    int s = cell_start[cell[i]] + rank[i];
+    int s = atomicAdd(&cell_start[cell[i] + 1], 1);
     if (D == 2) {
         spos2[s] = reinterpret_cast<const float2 *>(p)[i];
     } else {
@@ -249,26 +258,50 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
 // cells, and clamping is non-expansive), so its distance is >= bound = min over those faces of
 // the query's distance to the face.  Stop only when s2 < (bound*shrink)^2, strictly; shrink
 // absorbs the O(u*G) error of computed faces.  No face left = whole grid scanned = stop.
+//
+// Candidate ranges are scanned 4 records per step from a 4-aligned start: records in front of the
+// range belong to neighbouring cells and the records behind the last slot are NaN padding, so
+// the extra ones are either legitimate candidates or inert (every comparison with NaN is false).
+// A candidate can therefore be offered more than once; the insertion skips ids already held.
+__device__ __forceinline__ void offer_once(Top2 &best, float s, int j, int self)
+{
+    if (s <= best.s2 && j >= 0 && j != self && j != best.j1 && j != best.j2) best.offer(s, j);
+}
+template <int D>
+__device__ __noinline__ Top2 slow_offer4(const View &v, Top2 best, int t, float s0, float s1,
+                                         float s2, float s3, int self)
+{
+    if (D == 2) {
+        if (s0 <= best.s2) offer_once(best, s0, v.sidx[t + 0], self);
+        if (s1 <= best.s2) offer_once(best, s1, v.sidx[t + 1], self);
+        if (s2 <= best.s2) offer_once(best, s2, v.sidx[t + 2], self);
+        if (s3 <= best.s2) offer_once(best, s3, v.sidx[t + 3], self);
+    } else {
+        if (s0 <= best.s2) offer_once(best, s0, __float_as_int(v.spos4[t + 0].w), self);
+        if (s1 <= best.s2) offer_once(best, s1, __float_as_int(v.spos4[t + 1].w), self);
+        if (s2 <= best.s2) offer_once(best, s2, __float_as_int(v.spos4[t + 2].w), self);
+        if (s3 <= best.s2) offer_once(best, s3, __float_as_int(v.spos4[t + 3].w), self);
+    }
+    return best;
+}
 template <int D>
 __device__ __forceinline__ void scan_range(const View &v, int b, int e, float qx, float qy, float qz,
                                            int self, Top2 &best)
 {
-    for (int t = b; t < e; ++t) {
+    for (int t = b & ~3; t < e; t += 4) {
+        float s0, s1, s2, s3;
         if (D == 2) {
-            float2 c = v.spos2[t];
-            float s = sqd2(qx, qy, c.x, c.y);
-            if (s <= best.s2) {
-                int j = v.sidx[t];
-                if (j != self && j >= 0) best.offer(s, j);
-            }
+            const float4 A = *reinterpret_cast<const float4 *>(v.spos2 + t);       // x0 y0 x1 y1
+            const float4 B = *reinterpret_cast<const float4 *>(v.spos2 + t + 2);   // x2 y2 x3 y3
+            s0 = sqd2(qx, qy, A.x, A.y); s1 = sqd2(qx, qy, A.z, A.w);
+            s2 = sqd2(qx, qy, B.x, B.y); s3 = sqd2(qx, qy, B.z, B.w);
         } else {
-            float4 c = v.spos4[t];
-            float s = sqd3(qx, qy, qz, c.x, c.y, c.z);
-            if (s <= best.s2) {
-                int j = __float_as_int(c.w);
-                if (j != self && j >= 0) best.offer(s, j);
-            }
+            const float4 c0 = v.spos4[t], c1 = v.spos4[t + 1], c2 = v.spos4[t + 2], c3 = v.spos4[t + 3];
+            s0 = sqd3(qx, qy, qz, c0.x, c0.y, c0.z); s1 = sqd3(qx, qy, qz, c1.x, c1.y, c1.z);
+            s2 = sqd3(qx, qy, qz, c2.x, c2.y, c2.z); s3 = sqd3(qx, qy, qz, c3.x, c3.y, c3.z);
         }
+        float m = fminf(fminf(s0, s1), fminf(s2, s3));
+        if (m <= best.s2) best = slow_offer4<D>(v, best, t, s0, s1, s2, s3, self);
     }
 }
 template <int D>
@@ -278,7 +311,7 @@ __device__ __forceinline__ void scan_chain(const View &v, int cidx, float qx, fl
     for (int e = v.head[cidx]; e >= 0; e = v.next[e]) {
         float4 c = v.opos[e];
         float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
-        if (s <= best.s2 && e != self) best.offer(s, e);
+        offer_once(best, s, e, self);
     }
 }
 template <int D>
@@ -291,41 +324,47 @@ __device__ __forceinline__ void scan_row(const View &v, bool chains, int rowbase
         for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
 }
 
+// distance from the query to the nearest face of the cell box [x0,x1]x[y0,y1]x[z0,z1] that is
+// interior to the grid (+inf if the box covers the grid)
 template <int D>
-__device__ int ring_search(const View &v, bool chains, float qx, float qy, float qz, int self,
-                           Top2 &best)
+__device__ __forceinline__ float box_bound(const View &v, float qx, float qy, float qz, int x0,
+                                           int x1, int y0, int y1, int z0, int z1)
 {
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    int r = 1;
-    // radius-1 block: all rows, full segments
-    {
-        int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
-        int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
-        int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y)
-                scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, x0, x1, qx, qy, qz, self, best);
+    float bound = CUDART_INF_F;
+    if (x0 >= 1) bound = fminf(bound, __fsub_rn(qx, __fadd_rn(v.lo0, __fmul_rn((float)x0, v.h))));
+    if (x1 < v.G0 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo0, __fmul_rn((float)(x1 + 1), v.h)), qx));
+    if (y0 >= 1) bound = fminf(bound, __fsub_rn(qy, __fadd_rn(v.lo1, __fmul_rn((float)y0, v.h))));
+    if (y1 < v.G1 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo1, __fmul_rn((float)(y1 + 1), v.h)), qy));
+    if (D == 3) {
+        if (z0 >= 1) bound = fminf(bound, __fsub_rn(qz, __fadd_rn(v.lo2, __fmul_rn((float)z0, v.h))));
+        if (z1 < v.G2 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo2, __fmul_rn((float)(z1 + 1), v.h)), qz));
     }
+    return bound;
+}
+__device__ __forceinline__ bool bound_ok(const View &v, float bound, float s2)
+{
+    if (bound == CUDART_INF_F) return true;               // nothing left outside the scanned box
+    float bs = __fmul_rn(bound, v.shrink);
+    return bs > 0.0f && s2 < __fmul_rn(bs, bs);
+}
+
+// Chebyshev rings r = 2, 3, ... around the query's own cell, entered with the radius-1 block
+// already scanned; leaves as soon as the bound of the scanned block allows it.
+template <int D>
+__device__ int ring_continue(const View &v, bool chains, float qx, float qy, float qz, int self,
+                             int cx, int cy, int cz, Top2 &best)
+{
+    int r = 1;
     for (;;) {
-        float bound = CUDART_INF_F;
-        if (cx - r >= 1) bound = fminf(bound, __fsub_rn(qx, __fadd_rn(v.lo0, __fmul_rn((float)(cx - r), v.h))));
-        if (cx + r < v.G0 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo0, __fmul_rn((float)(cx + r + 1), v.h)), qx));
-        if (cy - r >= 1) bound = fminf(bound, __fsub_rn(qy, __fadd_rn(v.lo1, __fmul_rn((float)(cy - r), v.h))));
-        if (cy + r < v.G1 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo1, __fmul_rn((float)(cy + r + 1), v.h)), qy));
-        if (D == 3) {
-            if (cz - r >= 1) bound = fminf(bound, __fsub_rn(qz, __fadd_rn(v.lo2, __fmul_rn((float)(cz - r), v.h))));
-            if (cz + r < v.G2 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo2, __fmul_rn((float)(cz + r + 1), v.h)), qz));
-        }
-        if (bound == CUDART_INF_F) break;                 // the block covers the whole grid
-        float bs = __fmul_rn(bound, v.shrink);
-        if (bs > 0.0f && best.s2 < __fmul_rn(bs, bs)) break;
-        ++r;
-        // ring r: shell rows get the full segment, inner rows only the two end cells
         int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
         int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
         int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
+        if (bound_ok(v, box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) break;
+        ++r;
+        // ring r: shell rows get the full segment, inner rows only the two end cells
+        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
+        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
         for (int z = z0; z <= z1; ++z)
             for (int y = y0; y <= y1; ++y) {
                 int rowbase = (z * v.G1 + y) * v.G0;
@@ -341,24 +380,184 @@ __device__ int ring_search(const View &v, bool chains, float qx, float qy, float
     return r;
 }
 
+// Query in cell (cx,cy,cz).  First the cell box [bx0,bx1] x [cy-1,cy+1] x [cz-1,cz+1] (a superset of
+// the 3^d block: neighbouring queries of one row share it so that their loops and loads coincide),
+// then Chebyshev rings r = 2, 3, ... around the query's own cell while the bound requires it.
+template <int D>
+__device__ int ring_search(const View &v, bool chains, float qx, float qy, float qz, int self,
+                           int cx, int cy, int cz, int bx0, int bx1, Top2 &best)
+{
+    {
+        int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
+        int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y)
+                scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, bx0, bx1, qx, qy, qz, self, best);
+        if (bound_ok(v, box_bound<D>(v, qx, qy, qz, bx0, bx1, y0, y1, z0, z1), best.s2)) return 1;
+    }
+    return ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+}
+
+constexpr int GROUP = 8;        // consecutive sorted slots that share one cell box
+constexpr int GROUP_MAXW = 12;  // ... unless they span more cells than this (sparse region)
+
 template <int D>
 __global__ void __launch_bounds__(128)
 search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
 {
-    int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int sc = min(s, N - 1);                 // tail lanes mirror the last slot (no store)
     float qx, qy, qz = 0.f;
     int self;
     if (D == 2) {
-        float2 q = v.spos2[s];
-        qx = q.x; qy = q.y; self = v.sidx[s];
+        float2 q = v.spos2[sc];
+        qx = q.x; qy = q.y; self = v.sidx[sc];
     } else {
-        float4 q = v.spos4[s];
+        float4 q = v.spos4[sc];
         qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
     }
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    // slots are cell-sorted: the first and last member of a group bracket the cells of all members
+    const int lane = threadIdx.x & 31, g0 = lane & ~(GROUP - 1);
+    const int fx = __shfl_sync(0xffffffffu, cx, g0), lx = __shfl_sync(0xffffffffu, cx, g0 + GROUP - 1);
+    const int fr = __shfl_sync(0xffffffffu, cz * v.G1 + cy, g0);
+    const int lr = __shfl_sync(0xffffffffu, cz * v.G1 + cy, g0 + GROUP - 1);
+    int bx0 = max(cx - 1, 0), bx1 = min(cx + 1, v.G0 - 1);
+    if (fr == lr && lx - fx <= GROUP_MAXW) { bx0 = max(fx - 1, 0); bx1 = min(lx + 1, v.G0 - 1); }
     Top2 best;
     best.init();
-    int r = ring_search<D>(v, false, qx, qy, qz, self, best);
+    int r = ring_search<D>(v, false, qx, qy, qz, self, cx, cy, cz, bx0, bx1, best);
+    if (s >= N) return;
+    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    store_cert(best, self, nn, nn2, d1, d2, c);
+}
+
+// ---- A3, warp-tiled: the whole-set search of a freshly built grid --------------------------
+// A warp owns 32 consecutive sorted slots.  Slots are cell-sorted, so the lanes of one grid row
+// form a contiguous lane segment whose 3^(d-1) neighbour rows are each ONE contiguous record range
+// [B, E) of the sorted array.  The warp streams that range through its own shared-memory tile
+// with coalesced loads (one global round trip per tile instead of one per candidate), and every
+// lane scans only its own 3-cell sub-range [b, e) of it from shared memory, 4 records per step.
+// In dense cells all lanes share the same sub-range and the loop degenerates into a broadcast
+// all-pairs tile.  Lanes whose radius-1 block does not satisfy the bound continue with the
+// generic ring loop from global memory (rare).
+constexpr int WT_TILE = 128;   // records per warp tile
+constexpr int WT_WARPS = 4;
+
+template <int D>
+__device__ __forceinline__ void tile_scan(const float2 *tp2, const float4 *tp4, const int *tidx, int lb,
+                                          int le, float qx, float qy, float qz, int self, Top2 &best)
+{
+    for (int t = lb; t < le; t += 4) {
+        float s0, s1, s2, s3;
+        int j0, j1, j2, j3;
+        if (D == 2) {
+            const float2 c0 = tp2[t], c1 = tp2[t + 1], c2 = tp2[t + 2], c3 = tp2[t + 3];
+            s0 = sqd2(qx, qy, c0.x, c0.y); s1 = sqd2(qx, qy, c1.x, c1.y);
+            s2 = sqd2(qx, qy, c2.x, c2.y); s3 = sqd2(qx, qy, c3.x, c3.y);
+        } else {
+            const float4 c0 = tp4[t], c1 = tp4[t + 1], c2 = tp4[t + 2], c3 = tp4[t + 3];
+            s0 = sqd3(qx, qy, qz, c0.x, c0.y, c0.z); s1 = sqd3(qx, qy, qz, c1.x, c1.y, c1.z);
+            s2 = sqd3(qx, qy, qz, c2.x, c2.y, c2.z); s3 = sqd3(qx, qy, qz, c3.x, c3.y, c3.z);
+            j0 = __float_as_int(c0.w); j1 = __float_as_int(c1.w);
+            j2 = __float_as_int(c2.w); j3 = __float_as_int(c3.w);
+        }
+        float m = fminf(fminf(s0, s1), fminf(s2, s3));
+        if (m <= best.s2) {
+            if (D == 2) { j0 = tidx[t]; j1 = tidx[t + 1]; j2 = tidx[t + 2]; j3 = tidx[t + 3]; }
+            offer_once(best, s0, j0, self);
+            offer_once(best, s1, j1, self);
+            offer_once(best, s2, j2, self);
+            offer_once(best, s3, j3, self);
+        }
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(32 * WT_WARPS)
+search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2,
+                        float *c)
+{
+    __shared__ __align__(16) float4 s_p4[D == 3 ? WT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
+    __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float qnan = __int_as_float(0x7fc00000);
+    float4 *tp4 = s_p4[D == 3 ? warp : 0];
+    float2 *tp2 = s_p2[D == 2 ? warp : 0];
+    int *tix = s_ix[D == 2 ? warp : 0];
+    if (lane < 4) {                                // inert records behind the tile
+        if (D == 3) tp4[WT_TILE + lane] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        else { tp2[WT_TILE + lane] = make_float2(qnan, qnan); tix[WT_TILE + lane] = -1; }
+    }
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s - lane >= N) return;                     // whole warp past the end
+    const int sc = min(s, N - 1);                  // tail lanes mirror the last slot (no store)
+    float qx, qy, qz = 0.f;
+    int self;
+    if (D == 2) {
+        float2 q = v.spos2[sc];
+        qx = q.x; qy = q.y; self = v.sidx[sc];
+    } else {
+        float4 q = v.spos4[sc];
+        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
+    }
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    const int rowid = cz * v.G1 + cy;
+    const int lx0 = max(cx - 1, 0), lx1 = min(cx + 1, v.G0 - 1);
+    Top2 best;
+    best.init();
+    unsigned todo = 0xffffffffu;
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int R = __shfl_sync(0xffffffffu, rowid, leader);
+        const unsigned seg = __ballot_sync(0xffffffffu, rowid == R) & todo;
+        const int first = __ffs(seg) - 1, last = 31 - __clz(seg);
+        const int xf = __shfl_sync(0xffffffffu, cx, first), xl = __shfl_sync(0xffffffffu, cx, last);
+        const int ry = __shfl_sync(0xffffffffu, cy, first), rz = __shfl_sync(0xffffffffu, cz, first);
+        const bool mine = (seg >> lane) & 1u;
+        const int ux0 = max(xf - 1, 0), ux1 = min(xl + 1, v.G0 - 1);
+        const int z0 = D == 3 ? max(rz - 1, 0) : 0, z1 = D == 3 ? min(rz + 1, v.G2 - 1) : 0;
+        const int y0 = max(ry - 1, 0), y1 = min(ry + 1, v.G1 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y) {
+                const int rowbase = (z * v.G1 + y) * v.G0;
+                const int B = v.cell_start[rowbase + ux0], E = v.cell_start[rowbase + ux1 + 1];
+                int b = 0, e = 0;
+                if (mine) { b = v.cell_start[rowbase + lx0]; e = v.cell_start[rowbase + lx1 + 1]; }
+                for (int T0 = B; T0 < E; T0 += WT_TILE) {
+#pragma unroll
+                    for (int k = lane; k < WT_TILE; k += 32) {
+                        const int g = T0 + k;
+                        if (D == 3) {
+                            tp4[k] = g < N ? v.spos4[g] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
+                        } else {
+                            tp2[k] = g < N ? v.spos2[g] : make_float2(qnan, qnan);
+                            tix[k] = g < N ? v.sidx[g] : -1;
+                        }
+                    }
+                    __syncwarp();
+                    if (mine) {
+                        const int lb = max(b, T0) - T0, le = min(e, T0 + WT_TILE) - T0;
+                        tile_scan<D>(tp2, tp4, tix, lb, le, qx, qy, qz, self, best);
+                    }
+                    __syncwarp();
+                }
+            }
+        todo &= ~seg;
+    }
+    int r = 1;
+    {
+        const int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
+        const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
+        if (!bound_ok(v, box_bound<D>(v, qx, qy, qz, lx0, lx1, y0, y1, z0, z1), best.s2))
+            r = ring_continue<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
+    }
+    if (s >= N) return;
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
     store_cert(best, self, nn, nn2, d1, d2, c);
 }
@@ -377,7 +576,10 @@ search_frontier_kernel(View v, const float *__restrict__ p_new, const int32_t *_
         float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
         Top2 best;
         best.init();
-        int r = ring_search<D>(v, chains, qx, qy, qz, i, best);
+        const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+        const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+        const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+        int r = ring_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, max(cx - 1, 0), min(cx + 1, v.G0 - 1), best);
         if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
         store_cert(best, i, nn, nn2, d1, d2, c);
     }
@@ -543,16 +745,16 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
         g->bytes += bytes;
     };
     size_t n = (size_t)N_max, nc = (size_t)n_cells;
-    alloc((void **)&g->cell, n * 4); alloc((void **)&g->rank, n * 4);
+    alloc((void **)&g->cell, n * 4);
     alloc((void **)&g->counts, nc * 4); alloc((void **)&g->cell_start, (nc + 1) * 4);
-    alloc((void **)&g->sidx, n * 4); alloc((void **)&g->slot, n * 4);
+    alloc((void **)&g->sidx, (n + 8) * 4); alloc((void **)&g->slot, n * 4);
     alloc((void **)&g->head, nc * 4); alloc((void **)&g->next, n * 4);
     alloc((void **)&g->mlist, n * 4); alloc((void **)&g->fcount, nc * 4);
     alloc((void **)&g->mhist, MHIST * 4);
     alloc((void **)&g->blocksums, (size_t)g->n_scan_blocks * 4 + 4);
     g->spos2 = nullptr; g->spos4 = nullptr;
-    if (geom->d == 2) alloc((void **)&g->spos2, n * sizeof(float2));
-    else alloc((void **)&g->spos4, n * sizeof(float4));
+    if (geom->d == 2) alloc((void **)&g->spos2, (n + 8) * sizeof(float2));
+    else alloc((void **)&g->spos4, (n + 8) * sizeof(float4));
     alloc((void **)&g->opos, n * sizeof(float4));
     alloc((void **)&g->ctr, sizeof(Counters));
     if (!ok) {
@@ -578,7 +780,7 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
 extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
-    void *ptrs[] = {g->cell, g->rank, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
+    void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
                     g->mlist, g->fcount, g->mhist, g->blocksums, g->spos2, g->spos4, g->opos, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
@@ -601,15 +803,15 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     clear_chains_kernel<<<blocks_for(g->N, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
     reset_counters_kernel<<<1, 1, 0, st>>>(g->ctr, 1);
     KC_CUDA(cudaMemsetAsync(g->counts, 0, (size_t)nc * 4, st));
-    if (g->geom.d == 2) cellid_rank_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->rank, g->counts);
-    else cellid_rank_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->rank, g->counts);
+    if (g->geom.d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts);
+    else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts);
     scan_reduce_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->ctr);
     scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, g->n_scan_blocks);
     scan_write_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->cell_start, n);
     if (g->geom.d == 2)
-        scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+        scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
     else
-        scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->rank, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+        scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
     count_launches(7);   // + one memset node
     KC_LAUNCH_CHECK("kc_grid_build");
     g->N = N; g->built = 1; g->dirty = 0;
@@ -629,8 +831,15 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)g->N;
-    if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-    else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 1;
+    const int tb = 32 * WT_WARPS;
+    if (variant == 1) {
+        if (g->geom.d == 2) search_all_tiled_kernel<2><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+        else search_all_tiled_kernel<3><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    } else {
+        if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+        else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+    }
     count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
     return KC_OK;
