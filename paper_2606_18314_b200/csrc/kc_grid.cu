@@ -13,6 +13,7 @@
 //   fcount[C_tot], mhist[]  scratch of A5 (always left zeroed)
 // Rows of cells along x are contiguous in the sorted arrays (linear id has x fastest), so a
 // (2r+1)-cell row segment is ONE contiguous candidate range: two cell_start reads per row.
+#include <math.h>
 #include <stdlib.h>
 
 #include <new>
@@ -38,6 +39,8 @@ struct Counters {
 struct View {
     int G0, G1, G2;
     float lo0, lo1, lo2, h, inv_h, shrink;
+    float slk0, slk1, slk2;   // absolute rounding slack of a computed face / cell boundary per axis
+    int dense_thr;            // a row range of at least this many records is handled as dense (A3)
     const int32_t *cell_start;
     const float2 *spos2;
     const float4 *spos4;
@@ -76,6 +79,15 @@ View make_view(const kc_grid *g)
     if (v.G2 > Gm) Gm = v.G2;
     // rounding slack of the ring bound: computed cell faces are off by O(u*G) cell widths
     v.shrink = 1.0f - (1.0f / 512.0f + (float)Gm * (1.0f / 524288.0f));
+    const int Ga[3] = {v.G0, v.G1, v.G2};
+    float slk[3];
+    for (int a = 0; a < 3; ++a) {
+        double t = (fabs((double)g->geom.lo[a]) + (double)Ga[a] * (double)g->geom.h) / 1048576.0;
+        slk[a] = nextafterf((float)t, INFINITY);
+    }
+    v.slk0 = slk[0]; v.slk1 = slk[1]; v.slk2 = slk[2];
+    static const int dense_env = getenv("KC_DENSE_THR") ? atoi(getenv("KC_DENSE_THR")) : 0;
+    v.dense_thr = dense_env > 0 ? dense_env : 128;
     v.cell_start = g->cell_start;
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;
@@ -252,12 +264,28 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
 // ------------------------------------------------------------------ A3 / A7 ring search
 // Exact top-2 of query (qx,qy,qz), excluding point id `self`, over the grid's sorted ranges and
 // (if chains) its overflow chains.  Corollary 1: the block is widened until
-// the second neighbour is provably enclosed.  After the Chebyshev-radius-r block around the
-// query's cell (cx,cy,cz) has been scanned, every unscanned point lies beyond one of the
-// block's faces that are interior to the grid (points outside the box are filed in boundary
-// cells, and clamping is non-expansive), so its distance is >= bound = min over those faces of
-// the query's distance to the face.  Stop only when s2 < (bound*shrink)^2, strictly; shrink
-// absorbs the O(u*G) error of computed faces.  No face left = whole grid scanned = stop.
+// the second neighbour is provably enclosed.
+//
+// Filing invariant: every record listed in cell k of an axis has a coordinate x with
+// cell_axis(x) = k, and cell_axis is monotone, so for a query in cell c < k the real distance
+// along that axis is at least  face(k) - q  minus the rounding of the computed face and cell id:
+//     x - q >= fl(face_k - q)(1 - u) - u(|lo| + 5.01 G h),      u = 2^-24
+// (3 roundings in cell_axis move a cell boundary by <= 3.01 u G h, 2 roundings in
+// face_k = fl(lo + fl(k h)) move the face by <= u(|lo| + 2 G h)).  gap_lb() therefore subtracts
+// the absolute slack slk = (|lo| + G h) 2^-20 and multiplies by shrink = 1 - 2^-9 - G 2^-19,
+// which also covers the <= 3u relative undershoot of an fp32 squared distance.  Points outside
+// the grid box are filed in boundary cells; only faces between two cells are ever used, so the
+// bound holds for them too (clamping is monotone).
+//
+// Two uses of the bound, both strict (a tie at equal distance must still be seen, the index
+// decides it):
+//  * cell pruning inside the 3^d block: a cell whose box is provably farther than the current
+//    second-best (sum over axes of the squared shrunk gaps > s2) is skipped.  The query's own
+//    cell is scanned first, then its row neighbours, then the other rows nearest first, so in
+//    dense cells (occupancy >> 1, d2 << h) most of the block is never touched;
+//  * termination: after the Chebyshev-radius-r block is done, every unscanned point lies beyond
+//    a block face interior to the grid; stop only when s2 < (min face distance)^2, else scan
+//    ring r+1.  No face left = whole grid scanned = stop.  Never a cap.
 //
 // Candidate ranges are scanned 4 records per step from a 4-aligned start: records in front of the
 // range belong to neighbouring cells and the records behind the last slot are NaN padding, so
@@ -324,42 +352,80 @@ __device__ __forceinline__ void scan_row(const View &v, bool chains, int rowbase
         for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
 }
 
-// distance from the query to the nearest face of the cell box [x0,x1]x[y0,y1]x[z0,z1] that is
-// interior to the grid (+inf if the box covers the grid)
+__device__ __forceinline__ float face_at(float lo, int k, float h)
+{
+    return __fadd_rn(lo, __fmul_rn((float)k, h));
+}
+// lower bound of the real axis distance behind a computed face at computed distance `gap`
+__device__ __forceinline__ float gap_lb(const View &v, float gap, float slk)
+{
+    return __fmul_rn(fmaxf(__fsub_rn(gap, slk), 0.0f), v.shrink);
+}
+// squared lower bounds of the axis distance from the query to its six neighbour cells
+struct Gaps { float xm, xp, ym, yp, zm, zp; };
+template <int D>
+__device__ __forceinline__ Gaps make_gaps(const View &v, float qx, float qy, float qz, int cx, int cy, int cz)
+{
+    Gaps g;
+    float t;
+    t = gap_lb(v, __fsub_rn(qx, face_at(v.lo0, cx, v.h)), v.slk0); g.xm = __fmul_rn(t, t);
+    t = gap_lb(v, __fsub_rn(face_at(v.lo0, cx + 1, v.h), qx), v.slk0); g.xp = __fmul_rn(t, t);
+    t = gap_lb(v, __fsub_rn(qy, face_at(v.lo1, cy, v.h)), v.slk1); g.ym = __fmul_rn(t, t);
+    t = gap_lb(v, __fsub_rn(face_at(v.lo1, cy + 1, v.h), qy), v.slk1); g.yp = __fmul_rn(t, t);
+    g.zm = 0.f; g.zp = 0.f;
+    if (D == 3) {
+        t = gap_lb(v, __fsub_rn(qz, face_at(v.lo2, cz, v.h)), v.slk2); g.zm = __fmul_rn(t, t);
+        t = gap_lb(v, __fsub_rn(face_at(v.lo2, cz + 1, v.h), qz), v.slk2); g.zp = __fmul_rn(t, t);
+    }
+    return g;
+}
+// The 3^(d-1) - 1 rows of the block other than the query's own, nearest first: offsets (oy, oz)
+// packed two bits each as offset + 1.
+//   k:   0       1       2       3       4        5        6        7
+//  oy:  -1      +1       0       0      -1       +1       -1       +1
+//  oz:   0       0      -1      +1      -1       -1       +1       +1
+constexpr unsigned ROW_OY = 0u | (2u << 2) | (1u << 4) | (1u << 6) | (0u << 8) | (2u << 10) | (0u << 12) | (2u << 14);
+constexpr unsigned ROW_OZ = 1u | (1u << 2) | (0u << 4) | (2u << 6) | (0u << 8) | (0u << 10) | (2u << 12) | (2u << 14);
+__device__ __forceinline__ int row_oy(int k) { return (int)((ROW_OY >> (2 * k)) & 3u) - 1; }
+__device__ __forceinline__ int row_oz(int k) { return (int)((ROW_OZ >> (2 * k)) & 3u) - 1; }
+
+// distance (lower bound) from the query to the nearest face of the cell box
+// [x0,x1]x[y0,y1]x[z0,z1] that is interior to the grid (+inf if the box covers the grid)
 template <int D>
 __device__ __forceinline__ float box_bound(const View &v, float qx, float qy, float qz, int x0,
                                            int x1, int y0, int y1, int z0, int z1)
 {
     float bound = CUDART_INF_F;
-    if (x0 >= 1) bound = fminf(bound, __fsub_rn(qx, __fadd_rn(v.lo0, __fmul_rn((float)x0, v.h))));
-    if (x1 < v.G0 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo0, __fmul_rn((float)(x1 + 1), v.h)), qx));
-    if (y0 >= 1) bound = fminf(bound, __fsub_rn(qy, __fadd_rn(v.lo1, __fmul_rn((float)y0, v.h))));
-    if (y1 < v.G1 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo1, __fmul_rn((float)(y1 + 1), v.h)), qy));
+    if (x0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qx, face_at(v.lo0, x0, v.h)), v.slk0));
+    if (x1 < v.G0 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo0, x1 + 1, v.h), qx), v.slk0));
+    if (y0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qy, face_at(v.lo1, y0, v.h)), v.slk1));
+    if (y1 < v.G1 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo1, y1 + 1, v.h), qy), v.slk1));
     if (D == 3) {
-        if (z0 >= 1) bound = fminf(bound, __fsub_rn(qz, __fadd_rn(v.lo2, __fmul_rn((float)z0, v.h))));
-        if (z1 < v.G2 - 1) bound = fminf(bound, __fsub_rn(__fadd_rn(v.lo2, __fmul_rn((float)(z1 + 1), v.h)), qz));
+        if (z0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qz, face_at(v.lo2, z0, v.h)), v.slk2));
+        if (z1 < v.G2 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo2, z1 + 1, v.h), qz), v.slk2));
     }
     return bound;
 }
-__device__ __forceinline__ bool bound_ok(const View &v, float bound, float s2)
+__device__ __forceinline__ bool bound_ok(float bound, float s2)
 {
     if (bound == CUDART_INF_F) return true;               // nothing left outside the scanned box
-    float bs = __fmul_rn(bound, v.shrink);
-    return bs > 0.0f && s2 < __fmul_rn(bs, bs);
+    return bound > 0.0f && s2 < __fmul_rn(bound, bound);
 }
 
 // Chebyshev rings r = 2, 3, ... around the query's own cell, entered with the radius-1 block
-// already scanned; leaves as soon as the bound of the scanned block allows it.
+// already done; leaves as soon as the bound of the scanned block allows it.  (Rare path: kept out
+// of line, state passed by value.)
+struct RingOut { Top2 best; int r; };
 template <int D>
-__device__ int ring_continue(const View &v, bool chains, float qx, float qy, float qz, int self,
-                             int cx, int cy, int cz, Top2 &best)
+__device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float qx, float qy, float qz,
+                                              int self, int cx, int cy, int cz, Top2 best)
 {
     int r = 1;
     for (;;) {
         int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
         int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
         int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-        if (bound_ok(v, box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) break;
+        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) break;
         ++r;
         // ring r: shell rows get the full segment, inner rows only the two end cells
         z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
@@ -377,72 +443,101 @@ __device__ int ring_continue(const View &v, bool chains, float qx, float qy, flo
                 }
             }
     }
-    return r;
+    RingOut o;
+    o.best = best; o.r = r;
+    return o;
 }
-
-// Query in cell (cx,cy,cz).  First the cell box [bx0,bx1] x [cy-1,cy+1] x [cz-1,cz+1] (a superset of
-// the 3^d block: neighbouring queries of one row share it so that their loops and loads coincide),
-// then Chebyshev rings r = 2, 3, ... around the query's own cell while the bound requires it.
+// final check of the radius-1 block, then wider rings if the bound requires them
 template <int D>
-__device__ int ring_search(const View &v, bool chains, float qx, float qy, float qz, int self,
-                           int cx, int cy, int cz, int bx0, int bx1, Top2 &best)
+__device__ __forceinline__ int finish_block(const View &v, bool chains, float qx, float qy, float qz, int self,
+                                            int cx, int cy, int cz, Top2 &best)
 {
-    {
-        int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
-        int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y)
-                scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, bx0, bx1, qx, qy, qz, self, best);
-        if (bound_ok(v, box_bound<D>(v, qx, qy, qz, bx0, bx1, y0, y1, z0, z1), best.s2)) return 1;
-    }
-    return ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    const int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
+    const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
+    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
+    if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) return 1;
+    const RingOut o = ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    best = o.best;
+    return o.r;
 }
 
-constexpr int GROUP = 8;        // consecutive sorted slots that share one cell box
-constexpr int GROUP_MAXW = 12;  // ... unless they span more cells than this (sparse region)
+// One thread per query, straight from global memory (A7, and A3's comparison variant): own
+// cell, row neighbours, other rows nearest first, every cell subject to pruning; then rings.
+template <int D>
+__device__ int block_search(const View &v, bool chains, float qx, float qy, float qz, int self,
+                            int cx, int cy, int cz, Top2 &best)
+{
+    const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
+    const int rb0 = (cz * v.G1 + cy) * v.G0;
+    {
+        const int32_t *cs = v.cell_start + rb0 + cx;
+        const int s0 = cs[0], s1 = cs[1];
+        scan_range<D>(v, s0, s1, qx, qy, qz, self, best);
+        if (chains) scan_chain<D>(v, rb0 + cx, qx, qy, qz, self, best);
+        if (cx > 0 && !(best.s2 < g.xm)) {
+            scan_range<D>(v, cs[-1], s0, qx, qy, qz, self, best);
+            if (chains) scan_chain<D>(v, rb0 + cx - 1, qx, qy, qz, self, best);
+        }
+        if (cx < v.G0 - 1 && !(best.s2 < g.xp)) {
+            scan_range<D>(v, s1, cs[2], qx, qy, qz, self, best);
+            if (chains) scan_chain<D>(v, rb0 + cx + 1, qx, qy, qz, self, best);
+        }
+    }
+#pragma unroll 1
+    for (int k = 0; k < (D == 3 ? 8 : 2); ++k) {
+        const int oy = row_oy(k), oz = row_oz(k);
+        const int y = cy + oy, z = cz + oz;
+        if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
+        const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
+        if (best.s2 < rb2) continue;
+        int x0 = cx, x1 = cx;
+        if (cx > 0 && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
+        if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
+        scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, x0, x1, qx, qy, qz, self, best);
+    }
+    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+}
 
 template <int D>
 __global__ void __launch_bounds__(128)
 search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    const int sc = min(s, N - 1);                 // tail lanes mirror the last slot (no store)
+    if (s >= N) return;
     float qx, qy, qz = 0.f;
     int self;
     if (D == 2) {
-        float2 q = v.spos2[sc];
-        qx = q.x; qy = q.y; self = v.sidx[sc];
+        float2 q = v.spos2[s];
+        qx = q.x; qy = q.y; self = v.sidx[s];
     } else {
-        float4 q = v.spos4[sc];
+        float4 q = v.spos4[s];
         qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
     }
     const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
     const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
     const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    // slots are cell-sorted: the first and last member of a group bracket the cells of all members
-    const int lane = threadIdx.x & 31, g0 = lane & ~(GROUP - 1);
-    const int fx = __shfl_sync(0xffffffffu, cx, g0), lx = __shfl_sync(0xffffffffu, cx, g0 + GROUP - 1);
-    const int fr = __shfl_sync(0xffffffffu, cz * v.G1 + cy, g0);
-    const int lr = __shfl_sync(0xffffffffu, cz * v.G1 + cy, g0 + GROUP - 1);
-    int bx0 = max(cx - 1, 0), bx1 = min(cx + 1, v.G0 - 1);
-    if (fr == lr && lx - fx <= GROUP_MAXW) { bx0 = max(fx - 1, 0); bx1 = min(lx + 1, v.G0 - 1); }
     Top2 best;
     best.init();
-    int r = ring_search<D>(v, false, qx, qy, qz, self, cx, cy, cz, bx0, bx1, best);
-    if (s >= N) return;
+    int r = block_search<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
     store_cert(best, self, nn, nn2, d1, d2, c);
 }
 
 // ---- A3, warp-tiled: the whole-set search of a freshly built grid --------------------------
 // A warp owns 32 consecutive sorted slots.  Slots are cell-sorted, so the lanes of one grid row
-// form a contiguous lane segment whose 3^(d-1) neighbour rows are each ONE contiguous record range
-// [B, E) of the sorted array.  The warp streams that range through its own shared-memory tile
-// with coalesced loads (one global round trip per tile instead of one per candidate), and every
-// lane scans only its own 3-cell sub-range [b, e) of it from shared memory, 4 records per step.
-// In dense cells all lanes share the same sub-range and the loop degenerates into a broadcast
-// all-pairs tile.  Lanes whose radius-1 block does not satisfy the bound continue with the
-// generic ring loop from global memory (rare).
+// form a contiguous lane segment, and what they need from any row of the 3^d block is ONE
+// contiguous record range [B, E) of the sorted array (cells xf-1 .. xl+1 of that row).
+//  * sparse row (E - B < dense_thr records): the warp loads the range into its shared-memory tile
+//    with coalesced loads (one global round trip instead of one per candidate) and every lane
+//    scans its own 3-cell sub-range [b, e) from shared memory, 4 records per step;
+//  * dense row (a few cells under 32 lanes, occupancy >> 1, d2 << h): cell pruning pays.  In the
+//    lanes' own row the own cell is scanned first, then only the row neighbours a lane cannot
+//    rule out; in the other rows only the cells it cannot rule out.  What is left after pruning
+//    is long ranges for a few lanes; a tile pass would cost as much as if all 32 lanes needed
+//    them, so such a pass is served cooperatively instead: for each lane that still has a range,
+//    all 32 lanes take different records of it (coalesced, straight from global memory) and the
+//    two best are extracted with warp reductions.
+// Lanes whose radius-1 block does not satisfy the bound continue with the ring loop (rare).
 constexpr int WT_TILE = 128;   // records per warp tile
 constexpr int WT_WARPS = 4;
 
@@ -475,6 +570,116 @@ __device__ __forceinline__ void tile_scan(const float2 *tp2, const float4 *tp4, 
     }
 }
 
+// Tile pass: records [B, E) (warp-uniform) go through the warp's tile, every lane scans its own
+// (up to two) ranges [b1,e1), [b2,e2) (empty when b >= e).  Called by all 32 lanes.
+template <int D>
+__device__ __forceinline__ void tile_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
+                                          int B, int E, int b1, int e1, int b2, int e2, float qx, float qy,
+                                          float qz, int self, Top2 &best)
+{
+    const float qnan = __int_as_float(0x7fc00000);
+    for (int T0 = B; T0 < E; T0 += WT_TILE) {
+        const int T1 = T0 + WT_TILE;
+        const int lb1 = max(b1, T0), le1 = min(e1, T1), lb2 = max(b2, T0), le2 = min(e2, T1);
+        if (E - B > WT_TILE && !__any_sync(0xffffffffu, lb1 < le1 || lb2 < le2)) continue;
+        const int need = min(WT_TILE, E - T0 + 3);               // records of this tile anyone can touch
+#pragma unroll
+        for (int k = lane; k < WT_TILE; k += 32) {
+            const int g = T0 + k;
+            if (k < need) {
+                if (D == 3) {
+                    tp4[k] = g < N ? v.spos4[g] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
+                } else {
+                    tp2[k] = g < N ? v.spos2[g] : make_float2(qnan, qnan);
+                    tix[k] = g < N ? v.sidx[g] : -1;
+                }
+            }
+        }
+        __syncwarp();
+        if (lb1 < le1) tile_scan<D>(tp2, tp4, tix, lb1 - T0, le1 - T0, qx, qy, qz, self, best);
+        if (lb2 < le2) tile_scan<D>(tp2, tp4, tix, lb2 - T0, le2 - T0, qx, qy, qz, self, best);
+        __syncwarp();
+    }
+}
+
+// Warp-cooperative scan of one lane's range: all 32 lanes take different records of [b, e) for the
+// query of lane L (coalesced loads straight from global memory) and keep their own partial top-2.
+template <int D>
+__device__ __forceinline__ void coop_range(const View &v, int lane, int b, int e, float qx, float qy,
+                                           float qz, int self, float thr, int h1, int h2, Top2 &tmp)
+{
+    for (int t = b + lane; t < e; t += 32) {
+        float s;
+        int j;
+        if (D == 2) {
+            const float2 c = v.spos2[t];
+            s = sqd2(qx, qy, c.x, c.y);
+            j = s <= thr ? v.sidx[t] : -1;
+        } else {
+            const float4 c = v.spos4[t];
+            s = sqd3(qx, qy, qz, c.x, c.y, c.z);
+            j = __float_as_int(c.w);
+        }
+        if (s <= thr && j >= 0 && j != self && j != h1 && j != h2) tmp.offer(s, j);
+    }
+}
+// smallest key (s, j) over the warp's partial lists, removed from the list that held it
+__device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
+{
+    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
+    const unsigned m = __reduce_min_sync(0xffffffffu, key);
+    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
+    s = __uint_as_float(m);
+    if (key == m && tmp.j1 == j) {
+        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
+        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
+    }
+}
+// Dense pass: every lane brings up to two ranges left after pruning.  Served lane by lane by the
+// whole warp when that is cheaper than a tile pass over the hull [B, E) (issue-slot estimates:
+// tile pass ~11 per record of the longest lane, cooperative ~45 per served lane + 12 per 32
+// records).  Called by all 32 lanes.
+template <int D>
+__device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
+                                           int b1, int e1, int b2, int e2, float qx, float qy, float qz,
+                                           int self, Top2 &best)
+{
+    const bool h1 = b1 < e1, h2 = b2 < e2;
+    const int len = (h1 ? e1 - b1 : 0) + (h2 ? e2 - b2 : 0);
+    const unsigned active = __ballot_sync(0xffffffffu, len > 0);
+    if (!active) return;
+    const int maxlen = __reduce_max_sync(0xffffffffu, len);
+    const int sumlen = __reduce_add_sync(0xffffffffu, len);
+    if (__popc(active) * 360 + sumlen * 3 < maxlen * 88) {
+        for (unsigned a = active; a; a &= a - 1) {
+            const int L = __ffs(a) - 1;
+            const float Lx = __shfl_sync(0xffffffffu, qx, L), Ly = __shfl_sync(0xffffffffu, qy, L);
+            const float Lz = D == 3 ? __shfl_sync(0xffffffffu, qz, L) : 0.f;
+            const int Lself = __shfl_sync(0xffffffffu, self, L);
+            const float thr = __shfl_sync(0xffffffffu, best.s2, L);
+            const int Lj1 = __shfl_sync(0xffffffffu, best.j1, L), Lj2 = __shfl_sync(0xffffffffu, best.j2, L);
+            const int Lb1 = __shfl_sync(0xffffffffu, b1, L), Le1 = __shfl_sync(0xffffffffu, e1, L);
+            const int Lb2 = __shfl_sync(0xffffffffu, b2, L), Le2 = __shfl_sync(0xffffffffu, e2, L);
+            Top2 tmp;
+            tmp.init();
+            coop_range<D>(v, lane, Lb1, Le1, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
+            coop_range<D>(v, lane, Lb2, Le2, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
+            float sa, sb;
+            int ja, jb;
+            coop_pop(tmp, sa, ja);
+            coop_pop(tmp, sb, jb);
+            if (lane == L) {
+                if (ja != KC_NOIDX) best.offer(sa, ja);
+                if (jb != KC_NOIDX) best.offer(sb, jb);
+            }
+        }
+        return;
+    }
+    const int B = __reduce_min_sync(0xffffffffu, min(h1 ? b1 : 0x7fffffff, h2 ? b2 : 0x7fffffff));
+    const int E = __reduce_max_sync(0xffffffffu, max(h1 ? e1 : 0, h2 ? e2 : 0));
+    tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
+}
+
 template <int D>
 __global__ void __launch_bounds__(32 * WT_WARPS)
 search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2,
@@ -488,9 +693,10 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
     float4 *tp4 = s_p4[D == 3 ? warp : 0];
     float2 *tp2 = s_p2[D == 2 ? warp : 0];
     int *tix = s_ix[D == 2 ? warp : 0];
-    if (lane < 4) {                                // inert records behind the tile
-        if (D == 3) tp4[WT_TILE + lane] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-        else { tp2[WT_TILE + lane] = make_float2(qnan, qnan); tix[WT_TILE + lane] = -1; }
+    // the whole tile starts inert: a short range leaves records behind it untouched
+    for (int k = lane; k < WT_TILE + 4; k += 32) {
+        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
     }
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s - lane >= N) return;                     // whole warp past the end
@@ -508,7 +714,7 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
     const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
     const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
     const int rowid = cz * v.G1 + cy;
-    const int lx0 = max(cx - 1, 0), lx1 = min(cx + 1, v.G0 - 1);
+    const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
     Top2 best;
     best.init();
     unsigned todo = 0xffffffffu;
@@ -521,42 +727,46 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
         const int ry = __shfl_sync(0xffffffffu, cy, first), rz = __shfl_sync(0xffffffffu, cz, first);
         const bool mine = (seg >> lane) & 1u;
         const int ux0 = max(xf - 1, 0), ux1 = min(xl + 1, v.G0 - 1);
-        const int z0 = D == 3 ? max(rz - 1, 0) : 0, z1 = D == 3 ? min(rz + 1, v.G2 - 1) : 0;
-        const int y0 = max(ry - 1, 0), y1 = min(ry + 1, v.G1 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y) {
-                const int rowbase = (z * v.G1 + y) * v.G0;
-                const int B = v.cell_start[rowbase + ux0], E = v.cell_start[rowbase + ux1 + 1];
+#pragma unroll 1
+        for (int k = -1; k < (D == 3 ? 8 : 2); ++k) {          // k = -1: the lanes' own row
+            const int oy = k < 0 ? 0 : row_oy(k), oz = k < 0 ? 0 : row_oz(k);
+            const int y = ry + oy, z = rz + oz;
+            if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
+            const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
+            const int B = crow[ux0], E = crow[ux1 + 1];
+            if (B == E) continue;
+            if (E - B < v.dense_thr) {
                 int b = 0, e = 0;
-                if (mine) { b = v.cell_start[rowbase + lx0]; e = v.cell_start[rowbase + lx1 + 1]; }
-                for (int T0 = B; T0 < E; T0 += WT_TILE) {
-#pragma unroll
-                    for (int k = lane; k < WT_TILE; k += 32) {
-                        const int g = T0 + k;
-                        if (D == 3) {
-                            tp4[k] = g < N ? v.spos4[g] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
-                        } else {
-                            tp2[k] = g < N ? v.spos2[g] : make_float2(qnan, qnan);
-                            tix[k] = g < N ? v.sidx[g] : -1;
-                        }
-                    }
-                    __syncwarp();
-                    if (mine) {
-                        const int lb = max(b, T0) - T0, le = min(e, T0 + WT_TILE) - T0;
-                        tile_scan<D>(tp2, tp4, tix, lb, le, qx, qy, qz, self, best);
-                    }
-                    __syncwarp();
-                }
+                if (mine) { b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1]; }
+                tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b, e, 0, 0, qx, qy, qz, self, best);
+                continue;
             }
+            const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
+            if (k < 0) {
+                int s0 = 0, s1 = 0;
+                if (mine) { s0 = crow[cx]; s1 = crow[cx + 1]; }
+                tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
+                int bl = 0, el = 0, br = 0, er = 0;
+                if (mine && has_l && !(best.s2 < g.xm)) { bl = crow[cx - 1]; el = s0; }
+                if (mine && has_r && !(best.s2 < g.xp)) { br = s1; er = crow[cx + 2]; }
+                dense_pass<D>(v, N, lane, tp2, tp4, tix, bl, el, br, er, qx, qy, qz, self, best);
+            } else {
+                int b = 0, e = 0;
+                if (mine) {
+                    const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
+                    if (!(best.s2 < rb2)) {
+                        int x0 = cx, x1 = cx + 1;
+                        if (has_l && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
+                        if (has_r && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 2;
+                        b = crow[x0]; e = crow[x1];
+                    }
+                }
+                dense_pass<D>(v, N, lane, tp2, tp4, tix, b, e, 0, 0, qx, qy, qz, self, best);
+            }
+        }
         todo &= ~seg;
     }
-    int r = 1;
-    {
-        const int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
-        const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
-        if (!bound_ok(v, box_bound<D>(v, qx, qy, qz, lx0, lx1, y0, y1, z0, z1), best.s2))
-            r = ring_continue<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
-    }
+    const int r = finish_block<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
     if (s >= N) return;
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
     store_cert(best, self, nn, nn2, d1, d2, c);
@@ -579,7 +789,7 @@ search_frontier_kernel(View v, const float *__restrict__ p_new, const int32_t *_
         const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
         const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
         const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-        int r = ring_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, max(cx - 1, 0), min(cx + 1, v.G0 - 1), best);
+        int r = block_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
         if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
         store_cert(best, i, nn, nn2, d1, d2, c);
     }
