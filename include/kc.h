@@ -101,19 +101,33 @@ kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d,
                               void *stream);
 
 /* ---- A1: exact all-pairs certificates ("exact N x N pass", Table 2) ---------- */
-/* Workspace the tiled kernel needs for (N, d), in bytes (host; 0 is possible). */
+/* Workspace the tiled kernel needs for (N, d), in bytes (host; 0 only for invalid arguments). */
 size_t kc_cert_allpairs_workspace(int64_t N, int d);
-/* nn,d1,d2,c: device [N]; nn2 device [N] or NULL; workspace: device, >= the size above
- * (may be NULL when that size is 0). */
+/* nn,d1,d2,c: device [N]; nn2 device [N] or NULL; workspace: device, 16-byte aligned, >= the size
+ * above. */
 kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t *nn, int32_t *nn2, float *d1,
                            float *d2, float *c, void *workspace, size_t workspace_bytes,
                            void *stream);
+
+/* A1 started from a kinetic bound.  The certificate logic of Lemma 1: a step in
+ * which no point moves by more than eps changes every pairwise distance by at most 2 eps, so the
+ * new second-neighbour distance of point i is at most d2_prev[i] + 2 eps.  Given such a bound per
+ * point (d2_prev: device float[N], any upper bounds on the previous second-neighbour distances,
+ * e.g. the maintained certificates; eps: device float[1], e.g. kc_max_displacement's output), the
+ * N x N pass evaluates the same N(N-1) pairs but offers only candidates inside the bound to the
+ * top-2 insertion, which a cold start pays ~2 ln N times per point (and, with 32 independent
+ * lanes per warp, in almost every step when N is small).  The result never depends on the bound:
+ * a point for which fewer than two candidates fall inside it (the bound was wrong, NaN, or
+ * stale) is recomputed from scratch in the same call.  Output and workspace as kc_cert_allpairs. */
+kc_status kc_cert_allpairs_bounded(const float *p, int64_t N, int d, const float *d2_prev,
+                                   const float *eps, int32_t *nn, int32_t *nn2, float *d1, float *d2,
+                                   float *c, void *workspace, size_t workspace_bytes, void *stream);
 
 /* ---- NEXT #1: frontier oracle (PAPER.md:69 rtx_frontier_oracle) -------------------------- */
 /* Relabel the queries q[0..*nq) (device int32, distinct ids; *nq read on the device, at most
  * nq_max) against ALL N points by tiled brute force, O(|q| N).  Results are written in place at
  * the query ids (nn[q[k]] ...), other entries are untouched.  workspace: device scratch of at
- * least kc_frontier_oracle_workspace(N, d, nq_max) bytes (NULL allowed when that is 0). */
+ * least kc_frontier_oracle_workspace(N, d, nq_max) bytes, 16-byte aligned. */
 size_t kc_frontier_oracle_workspace(int64_t N, int d, int64_t nq_max);
 kc_status kc_frontier_oracle(const float *p, int64_t N, int d, const int32_t *q, const int32_t *nq,
                              int64_t nq_max, int32_t *nn, int32_t *nn2, float *d1, float *d2,

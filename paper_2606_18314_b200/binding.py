@@ -21,7 +21,8 @@ LIB_PATH = os.path.join(_HERE, "libkc.so")
 
 EXPORTS = (
     "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_max_displacement",
-    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_frontier_oracle_workspace",
+    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded",
+    "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
     "kc_frontier_repair", "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
@@ -75,6 +76,7 @@ def lib():
     L.kc_cert_allpairs_workspace.restype = sz
     L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
     L.kc_cert_allpairs.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.kc_cert_allpairs_bounded.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     L.kc_frontier_oracle_workspace.restype = sz
     L.kc_frontier_oracle_workspace.argtypes = [i64, ci, i64]
     L.kc_frontier_oracle.argtypes = [vp, i64, ci, vp, vp, i64, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -207,14 +209,26 @@ def _workspace(nbytes, device):
     return w
 
 
-def kc_cert_allpairs(p, out: Certs | None = None, workspace=None) -> Certs:
-    """A1: exact all-pairs certificates (Table 2)."""
+def kc_cert_allpairs(p, out: Certs | None = None, workspace=None, d2_prev=None, eps=None) -> Certs:
+    """A1: exact all-pairs certificates (Table 2).  With ``d2_prev`` (float32[N]) and
+    ``eps`` (float32[1]) the pass starts from the kinetic bound d2_prev + 2 eps
+    (kc_cert_allpairs_bounded); the result is the same bits either way."""
     pp, N, d = _pos(p)
     out = out or Certs.empty(N, p.device)
     need = lib().kc_cert_allpairs_workspace(N, d)
     ws = workspace if workspace is not None else _workspace(need, p.device)
-    _check(lib().kc_cert_allpairs(pp, N, d, *out._ptrs(), _ptr(ws), ws.numel() if ws is not None else 0,
-                                  _stream()), "kc_cert_allpairs")
+    if (d2_prev is None) != (eps is None):
+        raise ValueError("d2_prev and eps go together")
+    if d2_prev is None:
+        _check(lib().kc_cert_allpairs(pp, N, d, *out._ptrs(), _ptr(ws), ws.numel() if ws is not None else 0,
+                                      _stream()), "kc_cert_allpairs")
+    else:
+        if d2_prev.numel() != N:
+            raise ValueError("d2_prev must have N entries")
+        _check(lib().kc_cert_allpairs_bounded(pp, N, d, _ptr(d2_prev, torch.float32, "d2_prev"),
+                                              _ptr(eps, torch.float32, "eps"), *out._ptrs(), _ptr(ws),
+                                              ws.numel() if ws is not None else 0, _stream()),
+               "kc_cert_allpairs_bounded")
     return out
 
 

@@ -9,8 +9,13 @@
 //   * fast path per (query, 4 candidates): 4 distances, min of them, ONE compare against the
 //     current second-best; the exact (s, j)-ordered insertion (ties, self, tail) runs only in the
 //     rarely taken slow path (~2 ln N times per query);
-//   * j is split across gridDim.y so small N still fills 148 SMs; partial top-2s are merged by
-//     a second kernel under the same total order, so the split never changes a result.
+//   * j is split across gridDim.y so small N still fills 148 SMs; the CTA that finishes a query
+//     block's last chunk merges the partial top-2s under the same total order, so the split never
+//     changes a result;
+//   * when j is split, a seed pass first gives every query its exact top-2 over the first AP_SEED
+//     points (warp-cooperative, branch-free), and every chunk starts from that instead of from
+//     +inf: a chunk that starts cold pays ~2 ln(chunk) insertions per lane, and with 32 independent
+//     lanes that puts some lane on the insertion path in almost every step of a short chunk.
 #include <stdlib.h>
 
 #include "kc_common.cuh"
@@ -20,6 +25,7 @@ using namespace kc;
 namespace {
 
 constexpr int AP_TJ = 1024;   // candidates per shared-memory tile
+constexpr int AP_SEED = 256;  // points scanned by the seed pass of a j-split launch
 
 struct Partial { float s1, s2; int j1, j2; };   // 16 B
 
@@ -160,70 +166,207 @@ __device__ __forceinline__ void scan_chunk(const float *__restrict__ p, int64_t 
     }
 }
 
-// grid = (ceil(nq / (QPT*THREADS)), JS).  qlist == nullptr: queries are 0..N-1.
+// Everything a launch needs; passed by value.
+struct ApArgs {
+    const float *p;
+    int64_t N;
+    const int32_t *qlist;        // null: queries are 0..N-1
+    const int32_t *nq_dev;       // null: nq_host queries
+    int64_t nq_host;
+    int64_t jchunk, jfirst;      // chunk y scans candidates [jfirst + y*jchunk, +jchunk)
+    u64 one2;
+    const Partial *seed;         // unbounded j-split: exact top-2 over points [0, jfirst)
+    const float *bound_d2;       // kinetic bound (both or neither): every query's second neighbour is
+    const float *bound_eps;      //   claimed to lie within bound_d2[i] + 2 * bound_eps[0]
+    Partial *part;               // j-split: partial lists [js][nq_host]; null: store certificates
+    int32_t *redo, *n_redo;      // queries whose bound admitted fewer than two candidates
+    int32_t *tickets;            // j-split: chunks finished per query block (the last one merges)
+    int32_t *nn, *nn2;
+    float *d1, *d2, *c;
+};
+
+// grid = (ceil(nq / (QPT*THREADS)), JS).
 template <int D, int QPT, int C4, int THREADS>
 __global__ void __launch_bounds__(THREADS)
-allpairs_kernel(const float *__restrict__ p, int64_t N, const int32_t *__restrict__ qlist,
-                const int32_t *__restrict__ nq_dev, int64_t nq_host, int64_t jchunk, u64 one2,
-                Partial *__restrict__ part, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
+allpairs_kernel(const ApArgs a)
 {
     __shared__ __align__(16) float sx[AP_TJ];
     __shared__ __align__(16) float sy[AP_TJ];
     __shared__ __align__(16) float sz[D == 3 ? AP_TJ : 4];
-    const int64_t nq = nq_dev ? (int64_t)*nq_dev : nq_host;
+    const float *__restrict__ p = a.p;
+    const int64_t nq = a.nq_dev ? (int64_t)*a.nq_dev : a.nq_host;
     const int64_t q0 = blockIdx.x * (int64_t)(QPT * THREADS);
     if (q0 >= nq) return;
     float qx[QPT], qy[QPT], qz[QPT];
     int qi[QPT];
     Top2 best[QPT];
+    const float eps2 = a.bound_d2 ? 2.0f * a.bound_eps[0] : 0.f;
 #pragma unroll
     for (int k = 0; k < QPT; ++k) {
         int64_t q = q0 + k * THREADS + threadIdx.x;
         int i = -1;
-        if (q < nq) i = qlist ? qlist[q] : (int)q;
+        if (q < nq) i = a.qlist ? a.qlist[q] : (int)q;
         qi[k] = i;
         qx[k] = qy[k] = qz[k] = 0.f;
+        best[k].init();
         if (i >= 0) {
             qx[k] = p[(int64_t)i * D + 0];
             qy[k] = p[(int64_t)i * D + 1];
             if (D == 3) qz[k] = p[(int64_t)i * D + 2];
+            if (a.seed) {                         // exact top-2 over points [0, jfirst)
+                const int4 raw = reinterpret_cast<const int4 *>(a.seed)[q];
+                best[k].s1 = __int_as_float(raw.x); best[k].s2 = __int_as_float(raw.y);
+                best[k].j1 = raw.z; best[k].j2 = raw.w;
+            }
+            if (a.bound_d2) {
+                // start from two placeholders (T, no index): candidates beyond T are never
+                // inserted; T is inflated by 2^-9, far above every rounding on the way
+                const float b = (a.bound_d2[i] + eps2) * 1.001953125f;
+                best[k].s1 = best[k].s2 = b * b;
+            }
         }
-        best[k].init();
     }
-    const int64_t jbeg = blockIdx.y * jchunk;
-    const int64_t jend = min(N, jbeg + jchunk);
-    scan_chunk<D, QPT, C4, THREADS>(p, N, jbeg, jend, qx, qy, qz, qi, best, sx, sy, sz, one2);
+    const int64_t jbeg = a.jfirst + blockIdx.y * a.jchunk;
+    const int64_t jend = min(a.N, jbeg + a.jchunk);
+    scan_chunk<D, QPT, C4, THREADS>(p, a.N, jbeg, jend, qx, qy, qz, qi, best, sx, sy, sz, a.one2);
+    if (a.part) {
+        // j-split: publish this chunk's partial lists; the CTA that takes the last ticket of the
+        // query block merges all of them (they are read through L2: other SMs wrote them)
 #pragma unroll
-    for (int k = 0; k < QPT; ++k) {
-        int64_t q = q0 + k * THREADS + threadIdx.x;
-        if (qi[k] < 0) continue;
-        if (gridDim.y == 1) {
-            store_cert(best[k], qi[k], nn, nn2, d1, d2, c);
-        } else {
+        for (int k = 0; k < QPT; ++k) {
+            int64_t q = q0 + k * THREADS + threadIdx.x;
+            if (qi[k] < 0) continue;
             Partial o;
             o.s1 = best[k].s1; o.s2 = best[k].s2; o.j1 = best[k].j1; o.j2 = best[k].j2;
-            part[blockIdx.y * nq_host + q] = o;
+            a.part[blockIdx.y * a.nq_host + q] = o;
         }
+        __shared__ int s_last;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) s_last = atomicAdd(&a.tickets[blockIdx.x], 1) == (int)gridDim.y - 1;
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+#pragma unroll
+        for (int k = 0; k < QPT; ++k) {
+            int64_t q = q0 + k * THREADS + threadIdx.x;
+            if (qi[k] < 0) continue;
+            Top2 t;
+            t.init();
+            // every list starts from the same seed entries (or placeholders): skip ids already
+            // held and entries without an index
+            for (int y = 0; y < (int)gridDim.y; ++y) {
+                const int4 raw = __ldcg(reinterpret_cast<const int4 *>(a.part) + (y * a.nq_host + q));
+                const float s1 = __int_as_float(raw.x), s2 = __int_as_float(raw.y);
+                if (raw.z != KC_NOIDX && raw.z != t.j1 && raw.z != t.j2) t.offer(s1, raw.z);
+                if (raw.w != KC_NOIDX && raw.w != t.j1 && raw.w != t.j2) t.offer(s2, raw.w);
+            }
+            best[k] = t;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < QPT; ++k) {
+        if (qi[k] < 0) continue;
+        if (a.bound_d2 && best[k].j2 == KC_NOIDX) a.redo[atomicAdd(a.n_redo, 1)] = qi[k];
+        else store_cert(best[k], qi[k], a.nn, a.nn2, a.d1, a.d2, a.c);
     }
 }
 
-__global__ void __launch_bounds__(256)
-allpairs_merge_kernel(const Partial *__restrict__ part, int64_t nq_host, int js,
-                      const int32_t *__restrict__ qlist, const int32_t *__restrict__ nq_dev,
-                      int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
+__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
 {
-    const int64_t nq = nq_dev ? (int64_t)*nq_dev : nq_host;
-    int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (q >= nq) return;
-    Top2 t;
-    t.init();
-    for (int s = 0; s < js; ++s) {
-        const int4 raw = reinterpret_cast<const int4 *>(part)[s * nq_host + q];
-        Top2 o;
-        o.s1 = __int_as_float(raw.x); o.s2 = __int_as_float(raw.y); o.j1 = raw.z; o.j2 = raw.w;
-        t.merge(o);
+    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
+    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
+    const float ns2 = lt1 ? b.s1 : s;
+    const int nj2 = lt1 ? b.j1 : j;
+    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
+    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
+}
+// smallest key (s, j) over the warp's private lists, removed from the list that held it
+__device__ __forceinline__ void warp_pop(Top2 &tmp, float &s, int &j)
+{
+    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
+    const unsigned m = __reduce_min_sync(0xffffffffu, key);
+    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
+    s = __uint_as_float(m);
+    if (key == m && tmp.j1 == j) {
+        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
+        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
     }
-    store_cert(t, qlist ? qlist[q] : (int)q, nn, nn2, d1, d2, c);
+}
+// Seed pass: one warp per query at a time, the 32 lanes take different candidates of [0, S) and
+// keep a private top-2 with branch-free selects; two warp reductions pick the two smallest keys.
+template <int D>
+__global__ void __launch_bounds__(256)
+allpairs_seed_kernel(const ApArgs a, int S, Partial *__restrict__ seed)
+{
+    __shared__ float sx[AP_SEED], sy[AP_SEED], sz[D == 3 ? AP_SEED : 1];
+    const float *__restrict__ p = a.p;
+    for (int t = threadIdx.x; t < S; t += blockDim.x) {
+        sx[t] = p[(int64_t)t * D]; sy[t] = p[(int64_t)t * D + 1];
+        if (D == 3) sz[t] = p[(int64_t)t * D + 2];
+    }
+    __syncthreads();
+    const int64_t nq = a.nq_dev ? (int64_t)*a.nq_dev : a.nq_host;
+    const int lane = threadIdx.x & 31;
+    const int64_t w0 = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int64_t nw = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t q = w0; q < nq; q += nw) {
+        const int i = a.qlist ? a.qlist[q] : (int)q;
+        const float qx = p[(int64_t)i * D], qy = p[(int64_t)i * D + 1];
+        const float qz = D == 3 ? p[(int64_t)i * D + 2] : 0.f;
+        Top2 tmp;
+        tmp.init();
+        for (int t = lane; t < S; t += 32) {
+            const float s = D == 2 ? sqd2(qx, qy, sx[t], sy[t]) : sqd3(qx, qy, qz, sx[t], sy[t], sz[t]);
+            insert_bf(tmp, s, t, t != i);
+        }
+        Partial o;
+        warp_pop(tmp, o.s1, o.j1);
+        warp_pop(tmp, o.s2, o.j2);
+        if (lane == 0) seed[q] = o;
+    }
+}
+
+// Redo pass of a bounded launch: the queries whose bound admitted fewer than two candidates (a
+// bound that was not one) are recomputed from scratch, one CTA per query, so that the result
+// never depends on the bound.  Empty in normal operation.
+template <int D>
+__global__ void __launch_bounds__(256)
+allpairs_redo_kernel(const ApArgs a)
+{
+    __shared__ float ws[8][2];
+    __shared__ int wj[8][2];
+    const float *__restrict__ p = a.p;
+    const int n = *a.n_redo;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int r = blockIdx.x; r < n; r += gridDim.x) {
+        const int i = a.redo[r];
+        const float qx = p[(int64_t)i * D], qy = p[(int64_t)i * D + 1];
+        const float qz = D == 3 ? p[(int64_t)i * D + 2] : 0.f;
+        Top2 tmp;
+        tmp.init();
+        for (int64_t t = threadIdx.x; t < a.N; t += 256) {
+            const float s = D == 2 ? sqd2(qx, qy, p[t * D], p[t * D + 1])
+                                   : sqd3(qx, qy, qz, p[t * D], p[t * D + 1], p[t * D + 2]);
+            insert_bf(tmp, s, (int)t, t != i);
+        }
+        float s1, s2;
+        int j1, j2;
+        warp_pop(tmp, s1, j1);
+        warp_pop(tmp, s2, j2);
+        if (lane == 0) { ws[warp][0] = s1; ws[warp][1] = s2; wj[warp][0] = j1; wj[warp][1] = j2; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            Top2 t;
+            t.init();
+            for (int w = 0; w < 8; ++w) {
+                if (wj[w][0] != KC_NOIDX) t.offer(ws[w][0], wj[w][0]);
+                if (wj[w][1] != KC_NOIDX) t.offer(ws[w][1], wj[w][1]);
+            }
+            store_cert(t, i, a.nn, a.nn2, a.d1, a.d2, a.c);
+        }
+        __syncthreads();
+    }
 }
 
 // Launch shape.  Tuning overrides for experiments: KC_AP_QPT, KC_AP_C4, KC_AP_THREADS, KC_AP_JS
@@ -247,12 +390,12 @@ Shape choose_shape(int64_t nq, int64_t N)
     s.c4 = s.qpt == 4 ? 2 : (s.qpt == 2 ? 2 : 4);
     if (e_c4 == 1 || e_c4 == 2 || e_c4 == 4) s.c4 = e_c4;
     if (e_thr == 32 || e_thr == 64 || e_thr == 128) s.threads = e_thr;
-    // j-split: many waves deep, but every CTA still scans >= 4 tiles (short chunks pay the
-    // ~2 ln(n) insertions per lane again in every chunk)
+    // j-split: many waves deep; chunks are whole tiles and start from the seed pass (or from the
+    // caller's bound), so one tile per chunk is enough
     int64_t per = (int64_t)s.qpt * s.threads;
     int64_t itiles = (nq + per - 1) / per;
     int64_t want = (148 * 8 * 8 + itiles - 1) / itiles;
-    int64_t cap = N / (4 * AP_TJ);
+    int64_t cap = (N - AP_SEED) / AP_TJ;
     int64_t js = want < cap ? want : cap;
     if (e_js > 0) js = e_js;
     if (js < 1) js = 1;
@@ -261,34 +404,64 @@ Shape choose_shape(int64_t nq, int64_t N)
     return s;
 }
 
-template <int D, int QPT, int C4>
-void launch_t(int threads, dim3 grid, cudaStream_t st, const float *p, int64_t N, const int32_t *q,
-              const int32_t *nq_dev, int64_t nq, int64_t jchunk, Partial *part, int32_t *nn,
-              int32_t *nn2, float *d1, float *d2, float *c)
+// Workspace layout: [n_redo: 16 B][tickets: one int32 per query block, padded to 16 B]
+// [redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last two only for a j-split
+// shape).  n_redo and the tickets are zeroed by one memset per call.
+size_t pad16(size_t b) { return (b + 15) & ~(size_t)15; }
+size_t qblocks_for(int64_t nq, const Shape &sh)
 {
-    const u64 one2 = 0x3f8000003f800000ull;
-    if (threads == 32)
-        allpairs_kernel<D, QPT, C4, 32><<<grid, 32, 0, st>>>(p, N, q, nq_dev, nq, jchunk, one2, part, nn, nn2, d1, d2, c);
-    else if (threads == 64)
-        allpairs_kernel<D, QPT, C4, 64><<<grid, 64, 0, st>>>(p, N, q, nq_dev, nq, jchunk, one2, part, nn, nn2, d1, d2, c);
-    else
-        allpairs_kernel<D, QPT, C4, 128><<<grid, 128, 0, st>>>(p, N, q, nq_dev, nq, jchunk, one2, part, nn, nn2, d1, d2, c);
+    const int64_t per = (int64_t)sh.qpt * sh.threads;
+    return (size_t)((nq + per - 1) / per);
+}
+size_t head_bytes(int64_t nq, const Shape &sh) { return 16 + pad16(4 * qblocks_for(nq, sh)); }
+size_t workspace_bytes_for(int64_t nq, const Shape &sh)
+{
+    return head_bytes(nq, sh) + pad16((size_t)nq * 4) +
+           (sh.js > 1 ? ((size_t)sh.js + 1) * (size_t)nq * sizeof(Partial) : 0);
+}
+
+template <int D, int QPT, int C4>
+void launch_t(int threads, dim3 grid, cudaStream_t st, const ApArgs &a)
+{
+    if (threads == 32) allpairs_kernel<D, QPT, C4, 32><<<grid, 32, 0, st>>>(a);
+    else if (threads == 64) allpairs_kernel<D, QPT, C4, 64><<<grid, 64, 0, st>>>(a);
+    else allpairs_kernel<D, QPT, C4, 128><<<grid, 128, 0, st>>>(a);
 }
 
 template <int D>
-kc_status launch(const float *p, int64_t N, const int32_t *q, const int32_t *nq_dev, int64_t nq,
-                 int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c, Partial *part, Shape sh,
-                 cudaStream_t st)
+kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
 {
+    const int64_t nq = a.nq_host;
+    const bool split = sh.js > 1, bounded = a.bound_d2 != nullptr;
+    a.one2 = 0x3f8000003f800000ull;
+    a.n_redo = reinterpret_cast<int32_t *>(ws);
+    a.tickets = reinterpret_cast<int32_t *>(ws + 16);
+    a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
+    Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
+    if (split || bounded) KC_CUDA(cudaMemsetAsync(ws, 0, split ? head_bytes(nq, sh) : 16, st));
+    a.jfirst = split && !bounded ? AP_SEED : 0;
     int js = sh.js;
-    int64_t jchunk = (N + js - 1) / js;
-    jchunk = (jchunk + 15) / 16 * 16;
-    js = (int)((N + jchunk - 1) / jchunk);
+    int64_t jchunk = (a.N - a.jfirst + js - 1) / js;
+    // whole tiles per chunk when split (a tile is evaluated in full, +inf padding included)
+    const int64_t gran = split ? AP_TJ : 16;
+    jchunk = (jchunk + gran - 1) / gran * gran;
+    js = (int)((a.N - a.jfirst + jchunk - 1) / jchunk);
+    a.jchunk = jchunk;
+    a.seed = nullptr;
+    a.part = split ? seed + nq : nullptr;
+    int launches = 1;
+    if (split && !bounded) {
+        const int blocks = (int)((nq + 7) / 8 < 148 * 8 ? (nq + 7) / 8 : 148 * 8);
+        if (D == 2) allpairs_seed_kernel<2><<<blocks, 256, 0, st>>>(a, (int)a.jfirst, seed);
+        else allpairs_seed_kernel<3><<<blocks, 256, 0, st>>>(a, (int)a.jfirst, seed);
+        a.seed = seed;
+        ++launches;
+    }
     const int per = sh.qpt * sh.threads;
     dim3 grid((unsigned)((nq + per - 1) / per), (unsigned)js);
-#define KC_AP_CASE(Q, C)                                                                            \
-    if (sh.qpt == Q && sh.c4 == C) {                                                                \
-        launch_t<D, Q, C>(sh.threads, grid, st, p, N, q, nq_dev, nq, jchunk, part, nn, nn2, d1, d2, c); \
+#define KC_AP_CASE(Q, C)                                           \
+    if (sh.qpt == Q && sh.c4 == C) {                               \
+        launch_t<D, Q, C>(sh.threads, grid, st, a);                \
     } else
     KC_AP_CASE(4, 1) KC_AP_CASE(4, 2) KC_AP_CASE(2, 1) KC_AP_CASE(2, 2) KC_AP_CASE(2, 4)
     KC_AP_CASE(1, 1) KC_AP_CASE(1, 2) KC_AP_CASE(1, 4)
@@ -297,11 +470,38 @@ kc_status launch(const float *p, int64_t N, const int32_t *q, const int32_t *nq_
         return KC_EINVAL;
     }
 #undef KC_AP_CASE
-    if (js > 1)
-        allpairs_merge_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(part, nq, js, q, nq_dev, nn, nn2, d1, d2, c);
-    count_launches(js > 1 ? 2 : 1);
+    if (bounded) {
+        const int blocks = (int)(nq < 148 * 4 ? nq : 148 * 4);
+        if (D == 2) allpairs_redo_kernel<2><<<blocks, 256, 0, st>>>(a);
+        else allpairs_redo_kernel<3><<<blocks, 256, 0, st>>>(a);
+        ++launches;
+    }
+    count_launches(launches);
     KC_LAUNCH_CHECK("kc_cert_allpairs");
     return KC_OK;
+}
+
+kc_status run(const char *who, const float *p, int64_t N, int d, const int32_t *q, const int32_t *nq_dev,
+              int64_t nq, const float *d2_prev, const float *eps, int32_t *nn, int32_t *nn2, float *d1,
+              float *d2, float *c, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!p || !nn || !d1 || !d2 || !c || N < 2 || N > 0x7ffffff0 || (d != 2 && d != 3) ||
+        (reinterpret_cast<uintptr_t>(p) & 7) || (d2_prev != nullptr) != (eps != nullptr)) {
+        set_error("%s: bad argument", who);
+        return KC_EINVAL;
+    }
+    const Shape sh = choose_shape(nq, N);
+    const size_t need = workspace_bytes_for(nq, sh);
+    if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15)) {
+        set_error("%s: workspace of %zu bytes (16-byte aligned) required", who, need);
+        return KC_EINVAL;
+    }
+    ApArgs a = {};
+    a.p = p; a.N = N; a.qlist = q; a.nq_dev = nq_dev; a.nq_host = nq;
+    a.bound_d2 = d2_prev; a.bound_eps = eps;
+    a.nn = nn; a.nn2 = nn2; a.d1 = d1; a.d2 = d2; a.c = c;
+    if (d == 2) return launch<2>(a, (char *)workspace, sh, (cudaStream_t)stream);
+    return launch<3>(a, (char *)workspace, sh, (cudaStream_t)stream);
 }
 
 }  // namespace
@@ -309,29 +509,28 @@ kc_status launch(const float *p, int64_t N, const int32_t *q, const int32_t *nq_
 extern "C" size_t kc_cert_allpairs_workspace(int64_t N, int d)
 {
     if (N < 2 || (d != 2 && d != 3)) return 0;
-    int js = choose_shape(N, N).js;
-    return js > 1 ? (size_t)js * (size_t)N * sizeof(Partial) : 0;
+    return workspace_bytes_for(N, choose_shape(N, N));
 }
 
 extern "C" kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t *nn, int32_t *nn2,
                                       float *d1, float *d2, float *c, void *workspace,
                                       size_t workspace_bytes, void *stream)
 {
-    if (!p || !nn || !d1 || !d2 || !c || N < 2 || N > 0x7ffffff0 || (d != 2 && d != 3) ||
-        (reinterpret_cast<uintptr_t>(p) & 7)) {
-        set_error("kc_cert_allpairs: bad argument");
+    return run("kc_cert_allpairs", p, N, d, nullptr, nullptr, N, nullptr, nullptr, nn, nn2, d1, d2, c,
+               workspace, workspace_bytes, stream);
+}
+
+extern "C" kc_status kc_cert_allpairs_bounded(const float *p, int64_t N, int d, const float *d2_prev,
+                                              const float *eps, int32_t *nn, int32_t *nn2, float *d1,
+                                              float *d2, float *c, void *workspace,
+                                              size_t workspace_bytes, void *stream)
+{
+    if (!d2_prev || !eps) {
+        set_error("kc_cert_allpairs_bounded: d2_prev and eps must be non-NULL");
         return KC_EINVAL;
     }
-    size_t need = kc_cert_allpairs_workspace(N, d);
-    if (need > 0 && (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15))) {
-        set_error("kc_cert_allpairs: workspace of %zu bytes (16-byte aligned) required", need);
-        return KC_EINVAL;
-    }
-    Shape sh = choose_shape(N, N);
-    cudaStream_t st = (cudaStream_t)stream;
-    if (d == 2)
-        return launch<2>(p, N, nullptr, nullptr, N, nn, nn2, d1, d2, c, (Partial *)workspace, sh, st);
-    return launch<3>(p, N, nullptr, nullptr, N, nn, nn2, d1, d2, c, (Partial *)workspace, sh, st);
+    return run("kc_cert_allpairs_bounded", p, N, d, nullptr, nullptr, N, d2_prev, eps, nn, nn2, d1, d2, c,
+               workspace, workspace_bytes, stream);
 }
 
 // NEXT #1 (PAPER.md:69 rtx_frontier_oracle): relabel a query subset against all N points.
@@ -340,8 +539,7 @@ extern "C" kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t 
 extern "C" size_t kc_frontier_oracle_workspace(int64_t N, int d, int64_t nq_max)
 {
     if (N < 2 || nq_max < 1 || (d != 2 && d != 3)) return 0;
-    int js = choose_shape(nq_max, N).js;
-    return js > 1 ? (size_t)js * (size_t)nq_max * sizeof(Partial) : 0;
+    return workspace_bytes_for(nq_max, choose_shape(nq_max, N));
 }
 
 extern "C" kc_status kc_frontier_oracle(const float *p, int64_t N, int d, const int32_t *q,
@@ -349,19 +547,11 @@ extern "C" kc_status kc_frontier_oracle(const float *p, int64_t N, int d, const 
                                         float *d1, float *d2, float *c, void *workspace,
                                         size_t workspace_bytes, void *stream)
 {
-    if (!p || !q || !nq || !nn || !d1 || !d2 || !c || N < 2 || N > 0x7ffffff0 || nq_max < 0 ||
-        (d != 2 && d != 3) || (reinterpret_cast<uintptr_t>(p) & 7)) {
+    if (!q || !nq || nq_max < 0) {
         set_error("kc_frontier_oracle: bad argument");
         return KC_EINVAL;
     }
     if (nq_max == 0) return KC_OK;
-    size_t need = kc_frontier_oracle_workspace(N, d, nq_max);
-    if (need > 0 && (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 15))) {
-        set_error("kc_frontier_oracle: workspace of %zu bytes (16-byte aligned) required", need);
-        return KC_EINVAL;
-    }
-    cudaStream_t st = (cudaStream_t)stream;
-    Shape sh = choose_shape(nq_max, N);
-    if (d == 2) return launch<2>(p, N, q, nq, nq_max, nn, nn2, d1, d2, c, (Partial *)workspace, sh, st);
-    return launch<3>(p, N, q, nq, nq_max, nn, nn2, d1, d2, c, (Partial *)workspace, sh, st);
+    return run("kc_frontier_oracle", p, N, d, q, nq, nq_max, nullptr, nullptr, nn, nn2, d1, d2, c,
+               workspace, workspace_bytes, stream);
 }

@@ -864,18 +864,39 @@ __global__ void __launch_bounds__(256)
 entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF,
                        const int32_t *__restrict__ cell, int32_t *fcount, int32_t *mhist, Counters *ctr)
 {
+    // almost every cell holds a handful of frontier points, so the low bins of M[k] would take one
+    // global atomic per cell on a few addresses: they are aggregated per block in shared memory
+    constexpr int LOW = 64;
+    __shared__ int low[LOW];
+    if (threadIdx.x < LOW) low[threadIdx.x] = 0;
+    __syncthreads();
     int n = *nF;
     int m_local = 0;
+    int c1 = 0, c2 = 0, c3 = 0, c4 = 0;             // the commonest counts stay in registers
     for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
         int k = atomicExch(&fcount[cell[F[f]]], 0);     // first visitor collects and re-zeroes
         if (k > 0) {
             ++m_local;
-            if (k < MHIST) atomicAdd(&mhist[k], 1);
-            else atomicAdd(&ctr->big, (double)k * log((double)k));
+            c1 += k == 1; c2 += k == 2; c3 += k == 3; c4 += k == 4;
+            if (k > 4) {
+                if (k < LOW) atomicAdd(&low[k], 1);
+                else if (k < MHIST) atomicAdd(&mhist[k], 1);
+                else atomicAdd(&ctr->big, (double)k * log((double)k));
+            }
         }
     }
     m_local = __reduce_add_sync(0xffffffffu, m_local);
-    if ((threadIdx.x & 31) == 0 && m_local) atomicAdd(&ctr->m_cells, m_local);
+    c1 = __reduce_add_sync(0xffffffffu, c1); c2 = __reduce_add_sync(0xffffffffu, c2);
+    c3 = __reduce_add_sync(0xffffffffu, c3); c4 = __reduce_add_sync(0xffffffffu, c4);
+    if ((threadIdx.x & 31) == 0) {
+        if (m_local) atomicAdd(&ctr->m_cells, m_local);
+        if (c1) atomicAdd(&low[1], c1);
+        if (c2) atomicAdd(&low[2], c2);
+        if (c3) atomicAdd(&low[3], c3);
+        if (c4) atomicAdd(&low[4], c4);
+    }
+    __syncthreads();
+    if (threadIdx.x < LOW && low[threadIdx.x]) atomicAdd(&mhist[threadIdx.x], low[threadIdx.x]);
 }
 __global__ void __launch_bounds__(1024)
 entropy_finish_kernel(const int32_t *__restrict__ nF, int32_t *mhist, Counters *ctr, double *H,

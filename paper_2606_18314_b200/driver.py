@@ -9,7 +9,7 @@ PAPER.md:69-73):
     A6+A7  REPAIR path: incremental cell update + search of F  kc_frontier_repair  (Alg. 1 l.3-7)
     A5  H(F), m, C on the updated filing                     kc_frontier_entropy   (Def. 2)
     A2+A3  REBUILD path: O(N) grid rebuild at p'             kc_cert_grid_rebuild
-    A1  all-pairs certification at p'                        kc_cert_allpairs
+    A1  all-pairs certification at p'                        kc_cert_allpairs[_bounded]
 
 This module is host orchestration only: every arithmetic step runs in libkc's kernels.  It owns
 the device buffers (torch tensors) and hands pointers to the C-ABI through :mod:`.binding`.
@@ -69,7 +69,7 @@ class Maintainer:
 
     def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None,
              frontier: torch.Tensor | None = None, time_phases: bool = False,
-             do_allpairs: bool = True) -> StepResult:
+             do_allpairs: bool = True, bounded_allpairs: bool = True) -> StepResult:
         """One transition p -> p_next through every row of the hot path.
 
         ``movers``: optional int32 id list of the points that moved (None = all may have moved).
@@ -105,7 +105,13 @@ class Maintainer:
         self.certs, self.other = self.other, self.certs
         mark("rebuild")
         if do_allpairs and self.ap is not None:
-            kc.kc_cert_allpairs(p_next, self.ap, self.ws)
+            # the maintained certificates bound the new second-neighbour distance by d2 + 2 eps_t
+            # (Lemma 1's triangle inequality; entries repaired above already hold the
+            # new d2); the pass is exact whatever the bound (kc_cert_allpairs_bounded)
+            if bounded_allpairs:
+                kc.kc_cert_allpairs(p_next, self.ap, self.ws, d2_prev=repaired.d2, eps=self.eps)
+            else:
+                kc.kc_cert_allpairs(p_next, self.ap, self.ws)
         mark("allpairs")
         self.p = p_next
         res = StepResult(self.eps, nF, self.H, self.m, self.C, repaired, self.certs,

@@ -63,7 +63,7 @@ def test_bad_arguments_are_rejected(L):
         binding.kc_geom_from_bbox(100, 4, [0, 0, 0], [1, 1, 1])
     with pytest.raises(binding.KcError):
         binding.kc_geom_from_bbox(100, 2, [0, 0, 0], [1, 1, 1], occ=0.0)
-    assert L.kc_cert_allpairs_workspace(1, 2) == 0
+    assert L.kc_cert_allpairs_workspace(1, 2) == 0 and L.kc_cert_allpairs_workspace(1000, 2) > 0
     # NULL pointers are refused before any CUDA call
     assert L.kc_cert_allpairs(None, 100, 2, None, None, None, None, None, None, 0, None) == binding.KC_EINVAL
     assert L.kc_max_displacement(None, None, 10, 2, None, None) == binding.KC_EINVAL

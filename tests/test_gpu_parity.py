@@ -101,6 +101,31 @@ def test_allpairs_and_rebuild_configs(cfg, N):
     assert_same(kc.kc_cert_grid_rebuild(grid, P), want, what=f"rebuild {cfg} {N}")
 
 
+@pytest.mark.parametrize("cfg,N", [("cfg1", 1000), ("cfg2", 16000), ("cfg3", 16000), ("cfg4", 100000)])
+def test_allpairs_bounded_is_exact_for_any_bound(cfg, N):
+    """kc_cert_allpairs_bounded (kinetic bound d2_prev + 2 eps, Lemma 1's triangle inequality,
+    PAPER.md:33): same bits as the oracle for a true bound, a useless one, a wrong one and NaN."""
+    p, mot = wl.make_scene(cfg) if cfg != "cfg4" else (wl.make_points(cfg, N=N), None)
+    if mot is None:
+        q = (p + np.float32(1e-4) * wl.uniform_points(N, p.shape[1], 5)).astype(np.float32)
+    else:
+        q, _ = mot.step(p)
+    pre, want = ref_certs(p), ref_certs(q)
+    Q = dev(q)
+    eps = dev(np.array([oracle.max_displacement(p, q)], np.float32))
+    rng = np.random.default_rng(3)
+    wrong = pre.d2.copy()
+    k = rng.choice(N, N // 7, replace=False)
+    wrong[k] = 0.0                                     # no candidate inside: recomputed from scratch
+    wrong[rng.choice(N, 50, replace=False)] = np.nan
+    half = np.maximum(want.d1 - 2 * eps.cpu().numpy()[0], 0).astype(np.float32)   # admits only the nearest
+    bounds = {"kinetic": pre.d2, "inf": np.full(N, np.inf, np.float32), "huge": np.full(N, 10.0, np.float32),
+              "zero": np.zeros(N, np.float32), "mixed": wrong, "one_candidate": half}
+    for name, b in bounds.items():
+        got = kc.kc_cert_allpairs(Q, d2_prev=dev(b), eps=eps)
+        assert_same(got, want, what=f"bounded allpairs {cfg} bound={name}")
+
+
 def test_grid_with_points_outside_the_box():
     # geometry fitted to the central half of the points: the rest is clamped into boundary cells
     p = wl.uniform_points(20000, 3, 31)
