@@ -32,7 +32,8 @@ struct Counters {
     int max_occ;
     int n_stragglers;
     int m_cells;
-    int pad[3];
+    int n_list2;              // frontier points of the current sweep that live in chains
+    int pad[2];
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -41,6 +42,7 @@ struct View {
     float lo0, lo1, lo2, h, inv_h, shrink;
     float slk0, slk1, slk2;   // absolute rounding slack of a computed face / cell boundary per axis
     int dense_thr;            // a row range of at least this many records is handled as dense (A3)
+    int wpq_max;              // id lists up to this long are served one warp per query (A7)
     const int32_t *cell_start;
     const float2 *spos2;
     const float4 *spos4;
@@ -59,6 +61,9 @@ struct kc_grid {
     size_t bytes;
     int32_t *cell, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
     int32_t *blocksums;
+    int32_t *mark;            // per sorted slot: epoch of the last sweep that queried it
+    int32_t *list2;           // frontier points of the current sweep that live in chains
+    int epoch;
     float2 *spos2;
     float4 *spos4, *opos;
     Counters *ctr;
@@ -88,6 +93,8 @@ View make_view(const kc_grid *g)
     v.slk0 = slk[0]; v.slk1 = slk[1]; v.slk2 = slk[2];
     static const int dense_env = getenv("KC_DENSE_THR") ? atoi(getenv("KC_DENSE_THR")) : 0;
     v.dense_thr = dense_env > 0 ? dense_env : 128;
+    static const int wpq_env = getenv("KC_WPQ_MAX") ? atoi(getenv("KC_WPQ_MAX")) : -1;
+    v.wpq_max = wpq_env >= 0 ? wpq_env : 32768;
     v.cell_start = g->cell_start;
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;
@@ -294,6 +301,16 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
 __device__ __forceinline__ void offer_once(Top2 &best, float s, int j, int self)
 {
     if (s <= best.s2 && j >= 0 && j != self && j != best.j1 && j != best.j2) best.offer(s, j);
+}
+// branch-free (s, j)-ordered insertion (converged code for loops whose lanes all insert)
+__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
+{
+    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
+    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
+    const float ns2 = lt1 ? b.s1 : s;
+    const int nj2 = lt1 ? b.j1 : j;
+    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
+    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
 }
 template <int D>
 __device__ __noinline__ Top2 slow_offer4(const View &v, Top2 best, int t, float s0, float s1,
@@ -680,14 +697,23 @@ __device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float
     tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
 }
 
-template <int D>
+// SWEEP = false: A3, every slot of a freshly built grid is a query.
+// SWEEP = true:  A7 for a large frontier: the same slot-ordered sweep over the incrementally
+//   updated grid, but only the slots marked with this call's epoch are queries (their lanes stay
+//   idle otherwise; warps without a marked slot leave at once), tombstones are inert records and
+//   the overflow chains of every visited cell are scanned too.  Runs only when *nF * sweep_div >= N
+//   (the list kernel serves smaller frontiers and the frontier points that live in chains).
+template <int D, bool SWEEP>
 __global__ void __launch_bounds__(32 * WT_WARPS)
-search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2,
-                        float *c)
+search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
+                    const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
+                    float *d2, float *c)
 {
     __shared__ __align__(16) float4 s_p4[D == 3 ? WT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
     __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
     __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    if (SWEEP && (int64_t)*nF * sweep_div < N) return;
+    const bool chains = SWEEP && ctr->n_misfiled > 0;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float qnan = __int_as_float(0x7fc00000);
     float4 *tp4 = s_p4[D == 3 ? warp : 0];
@@ -717,7 +743,9 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
     const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
     Top2 best;
     best.init();
-    unsigned todo = 0xffffffffu;
+    // queries of this warp (marked slots are never tombstones, so their cells are in slot order)
+    const bool query = SWEEP ? (s < N && mark[sc] == epoch) : true;
+    unsigned todo = __ballot_sync(0xffffffffu, query);
     while (todo) {
         const int leader = __ffs(todo) - 1;
         const int R = __shfl_sync(0xffffffffu, rowid, leader);
@@ -733,6 +761,9 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
             const int y = ry + oy, z = rz + oz;
             if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
             const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
+            if (chains && mine)
+                for (int x = has_l ? cx - 1 : cx; x <= (has_r ? cx + 1 : cx); ++x)
+                    scan_chain<D>(v, (z * v.G1 + y) * v.G0 + x, qx, qy, qz, self, best);
             const int B = crow[ux0], E = crow[ux1 + 1];
             if (B == E) continue;
             if (E - B < v.dense_thr) {
@@ -766,32 +797,165 @@ search_all_tiled_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2,
         }
         todo &= ~seg;
     }
-    const int r = finish_block<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
+    if (!query) return;
+    const int r = finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
     if (s >= N) return;
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
     store_cert(best, self, nn, nn2, d1, d2, c);
 }
 
-template <int D>
-__global__ void __launch_bounds__(128)
-search_frontier_kernel(View v, const float *__restrict__ p_new, const int32_t *__restrict__ F,
-                       const int32_t *__restrict__ nF, Counters *ctr, int32_t *nn, int32_t *nn2,
-                       float *d1, float *d2, float *c)
+// A7, large frontier: stamp the slots of the frontier points with this call's epoch; frontier
+// points that live in an overflow chain have no slot and go to the list kernel (list2).
+__global__ void __launch_bounds__(256)
+mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF, int N, int sweep_div,
+                     const int32_t *__restrict__ slot, int32_t *mark, int epoch, int32_t *list2,
+                     Counters *ctr)
 {
     const int n = *nF;
-    const bool chains = ctr->n_misfiled > 0;
+    if ((int64_t)n * sweep_div < N) return;
     for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
-        int i = F[f];
-        float qx = p_new[(int64_t)i * D], qy = p_new[(int64_t)i * D + 1];
-        float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
+        const int i = F[f];
+        const int sl = slot[i];
+        if (sl >= 0) mark[sl] = epoch;
+        else list2[atomicAdd(&ctr->n_list2, 1)] = i;
+    }
+}
+
+// ---- warp per query ---------------------------------------------------------------------------
+// One warp serves one query, one lane per cell of the 3^d block: every lane fetches its cell's
+// record range and chain head at once (one memory round trip for the whole block instead of one
+// per row), the own cell is scanned first by the whole warp, then every lane prunes its cell
+// against the second-best found so far; short surviving ranges are scanned by their lanes, long
+// ones (dense cells) by the whole warp, and two warp reductions extract the two smallest keys.
+// No lane ever waits for another query's insertions, and the order of the queries is irrelevant,
+// which is what a frontier list in id order needs (A7).  SLOTS = true runs the same search for
+// every sorted slot of a fresh grid (A3 variant, for comparison with the tiled sweep).
+template <int D>
+__device__ __forceinline__ void lane_offer(Top2 &tmp, float s, int j, float thr, int self)
+{
+    insert_bf(tmp, s, j, s <= thr && j >= 0 && j != self);
+}
+template <int D>
+__device__ int wpq_search(const View &v, bool chains, int lane, float qx, float qy, float qz, int self,
+                          Top2 &best)
+{
+    constexpr int NC = D == 3 ? 27 : 9, OWN = NC / 2;
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    const int ox = lane % 3 - 1, oy = (lane / 3) % 3 - 1, oz = D == 3 ? lane / 9 - 1 : 0;
+    const int x = cx + ox, y = cy + oy, z = cz + oz;
+    const bool valid = lane < NC && x >= 0 && x < v.G0 && y >= 0 && y < v.G1 && z >= 0 && z < v.G2;
+    const int cid = valid ? (z * v.G1 + y) * v.G0 + x : 0;
+    int b = 0, e = 0, hd = -1;
+    if (valid) {
+        b = v.cell_start[cid]; e = v.cell_start[cid + 1];
+        if (chains) hd = v.head[cid];
+    }
+    // own cell: the whole warp
+    Top2 tmp;
+    tmp.init();
+    const int ob = __shfl_sync(0xffffffffu, b, OWN), oe = __shfl_sync(0xffffffffu, e, OWN);
+    coop_range<D>(v, lane, ob, oe, qx, qy, qz, self, CUDART_INF_F, KC_NOIDX, KC_NOIDX, tmp);
+    if (lane == OWN)
+        for (int c = hd; c >= 0; c = v.next[c]) {
+            const float4 o = v.opos[c];
+            lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, o.x, o.y) : sqd3(qx, qy, qz, o.x, o.y, o.z), c, CUDART_INF_F, self);
+        }
+    float sa, sb;
+    int ja, jb;
+    coop_pop(tmp, sa, ja);
+    coop_pop(tmp, sb, jb);
+    best.s1 = sa; best.j1 = ja; best.s2 = sb; best.j2 = jb;         // ordered: sa <= sb (or none)
+    const float thr = best.s2;
+    // the other cells: prune, then short ranges by their lanes, long ones by the warp
+    const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
+    const float lb2 = __fadd_rn(__fadd_rn(ox < 0 ? g.xm : (ox > 0 ? g.xp : 0.f), oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f)),
+                                oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
+    const bool need = valid && lane != OWN && !(thr < lb2);
+    const int len = need ? e - b : 0;
+    tmp.init();
+    for (unsigned m = __ballot_sync(0xffffffffu, len > 16); m; m &= m - 1) {
+        const int L = __ffs(m) - 1;
+        coop_range<D>(v, lane, __shfl_sync(0xffffffffu, b, L), __shfl_sync(0xffffffffu, e, L), qx, qy, qz, self,
+                      thr, KC_NOIDX, KC_NOIDX, tmp);
+    }
+    if (len <= 16)
+        for (int t = b; t < b + len; ++t) {
+            if (D == 2) {
+                const float2 c = v.spos2[t];
+                const float s = sqd2(qx, qy, c.x, c.y);
+                lane_offer<D>(tmp, s, s <= thr ? v.sidx[t] : -1, thr, self);
+            } else {
+                const float4 c = v.spos4[t];
+                lane_offer<D>(tmp, sqd3(qx, qy, qz, c.x, c.y, c.z), __float_as_int(c.w), thr, self);
+            }
+        }
+    if (need)
+        for (int c = hd; c >= 0; c = v.next[c]) {
+            const float4 o = v.opos[c];
+            lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, o.x, o.y) : sqd3(qx, qy, qz, o.x, o.y, o.z), c, thr, self);
+        }
+    coop_pop(tmp, sa, ja);
+    coop_pop(tmp, sb, jb);
+    if (ja != KC_NOIDX) best.offer(sa, ja);
+    if (jb != KC_NOIDX) best.offer(sb, jb);
+    // every lane holds the same state: the rare ring continuation runs redundantly on all of them
+    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+}
+
+template <int D, bool SLOTS>
+__global__ void __launch_bounds__(128)
+search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__restrict__ F,
+                  const int32_t *__restrict__ nF, const int32_t *__restrict__ list2, int sweep_div,
+                  Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
+{
+    const int lane = threadIdx.x & 31;
+    const int w0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
+    int n = N;
+    const int32_t *__restrict__ Q = nullptr;
+    bool chains = false;
+    if (!SLOTS) {
+        // a large frontier is served by the slot sweep; only its chain residents (list2) come here
+        const bool swept = sweep_div > 0 && (int64_t)*nF * sweep_div >= N;
+        n = swept ? ctr->n_list2 : *nF;
+        Q = swept ? list2 : F;
+        chains = ctr->n_misfiled > 0;
+    }
+    if (!SLOTS && n > v.wpq_max) {
+        // long list: one thread per query keeps more queries in flight
+        for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
+            const int i = Q[f];
+            const float qx = p_new[(int64_t)i * D], qy = p_new[(int64_t)i * D + 1];
+            const float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
+            Top2 best;
+            best.init();
+            const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+            const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+            const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+            const int r = block_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
+            if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+            store_cert(best, i, nn, nn2, d1, d2, c);
+        }
+        return;
+    }
+    for (int f = w0; f < n; f += nw) {
+        float qx, qy, qz = 0.f;
+        int i;
+        if (SLOTS) {
+            if (D == 2) { const float2 q = v.spos2[f]; qx = q.x; qy = q.y; i = v.sidx[f]; }
+            else { const float4 q = v.spos4[f]; qx = q.x; qy = q.y; qz = q.z; i = __float_as_int(q.w); }
+        } else {
+            i = Q[f];
+            qx = p_new[(int64_t)i * D]; qy = p_new[(int64_t)i * D + 1];
+            if (D == 3) qz = p_new[(int64_t)i * D + 2];
+        }
         Top2 best;
-        best.init();
-        const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-        const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-        const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-        int r = block_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
-        if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-        store_cert(best, i, nn, nn2, d1, d2, c);
+        const int r = wpq_search<D>(v, chains, lane, qx, qy, qz, i, best);
+        if (lane == 0) {
+            if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+            store_cert(best, i, nn, nn2, d1, d2, c);
+        }
     }
 }
 
@@ -838,9 +1002,10 @@ refresh_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__
     }
 }
 __global__ void link_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
-                                   int32_t *head, int32_t *next, const Counters *ctr)
+                                   int32_t *head, int32_t *next, Counters *ctr)
 {
     int n = ctr->n_misfiled;
+    if (blockIdx.x == 0 && threadIdx.x == 0) ctr->n_list2 = 0;
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
         int i = mlist[e];
         next[i] = atomicExch(&head[cell[i]], i);
@@ -983,6 +1148,8 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     alloc((void **)&g->mlist, n * 4); alloc((void **)&g->fcount, nc * 4);
     alloc((void **)&g->mhist, MHIST * 4);
     alloc((void **)&g->blocksums, (size_t)g->n_scan_blocks * 4 + 4);
+    alloc((void **)&g->mark, (n + 8) * 4);
+    alloc((void **)&g->list2, n * 4);
     g->spos2 = nullptr; g->spos4 = nullptr;
     if (geom->d == 2) alloc((void **)&g->spos2, (n + 8) * sizeof(float2));
     else alloc((void **)&g->spos4, (n + 8) * sizeof(float4));
@@ -997,6 +1164,7 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     bool e = cudaMemset(g->head, 0xff, nc * 4) != cudaSuccess ||
              cudaMemset(g->fcount, 0, nc * 4) != cudaSuccess ||
              cudaMemset(g->mhist, 0, MHIST * 4) != cudaSuccess ||
+             (g->epoch = 0, cudaMemset(g->mark, 0, (n + 8) * 4)) != cudaSuccess ||
              cudaMemset(g->ctr, 0, sizeof(Counters)) != cudaSuccess ||
              cudaDeviceSynchronize() != cudaSuccess;
     if (e) {
@@ -1012,7 +1180,7 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
     void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
-                    g->mlist, g->fcount, g->mhist, g->blocksums, g->spos2, g->spos4, g->opos, g->ctr};
+                    g->mlist, g->fcount, g->mhist, g->blocksums, g->mark, g->list2, g->spos2, g->spos4, g->opos, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete g;
@@ -1065,8 +1233,12 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 1;
     const int tb = 32 * WT_WARPS;
     if (variant == 1) {
-        if (g->geom.d == 2) search_all_tiled_kernel<2><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-        else search_all_tiled_kernel<3><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
+        if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+        else search_tiled_kernel<3, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+    } else if (variant == 2) {
+        const int blocks = blocks_for(n, 4, 148 * 16);
+        if (g->geom.d == 2) search_wpq_kernel<2, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
+        else search_wpq_kernel<3, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
     } else {
         if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
         else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
@@ -1139,13 +1311,31 @@ extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t 
     }
     link_chains_kernel<<<blocks_for(nm > 0 || g->dirty ? N : 1, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->next, g->ctr);
     g->dirty = 1;
-    // lines 4-7: re-search the frontier only
+    // lines 4-7: re-search the frontier only.  On a large grid a frontier of at least N / sweep_div
+    // points (decided on the device from *nF) is served in slot order by the tiled sweep, anything
+    // else straight from the id list (one warp per query while the list is short: latency; one
+    // thread per query when it is long: throughput); both kernels are launched when the host
+    // bound allows either.
     if (nF_max > 0) {
-        int blocks = blocks_for(nF_max, 128, 148 * 32);
+        static const int div_env = getenv("KC_SWEEP_DIV") ? atoi(getenv("KC_SWEEP_DIV")) : 8;
+        static const int min_env = getenv("KC_SWEEP_MIN_N") ? atoi(getenv("KC_SWEEP_MIN_N")) : 200000;
+        const int sweep_div = N >= min_env && nF_max * (int64_t)div_env >= N ? div_env : 0;
+        const int tb = 32 * WT_WARPS;
+        if (sweep_div > 0) {
+            ++g->epoch;
+            mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
+            if (g->geom.d == 2)
+                search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+            else
+                search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+            count_launches(2);
+        }
+        int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
+        if (nF_max > v.wpq_max) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
         if (g->geom.d == 2)
-            search_frontier_kernel<2><<<blocks, 128, 0, st>>>(v, p_new, F, nF, g->ctr, nn, nn2, d1, d2, c);
+            search_wpq_kernel<2, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
         else
-            search_frontier_kernel<3><<<blocks, 128, 0, st>>>(v, p_new, F, nF, g->ctr, nn, nn2, d1, d2, c);
+            search_wpq_kernel<3, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
     }
     KC_LAUNCH_CHECK("kc_frontier_repair");
     return KC_OK;
