@@ -33,7 +33,8 @@ struct Counters {
     int n_stragglers;
     int m_cells;
     int n_list2;              // frontier points of the current sweep that live in chains
-    int pad[2];
+    int ticket;               // blocks of entropy_collect_kernel that are done (the last one finishes)
+    int pad[1];
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -109,11 +110,17 @@ __global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
         head[cell[mlist[e]]] = -1;
 }
-__global__ void reset_counters_kernel(Counters *ctr, int full)
+// start of a build: drop the overflow chains of the previous residency and empty the histogram
+__global__ void __launch_bounds__(256)
+build_prep_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell, int32_t *head,
+                  const Counters *ctr, int32_t *counts, int n_cells)
 {
-    ctr->n_misfiled = 0;
-    if (full) { ctr->c_occ = 0; ctr->max_occ = 0; }
-    ctr->n_stragglers = 0;
+    const int n = ctr->n_misfiled;
+    const int t0 = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
+    for (int e = t0; e < n; e += nt) head[cell[mlist[e]]] = -1;
+    int4 *c4 = reinterpret_cast<int4 *>(counts);
+    for (int k = t0; k < n_cells / 4; k += nt) c4[k] = make_int4(0, 0, 0, 0);
+    for (int k = (n_cells & ~3) + t0; k < n_cells; k += nt) counts[k] = 0;
 }
 
 template <int D>
@@ -128,9 +135,12 @@ __device__ __forceinline__ int cell_of(const View &v, float x, float y, float z)
 template <int D>
 __global__ void __launch_bounds__(256)
 cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restrict__ cell,
-                   int32_t *counts)
+                   int32_t *counts, Counters *ctr)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {          // the chains were dropped by the previous kernel; the scan recounts C
+        ctr->n_misfiled = 0; ctr->c_occ = 0; ctr->max_occ = 0; ctr->n_stragglers = 0;
+    }
     if (i >= N) return;
     float x, y, z = 0.f;
     if (D == 2) {
@@ -241,6 +251,56 @@ scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, const int32_t
         run += v[k];
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[0] = 0;
+}
+
+// Small grids: the whole scan in one CTA (thread t owns PER consecutive cells).
+constexpr int SCAN_SMALL_MAX = 16384;
+__global__ void __launch_bounds__(1024)
+scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *__restrict__ cell_start,
+                  Counters *ctr)
+{
+    const int per = (n_cells + 1023) / 1024;
+    const int base = threadIdx.x * per;
+    int tsum = 0, occ = 0, mx = 0;
+    for (int k = 0; k < per; ++k) {
+        const int cnt = base + k < n_cells ? counts[base + k] : 0;
+        tsum += cnt; occ += cnt > 0; mx = max(mx, cnt);
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int incl = tsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    occ = __reduce_add_sync(0xffffffffu, occ);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    __shared__ int wsum[32], wocc[32], wmx[32];
+    if (lane == 31) wsum[w] = incl;
+    if (lane == 0) { wocc[w] = occ; wmx[w] = mx; }
+    __syncthreads();
+    if (w == 0) {
+        int x = wsum[lane], xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, xi, o);
+            if (lane >= o) xi += t;
+        }
+        wsum[lane] = xi - x;
+        const int a = __reduce_add_sync(0xffffffffu, wocc[lane]);
+        const int b = __reduce_max_sync(0xffffffffu, wmx[lane]);
+        if (lane == 0) { ctr->c_occ = a; ctr->max_occ = b; }
+    }
+    __syncthreads();
+    int run = wsum[w] + incl - tsum;
+    for (int k = 0; k < per; ++k) {
+        // stored one slot to the right, as in scan_write_kernel (the scatter's cursors)
+        if (base + k < n_cells) {
+            cell_start[base + k + 1] = run;
+            run += counts[base + k];
+        }
+    }
+    if (threadIdx.x == 0) cell_start[0] = 0;
 }
 
 template <int D>
@@ -1027,7 +1087,8 @@ entropy_count_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ 
 }
 __global__ void __launch_bounds__(256)
 entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF,
-                       const int32_t *__restrict__ cell, int32_t *fcount, int32_t *mhist, Counters *ctr)
+                       const int32_t *__restrict__ cell, int32_t *fcount, int32_t *mhist, Counters *ctr,
+                       double *H, int32_t *m_cells, int32_t *C_occ)
 {
     // almost every cell holds a handful of frontier points, so the low bins of M[k] would take one
     // global atomic per cell on a few addresses: they are aggregated per block in shared memory
@@ -1062,15 +1123,19 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
     }
     __syncthreads();
     if (threadIdx.x < LOW && low[threadIdx.x]) atomicAdd(&mhist[threadIdx.x], low[threadIdx.x]);
-}
-__global__ void __launch_bounds__(1024)
-entropy_finish_kernel(const int32_t *__restrict__ nF, int32_t *mhist, Counters *ctr, double *H,
-                      int32_t *m_cells, int32_t *C_occ)
-{
-    __shared__ double part[32];
+    // the block that takes the last ticket evaluates H from the finished histogram-of-counts
+    // (fixed order, double: independent of atomic ordering) and leaves the scratch zeroed
+    __shared__ int s_last;
+    __shared__ double part[8];
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&ctr->ticket, 1) == (int)gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
     double acc = 0.0;
-    for (int k = threadIdx.x; k < MHIST; k += 1024) {
-        int M = mhist[k];
+    for (int k = threadIdx.x; k < MHIST; k += 256) {
+        int M = __ldcg(&mhist[k]);
         if (M) {
             if (k > 1) acc += (double)M * ((double)k * log((double)k));
             mhist[k] = 0;
@@ -1081,16 +1146,17 @@ entropy_finish_kernel(const int32_t *__restrict__ nF, int32_t *mhist, Counters *
     if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = acc;
     __syncthreads();
     if (threadIdx.x == 0) {
-        double S = ctr->big;
-        for (int w = 0; w < 32; ++w) S += part[w];
-        int n = *nF, C = ctr->c_occ;
+        double S = __ldcg(&ctr->big);
+        for (int w = 0; w < 8; ++w) S += part[w];
+        const int C = ctr->c_occ;
         double h = 0.0;
         if (n > 0 && C > 1) h = (log((double)n) - S / (double)n) / log((double)C);
         *H = h;
-        if (m_cells) *m_cells = ctr->m_cells;
+        if (m_cells) *m_cells = __ldcg(&ctr->m_cells);
         if (C_occ) *C_occ = C;
         ctr->m_cells = 0;
         ctr->big = 0.0;
+        ctr->ticket = 0;
     }
 }
 
@@ -1198,20 +1264,24 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)N, nc = (int)g->n_cells;
-    // drop the overflow chains of the previous residency, then start from an empty histogram
-    clear_chains_kernel<<<blocks_for(g->N, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
-    reset_counters_kernel<<<1, 1, 0, st>>>(g->ctr, 1);
-    KC_CUDA(cudaMemsetAsync(g->counts, 0, (size_t)nc * 4, st));
-    if (g->geom.d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts);
-    else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts);
-    scan_reduce_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->ctr);
-    scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, g->n_scan_blocks);
-    scan_write_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->cell_start, n);
+    // drop the overflow chains of the previous residency and empty the histogram, then cell ids +
+    // histogram, scan (one CTA for a small grid), scatter
+    build_prep_kernel<<<blocks_for(nc / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr, g->counts, nc);
+    if (g->geom.d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
+    else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
+    if (nc <= SCAN_SMALL_MAX) {
+        scan_small_kernel<<<1, 1024, 0, st>>>(g->counts, nc, g->cell_start, g->ctr);
+        count_launches(4);
+    } else {
+        scan_reduce_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->ctr);
+        scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, g->n_scan_blocks);
+        scan_write_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->cell_start, n);
+        count_launches(6);
+    }
     if (g->geom.d == 2)
         scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
     else
         scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
-    count_launches(7);   // + one memset node
     KC_LAUNCH_CHECK("kc_grid_build");
     g->N = N; g->built = 1; g->dirty = 0;
     return KC_OK;
@@ -1270,9 +1340,8 @@ extern "C" kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int
     cudaStream_t st = (cudaStream_t)stream;
     int blocks = blocks_for(nF_max, 256, 148 * 8);
     entropy_count_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount);
-    entropy_collect_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount, g->mhist, g->ctr);
-    entropy_finish_kernel<<<1, 1024, 0, st>>>(nF, g->mhist, g->ctr, H, m_cells, C_occ);
-    count_launches(3);
+    entropy_collect_kernel<<<blocks, 256, 0, st>>>(F, nF, g->cell, g->fcount, g->mhist, g->ctr, H, m_cells, C_occ);
+    count_launches(2);
     KC_LAUNCH_CHECK("kc_frontier_entropy");
     return KC_OK;
 }

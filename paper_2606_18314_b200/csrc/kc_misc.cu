@@ -178,6 +178,37 @@ __global__ void __launch_bounds__(256) maxdisp_kernel(const float *__restrict__ 
 }
 __global__ void sqrt_inplace_kernel(float *x) { *x = __fsqrt_rn(*x); }
 
+// Small N: one CTA does the whole reduction and the square root (one launch instead of three;
+// below a few 10^4 points the call is launch-latency, not bandwidth).
+constexpr int64_t SMALL_N = 32768;
+template <int D>
+__global__ void __launch_bounds__(1024) maxdisp_small_kernel(const float *__restrict__ p,
+                                                             const float *__restrict__ p2, int N,
+                                                             float *eps_out)
+{
+    float m = 0.0f;
+    for (int i = threadIdx.x; i < N; i += 1024) {
+        float s;
+        if (D == 2) {
+            float2 a = reinterpret_cast<const float2 *>(p)[i];
+            float2 b = reinterpret_cast<const float2 *>(p2)[i];
+            s = sqd2(b.x, b.y, a.x, a.y);
+        } else {
+            const float *a = p + (int64_t)i * 3, *b = p2 + (int64_t)i * 3;
+            s = sqd3(b[0], b[1], b[2], a[0], a[1], a[2]);
+        }
+        m = fmaxf(m, s);
+    }
+    unsigned k = __reduce_max_sync(0xffffffffu, __float_as_uint(m));
+    __shared__ unsigned sm[32];
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = k;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        k = __reduce_max_sync(0xffffffffu, sm[threadIdx.x]);
+        if (threadIdx.x == 0) *eps_out = __fsqrt_rn(__uint_as_float(k));
+    }
+}
+
 extern "C" kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d,
                                          float *eps_out, void *stream)
 {
@@ -187,6 +218,13 @@ extern "C" kc_status kc_max_displacement(const float *p, const float *p2, int64_
         return KC_EINVAL;
     }
     cudaStream_t st = (cudaStream_t)stream;
+    if (N <= SMALL_N) {
+        if (d == 2) maxdisp_small_kernel<2><<<1, 1024, 0, st>>>(p, p2, (int)N, eps_out);
+        else maxdisp_small_kernel<3><<<1, 1024, 0, st>>>(p, p2, (int)N, eps_out);
+        count_launches(1);
+        KC_LAUNCH_CHECK("kc_max_displacement");
+        return KC_OK;
+    }
     unsigned *out = reinterpret_cast<unsigned *>(eps_out);
     zero_u32_kernel<<<1, 1, 0, st>>>(out);
     int blocks = (int)((N + 255) / 256 < 148 * 8 ? (N + 255) / 256 : 148 * 8);
