@@ -109,6 +109,21 @@ def run_oracle_arm(cfg, K, W, time_budget_s=None, pair_budget=1.5e11):
 
 
 # ------------------------------------------------------------------------------------------
+def aggregate_over_ranks(local_ms, local_units, device):
+    """Replicas only (multi-GPU): the job's time is the MAX of the ranks' device times,
+    its work the SUM of their units.  Works on any initialised process group (nccl on the GPU
+    box, gloo in the CPU tests); without one it is the identity."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(local_ms), int(local_units)
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.int64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(u.item())
+
+
 class ClockSampler:
     """SM clock / throttle reasons sampled through NVML from a thread DURING the timed region
     (the region is tens of milliseconds: an nvidia-smi subprocess would not even start in time)."""
@@ -241,11 +256,8 @@ def run_gpu_arm(args):
         s = fam_stats[f]
         s["steps"] += 1; s["repair_ms"] += pt["repair"] + pt["classify"] + pt["maxdisp"]
         s["rebuild_ms"] += pt["rebuild"]; s["frontier"] += int(nF.item()); s["H"] += float(H.item())
-    tmax = torch.tensor([dev_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    dev_ms_max = float(tmax.item())
-    value = N * K * world / (dev_ms_max * 1e-3)
+    dev_ms_max, units = aggregate_over_ranks(dev_ms, N * K, dev)
+    value = units / (dev_ms_max * 1e-3)
 
     # ---- end to end through the public API: pinned host inputs, H2D + step + D2H per step ----
     host_next = {f: [torch.from_numpy(p).pin_memory() for p in traj[f][0]] for f in fams}
@@ -285,10 +297,8 @@ def run_gpu_arm(args):
             e2e_events.append((e0, e1))
     barrier()
     e2e_ms = sum(a.elapsed_time(b) for a, b in e2e_events)
-    tmax = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    e2e_value = N * K * world / (float(tmax.item()) * 1e-3)
+    e2e_ms_max, units = aggregate_over_ranks(e2e_ms, N * K, dev)
+    e2e_value = units / (e2e_ms_max * 1e-3)
 
     out = None
     if rank == 0:
@@ -330,7 +340,9 @@ def run_gpu_arm(args):
             "ms_per_step": dev_ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{cfg}: N={N}, d={d}, eps={c['eps']}, families {','.join(fams)} "
-                                   f"({'/'.join(map(str, per))} steps), grid occupancy 2, every step = A0,A4,A6+A7,A5,A2+A3,A1",
+                                   f"({'/'.join(map(str, per))} steps), grid occupancy 2, every step = A0,A4,A6+A7,A5,A2+A3,A1 "
+                                   f"(A1 = the full N(N-1)-pair pass, started from the kinetic bound d2+2eps of the "
+                                   f"maintained certificates, kc_cert_allpairs_bounded)",
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
                        "certified": certified},

@@ -126,6 +126,36 @@ def test_allpairs_bounded_is_exact_for_any_bound(cfg, N):
         assert_same(got, want, what=f"bounded allpairs {cfg} bound={name}")
 
 
+@pytest.mark.parametrize("d", [2, 3])
+@pytest.mark.parametrize("offset", [0.0, 1000.0, -4096.5, 3.0e5])
+def test_grid_far_from_origin_and_on_cell_faces(d, offset):
+    """Pruning / ring bounds under coarse coordinates: boxes far from the origin (fp32 spacing up
+    to h/30), points exactly on computed cell faces, dense and sparse cells mixed; rebuild and
+    repair (both search kernels) against brute force."""
+    rng = np.random.default_rng(int(abs(offset)) + d)
+    N = 24000
+    base = wl.mixture_points(N, d, 60 + d, 12, 0.004).astype(np.float64)
+    p = (base + offset).astype(np.float32)
+    g_or, g_kc = geoms(p)
+    # a tenth of the points snapped onto cell faces of the grid actually used
+    k = rng.choice(N, N // 10, replace=False)
+    lo = np.array(list(g_or.lo)[:d], np.float32)
+    p[k] = (lo + np.round((p[k] - lo) / g_or.h).astype(np.float32) * g_or.h).astype(np.float32)
+    g_or, g_kc = geoms(p)
+    want = oracle.bruteforce_top2(p)
+    grid = kc.Grid(N, g_kc)
+    certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+    assert_same(certs, want, what=f"offset {offset} d{d} rebuild")
+    step = np.float32(g_or.h * 0.3)
+    q = (p + (rng.random((N, d)).astype(np.float32) - np.float32(0.5)) * step).astype(np.float32)
+    post = oracle.bruteforce_top2(q)
+    for F in (np.arange(N, dtype=np.int32), np.sort(rng.choice(N, 900, replace=False)).astype(np.int32)):
+        kc.kc_grid_build(grid, dev(p))
+        work = kc.Certs.empty(N)
+        kc.kc_frontier_repair(grid, dev(q), dev(F), dev(np.array([F.size], np.int32)), work)
+        assert_same(work, post, idx=F, what=f"offset {offset} d{d} repair |F|={F.size}")
+
+
 def test_grid_with_points_outside_the_box():
     # geometry fitted to the central half of the points: the rest is clamped into boundary cells
     p = wl.uniform_points(20000, 3, 31)
