@@ -308,7 +308,7 @@ def run_gpu_arm(args):
         except OSError:
             pass
         # ---- parity of the timed outputs against the CPU oracle (outside the timed region) ----
-        certified = verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams)
+        certified, audit = verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams)
         # ---- roofline of the dominant kernel (all-pairs; FP32 ALU bound) ----
         ops_per_pair = 5 if d == 2 else 8
         ap_ms = phase_sum["allpairs"] / K
@@ -333,7 +333,11 @@ def run_gpu_arm(args):
                             H=s["H"] / max(1, s["steps"]),
                             repair_path_ms=s["repair_ms"] / max(1, s["steps"]),
                             rebuild_path_ms=s["rebuild_ms"] / max(1, s["steps"]),
-                            repair_over_rebuild=s["repair_ms"] / max(s["rebuild_ms"], 1e-12))
+                            repair_over_rebuild=s["repair_ms"] / max(s["rebuild_ms"], 1e-12),
+                            # Definition 2 / Table 1 on the certified transitions: P_t = |F_t|/N,
+                            # fraction re-validated although still valid, Lemma-1 misses (must be 0)
+                            pressure_true=audit[f]["pressure"], false_frac=audit[f]["false_frac"],
+                            missed_safe=audit[f]["missed"])
                     for f, s in fam_stats.items()}
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -372,6 +376,7 @@ def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per
     import oracle
     N = wl.CONFIGS[cfg]["N"]
     checked = 0
+    audit = {}
     for f in fams:
         ps, mvs = traj[f]
         m = Maintainer(torch.from_numpy(ps[0]).to(dev))
@@ -380,7 +385,7 @@ def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per
         for t in range(steps_per_family):
             q = ps[t + 1]
             mv = None if mvs[t + 1] is None else torch.from_numpy(mvs[t + 1]).to(dev)
-            res = m.step(torch.from_numpy(q).to(dev), movers=mv)
+            res = m.step(torch.from_numpy(q).to(dev), movers=mv, audit=True)
             torch.cuda.synchronize()
             post = oracle.bruteforce_top2(q)
             eps = oracle.max_displacement(ps[t], q)
@@ -394,11 +399,20 @@ def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per
                 ok &= bool(np.array_equal(getattr(res.repaired, name).cpu().numpy().view(np.uint32)[F], want.view(np.uint32)[F]))
             H, mm, C = oracle.entropy(oracle.cell_ids(q, g), F, g.n_cells)
             ok &= abs(float(res.H.item()) - H) <= 1e-6 and int(res.m_cells.item()) == mm and int(res.C_occ.item()) == C
+            wFt, wcounts = oracle.failure_audit(pre.nn, post.nn, flags)
+            got_counts = res.audit.cpu().numpy()
+            ok &= got_counts.tolist() == wcounts.tolist() and int(wcounts[2]) == 0
+            a = audit.setdefault(f, dict(pressure=0.0, false_frac=0.0, missed=0, n=0))
+            a["pressure"] += float(wcounts[0]) / N; a["false_frac"] += float(wcounts[3]) / N
+            a["missed"] += int(got_counts[2]); a["n"] += 1
             if not ok:
                 raise RuntimeError(f"parity failure against the CPU oracle: {cfg}/{f} step {t}")
             pre = post
             checked += 1
-    return f"{checked} transitions ({steps_per_family} per family) bit-exact vs CPU oracle, H within 1e-6"
+    for a in audit.values():
+        a["pressure"] /= a["n"]; a["false_frac"] /= a["n"]
+    return (f"{checked} transitions ({steps_per_family} per family) bit-exact vs CPU oracle, H within 1e-6",
+            audit)
 
 
 def _median_ms(torch, fn, reps, setup=None, flush=None):

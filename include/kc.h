@@ -161,6 +161,17 @@ kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *n
 kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps, uint8_t *flags,
                                int32_t *F, int32_t *nF, void *stream);
 
+/* ---- NEXT #2: certificate-failure audit (Definition 2; Table 1) -- */
+/* The true repair frontier F_t = { i : nn_post[i] != nn_pre[i] } of a step and the audit of the
+ * Lemma-1 rule against it.  nn_pre / nn_post: device int32[N], exact certificates before / after
+ * the step; flags: device uint8[N] from kc_frontier_classify (1 = c_i <= 4 eps_t).
+ * counts: device int32[4] = { |F_t|, detected = failed and flagged, missed = failed but called safe
+ * (Lemma 1 guarantees 0), false = flagged but still valid } (the dataset's n_detect_safe /
+ * n_missed_safe / n_false_safe).  Ft: device int32[N] or NULL; receives the ids of
+ * F_t in arbitrary order (counts[0] entries), ready for kc_frontier_entropy (H(F_t), P_t = |F_t|/N). */
+kc_status kc_failure_audit(const int32_t *nn_pre, const int32_t *nn_post, const uint8_t *flags,
+                           int64_t N, int32_t *Ft, int32_t *counts, void *stream);
+
 /* ---- A5: Definition 2, H(F) over the grid's cells ------------------------ */
 /* F: device int32 list of DISTINCT point ids, *nF entries (device int32[1]), at most nF_max
  * (host upper bound used only to size launches; pass N if unknown).  Cells are the grid's

@@ -241,3 +241,18 @@ def entropy(cell_all, F, n_cells):
     if rc != 0:
         raise ValueError(f"orc_entropy rc={rc}")
     return float(H.value), int(m.value), int(Cc.value)
+
+
+def failure_audit(nn_pre, nn_post, flags):
+    """Definition 2 and the audit columns of Table 1 / the dataset (PAPER.md:75-88,
+    :131), written out: F_t = {i : nn changed}; returns (F_t ascending, counts) with counts =
+    [|F_t|, detected = failed and flagged, missed = failed but called safe, false = flagged but
+    still valid]."""
+    nn_pre = np.asarray(nn_pre, np.int32)
+    nn_post = np.asarray(nn_post, np.int32)
+    flagged = np.asarray(flags) != 0
+    failed = nn_pre != nn_post
+    Ft = np.flatnonzero(failed).astype(np.int32)
+    counts = np.array([failed.sum(), (failed & flagged).sum(), (failed & ~flagged).sum(),
+                       (~failed & flagged).sum()], np.int32)
+    return Ft, counts

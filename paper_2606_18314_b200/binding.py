@@ -25,7 +25,7 @@ EXPORTS = (
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
+    "kc_frontier_repair", "kc_failure_audit", "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
 
@@ -90,6 +90,7 @@ def lib():
     L.kc_frontier_classify.argtypes = [vp, i64, vp, vp, vp, vp, vp]
     L.kc_frontier_entropy.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
     L.kc_frontier_repair.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    L.kc_failure_audit.argtypes = [vp, vp, vp, i64, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
@@ -342,6 +343,19 @@ def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_mo
                                     _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
                                     *certs._ptrs(), _stream()), "kc_frontier_repair")
     return certs
+
+
+def kc_failure_audit(nn_pre, nn_post, flags, Ft=None, counts=None, want_list=True):
+    """NEXT #2, Definition 2 / Table 1: true frontier F_t = {nn changed} and
+    the audit of the Lemma-1 rule.  Returns (counts int32[4] = |F_t|, detected, missed, false; Ft)."""
+    N = nn_pre.numel()
+    counts = counts if counts is not None else torch.empty(4, dtype=torch.int32, device=nn_pre.device)
+    if Ft is None and want_list:
+        Ft = torch.empty(N, dtype=torch.int32, device=nn_pre.device)
+    _check(lib().kc_failure_audit(_ptr(nn_pre, torch.int32, "nn_pre"), _ptr(nn_post, torch.int32, "nn_post"),
+                                  _ptr(flags, torch.uint8, "flags"), N, _ptr(Ft, torch.int32, "Ft"),
+                                  _ptr(counts, torch.int32, "counts"), _stream()), "kc_failure_audit")
+    return counts, Ft
 
 
 def kc_launch_count() -> int:

@@ -307,6 +307,63 @@ extern "C" kc_status kc_frontier_classify(const float *c, int64_t N, const float
     return KC_OK;
 }
 
+// ------------------------------------------------------------------ NEXT #2: failure audit
+// Definition 2: the repair frontier F_t is the set of certificates whose nearest
+// neighbour actually changes across the step; Table 1 / the dataset columns
+// audit the Lemma-1 rule against it.  counts = { |F_t|, detected (failed and flagged),
+// missed (failed but called safe; Lemma 1 guarantees 0), false (flagged but still valid) }.
+__global__ void __launch_bounds__(256) audit_kernel(const int32_t *__restrict__ nn_pre,
+                                                    const int32_t *__restrict__ nn_post,
+                                                    const uint8_t *__restrict__ flags, int64_t N,
+                                                    int32_t *__restrict__ Ft, int32_t *counts)
+{
+    int det = 0, mis = 0, fal = 0;
+    const int lane = threadIdx.x & 31;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t rounds = (N + stride - 1) / stride;
+    for (int64_t r = 0; r < rounds; ++r) {
+        const int64_t i = r * stride + blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+        bool failed = false;
+        if (i < N) {
+            failed = nn_pre[i] != nn_post[i];
+            const bool flagged = flags[i] != 0;
+            det += failed && flagged; mis += failed && !flagged; fal += !failed && flagged;
+        }
+        // |F_t| doubles as the append cursor of the list: one atomic per warp
+        const unsigned m = __ballot_sync(0xffffffffu, failed);
+        if (m) {
+            int base = 0;
+            if (lane == __ffs(m) - 1) base = atomicAdd(&counts[0], __popc(m));
+            base = __shfl_sync(0xffffffffu, base, __ffs(m) - 1);
+            if (failed && Ft) Ft[base + __popc(m & ((1u << lane) - 1))] = (int32_t)i;
+        }
+    }
+    det = __reduce_add_sync(0xffffffffu, det);
+    mis = __reduce_add_sync(0xffffffffu, mis);
+    fal = __reduce_add_sync(0xffffffffu, fal);
+    if (lane == 0) {
+        if (det) atomicAdd(&counts[1], det);
+        if (mis) atomicAdd(&counts[2], mis);
+        if (fal) atomicAdd(&counts[3], fal);
+    }
+}
+
+extern "C" kc_status kc_failure_audit(const int32_t *nn_pre, const int32_t *nn_post, const uint8_t *flags,
+                                      int64_t N, int32_t *Ft, int32_t *counts, void *stream)
+{
+    if (!nn_pre || !nn_post || !flags || !counts || N < 1 || N > 0x7fffffff) {
+        set_error("kc_failure_audit: bad argument");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    KC_CUDA(cudaMemsetAsync(counts, 0, 16, st));
+    int blocks = (int)((N + 255) / 256 < 148 * 8 ? (N + 255) / 256 : 148 * 8);
+    audit_kernel<<<blocks, 256, 0, st>>>(nn_pre, nn_post, flags, N, Ft, counts);
+    count_launches(1);
+    KC_LAUNCH_CHECK("kc_failure_audit");
+    return KC_OK;
+}
+
 // ------------------------------------------------------------------ FP32 probe
 // 16 independent dependent-chains per thread of alternating non-fused FMUL / FADD: the empirical
 // separately-rounded FP32 lane-op rate the A1 roofline is quoted against.

@@ -39,6 +39,8 @@ class StepResult:
     rebuilt: kc.Certs          # exact certificates at p' from the grid rebuild
     certified: kc.Certs | None # exact certificates at p' from the all-pairs pass
     phase_ms: dict = field(default_factory=dict)
+    audit: torch.Tensor | None = None   # int32[4]: |F_t|, detected, missed, false (kc_failure_audit)
+    Ft: torch.Tensor | None = None      # ids of the true frontier F_t (audit[0] entries)
 
 
 class Maintainer:
@@ -69,7 +71,7 @@ class Maintainer:
 
     def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None,
              frontier: torch.Tensor | None = None, time_phases: bool = False,
-             do_allpairs: bool = True, bounded_allpairs: bool = True) -> StepResult:
+             do_allpairs: bool = True, bounded_allpairs: bool = True, audit: bool = False) -> StepResult:
         """One transition p -> p_next through every row of the hot path.
 
         ``movers``: optional int32 id list of the points that moved (None = all may have moved).
@@ -83,6 +85,7 @@ class Maintainer:
                 e.record()
                 ev[name] = e
 
+        nn_pre = self.certs.nn.clone() if audit else None    # the repair below overwrites nn at F
         mark("t0")
         kc.kc_max_displacement(self.p, p_next, self.eps)
         mark("maxdisp")
@@ -118,6 +121,10 @@ class Maintainer:
                          self.ap if do_allpairs else None)
         if time_phases:
             res.phase_ms = ev
+        if audit:
+            # Definition 2: the true frontier F_t and the Lemma-1 audit, from the exact
+            # certificates before and after the step (outside the timed phases)
+            res.audit, res.Ft = kc.kc_failure_audit(nn_pre, self.certs.nn, self.flags)
         return res
 
     @staticmethod

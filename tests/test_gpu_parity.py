@@ -311,6 +311,29 @@ def test_repair_mover_list_as_frontier_cfg4_style():
             run_repair_steps("cfg4", "fraction", 40000, 2, use_movers=True, frontier="movers", fraction=f, ball=ball)
 
 
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "cluster_drift"), ("cfg3", "ball5")])
+def test_failure_audit_and_true_frontier_entropy(cfg, fam):
+    """NEXT #2: F_t = {nn changed} (Definition 2), the Lemma-1 audit counts (Table 1) and H(F_t)."""
+    p, mot = wl.make_scene(cfg, fam)
+    q, _ = mot.step(p)
+    N = p.shape[0]
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    pre = kc.kc_cert_grid_rebuild(grid, dev(p))
+    eps = kc.kc_max_displacement(dev(p), dev(q))
+    flags, F, nF = kc.kc_frontier_classify(pre.c, eps)
+    post = kc.kc_cert_grid_rebuild(grid, dev(q))
+    counts, Ft = kc.kc_failure_audit(pre.nn, post.nn, flags)
+    o_pre, o_post = oracle.bruteforce_top2(p), oracle.bruteforce_top2(q)
+    o_flags, _ = oracle.frontier(o_pre.c, oracle.max_displacement(p, q))
+    wFt, wcounts = oracle.failure_audit(o_pre.nn, o_post.nn, o_flags)
+    assert counts.cpu().numpy().tolist() == wcounts.tolist() and wcounts[2] == 0
+    assert np.array_equal(np.sort(Ft.cpu().numpy()[: int(wcounts[0])]), wFt)
+    H, m, C = kc.kc_frontier_entropy(grid, Ft, counts[:1])
+    wH, wm, wC = oracle.entropy(oracle.cell_ids(q, g_or), wFt, g_or.n_cells)
+    assert abs(float(H.item()) - wH) <= 1e-6 and int(m.item()) == wm and int(C.item()) == wC
+
+
 def test_search_refused_on_dirty_grid():
     p, mot = wl.make_scene("cfg1")
     grid = kc.Grid(p.shape[0], geoms(p)[1])

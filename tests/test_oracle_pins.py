@@ -64,6 +64,11 @@ def test_theorem1_tightness(golden_dir):
         assert post.nn[0] == case["nn_post"]
         assert float(post.d1[0]) == case["d1_post"]
         assert float(post.d2[0]) == case["d2_post"]
+        # Definition 2 / Table 1 audit on the same scene: only i can fail (a and k keep nn = i and
+        # have clearance ~d1 >> 4 eps); eta = 3 fails and is detected, eta = 4 is flagged but holds
+        Ft, counts = oracle.failure_audit(pre.nn, post.nn, flags)
+        want = {3: ([0], [1, 1, 0, 0]), 4: ([], [0, 0, 0, 1]), 5: ([], [0, 0, 0, 0])}[eta]
+        assert Ft.tolist() == want[0] and counts.tolist() == want[1]
 
 
 # ------------------------------------------------------------------ O1 against exact rationals
@@ -312,4 +317,7 @@ def test_lemma1_no_missed_failure(cfg, fam):
         post = oracle.kdtree_top2(q)
         changed = np.flatnonzero(pre.nn != post.nn)
         assert np.all(flags[changed] == 1)                       # Table 1 "miss (safe)" = 0
+        Ft, counts = oracle.failure_audit(pre.nn, post.nn, flags)
+        assert np.array_equal(Ft, changed) and counts[2] == 0
+        assert counts[0] == counts[1] == changed.size and counts[1] + counts[3] == F.size
         p, pre = q, post
