@@ -102,6 +102,19 @@ View make_view(const kc_grid *g)
     return v;
 }
 
+// Append `id` to list[] for the lanes with `want` set: one atomic per warp on the shared cursor
+// (every lane of the warp must call it).
+__device__ __forceinline__ void warp_append(bool want, int id, int32_t *list, int *cursor)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, want);
+    if (!m) return;
+    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(cursor, __popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (want) list[base + __popc(m & ((1u << lane) - 1))] = id;
+}
+
 // ------------------------------------------------------------------ A2 build
 __global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
                                     int32_t *head, const Counters *ctr)
@@ -873,11 +886,18 @@ mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ 
 {
     const int n = *nF;
     if ((int64_t)n * sweep_div < N) return;
-    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
-        const int i = F[f];
-        const int sl = slot[i];
-        if (sl >= 0) mark[sl] = epoch;
-        else list2[atomicAdd(&ctr->n_list2, 1)] = i;
+    const int stride = gridDim.x * blockDim.x;
+    for (int f0 = blockIdx.x * blockDim.x; f0 < n; f0 += stride) {     // warp-uniform trip count
+        const int f = f0 + threadIdx.x;
+        int i = -1;
+        bool chain = false;
+        if (f < n) {
+            i = F[f];
+            const int sl = slot[i];
+            if (sl >= 0) mark[sl] = epoch;
+            else chain = true;
+        }
+        warp_append(chain, i, list2, &ctr->n_list2);
     }
 }
 
@@ -1033,32 +1053,41 @@ refresh_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__
                Counters *ctr)
 {
     const int n = movers ? *n_movers : N;
-    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) {
-        int i = movers ? movers[k] : k;
-        float x = p_new[(int64_t)i * D], y = p_new[(int64_t)i * D + 1];
-        float z = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
-        int cnew = cell_of<D>(v, x, y, z);
-        int cold = cell[i];
-        int sl = slot[i];
-        if (sl >= 0) {
-            if (cnew == cold) {
-                if (D == 2) spos2[sl] = make_float2(x, y);
-                else spos4[sl] = make_float4(x, y, z, __int_as_float(i));
-                continue;
+    const int stride = gridDim.x * blockDim.x;
+    for (int k0 = blockIdx.x * blockDim.x; k0 < n; k0 += stride) {     // warp-uniform trip count
+        const int k = k0 + threadIdx.x;
+        bool misfile = false;
+        int i = -1;
+        if (k < n) {
+            i = movers ? movers[k] : k;
+            float x = p_new[(int64_t)i * D], y = p_new[(int64_t)i * D + 1];
+            float z = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
+            int cnew = cell_of<D>(v, x, y, z);
+            int cold = cell[i];
+            int sl = slot[i];
+            bool in_chain = sl < 0;
+            if (sl >= 0) {
+                if (cnew == cold) {
+                    if (D == 2) spos2[sl] = make_float2(x, y);
+                    else spos4[sl] = make_float4(x, y, z, __int_as_float(i));
+                } else {
+                    const float qnan = __int_as_float(0x7fc00000);
+                    if (D == 2) spos2[sl] = make_float2(qnan, qnan);
+                    else spos4[sl] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+                    sidx[sl] = -1;
+                    slot[i] = -1;
+                    misfile = true;
+                    in_chain = true;
+                }
             }
-            const float qnan = __int_as_float(0x7fc00000);
-            if (D == 2) spos2[sl] = make_float2(qnan, qnan);
-            else spos4[sl] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-            sidx[sl] = -1;
-            slot[i] = -1;
-            mlist[atomicAdd(&ctr->n_misfiled, 1)] = i;
+            if (in_chain) opos[i] = make_float4(x, y, z, 0.f);
+            if (cnew != cold) {
+                cell[i] = cnew;
+                if (atomicSub(&counts[cold], 1) == 1) atomicSub(&ctr->c_occ, 1);
+                if (atomicAdd(&counts[cnew], 1) == 0) atomicAdd(&ctr->c_occ, 1);
+            }
         }
-        opos[i] = make_float4(x, y, z, 0.f);
-        if (cnew != cold) {
-            cell[i] = cnew;
-            if (atomicSub(&counts[cold], 1) == 1) atomicSub(&ctr->c_occ, 1);
-            if (atomicAdd(&counts[cnew], 1) == 0) atomicAdd(&ctr->c_occ, 1);
-        }
+        warp_append(misfile, i, mlist, &ctr->n_misfiled);
     }
 }
 __global__ void link_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
