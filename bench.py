@@ -28,6 +28,9 @@ METRIC = "certified_points_per_s"
 UNIT = "points/s"
 L2_FLUSH_BYTES = 256 << 20
 FP32_LANES = 148 * 128          # B200: 148 SMs x 128 FP32 lanes, one non-fused op / lane / clk
+# dram__bytes_read.sum + dram__bytes_write.sum of one allpairs_kernel launch, from the committed ncu
+# --set full capture of this command (profiles/r1c_allpairs_cfg2_full.txt); null for other workloads
+AP_TRAFFIC_BYTES = {("cfg2", 16000): 213504}
 
 
 def log(*a):
@@ -317,7 +320,7 @@ def run_gpu_arm(args):
         peak = FP32_LANES * sm_max * 1e6 / 1e12
         probe = kc.kc_fp32_probe() / 1e12
         roofline = dict(bound="alu", kernel="allpairs_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
-                        frac=achieved / peak, traffic=None,
+                        frac=achieved / peak, traffic=AP_TRAFFIC_BYTES.get((cfg, N)),
                         note=(f"{ops_per_pair} separately rounded FP32 ops per ordered pair (no FMA by contract); peak = "
                               f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md); measured non-fused "
                               f"FADD/FMUL chain rate {probe:.2f} Top/s; kernel share of step = "
