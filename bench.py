@@ -481,6 +481,42 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
         sweep["ball" if ball else "scattered"] = dict(
             rows=rows, crossover_f=crossover_fraction(fs, [r["repair_ms"] for r in rows], [r["rebuild_ms"] for r in rows]))
     ex["cfg4_sweep"] = sweep
+    # ---------------- NEXT #3: multi-step maintenance with the cumulative clock (Appendix A.2):
+    # 40 steps with no rebuild in between, against a rebuild every step
+    from paper_2606_18314_b200.driver import ClockMaintainer
+    clock = {}
+    for cfg, fam in (("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "walk"), ("cfg3", "ball5")):
+        p, mot = wl.make_scene(cfg, fam)
+        Ncl = p.shape[0]
+        ps, mv = [p], [None]
+        for _ in range(40):
+            q, movers = mot.step(ps[-1])
+            ps.append(q); mv.append(movers)
+        dps = [torch.from_numpy(x).to(dev) for x in ps]
+        dmv = [None if m_ is None else torch.from_numpy(m_).to(dev) for m_ in mv]
+        cm = ClockMaintainer(dps[0])
+        for t in range(1, 6):
+            cm.step(dps[t], movers=dmv[t])
+        fsum = torch.zeros(1, dtype=torch.int64, device=dev)
+        flush.zero_()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for t in range(6, 41):
+            _, nF = cm.step(dps[t], movers=dmv[t])
+            fsum += nF
+        e1.record(); e1.synchronize()
+        t_clock = e0.elapsed_time(e1) / 35
+        other = kc.Certs.empty(Ncl, dev)
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for t in range(6, 41):
+            kc.kc_cert_grid_rebuild(cm.grid, dps[t], other)
+        e1.record(); e1.synchronize()
+        clock[f"{cfg}/{fam}"] = dict(steps=35, clock_step_ms=t_clock, rebuild_step_ms=e0.elapsed_time(e1) / 35,
+                                     mean_revisited_frac=float(fsum.item()) / 35 / Ncl,
+                                     points_per_s=Ncl / (t_clock * 1e-3))
+        del cm
+    ex["clock_loop"] = clock
     # ---------------- config 5: 4,194,304 points, rebuild + Lemma-1 repair; all-pairs at 2^20
     for cfg in ("cfg5_d2", "cfg5_d3"):
         c5 = wl.CONFIGS[cfg]

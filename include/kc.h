@@ -161,6 +161,24 @@ kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *n
 kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps, uint8_t *flags,
                                int32_t *F, int32_t *nF, void *stream);
 
+/* ---- NEXT #3: multi-step maintenance with the cumulative clock (Appendix A.2) -- */
+/* S = sum over steps of eps_s.  A certificate last recomputed at clock value S_i stays valid while
+ * S - S_i < c_i / 4 (Theorem 1 applied to the cumulative displacement), so the points to revisit in
+ * a step are F = { i : c_i <= 4 (S - S_i) }: the flat GPU form of the paper's expiry min-heap.
+ *  c: device float[N], clearances as of each point's last recomputation; stamp: device float[N],
+ *  the clock value S_i of that recomputation (kc_clock_stamp);
+ *  S_in: device double[1], the clock before this step; eps: device float[1], this step's max
+ *  displacement; S_out: device double[1] (must differ from S_in), receives S_in + eps;
+ *  flags / F / nF: as kc_frontier_classify.
+ * The test is evaluated in double: (double)c_i <= 4.0 * (S_out - (double)stamp_i). */
+kc_status kc_frontier_classify_clock(const float *c, const float *stamp, int64_t N, const double *S_in,
+                                     const float *eps, double *S_out, uint8_t *flags, int32_t *F,
+                                     int32_t *nF, void *stream);
+/* stamp[i] = *S rounded toward -inf to float32 (the elapsed clock S - S_i is never under-estimated)
+ * for the ids in F (*nF on the device, at most nF_max), or for all N points when F is NULL. */
+kc_status kc_clock_stamp(const int32_t *F, const int32_t *nF, int64_t nF_max, int64_t N, const double *S,
+                         float *stamp, void *stream);
+
 /* ---- NEXT #2: certificate-failure audit (Definition 2; Table 1) -- */
 /* The true repair frontier F_t = { i : nn_post[i] != nn_pre[i] } of a step and the audit of the
  * Lemma-1 rule against it.  nn_pre / nn_post: device int32[N], exact certificates before / after

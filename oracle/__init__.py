@@ -256,3 +256,23 @@ def failure_audit(nn_pre, nn_post, flags):
     counts = np.array([failed.sum(), (failed & flagged).sum(), (failed & ~flagged).sum(),
                        (~failed & flagged).sum()], np.int32)
     return Ft, counts
+
+
+def clock_stamp(S) -> np.float32:
+    """Stamp of Appendix A.2's clock: S (float64) rounded toward -inf to float32, so the elapsed
+    clock S - S_i is never under-estimated."""
+    f = np.float32(S)
+    if np.float64(f) > np.float64(S):
+        f = np.nextafter(f, np.float32(-np.inf))
+    return np.float32(f)
+
+
+def clock_frontier(c, stamp, S_in, eps):
+    """Appendix A.2: S = S_in + eps_t; a certificate last recomputed at clock S_i
+    stays valid while S - S_i < c_i / 4, so F = {i : c_i <= 4 (S - S_i)} (inclusive, as Lemma 1 is
+    strict).  Evaluated in float64.  Returns (S, flags, F ascending)."""
+    S = np.float64(S_in) + np.float64(np.float32(eps))
+    c64 = np.asarray(c, np.float32).astype(np.float64)
+    st64 = np.asarray(stamp, np.float32).astype(np.float64)
+    flags = (c64 <= 4.0 * (S - st64)).astype(np.uint8)
+    return S, flags, np.flatnonzero(flags).astype(np.int32)

@@ -25,7 +25,8 @@ EXPORTS = (
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_failure_audit", "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
+    "kc_frontier_repair", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp",
+    "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
 
@@ -91,6 +92,8 @@ def lib():
     L.kc_frontier_entropy.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
     L.kc_frontier_repair.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, vp, vp, vp, vp]
     L.kc_failure_audit.argtypes = [vp, vp, vp, i64, vp, vp, vp]
+    L.kc_frontier_classify_clock.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp]
+    L.kc_clock_stamp.argtypes = [vp, vp, i64, i64, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
@@ -256,9 +259,9 @@ class Grid:
         self._h = h
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().kc_grid_destroy(self._h)
-            self._h = None
+        if getattr(self, "_h", None) and _lib is not None:      # _lib is gone at interpreter exit
+            _lib.kc_grid_destroy(self._h)
+        self._h = None
 
     __del__ = close
 
@@ -343,6 +346,30 @@ def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_mo
                                     _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
                                     *certs._ptrs(), _stream()), "kc_frontier_repair")
     return certs
+
+
+def kc_frontier_classify_clock(c, stamp, S_in, eps, S_out, flags=None, F=None, nF=None):
+    """NEXT #3, Appendix A.2: F = {i : c_i <= 4 (S - S_i)}, S = S_in + eps -> S_out."""
+    N = c.numel()
+    flags = flags if flags is not None else torch.empty(N, dtype=torch.uint8, device=c.device)
+    F = F if F is not None else torch.empty(N, dtype=torch.int32, device=c.device)
+    nF = nF if nF is not None else torch.empty(1, dtype=torch.int32, device=c.device)
+    _check(lib().kc_frontier_classify_clock(_ptr(c, torch.float32, "c"), _ptr(stamp, torch.float32, "stamp"), N,
+                                            _ptr(S_in, torch.float64, "S_in"), _ptr(eps, torch.float32, "eps"),
+                                            _ptr(S_out, torch.float64, "S_out"), _ptr(flags, torch.uint8, "flags"),
+                                            _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), _stream()),
+           "kc_frontier_classify_clock")
+    return flags, F, nF
+
+
+def kc_clock_stamp(stamp, S, F=None, nF=None, nF_max=None):
+    """stamp[i] = S rounded down for i in F (all points when F is None)."""
+    N = stamp.numel()
+    nF_max = 0 if F is None else int(F.numel() if nF_max is None else nF_max)
+    _check(lib().kc_clock_stamp(_ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max, N,
+                                _ptr(S, torch.float64, "S"), _ptr(stamp, torch.float32, "stamp"), _stream()),
+           "kc_clock_stamp")
+    return stamp
 
 
 def kc_failure_audit(nn_pre, nn_post, flags, Ft=None, counts=None, want_list=True):

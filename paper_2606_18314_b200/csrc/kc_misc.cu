@@ -307,6 +307,97 @@ extern "C" kc_status kc_frontier_classify(const float *c, int64_t N, const float
     return KC_OK;
 }
 
+// ------------------------------------------------------------------ NEXT #3: cumulative clock
+// Appendix A.2: S = sum of the per-step maxima eps_s; a certificate last recomputed at
+// clock value S_i stays valid while S - S_i < c_i / 4.  The GPU form of the expiry heap is a flat
+// test of every point, c_i <= 4 (S - S_i), i.e. A4 with a per-point threshold.  S is a double
+// (exact sum of the float32 eps values for any realistic run), stamps are S rounded DOWN to
+// float32 (the elapsed clock is never under-estimated), the test is evaluated in double.
+__global__ void __launch_bounds__(256) classify_clock_kernel(const float *__restrict__ c,
+                                                             const float *__restrict__ stamp, int64_t N,
+                                                             const double *__restrict__ S_in,
+                                                             const float *__restrict__ eps, double *S_out,
+                                                             uint8_t *__restrict__ flags,
+                                                             int32_t *__restrict__ F, int32_t *nF)
+{
+    const double S = *S_in + (double)*eps;
+    const int64_t base = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) * 4;
+    if (base == 0) *S_out = S;
+    unsigned bits = 0;
+    for (int k = 0; k < 4; ++k)
+        if (base + k < N) {
+            const unsigned f = (double)c[base + k] <= 4.0 * (S - (double)stamp[base + k]);
+            bits |= f << k;
+            if (flags) flags[base + k] = (uint8_t)f;
+        }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int cnt = __popc(bits);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __shared__ int wsum[8];
+    __shared__ int bbase;
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
+        bbase = tot ? atomicAdd(nF, tot) : 0;
+    }
+    __syncthreads();
+    int pos = bbase + wsum[warp] + incl - cnt;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (bits & (1u << k)) F[pos++] = (int32_t)(base + k);
+}
+// stamp[i] = S rounded down, for the ids in F (NULL: all N points)
+__global__ void __launch_bounds__(256) clock_stamp_kernel(const int32_t *__restrict__ F,
+                                                          const int32_t *__restrict__ nF, int64_t N,
+                                                          const double *__restrict__ S, float *stamp)
+{
+    const float v = __double2float_rd(*S);
+    const int64_t n = F ? (int64_t)*nF : N;
+    for (int64_t f = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; f < n; f += (int64_t)gridDim.x * blockDim.x)
+        stamp[F ? F[f] : f] = v;
+}
+
+extern "C" kc_status kc_frontier_classify_clock(const float *c, const float *stamp, int64_t N,
+                                                const double *S_in, const float *eps, double *S_out,
+                                                uint8_t *flags, int32_t *F, int32_t *nF, void *stream)
+{
+    if (!c || !stamp || !S_in || !eps || !S_out || S_in == S_out || !F || !nF || N < 1 || N > 0x7fffffff) {
+        set_error("kc_frontier_classify_clock: bad argument (S_in and S_out must differ)");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    zero_u32_kernel<<<1, 1, 0, st>>>(reinterpret_cast<unsigned *>(nF));
+    int64_t blocks = (N + 1023) / 1024;
+    classify_clock_kernel<<<(unsigned)blocks, 256, 0, st>>>(c, stamp, N, S_in, eps, S_out, flags, F, nF);
+    count_launches(2);
+    KC_LAUNCH_CHECK("kc_frontier_classify_clock");
+    return KC_OK;
+}
+
+extern "C" kc_status kc_clock_stamp(const int32_t *F, const int32_t *nF, int64_t nF_max, int64_t N,
+                                    const double *S, float *stamp, void *stream)
+{
+    if (!S || !stamp || N < 1 || (F && (!nF || nF_max < 0))) {
+        set_error("kc_clock_stamp: bad argument");
+        return KC_EINVAL;
+    }
+    const int64_t n = F ? nF_max : N;
+    if (n == 0) return KC_OK;
+    int blocks = (int)((n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8);
+    clock_stamp_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(F, nF, N, S, stamp);
+    count_launches(1);
+    KC_LAUNCH_CHECK("kc_clock_stamp");
+    return KC_OK;
+}
+
 // ------------------------------------------------------------------ NEXT #2: failure audit
 // Definition 2: the repair frontier F_t is the set of certificates whose nearest
 // neighbour actually changes across the step; Table 1 / the dataset columns

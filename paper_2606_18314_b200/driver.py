@@ -151,3 +151,59 @@ def crossover_fraction(fracs, t_repair, t_rebuild):
             w = (1.0 - r[k - 1]) / (r[k] - r[k - 1])
             return float(np.exp(a + w * (b - a)))
     return None
+
+
+class ClockMaintainer:
+    """NEXT #3: multi-step maintenance with the cumulative clock of Appendix A.2.
+
+    No rebuild between steps: the clock S accumulates the per-step maxima eps_s, a certificate last
+    recomputed at clock S_i is revisited when c_i <= 4 (S - S_i), and only those points are
+    re-searched against the incrementally updated grid.  Nearest neighbours stay exact for every
+    point (Theorem 1 on cumulative displacement); d1, d2, c are exact for the points revisited in
+    the current step and stale for the rest, by design."""
+
+    def __init__(self, p0: torch.Tensor, occ: float = 2.0, rebin_every: int = 4):
+        assert p0.is_cuda and p0.dtype == torch.float32 and p0.dim() == 2
+        self.N = int(p0.shape[0])
+        dev = p0.device
+        # every `rebin_every` steps the grid is re-binned at the new positions (A2 only: O(N), no
+        # certificate is recomputed) instead of updated incrementally, so the overflow chains of
+        # re-filed points never grow long; 0 = never
+        self.rebin_every = int(rebin_every)
+        self.k = 0
+        self.none = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.geom = kc.kc_geom_for(p0, occ)
+        self.grid = kc.Grid(self.N, self.geom)
+        self.certs = kc.Certs.empty(self.N, dev)
+        self.stamp = torch.zeros(self.N, dtype=torch.float32, device=dev)
+        self.S = [torch.zeros(1, dtype=torch.float64, device=dev), torch.zeros(1, dtype=torch.float64, device=dev)]
+        self.flags = torch.empty(self.N, dtype=torch.uint8, device=dev)
+        self.F = torch.empty(self.N, dtype=torch.int32, device=dev)
+        self.nF = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.eps = torch.zeros(1, dtype=torch.float32, device=dev)
+        self.rebuild(p0)
+
+    def rebuild(self, p: torch.Tensor):
+        """Fresh grid and exact certificates at p; every stamp is set to the current clock."""
+        kc.kc_cert_grid_rebuild(self.grid, p, self.certs)
+        kc.kc_clock_stamp(self.stamp, self.S[0])
+        self.p = p
+
+    def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None):
+        """p -> p_next: A0, clock classify, A6 + A7 on the expired certificates, re-stamp.  No host
+        sync.  Returns (F, nF) of this step (device tensors)."""
+        kc.kc_max_displacement(self.p, p_next, self.eps)
+        kc.kc_frontier_classify_clock(self.certs.c, self.stamp, self.S[0], self.eps, self.S[1],
+                                      self.flags, self.F, self.nF)
+        self.S.reverse()
+        self.k += 1
+        if self.rebin_every and self.k % self.rebin_every == 0:
+            kc.kc_grid_build(self.grid, p_next)
+            movers, n_movers = self.F, self.none          # nothing left to refresh
+        else:
+            n_movers = None
+        kc.kc_frontier_repair(self.grid, p_next, self.F, self.nF, self.certs, movers=movers,
+                              n_movers=n_movers, nF_max=self.N)
+        kc.kc_clock_stamp(self.stamp, self.S[0], self.F, self.nF, self.N)
+        self.p = p_next
+        return self.F, self.nF

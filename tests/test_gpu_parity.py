@@ -334,6 +334,33 @@ def test_failure_audit_and_true_frontier_entropy(cfg, fam):
     assert abs(float(H.item()) - wH) <= 1e-6 and int(m.item()) == wm and int(C.item()) == wC
 
 
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "cluster_drift"), ("cfg3", "vortex")])
+def test_clock_maintenance_multi_step(cfg, fam):
+    """NEXT #3 (Appendix A.2): 15 steps without a rebuild; every step the expired set equals the
+    oracle's clock rule, repaired certificates are exact, and nn is exact for ALL points."""
+    from paper_2606_18314_b200.driver import ClockMaintainer
+    p, mot = wl.make_scene(cfg, fam, N=6000)
+    N = p.shape[0]
+    m = ClockMaintainer(dev(p))
+    o = oracle.bruteforce_top2(p)
+    o_c, o_stamp, o_S = o.c.copy(), np.zeros(N, np.float32), 0.0
+    for step in range(15):
+        q, movers = mot.step(p)
+        F, nF = m.step(dev(q), movers=None if movers is None else dev(movers))
+        o_S, o_flags, o_F = oracle.clock_frontier(o_c, o_stamp, o_S, oracle.max_displacement(p, q))
+        post = oracle.bruteforce_top2(q)
+        got = host(m.certs)
+        assert float(m.S[0].item()) == o_S
+        assert np.array_equal(m.flags.cpu().numpy(), o_flags), f"step {step}: expired set differs"
+        assert np.array_equal(np.sort(F.cpu().numpy()[: int(nF.item())]), o_F)
+        assert_same(got, post, idx=o_F, what=f"clock {cfg}/{fam} step {step}")
+        assert np.array_equal(got.nn, post.nn), f"step {step}: a stale certificate holds a wrong nn"
+        o_c[o_F] = post.c[o_F]
+        o_stamp[o_F] = oracle.clock_stamp(o_S)
+        assert np.array_equal(m.stamp.cpu().numpy().view(np.uint32), o_stamp.view(np.uint32))
+        p = q
+
+
 def test_search_refused_on_dirty_grid():
     p, mot = wl.make_scene("cfg1")
     grid = kc.Grid(p.shape[0], geoms(p)[1])

@@ -321,3 +321,47 @@ def test_lemma1_no_missed_failure(cfg, fam):
         assert np.array_equal(Ft, changed) and counts[2] == 0
         assert counts[0] == counts[1] == changed.size and counts[1] + counts[3] == F.size
         p, pre = q, post
+
+
+# ------------------------------------------------------------------ NEXT #3: cumulative clock (A.2)
+def test_clock_rule_hand_worked():
+    """Appendix A.2: valid while S - S_i < c_i/4.  eps = 2^-10 per step (dyadic, exact):
+    c = 10 eps expires at step 3 (4*3 eps >= 10 eps), c = 8 eps at step 2 (inclusive), c = 4 eps at
+    step 1, c = 4.5 eps at step 2; a point re-stamped at step 2 with c = 8 eps expires again at step 4."""
+    eps = np.float32(2.0 ** -10)
+    c = np.array([10, 8, 4, 4.5, 1000], np.float32) * eps
+    stamp = np.zeros(5, np.float32)
+    S = 0.0
+    seen = []
+    for step in (1, 2, 3, 4):
+        S, flags, F = oracle.clock_frontier(c, stamp, S, eps)
+        assert S == step * float(eps)
+        seen.append(F.tolist())
+        stamp[F] = oracle.clock_stamp(S)
+    assert seen == [[2], [1, 2, 3], [0, 2], [1, 2, 3]]
+    # stamps round DOWN: the elapsed clock is never under-estimated
+    for S in (0.1, 1.0 / 3.0, 1e-7, 123.456789):
+        st = oracle.clock_stamp(S)
+        assert float(st) <= S < float(np.nextafter(st, np.float32(np.inf)))
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg2", "shear"), ("cfg3", "cluster_drift"), ("cfg3", "vortex")])
+def test_clock_maintenance_keeps_nn_exact(cfg, fam):
+    """The rule itself (Theorem 1 on cumulative displacement): recomputing only the expired points
+    keeps every nearest neighbour exact over many steps, although most d1, d2 go stale."""
+    p, mot = wl.make_scene(cfg, fam, N=2500)
+    N = p.shape[0]
+    cert = oracle.kdtree_top2(p)
+    nn, c = cert.nn.copy(), cert.c.copy()
+    stamp = np.zeros(N, np.float32)
+    S, skipped = 0.0, 0
+    for _ in range(12):
+        q, _ = mot.step(p)
+        S, flags, F = oracle.clock_frontier(c, stamp, S, oracle.max_displacement(p, q))
+        post = oracle.kdtree_top2(q)
+        nn[F], c[F] = post.nn[F], post.c[F]
+        stamp[F] = oracle.clock_stamp(S)
+        assert np.array_equal(nn, post.nn)
+        skipped += N - F.size
+        p = q
+    assert skipped > 0
