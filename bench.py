@@ -470,16 +470,26 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
             def rebuild():
                 kc.kc_cert_grid_rebuild(m.grid, Q, m.other)
 
+            def repair_local():        # NEXT #2: the provable frontier of the per-point budget
+                kc.kc_max_displacement(P, Q, eps)
+                kc.kc_frontier_classify_local(m.grid, P, Q, certs0, eps, m.flags, m.F, m.nF)
+                kc.kc_frontier_repair(m.grid, Q, m.F, m.nF, certs, movers=MV, n_movers=nMV)
+
+            certs0 = m.certs.clone()
             t_rep = _median_ms(torch, repair, 7, setup=reset, flush=flush)
+            lemma = int(m.nF.item())
+            t_loc = _median_ms(torch, repair_local, 7, setup=reset, flush=flush)
+            local_frac = int(m.nF.item()) / N
             t_reb = _median_ms(torch, rebuild, 7, flush=flush)
             kc.kc_frontier_entropy(m.grid, MV, nMV, out=(H, mc, Cc))
-            lemma = int(m.nF.item())
             rows.append(dict(f=f, movers=int(movers.size), repair_ms=t_rep, rebuild_ms=t_reb, H=float(H.item()),
-                             m_cells=int(mc.item()), lemma1_frontier_frac=lemma / N))
+                             m_cells=int(mc.item()), lemma1_frontier_frac=lemma / N,
+                             local_frontier_frac=local_frac, repair_local_ms=t_loc))
             del m
         fs = [r["f"] for r in rows]
         sweep["ball" if ball else "scattered"] = dict(
-            rows=rows, crossover_f=crossover_fraction(fs, [r["repair_ms"] for r in rows], [r["rebuild_ms"] for r in rows]))
+            rows=rows, crossover_f=crossover_fraction(fs, [r["repair_ms"] for r in rows], [r["rebuild_ms"] for r in rows]),
+            crossover_f_local=crossover_fraction(fs, [r["repair_local_ms"] for r in rows], [r["rebuild_ms"] for r in rows]))
     ex["cfg4_sweep"] = sweep
     # ---------------- NEXT #3: multi-step maintenance with the cumulative clock (Appendix A.2):
     # 40 steps with no rebuild in between, against a rebuild every step
@@ -535,6 +545,22 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
         certs = m.certs.clone()
         t_rep = _median_ms(torch, lambda: kc.kc_frontier_repair(m.grid, Q, m.F, m.nF, certs), 3,
                            setup=lambda: kc.kc_grid_build(m.grid, P), flush=flush)
+        # NEXT #2 at scale: 1 % scattered movers, frontier from the per-point motion budget
+        pf, motf = wl.make_scene(cfg, "fraction", fraction=0.01, ball=False)
+        qf, mvf = motf.step(pf)
+        Qf, MVf = torch.from_numpy(qf).to(dev), torch.from_numpy(mvf).to(dev)
+        nMVf = torch.tensor([mvf.size], dtype=torch.int32, device=dev)
+        epsf = torch.zeros(1, device=dev)
+        kc.kc_cert_grid_rebuild(m.grid, P, m.certs)
+        scratch = m.certs.clone()
+
+        def repair_local():
+            kc.kc_max_displacement(P, Qf, epsf)
+            kc.kc_frontier_classify_local(m.grid, P, Qf, m.certs, epsf, m.flags, m.F, m.nF)
+            kc.kc_frontier_repair(m.grid, Qf, m.F, m.nF, scratch, movers=MVf, n_movers=nMVf)
+
+        t_loc = _median_ms(torch, repair_local, 3, setup=lambda: kc.kc_grid_build(m.grid, P), flush=flush)
+        local_frac = int(m.nF.item()) / N
         # algorithmic bytes per point of the rebuild: positions read twice,
         # cell+rank written and read, histogram + scan, sorted records, idx, slot, certificates
         pos = 4 * d
@@ -552,6 +578,8 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
                        rebuild_frac_of_hbm=N * bpp / (t_reb * 1e-3) / 1e9 / hbm,
                        max_cell_occupancy=int(info.max_occ), occupied_cells=int(info.c_occ),
                        lemma1_frontier_frac=nF / N, repair_ms=t_rep, repair_points_per_s=nF / (t_rep * 1e-3),
+                       local_budget_1pct_movers=dict(frontier_frac=local_frac, repair_ms=t_loc,
+                                                     repair_over_rebuild=t_loc / t_reb),
                        allpairs_N=n_ap, allpairs_ms=t_ap, allpairs_pairs_per_s=n_ap * (n_ap - 1) / (t_ap * 1e-3),
                        allpairs_points_per_s=n_ap / (t_ap * 1e-3),
                        allpairs_tflops=n_ap * (n_ap - 1) * ops / (t_ap * 1e-3) / 1e12)

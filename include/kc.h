@@ -161,6 +161,21 @@ kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *n
 kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps, uint8_t *flags,
                                int32_t *F, int32_t *nF, void *stream);
 
+/* ---- NEXT #2: frontier from a per-point motion budget ----------------------- */
+/* The grid must be resident at p (the pre-step positions; KC_EREBUILD otherwise).  With
+ * delta_k = ||p2_k - p_k||, a = nn_i, Delta_B(i) = max delta_k over the points filed in the 3^d cell
+ * block of i's cell and R = fl(fl(h (1 - 2^-8)) - max_axis slk) (slk = (|lo| + G h) 2^-20 rounded up):
+ *   safe_local(i)  =  c_i > fl(fl(fl(fl(2 delta_i) + delta_a) + Delta_B) K) + m_i
+ *                 and  R  > fl(fl(fl(fl(d1_i + fl(2 delta_i)) + delta_a) + eps) K) + m_i,
+ *   K = 1 + 2^-18, m_i = fl(fl(d1_i + c_i) 2^-18), every fl one float32 operation, left to right;
+ *   F = { i : not ( c_i > fl(4 eps)  or  safe_local(i) ) }   (a subset of kc_frontier_classify's F).
+ * Proof sketch: Lemma 1's triangle inequality with individual displacements; points
+ * outside the block are at least R away before the step.  nn, d1, c: device [N], exact pre-step
+ * certificates; eps: device float[1] = max_k delta_k; flags / F / nF as kc_frontier_classify. */
+kc_status kc_frontier_classify_local(kc_grid *g, const float *p, const float *p2, int64_t N,
+                                     const int32_t *nn, const float *d1, const float *c, const float *eps,
+                                     uint8_t *flags, int32_t *F, int32_t *nF, void *stream);
+
 /* ---- NEXT #3: multi-step maintenance with the cumulative clock (Appendix A.2) -- */
 /* S = sum over steps of eps_s.  A certificate last recomputed at clock value S_i stays valid while
  * S - S_i < c_i / 4 (Theorem 1 applied to the cumulative displacement), so the points to revisit in

@@ -276,3 +276,54 @@ def clock_frontier(c, stamp, S_in, eps):
     st64 = np.asarray(stamp, np.float32).astype(np.float64)
     flags = (c64 <= 4.0 * (S - st64)).astype(np.uint8)
     return S, flags, np.flatnonzero(flags).astype(np.int32)
+
+
+def local_frontier(p, p2, g: Geom, nn, d1, c, eps):
+    """Per-point motion budget (reading R19), written out in float32:
+    delta_k = ||p2_k - p_k|| (O1 arithmetic), Delta_B(i) = max delta over the points filed in the
+    3^d cell block of i's cell (cells of p), a = nn_i,
+      safe_local(i) = c_i > ((2 delta_i + delta_a) + Delta_B) K + m_i
+                  and  R  > (((d1_i + 2 delta_i) + delta_a) + eps) K + m_i,
+      K = 1 + 2^-18, m_i = (d1_i + c_i) 2^-18, R = h (1 - 2^-8) - max_axis slk,
+      F = {i : not (c_i > 4 eps or safe_local(i))}.  Returns (flags, F ascending)."""
+    f32 = np.float32
+    p = _f32(p, g.d)
+    p2 = _f32(p2, g.d)
+    N, d = p.shape
+    diff = (p2 - p).astype(f32)
+    sq = (diff * diff).astype(f32)
+    s = (sq[:, 0] + sq[:, 1]).astype(f32)
+    if d == 3:
+        s = (s + sq[:, 2]).astype(f32)
+    delta = np.sqrt(s).astype(f32)
+    cid = cell_ids(p, g)
+    G = [int(x) for x in g.G]
+    cellmax = np.zeros(G[0] * G[1] * G[2], f32)
+    np.maximum.at(cellmax, cid, delta)
+    cm = np.pad(cellmax.reshape(G[2], G[1], G[0]), 1)
+    blk = np.zeros((G[2], G[1], G[0]), f32)
+    for dz in (0, 1, 2):
+        for dy in (0, 1, 2):
+            for dx in (0, 1, 2):
+                blk = np.maximum(blk, cm[dz:dz + G[2], dy:dy + G[1], dx:dx + G[0]])
+    dB = blk.reshape(-1)[cid]
+    slk = []
+    for a in range(3):
+        t = (abs(float(g.lo[a])) + G[a] * float(g.h)) / 1048576.0
+        slk.append(np.nextafter(f32(t), f32(np.inf)))
+    R = f32(f32(f32(g.h) * f32(0.99609375)) - max(slk))
+    eps = f32(eps)
+    nn = np.asarray(nn, np.int32)
+    d1 = np.asarray(d1, f32)
+    c = np.asarray(c, f32)
+    da = np.where(nn >= 0, delta[np.maximum(nn, 0)], f32(0)).astype(f32)
+    K = f32(1.0 + 2.0 ** -18)
+    k18 = f32(2.0 ** -18)
+    two = (f32(2) * delta).astype(f32)
+    with np.errstate(invalid="ignore", over="ignore"):
+        m = ((d1 + c).astype(f32) * k18).astype(f32)
+        rhs1 = ((((two + da).astype(f32) + dB).astype(f32) * K).astype(f32) + m).astype(f32)
+        rhs2 = (((((d1 + two).astype(f32) + da).astype(f32) + eps).astype(f32) * K).astype(f32) + m).astype(f32)
+        safe = (c > f32(f32(4) * eps)) | ((c > rhs1) & (R > rhs2))
+    flags = (~safe).astype(np.uint8)
+    return flags, np.flatnonzero(flags).astype(np.int32)

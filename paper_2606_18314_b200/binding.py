@@ -25,7 +25,7 @@ EXPORTS = (
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp",
+    "kc_frontier_repair", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
     "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
@@ -94,6 +94,7 @@ def lib():
     L.kc_failure_audit.argtypes = [vp, vp, vp, i64, vp, vp, vp]
     L.kc_frontier_classify_clock.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp]
     L.kc_clock_stamp.argtypes = [vp, vp, i64, i64, vp, vp, vp]
+    L.kc_frontier_classify_local.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
@@ -346,6 +347,24 @@ def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_mo
                                     _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
                                     *certs._ptrs(), _stream()), "kc_frontier_repair")
     return certs
+
+
+def kc_frontier_classify_local(grid: Grid, p, p2, certs: Certs, eps, flags=None, F=None, nF=None):
+    """NEXT #2: frontier from per-point displacements and the per-block maximum; a
+    subset of the Lemma-1 frontier that shrinks with the number of movers.  Grid resident at p."""
+    pp, N, d = _pos(p)
+    pq, N2, d2 = _pos(p2, "p2")
+    if (N, d) != (N2, d2):
+        raise ValueError("p and p2 must have the same shape")
+    flags = flags if flags is not None else torch.empty(N, dtype=torch.uint8, device=p.device)
+    F = F if F is not None else torch.empty(N, dtype=torch.int32, device=p.device)
+    nF = nF if nF is not None else torch.empty(1, dtype=torch.int32, device=p.device)
+    _check(lib().kc_frontier_classify_local(grid._h, pp, pq, N, _ptr(certs.nn, torch.int32, "nn"),
+                                            _ptr(certs.d1, torch.float32, "d1"), _ptr(certs.c, torch.float32, "c"),
+                                            _ptr(eps, torch.float32, "eps"), _ptr(flags, torch.uint8, "flags"),
+                                            _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), _stream()),
+           "kc_frontier_classify_local")
+    return flags, F, nF
 
 
 def kc_frontier_classify_clock(c, stamp, S_in, eps, S_out, flags=None, F=None, nF=None):

@@ -64,6 +64,8 @@ struct kc_grid {
     int32_t *blocksums;
     int32_t *mark;            // per sorted slot: epoch of the last sweep that queried it
     int32_t *list2;           // frontier points of the current sweep that live in chains
+    float *delta;             // NEXT #2: displacement of every point in the current step
+    unsigned *cellmax;        // NEXT #2: largest displacement (float bits) per cell
     int epoch;
     float2 *spos2;
     float4 *spos4, *opos;
@@ -1189,6 +1191,83 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
     }
 }
 
+// ------------------------------------------------------------------ NEXT #2: local motion budget
+// "A per-point motion budget would tighten the safe set without affecting the no-miss guarantee"
+// (PAPER.md:127).  With delta_k = ||p'_k - p_k|| the displacement of point k, a = nn_i, B(i) the 3^d
+// cell block around i's (pre-step) cell and Delta_B(i) = max of delta_k over the points filed in
+// B(i), certificate i keeps its nearest neighbour if
+//   (1)  c_i > 2 delta_i + delta_a + Delta_B(i)          (every k in the block stays behind a), and
+//   (2)  R   > d1_i + 2 delta_i + delta_a + eps_t         (every k outside the block, at distance
+//                                                          >= R ~ h before the step, stays behind a),
+// by the triangle-inequality argument of Lemma 1 with the individual displacements in
+// place of eps.  Lemma 1's own test c_i > 4 eps_t remains a sufficient alternative.  The frontier is
+//   F_local = { i : not ( c_i > 4 eps_t  or  ((1) and (2)) ) }  (a subset of Lemma 1's set),
+// and it shrinks with the number of movers, which the global rule does not (reading R12).
+// All tests in float32, fixed operation order, right-hand sides inflated by K = 1 + 2^-18 plus
+// 2^-18 d2_i for the roundings of c, d1, delta (reading R19); the oracle restates them.
+__global__ void __launch_bounds__(256)
+motion_field_kernel(int D, const float *__restrict__ p, const float *__restrict__ p2, int N,
+                    const int32_t *__restrict__ cell, float *__restrict__ delta, unsigned *cellmax)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float s;
+    if (D == 2) s = sqd2(p2[2 * (int64_t)i], p2[2 * (int64_t)i + 1], p[2 * (int64_t)i], p[2 * (int64_t)i + 1]);
+    else s = sqd3(p2[3 * (int64_t)i], p2[3 * (int64_t)i + 1], p2[3 * (int64_t)i + 2], p[3 * (int64_t)i],
+                  p[3 * (int64_t)i + 1], p[3 * (int64_t)i + 2]);
+    const float dl = __fsqrt_rn(s);
+    delta[i] = dl;
+    if (dl > 0.0f) atomicMax(&cellmax[cell[i]], __float_as_uint(dl));     // delta >= 0: bits are ordered
+}
+
+__global__ void __launch_bounds__(256)
+classify_local_kernel(View v, float R, int N, const int32_t *__restrict__ cell,
+                      const float *__restrict__ delta, const unsigned *__restrict__ cellmax,
+                      const int32_t *__restrict__ nn, const float *__restrict__ d1, const float *__restrict__ c,
+                      const float *__restrict__ eps, uint8_t *__restrict__ flags, int32_t *__restrict__ F,
+                      int32_t *nF)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool infr = false;
+    if (i < N) {
+        const float e = *eps, ci = c[i];
+        if (!(ci > __fmul_rn(4.0f, e))) {
+            const float K = 1.0f + 1.0f / 262144.0f;
+            const int cid = cell[i];
+            const int cx = cid % v.G0, cy = (cid / v.G0) % v.G1, cz = cid / (v.G0 * v.G1);
+            unsigned mx = 0;
+            for (int z = max(cz - 1, 0); z <= min(cz + 1, v.G2 - 1); ++z)
+                for (int y = max(cy - 1, 0); y <= min(cy + 1, v.G1 - 1); ++y)
+                    for (int x = max(cx - 1, 0); x <= min(cx + 1, v.G0 - 1); ++x)
+                        mx = max(mx, cellmax[(z * v.G1 + y) * v.G0 + x]);
+            const float dB = __uint_as_float(mx);
+            const int a = nn[i];
+            const float di = delta[i], da = a >= 0 ? delta[a] : 0.0f, d1i = d1[i];
+            const float two = __fmul_rn(2.0f, di);
+            const float m = __fmul_rn(__fadd_rn(d1i, ci), 1.0f / 262144.0f);
+            const float rhs1 = __fadd_rn(__fmul_rn(__fadd_rn(__fadd_rn(two, da), dB), K), m);
+            const float rhs2 = __fadd_rn(__fmul_rn(__fadd_rn(__fadd_rn(__fadd_rn(d1i, two), da), e), K), m);
+            infr = !(ci > rhs1 && R > rhs2);
+        }
+        if (flags) flags[i] = (uint8_t)infr;
+    }
+    // compaction: ids ascending inside the block, one atomicAdd per block
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned m = __ballot_sync(0xffffffffu, infr);
+    __shared__ int wsum[8];
+    __shared__ int bbase;
+    if (lane == 0) wsum[warp] = __popc(m);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
+        bbase = tot ? atomicAdd(nF, tot) : 0;
+    }
+    __syncthreads();
+    if (infr) F[bbase + wsum[warp] + __popc(m & ((1u << lane) - 1))] = i;
+}
+
 inline int blocks_for(int64_t n, int threads, int cap = 148 * 16)
 {
     int64_t b = (n + threads - 1) / threads;
@@ -1245,6 +1324,7 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     alloc((void **)&g->blocksums, (size_t)g->n_scan_blocks * 4 + 4);
     alloc((void **)&g->mark, (n + 8) * 4);
     alloc((void **)&g->list2, n * 4);
+    alloc((void **)&g->delta, n * 4); alloc((void **)&g->cellmax, nc * 4);
     g->spos2 = nullptr; g->spos4 = nullptr;
     if (geom->d == 2) alloc((void **)&g->spos2, (n + 8) * sizeof(float2));
     else alloc((void **)&g->spos4, (n + 8) * sizeof(float4));
@@ -1275,7 +1355,7 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
     void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
-                    g->mlist, g->fcount, g->mhist, g->blocksums, g->mark, g->list2, g->spos2, g->spos4, g->opos, g->ctr};
+                    g->mlist, g->fcount, g->mhist, g->blocksums, g->mark, g->list2, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete g;
@@ -1355,6 +1435,36 @@ extern "C" kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N,
     s = kc_grid_build(g, p, N, stream);
     if (s != KC_OK) return s;
     return kc_cert_grid_search(g, nn, nn2, d1, d2, c, stream);
+}
+
+extern "C" kc_status kc_frontier_classify_local(kc_grid *g, const float *p, const float *p2, int64_t N,
+                                                const int32_t *nn, const float *d1, const float *c,
+                                                const float *eps, uint8_t *flags, int32_t *F, int32_t *nF,
+                                                void *stream)
+{
+    if (!g || !p || !p2 || !nn || !d1 || !c || !eps || !F || !nF) {
+        set_error("kc_frontier_classify_local: bad argument");
+        return KC_EINVAL;
+    }
+    if (!g->built || N != g->N) {
+        set_error("kc_frontier_classify_local: grid not resident at p for this N");
+        return KC_EREBUILD;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    View v = make_view(g);
+    // everything outside the 3^d block of a point's cell is at least R away from it
+    const float slkmax = fmaxf(v.slk0, fmaxf(v.slk1, v.slk2));
+    volatile float hr = g->geom.h * 0.99609375f;          // two separately rounded float32 ops
+    const float R = hr - slkmax;
+    const int n = (int)N;
+    KC_CUDA(cudaMemsetAsync(g->cellmax, 0, (size_t)g->n_cells * 4, st));
+    KC_CUDA(cudaMemsetAsync(nF, 0, 4, st));
+    motion_field_kernel<<<(n + 255) / 256, 256, 0, st>>>(g->geom.d, p, p2, n, g->cell, g->delta, g->cellmax);
+    classify_local_kernel<<<(n + 255) / 256, 256, 0, st>>>(v, R, n, g->cell, g->delta, g->cellmax, nn, d1, c, eps,
+                                                           flags, F, nF);
+    count_launches(2);
+    KC_LAUNCH_CHECK("kc_frontier_classify_local");
+    return KC_OK;
 }
 
 extern "C" kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF,

@@ -361,6 +361,34 @@ def test_clock_maintenance_multi_step(cfg, fam):
         p = q
 
 
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "cluster_drift"), ("cfg3", "diffuse5"),
+                                     ("cfg3", "ball5"), ("cfg4", "fraction")])
+def test_local_motion_budget_frontier(cfg, fam):
+    """NEXT #2: kc_frontier_classify_local, flags bit-exact against the oracle's
+    float32 restatement, F as a set, and the repaired certificates keep nn exact for all points."""
+    if cfg == "cfg4":
+        p, mot = wl.make_scene("cfg4", "fraction", fraction=0.01, ball=False, N=60000)
+    else:
+        p, mot = wl.make_scene(cfg, fam)
+    q, movers = mot.step(p)
+    N = p.shape[0]
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    P, Q = dev(p), dev(q)
+    certs = kc.kc_cert_grid_rebuild(grid, P)
+    eps = kc.kc_max_displacement(P, Q)
+    flags, F, nF = kc.kc_frontier_classify_local(grid, P, Q, certs, eps)
+    pre = ref_certs(p)
+    wflags, wF = oracle.local_frontier(p, q, g_or, pre.nn, pre.d1, pre.c, oracle.max_displacement(p, q))
+    assert np.array_equal(flags.cpu().numpy(), wflags)
+    assert int(nF.item()) == wF.size and np.array_equal(np.sort(F.cpu().numpy()[: wF.size]), wF)
+    kc.kc_frontier_repair(grid, Q, F, nF, certs, movers=None if movers is None else dev(movers))
+    post = ref_certs(q)
+    got = host(certs)
+    assert_same(got, post, idx=wF, what=f"local budget repair {cfg}/{fam}")
+    assert np.array_equal(got.nn, post.nn)                       # no missed failure
+
+
 def test_search_refused_on_dirty_grid():
     p, mot = wl.make_scene("cfg1")
     grid = kc.Grid(p.shape[0], geoms(p)[1])

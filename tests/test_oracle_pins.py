@@ -365,3 +365,49 @@ def test_clock_maintenance_keeps_nn_exact(cfg, fam):
         skipped += N - F.size
         p = q
     assert skipped > 0
+
+
+# ------------------------------------------------------------------ NEXT #2: local motion budget
+def test_local_budget_hand_worked():
+    """One far mover: Lemma 1's global rule flags every low-clearance certificate, the per-point
+    budget only those whose block holds the mover.  Dyadic scene, h = 1/8."""
+    p = np.array([[0.0, 0.0], [1 / 64, 0.0], [-5 / 256, 0.0],          # i, a, k: c_i = 1/256
+                  [0.875, 0.875], [0.875 + 1 / 64, 0.875], [0.875, 0.875 - 5 / 256],   # the mover and two bystanders
+                  [1.0, 1.0], [-0.0625, -0.0625]], np.float32)
+    q = p.copy()
+    q[3] += np.float32(1 / 256)                                        # eps = sqrt(2)/256 ~ 0.00552
+    g = oracle.geom_from_bbox(8, 2, np.array([-0.0625, -0.0625, 0], np.float32), np.array([1, 1, 0], np.float32), 0.125)
+    assert tuple(g.G[:2]) == (8, 8)
+    pre = oracle.bruteforce_top2(p)
+    eps = oracle.max_displacement(p, q)
+    gflags, _ = oracle.frontier(pre.c, eps)
+    lflags, LF = oracle.local_frontier(p, q, g, pre.nn, pre.d1, pre.c, eps)
+    assert float(pre.c[0]) == 1 / 256 and gflags[0] == 1               # 4 eps ~ 0.022 > c_i
+    assert lflags[0] == 0 and lflags[1] == 0 and lflags[2] == 0        # nothing moved in their block
+    # the mover's block: c_3 = 0.0039 <= 3 eps, c_4 = 0.0094 and c_5 = 0.0055 <= d_a + D_B = 2 eps = 0.011
+    assert lflags[3] == 1 and lflags[4] == 1 and lflags[5] == 1
+    assert np.all(lflags <= gflags)
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", f) for f in wl.CONFIGS["cfg2"]["families"]] +
+                         [("cfg3", f) for f in wl.CONFIGS["cfg3"]["families"]])
+def test_local_budget_never_misses(cfg, fam):
+    """No-miss guarantee of the per-point budget and F_local subset of Lemma 1's set, on all ten
+    families; on the partial-motion families the local frontier is several times smaller."""
+    p, mot = wl.make_scene(cfg, fam, N=4000)
+    pre = oracle.kdtree_top2(p)
+    ratio = []
+    for _ in range(3):
+        q, movers = mot.step(p)
+        g = oracle.geom_for(p)
+        eps = oracle.max_displacement(p, q)
+        gflags, GF = oracle.frontier(pre.c, eps)
+        lflags, LF = oracle.local_frontier(p, q, g, pre.nn, pre.d1, pre.c, eps)
+        post = oracle.kdtree_top2(q)
+        changed = np.flatnonzero(pre.nn != post.nn)
+        assert np.all(lflags[changed] == 1)
+        assert np.all(lflags <= gflags)
+        ratio.append(LF.size / max(GF.size, 1))
+        p, pre = q, post
+    if fam in ("local", "diffuse5", "ball5"):
+        assert max(ratio) < 0.5
