@@ -69,7 +69,8 @@ typedef struct kc_grid kc_grid;
 typedef struct {
     int64_t n_points;    /* N of the last build */
     int64_t n_cells;     /* G[0]*G[1]*G[2] */
-    int32_t c_occ;       /* C: cells holding >= 1 point at the current filing */
+    int32_t c_occ;       /* C: cells holding >= 1 point, as of the last build or the last
+                          * kc_frontier_entropy call, whichever is later */
     int32_t max_occ;     /* largest cell occupancy seen by the last build */
     int32_t n_misfiled;  /* points re-filed into overflow chains since the last build */
     int32_t built;       /* 1 once kc_grid_build has run */
