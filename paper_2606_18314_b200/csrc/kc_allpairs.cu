@@ -395,7 +395,7 @@ Shape choose_shape(int64_t nq, int64_t N)
     int64_t per = (int64_t)s.qpt * s.threads;
     int64_t itiles = (nq + per - 1) / per;
     int64_t want = (148 * 8 * 8 + itiles - 1) / itiles;
-    int64_t cap = (N - AP_SEED) / AP_TJ;
+    int64_t cap = (N - AP_SEED + AP_TJ - 1) / AP_TJ;
     int64_t js = want < cap ? want : cap;
     if (e_js > 0) js = e_js;
     if (js < 1) js = 1;
@@ -441,10 +441,16 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     if (split || bounded) KC_CUDA(cudaMemsetAsync(ws, 0, split ? head_bytes(nq, sh) : 16, st));
     a.jfirst = split && !bounded ? AP_SEED : 0;
     int js = sh.js;
-    int64_t jchunk = (a.N - a.jfirst + js - 1) / js;
-    // whole tiles per chunk when split (a tile is evaluated in full, +inf padding included)
-    const int64_t gran = split ? AP_TJ : 16;
-    jchunk = (jchunk + gran - 1) / gran * gran;
+    int64_t jchunk;
+    if (split) {
+        // whole tiles per chunk (a tile is evaluated in full, +inf padding included): as many
+        // chunks as the shape wants, but never a chunk of less than one tile
+        const int64_t tiles = (a.N - a.jfirst + AP_TJ - 1) / AP_TJ;
+        const int64_t want = js < tiles ? js : tiles;
+        jchunk = (tiles + want - 1) / want * AP_TJ;
+    } else {
+        jchunk = (a.N + 15) / 16 * 16;
+    }
     js = (int)((a.N - a.jfirst + jchunk - 1) / jchunk);
     a.jchunk = jchunk;
     a.seed = nullptr;
