@@ -193,7 +193,7 @@ def run_gpu_arm(args):
     import torch.distributed as dist
 
     from paper_2606_18314_b200 import binding as kc
-    from paper_2606_18314_b200.driver import Maintainer, crossover_fraction
+    from paper_2606_18314_b200.driver import GraphMaintainer, Maintainer, crossover_fraction
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -223,42 +223,75 @@ def run_gpu_arm(args):
     dev_traj = {f: [torch.from_numpy(p).to(dev) for p in traj[f][0][: per[i] + W + 1]] for i, f in enumerate(fams)}
     dev_mv = {f: [None if m is None else torch.from_numpy(m).to(dev) for m in traj[f][1][: per[i] + W + 1]]
               for i, f in enumerate(fams)}
-    maint = {f: Maintainer(dev_traj[f][0]) for f in fams}
+    # the step is launch-bound at this N (~20 short kernels): it runs as two CUDA graphs per step
+    # (everything but all-pairs | all-pairs, so that the dominant kernel is still bracketed by
+    # events); --no-graph issues the same calls eagerly
+    use_graph = (not args.no_graph) and N <= GraphMaintainer.MAX_N
+    maint = {f: (GraphMaintainer if use_graph else Maintainer)(dev_traj[f][0]) for f in fams}
     torch.cuda.synchronize()
+
+    def do_step(f, t, timed):
+        if use_graph:
+            return maint[f].step(dev_traj[f][t], time_allpairs=timed)
+        return maint[f].step(dev_traj[f][t], movers=dev_mv[f][t], time_phases=timed)
 
     phase_sum = {ph: 0.0 for ph in ("maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs")}
     fam_stats = {f: dict(steps=0, repair_ms=0.0, rebuild_ms=0.0, frontier=0, H=0.0) for f in fams}
-    step_events, phase_events = [], []
-    # warm-up (first family), untimed
-    for t in range(W):
-        maint[fams[0]].step(dev_traj[fams[0]][t + 1], movers=dev_mv[fams[0]][t + 1])
+    step_events, step_info = [], []
+    # warm-up, untimed: W steps of every family (graphs of both ping-pong parities get captured here)
+    for f in fams:
+        for t in range(W):
+            do_step(f, t + 1, False)
     barrier()
     sampler = ClockSampler(local)
     launches0 = kc.kc_launch_count()
+    graph_launches = 0
     t_wall0 = time.perf_counter()
     for fi, f in enumerate(fams):
-        off = W if fi == 0 else 0
         for t in range(per[fi]):
             flush.zero_()                                            # L2 flush between timed steps
             e0 = torch.cuda.Event(enable_timing=True)
             e1 = torch.cuda.Event(enable_timing=True)
+            if use_graph:
+                graph_launches += maint[f].launches_per_step()
             e0.record()
-            res = maint[f].step(dev_traj[f][off + t + 1], movers=dev_mv[f][off + t + 1], time_phases=True)
+            res = do_step(f, W + t + 1, True)
             e1.record()
             step_events.append((e0, e1))
-            phase_events.append((f, res.phase_ms, res.nF.clone(), res.H.clone()))
+            step_info.append((f, maint[f].ap_events if use_graph else res.phase_ms, res.nF.clone(), res.H.clone()))
     barrier()
     t_wall = time.perf_counter() - t_wall0
-    launches = kc.kc_launch_count() - launches0
+    launches = kc.kc_launch_count() - launches0 + graph_launches
     clocks = sampler.stop()
     dev_ms = sum(a.elapsed_time(b) for a, b in step_events)
-    for f, ev, nF, H in phase_events:
-        pt = Maintainer.phase_times(ev)
-        for ph in phase_sum:
-            phase_sum[ph] += pt[ph]
+    ap_ms_sum = 0.0
+    for f, ev, nF, H in step_info:
         s = fam_stats[f]
-        s["steps"] += 1; s["repair_ms"] += pt["repair"] + pt["classify"] + pt["maxdisp"]
-        s["rebuild_ms"] += pt["rebuild"]; s["frontier"] += int(nF.item()); s["H"] += float(H.item())
+        s["steps"] += 1; s["frontier"] += int(nF.item()); s["H"] += float(H.item())
+        if use_graph:
+            ap_ms_sum += ev[0].elapsed_time(ev[1])
+        else:
+            pt = Maintainer.phase_times(ev)
+            ap_ms_sum += pt["allpairs"]
+    # per-phase times: an eager pass of the same steps outside the timed region (events between
+    # the calls; inside a graph there is nothing to bracket)
+    ph_steps = 0
+    em = {f: Maintainer(dev_traj[f][0]) for f in fams}
+    for fi, f in enumerate(fams):
+        for t in range(W + min(per[fi], 10)):
+            if t >= W:
+                flush.zero_()
+            r = em[f].step(dev_traj[f][t + 1], movers=dev_mv[f][t + 1], time_phases=t >= W)
+            if t >= W:
+                torch.cuda.synchronize()
+                pt = Maintainer.phase_times(r.phase_ms)
+                for ph in phase_sum:
+                    phase_sum[ph] += pt[ph]
+                ph_steps += 1
+                fs = fam_stats[f]
+                fs["repair_ms"] += pt["repair"] + pt["classify"] + pt["maxdisp"]; fs["rebuild_ms"] += pt["rebuild"]
+                fs["ph_steps"] = fs.get("ph_steps", 0) + 1
+    del em
     dev_ms_max, units = aggregate_over_ranks(dev_ms, N * K, dev)
     value = units / (dev_ms_max * 1e-3)
 
@@ -275,7 +308,7 @@ def run_gpu_arm(args):
     barrier()
     k = 0
     for fi, f in enumerate(fams):
-        base = per[fi] + (W if fi == 0 else 0)        # continue each family's trajectory
+        base = per[fi] + W                            # continue each family's trajectory
         m = maint[f]
         for t in range(per[fi]):
             flush.zero_()
@@ -287,7 +320,7 @@ def run_gpu_arm(args):
             buf.copy_(host_next[f][base + t + 1], non_blocking=True)
             mv = traj[f][1][base + t + 1]
             mvd = None if mv is None else torch.from_numpy(mv).to(dev, non_blocking=True)
-            res = m.step(buf, movers=mvd)
+            res = m.step(buf) if use_graph else m.step(buf, movers=mvd)
             host_out["nn"].copy_(res.rebuilt.nn, non_blocking=True)
             host_out["d1"].copy_(res.rebuilt.d1, non_blocking=True)
             host_out["d2"].copy_(res.rebuilt.d2, non_blocking=True)
@@ -311,10 +344,11 @@ def run_gpu_arm(args):
         except OSError:
             pass
         # ---- parity of the timed outputs against the CPU oracle (outside the timed region) ----
-        certified, audit = verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams)
+        certified, audit = verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams,
+                                                 graph_cls=GraphMaintainer if use_graph else None)
         # ---- roofline of the dominant kernel (all-pairs; FP32 ALU bound) ----
         ops_per_pair = 5 if d == 2 else 8
-        ap_ms = phase_sum["allpairs"] / K
+        ap_ms = ap_ms_sum / K                      # live CUDA events around the kernel's launch, timed region
         achieved = N * (N - 1) * ops_per_pair / (ap_ms * 1e-3) / 1e12
         sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
         peak = FP32_LANES * sm_max * 1e6 / 1e12
@@ -324,7 +358,7 @@ def run_gpu_arm(args):
                         note=(f"{ops_per_pair} separately rounded FP32 ops per ordered pair (no FMA by contract); peak = "
                               f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md); measured non-fused "
                               f"FADD/FMUL chain rate {probe:.2f} Top/s; kernel share of step = "
-                              f"{phase_sum['allpairs'] / sum(phase_sum.values()):.2f}"),
+                              f"{ap_ms / (dev_ms_max / K):.2f}"),
                         pairs_per_s=N * (N - 1) / (ap_ms * 1e-3), ms_per_launch=ap_ms, fp32_probe_tops=probe)
         cpu = run_oracle_arm(cfg, K=30, W=0, time_budget_s=25.0)
         cpu_baseline = dict(value=cpu["value"], unit=UNIT, cores=cpu["cores"], kind="oracle", sample=cpu["sample"],
@@ -334,8 +368,8 @@ def run_gpu_arm(args):
             extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks)
         families = {f: dict(steps=s["steps"], frontier_frac=s["frontier"] / max(1, s["steps"]) / N,
                             H=s["H"] / max(1, s["steps"]),
-                            repair_path_ms=s["repair_ms"] / max(1, s["steps"]),
-                            rebuild_path_ms=s["rebuild_ms"] / max(1, s["steps"]),
+                            repair_path_ms=s["repair_ms"] / max(1, s.get("ph_steps", 0)),
+                            rebuild_path_ms=s["rebuild_ms"] / max(1, s.get("ph_steps", 0)),
                             repair_over_rebuild=s["repair_ms"] / max(s["rebuild_ms"], 1e-12),
                             # Definition 2 / Table 1 on the certified transitions: P_t = |F_t|/N,
                             # fraction re-validated although still valid, Lemma-1 misses (must be 0)
@@ -351,6 +385,8 @@ def run_gpu_arm(args):
                                    f"(A1 = the full N(N-1)-pair pass, started from the kinetic bound d2+2eps of the "
                                    f"maintained certificates, kc_cert_allpairs_bounded)",
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
+                       "launch": ("two CUDA graphs per step (all rows but A1 | A1), replayed; all-pairs bracketed by events"
+                                  if use_graph else "eager stream launches"),
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
                        "certified": certified},
             "clocks": clocks,
@@ -358,10 +394,11 @@ def run_gpu_arm(args):
             "gpu_launches": int(launches),
             "roofline": roofline,
             "cpu_baseline": cpu_baseline,
-            "phases_ms_per_step": {ph: v / K for ph, v in phase_sum.items()},
-            "paths_points_per_s": {"allpairs": N / (phase_sum["allpairs"] / K * 1e-3),
-                                   "grid_rebuild": N / (phase_sum["rebuild"] / K * 1e-3),
-                                   "frontier_repair": N / ((phase_sum["repair"] + phase_sum["classify"] + phase_sum["maxdisp"]) / K * 1e-3)},
+            # eager (ungraphed) pass of the same steps outside the timed region
+            "phases_ms_per_step": {ph: v / max(ph_steps, 1) for ph, v in phase_sum.items()},
+            "paths_points_per_s": {"allpairs": N / (ap_ms * 1e-3),
+                                   "grid_rebuild": N / (phase_sum["rebuild"] / max(ph_steps, 1) * 1e-3),
+                                   "frontier_repair": N / ((phase_sum["repair"] + phase_sum["classify"] + phase_sum["maxdisp"]) / max(ph_steps, 1) * 1e-3)},
             "families": families,
             "wall_s_timed_region": t_wall,
             "extras": extras,
@@ -372,7 +409,7 @@ def run_gpu_arm(args):
     return out
 
 
-def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per_family=2):
+def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per_family=2, graph_cls=None):
     """'Certified' = the outputs of the timed configuration equal the CPU oracle's bit for bit
     (H within 1e-6).  Checked outside the timed region on the first transitions of every family;
     raises on any mismatch."""
@@ -382,13 +419,18 @@ def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per
     audit = {}
     for f in fams:
         ps, mvs = traj[f]
-        m = Maintainer(torch.from_numpy(ps[0]).to(dev))
+        m = (graph_cls or Maintainer)(torch.from_numpy(ps[0]).to(dev))
         g = oracle.geom_for(ps[0])
         pre = oracle.bruteforce_top2(ps[0])
         for t in range(steps_per_family):
             q = ps[t + 1]
             mv = None if mvs[t + 1] is None else torch.from_numpy(mvs[t + 1]).to(dev)
-            res = m.step(torch.from_numpy(q).to(dev), movers=mv, audit=True)
+            if graph_cls is not None:                      # the launch configuration the bench times
+                nn_pre = m.cert[m.k].nn.clone()
+                res = m.step(torch.from_numpy(q).to(dev))
+                res.audit, res.Ft = kc.kc_failure_audit(nn_pre, res.rebuilt.nn, m.m.flags)
+            else:
+                res = m.step(torch.from_numpy(q).to(dev), movers=mv, audit=True)
             torch.cuda.synchronize()
             post = oracle.bruteforce_top2(q)
             eps = oracle.max_displacement(ps[t], q)
@@ -595,6 +637,7 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"])
     ap.add_argument("--no-extras", action="store_true", help="skip the config 4 / config 5 side measurements")
+    ap.add_argument("--no-graph", action="store_true", help="issue the step eagerly instead of replaying CUDA graphs")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

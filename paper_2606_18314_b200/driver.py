@@ -207,3 +207,77 @@ class ClockMaintainer:
         kc.kc_clock_stamp(self.stamp, self.S[0], self.F, self.nF, self.N)
         self.p = p_next
         return self.F, self.nF
+
+
+class GraphMaintainer:
+    """The step of :class:`Maintainer` captured in CUDA graphs (small N is launch-bound: ~20 short
+    kernels per step).  Two graphs per ping-pong parity: A = A0, A4, A6+A7, A5, A2+A3 and B = the
+    all-pairs certification, so that the dominant kernel can still be bracketed by CUDA events.
+
+    Device pointers are fixed: positions live in two library-side buffers (the caller's p_next is
+    copied in, 4 d N bytes), certificates ping-pong between two buffers.  Every point is treated as
+    a potential mover (no mover list: its length varies from step to step), which changes no
+    result.  Only for grids below the sweep threshold of kc_frontier_repair (its epoch is a
+    host-side counter); larger problems are not launch-bound and use :class:`Maintainer`."""
+
+    MAX_N = 199_999
+
+    def __init__(self, p0: torch.Tensor, occ: float = 2.0):
+        assert int(p0.shape[0]) <= self.MAX_N, "GraphMaintainer is for launch-bound (small) problems"
+        self.m = Maintainer(p0, occ)
+        self.N = self.m.N
+        self.pos = [p0.clone(), torch.empty_like(p0)]
+        self.cert = [self.m.certs, self.m.other]
+        self.k = 0
+        self.graphs = [None, None]
+        self.launches = [0, 0]
+        self.ap_events = None
+
+    def _body_a(self, k):
+        m, cur, nxt = self.m, self.pos[k], self.pos[1 - k]
+        certs, other = self.cert[k], self.cert[1 - k]
+        kc.kc_max_displacement(cur, nxt, m.eps)
+        kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
+        kc.kc_frontier_repair(m.grid, nxt, m.F, m.nF, certs, nF_max=self.N)
+        kc.kc_frontier_entropy(m.grid, m.F, m.nF, nF_max=self.N, out=(m.H, m.m, m.C))
+        kc.kc_cert_grid_rebuild(m.grid, nxt, other)
+
+    def _body_b(self, k):
+        m = self.m
+        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=self.cert[k].d2, eps=m.eps)
+
+    def _capture(self, k):
+        n0 = kc.kc_launch_count()
+        ga, gb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+        with torch.cuda.graph(ga):
+            self._body_a(k)
+        with torch.cuda.graph(gb):
+            self._body_b(k)
+        self.graphs[k] = (ga, gb)
+        self.launches[k] = kc.kc_launch_count() - n0
+
+    def step(self, p_next: torch.Tensor, time_allpairs: bool = False) -> StepResult:
+        """One transition; returns the same StepResult as Maintainer.step (no host sync).  With
+        ``time_allpairs`` two CUDA events bracket the all-pairs graph (``self.ap_events``)."""
+        k, m = self.k, self.m
+        self.pos[1 - k].copy_(p_next, non_blocking=True)
+        if self.graphs[k] is None:
+            torch.cuda.synchronize()
+            self._capture(k)
+        ga, gb = self.graphs[k]
+        ga.replay()
+        if time_allpairs:
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            gb.replay()
+            e1.record()
+            self.ap_events = (e0, e1)
+        else:
+            gb.replay()
+        self.k = 1 - k
+        return StepResult(m.eps, m.nF, m.H, m.m, m.C, self.cert[k], self.cert[1 - k], m.ap)
+
+    def launches_per_step(self, k=None):
+        """Kernels of this library launched by one replayed step (counted at capture)."""
+        return self.launches[self.k if k is None else k]

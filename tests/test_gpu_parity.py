@@ -389,6 +389,34 @@ def test_local_motion_budget_frontier(cfg, fam):
     assert np.array_equal(got.nn, post.nn)                       # no missed failure
 
 
+@pytest.mark.parametrize("cfg,fam", [("cfg1", "walk"), ("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "cluster_drift")])
+def test_graphed_step_matches_the_oracle(cfg, fam):
+    """The CUDA-graph form of the step (driver.GraphMaintainer): 5 replayed transitions, every
+    output bit-exact against the oracle, and identical to the eager step."""
+    from paper_2606_18314_b200.driver import GraphMaintainer, Maintainer
+    p, mot = wl.make_scene(cfg, fam)
+    g_or, _ = geoms(p)
+    gm, em = GraphMaintainer(dev(p)), Maintainer(dev(p))
+    pre = oracle.bruteforce_top2(p)
+    for step in range(5):
+        q, movers = mot.step(p)
+        res = gm.step(dev(q))
+        ref = em.step(dev(q), movers=None if movers is None else dev(movers))
+        post = oracle.bruteforce_top2(q)
+        eps = oracle.max_displacement(p, q)
+        flags, F = oracle.frontier(pre.c, eps)
+        assert float(res.eps.item()) == float(eps) and int(res.nF.item()) == F.size
+        assert_same(res.rebuilt, post, what=f"graph rebuilt {step}")
+        assert_same(res.certified, post, what=f"graph allpairs {step}")
+        assert_same(res.repaired, post, idx=F, what=f"graph repaired {step}")
+        H, mm, C = oracle.entropy(oracle.cell_ids(q, g_or), F, g_or.n_cells)
+        assert abs(float(res.H.item()) - H) <= 1e-6 and int(res.m_cells.item()) == mm and int(res.C_occ.item()) == C
+        for f in ("nn", "nn2", "d1", "d2", "c"):
+            assert torch.equal(getattr(res.rebuilt, f), getattr(ref.rebuilt, f))
+        assert gm.launches_per_step(0) > 0
+        p, pre = q, post
+
+
 def test_search_refused_on_dirty_grid():
     p, mot = wl.make_scene("cfg1")
     grid = kc.Grid(p.shape[0], geoms(p)[1])
