@@ -35,6 +35,7 @@ struct Counters {
     int n_list2;              // frontier points of the current sweep that live in chains
     int ticket;               // blocks of entropy_collect_kernel that are done (the last one finishes)
     int c_occ_acc;            // recount of the occupied cells in progress (A5 after an incremental update)
+    int kmax;                 // largest per-cell frontier count seen by the current A5 call
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -1140,10 +1141,12 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
     int n = *nF;
     int m_local = 0;
     int c1 = 0, c2 = 0, c3 = 0, c4 = 0;             // the commonest counts stay in registers
+    int kmax_local = 0;
     for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
         int k = atomicExch(&fcount[cell[F[f]]], 0);     // first visitor collects and re-zeroes
         if (k > 0) {
             ++m_local;
+            kmax_local = max(kmax_local, k);
             c1 += k == 1; c2 += k == 2; c3 += k == 3; c4 += k == 4;
             if (k > 4) {
                 if (k < LOW) atomicAdd(&low[k], 1);
@@ -1155,7 +1158,9 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
     m_local = __reduce_add_sync(0xffffffffu, m_local);
     c1 = __reduce_add_sync(0xffffffffu, c1); c2 = __reduce_add_sync(0xffffffffu, c2);
     c3 = __reduce_add_sync(0xffffffffu, c3); c4 = __reduce_add_sync(0xffffffffu, c4);
+    kmax_local = __reduce_max_sync(0xffffffffu, kmax_local);
     if ((threadIdx.x & 31) == 0) {
+        if (kmax_local > 4) atomicMax(&ctr->kmax, kmax_local);
         if (m_local) atomicAdd(&ctr->m_cells, m_local);
         if (c1) atomicAdd(&low[1], c1);
         if (c2) atomicAdd(&low[2], c2);
@@ -1175,7 +1180,8 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
     if (!s_last) return;
     __threadfence();
     double acc = 0.0;
-    for (int k = threadIdx.x; k < MHIST; k += 256) {
+    const int lim = min(MHIST, max(__ldcg(&ctr->kmax), 4) + 1);     // bins above the largest count are empty
+    for (int k = threadIdx.x; k < lim; k += 256) {
         int M = __ldcg(&mhist[k]);
         if (M) {
             if (k > 1) acc += (double)M * ((double)k * log((double)k));
@@ -1203,6 +1209,7 @@ entropy_collect_kernel(const int32_t *__restrict__ F, const int32_t *__restrict_
         ctr->m_cells = 0;
         ctr->big = 0.0;
         ctr->ticket = 0;
+        ctr->kmax = 0;
     }
 }
 
