@@ -275,13 +275,24 @@ __global__ void __launch_bounds__(1024)
 scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *__restrict__ cell_start,
                   Counters *ctr)
 {
-    const int per = (n_cells + 1023) / 1024;
-    const int base = threadIdx.x * per;
-    int tsum = 0, occ = 0, mx = 0;
-    for (int k = 0; k < per; ++k) {
-        const int cnt = base + k < n_cells ? counts[base + k] : 0;
-        tsum += cnt; occ += cnt > 0; mx = max(mx, cnt);
+    // thread t owns the 16 cells from 16 t; all its loads are issued before the first is used
+    const int base = threadIdx.x * 16;
+    int v[16];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int i = base + 4 * q;
+        int4 x = make_int4(0, 0, 0, 0);
+        if (i + 3 < n_cells) x = *reinterpret_cast<const int4 *>(counts + i);
+        else if (i < n_cells) {
+            x.x = counts[i];
+            if (i + 1 < n_cells) x.y = counts[i + 1];
+            if (i + 2 < n_cells) x.z = counts[i + 2];
+        }
+        v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
     }
+    int tsum = 0, occ = 0, mx = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { tsum += v[k]; occ += v[k] > 0; mx = max(mx, v[k]); }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     int incl = tsum;
 #pragma unroll
@@ -309,12 +320,11 @@ scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *__re
     }
     __syncthreads();
     int run = wsum[w] + incl - tsum;
-    for (int k = 0; k < per; ++k) {
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
         // stored one slot to the right, as in scan_write_kernel (the scatter's cursors)
-        if (base + k < n_cells) {
-            cell_start[base + k + 1] = run;
-            run += counts[base + k];
-        }
+        if (base + k < n_cells) cell_start[base + k + 1] = run;
+        run += v[k];
     }
     if (threadIdx.x == 0) cell_start[0] = 0;
 }
