@@ -213,6 +213,8 @@ class GraphMaintainer:
     """The step of :class:`Maintainer` captured in CUDA graphs (small N is launch-bound: ~20 short
     kernels per step).  Two graphs per ping-pong parity: A = A0, A4, A6+A7, A5, A2+A3 and B = the
     all-pairs certification, so that the dominant kernel can still be bracketed by CUDA events.
+    Inside A the repair path (A0, A4, A6+A7, A5 on the grid resident at p) and the rebuild path
+    (A2+A3 of p' into a second grid) are independent and run on two streams.
 
     Device pointers are fixed: positions live in two library-side buffers (the caller's p_next is
     copied in, 4 d N bytes), certificates ping-pong between two buffers.  Every point is treated as
@@ -226,6 +228,10 @@ class GraphMaintainer:
         assert int(p0.shape[0]) <= self.MAX_N, "GraphMaintainer is for launch-bound (small) problems"
         self.m = Maintainer(p0, occ)
         self.N = self.m.N
+        # two grids: the repair path updates the one resident at p while the rebuild path builds
+        # the other at p' on a second stream (fork / join inside graph A); next step they swap
+        self.grid = [self.m.grid, kc.Grid(self.N, self.m.geom)]
+        self.side = torch.cuda.Stream(device=p0.device)
         self.pos = [p0.clone(), torch.empty_like(p0)]
         self.cert = [self.m.certs, self.m.other]
         self.k = 0
@@ -236,11 +242,15 @@ class GraphMaintainer:
     def _body_a(self, k):
         m, cur, nxt = self.m, self.pos[k], self.pos[1 - k]
         certs, other = self.cert[k], self.cert[1 - k]
-        kc.kc_max_displacement(cur, nxt, m.eps)
+        main = torch.cuda.current_stream()
+        self.side.wait_stream(main)
+        with torch.cuda.stream(self.side):                 # rebuild path: needs only p'
+            kc.kc_cert_grid_rebuild(self.grid[1 - k], nxt, other)
+        kc.kc_max_displacement(cur, nxt, m.eps)            # repair path, on the grid resident at p
         kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
-        kc.kc_frontier_repair(m.grid, nxt, m.F, m.nF, certs, nF_max=self.N)
-        kc.kc_frontier_entropy(m.grid, m.F, m.nF, nF_max=self.N, out=(m.H, m.m, m.C))
-        kc.kc_cert_grid_rebuild(m.grid, nxt, other)
+        kc.kc_frontier_repair(self.grid[k], nxt, m.F, m.nF, certs, nF_max=self.N)
+        kc.kc_frontier_entropy(self.grid[k], m.F, m.nF, nF_max=self.N, out=(m.H, m.m, m.C))
+        main.wait_stream(self.side)
 
     def _body_b(self, k):
         m = self.m
