@@ -716,8 +716,8 @@ __device__ __forceinline__ void coop_range(const View &v, int lane, int b, int e
         int j;
         if (D == 2) {
             const float2 c = v.spos2[t];
+            j = v.sidx[t];                         // issued with the position: one round trip
             s = sqd2(qx, qy, c.x, c.y);
-            j = s <= thr ? v.sidx[t] : -1;
         } else {
             const float4 c = v.spos4[t];
             s = sqd3(qx, qy, qz, c.x, c.y, c.z);
@@ -974,15 +974,26 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
                       thr, KC_NOIDX, KC_NOIDX, tmp);
     }
     if (len <= 16)
-        for (int t = b; t < b + len; ++t) {
-            if (D == 2) {
-                const float2 c = v.spos2[t];
-                const float s = sqd2(qx, qy, c.x, c.y);
-                lane_offer<D>(tmp, s, s <= thr ? v.sidx[t] : -1, thr, self);
-            } else {
-                const float4 c = v.spos4[t];
-                lane_offer<D>(tmp, sqd3(qx, qy, qz, c.x, c.y, c.z), __float_as_int(c.w), thr, self);
+        for (int t0 = b; t0 < b + len; t0 += 4) {        // 4 records per round trip, loads issued together
+            const float qnan = __int_as_float(0x7fc00000);
+            float4 c[4];
+            int j[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const bool ok = t0 + k < b + len;
+                if (D == 2) {
+                    const float2 r = ok ? v.spos2[t0 + k] : make_float2(qnan, qnan);
+                    c[k] = make_float4(r.x, r.y, 0.f, 0.f);
+                    j[k] = ok ? v.sidx[t0 + k] : -1;
+                } else {
+                    c[k] = ok ? v.spos4[t0 + k] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
+                    j[k] = __float_as_int(c[k].w);
+                }
             }
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+                lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, c[k].x, c[k].y) : sqd3(qx, qy, qz, c[k].x, c[k].y, c[k].z),
+                              j[k], thr, self);
         }
     if (need)
         for (int c = hd; c >= 0; c = v.next[c]) {
