@@ -230,6 +230,16 @@ kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const in
                              const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
                              float *d1, float *d2, float *c, void *stream);
 
+/* The two halves of kc_frontier_repair as separate calls (rows A6 and A7): kc_grid_update brings the
+ * resident grid to positions p_new (movers as above); kc_frontier_search re-searches the ids in F
+ * against the grid as it stands and updates the certificates in place at those ids.  After the
+ * update, kc_frontier_entropy and kc_frontier_search touch disjoint state and may run on two streams. */
+kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
+                         const int32_t *n_movers, int64_t n_movers_max, void *stream);
+kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const int32_t *F, const int32_t *nF,
+                             int64_t nF_max, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
+                             void *stream);
+
 /* ---- inspection (tests, reports) ---------------------------------------------------------- */
 /* Synchronises `stream`, copies the device counters to *out (host). */
 kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream);

@@ -25,7 +25,7 @@ EXPORTS = (
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
+    "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
     "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
@@ -91,6 +91,8 @@ def lib():
     L.kc_frontier_classify.argtypes = [vp, i64, vp, vp, vp, vp, vp]
     L.kc_frontier_entropy.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp]
     L.kc_frontier_repair.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    L.kc_grid_update.argtypes = [vp, vp, i64, vp, vp, i64, vp]
+    L.kc_frontier_search.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp, vp, vp, vp, vp]
     L.kc_failure_audit.argtypes = [vp, vp, vp, i64, vp, vp, vp]
     L.kc_frontier_classify_clock.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp]
     L.kc_clock_stamp.argtypes = [vp, vp, i64, i64, vp, vp, vp]
@@ -346,6 +348,28 @@ def kc_frontier_repair(grid: Grid, p_new, F, nF, certs: Certs, movers=None, n_mo
                                     _ptr(n_movers, torch.int32, "n_movers"), n_movers_max,
                                     _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
                                     *certs._ptrs(), _stream()), "kc_frontier_repair")
+    return certs
+
+
+def kc_grid_update(grid: Grid, p_new, movers=None, n_movers=None, n_movers_max=None):
+    """A6, Algorithm 1 line 3: bring the resident grid to positions p_new."""
+    pp, N, d = _pos(p_new, "p_new")
+    if movers is not None:
+        n_movers_max = int(movers.numel() if n_movers_max is None else n_movers_max)
+        if n_movers is None:
+            n_movers = torch.tensor([movers.numel()], dtype=torch.int32, device=p_new.device)
+    else:
+        n_movers_max = 0
+    _check(lib().kc_grid_update(grid._h, pp, N, _ptr(movers, torch.int32, "movers"),
+                                _ptr(n_movers, torch.int32, "n_movers"), n_movers_max, _stream()), "kc_grid_update")
+
+
+def kc_frontier_search(grid: Grid, p_new, F, nF, certs: Certs, nF_max=None) -> Certs:
+    """A7, Algorithm 1 lines 4-7: re-search the ids in F, in place."""
+    pp, N, d = _pos(p_new, "p_new")
+    nF_max = int(F.numel() if nF_max is None else nF_max)
+    _check(lib().kc_frontier_search(grid._h, pp, N, _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
+                                    *certs._ptrs(), _stream()), "kc_frontier_search")
     return certs
 
 

@@ -1530,19 +1530,17 @@ extern "C" kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int
     return KC_OK;
 }
 
-extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
-                                        const int32_t *n_movers, int64_t n_movers_max, const int32_t *F,
-                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
-                                        float *d1, float *d2, float *c, void *stream)
+// A6, Algorithm 1 line 3: unlink every chain, refresh positions / re-file cell
+// changers, link again.
+extern "C" kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
+                                    const int32_t *n_movers, int64_t n_movers_max, void *stream)
 {
-    if (!g || !p_new || !F || !nF || nF_max < 0 || (movers && (!n_movers || n_movers_max < 0))) {
-        set_error("kc_frontier_repair: bad argument");
+    if (!g || !p_new || (movers && (!n_movers || n_movers_max < 0))) {
+        set_error("kc_grid_update: bad argument");
         return KC_EINVAL;
     }
-    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_repair");
-    if (s != KC_OK) return s;
     if (!g->built || N != g->N) {
-        set_error("kc_frontier_repair: grid not built for this N");
+        set_error("kc_grid_update: grid not built for this N");
         return KC_EREBUILD;
     }
     cudaStream_t st = (cudaStream_t)stream;
@@ -1550,9 +1548,8 @@ extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t 
     const int n = (int)N;
     const int64_t nm = movers ? n_movers_max : N;
     const int chain_blocks = blocks_for(g->dirty ? N : 1, 256, 148 * 4);
-    // line 3: unlink every chain, refresh positions / re-file cell changers, link again
     if (g->dirty) clear_chains_kernel<<<chain_blocks, 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
-    count_launches((g->dirty ? 1 : 0) + (nm > 0 ? 1 : 0) + 1 + (nF_max > 0 ? 1 : 0));
+    count_launches((g->dirty ? 1 : 0) + (nm > 0 ? 1 : 0) + 1);
     if (nm > 0) {
         int blocks = blocks_for(nm, 256, 148 * 16);
         if (g->geom.d == 2)
@@ -1564,34 +1561,72 @@ extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t 
     }
     link_chains_kernel<<<blocks_for(nm > 0 || g->dirty ? N : 1, 256, 148 * 4), 256, 0, st>>>(g->mlist, g->cell, g->head, g->next, g->ctr);
     g->dirty = 1;
-    // lines 4-7: re-search the frontier only.  On a large grid a frontier of at least N / sweep_div
-    // points (decided on the device from *nF) is served in slot order by the tiled sweep, anything
-    // else straight from the id list (one warp per query while the list is short: latency; one
-    // thread per query when it is long: throughput); both kernels are launched when the host
-    // bound allows either.
-    if (nF_max > 0) {
-        static const int div_env = getenv("KC_SWEEP_DIV") ? atoi(getenv("KC_SWEEP_DIV")) : 8;
-        static const int min_env = getenv("KC_SWEEP_MIN_N") ? atoi(getenv("KC_SWEEP_MIN_N")) : 200000;
-        const int sweep_div = N >= min_env && nF_max * (int64_t)div_env >= N ? div_env : 0;
-        const int tb = 32 * WT_WARPS;
-        if (sweep_div > 0) {
-            ++g->epoch;
-            mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
-            if (g->geom.d == 2)
-                search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-            else
-                search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-            count_launches(2);
-        }
-        int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
-        if (nF_max > v.wpq_max) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
-        if (g->geom.d == 2)
-            search_wpq_kernel<2, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
-        else
-            search_wpq_kernel<3, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
-    }
-    KC_LAUNCH_CHECK("kc_frontier_repair");
+    KC_LAUNCH_CHECK("kc_grid_update");
     return KC_OK;
+}
+
+// A7, Algorithm 1 lines 4-7: re-search the frontier only.  On a large grid a
+// frontier of at least N / sweep_div points (decided on the device from *nF) is served in slot
+// order by the tiled sweep, anything else straight from the id list (one warp per query while the
+// list is short: latency; one thread per query when it is long: throughput); both kernels are
+// launched when the host bound allows either.
+extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const int32_t *F,
+                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
+                                        float *d1, float *d2, float *c, void *stream)
+{
+    if (!g || !p_new || !F || !nF || nF_max < 0) {
+        set_error("kc_frontier_search: bad argument");
+        return KC_EINVAL;
+    }
+    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_search");
+    if (s != KC_OK) return s;
+    if (!g->built || N != g->N) {
+        set_error("kc_frontier_search: grid not built for this N");
+        return KC_EREBUILD;
+    }
+    if (nF_max == 0) return KC_OK;
+    cudaStream_t st = (cudaStream_t)stream;
+    View v = make_view(g);
+    const int n = (int)N;
+    static const int div_env = getenv("KC_SWEEP_DIV") ? atoi(getenv("KC_SWEEP_DIV")) : 8;
+    static const int min_env = getenv("KC_SWEEP_MIN_N") ? atoi(getenv("KC_SWEEP_MIN_N")) : 200000;
+    const int sweep_div = N >= min_env && nF_max * (int64_t)div_env >= N ? div_env : 0;
+    const int tb = 32 * WT_WARPS;
+    if (sweep_div > 0) {
+        ++g->epoch;
+        mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
+        if (g->geom.d == 2)
+            search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+        else
+            search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+        count_launches(2);
+    }
+    int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
+    if (nF_max > v.wpq_max) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
+    if (g->geom.d == 2)
+        search_wpq_kernel<2, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
+    else
+        search_wpq_kernel<3, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
+    count_launches(1);
+    KC_LAUNCH_CHECK("kc_frontier_search");
+    return KC_OK;
+}
+
+// A6 + A7 in one call.
+extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
+                                        const int32_t *n_movers, int64_t n_movers_max, const int32_t *F,
+                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
+                                        float *d1, float *d2, float *c, void *stream)
+{
+    if (!F || !nF || nF_max < 0) {
+        set_error("kc_frontier_repair: bad argument");
+        return KC_EINVAL;
+    }
+    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_repair");
+    if (s != KC_OK) return s;
+    s = kc_grid_update(g, p_new, N, movers, n_movers, n_movers_max, stream);
+    if (s != KC_OK) return s;
+    return kc_frontier_search(g, p_new, N, F, nF, nF_max, nn, nn2, d1, d2, c, stream);
 }
 
 extern "C" kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream)

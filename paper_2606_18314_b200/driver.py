@@ -232,6 +232,7 @@ class GraphMaintainer:
         # the other at p' on a second stream (fork / join inside graph A); next step they swap
         self.grid = [self.m.grid, kc.Grid(self.N, self.m.geom)]
         self.side = torch.cuda.Stream(device=p0.device)
+        self.side2 = torch.cuda.Stream(device=p0.device)
         self.pos = [p0.clone(), torch.empty_like(p0)]
         self.cert = [self.m.certs, self.m.other]
         self.k = 0
@@ -248,8 +249,12 @@ class GraphMaintainer:
             kc.kc_cert_grid_rebuild(self.grid[1 - k], nxt, other)
         kc.kc_max_displacement(cur, nxt, m.eps)            # repair path, on the grid resident at p
         kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
-        kc.kc_frontier_repair(self.grid[k], nxt, m.F, m.nF, certs, nF_max=self.N)
-        kc.kc_frontier_entropy(self.grid[k], m.F, m.nF, nF_max=self.N, out=(m.H, m.m, m.C))
+        kc.kc_grid_update(self.grid[k], nxt)
+        self.side2.wait_stream(main)
+        with torch.cuda.stream(self.side2):                # A5 and A7 touch disjoint state
+            kc.kc_frontier_entropy(self.grid[k], m.F, m.nF, nF_max=self.N, out=(m.H, m.m, m.C))
+        kc.kc_frontier_search(self.grid[k], nxt, m.F, m.nF, certs, nF_max=self.N)
+        main.wait_stream(self.side2)
         main.wait_stream(self.side)
 
     def _body_b(self, k):
