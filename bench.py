@@ -227,7 +227,8 @@ def run_gpu_arm(args):
     # (everything but all-pairs | all-pairs, so that the dominant kernel is still bracketed by
     # events); --no-graph issues the same calls eagerly
     use_graph = (not args.no_graph) and N <= GraphMaintainer.MAX_N
-    maint = {f: (GraphMaintainer if use_graph else Maintainer)(dev_traj[f][0]) for f in fams}
+    ov = bool(int(os.environ.get('KC_BENCH_OVERLAP', '1')))     # all-pairs graph beside graph A
+    maint = {f: (GraphMaintainer(dev_traj[f][0], overlap_allpairs=ov) if use_graph else Maintainer(dev_traj[f][0])) for f in fams}
     torch.cuda.synchronize()
 
     def do_step(f, t, timed):
@@ -349,6 +350,12 @@ def run_gpu_arm(args):
         # ---- roofline of the dominant kernel (all-pairs; FP32 ALU bound) ----
         ops_per_pair = 5 if d == 2 else 8
         ap_ms = ap_ms_sum / K                      # live CUDA events around the kernel's launch, timed region
+        ap_alone_ms = None
+        if use_graph:                              # the same graph with nothing beside it, for comparison
+            gm0 = maint[fams[0]]
+            gb = gm0.graphs[gm0.k][1] if gm0.graphs[gm0.k] is not None else None
+            if gb is not None:
+                ap_alone_ms = _median_ms(torch, gb.replay, 9, flush=flush)
         achieved = N * (N - 1) * ops_per_pair / (ap_ms * 1e-3) / 1e12
         sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
         peak = FP32_LANES * sm_max * 1e6 / 1e12
@@ -359,7 +366,10 @@ def run_gpu_arm(args):
                               f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md); measured non-fused "
                               f"FADD/FMUL chain rate {probe:.2f} Top/s; kernel share of step = "
                               f"{ap_ms / (dev_ms_max / K):.2f}"),
-                        pairs_per_s=N * (N - 1) / (ap_ms * 1e-3), ms_per_launch=ap_ms, fp32_probe_tops=probe)
+                        pairs_per_s=N * (N - 1) / (ap_ms * 1e-3), ms_per_launch=ap_ms, fp32_probe_tops=probe,
+                        # the same launch with the GPU to itself (the timed one shares it with graph A)
+                        ms_per_launch_alone=ap_alone_ms,
+                        frac_alone=None if not ap_alone_ms else N * (N - 1) * ops_per_pair / (ap_alone_ms * 1e-3) / 1e12 / peak)
         cpu = run_oracle_arm(cfg, K=30, W=0, time_budget_s=25.0)
         cpu_baseline = dict(value=cpu["value"], unit=UNIT, cores=cpu["cores"], kind="oracle", sample=cpu["sample"],
                             ms_per_step=cpu["ms_per_step"])
@@ -385,7 +395,8 @@ def run_gpu_arm(args):
                                    f"(A1 = the full N(N-1)-pair pass, started from the kinetic bound d2+2eps of the "
                                    f"maintained certificates, kc_cert_allpairs_bounded)",
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
-                       "launch": ("two CUDA graphs per step (all rows but A1 | A1), replayed; all-pairs bracketed by events"
+                       "launch": ("CUDA graphs per step (A0 + bound snapshot | all other rows | A1), replayed; A1 on its own "
+                                  "stream beside the other rows, bracketed by events"
                                   if use_graph else "eager stream launches"),
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
                        "certified": certified},

@@ -213,6 +213,9 @@ class GraphMaintainer:
     """The step of :class:`Maintainer` captured in CUDA graphs (small N is launch-bound: ~20 short
     kernels per step).  Two graphs per ping-pong parity: A = A0, A4, A6+A7, A5, A2+A3 and B = the
     all-pairs certification, so that the dominant kernel can still be bracketed by CUDA events.
+    B needs only p', eps_t and a bound on the old second-neighbour distances, so (overlap_allpairs)
+    it is launched on its own stream right after a small graph 0 = {snapshot of d2, A0} and runs
+    beside A; the short latency-bound kernels of A fill the issue slots the N x N pass leaves free.
     Inside A the repair path (A0, A4, A6+A7, A5 on the grid resident at p) and the rebuild path
     (A2+A3 of p' into a second grid) are independent and run on two streams.
 
@@ -224,8 +227,11 @@ class GraphMaintainer:
 
     MAX_N = 199_999
 
-    def __init__(self, p0: torch.Tensor, occ: float = 2.0):
+    def __init__(self, p0: torch.Tensor, occ: float = 2.0, overlap_allpairs: bool = True):
         assert int(p0.shape[0]) <= self.MAX_N, "GraphMaintainer is for launch-bound (small) problems"
+        # overlap_allpairs: graph B starts as soon as eps_t is known (bound = a snapshot of the
+        # pre-step d2, equally valid) and runs beside graph A on its own stream
+        self.overlap = bool(overlap_allpairs)
         self.m = Maintainer(p0, occ)
         self.N = self.m.N
         # two grids: the repair path updates the one resident at p while the rebuild path builds
@@ -233,6 +239,8 @@ class GraphMaintainer:
         self.grid = [self.m.grid, kc.Grid(self.N, self.m.geom)]
         self.side = torch.cuda.Stream(device=p0.device)
         self.side2 = torch.cuda.Stream(device=p0.device)
+        self.side_ap = torch.cuda.Stream(device=p0.device)
+        self.bound = torch.empty(int(p0.shape[0]), dtype=torch.float32, device=p0.device)
         self.pos = [p0.clone(), torch.empty_like(p0)]
         self.cert = [self.m.certs, self.m.other]
         self.k = 0
@@ -247,7 +255,8 @@ class GraphMaintainer:
         self.side.wait_stream(main)
         with torch.cuda.stream(self.side):                 # rebuild path: needs only p'
             kc.kc_cert_grid_rebuild(self.grid[1 - k], nxt, other)
-        kc.kc_max_displacement(cur, nxt, m.eps)            # repair path, on the grid resident at p
+        if not self.overlap:
+            kc.kc_max_displacement(cur, nxt, m.eps)        # repair path, on the grid resident at p
         kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
         kc.kc_grid_update(self.grid[k], nxt)
         self.side2.wait_stream(main)
@@ -257,18 +266,27 @@ class GraphMaintainer:
         main.wait_stream(self.side2)
         main.wait_stream(self.side)
 
+    def _body_0(self, k):
+        self.bound.copy_(self.cert[k].d2)
+        kc.kc_max_displacement(self.pos[k], self.pos[1 - k], self.m.eps)
+
     def _body_b(self, k):
         m = self.m
-        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=self.cert[k].d2, eps=m.eps)
+        bound = self.bound if self.overlap else self.cert[k].d2
+        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=bound, eps=m.eps)
 
     def _capture(self, k):
         n0 = kc.kc_launch_count()
-        ga, gb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+        ga, gb, g0 = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph(), None
+        if self.overlap:
+            g0 = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g0):
+                self._body_0(k)
         with torch.cuda.graph(ga):
             self._body_a(k)
         with torch.cuda.graph(gb):
             self._body_b(k)
-        self.graphs[k] = (ga, gb)
+        self.graphs[k] = (ga, gb, g0)
         self.launches[k] = kc.kc_launch_count() - n0
 
     def step(self, p_next: torch.Tensor, time_allpairs: bool = False) -> StepResult:
@@ -279,17 +297,34 @@ class GraphMaintainer:
         if self.graphs[k] is None:
             torch.cuda.synchronize()
             self._capture(k)
-        ga, gb = self.graphs[k]
-        ga.replay()
-        if time_allpairs:
-            e0 = torch.cuda.Event(enable_timing=True)
-            e1 = torch.cuda.Event(enable_timing=True)
-            e0.record()
-            gb.replay()
-            e1.record()
-            self.ap_events = (e0, e1)
+        ga, gb, g0 = self.graphs[k]
+        main = torch.cuda.current_stream()
+        if self.overlap:
+            g0.replay()
+            self.side_ap.wait_stream(main)
+            with torch.cuda.stream(self.side_ap):
+                if time_allpairs:
+                    e0 = torch.cuda.Event(enable_timing=True)
+                    e1 = torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    gb.replay()
+                    e1.record()
+                    self.ap_events = (e0, e1)
+                else:
+                    gb.replay()
+            ga.replay()
+            main.wait_stream(self.side_ap)
         else:
-            gb.replay()
+            ga.replay()
+            if time_allpairs:
+                e0 = torch.cuda.Event(enable_timing=True)
+                e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                gb.replay()
+                e1.record()
+                self.ap_events = (e0, e1)
+            else:
+                gb.replay()
         self.k = 1 - k
         return StepResult(m.eps, m.nF, m.H, m.m, m.C, self.cert[k], self.cert[1 - k], m.ap)
 

@@ -389,14 +389,15 @@ def test_local_motion_budget_frontier(cfg, fam):
     assert np.array_equal(got.nn, post.nn)                       # no missed failure
 
 
+@pytest.mark.parametrize("overlap", [True, False])
 @pytest.mark.parametrize("cfg,fam", [("cfg1", "walk"), ("cfg2", "walk"), ("cfg2", "local"), ("cfg3", "cluster_drift")])
-def test_graphed_step_matches_the_oracle(cfg, fam):
+def test_graphed_step_matches_the_oracle(cfg, fam, overlap):
     """The CUDA-graph form of the step (driver.GraphMaintainer): 5 replayed transitions, every
     output bit-exact against the oracle, and identical to the eager step."""
     from paper_2606_18314_b200.driver import GraphMaintainer, Maintainer
     p, mot = wl.make_scene(cfg, fam)
     g_or, _ = geoms(p)
-    gm, em = GraphMaintainer(dev(p)), Maintainer(dev(p))
+    gm, em = GraphMaintainer(dev(p), overlap_allpairs=overlap), Maintainer(dev(p))
     pre = oracle.bruteforce_top2(p)
     for step in range(5):
         q, movers = mot.step(p)
