@@ -26,6 +26,8 @@ namespace {
 
 constexpr int AP_TJ = 1024;   // candidates per shared-memory tile
 constexpr int AP_SEED = 256;  // points scanned by the seed pass of a j-split launch
+constexpr int AP_GRAN = 64;   // chunk granularity of a j-split launch (a multiple of every step size 4*C4)
+constexpr int AP_RESIDENT = 10;   // CTAs of 128 threads an SM holds at the kernel's ~48 registers per thread
 
 struct Partial { float s1, s2; int j1, j2; };   // 16 B
 
@@ -67,12 +69,12 @@ __device__ __forceinline__ void unpack2(u64 v, float &lo, float &hi)
 }
 
 template <int D, int THREADS>
-__device__ __forceinline__ void load_tile(const float *__restrict__ p, int64_t N, int64_t j0,
+__device__ __forceinline__ void load_tile(const float *__restrict__ p, int64_t N, int64_t j0, int tl,
                                           float *sx, float *sy, float *sz)
 {
     // pad the tail with +inf: s = +inf never beats a finite second-best, and the slow path
     // rejects j >= N explicitly while second-best is still +inf.
-    for (int t = threadIdx.x; t < AP_TJ; t += THREADS) {
+    for (int t = threadIdx.x; t < tl; t += THREADS) {
         int64_t j = j0 + t;
         float x = CUDART_INF_F, y = CUDART_INF_F, z = CUDART_INF_F;
         if (j < N) {
@@ -117,11 +119,13 @@ __device__ __forceinline__ void scan_chunk(const float *__restrict__ p, int64_t 
         qx2[k] = pack2(qx[k], qx[k]); qy2[k] = pack2(qy[k], qy[k]); qz2[k] = pack2(qz[k], qz[k]);
     }
     for (int64_t j0 = jbeg; j0 < jend; j0 += AP_TJ) {
+        // the chunk's last tile may be short: only whole steps of it are staged and evaluated
+        const int tl = (int)min((int64_t)AP_TJ, (jend - j0 + 4 * C4 - 1) / (4 * C4) * (4 * C4));
         __syncthreads();
-        load_tile<D, THREADS>(p, lim, j0, sx, sy, sz);
+        load_tile<D, THREADS>(p, lim, j0, tl, sx, sy, sz);
         __syncthreads();
 #pragma unroll 1
-        for (int t = 0; t < AP_TJ; t += 4 * C4) {
+        for (int t = 0; t < tl; t += 4 * C4) {
             u64 sa[QPT][C4], sb[QPT][C4];
             float m[QPT][C4];
 #pragma unroll
@@ -390,12 +394,15 @@ Shape choose_shape(int64_t nq, int64_t N)
     s.c4 = s.qpt == 4 ? 2 : (s.qpt == 2 ? 2 : 4);
     if (e_c4 == 1 || e_c4 == 2 || e_c4 == 4) s.c4 = e_c4;
     if (e_thr == 32 || e_thr == 64 || e_thr == 128) s.threads = e_thr;
-    // j-split: many waves deep; chunks are whole tiles and start from the seed pass (or from the
-    // caller's bound), so one tile per chunk is enough
+    // j-split (chunks start from the seed pass or from the caller's bound, so short chunks are
+    // fine; granularity AP_GRAN candidates, at least 4 units per chunk).  Few query blocks: as many
+    // chunks as make ONE full wave of resident CTAs (a second, partly filled wave of this
+    // latency-bound kernel would cost as much as a full one).  Many query blocks: many waves deep.
     int64_t per = (int64_t)s.qpt * s.threads;
     int64_t itiles = (nq + per - 1) / per;
-    int64_t want = (148 * 8 * 8 + itiles - 1) / itiles;
-    int64_t cap = (N - AP_SEED + AP_TJ - 1) / AP_TJ;
+    const int64_t resident = 148 * (int64_t)AP_RESIDENT;
+    int64_t want = itiles * 2 <= resident ? resident / itiles : (148 * 8 * 8 + itiles - 1) / itiles;
+    int64_t cap = (N - AP_SEED) / (4 * AP_GRAN);
     int64_t js = want < cap ? want : cap;
     if (e_js > 0) js = e_js;
     if (js < 1) js = 1;
@@ -443,11 +450,10 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     int js = sh.js;
     int64_t jchunk;
     if (split) {
-        // whole tiles per chunk (a tile is evaluated in full, +inf padding included): as many
-        // chunks as the shape wants, but never a chunk of less than one tile
-        const int64_t tiles = (a.N - a.jfirst + AP_TJ - 1) / AP_TJ;
-        const int64_t want = js < tiles ? js : tiles;
-        jchunk = (tiles + want - 1) / want * AP_TJ;
+        // equal chunks of whole AP_GRAN units, as many as the shape wants
+        const int64_t units = (a.N - a.jfirst + AP_GRAN - 1) / AP_GRAN;
+        const int64_t want = js < units ? js : units;
+        jchunk = (units + want - 1) / want * AP_GRAN;
     } else {
         jchunk = (a.N + 15) / 16 * 16;
     }
