@@ -316,12 +316,12 @@ def run_gpu_arm(args):
             e0 = torch.cuda.Event(enable_timing=True)
             e1 = torch.cuda.Event(enable_timing=True)
             e0.record()
-            buf = bufs[k & 1]
+            buf = m.next_buffer() if use_graph else bufs[k & 1]
             k += 1
             buf.copy_(host_next[f][base + t + 1], non_blocking=True)
             mv = traj[f][1][base + t + 1]
             mvd = None if mv is None else torch.from_numpy(mv).to(dev, non_blocking=True)
-            res = m.step(buf) if use_graph else m.step(buf, movers=mvd)
+            res = m.step(None) if use_graph else m.step(buf, movers=mvd)
             host_out["nn"].copy_(res.rebuilt.nn, non_blocking=True)
             host_out["d1"].copy_(res.rebuilt.d1, non_blocking=True)
             host_out["d2"].copy_(res.rebuilt.d2, non_blocking=True)
@@ -353,7 +353,7 @@ def run_gpu_arm(args):
         ap_alone_ms = None
         if use_graph:                              # the same graph with nothing beside it, for comparison
             gm0 = maint[fams[0]]
-            gb = gm0.graphs[gm0.k][1] if gm0.graphs[gm0.k] is not None else None
+            gb = gm0.graphs[gm0.k][2] if gm0.graphs[gm0.k] is not None else None
             if gb is not None:
                 ap_alone_ms = _median_ms(torch, gb.replay, 9, flush=flush)
         achieved = N * (N - 1) * ops_per_pair / (ap_ms * 1e-3) / 1e12
@@ -395,7 +395,7 @@ def run_gpu_arm(args):
                                    f"(A1 = the full N(N-1)-pair pass, started from the kinetic bound d2+2eps of the "
                                    f"maintained certificates, kc_cert_allpairs_bounded)",
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
-                       "launch": ("CUDA graphs per step (A0 + bound snapshot | all other rows | A1), replayed; A1 on its own "
+                       "launch": ("CUDA graphs per step (all rows but A1 | A0 again | A1), replayed; A1 on its own "
                                   "stream beside the other rows, bracketed by events"
                                   if use_graph else "eager stream launches"),
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",

@@ -27,7 +27,7 @@ namespace {
 constexpr int AP_TJ = 1024;   // candidates per shared-memory tile
 constexpr int AP_SEED = 256;  // points scanned by the seed pass of a j-split launch
 constexpr int AP_GRAN = 64;   // chunk granularity of a j-split launch (a multiple of every step size 4*C4)
-constexpr int AP_RESIDENT = 10;   // CTAs of 128 threads an SM holds at the kernel's ~48 registers per thread
+constexpr int AP_RESIDENT = 12;   // CTAs of 128 threads an SM holds at the kernel's ~48 registers per thread
 
 struct Partial { float s1, s2; int j1, j2; };   // 16 B
 
@@ -191,7 +191,7 @@ struct ApArgs {
 
 // grid = (ceil(nq / (QPT*THREADS)), JS).
 template <int D, int QPT, int C4, int THREADS>
-__global__ void __launch_bounds__(THREADS)
+__global__ void __launch_bounds__(THREADS, (QPT == 1 && THREADS == 128) ? 12 : 1)
 allpairs_kernel(const ApArgs a)
 {
     __shared__ __align__(16) float sx[AP_TJ];

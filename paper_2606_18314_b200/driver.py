@@ -211,38 +211,39 @@ class ClockMaintainer:
 
 class GraphMaintainer:
     """The step of :class:`Maintainer` captured in CUDA graphs (small N is launch-bound: ~20 short
-    kernels per step).  Two graphs per ping-pong parity: A = A0, A4, A6+A7, A5, A2+A3 and B = the
-    all-pairs certification, so that the dominant kernel can still be bracketed by CUDA events.
-    B needs only p', eps_t and a bound on the old second-neighbour distances, so (overlap_allpairs)
-    it is launched on its own stream right after a small graph 0 = {snapshot of d2, A0} and runs
-    beside A; the short latency-bound kernels of A fill the issue slots the N x N pass leaves free.
-    Inside A the repair path (A0, A4, A6+A7, A5 on the grid resident at p) and the rebuild path
-    (A2+A3 of p' into a second grid) are independent and run on two streams.
+    kernels per step).  Per ping-pong parity:
+      graph A  = A0, A4, A6, A7 || A5 on the grid resident at p, beside them (second stream, fork /
+                 join inside the graph) A2+A3 of p' into a second grid, then a snapshot of the new d2
+                 as the NEXT step's all-pairs bound;
+      graph B0 = A0 once more into a buffer of its own, graph B = the all-pairs certification of p'
+                 from that eps_t and the snapshot taken by the previous step.
+    B0 + B depend on nothing A computes, so (overlap_allpairs) they run on their own stream beside A,
+    B still bracketed by CUDA events; the short latency-bound kernels of A fill the issue slots the
+    N x N pass leaves free.  With overlap_allpairs=False B is replayed after A on the same stream.
 
     Device pointers are fixed: positions live in two library-side buffers (the caller's p_next is
-    copied in, 4 d N bytes), certificates ping-pong between two buffers.  Every point is treated as
-    a potential mover (no mover list: its length varies from step to step), which changes no
-    result.  Only for grids below the sweep threshold of kc_frontier_repair (its epoch is a
+    copied in, 4 d N bytes), certificates and grids ping-pong.  Every point is treated as a
+    potential mover (no mover list: its length varies from step to step), which changes no
+    result.  Only for grids below the sweep threshold of kc_frontier_search (its epoch is a
     host-side counter); larger problems are not launch-bound and use :class:`Maintainer`."""
 
     MAX_N = 199_999
 
     def __init__(self, p0: torch.Tensor, occ: float = 2.0, overlap_allpairs: bool = True):
         assert int(p0.shape[0]) <= self.MAX_N, "GraphMaintainer is for launch-bound (small) problems"
-        # overlap_allpairs: graph B starts as soon as eps_t is known (bound = a snapshot of the
-        # pre-step d2, equally valid) and runs beside graph A on its own stream
         self.overlap = bool(overlap_allpairs)
         self.m = Maintainer(p0, occ)
         self.N = self.m.N
-        # two grids: the repair path updates the one resident at p while the rebuild path builds
-        # the other at p' on a second stream (fork / join inside graph A); next step they swap
+        dev = p0.device
         self.grid = [self.m.grid, kc.Grid(self.N, self.m.geom)]
-        self.side = torch.cuda.Stream(device=p0.device)
-        self.side2 = torch.cuda.Stream(device=p0.device)
-        self.side_ap = torch.cuda.Stream(device=p0.device)
-        self.bound = torch.empty(int(p0.shape[0]), dtype=torch.float32, device=p0.device)
+        self.side = torch.cuda.Stream(device=dev)
+        self.side2 = torch.cuda.Stream(device=dev)
+        self.side_ap = torch.cuda.Stream(device=dev)
         self.pos = [p0.clone(), torch.empty_like(p0)]
         self.cert = [self.m.certs, self.m.other]
+        # bound[k]: upper bounds on the second-neighbour distances at pos[k] (the exact d2 there)
+        self.bound = [self.cert[0].d2.clone(), torch.empty(self.N, dtype=torch.float32, device=dev)]
+        self.eps_b = torch.zeros(1, dtype=torch.float32, device=dev)
         self.k = 0
         self.graphs = [None, None]
         self.launches = [0, 0]
@@ -255,8 +256,8 @@ class GraphMaintainer:
         self.side.wait_stream(main)
         with torch.cuda.stream(self.side):                 # rebuild path: needs only p'
             kc.kc_cert_grid_rebuild(self.grid[1 - k], nxt, other)
-        if not self.overlap:
-            kc.kc_max_displacement(cur, nxt, m.eps)        # repair path, on the grid resident at p
+            self.bound[1 - k].copy_(other.d2)              # the next step's all-pairs bound
+        kc.kc_max_displacement(cur, nxt, m.eps)            # repair path, on the grid resident at p
         kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
         kc.kc_grid_update(self.grid[k], nxt)
         self.side2.wait_stream(main)
@@ -266,67 +267,64 @@ class GraphMaintainer:
         main.wait_stream(self.side2)
         main.wait_stream(self.side)
 
-    def _body_0(self, k):
-        self.bound.copy_(self.cert[k].d2)
-        kc.kc_max_displacement(self.pos[k], self.pos[1 - k], self.m.eps)
+    def _body_b0(self, k):
+        kc.kc_max_displacement(self.pos[k], self.pos[1 - k], self.eps_b)
 
     def _body_b(self, k):
         m = self.m
-        bound = self.bound if self.overlap else self.cert[k].d2
-        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=bound, eps=m.eps)
+        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=self.bound[k], eps=self.eps_b)
 
     def _capture(self, k):
         n0 = kc.kc_launch_count()
-        ga, gb, g0 = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph(), None
-        if self.overlap:
-            g0 = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g0):
-                self._body_0(k)
+        ga, gb0, gb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
         with torch.cuda.graph(ga):
             self._body_a(k)
+        with torch.cuda.graph(gb0):
+            self._body_b0(k)
         with torch.cuda.graph(gb):
             self._body_b(k)
-        self.graphs[k] = (ga, gb, g0)
+        self.graphs[k] = (ga, gb0, gb)
         self.launches[k] = kc.kc_launch_count() - n0
 
-    def step(self, p_next: torch.Tensor, time_allpairs: bool = False) -> StepResult:
+    def _replay_b(self, gb0, gb, timed):
+        gb0.replay()
+        if timed:
+            e0 = torch.cuda.Event(enable_timing=True)
+            e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            gb.replay()
+            e1.record()
+            self.ap_events = (e0, e1)
+        else:
+            gb.replay()
+
+    def step(self, p_next: torch.Tensor | None, time_allpairs: bool = False) -> StepResult:
         """One transition; returns the same StepResult as Maintainer.step (no host sync).  With
-        ``time_allpairs`` two CUDA events bracket the all-pairs graph (``self.ap_events``)."""
+        ``time_allpairs`` two CUDA events bracket the all-pairs graph (``self.ap_events``).
+        ``p_next`` None: the caller has already written the new positions into next_buffer()."""
         k, m = self.k, self.m
-        self.pos[1 - k].copy_(p_next, non_blocking=True)
+        if p_next is not None:
+            self.pos[1 - k].copy_(p_next, non_blocking=True)
         if self.graphs[k] is None:
             torch.cuda.synchronize()
             self._capture(k)
-        ga, gb, g0 = self.graphs[k]
+        ga, gb0, gb = self.graphs[k]
         main = torch.cuda.current_stream()
         if self.overlap:
-            g0.replay()
             self.side_ap.wait_stream(main)
             with torch.cuda.stream(self.side_ap):
-                if time_allpairs:
-                    e0 = torch.cuda.Event(enable_timing=True)
-                    e1 = torch.cuda.Event(enable_timing=True)
-                    e0.record()
-                    gb.replay()
-                    e1.record()
-                    self.ap_events = (e0, e1)
-                else:
-                    gb.replay()
+                self._replay_b(gb0, gb, time_allpairs)
             ga.replay()
             main.wait_stream(self.side_ap)
         else:
             ga.replay()
-            if time_allpairs:
-                e0 = torch.cuda.Event(enable_timing=True)
-                e1 = torch.cuda.Event(enable_timing=True)
-                e0.record()
-                gb.replay()
-                e1.record()
-                self.ap_events = (e0, e1)
-            else:
-                gb.replay()
+            self._replay_b(gb0, gb, time_allpairs)
         self.k = 1 - k
         return StepResult(m.eps, m.nF, m.H, m.m, m.C, self.cert[k], self.cert[1 - k], m.ap)
+
+    def next_buffer(self) -> torch.Tensor:
+        """The device buffer the next step reads p' from (for callers that upload straight into it)."""
+        return self.pos[1 - self.k]
 
     def launches_per_step(self, k=None):
         """Kernels of this library launched by one replayed step (counted at capture)."""
