@@ -68,6 +68,21 @@ def test_bad_arguments_are_rejected(L):
     assert L.kc_cert_allpairs(None, 100, 2, None, None, None, None, None, None, 0, None) == binding.KC_EINVAL
     assert L.kc_max_displacement(None, None, 10, 2, None, None) == binding.KC_EINVAL
     assert b"kc_max_displacement" in L.kc_last_error()
+    E = binding.KC_EINVAL
+    assert L.kc_cert_allpairs_bounded(None, 100, 2, None, None, None, None, None, None, None, None, 0, None) == E
+    assert L.kc_frontier_oracle(None, 100, 2, None, None, 5, None, None, None, None, None, None, 0, None) == E
+    assert L.kc_grid_build(None, None, 100, None) == E
+    assert L.kc_cert_grid_search(None, None, None, None, None, None, None) == E
+    assert L.kc_frontier_classify(None, 100, None, None, None, None, None) == E
+    assert L.kc_frontier_classify_clock(None, None, 100, None, None, None, None, None, None, None) == E
+    assert L.kc_frontier_classify_local(None, None, None, 100, None, None, None, None, None, None, None, None) == E
+    assert L.kc_clock_stamp(None, None, 0, 100, None, None, None) == E
+    assert L.kc_frontier_entropy(None, None, None, 10, None, None, None, None) == E
+    assert L.kc_grid_update(None, None, 100, None, None, 0, None) == E
+    assert L.kc_frontier_search(None, None, 100, None, None, 10, None, None, None, None, None, None) == E
+    assert L.kc_frontier_repair(None, None, 100, None, None, 0, None, None, 10, None, None, None, None, None, None) == E
+    assert L.kc_failure_audit(None, None, None, 100, None, None, None) == E
+    assert L.kc_grid_destroy(None) == binding.KC_OK and L.kc_grid_bytes(None) == 0
 
 
 def test_no_cpu_fallback_without_gpu(L):
