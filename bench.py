@@ -353,7 +353,7 @@ def run_gpu_arm(args):
         ap_alone_ms = None
         if use_graph:                              # the same graph with nothing beside it, for comparison
             gm0 = maint[fams[0]]
-            gb = gm0.graphs[gm0.k][2] if gm0.graphs[gm0.k] is not None else None
+            gb = gm0.graphs[gm0.k][1] if gm0.graphs[gm0.k] is not None else None
             if gb is not None:
                 ap_alone_ms = _median_ms(torch, gb.replay, 9, flush=flush)
         achieved = N * (N - 1) * ops_per_pair / (ap_ms * 1e-3) / 1e12
@@ -392,10 +392,10 @@ def run_gpu_arm(args):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{cfg}: N={N}, d={d}, eps={c['eps']}, families {','.join(fams)} "
                                    f"({'/'.join(map(str, per))} steps), grid occupancy 2, every step = A0,A4,A6+A7,A5,A2+A3,A1 "
-                                   f"(A1 = the full N(N-1)-pair pass, started from the kinetic bound d2+2eps of the "
-                                   f"maintained certificates, kc_cert_allpairs_bounded)",
+                                   f"(A1 = the full N(N-1)-pair pass, started from each point's previous two neighbours, "
+                                   f"kc_cert_allpairs_seeded)",
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
-                       "launch": ("CUDA graphs per step (all rows but A1 | A0 again | A1), replayed; A1 on its own "
+                       "launch": ("CUDA graphs per step (all rows but A1 | A1), replayed; A1 on its own "
                                   "stream beside the other rows, bracketed by events"
                                   if use_graph else "eager stream launches"),
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",

@@ -124,6 +124,19 @@ kc_status kc_cert_allpairs_bounded(const float *p, int64_t N, int d, const float
                                    const float *eps, int32_t *nn, int32_t *nn2, float *d1, float *d2,
                                    float *c, void *workspace, size_t workspace_bytes, void *stream);
 
+/* A1 started from two known points per query.  Two distinct points a, b other than i at squared
+ * distances s_a <= s_b (at the CURRENT positions p) prove that i's second neighbour is no farther
+ * than b, so the top-2 list (s_a, a), (s_b, b) is a valid start of the N x N pass: the same
+ * N(N-1) pairs are evaluated, only candidates that beat the list reach the insertion.  In a
+ * maintenance loop the natural seeds are the point's previous neighbours nn, nn2 (the certificate
+ * of Definition 1): after a small step they are still near, and unlike the kinetic
+ * bound no eps_t is needed.  seed1, seed2: device int32[N], ANY ids; an id that is out of range,
+ * equal to i or (for seed2) equal to seed1[i] is ignored, so the result never depends on the seeds.
+ * Output and workspace as kc_cert_allpairs. */
+kc_status kc_cert_allpairs_seeded(const float *p, int64_t N, int d, const int32_t *seed1,
+                                  const int32_t *seed2, int32_t *nn, int32_t *nn2, float *d1, float *d2,
+                                  float *c, void *workspace, size_t workspace_bytes, void *stream);
+
 /* ---- NEXT #1: frontier oracle (PAPER.md:69 rtx_frontier_oracle) -------------------------- */
 /* Relabel the queries q[0..*nq) (device int32, distinct ids; *nq read on the device, at most
  * nq_max) against ALL N points by tiled brute force, O(|q| N).  Results are written in place at

@@ -21,7 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libkc.so")
 
 EXPORTS = (
     "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_max_displacement",
-    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded",
+    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded", "kc_cert_allpairs_seeded",
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
@@ -78,6 +78,7 @@ def lib():
     L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
     L.kc_cert_allpairs.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
     L.kc_cert_allpairs_bounded.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.kc_cert_allpairs_seeded.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
     L.kc_frontier_oracle_workspace.restype = sz
     L.kc_frontier_oracle_workspace.argtypes = [i64, ci, i64]
     L.kc_frontier_oracle.argtypes = [vp, i64, ci, vp, vp, i64, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -216,16 +217,28 @@ def _workspace(nbytes, device):
     return w
 
 
-def kc_cert_allpairs(p, out: Certs | None = None, workspace=None, d2_prev=None, eps=None) -> Certs:
+def kc_cert_allpairs(p, out: Certs | None = None, workspace=None, d2_prev=None, eps=None,
+                     seed1=None, seed2=None) -> Certs:
     """A1: exact all-pairs certificates (Table 2).  With ``d2_prev`` (float32[N]) and
     ``eps`` (float32[1]) the pass starts from the kinetic bound d2_prev + 2 eps
-    (kc_cert_allpairs_bounded); the result is the same bits either way."""
+    (kc_cert_allpairs_bounded); with ``seed1``, ``seed2`` (int32[N], e.g. the previous nn, nn2) from
+    those two points (kc_cert_allpairs_seeded); the result is the same bits in every case."""
     pp, N, d = _pos(p)
     out = out or Certs.empty(N, p.device)
     need = lib().kc_cert_allpairs_workspace(N, d)
     ws = workspace if workspace is not None else _workspace(need, p.device)
     if (d2_prev is None) != (eps is None):
         raise ValueError("d2_prev and eps go together")
+    if (seed1 is None) != (seed2 is None):
+        raise ValueError("seed1 and seed2 go together")
+    if seed1 is not None:
+        if seed1.numel() != N or seed2.numel() != N:
+            raise ValueError("seeds must have N entries")
+        _check(lib().kc_cert_allpairs_seeded(pp, N, d, _ptr(seed1, torch.int32, "seed1"),
+                                             _ptr(seed2, torch.int32, "seed2"), *out._ptrs(), _ptr(ws),
+                                             ws.numel() if ws is not None else 0, _stream()),
+               "kc_cert_allpairs_seeded")
+        return out
     if d2_prev is None:
         _check(lib().kc_cert_allpairs(pp, N, d, *out._ptrs(), _ptr(ws), ws.numel() if ws is not None else 0,
                                       _stream()), "kc_cert_allpairs")

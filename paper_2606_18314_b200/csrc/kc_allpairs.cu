@@ -94,10 +94,11 @@ __device__ __forceinline__ void load_tile(const float *__restrict__ p, int64_t N
 __device__ __noinline__ Top2 slow_offer4(Top2 best, float s0, float s1, float s2, float s3, int j,
                                          int lim, int self)
 {
-    if (s0 <= best.s2 && j + 0 < lim && j + 0 != self) best.offer(s0, j + 0);
-    if (s1 <= best.s2 && j + 1 < lim && j + 1 != self) best.offer(s1, j + 1);
-    if (s2 <= best.s2 && j + 2 < lim && j + 2 != self) best.offer(s2, j + 2);
-    if (s3 <= best.s2 && j + 3 < lim && j + 3 != self) best.offer(s3, j + 3);
+    // ids already held are skipped: a list seeded from two known points meets them again
+    if (s0 <= best.s2 && j + 0 < lim && j + 0 != self && j + 0 != best.j1 && j + 0 != best.j2) best.offer(s0, j + 0);
+    if (s1 <= best.s2 && j + 1 < lim && j + 1 != self && j + 1 != best.j1 && j + 1 != best.j2) best.offer(s1, j + 1);
+    if (s2 <= best.s2 && j + 2 < lim && j + 2 != self && j + 2 != best.j1 && j + 2 != best.j2) best.offer(s2, j + 2);
+    if (s3 <= best.s2 && j + 3 < lim && j + 3 != self && j + 3 != best.j1 && j + 3 != best.j2) best.offer(s3, j + 3);
     return best;
 }
 
@@ -182,6 +183,7 @@ struct ApArgs {
     const Partial *seed;         // unbounded j-split: exact top-2 over points [0, jfirst)
     const float *bound_d2;       // kinetic bound (both or neither): every query's second neighbour is
     const float *bound_eps;      //   claimed to lie within bound_d2[i] + 2 * bound_eps[0]
+    const int32_t *seed1, *seed2;   // two known points per query (e.g. its previous neighbours), or null
     Partial *part;               // j-split: partial lists [js][nq_host]; null: store certificates
     int32_t *redo, *n_redo;      // queries whose bound admitted fewer than two candidates
     int32_t *tickets;            // j-split: chunks finished per query block (the last one merges)
@@ -331,6 +333,38 @@ allpairs_seed_kernel(const ApArgs a, int S, Partial *__restrict__ seed)
     }
 }
 
+// Seeds from two known points per query (kc_cert_allpairs_seeded): their exact keys at the
+// CURRENT positions.  Two distinct points other than i at squared distances s_a <= s_b prove
+// s2_i <= s_b, so the list (s_a, a), (s_b, b) is a valid start that nothing in the pass can
+// invalidate; ids that are out of range, equal to i or to each other are dropped (cold start).
+template <int D>
+__global__ void __launch_bounds__(256)
+allpairs_idseed_kernel(const ApArgs a, Partial *__restrict__ seed)
+{
+    const float *__restrict__ p = a.p;
+    const int64_t nq = a.nq_dev ? (int64_t)*a.nq_dev : a.nq_host;
+    const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (q >= nq) return;
+    const int i = a.qlist ? a.qlist[q] : (int)q;
+    const float qx = p[(int64_t)i * D], qy = p[(int64_t)i * D + 1];
+    const float qz = D == 3 ? p[(int64_t)i * D + 2] : 0.f;
+    Top2 t;
+    t.init();
+    const int ids[2] = {a.seed1[i], a.seed2[i]};
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const int j = ids[k];
+        if (j >= 0 && j < a.N && j != i && j != t.j1) {
+            const float s = D == 2 ? sqd2(qx, qy, p[(int64_t)j * D], p[(int64_t)j * D + 1])
+                                   : sqd3(qx, qy, qz, p[(int64_t)j * D], p[(int64_t)j * D + 1], p[(int64_t)j * D + 2]);
+            if (s == s) t.offer(s, j);         // a NaN coordinate seeds nothing
+        }
+    }
+    Partial o;
+    o.s1 = t.s1; o.s2 = t.s2; o.j1 = t.j1; o.j2 = t.j2;
+    seed[q] = o;
+}
+
 // Redo pass of a bounded launch: the queries whose bound admitted fewer than two candidates (a
 // bound that was not one) are recomputed from scratch, one CTA per query, so that the result
 // never depends on the bound.  Empty in normal operation.
@@ -412,7 +446,7 @@ Shape choose_shape(int64_t nq, int64_t N)
 }
 
 // Workspace layout: [n_redo: 16 B][tickets: one int32 per query block, padded to 16 B]
-// [redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last two only for a j-split
+// [redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last only for a j-split
 // shape).  n_redo and the tickets are zeroed by one memset per call.
 size_t pad16(size_t b) { return (b + 15) & ~(size_t)15; }
 size_t qblocks_for(int64_t nq, const Shape &sh)
@@ -423,8 +457,8 @@ size_t qblocks_for(int64_t nq, const Shape &sh)
 size_t head_bytes(int64_t nq, const Shape &sh) { return 16 + pad16(4 * qblocks_for(nq, sh)); }
 size_t workspace_bytes_for(int64_t nq, const Shape &sh)
 {
-    return head_bytes(nq, sh) + pad16((size_t)nq * 4) +
-           (sh.js > 1 ? ((size_t)sh.js + 1) * (size_t)nq * sizeof(Partial) : 0);
+    return head_bytes(nq, sh) + pad16((size_t)nq * 4) + (size_t)nq * sizeof(Partial) +
+           (sh.js > 1 ? (size_t)sh.js * (size_t)nq * sizeof(Partial) : 0);
 }
 
 template <int D, int QPT, int C4>
@@ -446,7 +480,8 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
     if (split || bounded) KC_CUDA(cudaMemsetAsync(ws, 0, split ? head_bytes(nq, sh) : 16, st));
-    a.jfirst = split && !bounded ? AP_SEED : 0;
+    const bool idseed = a.seed1 != nullptr;
+    a.jfirst = split && !bounded && !idseed ? AP_SEED : 0;
     int js = sh.js;
     int64_t jchunk;
     if (split) {
@@ -462,7 +497,12 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.seed = nullptr;
     a.part = split ? seed + nq : nullptr;
     int launches = 1;
-    if (split && !bounded) {
+    if (idseed) {
+        if (D == 2) allpairs_idseed_kernel<2><<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(a, seed);
+        else allpairs_idseed_kernel<3><<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(a, seed);
+        a.seed = seed;
+        ++launches;
+    } else if (split && !bounded) {
         const int blocks = (int)((nq + 7) / 8 < 148 * 8 ? (nq + 7) / 8 : 148 * 8);
         if (D == 2) allpairs_seed_kernel<2><<<blocks, 256, 0, st>>>(a, (int)a.jfirst, seed);
         else allpairs_seed_kernel<3><<<blocks, 256, 0, st>>>(a, (int)a.jfirst, seed);
@@ -494,8 +534,9 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
 }
 
 kc_status run(const char *who, const float *p, int64_t N, int d, const int32_t *q, const int32_t *nq_dev,
-              int64_t nq, const float *d2_prev, const float *eps, int32_t *nn, int32_t *nn2, float *d1,
-              float *d2, float *c, void *workspace, size_t workspace_bytes, void *stream)
+              int64_t nq, const float *d2_prev, const float *eps, const int32_t *seed1,
+              const int32_t *seed2, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
+              void *workspace, size_t workspace_bytes, void *stream)
 {
     if (!p || !nn || !d1 || !d2 || !c || N < 2 || N > 0x7ffffff0 || (d != 2 && d != 3) ||
         (reinterpret_cast<uintptr_t>(p) & 7) || (d2_prev != nullptr) != (eps != nullptr)) {
@@ -511,6 +552,7 @@ kc_status run(const char *who, const float *p, int64_t N, int d, const int32_t *
     ApArgs a = {};
     a.p = p; a.N = N; a.qlist = q; a.nq_dev = nq_dev; a.nq_host = nq;
     a.bound_d2 = d2_prev; a.bound_eps = eps;
+    a.seed1 = seed1; a.seed2 = seed2;
     a.nn = nn; a.nn2 = nn2; a.d1 = d1; a.d2 = d2; a.c = c;
     if (d == 2) return launch<2>(a, (char *)workspace, sh, (cudaStream_t)stream);
     return launch<3>(a, (char *)workspace, sh, (cudaStream_t)stream);
@@ -528,7 +570,7 @@ extern "C" kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t 
                                       float *d1, float *d2, float *c, void *workspace,
                                       size_t workspace_bytes, void *stream)
 {
-    return run("kc_cert_allpairs", p, N, d, nullptr, nullptr, N, nullptr, nullptr, nn, nn2, d1, d2, c,
+    return run("kc_cert_allpairs", p, N, d, nullptr, nullptr, N, nullptr, nullptr, nullptr, nullptr, nn, nn2, d1, d2, c,
                workspace, workspace_bytes, stream);
 }
 
@@ -541,8 +583,21 @@ extern "C" kc_status kc_cert_allpairs_bounded(const float *p, int64_t N, int d, 
         set_error("kc_cert_allpairs_bounded: d2_prev and eps must be non-NULL");
         return KC_EINVAL;
     }
-    return run("kc_cert_allpairs_bounded", p, N, d, nullptr, nullptr, N, d2_prev, eps, nn, nn2, d1, d2, c,
+    return run("kc_cert_allpairs_bounded", p, N, d, nullptr, nullptr, N, d2_prev, eps, nullptr, nullptr, nn, nn2, d1, d2, c,
                workspace, workspace_bytes, stream);
+}
+
+extern "C" kc_status kc_cert_allpairs_seeded(const float *p, int64_t N, int d, const int32_t *seed1,
+                                             const int32_t *seed2, int32_t *nn, int32_t *nn2, float *d1,
+                                             float *d2, float *c, void *workspace, size_t workspace_bytes,
+                                             void *stream)
+{
+    if (!seed1 || !seed2) {
+        set_error("kc_cert_allpairs_seeded: seed1 and seed2 must be non-NULL");
+        return KC_EINVAL;
+    }
+    return run("kc_cert_allpairs_seeded", p, N, d, nullptr, nullptr, N, nullptr, nullptr, seed1, seed2, nn, nn2,
+               d1, d2, c, workspace, workspace_bytes, stream);
 }
 
 // NEXT #1 (PAPER.md:69 rtx_frontier_oracle): relabel a query subset against all N points.
@@ -564,6 +619,6 @@ extern "C" kc_status kc_frontier_oracle(const float *p, int64_t N, int d, const 
         return KC_EINVAL;
     }
     if (nq_max == 0) return KC_OK;
-    return run("kc_frontier_oracle", p, N, d, q, nq, nq_max, nullptr, nullptr, nn, nn2, d1, d2, c,
+    return run("kc_frontier_oracle", p, N, d, q, nq, nq_max, nullptr, nullptr, nullptr, nullptr, nn, nn2, d1, d2, c,
                workspace, workspace_bytes, stream);
 }

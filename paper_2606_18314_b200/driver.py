@@ -71,7 +71,8 @@ class Maintainer:
 
     def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None,
              frontier: torch.Tensor | None = None, time_phases: bool = False,
-             do_allpairs: bool = True, bounded_allpairs: bool = True, audit: bool = False) -> StepResult:
+             do_allpairs: bool = True, bounded_allpairs: bool = True, seeded_allpairs: bool = True,
+             audit: bool = False) -> StepResult:
         """One transition p -> p_next through every row of the hot path.
 
         ``movers``: optional int32 id list of the points that moved (None = all may have moved).
@@ -111,7 +112,11 @@ class Maintainer:
             # the maintained certificates bound the new second-neighbour distance by d2 + 2 eps_t
             # (Lemma 1's triangle inequality; entries repaired above already hold the
             # new d2); the pass is exact whatever the bound (kc_cert_allpairs_bounded)
-            if bounded_allpairs:
+            if seeded_allpairs:
+                # ... or, tighter and without eps_t: the maintained neighbours themselves are two
+                # known points, their new distances bound the new d2 (kc_cert_allpairs_seeded)
+                kc.kc_cert_allpairs(p_next, self.ap, self.ws, seed1=repaired.nn, seed2=repaired.nn2)
+            elif bounded_allpairs:
                 kc.kc_cert_allpairs(p_next, self.ap, self.ws, d2_prev=repaired.d2, eps=self.eps)
             else:
                 kc.kc_cert_allpairs(p_next, self.ap, self.ws)
@@ -213,11 +218,11 @@ class GraphMaintainer:
     """The step of :class:`Maintainer` captured in CUDA graphs (small N is launch-bound: ~20 short
     kernels per step).  Per ping-pong parity:
       graph A  = A0, A4, A6, A7 || A5 on the grid resident at p, beside them (second stream, fork /
-                 join inside the graph) A2+A3 of p' into a second grid, then a snapshot of the new d2
-                 as the NEXT step's all-pairs bound;
-      graph B0 = A0 once more into a buffer of its own, graph B = the all-pairs certification of p'
-                 from that eps_t and the snapshot taken by the previous step.
-    B0 + B depend on nothing A computes, so (overlap_allpairs) they run on their own stream beside A,
+                 join inside the graph) A2+A3 of p' into a second grid, then a snapshot of the new nn,
+                 nn2 as the NEXT step's all-pairs seeds;
+      graph B  = the all-pairs certification of p' started from every point's previous nn, nn2
+                 (kc_cert_allpairs_seeded; the ids are the snapshot the previous step left).
+    B depends on nothing A computes, so (overlap_allpairs) it runs on its own stream beside A,
     B still bracketed by CUDA events; the short latency-bound kernels of A fill the issue slots the
     N x N pass leaves free.  With overlap_allpairs=False B is replayed after A on the same stream.
 
@@ -241,9 +246,9 @@ class GraphMaintainer:
         self.side_ap = torch.cuda.Stream(device=dev)
         self.pos = [p0.clone(), torch.empty_like(p0)]
         self.cert = [self.m.certs, self.m.other]
-        # bound[k]: upper bounds on the second-neighbour distances at pos[k] (the exact d2 there)
-        self.bound = [self.cert[0].d2.clone(), torch.empty(self.N, dtype=torch.float32, device=dev)]
-        self.eps_b = torch.zeros(1, dtype=torch.float32, device=dev)
+        # seed1/2[k]: two known points per query at pos[k] (its exact neighbours there)
+        self.seed1 = [self.cert[0].nn.clone(), torch.empty(self.N, dtype=torch.int32, device=dev)]
+        self.seed2 = [self.cert[0].nn2.clone(), torch.empty(self.N, dtype=torch.int32, device=dev)]
         self.k = 0
         self.graphs = [None, None]
         self.launches = [0, 0]
@@ -256,7 +261,8 @@ class GraphMaintainer:
         self.side.wait_stream(main)
         with torch.cuda.stream(self.side):                 # rebuild path: needs only p'
             kc.kc_cert_grid_rebuild(self.grid[1 - k], nxt, other)
-            self.bound[1 - k].copy_(other.d2)              # the next step's all-pairs bound
+            self.seed1[1 - k].copy_(other.nn)              # the next step's all-pairs seeds
+            self.seed2[1 - k].copy_(other.nn2)
         kc.kc_max_displacement(cur, nxt, m.eps)            # repair path, on the grid resident at p
         kc.kc_frontier_classify(certs.c, m.eps, m.flags, m.F, m.nF)
         kc.kc_grid_update(self.grid[k], nxt)
@@ -267,27 +273,21 @@ class GraphMaintainer:
         main.wait_stream(self.side2)
         main.wait_stream(self.side)
 
-    def _body_b0(self, k):
-        kc.kc_max_displacement(self.pos[k], self.pos[1 - k], self.eps_b)
-
     def _body_b(self, k):
         m = self.m
-        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, d2_prev=self.bound[k], eps=self.eps_b)
+        kc.kc_cert_allpairs(self.pos[1 - k], m.ap, m.ws, seed1=self.seed1[k], seed2=self.seed2[k])
 
     def _capture(self, k):
         n0 = kc.kc_launch_count()
-        ga, gb0, gb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
+        ga, gb = torch.cuda.CUDAGraph(), torch.cuda.CUDAGraph()
         with torch.cuda.graph(ga):
             self._body_a(k)
-        with torch.cuda.graph(gb0):
-            self._body_b0(k)
         with torch.cuda.graph(gb):
             self._body_b(k)
-        self.graphs[k] = (ga, gb0, gb)
+        self.graphs[k] = (ga, gb)
         self.launches[k] = kc.kc_launch_count() - n0
 
-    def _replay_b(self, gb0, gb, timed):
-        gb0.replay()
+    def _replay_b(self, gb, timed):
         if timed:
             e0 = torch.cuda.Event(enable_timing=True)
             e1 = torch.cuda.Event(enable_timing=True)
@@ -308,17 +308,17 @@ class GraphMaintainer:
         if self.graphs[k] is None:
             torch.cuda.synchronize()
             self._capture(k)
-        ga, gb0, gb = self.graphs[k]
+        ga, gb = self.graphs[k]
         main = torch.cuda.current_stream()
         if self.overlap:
             self.side_ap.wait_stream(main)
             with torch.cuda.stream(self.side_ap):
-                self._replay_b(gb0, gb, time_allpairs)
+                self._replay_b(gb, time_allpairs)
             ga.replay()
             main.wait_stream(self.side_ap)
         else:
             ga.replay()
-            self._replay_b(gb0, gb, time_allpairs)
+            self._replay_b(gb, time_allpairs)
         self.k = 1 - k
         return StepResult(m.eps, m.nF, m.H, m.m, m.C, self.cert[k], self.cert[1 - k], m.ap)
 

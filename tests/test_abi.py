@@ -70,6 +70,7 @@ def test_bad_arguments_are_rejected(L):
     assert b"kc_max_displacement" in L.kc_last_error()
     E = binding.KC_EINVAL
     assert L.kc_cert_allpairs_bounded(None, 100, 2, None, None, None, None, None, None, None, None, 0, None) == E
+    assert L.kc_cert_allpairs_seeded(None, 100, 2, None, None, None, None, None, None, None, None, 0, None) == E
     assert L.kc_frontier_oracle(None, 100, 2, None, None, 5, None, None, None, None, None, None, 0, None) == E
     assert L.kc_grid_build(None, None, 100, None) == E
     assert L.kc_cert_grid_search(None, None, None, None, None, None, None) == E

@@ -156,6 +156,31 @@ def test_grid_far_from_origin_and_on_cell_faces(d, offset):
         assert_same(work, post, idx=F, what=f"offset {offset} d{d} repair |F|={F.size}")
 
 
+@pytest.mark.parametrize("cfg,N", [("cfg1", 1000), ("cfg2", 16000), ("cfg3", 16000), ("cfg4", 100000)])
+def test_allpairs_seeded_is_exact_for_any_seeds(cfg, N):
+    """kc_cert_allpairs_seeded: same bits as the oracle whether the seeds are the previous
+    neighbours, the true new ones, random ids, or garbage (self, duplicates, out of range)."""
+    p, mot = wl.make_scene(cfg) if cfg != "cfg4" else (wl.make_points(cfg, N=N), None)
+    if mot is None:
+        q = (p + np.float32(1e-4) * wl.uniform_points(N, p.shape[1], 5)).astype(np.float32)
+    else:
+        q, _ = mot.step(p)
+    pre, want = ref_certs(p), ref_certs(q)
+    Q = dev(q)
+    rng = np.random.default_rng(11)
+    ids = np.arange(N, dtype=np.int32)
+    garbage1 = rng.integers(-5, N + 5, N).astype(np.int32)
+    garbage2 = garbage1.copy()
+    garbage2[::3] = rng.integers(0, N, garbage2[::3].size)
+    seeds = {"previous": (pre.nn, pre.nn2), "true": (want.nn, want.nn2), "swapped": (want.nn2, want.nn),
+             "random": (rng.integers(0, N, N).astype(np.int32), rng.integers(0, N, N).astype(np.int32)),
+             "self": (ids, ids), "none": (np.full(N, -1, np.int32), np.full(N, -1, np.int32)),
+             "garbage": (garbage1, garbage2), "one": (want.nn, np.full(N, -1, np.int32))}
+    for name, (s1, s2) in seeds.items():
+        got = kc.kc_cert_allpairs(Q, seed1=dev(s1), seed2=dev(s2))
+        assert_same(got, want, what=f"seeded allpairs {cfg} seeds={name}")
+
+
 def test_grid_with_points_outside_the_box():
     # geometry fitted to the central half of the points: the rest is clamped into boundary cells
     p = wl.uniform_points(20000, 3, 31)
