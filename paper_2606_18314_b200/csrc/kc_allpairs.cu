@@ -339,11 +339,14 @@ allpairs_seed_kernel(const ApArgs a, int S, Partial *__restrict__ seed)
 // invalidate; ids that are out of range, equal to i or to each other are dropped (cold start).
 template <int D>
 __global__ void __launch_bounds__(256)
-allpairs_idseed_kernel(const ApArgs a, Partial *__restrict__ seed)
+allpairs_idseed_kernel(const ApArgs a, Partial *__restrict__ seed, int n_head_words)
 {
     const float *__restrict__ p = a.p;
     const int64_t nq = a.nq_dev ? (int64_t)*a.nq_dev : a.nq_host;
     const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    // this kernel runs right before the pass: it also zeroes the pass's tickets and redo counter
+    // (saves the memset node of the other start modes)
+    if (q < n_head_words) reinterpret_cast<int32_t *>(a.n_redo)[q] = 0;
     if (q >= nq) return;
     const int i = a.qlist ? a.qlist[q] : (int)q;
     const float qx = p[(int64_t)i * D], qy = p[(int64_t)i * D + 1];
@@ -479,8 +482,9 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.tickets = reinterpret_cast<int32_t *>(ws + 16);
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
-    if (split || bounded) KC_CUDA(cudaMemsetAsync(ws, 0, split ? head_bytes(nq, sh) : 16, st));
     const bool idseed = a.seed1 != nullptr;
+    const int n_head_words = (int)((split ? head_bytes(nq, sh) : 16) / 4);     // n_redo + tickets
+    if ((split || bounded) && !idseed) KC_CUDA(cudaMemsetAsync(ws, 0, (size_t)n_head_words * 4, st));
     a.jfirst = split && !bounded && !idseed ? AP_SEED : 0;
     int js = sh.js;
     int64_t jchunk;
@@ -498,8 +502,9 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.part = split ? seed + nq : nullptr;
     int launches = 1;
     if (idseed) {
-        if (D == 2) allpairs_idseed_kernel<2><<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(a, seed);
-        else allpairs_idseed_kernel<3><<<(unsigned)((nq + 255) / 256), 256, 0, st>>>(a, seed);
+        const int64_t nthr = nq > n_head_words ? nq : n_head_words;
+        if (D == 2) allpairs_idseed_kernel<2><<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(a, seed, n_head_words);
+        else allpairs_idseed_kernel<3><<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(a, seed, n_head_words);
         a.seed = seed;
         ++launches;
     } else if (split && !bounded) {
