@@ -68,6 +68,18 @@ def test_allpairs_small(name):
 
 
 @pytest.mark.parametrize("name", sorted(SMALL))
+def test_allpairs_small_warm_starts(name):
+    """The seeded and the bounded start on the tiny / degenerate scenes (N = 2 has nn2 = -1 and
+    d2 = inf; ties; duplicates; one point repeated)."""
+    p = SMALL[name]
+    want = oracle.bruteforce_top2(p)
+    P = dev(p)
+    assert_same(kc.kc_cert_allpairs(P, seed1=dev(want.nn), seed2=dev(want.nn2)), want, what=name + " seeded")
+    eps = dev(np.zeros(1, np.float32))
+    assert_same(kc.kc_cert_allpairs(P, d2_prev=dev(want.d2), eps=eps), want, what=name + " bounded")
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
 def test_grid_rebuild_small(name):
     p = SMALL[name]
     g_or, g_kc = geoms(p)
