@@ -455,6 +455,53 @@ def test_graphed_step_matches_the_oracle(cfg, fam, overlap):
         p, pre = q, post
 
 
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_randomized_scenes(seed):
+    """Random scenes (uniform / Gaussian / lattice with ties / tight clusters / mixtures; scaled and
+    shifted; occupancy 0.25-50; box sometimes smaller than the data): all-pairs, rebuild, two
+    successive repairs of a random id list (the second over overflow chains), seeded all-pairs,
+    rebuild again, each bit-exact against brute force."""
+    rng = np.random.default_rng(seed)
+    for it in range(60):
+        d = int(rng.integers(2, 4))
+        N = int(rng.integers(2, 3000))
+        kind = int(rng.integers(0, 5))
+        if kind == 0:
+            p = rng.random((N, d))
+        elif kind == 1:
+            p = 0.5 + 0.02 * rng.standard_normal((N, d))
+        elif kind == 2:
+            p = rng.integers(0, 12, (N, d)) / 12.0
+        elif kind == 3:
+            k = max(1, N // 50)
+            p = rng.random((k, d))[rng.integers(0, k, N)] + rng.choice([1e-4, 1e-2]) * rng.standard_normal((N, d))
+        else:
+            p = np.concatenate([rng.random((N - N // 2, d)), 0.3 + 1e-3 * rng.standard_normal((N // 2, d))])
+        p = (p * rng.choice([1.0, 100.0, 1e-3]) + rng.choice([0.0, 0.0, 1000.0, -77.7])).astype(np.float32)
+        tag = f"seed {seed} scene {it} (d={d}, N={N}, kind={kind})"
+        lo, hi = np.zeros(3, np.float32), np.zeros(3, np.float32)
+        lo[:d], hi[:d] = p.min(0), p.max(0)
+        if rng.random() < 0.2:
+            c = (lo + hi) / 2
+            lo, hi = (c - (c - lo) * 0.5).astype(np.float32), (c + (hi - c) * 0.5).astype(np.float32)
+        g_or, g_kc = geoms(p, occ=float(rng.choice([0.25, 1, 2, 2, 2, 8, 50])), lo=lo[:d], hi=hi[:d])
+        grid = kc.Grid(N, g_kc)
+        want = oracle.bruteforce_top2(p)
+        assert_same(kc.kc_cert_allpairs(dev(p)), want, what=tag + " allpairs")
+        certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+        assert_same(certs, want, what=tag + " rebuild")
+        step = float(rng.choice([1e-4, 1e-2, 0.3])) * float(max(hi.max() - lo.min(), 1e-6)) / max(1, int(round(N ** (1 / d))))
+        F = np.sort(rng.choice(N, int(rng.integers(1, N + 1)), replace=False)).astype(np.int32)
+        q = p
+        for rep in range(2):
+            q = (q + step * (rng.random((N, d)) - 0.5)).astype(np.float32)
+            post = oracle.bruteforce_top2(q)
+            kc.kc_frontier_repair(grid, dev(q), dev(F), dev(np.array([F.size], np.int32)), certs)
+            assert_same(certs, post, idx=F, what=tag + f" repair {rep}")
+        assert_same(kc.kc_cert_allpairs(dev(q), seed1=certs.nn, seed2=certs.nn2), post, what=tag + " seeded")
+        assert_same(kc.kc_cert_grid_rebuild(grid, dev(q)), post, what=tag + " rebuild 2")
+
+
 def test_search_refused_on_dirty_grid():
     p, mot = wl.make_scene("cfg1")
     grid = kc.Grid(p.shape[0], geoms(p)[1])
