@@ -76,6 +76,8 @@ def _load():
         L.orc_bruteforce_top2_subset.restype = C.c_int
         L.orc_bruteforce_top2_subset.argtypes = [fp, C.c_int64, C.c_int, ip, C.c_int64,
                                                  ip, ip, fp, fp, fp, C.c_int]
+        L.orc_bruteforce_topk.restype = C.c_int
+        L.orc_bruteforce_topk.argtypes = [fp, C.c_int64, C.c_int, C.c_int, ip, C.c_int64, ip, fp, fp, C.c_int]
         L.orc_kdtree_top2.restype = C.c_int
         L.orc_kdtree_top2.argtypes = [fp, C.c_int64, C.c_int, ip, C.c_int64,
                                       ip, ip, fp, fp, fp, C.c_int]
@@ -155,6 +157,27 @@ def bruteforce_top2(p, queries=None, nthreads: int | None = None) -> Certs:
     if rc != 0:
         raise ValueError(f"orc_bruteforce_top2 rc={rc}")
     return out
+
+
+def bruteforce_topk(p, K: int, queries=None, nthreads: int | None = None):
+    """NEXT #4, reading R20 (Definition 1 :29 generalised): the K smallest keys
+    (s, j) of every query by the O(N^2) definition.  Returns (nnk int32[nq,K], dk float32[nq,K],
+    ck float32[nq]) with ck = dk[:,K-1] - dk[:,K-2]."""
+    p = _f32(p)
+    N, d = p.shape
+    nthreads = nthreads or num_procs()
+    if queries is None:
+        qp, nq = None, N
+    else:
+        q = np.ascontiguousarray(queries, dtype=np.int32)
+        qp, nq = _ip(q), q.size
+    nnk = np.empty((nq, K), np.int32)
+    dk = np.empty((nq, K), np.float32)
+    ck = np.empty(nq, np.float32)
+    rc = _load().orc_bruteforce_topk(_fp(p), N, d, K, qp, nq, _ip(nnk), _fp(dk), _fp(ck), nthreads)
+    if rc != 0:
+        raise ValueError(f"orc_bruteforce_topk rc={rc}")
+    return nnk, dk, ck
 
 
 def kdtree_top2(p, queries=None, nthreads: int | None = None) -> Certs:

@@ -132,6 +132,53 @@ int orc_bruteforce_top2_subset(const float *p, int64_t N, int d, const int32_t *
     return 0;
 }
 
+/* ------------------------------------------------ NEXT #4: K-list certificate
+ * "Richer geometric certificates (... k-nearest-neighbour graphs ...) are left
+ * open" (Limitations); the paper studies "k=2 certificates", i.e.
+ * the list of the 2 smallest keys (Definition 1).  Reading R20
+ * (DESIGN.md): the K-list certificate of point i is the list of the K smallest
+ * keys (s(i,j), j), j != i, in ascending order of the same total order (O1, A2,
+ * A3): ids nnk[0..K), distances dk[q] = sqrtf(s_q), and the clearance of its
+ * (K-1)-nearest-neighbour SET,  ck = dk[K-1] - dk[K-2]  (one rounded
+ * subtraction).  K = 2 is Definition 1 exactly (nn = nnk[0], d1, d2, c).  A
+ * missing entry (fewer than K other points) has id -1 and distance +inf, and
+ * ck = +inf whenever dk[K-1] = +inf.
+ * Written as the definition: collect every key, keep the list sorted by plain
+ * insertion.  q == NULL means every point is a query.  O(nq N K).            */
+int orc_bruteforce_topk(const float *p, int64_t N, int d, int K, const int32_t *q, int64_t nq,
+                        int32_t *nnk, float *dk, float *ck, int nthreads)
+{
+    if (!p || !nnk || !dk || !ck || N < 2 || (d != 2 && d != 3) || K < 2 || K > 64) return -1;
+    if (!q) nq = N;
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(dynamic, 4) num_threads(nthreads)
+    for (int64_t k = 0; k < nq; ++k) {
+        int64_t i = q ? q[k] : k;
+        float ls[64];
+        int32_t lj[64];
+        int n = 0;                                   /* entries held, ascending in (s, j) */
+        const float *pi = p + i * d;
+        for (int64_t j = 0; j < N; ++j) {
+            if (j == i) continue;
+            float s = d == 2 ? sq2(pi, p + j * d) : sq3(pi, p + j * d);
+            int pos = n;                             /* first position whose key is larger */
+            while (pos > 0 && (s < ls[pos - 1] || (s == ls[pos - 1] && (int32_t)j < lj[pos - 1]))) --pos;
+            if (pos >= K) continue;
+            int last = n < K ? n : K - 1;
+            for (int t = last; t > pos; --t) { ls[t] = ls[t - 1]; lj[t] = lj[t - 1]; }
+            ls[pos] = s; lj[pos] = (int32_t)j;
+            if (n < K) ++n;
+        }
+        for (int t = 0; t < K; ++t) {
+            nnk[k * K + t] = t < n ? lj[t] : -1;
+            dk[k * K + t] = t < n ? sqrtf(ls[t]) : INFINITY;
+        }
+        float a = dk[k * K + K - 2], b = dk[k * K + K - 1];
+        ck[k] = isinf(b) ? INFINITY : b - a;
+    }
+    return 0;
+}
+
 /* ---------------------------------------------------------------- O7 ------
  * k-d tree ("Exact nearest neighbours for ground truth are
  * computed with a k-d tree"): median split on the widest axis, leaves of at

@@ -44,8 +44,25 @@ def check_scene(path):
         assert bits(f2 - f1) == g["c_bits"][i], (path, i)
 
 
+def check_topk(path):
+    """K-list certificates (reading R20): lists, exact squared distances, distance and clearance bits."""
+    for g in json.load(open(path))["scenes"]:
+        P = [[Fraction(v) for v in row] for row in g["points"]]
+        n, K = len(P), g["K"]
+        for i in range(n):
+            keys = sorted((sum((a - b) ** 2 for a, b in zip(P[i], P[j])), j) for j in range(n) if j != i)[:K]
+            assert [j for _, j in keys] == g["nnk"][i], (path, i)
+            assert [s for s, _ in keys] == [Fraction(v) for v in g["sk"][i]], (path, i)
+            db = [f32_bits_of((Decimal(s.numerator) / Decimal(s.denominator)).sqrt()) for s, _ in keys]
+            assert ["%08x" % b for b in db] == g["dk_bits"][i], (path, i)
+            f = [np.float32(struct.unpack("<f", struct.pack("<I", b))[0]) for b in db]
+            assert bits(f[K - 1] - f[K - 2]) == g["ck_bits"][i], (path, i)
+
+
 if __name__ == "__main__":
     here = os.path.dirname(os.path.abspath(__file__))
     for f in sorted(glob.glob(os.path.join(here, "p[12]*.json"))):
         check_scene(f)
         print("ok", os.path.basename(f))
+    check_topk(os.path.join(here, "p7_topk_lists.json"))
+    print("ok p7_topk_lists.json")

@@ -411,3 +411,92 @@ def test_local_budget_never_misses(cfg, fam):
         p, pre = q, post
     if fam in ("local", "diffuse5", "ball5"):
         assert max(ratio) < 0.5
+
+
+# ------------------------------------------------------------------ NEXT #4: K-list certificates
+def test_topk_hand_worked(golden_dir):
+    """Reading R20 on the hand-worked scenes (lists, distance bits, clearance bits, tie rule)."""
+    for g in load(golden_dir, "p7_topk_lists.json")["scenes"]:
+        p = np.array(g["points"], np.float32)
+        nnk, dk, ck = oracle.bruteforce_topk(p, g["K"])
+        assert nnk.tolist() == g["nnk"]
+        assert [[b for b in bits(row)] for row in dk] == g["dk_bits"]
+        assert [b for b in bits(ck)] == g["ck_bits"]
+
+
+def numpy_topk(p, K):
+    """Independent restatement with library routines: float32 numpy arithmetic (one rounding per
+    operation, left to right) and a lexicographic sort of the keys (s, j)."""
+    p = np.asarray(p, np.float32)
+    N, d = p.shape
+    ids = np.empty((N, K), np.int32)
+    dist = np.empty((N, K), np.float32)
+    for i in range(N):
+        df = p[i] - p
+        sq = df * df
+        s = sq[:, 0] + sq[:, 1]
+        if d == 3:
+            s = s + sq[:, 2]
+        j = np.delete(np.arange(N), i)
+        s = np.delete(s, i)
+        o = np.lexsort((j, s))[:K]
+        ids[i], dist[i] = j[o], np.sqrt(s[o])
+    return ids, dist, dist[:, K - 1] - dist[:, K - 2]
+
+
+@pytest.mark.parametrize("d", [2, 3])
+@pytest.mark.parametrize("K", [2, 3, 5, 8])
+def test_topk_against_numpy_lexsort(d, K):
+    rng = np.random.default_rng(100 * d + K)
+    scenes = [rng.random((400, d)).astype(np.float32),
+              (rng.integers(0, 6, (300, d)) / 8).astype(np.float32)]        # lattice: ties and duplicates
+    for p in scenes:
+        nnk, dk, ck = oracle.bruteforce_topk(p, K)
+        ids, dist, c = numpy_topk(p, K)
+        assert np.array_equal(nnk, ids)
+        assert np.array_equal(dk.view(np.uint32), dist.view(np.uint32))
+        assert np.array_equal(ck.view(np.uint32), c.view(np.uint32))
+    q = np.array([7, 0, 399, 7], np.int32)
+    a = oracle.bruteforce_topk(scenes[0], K, queries=q)
+    for x, y in zip(a, oracle.bruteforce_topk(scenes[0], K)):
+        assert np.array_equal(x, y[q])
+
+
+@pytest.mark.parametrize("cfg", ["cfg1", "cfg3"])
+def test_topk_with_K2_is_definition_1(cfg):
+    """K = 2 is the paper's certificate: same nn, nn2, d1, d2, c as the pinned top-2 oracle."""
+    p = wl.make_points(cfg, N=1500)
+    nnk, dk, ck = oracle.bruteforce_topk(p, 2)
+    ref = oracle.bruteforce_top2(p)
+    assert np.array_equal(nnk[:, 0], ref.nn) and np.array_equal(nnk[:, 1], ref.nn2)
+    assert np.array_equal(bits(dk[:, 0]), bits(ref.d1)) and np.array_equal(bits(dk[:, 1]), bits(ref.d2))
+    assert np.array_equal(bits(ck), bits(ref.c))
+
+
+def test_topk_short_lists():
+    """Fewer than K other points: missing entries are (-1, +inf), ck = +inf."""
+    p = np.array([[0, 0], [1, 0], [0, 2]], np.float32)
+    nnk, dk, ck = oracle.bruteforce_topk(p, 4)
+    assert nnk.tolist() == [[1, 2, -1, -1], [0, 2, -1, -1], [0, 1, -1, -1]]
+    assert np.all(np.isinf(dk[:, 2:])) and np.all(np.isinf(ck))
+    nnk, dk, ck = oracle.bruteforce_topk(p, 3)
+    assert np.all(nnk[:, 2] == -1) and np.all(np.isinf(ck))
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg2", "shear"), ("cfg3", "walk"), ("cfg3", "cluster_drift")])
+@pytest.mark.parametrize("K", [3, 5])
+def test_topk_set_is_stable_beyond_4eps(cfg, fam, K):
+    """Lemma 1's argument for the K-list: if dk[K-1] - dk[K-2] > 4 eps the SET of the
+    K-1 nearest neighbours survives the step (its order may change)."""
+    p, mot = wl.make_scene(cfg, fam, N=1500)
+    pre = oracle.bruteforce_topk(p, K)
+    for _ in range(3):
+        q, _ = mot.step(p)
+        eps = oracle.max_displacement(p, q)
+        post = oracle.bruteforce_topk(q, K)
+        safe = np.flatnonzero(pre[2] > np.float32(4) * eps)
+        a = np.sort(pre[0][safe, :K - 1], axis=1)
+        b = np.sort(post[0][safe, :K - 1], axis=1)
+        assert np.array_equal(a, b)
+        assert safe.size > 0
+        p, pre = q, post
