@@ -253,6 +253,31 @@ kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const in
                              int64_t nF_max, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
                              void *stream);
 
+/* ---- NEXT #4: K-list certificates ---------------------------------------------------------- */
+/* "Richer geometric certificates (Delaunay edges, k-nearest-neighbour graphs, ...) are left open"
+ * (PAPER.md:114); the paper's certificate is the list of the TWO smallest keys (Definition 1,
+ * PAPER.md:29).  The K-list certificate of point i is the list of the K smallest keys
+ * (s(i,j), j), j != i, ascending in the total order of "Arithmetic" above (equal s: smaller id):
+ *   nnk[i*K + q]  id of the q-th key, -1 if fewer than q+1 other points exist
+ *   dk [i*K + q]  sqrtf of its squared distance (+inf if missing)
+ *   ck [i]        dk[i*K+K-1] - dk[i*K+K-2] (one rounded subtraction), +inf if dk[i*K+K-1] = +inf:
+ *                 the clearance of the (K-1)-nearest-neighbour SET.  By the argument of Lemma 1
+ *                  a step with max displacement eps leaves that set unchanged when
+ *                 ck > 4 eps, so ck feeds kc_frontier_classify unchanged.
+ * K = 2 gives nn = nnk[2i], nn2 = nnk[2i+1], d1, d2, c of kc_cert_allpairs bit for bit.
+ * 2 <= K <= KC_TOPK_MAX.  All pointers device, caller-owned: nnk int32[N*K], dk float32[N*K],
+ * ck float32[N], row-major.  kc_cert_allpairs_topk: tiled N x N pass (FP32 ALU bound);
+ * workspace: device scratch of at least kc_cert_allpairs_topk_workspace(N, d, K) bytes (0 for
+ * large N), 4-byte aligned.  kc_cert_grid_topk: ring-expanding search of a freshly built grid,
+ * terminating only when the scanned block's bound exceeds the K-th distance (KC_EREBUILD if the
+ * grid was updated incrementally since its build).  Asynchronous on `stream`; KC_EINVAL on a NULL
+ * pointer, K out of range, N < 2 or d not in {2,3}. */
+#define KC_TOPK_MAX 8
+size_t kc_cert_allpairs_topk_workspace(int64_t N, int d, int K);
+kc_status kc_cert_allpairs_topk(const float *p, int64_t N, int d, int K, int32_t *nnk, float *dk, float *ck,
+                                void *workspace, size_t workspace_bytes, void *stream);
+kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *dk, float *ck, void *stream);
+
 /* ---- inspection (tests, reports) ---------------------------------------------------------- */
 /* Synchronises `stream`, copies the device counters to *out (host). */
 kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream);

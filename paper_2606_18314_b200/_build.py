@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libkc.so")
-SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_grid.cu"]
+SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_topk.cu", "kc_grid.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",

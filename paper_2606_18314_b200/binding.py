@@ -26,6 +26,7 @@ EXPORTS = (
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
     "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
+    "kc_cert_allpairs_topk_workspace", "kc_cert_allpairs_topk", "kc_cert_grid_topk",
     "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
@@ -98,6 +99,10 @@ def lib():
     L.kc_frontier_classify_clock.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp]
     L.kc_clock_stamp.argtypes = [vp, vp, i64, i64, vp, vp, vp]
     L.kc_frontier_classify_local.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.kc_cert_allpairs_topk_workspace.restype = sz
+    L.kc_cert_allpairs_topk_workspace.argtypes = [i64, ci, ci]
+    L.kc_cert_allpairs_topk.argtypes = [vp, i64, ci, ci, vp, vp, vp, vp, sz, vp]
+    L.kc_cert_grid_topk.argtypes = [vp, ci, vp, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
@@ -270,6 +275,7 @@ class Grid:
     def __init__(self, N_max: int, geom: kc_geom):
         self.geom = geom
         self.N_max = int(N_max)
+        self.N = 0                      # points of the last build
         h = C.c_void_p()
         _check(lib().kc_grid_create(C.byref(h), self.N_max, C.byref(geom)), "kc_grid_create")
         self._h = h
@@ -303,6 +309,7 @@ def kc_grid_build(grid: Grid, p):
     """A2: cell ids, histogram, scan, scatter."""
     pp, N, d = _pos(p)
     _check(lib().kc_grid_build(grid._h, pp, N, _stream()), "kc_grid_build")
+    grid.N = N
 
 
 def kc_cert_grid_search(grid: Grid, out: Certs | None = None, N=None) -> Certs:
@@ -317,7 +324,35 @@ def kc_cert_grid_rebuild(grid: Grid, p, out: Certs | None = None) -> Certs:
     pp, N, d = _pos(p)
     out = out or Certs.empty(N, p.device)
     _check(lib().kc_cert_grid_rebuild(grid._h, pp, N, *out._ptrs(), _stream()), "kc_cert_grid_rebuild")
+    grid.N = N
     return out
+
+
+def _topk_out(N, K, device):
+    return (torch.empty((N, K), dtype=torch.int32, device=device),
+            torch.empty((N, K), dtype=torch.float32, device=device),
+            torch.empty(N, dtype=torch.float32, device=device))
+
+
+def kc_cert_allpairs_topk(p, K: int, workspace=None):
+    """NEXT #4: K-list certificates by the tiled N x N pass (Definition 1 :29 with K
+    keys).  Returns (nnk int32[N,K], dk float32[N,K], ck float32[N])."""
+    pp, N, d = _pos(p)
+    nnk, dk, ck = _topk_out(N, K, p.device)
+    need = lib().kc_cert_allpairs_topk_workspace(N, d, K)
+    ws = workspace if workspace is not None else _workspace(need, p.device)
+    _check(lib().kc_cert_allpairs_topk(pp, N, d, K, _ptr(nnk), _ptr(dk), _ptr(ck), _ptr(ws),
+                                       ws.numel() if ws is not None else 0, _stream()), "kc_cert_allpairs_topk")
+    return nnk, dk, ck
+
+
+def kc_cert_grid_topk(grid: Grid, K: int, device=None):
+    """NEXT #4: K-list certificates of every point of a freshly built grid (ring search, exact)."""
+    if grid.N < 2:
+        raise RebuildRequired(KC_EREBUILD, "kc_cert_grid_topk", "the grid has not been built")
+    nnk, dk, ck = _topk_out(grid.N, K, device or torch.device("cuda"))
+    _check(lib().kc_cert_grid_topk(grid._h, K, _ptr(nnk), _ptr(dk), _ptr(ck), _stream()), "kc_cert_grid_topk")
+    return nnk, dk, ck
 
 
 def kc_frontier_classify(c, eps, flags=None, F=None, nF=None):

@@ -83,4 +83,43 @@ __device__ __forceinline__ int cell_axis(float x, float lo, float inv_h, int G)
     return k;
 }
 
+// NEXT #4 (reading R20): the K smallest keys under the same total order (s, j), ascending.
+// K is a compile-time constant, so the list lives in registers; a new key replaces the worst one
+// and bubbles up through K-1 compare-exchanges written as selects.
+template <int K>
+struct TopK {
+    float s[K];
+    int j[K];
+    __device__ __forceinline__ void init()
+    {
+#pragma unroll
+        for (int q = 0; q < K; ++q) { s[q] = CUDART_INF_F; j[q] = KC_NOIDX; }
+    }
+    __device__ __forceinline__ void offer(float x, int id)
+    {
+        if (!(x < s[K - 1] || (x == s[K - 1] && id < j[K - 1]))) return;
+        s[K - 1] = x; j[K - 1] = id;
+#pragma unroll
+        for (int q = K - 1; q > 0; --q) {
+            const bool sw = s[q] < s[q - 1] || (s[q] == s[q - 1] && j[q] < j[q - 1]);
+            const float ts = s[q];
+            const int tj = j[q];
+            s[q] = sw ? s[q - 1] : ts; j[q] = sw ? j[q - 1] : tj;
+            s[q - 1] = sw ? ts : s[q - 1]; j[q - 1] = sw ? tj : j[q - 1];
+        }
+    }
+    // dk[q] = sqrtf(s_q); ck = dk[K-1] - dk[K-2], +inf when the list is short (kc.h)
+    __device__ __forceinline__ void store(int64_t i, int32_t *nnk, float *dk, float *ck) const
+    {
+        float dq[K];
+#pragma unroll
+        for (int q = 0; q < K; ++q) {
+            dq[q] = __fsqrt_rn(s[q]);
+            nnk[i * K + q] = j[q] == KC_NOIDX ? -1 : j[q];
+            dk[i * K + q] = dq[q];
+        }
+        ck[i] = s[K - 1] == CUDART_INF_F ? CUDART_INF_F : __fsub_rn(dq[K - 1], dq[K - 2]);
+    }
+};
+
 }  // namespace kc

@@ -1063,6 +1063,90 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
     }
 }
 
+// ---- NEXT #4: K-list certificates through the grid ---------------------------------------------
+// One thread per sorted slot of a freshly built grid: own cell, then Chebyshev rings, until the
+// bound of the scanned block exceeds the K-th best distance (the same strict test as A3, with
+// s_K in the place of s_2: every unscanned point is then strictly farther than the K-th key).
+template <int D, int K>
+__device__ __forceinline__ void topk_scan_cells(const View &v, int rowbase, int x0, int x1, float qx, float qy,
+                                                float qz, int self, TopK<K> &best)
+{
+    const int b = v.cell_start[rowbase + x0], e = v.cell_start[rowbase + x1 + 1];
+    for (int t = b; t < e; ++t) {
+        float s;
+        int j;
+        if (D == 2) {
+            const float2 c = v.spos2[t];
+            s = sqd2(qx, qy, c.x, c.y);
+            j = v.sidx[t];
+        } else {
+            const float4 c = v.spos4[t];
+            s = sqd3(qx, qy, qz, c.x, c.y, c.z);
+            j = __float_as_int(c.w);
+        }
+        if (s <= best.s[K - 1] && j >= 0 && j != self) best.offer(s, j);
+    }
+}
+template <int D, int K>
+__global__ void __launch_bounds__(128)
+search_topk_kernel(View v, int N, int32_t *__restrict__ nnk, float *__restrict__ dk, float *__restrict__ ck)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= N) return;
+    float qx, qy, qz = 0.f;
+    int self;
+    if (D == 2) {
+        const float2 q = v.spos2[s];
+        qx = q.x; qy = q.y; self = v.sidx[s];
+    } else {
+        const float4 q = v.spos4[s];
+        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
+    }
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    TopK<K> best;
+    best.init();
+    topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
+    for (int r = 0;;) {
+        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
+        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
+        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
+        ++r;
+        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
+        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y) {
+                const int rowbase = (z * v.G1 + y) * v.G0;
+                const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
+                if (shell) {
+                    topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
+                } else {
+                    if (cx - r >= 0) topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
+                    if (cx + r <= v.G0 - 1) topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                }
+            }
+    }
+    best.store(self, nnk, dk, ck);
+}
+template <int D>
+bool dispatch_grid_topk(int K, const View &v, int n, int32_t *nnk, float *dk, float *ck, cudaStream_t st)
+{
+    const int nb = (n + 127) / 128;
+    switch (K) {
+    case 2: search_topk_kernel<D, 2><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 3: search_topk_kernel<D, 3><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 4: search_topk_kernel<D, 4><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 5: search_topk_kernel<D, 5><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 6: search_topk_kernel<D, 6><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 7: search_topk_kernel<D, 7><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    case 8: search_topk_kernel<D, 8><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
+    default: return false;
+    }
+}
+
 // ------------------------------------------------------------------ A6 incremental update
 // Algorithm 1 line 3: "update cell_i in G for points that changed cell".
 // A mover whose cell is unchanged is overwritten in its sorted slot; one whose cell changed is
@@ -1478,6 +1562,24 @@ extern "C" kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N,
     s = kc_grid_build(g, p, N, stream);
     if (s != KC_OK) return s;
     return kc_cert_grid_search(g, nn, nn2, d1, d2, c, stream);
+}
+
+extern "C" kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *dk, float *ck, void *stream)
+{
+    if (!g || !nnk || !dk || !ck || K < 2 || K > KC_TOPK_MAX) {
+        set_error("kc_cert_grid_topk: bad argument (need grid, nnk, dk, ck, 2 <= K <= %d)", KC_TOPK_MAX);
+        return KC_EINVAL;
+    }
+    if (!g->built || g->dirty) {
+        set_error("kc_cert_grid_topk: grid is not freshly built");
+        return KC_EREBUILD;
+    }
+    const View v = make_view(g);
+    if (g->geom.d == 2) dispatch_grid_topk<2>(K, v, (int)g->N, nnk, dk, ck, (cudaStream_t)stream);
+    else dispatch_grid_topk<3>(K, v, (int)g->N, nnk, dk, ck, (cudaStream_t)stream);
+    count_launches(1);
+    KC_LAUNCH_CHECK("kc_cert_grid_topk");
+    return KC_OK;
 }
 
 extern "C" kc_status kc_frontier_classify_local(kc_grid *g, const float *p, const float *p2, int64_t N,

@@ -1,0 +1,123 @@
+"""GPU parity of the K-list certificates (NEXT #4, reading R20; Definition 1 :29 with
+K keys): kc_cert_allpairs_topk and kc_cert_grid_topk against the brute-force oracle, bit for bit
+(ids, distances, set clearance), through the C-ABI."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_18314_b200 import binding as kc
+from paper_2606_18314_b200 import workloads as wl
+
+from _util import dev, geoms
+
+pytestmark = pytest.mark.gpu
+
+
+def same(got, want, what, idx=None):
+    torch.cuda.synchronize()
+    for name, g, w in zip(("nnk", "dk", "ck"), got, want):
+        g = g.cpu().numpy()
+        if idx is not None:
+            g = g[idx]
+        if g.dtype == np.float32:
+            g, w = g.view(np.uint32), w.view(np.uint32)
+        bad = np.argwhere(g != w)
+        assert bad.size == 0, f"{what}: {name} differs at {len(bad)} entries, first {bad[:4].tolist()}"
+
+
+def grid_topk(p, K, occ=2.0):
+    _, g_kc = geoms(p, occ)
+    grid = kc.Grid(p.shape[0], g_kc)
+    kc.kc_grid_build(grid, dev(p))
+    return kc.kc_cert_grid_topk(grid, K)
+
+
+def scenes(d):
+    rng = np.random.default_rng(7 + d)
+    out = {f"random{n}": rng.random((n, d)).astype(np.float32) for n in (2, 3, 5, 33, 1000, 4097)}
+    out["lattice"] = (np.stack(np.meshgrid(*[np.arange(9)] * d, indexing="ij"), -1).reshape(-1, d) / 8).astype(np.float32)
+    dup = rng.random((300, d)).astype(np.float32)
+    dup[100:200] = dup[:100]                                   # coincident points are neighbours at distance 0
+    out["duplicates"] = dup
+    far = (rng.random((500, d)) * 0.05).astype(np.float32)
+    far[-1] = 40.0                                             # the isolated point a capped search missed
+    out["outlier"] = far
+    out["one_cell"] = (0.5 + rng.random((200, d)) * 1e-4).astype(np.float32)
+    return out
+
+
+@pytest.mark.parametrize("d", [2, 3])
+@pytest.mark.parametrize("K", [2, 3, 4, 8])
+def test_topk_small_scenes(d, K):
+    for name, p in scenes(d).items():
+        want = oracle.bruteforce_topk(p, K)
+        same(kc.kc_cert_allpairs_topk(dev(p), K), want, f"allpairs_topk {name} d={d} K={K}")
+        same(grid_topk(p, K), want, f"grid_topk {name} d={d} K={K}")
+        if p.shape[0] > 50:
+            same(grid_topk(p, K, occ=0.25), want, f"grid_topk occ=.25 {name} d={d} K={K}")   # many rings
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg3", "cluster_drift")])
+@pytest.mark.parametrize("K", [3, 5])
+def test_topk_config_scenes(cfg, fam, K):
+    """N = 16,000 (the j-split launch + merge of the all-pairs pass; clustered cells for the grid)."""
+    p, mot = wl.make_scene(cfg, fam)
+    for _ in range(2):
+        want = oracle.bruteforce_topk(p, K)
+        same(kc.kc_cert_allpairs_topk(dev(p), K), want, f"allpairs_topk {cfg}/{fam} K={K}")
+        same(grid_topk(p, K), want, f"grid_topk {cfg}/{fam} K={K}")
+        p, _ = mot.step(p)
+
+
+@pytest.mark.parametrize("d", [2, 3])
+def test_topk_K2_is_the_papers_certificate(d):
+    p = wl.make_points("cfg2" if d == 2 else "cfg3", N=5000)
+    nnk, dk, ck = kc.kc_cert_allpairs_topk(dev(p), 2)
+    c = kc.kc_cert_allpairs(dev(p))
+    assert torch.equal(nnk[:, 0], c.nn) and torch.equal(nnk[:, 1], c.nn2)
+    assert torch.equal(dk[:, 0].view(torch.int32), c.d1.view(torch.int32))
+    assert torch.equal(dk[:, 1].view(torch.int32), c.d2.view(torch.int32))
+    assert torch.equal(ck.view(torch.int32), c.c.view(torch.int32))
+
+
+def test_topk_full_size_cfg4():
+    """N = 262,144 (config 4): grid and all-pairs lists identical on every point, 256 sampled
+    queries recomputed by the oracle's O(N) definition."""
+    p = wl.make_points("cfg4")
+    K = 4
+    a = kc.kc_cert_allpairs_topk(dev(p), K)
+    g = grid_topk(p, K)
+    for x, y in zip(a, g):
+        assert torch.equal(x.view(torch.int32), y.view(torch.int32))
+    q = np.sort(np.random.default_rng(3).choice(p.shape[0], 256, replace=False)).astype(np.int32)
+    same(g, oracle.bruteforce_topk(p, K, queries=q), "cfg4 grid_topk (sampled brute force)", idx=q)
+
+
+def test_topk_feeds_the_frontier():
+    """ck goes through kc_frontier_classify unchanged; the (K-1)-NN set of every unflagged point
+    survives the step (Lemma 1's argument)."""
+    p, mot = wl.make_scene("cfg2", "walk", N=6000)
+    K = 4
+    pre = kc.kc_cert_allpairs_topk(dev(p), K)
+    q, _ = mot.step(p)
+    eps = kc.kc_max_displacement(dev(p), dev(q))
+    flags, F, nF = kc.kc_frontier_classify(pre[2], eps)
+    wflags, wF = oracle.frontier(oracle.bruteforce_topk(p, K)[2], oracle.max_displacement(p, q))
+    assert np.array_equal(flags.cpu().numpy(), wflags) and int(nF.item()) == wF.size
+    post = kc.kc_cert_allpairs_topk(dev(q), K)
+    safe = (flags == 0).nonzero().flatten()
+    a = torch.sort(pre[0][safe, :K - 1], dim=1).values
+    b = torch.sort(post[0][safe, :K - 1], dim=1).values
+    assert safe.numel() > 0 and torch.equal(a, b)
+
+
+def test_topk_bad_arguments():
+    p = dev(np.random.default_rng(0).random((64, 2)).astype(np.float32))
+    for K in (1, 9):
+        with pytest.raises(kc.KcError):
+            kc.kc_cert_allpairs_topk(p, K)
+    _, g_kc = geoms(p.cpu().numpy())
+    grid = kc.Grid(64, g_kc)
+    with pytest.raises(kc.RebuildRequired):
+        kc.kc_cert_grid_topk(grid, 3)
