@@ -583,6 +583,28 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
                                      points_per_s=Ncl / (t_clock * 1e-3))
         del cm
     ex["clock_loop"] = clock
+    # ---------------- NEXT #4: K-list certificates (K = 4): all-pairs pass and grid search
+    topk = {}
+    for cfg, n_sub in (("cfg2", None), ("cfg4", 131072)):
+        ck_ = wl.CONFIGS[cfg]
+        p = wl.make_points(cfg)
+        P = torch.from_numpy(p).to(dev)
+        Nk, dk_ = p.shape
+        K = 4
+        lo_hi = kc.kc_geom_for(P)
+        gk = kc.Grid(Nk, lo_hi)
+        kc.kc_grid_build(gk, P)
+        t_grid = _median_ms(torch, lambda: kc.kc_cert_grid_topk(gk, K), 5, flush=flush)
+        PA = P if n_sub is None else P[:n_sub].contiguous()
+        na = PA.shape[0]
+        t_ap = _median_ms(torch, lambda: kc.kc_cert_allpairs_topk(PA, K), 3, flush=flush)
+        ops = 5 if dk_ == 2 else 8
+        topk[cfg] = dict(K=K, N=Nk, grid_topk_ms=t_grid, grid_topk_points_per_s=Nk / (t_grid * 1e-3),
+                         allpairs_topk_N=na, allpairs_topk_ms=t_ap,
+                         allpairs_topk_pairs_per_s=na * (na - 1) / (t_ap * 1e-3),
+                         allpairs_topk_tflops=na * (na - 1) * ops / (t_ap * 1e-3) / 1e12)
+        del gk
+    ex["topk"] = topk
     # ---------------- config 5: 4,194,304 points, rebuild + Lemma-1 repair; all-pairs at 2^20
     for cfg in ("cfg5_d2", "cfg5_d3"):
         c5 = wl.CONFIGS[cfg]
