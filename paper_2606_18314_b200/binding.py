@@ -144,22 +144,28 @@ def _pos(p, name="p"):
 
 @dataclass
 class Certs:
-    """Device certificate arrays of Definition 1, indexed by point id."""
+    """Device certificate arrays of Definition 1, indexed by point id.  ``empty``
+    carves the five arrays out of one (5, N) int32 allocation (``buf``: rows nn, nn2, d1, d2, c), so
+    a caller can move a whole certificate set with one copy."""
     nn: torch.Tensor
     nn2: torch.Tensor
     d1: torch.Tensor
     d2: torch.Tensor
     c: torch.Tensor
+    buf: torch.Tensor | None = None
+
+    @staticmethod
+    def _views(buf):
+        return Certs(buf[0], buf[1], buf[2].view(torch.float32), buf[3].view(torch.float32),
+                     buf[4].view(torch.float32), buf)
 
     @staticmethod
     def empty(N, device="cuda"):
-        return Certs(torch.empty(N, dtype=torch.int32, device=device),
-                     torch.empty(N, dtype=torch.int32, device=device),
-                     torch.empty(N, dtype=torch.float32, device=device),
-                     torch.empty(N, dtype=torch.float32, device=device),
-                     torch.empty(N, dtype=torch.float32, device=device))
+        return Certs._views(torch.empty((5, N), dtype=torch.int32, device=device))
 
     def clone(self):
+        if self.buf is not None:
+            return Certs._views(self.buf.clone())
         return Certs(self.nn.clone(), self.nn2.clone(), self.d1.clone(), self.d2.clone(), self.c.clone())
 
     def _ptrs(self):

@@ -59,11 +59,13 @@ class Maintainer:
         self.ap = kc.Certs.empty(N, dev) if allpairs else None
         self.flags = torch.empty(N, dtype=torch.uint8, device=dev)
         self.F = torch.empty(N, dtype=torch.int32, device=dev)
-        self.nF = torch.zeros(1, dtype=torch.int32, device=dev)
-        self.eps = torch.zeros(1, dtype=torch.float32, device=dev)
-        self.H = torch.zeros(1, dtype=torch.float64, device=dev)
-        self.m = torch.zeros(1, dtype=torch.int32, device=dev)
-        self.C = torch.zeros(1, dtype=torch.int32, device=dev)
+        # the step's scalar results share one 24-byte allocation (one device-to-host copy reads them all)
+        self.scalars = torch.zeros(24, dtype=torch.uint8, device=dev)
+        self.eps = self.scalars[0:4].view(torch.float32)
+        self.nF = self.scalars[4:8].view(torch.int32)
+        self.H = self.scalars[8:16].view(torch.float64)
+        self.m = self.scalars[16:20].view(torch.int32)
+        self.C = self.scalars[20:24].view(torch.int32)
         need = kc.lib().kc_cert_allpairs_workspace(N, self.d) if allpairs else 0
         self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
         self.p = p0
