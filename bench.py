@@ -26,7 +26,7 @@ from paper_2606_18314_b200 import workloads as wl  # noqa: E402
 
 METRIC = "certified_points_per_s"
 UNIT = "points/s"
-L2_FLUSH_BYTES = 256 << 20
+L2_FLUSH_BYTES = int(os.environ.get("KC_FLUSH_MB", "256")) << 20
 FP32_LANES = 148 * 128          # B200: 148 SMs x 128 FP32 lanes, one non-fused op / lane / clk
 # dram__bytes_read.sum + dram__bytes_write.sum of one allpairs_kernel launch, from the committed ncu
 # --set full capture of this command (profiles/r1e_allpairs_cfg2_full.txt); null for other workloads

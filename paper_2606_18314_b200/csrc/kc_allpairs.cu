@@ -18,13 +18,15 @@
 //     lanes that puts some lane on the insertion path in almost every step of a short chunk.
 #include <stdlib.h>
 
+#include <atomic>
+
 #include "kc_common.cuh"
 
 using namespace kc;
 
 namespace {
 
-constexpr int AP_TJ = 1024;   // candidates per shared-memory tile
+constexpr int AP_TJ = 1152;   // candidates per shared-memory tile (= one j-chunk of the N = 16,000 step: 18 units of AP_GRAN)
 constexpr int AP_SEED = 256;  // points scanned by the seed pass of a j-split launch
 constexpr int AP_GRAN = 64;   // chunk granularity of a j-split launch (a multiple of every step size 4*C4)
 constexpr int AP_RESIDENT = 12;   // CTAs of 128 threads an SM holds at the kernel's ~48 registers per thread
@@ -186,10 +188,31 @@ struct ApArgs {
     const int32_t *seed1, *seed2;   // two known points per query (e.g. its previous neighbours), or null
     Partial *part;               // j-split: partial lists [js][nq_host]; null: store certificates
     int32_t *redo, *n_redo;      // queries whose bound admitted fewer than two candidates
-    int32_t *tickets;            // j-split: chunks finished per query block (the last one merges)
+    u64 *tickets;                // j-split: (call generation << 32 | chunks finished) per query block
+    unsigned gen;                //   generation of this call (see take_ticket)
     int32_t *nn, *nn2;
     float *d1, *d2, *c;
 };
+
+// j-split: the CTA that finishes the last chunk of a query block merges the block's partial lists.
+// The counter needs no zeroing pass: a word is (generation << 32 | count); an arrival that finds
+// another generation in it (an earlier call, or memory never written) restarts the count, and the
+// last arrival leaves (generation, 0) behind, so a replay of the same launch from a CUDA graph
+// (same generation) starts clean as well.  Returns true for the last of `total` arrivals.
+__device__ __forceinline__ bool take_ticket(u64 *t, unsigned gen, unsigned total)
+{
+    const u64 fresh = (u64)gen << 32;
+    u64 cur = *reinterpret_cast<volatile u64 *>(t), nw;
+    for (;;) {
+        nw = ((cur >> 32) == gen ? cur : fresh) + 1;
+        const u64 prev = atomicCAS(t, cur, nw);
+        if (prev == cur) break;
+        cur = prev;
+    }
+    const bool last = (unsigned)nw == total;
+    if (last) *reinterpret_cast<volatile u64 *>(t) = fresh;
+    return last;
+}
 
 // grid = (ceil(nq / (QPT*THREADS)), JS).
 template <int D, int QPT, int C4, int THREADS>
@@ -224,6 +247,24 @@ allpairs_kernel(const ApArgs a)
                 best[k].s1 = __int_as_float(raw.x); best[k].s2 = __int_as_float(raw.y);
                 best[k].j1 = raw.z; best[k].j2 = raw.w;
             }
+            if (a.seed1) {
+                // kc_cert_allpairs_seeded: the exact keys, at the CURRENT positions, of two known
+                // points (e.g. the previous neighbours).  Two distinct points other than i at
+                // squared distances s_a <= s_b prove s2_i <= s_b, so this start can never be
+                // wrong; ids out of range, equal to i or to each other are dropped, and a NaN
+                // coordinate seeds nothing.  Every chunk of a j-split starts from the same two.
+                const int ids[2] = {a.seed1[i], a.seed2[i]};
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int j = ids[e];
+                    if (j >= 0 && j < a.N && j != i && j != best[k].j1) {
+                        const float s = D == 2 ? sqd2(qx[k], qy[k], p[(int64_t)j * D], p[(int64_t)j * D + 1])
+                                               : sqd3(qx[k], qy[k], qz[k], p[(int64_t)j * D], p[(int64_t)j * D + 1],
+                                                      p[(int64_t)j * D + 2]);
+                        if (s == s) best[k].offer(s, j);
+                    }
+                }
+            }
             if (a.bound_d2) {
                 // start from two placeholders (T, no index): candidates beyond T are never
                 // inserted; T is inflated by 2^-9, far above every rounding on the way
@@ -249,7 +290,7 @@ allpairs_kernel(const ApArgs a)
         __shared__ int s_last;
         __threadfence();
         __syncthreads();
-        if (threadIdx.x == 0) s_last = atomicAdd(&a.tickets[blockIdx.x], 1) == (int)gridDim.y - 1;
+        if (threadIdx.x == 0) s_last = take_ticket(&a.tickets[blockIdx.x], a.gen, gridDim.y);
         __syncthreads();
         if (!s_last) return;
         __threadfence();
@@ -333,41 +374,6 @@ allpairs_seed_kernel(const ApArgs a, int S, Partial *__restrict__ seed)
     }
 }
 
-// Seeds from two known points per query (kc_cert_allpairs_seeded): their exact keys at the
-// CURRENT positions.  Two distinct points other than i at squared distances s_a <= s_b prove
-// s2_i <= s_b, so the list (s_a, a), (s_b, b) is a valid start that nothing in the pass can
-// invalidate; ids that are out of range, equal to i or to each other are dropped (cold start).
-template <int D>
-__global__ void __launch_bounds__(256)
-allpairs_idseed_kernel(const ApArgs a, Partial *__restrict__ seed, int n_head_words)
-{
-    const float *__restrict__ p = a.p;
-    const int64_t nq = a.nq_dev ? (int64_t)*a.nq_dev : a.nq_host;
-    const int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    // this kernel runs right before the pass: it also zeroes the pass's tickets and redo counter
-    // (saves the memset node of the other start modes)
-    if (q < n_head_words) reinterpret_cast<int32_t *>(a.n_redo)[q] = 0;
-    if (q >= nq) return;
-    const int i = a.qlist ? a.qlist[q] : (int)q;
-    const float qx = p[(int64_t)i * D], qy = p[(int64_t)i * D + 1];
-    const float qz = D == 3 ? p[(int64_t)i * D + 2] : 0.f;
-    Top2 t;
-    t.init();
-    const int ids[2] = {a.seed1[i], a.seed2[i]};
-#pragma unroll
-    for (int k = 0; k < 2; ++k) {
-        const int j = ids[k];
-        if (j >= 0 && j < a.N && j != i && j != t.j1) {
-            const float s = D == 2 ? sqd2(qx, qy, p[(int64_t)j * D], p[(int64_t)j * D + 1])
-                                   : sqd3(qx, qy, qz, p[(int64_t)j * D], p[(int64_t)j * D + 1], p[(int64_t)j * D + 2]);
-            if (s == s) t.offer(s, j);         // a NaN coordinate seeds nothing
-        }
-    }
-    Partial o;
-    o.s1 = t.s1; o.s2 = t.s2; o.j1 = t.j1; o.j2 = t.j2;
-    seed[q] = o;
-}
-
 // Redo pass of a bounded launch: the queries whose bound admitted fewer than two candidates (a
 // bound that was not one) are recomputed from scratch, one CTA per query, so that the result
 // never depends on the bound.  Empty in normal operation.
@@ -448,16 +454,16 @@ Shape choose_shape(int64_t nq, int64_t N)
     return s;
 }
 
-// Workspace layout: [n_redo: 16 B][tickets: one int32 per query block, padded to 16 B]
+// Workspace layout: [n_redo: 16 B][tickets: one 8-byte word per query block, padded to 16 B]
 // [redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last only for a j-split
-// shape).  n_redo and the tickets are zeroed by one memset per call.
+// shape).  n_redo is zeroed by a memset in a bounded call; the tickets need none (take_ticket).
 size_t pad16(size_t b) { return (b + 15) & ~(size_t)15; }
 size_t qblocks_for(int64_t nq, const Shape &sh)
 {
     const int64_t per = (int64_t)sh.qpt * sh.threads;
     return (size_t)((nq + per - 1) / per);
 }
-size_t head_bytes(int64_t nq, const Shape &sh) { return 16 + pad16(4 * qblocks_for(nq, sh)); }
+size_t head_bytes(int64_t nq, const Shape &sh) { return 16 + pad16(8 * qblocks_for(nq, sh)); }
 size_t workspace_bytes_for(int64_t nq, const Shape &sh)
 {
     return head_bytes(nq, sh) + pad16((size_t)nq * 4) + (size_t)nq * sizeof(Partial) +
@@ -479,12 +485,13 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     const bool split = sh.js > 1, bounded = a.bound_d2 != nullptr;
     a.one2 = 0x3f8000003f800000ull;
     a.n_redo = reinterpret_cast<int32_t *>(ws);
-    a.tickets = reinterpret_cast<int32_t *>(ws + 16);
+    a.tickets = reinterpret_cast<u64 *>(ws + 16);
+    static std::atomic<unsigned> generation{1};
+    a.gen = generation.fetch_add(1, std::memory_order_relaxed);
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
     const bool idseed = a.seed1 != nullptr;
-    const int n_head_words = (int)((split ? head_bytes(nq, sh) : 16) / 4);     // n_redo + tickets
-    if ((split || bounded) && !idseed) KC_CUDA(cudaMemsetAsync(ws, 0, (size_t)n_head_words * 4, st));
+    if (bounded) KC_CUDA(cudaMemsetAsync(ws, 0, 16, st));
     a.jfirst = split && !bounded && !idseed ? AP_SEED : 0;
     int js = sh.js;
     int64_t jchunk;
@@ -502,11 +509,7 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.part = split ? seed + nq : nullptr;
     int launches = 1;
     if (idseed) {
-        const int64_t nthr = nq > n_head_words ? nq : n_head_words;
-        if (D == 2) allpairs_idseed_kernel<2><<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(a, seed, n_head_words);
-        else allpairs_idseed_kernel<3><<<(unsigned)((nthr + 255) / 256), 256, 0, st>>>(a, seed, n_head_words);
-        a.seed = seed;
-        ++launches;
+        // seeds are computed in the pass itself
     } else if (split && !bounded) {
         const int blocks = (int)((nq + 7) / 8 < 148 * 8 ? (nq + 7) / 8 : 148 * 8);
         if (D == 2) allpairs_seed_kernel<2><<<blocks, 256, 0, st>>>(a, (int)a.jfirst, seed);
