@@ -193,6 +193,40 @@ def test_allpairs_seeded_is_exact_for_any_seeds(cfg, N):
         assert_same(got, want, what=f"seeded allpairs {cfg} seeds={name}")
 
 
+@pytest.mark.parametrize("cfg,N", [("cfg2", 16000), ("cfg3", 5000)])
+def test_allpairs_workspace_needs_no_initialisation(cfg, N):
+    """The j-split tickets carry the call's generation, so a workspace that holds arbitrary bytes
+    (never zeroed, or left by another start mode, another N, or a replayed CUDA graph) is fine:
+    cold, bounded, seeded and query-subset calls back to back on the same dirty workspace."""
+    p = wl.make_points(cfg, N=N)
+    want = ref_certs(p)
+    P = dev(p)
+    need = max(kc.lib().kc_cert_allpairs_workspace(N, p.shape[1]),
+               kc.lib().kc_frontier_oracle_workspace(N, p.shape[1], N))
+    gen = torch.Generator(device="cuda").manual_seed(5)
+    ws = torch.randint(0, 256, (need + 64,), dtype=torch.uint8, device="cuda", generator=gen)
+    eps = dev(np.array([1e-4], np.float32))
+    for rnd in range(3):
+        assert_same(kc.kc_cert_allpairs(P, workspace=ws), want, what=f"cold, dirty workspace, round {rnd}")
+        assert_same(kc.kc_cert_allpairs(P, workspace=ws, seed1=dev(want.nn), seed2=dev(want.nn2)), want,
+                    what=f"seeded, dirty workspace, round {rnd}")
+        assert_same(kc.kc_cert_allpairs(P, workspace=ws, d2_prev=dev(want.d2), eps=eps), want,
+                    what=f"bounded, dirty workspace, round {rnd}")
+        ws[: 16 + 8 * 4096] = torch.randint(0, 256, (16 + 8 * 4096,), dtype=torch.uint8, device="cuda", generator=gen)
+    # the same launch replayed from a CUDA graph (same generation every replay)
+    out = kc.Certs.empty(N)
+    s1, s2 = dev(want.nn), dev(want.nn2)
+    kc.kc_cert_allpairs(P, out, ws, seed1=s1, seed2=s2)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        kc.kc_cert_allpairs(P, out, ws, seed1=s1, seed2=s2)
+    for rnd in range(4):
+        out.buf.zero_()
+        g.replay()
+        assert_same(out, want, what=f"graph replay {rnd}")
+
+
 def test_grid_with_points_outside_the_box():
     # geometry fitted to the central half of the points: the rest is clamped into boundary cells
     p = wl.uniform_points(20000, 3, 31)
