@@ -643,7 +643,7 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
         n_ap = 1 << 20
         PA = P[:n_ap].contiguous()
         ap = kc.Certs.empty(n_ap, dev)
-        ws = torch.empty(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
+        ws = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
         t_ap = _median_ms(torch, lambda: kc.kc_cert_allpairs(PA, ap, ws), 2, flush=flush)
         ops = 5 if d == 2 else 8
         ex[cfg] = dict(N=N, grid_build_ms=t_build, rebuild_ms=t_reb, rebuild_points_per_s=N / (t_reb * 1e-3),

@@ -102,7 +102,15 @@ kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d,
                               void *stream);
 
 /* ---- A1: exact all-pairs certificates ("exact N x N pass", Table 2) ---------- */
-/* Workspace the tiled kernel needs for (N, d), in bytes (host; 0 only for invalid arguments). */
+/* Workspace the tiled kernel needs for (N, d), in bytes (host; 0 only for invalid arguments).
+ * WORKSPACE CONTRACT (all kc_cert_allpairs* entry points and kc_frontier_oracle): the caller
+ * zero-fills a workspace ONCE, when it is allocated (cudaMemset, torch.zeros); after that it may be
+ * passed to any sequence of these calls, for any N, d and start mode, one call at a time (calls on
+ * one stream, or otherwise ordered).  Its first 16 + KC_AP_TICKET_BYTES bytes hold the counters of
+ * the split launches and nothing else; every call leaves them zero, so no call spends a launch on
+ * clearing them.  A counter value that a clean workspace cannot hold stops the kernel (the call
+ * after it reports KC_ECUDA) instead of producing a wrong merge. */
+#define KC_AP_TICKET_BYTES (148 * 8 * 8 * 4)
 size_t kc_cert_allpairs_workspace(int64_t N, int d);
 /* nn,d1,d2,c: device [N]; nn2 device [N] or NULL; workspace: device, 16-byte aligned, >= the size
  * above. */

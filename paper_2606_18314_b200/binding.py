@@ -217,13 +217,15 @@ def kc_max_displacement(p, p2, eps_out=None):
 _ws_cache = {}
 
 
-def _workspace(nbytes, device):
+def _workspace(nbytes, device, kind="allpairs"):
+    """Cached scratch per device and purpose.  The all-pairs workspace is zero-filled once and then
+    only ever passed to the all-pairs entry points (workspace contract, kc.h)."""
     if nbytes == 0:
         return None
-    key = str(device)
+    key = (str(device), kind)
     w = _ws_cache.get(key)
     if w is None or w.numel() < nbytes:
-        w = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        w = torch.zeros(nbytes, dtype=torch.uint8, device=device)
         _ws_cache[key] = w
     return w
 
@@ -346,7 +348,7 @@ def kc_cert_allpairs_topk(p, K: int, workspace=None):
     pp, N, d = _pos(p)
     nnk, dk, ck = _topk_out(N, K, p.device)
     need = lib().kc_cert_allpairs_topk_workspace(N, d, K)
-    ws = workspace if workspace is not None else _workspace(need, p.device)
+    ws = workspace if workspace is not None else _workspace(need, p.device, "topk")
     _check(lib().kc_cert_allpairs_topk(pp, N, d, K, _ptr(nnk), _ptr(dk), _ptr(ck), _ptr(ws),
                                        ws.numel() if ws is not None else 0, _stream()), "kc_cert_allpairs_topk")
     return nnk, dk, ck

@@ -18,8 +18,6 @@
 //     lanes that puts some lane on the insertion path in almost every step of a short chunk.
 #include <stdlib.h>
 
-#include <atomic>
-
 #include "kc_common.cuh"
 
 using namespace kc;
@@ -29,6 +27,7 @@ namespace {
 constexpr int AP_TJ = 1152;   // candidates per shared-memory tile (= one j-chunk of the N = 16,000 step: 18 units of AP_GRAN)
 constexpr int AP_SEED = 256;  // points scanned by the seed pass of a j-split launch
 constexpr int AP_GRAN = 64;   // chunk granularity of a j-split launch (a multiple of every step size 4*C4)
+constexpr int AP_TICKETS = 148 * 8 * 8;   // a j-split launch has fewer query blocks than this (choose_shape)
 constexpr int AP_RESIDENT = 12;   // CTAs of 128 threads an SM holds at the kernel's ~48 registers per thread
 
 struct Partial { float s1, s2; int j1, j2; };   // 16 B
@@ -188,29 +187,22 @@ struct ApArgs {
     const int32_t *seed1, *seed2;   // two known points per query (e.g. its previous neighbours), or null
     Partial *part;               // j-split: partial lists [js][nq_host]; null: store certificates
     int32_t *redo, *n_redo;      // queries whose bound admitted fewer than two candidates
-    u64 *tickets;                // j-split: (call generation << 32 | chunks finished) per query block
-    unsigned gen;                //   generation of this call (see take_ticket)
+    int32_t *tickets;            // j-split: chunks finished per query block (the last one merges and re-zeroes)
     int32_t *nn, *nn2;
     float *d1, *d2, *c;
 };
 
 // j-split: the CTA that finishes the last chunk of a query block merges the block's partial lists.
-// The counter needs no zeroing pass: a word is (generation << 32 | count); an arrival that finds
-// another generation in it (an earlier call, or memory never written) restarts the count, and the
-// last arrival leaves (generation, 0) behind, so a replay of the same launch from a CUDA graph
-// (same generation) starts clean as well.  Returns true for the last of `total` arrivals.
-__device__ __forceinline__ bool take_ticket(u64 *t, unsigned gen, unsigned total)
+// The counters live in a fixed area at the head of the workspace that holds nothing else, start
+// at zero (workspace contract, kc.h) and are put back to zero by the last arrival, so no call has
+// to clear them (a memset node or a kernel in front of the pass costs 3-5 us of a 70 us launch).
+// A count that cannot occur in a clean area stops the kernel instead of merging garbage.
+__device__ __forceinline__ bool take_ticket(int32_t *t, int total)
 {
-    const u64 fresh = (u64)gen << 32;
-    u64 cur = *reinterpret_cast<volatile u64 *>(t), nw;
-    for (;;) {
-        nw = ((cur >> 32) == gen ? cur : fresh) + 1;
-        const u64 prev = atomicCAS(t, cur, nw);
-        if (prev == cur) break;
-        cur = prev;
-    }
-    const bool last = (unsigned)nw == total;
-    if (last) *reinterpret_cast<volatile u64 *>(t) = fresh;
+    const int old = atomicAdd(t, 1);
+    if (old < 0 || old >= total) __trap();      // the workspace was not zero-initialised
+    const bool last = old == total - 1;
+    if (last) atomicExch(t, 0);
     return last;
 }
 
@@ -290,7 +282,7 @@ allpairs_kernel(const ApArgs a)
         __shared__ int s_last;
         __threadfence();
         __syncthreads();
-        if (threadIdx.x == 0) s_last = take_ticket(&a.tickets[blockIdx.x], a.gen, gridDim.y);
+        if (threadIdx.x == 0) s_last = take_ticket(&a.tickets[blockIdx.x], (int)gridDim.y);
         __syncthreads();
         if (!s_last) return;
         __threadfence();
@@ -450,20 +442,22 @@ Shape choose_shape(int64_t nq, int64_t N)
     if (e_js > 0) js = e_js;
     if (js < 1) js = 1;
     if (js > 65535) js = 65535;
+    if (itiles > AP_TICKETS) js = 1;             // the ticket area holds AP_TICKETS query blocks
     s.js = (int)js;
     return s;
 }
 
-// Workspace layout: [n_redo: 16 B][tickets: one 8-byte word per query block, padded to 16 B]
-// [redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last only for a j-split
-// shape).  n_redo is zeroed by a memset in a bounded call; the tickets need none (take_ticket).
+// Workspace layout: [n_redo: 16 B][tickets: AP_TICKETS int32, a fixed area that holds nothing
+// else][redo ids: nq int32, padded to 16 B][seed: nq][part: js x nq] (the last only for a j-split
+// shape).  n_redo is zeroed by a memset in a bounded call; the tickets are zero between calls
+// (take_ticket; the caller zero-fills a new workspace once, kc.h).
 size_t pad16(size_t b) { return (b + 15) & ~(size_t)15; }
 size_t qblocks_for(int64_t nq, const Shape &sh)
 {
     const int64_t per = (int64_t)sh.qpt * sh.threads;
     return (size_t)((nq + per - 1) / per);
 }
-size_t head_bytes(int64_t nq, const Shape &sh) { return 16 + pad16(8 * qblocks_for(nq, sh)); }
+size_t head_bytes(int64_t, const Shape &) { return 16 + (size_t)AP_TICKETS * 4; }
 size_t workspace_bytes_for(int64_t nq, const Shape &sh)
 {
     return head_bytes(nq, sh) + pad16((size_t)nq * 4) + (size_t)nq * sizeof(Partial) +
@@ -485,9 +479,7 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     const bool split = sh.js > 1, bounded = a.bound_d2 != nullptr;
     a.one2 = 0x3f8000003f800000ull;
     a.n_redo = reinterpret_cast<int32_t *>(ws);
-    a.tickets = reinterpret_cast<u64 *>(ws + 16);
-    static std::atomic<unsigned> generation{1};
-    a.gen = generation.fetch_add(1, std::memory_order_relaxed);
+    a.tickets = reinterpret_cast<int32_t *>(ws + 16);
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
     const bool idseed = a.seed1 != nullptr;

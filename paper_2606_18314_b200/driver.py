@@ -67,7 +67,7 @@ class Maintainer:
         self.m = self.scalars[16:20].view(torch.int32)
         self.C = self.scalars[20:24].view(torch.int32)
         need = kc.lib().kc_cert_allpairs_workspace(N, self.d) if allpairs else 0
-        self.ws = torch.empty(max(need, 16), dtype=torch.uint8, device=dev)
+        self.ws = torch.zeros(max(need, 16), dtype=torch.uint8, device=dev)   # zero-filled once (kc.h)
         self.p = p0
         kc.kc_cert_grid_rebuild(self.grid, p0, self.certs)
 

@@ -194,26 +194,32 @@ def test_allpairs_seeded_is_exact_for_any_seeds(cfg, N):
 
 
 @pytest.mark.parametrize("cfg,N", [("cfg2", 16000), ("cfg3", 5000)])
-def test_allpairs_workspace_needs_no_initialisation(cfg, N):
-    """The j-split tickets carry the call's generation, so a workspace that holds arbitrary bytes
-    (never zeroed, or left by another start mode, another N, or a replayed CUDA graph) is fine:
-    cold, bounded, seeded and query-subset calls back to back on the same dirty workspace."""
+def test_allpairs_workspace_is_reusable(cfg, N):
+    """Workspace contract (kc.h): zero-filled once, then any sequence of start modes and sizes on
+    the same workspace — cold, seeded, bounded, a query subset, another N, everything beyond the
+    ticket area scribbled over in between — and the same launch replayed from a CUDA graph."""
     p = wl.make_points(cfg, N=N)
+    d = p.shape[1]
     want = ref_certs(p)
-    P = dev(p)
-    need = max(kc.lib().kc_cert_allpairs_workspace(N, p.shape[1]),
-               kc.lib().kc_frontier_oracle_workspace(N, p.shape[1], N))
+    small = np.ascontiguousarray(p[: N // 3])
+    want_small = ref_certs(small)
+    P, S = dev(p), dev(small)
+    need = max(kc.lib().kc_cert_allpairs_workspace(N, d), kc.lib().kc_frontier_oracle_workspace(N, d, N))
+    ws = torch.zeros(need + 64, dtype=torch.uint8, device="cuda")
     gen = torch.Generator(device="cuda").manual_seed(5)
-    ws = torch.randint(0, 256, (need + 64,), dtype=torch.uint8, device="cuda", generator=gen)
     eps = dev(np.array([1e-4], np.float32))
+    head = 16 + 148 * 8 * 8 * 4                                   # KC_AP_TICKET_BYTES + 16
+    q = np.sort(np.random.default_rng(2).choice(N, N // 7, replace=False)).astype(np.int32)
     for rnd in range(3):
-        assert_same(kc.kc_cert_allpairs(P, workspace=ws), want, what=f"cold, dirty workspace, round {rnd}")
+        assert_same(kc.kc_cert_allpairs(P, workspace=ws), want, what=f"cold, round {rnd}")
+        assert_same(kc.kc_cert_allpairs(S, workspace=ws), want_small, what=f"cold, other N, round {rnd}")
         assert_same(kc.kc_cert_allpairs(P, workspace=ws, seed1=dev(want.nn), seed2=dev(want.nn2)), want,
-                    what=f"seeded, dirty workspace, round {rnd}")
-        assert_same(kc.kc_cert_allpairs(P, workspace=ws, d2_prev=dev(want.d2), eps=eps), want,
-                    what=f"bounded, dirty workspace, round {rnd}")
-        ws[: 16 + 8 * 4096] = torch.randint(0, 256, (16 + 8 * 4096,), dtype=torch.uint8, device="cuda", generator=gen)
-    # the same launch replayed from a CUDA graph (same generation every replay)
+                    what=f"seeded, round {rnd}")
+        ws[head:] = torch.randint(0, 256, (ws.numel() - head,), dtype=torch.uint8, device="cuda", generator=gen)
+        assert_same(kc.kc_cert_allpairs(P, workspace=ws, d2_prev=dev(want.d2), eps=eps), want, what=f"bounded, round {rnd}")
+        out = kc.Certs.empty(N)
+        kc.kc_frontier_oracle(P, dev(q), dev(np.array([q.size], np.int32)), out, workspace=ws)
+        assert_same(out, want, idx=q, what=f"query subset, round {rnd}")
     out = kc.Certs.empty(N)
     s1, s2 = dev(want.nn), dev(want.nn2)
     kc.kc_cert_allpairs(P, out, ws, seed1=s1, seed2=s2)
