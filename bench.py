@@ -30,7 +30,7 @@ L2_FLUSH_BYTES = int(os.environ.get("KC_FLUSH_MB", "256")) << 20
 FP32_LANES = 148 * 128          # B200: 148 SMs x 128 FP32 lanes, one non-fused op / lane / clk
 # dram__bytes_read.sum + dram__bytes_write.sum of one allpairs_kernel launch, from the committed ncu
 # --set full capture of this command (profiles/r1e_allpairs_cfg2_full.txt); null for other workloads
-AP_TRAFFIC_BYTES = {("cfg2", 16000): 405504}
+AP_TRAFFIC_BYTES = {("cfg2", 16000): 279552}   # profiles/r1f_allpairs_cfg2_full.txt: dram read + write per launch
 
 
 def log(*a):
