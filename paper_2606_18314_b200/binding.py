@@ -145,8 +145,8 @@ def _pos(p, name="p"):
 @dataclass
 class Certs:
     """Device certificate arrays of Definition 1, indexed by point id.  ``empty``
-    carves the five arrays out of one (5, N) int32 allocation (``buf``: rows nn, nn2, d1, d2, c), so
-    a caller can move a whole certificate set with one copy."""
+    carves the five arrays out of one (5, N) int32 allocation (``buf``: rows nn, d1, d2, c, nn2), so
+    a caller can move a certificate set with one copy (``buf[:4]`` without the runner-up index)."""
     nn: torch.Tensor
     nn2: torch.Tensor
     d1: torch.Tensor
@@ -156,8 +156,8 @@ class Certs:
 
     @staticmethod
     def _views(buf):
-        return Certs(buf[0], buf[1], buf[2].view(torch.float32), buf[3].view(torch.float32),
-                     buf[4].view(torch.float32), buf)
+        return Certs(buf[0], buf[4], buf[1].view(torch.float32), buf[2].view(torch.float32),
+                     buf[3].view(torch.float32), buf)
 
     @staticmethod
     def empty(N, device="cuda"):
