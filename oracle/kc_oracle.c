@@ -18,7 +18,10 @@
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): hand-worked dyadic scenes
  * (tests/golden/), Theorem-1 tightness construction, lattice
  * closed forms, entropy closed forms, Theorem 3, Lemma 1 invariant, brute
- * force vs k-d tree vs scipy fp64.  No function here is "parity unpinned".
+ * force vs k-d tree vs scipy fp64; the K-list certificate (orc_bruteforce_topk)
+ * by hand-worked lists with bit patterns, a numpy lexsort restatement, K = 2 =
+ * Definition 1 and the stability of the (K-1)-NN set beyond 4 eps.  No function
+ * here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
