@@ -600,6 +600,20 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
                          allpairs_topk_tflops=na * (na - 1) * ops / (t_ap * 1e-3) / 1e12)
         del gk
     ex["topk"] = topk
+    # ---------------- the sizes of the paper's Table 2 (54 ... 2,095 ms on an RTX PRO 6000,
+    # 30 -> 19 G pairs/s; context, another machine): one cold all-pairs pass per N, uniform points
+    t2 = {}
+    for dd in (2, 3):
+        rows = []
+        for n2 in (40000, 80000, 120000, 160000, 200000):
+            PT = torch.from_numpy(wl.uniform_points(n2, dd, 1000 + n2 // 1000 + dd)).to(dev)
+            out2 = kc.Certs.empty(n2, dev)
+            ws2 = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n2, dd)), dtype=torch.uint8, device=dev)
+            t_ms = _median_ms(torch, lambda: kc.kc_cert_allpairs(PT, out2, ws2), 3, flush=flush)
+            rows.append(dict(N=n2, ms=t_ms, pairs_per_s=n2 * (n2 - 1) / (t_ms * 1e-3),
+                             resident_bytes=int(PT.numel() * 4 + out2.buf.numel() * 4 + ws2.numel())))
+        t2[f"d{dd}"] = rows
+    ex["table2_sizes"] = t2
     # ---------------- config 5: 4,194,304 points, rebuild + Lemma-1 repair; all-pairs at 2^20
     for cfg in ("cfg5_d2", "cfg5_d3"):
         c5 = wl.CONFIGS[cfg]
