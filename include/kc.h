@@ -276,14 +276,18 @@ kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const in
  * 2 <= K <= KC_TOPK_MAX.  All pointers device, caller-owned: nnk int32[N*K], dk float32[N*K],
  * ck float32[N], row-major.  kc_cert_allpairs_topk: tiled N x N pass (FP32 ALU bound);
  * workspace: device scratch of at least kc_cert_allpairs_topk_workspace(N, d, K) bytes (0 for
- * large N), 4-byte aligned.  kc_cert_grid_topk: ring-expanding search of a freshly built grid,
+ * large N), 4-byte aligned; seed_ids: NULL, or device int32[N*K] with K known points per query
+ * (its list from the grid or from the previous step): the pass starts every list from their exact
+ * keys at the current positions, which can never make a result wrong (reading R17 for K keys);
+ * ANY ids are allowed (out of range, i itself and repeats are ignored); must not alias nnk.
+ * kc_cert_grid_topk: ring-expanding search of a freshly built grid,
  * terminating only when the scanned block's bound exceeds the K-th distance (KC_EREBUILD if the
  * grid was updated incrementally since its build).  Asynchronous on `stream`; KC_EINVAL on a NULL
  * pointer, K out of range, N < 2 or d not in {2,3}. */
 #define KC_TOPK_MAX 8
 size_t kc_cert_allpairs_topk_workspace(int64_t N, int d, int K);
-kc_status kc_cert_allpairs_topk(const float *p, int64_t N, int d, int K, int32_t *nnk, float *dk, float *ck,
-                                void *workspace, size_t workspace_bytes, void *stream);
+kc_status kc_cert_allpairs_topk(const float *p, int64_t N, int d, int K, const int32_t *seed_ids, int32_t *nnk,
+                                float *dk, float *ck, void *workspace, size_t workspace_bytes, void *stream);
 kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *dk, float *ck, void *stream);
 
 /* ---- inspection (tests, reports) ---------------------------------------------------------- */

@@ -101,7 +101,7 @@ def lib():
     L.kc_frontier_classify_local.argtypes = [vp, vp, vp, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     L.kc_cert_allpairs_topk_workspace.restype = sz
     L.kc_cert_allpairs_topk_workspace.argtypes = [i64, ci, ci]
-    L.kc_cert_allpairs_topk.argtypes = [vp, i64, ci, ci, vp, vp, vp, vp, sz, vp]
+    L.kc_cert_allpairs_topk.argtypes = [vp, i64, ci, ci, vp, vp, vp, vp, vp, sz, vp]
     L.kc_cert_grid_topk.argtypes = [vp, ci, vp, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
@@ -342,14 +342,18 @@ def _topk_out(N, K, device):
             torch.empty(N, dtype=torch.float32, device=device))
 
 
-def kc_cert_allpairs_topk(p, K: int, workspace=None):
+def kc_cert_allpairs_topk(p, K: int, workspace=None, seed_ids=None):
     """NEXT #4: K-list certificates by the tiled N x N pass (Definition 1 :29 with K
-    keys).  Returns (nnk int32[N,K], dk float32[N,K], ck float32[N])."""
+    keys).  ``seed_ids`` (int32[N,K], optional): K known points per query to start from.  Returns
+    (nnk int32[N,K], dk float32[N,K], ck float32[N])."""
     pp, N, d = _pos(p)
+    if seed_ids is not None and tuple(seed_ids.shape) != (N, K):
+        raise ValueError("seed_ids must be (N, K)")
     nnk, dk, ck = _topk_out(N, K, p.device)
     need = lib().kc_cert_allpairs_topk_workspace(N, d, K)
     ws = workspace if workspace is not None else _workspace(need, p.device, "topk")
-    _check(lib().kc_cert_allpairs_topk(pp, N, d, K, _ptr(nnk), _ptr(dk), _ptr(ck), _ptr(ws),
+    _check(lib().kc_cert_allpairs_topk(pp, N, d, K, _ptr(seed_ids, torch.int32, "seed_ids"), _ptr(nnk), _ptr(dk),
+                                       _ptr(ck), _ptr(ws),
                                        ws.numel() if ws is not None else 0, _stream()), "kc_cert_allpairs_topk")
     return nnk, dk, ck
 

@@ -452,11 +452,6 @@ Shape choose_shape(int64_t nq, int64_t N)
 // shape).  n_redo is zeroed by a memset in a bounded call; the tickets are zero between calls
 // (take_ticket; the caller zero-fills a new workspace once, kc.h).
 size_t pad16(size_t b) { return (b + 15) & ~(size_t)15; }
-size_t qblocks_for(int64_t nq, const Shape &sh)
-{
-    const int64_t per = (int64_t)sh.qpt * sh.threads;
-    return (size_t)((nq + per - 1) / per);
-}
 size_t head_bytes(int64_t, const Shape &) { return 16 + (size_t)AP_TICKETS * 4; }
 size_t workspace_bytes_for(int64_t nq, const Shape &sh)
 {

@@ -95,6 +95,13 @@ struct TopK {
 #pragma unroll
         for (int q = 0; q < K; ++q) { s[q] = CUDART_INF_F; j[q] = KC_NOIDX; }
     }
+    __device__ __forceinline__ bool holds(int id) const
+    {
+        bool h = false;
+#pragma unroll
+        for (int q = 0; q < K; ++q) h |= j[q] == id;
+        return h;
+    }
     __device__ __forceinline__ void offer(float x, int id)
     {
         if (!(x < s[K - 1] || (x == s[K - 1] && id < j[K - 1]))) return;

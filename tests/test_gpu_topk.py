@@ -121,3 +121,24 @@ def test_topk_bad_arguments():
     grid = kc.Grid(64, g_kc)
     with pytest.raises(kc.RebuildRequired):
         kc.kc_cert_grid_topk(grid, 3)
+
+
+@pytest.mark.parametrize("cfg", ["cfg2", "cfg3"])
+@pytest.mark.parametrize("K", [3, 6])
+def test_topk_seeded_is_exact_for_any_seeds(cfg, K):
+    """Seeds of the K-list N x N pass (reading R17 for K keys): the grid's lists, the previous
+    step's lists, the true lists shuffled, random ids and garbage all give the oracle's bits."""
+    p, mot = wl.make_scene(cfg)
+    q, _ = mot.step(p)
+    N = p.shape[0]
+    want = oracle.bruteforce_topk(q, K)
+    prev = oracle.bruteforce_topk(p, K)[0]
+    rng = np.random.default_rng(K)
+    garbage = rng.integers(-3, N + 3, (N, K)).astype(np.int32)
+    garbage[::2, 1] = garbage[::2, 0]                                   # repeats
+    garbage[::5, 2] = np.arange(N, dtype=np.int32)[::5]                 # the query itself
+    seeds = {"grid": grid_topk(q, K)[0], "previous": dev(prev), "true reversed": dev(want[0][:, ::-1].copy()),
+             "random": dev(rng.integers(0, N, (N, K)).astype(np.int32)), "garbage": dev(garbage),
+             "none": dev(np.full((N, K), -1, np.int32))}
+    for name, sd in seeds.items():
+        same(kc.kc_cert_allpairs_topk(dev(q), K, seed_ids=sd.contiguous()), want, f"seeded topk {cfg} K={K} seeds={name}")
