@@ -271,6 +271,36 @@ def test_frontier_oracle_subset():
             assert np.all(host(certs).nn[rest] == -7) and np.all(host(certs).c[rest] == -7.0)
 
 
+def test_empty_and_degenerate_frontiers():
+    """Empty id lists leave everything untouched (repair, frontier oracle, audit, entropy); a step that
+    moves nothing has eps = 0 and its frontier is exactly the points with c = 0 (ties, duplicates)."""
+    p = wl.make_points("cfg2", N=3000)
+    p[10] = p[11]                                             # a duplicate pair: d1 = 0
+    p[20], p[21], p[22] = (0.5, 0.5), (0.5 + 2.0 ** -8, 0.5), (0.5 - 2.0 ** -8, 0.5)   # point 20: d1 = d2
+    want = oracle.bruteforce_top2(p)
+    P = dev(p)
+    _, g_kc = geoms(p)
+    grid = kc.Grid(p.shape[0], g_kc)
+    certs = kc.kc_cert_grid_rebuild(grid, P)
+    assert_same(certs, want, what="degenerate scene")
+    eps = kc.kc_max_displacement(P, P)
+    flags, F, nF = kc.kc_frontier_classify(certs.c, eps)
+    wf, wF = oracle.frontier(want.c, np.float32(0))
+    assert float(eps.item()) == 0.0 and np.array_equal(flags.cpu().numpy(), wf)
+    assert int(nF.item()) == wF.size and 20 in wF and want.c[20] == 0
+    before = certs.clone()
+    zero = dev(np.array([0], np.int32))
+    nothing = dev(np.zeros(1, np.int32))                       # a valid pointer, zero entries
+    kc.kc_frontier_repair(grid, P, nothing, zero, certs)
+    kc.kc_frontier_oracle(P, nothing, zero, certs)
+    assert_same(certs, host(before), what="empty frontier leaves the certificates alone")
+    H, m, C = kc.kc_frontier_entropy(grid, nothing, zero)
+    assert float(H.item()) == 0.0 and int(m.item()) == 0 and int(C.item()) > 0
+    # the zero-motion frontier repaired in place gives the same certificates back
+    kc.kc_frontier_repair(grid, P, F, nF, certs)
+    assert_same(certs, want, what="repair of the c = 0 frontier")
+
+
 def test_max_displacement_and_classify():
     for cfg in ("cfg1", "cfg2", "cfg3"):
         for fam in wl.CONFIGS[cfg]["families"]:
