@@ -289,6 +289,14 @@ size_t kc_cert_allpairs_topk_workspace(int64_t N, int d, int K);
 kc_status kc_cert_allpairs_topk(const float *p, int64_t N, int d, int K, const int32_t *seed_ids, int32_t *nnk,
                                 float *dk, float *ck, void *workspace, size_t workspace_bytes, void *stream);
 kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *dk, float *ck, void *stream);
+/* A7 for K keys (Algorithm 1 lines 4-7, on K-list certificates): recompute the
+ * lists of the ids F[0..*nF) (device int32, *nF read on the device, at most nF_max) against the grid
+ * as kc_grid_update left it (p_new: the positions it holds, device [N][d]); rows F[k] of nnk, dk and
+ * entry F[k] of ck are overwritten, all others untouched.  With F = {i : ck_i <= 4 eps} the
+ * (K-1)-NN set of every other point is still valid (see above).  KC_EREBUILD if the grid was not
+ * built for this N. */
+kc_status kc_frontier_search_topk(kc_grid *g, const float *p_new, int64_t N, const int32_t *F, const int32_t *nF,
+                                  int64_t nF_max, int K, int32_t *nnk, float *dk, float *ck, void *stream);
 
 /* ---- inspection (tests, reports) ---------------------------------------------------------- */
 /* Synchronises `stream`, copies the device counters to *out (host). */

@@ -26,7 +26,7 @@ EXPORTS = (
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
     "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
-    "kc_cert_allpairs_topk_workspace", "kc_cert_allpairs_topk", "kc_cert_grid_topk",
+    "kc_cert_allpairs_topk_workspace", "kc_cert_allpairs_topk", "kc_cert_grid_topk", "kc_frontier_search_topk",
     "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
 
@@ -103,6 +103,7 @@ def lib():
     L.kc_cert_allpairs_topk_workspace.argtypes = [i64, ci, ci]
     L.kc_cert_allpairs_topk.argtypes = [vp, i64, ci, ci, vp, vp, vp, vp, vp, sz, vp]
     L.kc_cert_grid_topk.argtypes = [vp, ci, vp, vp, vp, vp]
+    L.kc_frontier_search_topk.argtypes = [vp, vp, i64, vp, vp, i64, ci, vp, vp, vp, vp]
     L.kc_grid_info.argtypes = [vp, C.POINTER(kc_grid_info_t), vp]
     L.kc_grid_export.argtypes = [vp, ci, vp, i64, C.POINTER(i64), vp]
     L.kc_fp32_probe.argtypes = [ci, ci, C.POINTER(C.c_double), vp]
@@ -365,6 +366,19 @@ def kc_cert_grid_topk(grid: Grid, K: int, device=None):
     nnk, dk, ck = _topk_out(grid.N, K, device or torch.device("cuda"))
     _check(lib().kc_cert_grid_topk(grid._h, K, _ptr(nnk), _ptr(dk), _ptr(ck), _stream()), "kc_cert_grid_topk")
     return nnk, dk, ck
+
+
+def kc_frontier_search_topk(grid: Grid, p_new, F, nF, lists, nF_max=None):
+    """A7 for K-list certificates: recompute rows F of ``lists`` = (nnk, dk, ck) against the updated
+    grid (call kc_grid_update first), in place."""
+    pp, N, d = _pos(p_new, "p_new")
+    nnk, dk, ck = lists
+    K = int(nnk.shape[1])
+    nF_max = int(F.numel() if nF_max is None else nF_max)
+    _check(lib().kc_frontier_search_topk(grid._h, pp, N, _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"),
+                                         nF_max, K, _ptr(nnk, torch.int32, "nnk"), _ptr(dk, torch.float32, "dk"),
+                                         _ptr(ck, torch.float32, "ck"), _stream()), "kc_frontier_search_topk")
+    return lists
 
 
 def kc_frontier_classify(c, eps, flags=None, F=None, nF=None):

@@ -1131,6 +1131,86 @@ search_topk_kernel(View v, int N, int32_t *__restrict__ nnk, float *__restrict__
     }
     best.store(self, nnk, dk, ck);
 }
+// K-list repair (A7 for K keys): one thread per id of the list, against the incrementally updated
+// grid: tombstones are inert records, the overflow chain of every visited cell is scanned too.
+template <int D, int K>
+__device__ __forceinline__ void topk_scan_chains(const View &v, int rowbase, int x0, int x1, float qx, float qy,
+                                                 float qz, int self, TopK<K> &best)
+{
+    for (int x = x0; x <= x1; ++x)
+        for (int e = v.head[rowbase + x]; e >= 0; e = v.next[e]) {
+            const float4 c = v.opos[e];
+            const float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
+            if (s <= best.s[K - 1] && e != self) best.offer(s, e);
+        }
+}
+template <int D, int K>
+__global__ void __launch_bounds__(128)
+search_topk_list_kernel(View v, const float *__restrict__ p_new, const int32_t *__restrict__ F,
+                        const int32_t *__restrict__ nF, const Counters *ctr, int32_t *__restrict__ nnk,
+                        float *__restrict__ dk, float *__restrict__ ck)
+{
+    const int n = *nF;
+    const bool chains = ctr->n_misfiled > 0;
+    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
+        const int self = F[f];
+        const float qx = p_new[(int64_t)self * D], qy = p_new[(int64_t)self * D + 1];
+        const float qz = D == 3 ? p_new[(int64_t)self * D + 2] : 0.f;
+        const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+        const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+        const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+        TopK<K> best;
+        best.init();
+        topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
+        if (chains) topk_scan_chains<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
+        for (int r = 0;;) {
+            int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+            int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
+            int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
+            if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
+            ++r;
+            z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+            y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
+            x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
+            for (int z = z0; z <= z1; ++z)
+                for (int y = y0; y <= y1; ++y) {
+                    const int rowbase = (z * v.G1 + y) * v.G0;
+                    const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
+                    if (shell) {
+                        topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
+                        if (chains) topk_scan_chains<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
+                    } else {
+                        if (cx - r >= 0) {
+                            topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
+                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
+                        }
+                        if (cx + r <= v.G0 - 1) {
+                            topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                        }
+                    }
+                }
+        }
+        best.store(self, nnk, dk, ck);
+    }
+}
+template <int D>
+bool dispatch_list_topk(int K, const View &v, const float *p_new, const int32_t *F, const int32_t *nF, int64_t nF_max,
+                        const Counters *ctr, int32_t *nnk, float *dk, float *ck, cudaStream_t st)
+{
+    int64_t want = (nF_max + 127) / 128;
+    const int nb = (int)(want < 1 ? 1 : (want < 148 * 16 ? want : 148 * 16));
+    switch (K) {
+    case 2: search_topk_list_kernel<D, 2><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 3: search_topk_list_kernel<D, 3><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 4: search_topk_list_kernel<D, 4><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 5: search_topk_list_kernel<D, 5><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 6: search_topk_list_kernel<D, 6><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 7: search_topk_list_kernel<D, 7><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    case 8: search_topk_list_kernel<D, 8><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
+    default: return false;
+    }
+}
 template <int D>
 bool dispatch_grid_topk(int K, const View &v, int n, int32_t *nnk, float *dk, float *ck, cudaStream_t st)
 {
@@ -1579,6 +1659,27 @@ extern "C" kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *d
     else dispatch_grid_topk<3>(K, v, (int)g->N, nnk, dk, ck, (cudaStream_t)stream);
     count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_topk");
+    return KC_OK;
+}
+
+extern "C" kc_status kc_frontier_search_topk(kc_grid *g, const float *p_new, int64_t N, const int32_t *F,
+                                             const int32_t *nF, int64_t nF_max, int K, int32_t *nnk, float *dk,
+                                             float *ck, void *stream)
+{
+    if (!g || !p_new || !F || !nF || nF_max < 0 || !nnk || !dk || !ck || K < 2 || K > KC_TOPK_MAX) {
+        set_error("kc_frontier_search_topk: bad argument (2 <= K <= %d)", KC_TOPK_MAX);
+        return KC_EINVAL;
+    }
+    if (!g->built || N != g->N) {
+        set_error("kc_frontier_search_topk: grid not built for this N");
+        return KC_EREBUILD;
+    }
+    if (nF_max == 0) return KC_OK;
+    const View v = make_view(g);
+    if (g->geom.d == 2) dispatch_list_topk<2>(K, v, p_new, F, nF, nF_max, g->ctr, nnk, dk, ck, (cudaStream_t)stream);
+    else dispatch_list_topk<3>(K, v, p_new, F, nF, nF_max, g->ctr, nnk, dk, ck, (cudaStream_t)stream);
+    count_launches(1);
+    KC_LAUNCH_CHECK("kc_frontier_search_topk");
     return KC_OK;
 }
 

@@ -85,6 +85,7 @@ def test_bad_arguments_are_rejected(L):
     assert L.kc_failure_audit(None, None, None, 100, None, None, None) == E
     assert L.kc_cert_allpairs_topk(None, 100, 2, 4, None, None, None, None, None, 0, None) == E
     assert L.kc_cert_grid_topk(None, 4, None, None, None, None) == E
+    assert L.kc_frontier_search_topk(None, None, 100, None, None, 10, 4, None, None, None, None) == E
     assert L.kc_cert_allpairs_topk_workspace(1000, 2, 9) == 0 and L.kc_cert_allpairs_topk_workspace(1000, 2, 4) > 0
     assert L.kc_grid_destroy(None) == binding.KC_OK and L.kc_grid_bytes(None) == 0
 

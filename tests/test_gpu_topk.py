@@ -142,3 +142,36 @@ def test_topk_seeded_is_exact_for_any_seeds(cfg, K):
              "none": dev(np.full((N, K), -1, np.int32))}
     for name, sd in seeds.items():
         same(kc.kc_cert_allpairs_topk(dev(q), K, seed_ids=sd.contiguous()), want, f"seeded topk {cfg} K={K} seeds={name}")
+
+
+@pytest.mark.parametrize("cfg,fam", [("cfg2", "walk"), ("cfg3", "cluster_drift"), ("cfg3", "ball5")])
+@pytest.mark.parametrize("K", [3, 5])
+def test_topk_frontier_repair(cfg, fam, K):
+    """The maintenance step on K-list certificates: eps_t, F = {ck <= 4 eps_t}, incremental cell
+    update, re-search of F only.  Rows F equal the oracle's new lists; every other point keeps a
+    valid (K-1)-NN set; several steps on the same grid, so overflow chains and tombstones build up."""
+    p, mot = wl.make_scene(cfg, fam)
+    N = p.shape[0]
+    _, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    kc.kc_grid_build(grid, dev(p))
+    lists = kc.kc_cert_grid_topk(grid, K)
+    same(lists, oracle.bruteforce_topk(p, K), f"{cfg}/{fam} K={K} initial lists")
+    for step in range(4):
+        q, _ = mot.step(p)
+        P, Q = dev(p), dev(q)
+        eps = kc.kc_max_displacement(P, Q)
+        flags, F, nF = kc.kc_frontier_classify(lists[2], eps)
+        kc.kc_grid_update(grid, Q)
+        kc.kc_frontier_search_topk(grid, Q, F, nF, lists)
+        want = oracle.bruteforce_topk(q, K)
+        fr = np.flatnonzero(flags.cpu().numpy())
+        assert fr.size == int(nF.item())
+        same(lists, tuple(w[fr] for w in want), f"{cfg}/{fam} K={K} step {step} at F", idx=fr)
+        rest = np.flatnonzero(flags.cpu().numpy() == 0)
+        a = np.sort(lists[0].cpu().numpy()[rest, :K - 1], axis=1)
+        b = np.sort(want[0][rest, :K - 1], axis=1)
+        assert np.array_equal(a, b)
+        # per-transition protocol (DESIGN.md R13): the next step starts from exact lists
+        lists = tuple(dev(w) for w in want)
+        p = q
