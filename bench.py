@@ -233,7 +233,7 @@ def run_gpu_arm(args):
 
     def do_step(f, t, timed):
         if use_graph:
-            return maint[f].step(dev_traj[f][t], time_allpairs=timed)
+            return maint[f].step(dev_traj[f][t], time_allpairs=timed, a_first=True)   # steps are queued back to back
         return maint[f].step(dev_traj[f][t], movers=dev_mv[f][t], time_phases=timed)
 
     phase_sum = {ph: 0.0 for ph in ("maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs")}

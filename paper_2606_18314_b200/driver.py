@@ -300,10 +300,14 @@ class GraphMaintainer:
         else:
             gb.replay()
 
-    def step(self, p_next: torch.Tensor | None, time_allpairs: bool = False) -> StepResult:
+    def step(self, p_next: torch.Tensor | None, time_allpairs: bool = False, a_first: bool = False) -> StepResult:
         """One transition; returns the same StepResult as Maintainer.step (no host sync).  With
         ``time_allpairs`` two CUDA events bracket the all-pairs graph (``self.ap_events``).
-        ``p_next`` None: the caller has already written the new positions into next_buffer()."""
+        ``p_next`` None: the caller has already written the new positions into next_buffer().
+        ``a_first``: replay graph A before graph B.  The N x N pass takes every CTA slot once it is
+        resident, so A's first kernels should be in before it; worth ~2 us when the host runs ahead
+        of the device (steps queued back to back), but when every step is synchronised the host-side
+        launch of the 20-node graph A then delays the pass, so the default launches B first."""
         k, m = self.k, self.m
         if p_next is not None:
             self.pos[1 - k].copy_(p_next, non_blocking=True)
@@ -314,9 +318,12 @@ class GraphMaintainer:
         main = torch.cuda.current_stream()
         if self.overlap:
             self.side_ap.wait_stream(main)
+            if a_first:
+                ga.replay()
             with torch.cuda.stream(self.side_ap):
                 self._replay_b(gb, time_allpairs)
-            ga.replay()
+            if not a_first:
+                ga.replay()
             main.wait_stream(self.side_ap)
         else:
             ga.replay()
