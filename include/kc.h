@@ -108,8 +108,12 @@ kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d,
  * passed to any sequence of these calls, for any N, d and start mode, one call at a time (calls on
  * one stream, or otherwise ordered).  Its first 16 + KC_AP_TICKET_BYTES bytes hold the counters of
  * the split launches and nothing else; every call leaves them zero, so no call spends a launch on
- * clearing them.  A counter value that a clean workspace cannot hold stops the kernel (the call
- * after it reports KC_ECUDA) instead of producing a wrong merge. */
+ * clearing them.  A counter value that a zero-filled workspace cannot hold never reaches a merge:
+ * the kernel reports it through a per-process error word in pinned host memory (no trap, the CUDA
+ * context stays usable), leaves the certificates of that query block unspecified, and the NEXT
+ * all-pairs call of the process returns KC_EINVAL without running, after clearing the counters of
+ * the workspace it was given; the call after that works again.  (The error word is allocated by
+ * the first of these calls that runs outside a stream capture.) */
 #define KC_AP_TICKET_BYTES (148 * 8 * 8 * 4)
 size_t kc_cert_allpairs_workspace(int64_t N, int d);
 /* nn,d1,d2,c: device [N]; nn2 device [N] or NULL; workspace: device, 16-byte aligned, >= the size

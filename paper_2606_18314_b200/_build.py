@@ -2,7 +2,9 @@
 
 ``python -m paper_2606_18314_b200._build`` or :func:`build`.  The flags are part of the
 arithmetic contract: ``-fmad=false`` (no FMA contraction), no ``--use_fast_math`` (no FTZ,
-IEEE sqrt/div), ``-lineinfo`` so ncu's source page maps to these files.
+IEEE sqrt/div), ``-lineinfo`` so ncu's source page maps to these files.  Every ``.cu`` file is
+compiled to its own object (in parallel, only when it or a header changed) and the objects are
+linked into the shared library.
 """
 from __future__ import annotations
 
@@ -10,17 +12,21 @@ import os
 import shutil
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libkc.so")
-SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_topk.cu", "kc_grid.cu"]
+SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_topk.cu", "kc_grid.cu", "kc_search.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
     "-fmad=false", "-ftz=false", "-prec-sqrt=true", "-prec-div=true",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC",
 ]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static",
+              "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -30,22 +36,46 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: libkc.so cannot be built (there is no CPU fallback)")
 
 
+def _headers():
+    return [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))] + [
+        os.path.join(HERE, "..", "include", "kc.h"), os.path.abspath(__file__)]
+
+
+def _sources():
+    return [s for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
+
+
 def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [
-        os.path.join(HERE, "..", "include", "kc.h"), os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, s) for s in _sources()] + _headers()
     return any(os.path.getmtime(d) > t for d in deps)
+
+
+def _compile(nvcc, src, force, verbose):
+    obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+    path = os.path.join(CSRC, src)
+    if not force and os.path.exists(obj):
+        t = os.path.getmtime(obj)
+        if all(os.path.getmtime(d) <= t for d in [path] + _headers()):
+            return obj
+    tmp = obj + f".tmp{os.getpid()}"
+    cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", path, "-o", tmp]
+    subprocess.check_call(cmd)
+    os.replace(tmp, obj)
+    return obj
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
+    nvcc = _nvcc()
+    os.makedirs(OBJ, exist_ok=True)
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(lambda s: _compile(nvcc, s, force, verbose), _sources()))
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [_nvcc(), *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []),
-           *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
-    subprocess.check_call(cmd)
+    subprocess.check_call([nvcc, *LINK_FLAGS, *objs, "-o", tmp])
     os.replace(tmp, LIB)
     return LIB
 

@@ -156,17 +156,20 @@ class Certs:
     buf: torch.Tensor | None = None
 
     @staticmethod
-    def _views(buf):
-        return Certs(buf[0], buf[4], buf[1].view(torch.float32), buf[2].view(torch.float32),
-                     buf[3].view(torch.float32), buf)
+    def _views(buf, N=None):
+        N = buf.shape[1] if N is None else N
+        return Certs(buf[0, :N], buf[4, :N], buf[1, :N].view(torch.float32), buf[2, :N].view(torch.float32),
+                     buf[3, :N].view(torch.float32), buf)
 
     @staticmethod
     def empty(N, device="cuda"):
-        return Certs._views(torch.empty((5, N), dtype=torch.int32, device=device))
+        # rows padded to a multiple of 4 entries: every row starts 16-byte aligned for any N
+        # (kc_frontier_classify reads c as float4)
+        return Certs._views(torch.empty((5, (N + 3) // 4 * 4), dtype=torch.int32, device=device), N)
 
     def clone(self):
         if self.buf is not None:
-            return Certs._views(self.buf.clone())
+            return Certs._views(self.buf.clone(), self.nn.numel())
         return Certs(self.nn.clone(), self.nn2.clone(), self.d1.clone(), self.d2.clone(), self.c.clone())
 
     def _ptrs(self):

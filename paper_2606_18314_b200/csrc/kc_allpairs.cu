@@ -188,6 +188,7 @@ struct ApArgs {
     Partial *part;               // j-split: partial lists [js][nq_host]; null: store certificates
     int32_t *redo, *n_redo;      // queries whose bound admitted fewer than two candidates
     int32_t *tickets;            // j-split: chunks finished per query block (the last one merges and re-zeroes)
+    int *errword;                // device error word (kc_common.cuh), or null
     int32_t *nn, *nn2;
     float *d1, *d2, *c;
 };
@@ -196,11 +197,18 @@ struct ApArgs {
 // The counters live in a fixed area at the head of the workspace that holds nothing else, start
 // at zero (workspace contract, kc.h) and are put back to zero by the last arrival, so no call has
 // to clear them (a memset node or a kernel in front of the pass costs 3-5 us of a 70 us launch).
-// A count that cannot occur in a clean area stops the kernel instead of merging garbage.
-__device__ __forceinline__ bool take_ticket(int32_t *t, int total)
+// A count that cannot occur in a clean area (the caller broke the workspace contract) is reported
+// through the device error word and the counter is put back to zero; nothing is merged for that
+// query block, so its certificates are unspecified, but the context stays usable (no trap) and the
+// next all-pairs call returns KC_EINVAL (run()).
+__device__ __forceinline__ bool take_ticket(int32_t *t, int total, int *errword)
 {
     const int old = atomicAdd(t, 1);
-    if (old < 0 || old >= total) __trap();      // the workspace was not zero-initialised
+    if (old < 0 || old >= total) {
+        if (errword) *reinterpret_cast<volatile int *>(errword) = KC_DEVERR_TICKETS;
+        atomicExch(t, 0);
+        return false;
+    }
     const bool last = old == total - 1;
     if (last) atomicExch(t, 0);
     return last;
@@ -282,7 +290,7 @@ allpairs_kernel(const ApArgs a)
         __shared__ int s_last;
         __threadfence();
         __syncthreads();
-        if (threadIdx.x == 0) s_last = take_ticket(&a.tickets[blockIdx.x], (int)gridDim.y);
+        if (threadIdx.x == 0) s_last = take_ticket(&a.tickets[blockIdx.x], (int)gridDim.y, a.errword);
         __syncthreads();
         if (!s_last) return;
         __threadfence();
@@ -475,6 +483,7 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     a.one2 = 0x3f8000003f800000ull;
     a.n_redo = reinterpret_cast<int32_t *>(ws);
     a.tickets = reinterpret_cast<int32_t *>(ws + 16);
+    a.errword = error_word_dev();
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
     const bool idseed = a.seed1 != nullptr;
@@ -544,6 +553,16 @@ kc_status run(const char *who, const float *p, int64_t N, int d, const int32_t *
         set_error("%s: workspace of %zu bytes (16-byte aligned) required", who, need);
         return KC_EINVAL;
     }
+    error_word_init();
+    if (error_word_take() == KC_DEVERR_TICKETS) {
+        // an earlier all-pairs kernel met split counters that a zero-filled workspace cannot hold:
+        // its results are unspecified.  Heal the workspace passed now and report; the call is not run.
+        KC_CUDA(cudaMemsetAsync(workspace, 0, 16 + (size_t)AP_TICKETS * 4, (cudaStream_t)stream));
+        set_error("%s: an earlier all-pairs call was given a workspace that had not been zero-filled "
+                  "(kc.h, workspace contract); its certificates are unspecified.  The counters of the "
+                  "workspace passed now have been cleared; call again", who);
+        return KC_EINVAL;
+    }
     ApArgs a = {};
     a.p = p; a.N = N; a.qlist = q; a.nq_dev = nq_dev; a.nq_host = nq;
     a.bound_d2 = d2_prev; a.bound_eps = eps;
@@ -558,6 +577,7 @@ kc_status run(const char *who, const float *p, int64_t N, int d, const int32_t *
 extern "C" size_t kc_cert_allpairs_workspace(int64_t N, int d)
 {
     if (N < 2 || (d != 2 && d != 3)) return 0;
+    error_word_init();
     return workspace_bytes_for(N, choose_shape(N, N));
 }
 
@@ -601,6 +621,7 @@ extern "C" kc_status kc_cert_allpairs_seeded(const float *p, int64_t N, int d, c
 extern "C" size_t kc_frontier_oracle_workspace(int64_t N, int d, int64_t nq_max)
 {
     if (N < 2 || nq_max < 1 || (d != 2 && d != 3)) return 0;
+    error_word_init();
     return workspace_bytes_for(nq_max, choose_shape(nq_max, N));
 }
 

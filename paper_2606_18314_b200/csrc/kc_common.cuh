@@ -15,6 +15,17 @@ void set_error(const char *fmt, ...);
 void count_launches(int n);   // host-side tally of kernel launches issued by the library
 kc_status cuda_fail(cudaError_t e, const char *where);
 
+// Device-side error word: ONE int per process in pinned host memory that kernels can write through
+// its device pointer (zero-copy).  A kernel that meets a state it cannot serve (e.g. a workspace
+// that was not zero-filled, kc.h) stores a code there instead of trapping -- a trap would poison
+// the CUDA context for the whole process -- and the next libkc call that checks the word reports
+// it as a status.  error_word_init() allocates it (cudaHostAlloc: call outside stream capture);
+// error_word_dev() is the pointer kernels get (nullptr until initialised: they then skip the store).
+enum { KC_DEVERR_NONE = 0, KC_DEVERR_TICKETS = 1 };
+void error_word_init();
+int *error_word_dev();
+int error_word_take();        // host: read and clear (0 when none or not initialised)
+
 #define KC_CUDA(call)                                              \
     do {                                                           \
         cudaError_t e_ = (call);                                   \

@@ -21,102 +21,16 @@
 #include "kc_common.cuh"
 
 using namespace kc;
+#include <new>
+
+#include "kc_grid.cuh"
+
+using namespace kc;
 
 namespace {
 
 constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
-
-struct Counters {
-    int n_misfiled;
-    int c_occ;
-    int max_occ;
-    int n_stragglers;
-    int m_cells;
-    int n_list2;              // frontier points of the current sweep that live in chains
-    int ticket;               // blocks of entropy_collect_kernel that are done (the last one finishes)
-    int c_occ_acc;            // recount of the occupied cells in progress (A5 after an incremental update)
-    int kmax;                 // largest per-cell frontier count seen by the current A5 call
-    double big;               // sum k ln k over cells with k >= MHIST (rare)
-};
-
-struct View {
-    int G0, G1, G2;
-    float lo0, lo1, lo2, h, inv_h, shrink;
-    float slk0, slk1, slk2;   // absolute rounding slack of a computed face / cell boundary per axis
-    int dense_thr;            // a row range of at least this many records is handled as dense (A3)
-    int wpq_max;              // id lists up to this long are served one warp per query (A7)
-    const int32_t *cell_start;
-    const float2 *spos2;
-    const float4 *spos4;
-    const int32_t *sidx;
-    const int32_t *head;
-    const int32_t *next;
-    const float4 *opos;
-};
-
-}  // namespace
-
-struct kc_grid {
-    kc_geom geom;
-    int64_t N_max, n_cells, N;
-    int built, dirty;
-    size_t bytes;
-    int32_t *cell, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
-    int32_t *blocksums;
-    int32_t *mark;            // per sorted slot: epoch of the last sweep that queried it
-    int32_t *list2;           // frontier points of the current sweep that live in chains
-    float *delta;             // NEXT #2: displacement of every point in the current step
-    unsigned *cellmax;        // NEXT #2: largest displacement (float bits) per cell
-    int epoch;
-    float2 *spos2;
-    float4 *spos4, *opos;
-    Counters *ctr;
-    int n_scan_blocks;
-};
-
-namespace {
-
 constexpr int SCAN_CHUNK = 2048;   // cells per scan block (256 threads x 8)
-
-View make_view(const kc_grid *g)
-{
-    View v;
-    v.G0 = g->geom.G[0]; v.G1 = g->geom.G[1]; v.G2 = g->geom.G[2];
-    v.lo0 = g->geom.lo[0]; v.lo1 = g->geom.lo[1]; v.lo2 = g->geom.lo[2];
-    v.h = g->geom.h; v.inv_h = g->geom.inv_h;
-    int Gm = v.G0 > v.G1 ? v.G0 : v.G1;
-    if (v.G2 > Gm) Gm = v.G2;
-    // rounding slack of the ring bound: computed cell faces are off by O(u*G) cell widths
-    v.shrink = 1.0f - (1.0f / 512.0f + (float)Gm * (1.0f / 524288.0f));
-    const int Ga[3] = {v.G0, v.G1, v.G2};
-    float slk[3];
-    for (int a = 0; a < 3; ++a) {
-        double t = (fabs((double)g->geom.lo[a]) + (double)Ga[a] * (double)g->geom.h) / 1048576.0;
-        slk[a] = nextafterf((float)t, INFINITY);
-    }
-    v.slk0 = slk[0]; v.slk1 = slk[1]; v.slk2 = slk[2];
-    static const int dense_env = getenv("KC_DENSE_THR") ? atoi(getenv("KC_DENSE_THR")) : 0;
-    v.dense_thr = dense_env > 0 ? dense_env : 128;
-    static const int wpq_env = getenv("KC_WPQ_MAX") ? atoi(getenv("KC_WPQ_MAX")) : -1;
-    v.wpq_max = wpq_env >= 0 ? wpq_env : 32768;
-    v.cell_start = g->cell_start;
-    v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
-    v.head = g->head; v.next = g->next; v.opos = g->opos;
-    return v;
-}
-
-// Append `id` to list[] for the lanes with `want` set: one atomic per warp on the shared cursor
-// (every lane of the warp must call it).
-__device__ __forceinline__ void warp_append(bool want, int id, int32_t *list, int *cursor)
-{
-    const unsigned m = __ballot_sync(0xffffffffu, want);
-    if (!m) return;
-    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
-    int base = 0;
-    if (lane == leader) base = atomicAdd(cursor, __popc(m));
-    base = __shfl_sync(0xffffffffu, base, leader);
-    if (want) list[base + __popc(m & ((1u << lane) - 1))] = id;
-}
 
 // ------------------------------------------------------------------ A2 build
 __global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
@@ -140,15 +54,6 @@ build_prep_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__
 }
 
 template <int D>
-__device__ __forceinline__ int cell_of(const View &v, float x, float y, float z)
-{
-    int kx = cell_axis(x, v.lo0, v.inv_h, v.G0);
-    int ky = cell_axis(y, v.lo1, v.inv_h, v.G1);
-    int kz = D == 3 ? cell_axis(z, v.lo2, v.inv_h, v.G2) : 0;
-    return (kz * v.G1 + ky) * v.G0 + kx;
-}
-
-template <int D>
 __global__ void __launch_bounds__(256)
 cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restrict__ cell,
                    int32_t *counts, Counters *ctr)
@@ -156,6 +61,7 @@ cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restri
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {          // the chains were dropped by the previous kernel; the scan recounts C
         ctr->n_misfiled = 0; ctr->c_occ = 0; ctr->max_occ = 0; ctr->n_stragglers = 0;
+        ctr->n_list2 = 0;
     }
     if (i >= N) return;
     float x, y, z = 0.f;
@@ -352,879 +258,6 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
     }
     sidx[s] = i;
     slot[i] = s;
-}
-
-// ------------------------------------------------------------------ A3 / A7 ring search
-// Exact top-2 of query (qx,qy,qz), excluding point id `self`, over the grid's sorted ranges and
-// (if chains) its overflow chains.  Corollary 1: the block is widened until
-// the second neighbour is provably enclosed.
-//
-// Filing invariant: every record listed in cell k of an axis has a coordinate x with
-// cell_axis(x) = k, and cell_axis is monotone, so for a query in cell c < k the real distance
-// along that axis is at least  face(k) - q  minus the rounding of the computed face and cell id:
-//     x - q >= fl(face_k - q)(1 - u) - u(|lo| + 5.01 G h),      u = 2^-24
-// (3 roundings in cell_axis move a cell boundary by <= 3.01 u G h, 2 roundings in
-// face_k = fl(lo + fl(k h)) move the face by <= u(|lo| + 2 G h)).  gap_lb() therefore subtracts
-// the absolute slack slk = (|lo| + G h) 2^-20 and multiplies by shrink = 1 - 2^-9 - G 2^-19,
-// which also covers the <= 3u relative undershoot of an fp32 squared distance.  Points outside
-// the grid box are filed in boundary cells; only faces between two cells are ever used, so the
-// bound holds for them too (clamping is monotone).
-//
-// Two uses of the bound, both strict (a tie at equal distance must still be seen, the index
-// decides it):
-//  * cell pruning inside the 3^d block: a cell whose box is provably farther than the current
-//    second-best (sum over axes of the squared shrunk gaps > s2) is skipped.  The query's own
-//    cell is scanned first, then its row neighbours, then the other rows nearest first, so in
-//    dense cells (occupancy >> 1, d2 << h) most of the block is never touched;
-//  * termination: after the Chebyshev-radius-r block is done, every unscanned point lies beyond
-//    a block face interior to the grid; stop only when s2 < (min face distance)^2, else scan
-//    ring r+1.  No face left = whole grid scanned = stop.  Never a cap.
-//
-// Candidate ranges are scanned 4 records per step from a 4-aligned start: records in front of the
-// range belong to neighbouring cells and the records behind the last slot are NaN padding, so
-// the extra ones are either legitimate candidates or inert (every comparison with NaN is false).
-// A candidate can therefore be offered more than once; the insertion skips ids already held.
-__device__ __forceinline__ void offer_once(Top2 &best, float s, int j, int self)
-{
-    if (s <= best.s2 && j >= 0 && j != self && j != best.j1 && j != best.j2) best.offer(s, j);
-}
-// branch-free (s, j)-ordered insertion (converged code for loops whose lanes all insert)
-__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
-{
-    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
-    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
-    const float ns2 = lt1 ? b.s1 : s;
-    const int nj2 = lt1 ? b.j1 : j;
-    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
-    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
-}
-template <int D>
-__device__ __noinline__ Top2 slow_offer4(const View &v, Top2 best, int t, float s0, float s1,
-                                         float s2, float s3, int self)
-{
-    if (D == 2) {
-        if (s0 <= best.s2) offer_once(best, s0, v.sidx[t + 0], self);
-        if (s1 <= best.s2) offer_once(best, s1, v.sidx[t + 1], self);
-        if (s2 <= best.s2) offer_once(best, s2, v.sidx[t + 2], self);
-        if (s3 <= best.s2) offer_once(best, s3, v.sidx[t + 3], self);
-    } else {
-        if (s0 <= best.s2) offer_once(best, s0, __float_as_int(v.spos4[t + 0].w), self);
-        if (s1 <= best.s2) offer_once(best, s1, __float_as_int(v.spos4[t + 1].w), self);
-        if (s2 <= best.s2) offer_once(best, s2, __float_as_int(v.spos4[t + 2].w), self);
-        if (s3 <= best.s2) offer_once(best, s3, __float_as_int(v.spos4[t + 3].w), self);
-    }
-    return best;
-}
-template <int D>
-__device__ __forceinline__ void scan_range(const View &v, int b, int e, float qx, float qy, float qz,
-                                           int self, Top2 &best)
-{
-    for (int t = b & ~3; t < e; t += 4) {
-        float s0, s1, s2, s3;
-        if (D == 2) {
-            const float4 A = *reinterpret_cast<const float4 *>(v.spos2 + t);       // x0 y0 x1 y1
-            const float4 B = *reinterpret_cast<const float4 *>(v.spos2 + t + 2);   // x2 y2 x3 y3
-            s0 = sqd2(qx, qy, A.x, A.y); s1 = sqd2(qx, qy, A.z, A.w);
-            s2 = sqd2(qx, qy, B.x, B.y); s3 = sqd2(qx, qy, B.z, B.w);
-        } else {
-            const float4 c0 = v.spos4[t], c1 = v.spos4[t + 1], c2 = v.spos4[t + 2], c3 = v.spos4[t + 3];
-            s0 = sqd3(qx, qy, qz, c0.x, c0.y, c0.z); s1 = sqd3(qx, qy, qz, c1.x, c1.y, c1.z);
-            s2 = sqd3(qx, qy, qz, c2.x, c2.y, c2.z); s3 = sqd3(qx, qy, qz, c3.x, c3.y, c3.z);
-        }
-        float m = fminf(fminf(s0, s1), fminf(s2, s3));
-        if (m <= best.s2) best = slow_offer4<D>(v, best, t, s0, s1, s2, s3, self);
-    }
-}
-template <int D>
-__device__ __forceinline__ void scan_chain(const View &v, int cidx, float qx, float qy, float qz,
-                                           int self, Top2 &best)
-{
-    for (int e = v.head[cidx]; e >= 0; e = v.next[e]) {
-        float4 c = v.opos[e];
-        float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
-        offer_once(best, s, e, self);
-    }
-}
-template <int D>
-__device__ __forceinline__ void scan_row(const View &v, bool chains, int rowbase, int x0, int x1,
-                                         float qx, float qy, float qz, int self, Top2 &best)
-{
-    int b = v.cell_start[rowbase + x0], e = v.cell_start[rowbase + x1 + 1];
-    scan_range<D>(v, b, e, qx, qy, qz, self, best);
-    if (chains)
-        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
-}
-
-__device__ __forceinline__ float face_at(float lo, int k, float h)
-{
-    return __fadd_rn(lo, __fmul_rn((float)k, h));
-}
-// lower bound of the real axis distance behind a computed face at computed distance `gap`
-__device__ __forceinline__ float gap_lb(const View &v, float gap, float slk)
-{
-    return __fmul_rn(fmaxf(__fsub_rn(gap, slk), 0.0f), v.shrink);
-}
-// squared lower bounds of the axis distance from the query to its six neighbour cells
-struct Gaps { float xm, xp, ym, yp, zm, zp; };
-template <int D>
-__device__ __forceinline__ Gaps make_gaps(const View &v, float qx, float qy, float qz, int cx, int cy, int cz)
-{
-    Gaps g;
-    float t;
-    t = gap_lb(v, __fsub_rn(qx, face_at(v.lo0, cx, v.h)), v.slk0); g.xm = __fmul_rn(t, t);
-    t = gap_lb(v, __fsub_rn(face_at(v.lo0, cx + 1, v.h), qx), v.slk0); g.xp = __fmul_rn(t, t);
-    t = gap_lb(v, __fsub_rn(qy, face_at(v.lo1, cy, v.h)), v.slk1); g.ym = __fmul_rn(t, t);
-    t = gap_lb(v, __fsub_rn(face_at(v.lo1, cy + 1, v.h), qy), v.slk1); g.yp = __fmul_rn(t, t);
-    g.zm = 0.f; g.zp = 0.f;
-    if (D == 3) {
-        t = gap_lb(v, __fsub_rn(qz, face_at(v.lo2, cz, v.h)), v.slk2); g.zm = __fmul_rn(t, t);
-        t = gap_lb(v, __fsub_rn(face_at(v.lo2, cz + 1, v.h), qz), v.slk2); g.zp = __fmul_rn(t, t);
-    }
-    return g;
-}
-// The 3^(d-1) - 1 rows of the block other than the query's own, nearest first: offsets (oy, oz)
-// packed two bits each as offset + 1.
-//   k:   0       1       2       3       4        5        6        7
-//  oy:  -1      +1       0       0      -1       +1       -1       +1
-//  oz:   0       0      -1      +1      -1       -1       +1       +1
-constexpr unsigned ROW_OY = 0u | (2u << 2) | (1u << 4) | (1u << 6) | (0u << 8) | (2u << 10) | (0u << 12) | (2u << 14);
-constexpr unsigned ROW_OZ = 1u | (1u << 2) | (0u << 4) | (2u << 6) | (0u << 8) | (0u << 10) | (2u << 12) | (2u << 14);
-__device__ __forceinline__ int row_oy(int k) { return (int)((ROW_OY >> (2 * k)) & 3u) - 1; }
-__device__ __forceinline__ int row_oz(int k) { return (int)((ROW_OZ >> (2 * k)) & 3u) - 1; }
-
-// distance (lower bound) from the query to the nearest face of the cell box
-// [x0,x1]x[y0,y1]x[z0,z1] that is interior to the grid (+inf if the box covers the grid)
-template <int D>
-__device__ __forceinline__ float box_bound(const View &v, float qx, float qy, float qz, int x0,
-                                           int x1, int y0, int y1, int z0, int z1)
-{
-    float bound = CUDART_INF_F;
-    if (x0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qx, face_at(v.lo0, x0, v.h)), v.slk0));
-    if (x1 < v.G0 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo0, x1 + 1, v.h), qx), v.slk0));
-    if (y0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qy, face_at(v.lo1, y0, v.h)), v.slk1));
-    if (y1 < v.G1 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo1, y1 + 1, v.h), qy), v.slk1));
-    if (D == 3) {
-        if (z0 >= 1) bound = fminf(bound, gap_lb(v, __fsub_rn(qz, face_at(v.lo2, z0, v.h)), v.slk2));
-        if (z1 < v.G2 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(face_at(v.lo2, z1 + 1, v.h), qz), v.slk2));
-    }
-    return bound;
-}
-__device__ __forceinline__ bool bound_ok(float bound, float s2)
-{
-    if (bound == CUDART_INF_F) return true;               // nothing left outside the scanned box
-    return bound > 0.0f && s2 < __fmul_rn(bound, bound);
-}
-
-// Chebyshev rings r = 2, 3, ... around the query's own cell, entered with the radius-1 block
-// already done; leaves as soon as the bound of the scanned block allows it.  (Rare path: kept out
-// of line, state passed by value.)
-struct RingOut { Top2 best; int r; };
-template <int D>
-__device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float qx, float qy, float qz,
-                                              int self, int cx, int cy, int cz, Top2 best)
-{
-    int r = 1;
-    for (;;) {
-        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
-        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) break;
-        ++r;
-        // ring r: shell rows get the full segment, inner rows only the two end cells
-        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
-        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y) {
-                int rowbase = (z * v.G1 + y) * v.G0;
-                bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
-                if (shell) {
-                    scan_row<D>(v, chains, rowbase, x0, x1, qx, qy, qz, self, best);
-                } else {
-                    if (cx - r >= 0) scan_row<D>(v, chains, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                    if (cx + r <= v.G0 - 1) scan_row<D>(v, chains, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                }
-            }
-    }
-    RingOut o;
-    o.best = best; o.r = r;
-    return o;
-}
-// final check of the radius-1 block, then wider rings if the bound requires them
-template <int D>
-__device__ __forceinline__ int finish_block(const View &v, bool chains, float qx, float qy, float qz, int self,
-                                            int cx, int cy, int cz, Top2 &best)
-{
-    const int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
-    const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
-    const int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
-    if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) return 1;
-    const RingOut o = ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
-    best = o.best;
-    return o.r;
-}
-
-// One thread per query, straight from global memory (A7, and A3's comparison variant): own
-// cell, row neighbours, other rows nearest first, every cell subject to pruning; then rings.
-template <int D>
-__device__ int block_search(const View &v, bool chains, float qx, float qy, float qz, int self,
-                            int cx, int cy, int cz, Top2 &best)
-{
-    const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
-    const int rb0 = (cz * v.G1 + cy) * v.G0;
-    {
-        const int32_t *cs = v.cell_start + rb0 + cx;
-        const int s0 = cs[0], s1 = cs[1];
-        scan_range<D>(v, s0, s1, qx, qy, qz, self, best);
-        if (chains) scan_chain<D>(v, rb0 + cx, qx, qy, qz, self, best);
-        if (cx > 0 && !(best.s2 < g.xm)) {
-            scan_range<D>(v, cs[-1], s0, qx, qy, qz, self, best);
-            if (chains) scan_chain<D>(v, rb0 + cx - 1, qx, qy, qz, self, best);
-        }
-        if (cx < v.G0 - 1 && !(best.s2 < g.xp)) {
-            scan_range<D>(v, s1, cs[2], qx, qy, qz, self, best);
-            if (chains) scan_chain<D>(v, rb0 + cx + 1, qx, qy, qz, self, best);
-        }
-    }
-#pragma unroll 1
-    for (int k = 0; k < (D == 3 ? 8 : 2); ++k) {
-        const int oy = row_oy(k), oz = row_oz(k);
-        const int y = cy + oy, z = cz + oz;
-        if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
-        const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
-        if (best.s2 < rb2) continue;
-        int x0 = cx, x1 = cx;
-        if (cx > 0 && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
-        if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
-        scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, x0, x1, qx, qy, qz, self, best);
-    }
-    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
-}
-
-template <int D>
-__global__ void __launch_bounds__(128)
-search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
-{
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    float qx, qy, qz = 0.f;
-    int self;
-    if (D == 2) {
-        float2 q = v.spos2[s];
-        qx = q.x; qy = q.y; self = v.sidx[s];
-    } else {
-        float4 q = v.spos4[s];
-        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
-    }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    Top2 best;
-    best.init();
-    int r = block_search<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
-    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, self, nn, nn2, d1, d2, c);
-}
-
-// ---- A3, warp-tiled: the whole-set search of a freshly built grid --------------------------
-// A warp owns 32 consecutive sorted slots.  Slots are cell-sorted, so the lanes of one grid row
-// form a contiguous lane segment, and what they need from any row of the 3^d block is ONE
-// contiguous record range [B, E) of the sorted array (cells xf-1 .. xl+1 of that row).
-//  * sparse row (E - B < dense_thr records): the warp loads the range into its shared-memory tile
-//    with coalesced loads (one global round trip instead of one per candidate) and every lane
-//    scans its own 3-cell sub-range [b, e) from shared memory, 4 records per step;
-//  * dense row (a few cells under 32 lanes, occupancy >> 1, d2 << h): cell pruning pays.  In the
-//    lanes' own row the own cell is scanned first, then only the row neighbours a lane cannot
-//    rule out; in the other rows only the cells it cannot rule out.  What is left after pruning
-//    is long ranges for a few lanes; a tile pass would cost as much as if all 32 lanes needed
-//    them, so such a pass is served cooperatively instead: for each lane that still has a range,
-//    all 32 lanes take different records of it (coalesced, straight from global memory) and the
-//    two best are extracted with warp reductions.
-// Lanes whose radius-1 block does not satisfy the bound continue with the ring loop (rare).
-constexpr int WT_TILE = 128;   // records per warp tile
-constexpr int WT_WARPS = 4;
-
-template <int D>
-__device__ __forceinline__ void tile_scan(const float2 *tp2, const float4 *tp4, const int *tidx, int lb,
-                                          int le, float qx, float qy, float qz, int self, Top2 &best)
-{
-    for (int t = lb; t < le; t += 4) {
-        float s0, s1, s2, s3;
-        int j0, j1, j2, j3;
-        if (D == 2) {
-            const float2 c0 = tp2[t], c1 = tp2[t + 1], c2 = tp2[t + 2], c3 = tp2[t + 3];
-            s0 = sqd2(qx, qy, c0.x, c0.y); s1 = sqd2(qx, qy, c1.x, c1.y);
-            s2 = sqd2(qx, qy, c2.x, c2.y); s3 = sqd2(qx, qy, c3.x, c3.y);
-        } else {
-            const float4 c0 = tp4[t], c1 = tp4[t + 1], c2 = tp4[t + 2], c3 = tp4[t + 3];
-            s0 = sqd3(qx, qy, qz, c0.x, c0.y, c0.z); s1 = sqd3(qx, qy, qz, c1.x, c1.y, c1.z);
-            s2 = sqd3(qx, qy, qz, c2.x, c2.y, c2.z); s3 = sqd3(qx, qy, qz, c3.x, c3.y, c3.z);
-            j0 = __float_as_int(c0.w); j1 = __float_as_int(c1.w);
-            j2 = __float_as_int(c2.w); j3 = __float_as_int(c3.w);
-        }
-        float m = fminf(fminf(s0, s1), fminf(s2, s3));
-        if (m <= best.s2) {
-            if (D == 2) { j0 = tidx[t]; j1 = tidx[t + 1]; j2 = tidx[t + 2]; j3 = tidx[t + 3]; }
-            offer_once(best, s0, j0, self);
-            offer_once(best, s1, j1, self);
-            offer_once(best, s2, j2, self);
-            offer_once(best, s3, j3, self);
-        }
-    }
-}
-
-// Tile pass: records [B, E) (warp-uniform) go through the warp's tile, every lane scans its own
-// (up to two) ranges [b1,e1), [b2,e2) (empty when b >= e).  Called by all 32 lanes.
-template <int D>
-__device__ __forceinline__ void tile_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
-                                          int B, int E, int b1, int e1, int b2, int e2, float qx, float qy,
-                                          float qz, int self, Top2 &best)
-{
-    const float qnan = __int_as_float(0x7fc00000);
-    for (int T0 = B; T0 < E; T0 += WT_TILE) {
-        const int T1 = T0 + WT_TILE;
-        const int lb1 = max(b1, T0), le1 = min(e1, T1), lb2 = max(b2, T0), le2 = min(e2, T1);
-        if (E - B > WT_TILE && !__any_sync(0xffffffffu, lb1 < le1 || lb2 < le2)) continue;
-        const int need = min(WT_TILE, E - T0 + 3);               // records of this tile anyone can touch
-#pragma unroll
-        for (int k = lane; k < WT_TILE; k += 32) {
-            const int g = T0 + k;
-            if (k < need) {
-                if (D == 3) {
-                    tp4[k] = g < N ? v.spos4[g] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
-                } else {
-                    tp2[k] = g < N ? v.spos2[g] : make_float2(qnan, qnan);
-                    tix[k] = g < N ? v.sidx[g] : -1;
-                }
-            }
-        }
-        __syncwarp();
-        if (lb1 < le1) tile_scan<D>(tp2, tp4, tix, lb1 - T0, le1 - T0, qx, qy, qz, self, best);
-        if (lb2 < le2) tile_scan<D>(tp2, tp4, tix, lb2 - T0, le2 - T0, qx, qy, qz, self, best);
-        __syncwarp();
-    }
-}
-
-// Warp-cooperative scan of one lane's range: all 32 lanes take different records of [b, e) for the
-// query of lane L (coalesced loads straight from global memory) and keep their own partial top-2.
-template <int D>
-__device__ __forceinline__ void coop_range(const View &v, int lane, int b, int e, float qx, float qy,
-                                           float qz, int self, float thr, int h1, int h2, Top2 &tmp)
-{
-    for (int t = b + lane; t < e; t += 32) {
-        float s;
-        int j;
-        if (D == 2) {
-            const float2 c = v.spos2[t];
-            j = v.sidx[t];                         // issued with the position: one round trip
-            s = sqd2(qx, qy, c.x, c.y);
-        } else {
-            const float4 c = v.spos4[t];
-            s = sqd3(qx, qy, qz, c.x, c.y, c.z);
-            j = __float_as_int(c.w);
-        }
-        if (s <= thr && j >= 0 && j != self && j != h1 && j != h2) tmp.offer(s, j);
-    }
-}
-// smallest key (s, j) over the warp's partial lists, removed from the list that held it
-__device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
-{
-    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
-    const unsigned m = __reduce_min_sync(0xffffffffu, key);
-    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
-    s = __uint_as_float(m);
-    if (key == m && tmp.j1 == j) {
-        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
-        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
-    }
-}
-// Dense pass: every lane brings up to two ranges left after pruning.  Served lane by lane by the
-// whole warp when that is cheaper than a tile pass over the hull [B, E) (issue-slot estimates:
-// tile pass ~11 per record of the longest lane, cooperative ~45 per served lane + 12 per 32
-// records).  Called by all 32 lanes.
-template <int D>
-__device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
-                                           int b1, int e1, int b2, int e2, float qx, float qy, float qz,
-                                           int self, Top2 &best)
-{
-    const bool h1 = b1 < e1, h2 = b2 < e2;
-    const int len = (h1 ? e1 - b1 : 0) + (h2 ? e2 - b2 : 0);
-    const unsigned active = __ballot_sync(0xffffffffu, len > 0);
-    if (!active) return;
-    const int maxlen = __reduce_max_sync(0xffffffffu, len);
-    const int sumlen = __reduce_add_sync(0xffffffffu, len);
-    if (__popc(active) * 360 + sumlen * 3 < maxlen * 88) {
-        for (unsigned a = active; a; a &= a - 1) {
-            const int L = __ffs(a) - 1;
-            const float Lx = __shfl_sync(0xffffffffu, qx, L), Ly = __shfl_sync(0xffffffffu, qy, L);
-            const float Lz = D == 3 ? __shfl_sync(0xffffffffu, qz, L) : 0.f;
-            const int Lself = __shfl_sync(0xffffffffu, self, L);
-            const float thr = __shfl_sync(0xffffffffu, best.s2, L);
-            const int Lj1 = __shfl_sync(0xffffffffu, best.j1, L), Lj2 = __shfl_sync(0xffffffffu, best.j2, L);
-            const int Lb1 = __shfl_sync(0xffffffffu, b1, L), Le1 = __shfl_sync(0xffffffffu, e1, L);
-            const int Lb2 = __shfl_sync(0xffffffffu, b2, L), Le2 = __shfl_sync(0xffffffffu, e2, L);
-            Top2 tmp;
-            tmp.init();
-            coop_range<D>(v, lane, Lb1, Le1, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
-            coop_range<D>(v, lane, Lb2, Le2, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
-            float sa, sb;
-            int ja, jb;
-            coop_pop(tmp, sa, ja);
-            coop_pop(tmp, sb, jb);
-            if (lane == L) {
-                if (ja != KC_NOIDX) best.offer(sa, ja);
-                if (jb != KC_NOIDX) best.offer(sb, jb);
-            }
-        }
-        return;
-    }
-    const int B = __reduce_min_sync(0xffffffffu, min(h1 ? b1 : 0x7fffffff, h2 ? b2 : 0x7fffffff));
-    const int E = __reduce_max_sync(0xffffffffu, max(h1 ? e1 : 0, h2 ? e2 : 0));
-    tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
-}
-
-// SWEEP = false: A3, every slot of a freshly built grid is a query.
-// SWEEP = true:  A7 for a large frontier: the same slot-ordered sweep over the incrementally
-//   updated grid, but only the slots marked with this call's epoch are queries (their lanes stay
-//   idle otherwise; warps without a marked slot leave at once), tombstones are inert records and
-//   the overflow chains of every visited cell are scanned too.  Runs only when *nF * sweep_div >= N
-//   (the list kernel serves smaller frontiers and the frontier points that live in chains).
-template <int D, bool SWEEP>
-__global__ void __launch_bounds__(32 * WT_WARPS)
-search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
-                    const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
-                    float *d2, float *c)
-{
-    __shared__ __align__(16) float4 s_p4[D == 3 ? WT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
-    __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    if (SWEEP && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = SWEEP && ctr->n_misfiled > 0;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const float qnan = __int_as_float(0x7fc00000);
-    float4 *tp4 = s_p4[D == 3 ? warp : 0];
-    float2 *tp2 = s_p2[D == 2 ? warp : 0];
-    int *tix = s_ix[D == 2 ? warp : 0];
-    // the whole tile starts inert: a short range leaves records behind it untouched
-    for (int k = lane; k < WT_TILE + 4; k += 32) {
-        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
-    }
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s - lane >= N) return;                     // whole warp past the end
-    const int sc = min(s, N - 1);                  // tail lanes mirror the last slot (no store)
-    float qx, qy, qz = 0.f;
-    int self;
-    if (D == 2) {
-        float2 q = v.spos2[sc];
-        qx = q.x; qy = q.y; self = v.sidx[sc];
-    } else {
-        float4 q = v.spos4[sc];
-        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
-    }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    const int rowid = cz * v.G1 + cy;
-    const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
-    Top2 best;
-    best.init();
-    // queries of this warp (marked slots are never tombstones, so their cells are in slot order)
-    const bool query = SWEEP ? (s < N && mark[sc] == epoch) : true;
-    unsigned todo = __ballot_sync(0xffffffffu, query);
-    while (todo) {
-        const int leader = __ffs(todo) - 1;
-        const int R = __shfl_sync(0xffffffffu, rowid, leader);
-        const unsigned seg = __ballot_sync(0xffffffffu, rowid == R) & todo;
-        const int first = __ffs(seg) - 1, last = 31 - __clz(seg);
-        const int xf = __shfl_sync(0xffffffffu, cx, first), xl = __shfl_sync(0xffffffffu, cx, last);
-        const int ry = __shfl_sync(0xffffffffu, cy, first), rz = __shfl_sync(0xffffffffu, cz, first);
-        const bool mine = (seg >> lane) & 1u;
-        const int ux0 = max(xf - 1, 0), ux1 = min(xl + 1, v.G0 - 1);
-#pragma unroll 1
-        for (int k = -1; k < (D == 3 ? 8 : 2); ++k) {          // k = -1: the lanes' own row
-            const int oy = k < 0 ? 0 : row_oy(k), oz = k < 0 ? 0 : row_oz(k);
-            const int y = ry + oy, z = rz + oz;
-            if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
-            const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
-            if (chains && mine)
-                for (int x = has_l ? cx - 1 : cx; x <= (has_r ? cx + 1 : cx); ++x)
-                    scan_chain<D>(v, (z * v.G1 + y) * v.G0 + x, qx, qy, qz, self, best);
-            const int B = crow[ux0], E = crow[ux1 + 1];
-            if (B == E) continue;
-            if (E - B < v.dense_thr) {
-                int b = 0, e = 0;
-                if (mine) { b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1]; }
-                tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b, e, 0, 0, qx, qy, qz, self, best);
-                continue;
-            }
-            const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
-            if (k < 0) {
-                int s0 = 0, s1 = 0;
-                if (mine) { s0 = crow[cx]; s1 = crow[cx + 1]; }
-                tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
-                int bl = 0, el = 0, br = 0, er = 0;
-                if (mine && has_l && !(best.s2 < g.xm)) { bl = crow[cx - 1]; el = s0; }
-                if (mine && has_r && !(best.s2 < g.xp)) { br = s1; er = crow[cx + 2]; }
-                dense_pass<D>(v, N, lane, tp2, tp4, tix, bl, el, br, er, qx, qy, qz, self, best);
-            } else {
-                int b = 0, e = 0;
-                if (mine) {
-                    const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
-                    if (!(best.s2 < rb2)) {
-                        int x0 = cx, x1 = cx + 1;
-                        if (has_l && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
-                        if (has_r && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 2;
-                        b = crow[x0]; e = crow[x1];
-                    }
-                }
-                dense_pass<D>(v, N, lane, tp2, tp4, tix, b, e, 0, 0, qx, qy, qz, self, best);
-            }
-        }
-        todo &= ~seg;
-    }
-    if (!query) return;
-    const int r = finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
-    if (s >= N) return;
-    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, self, nn, nn2, d1, d2, c);
-}
-
-// A7, large frontier: stamp the slots of the frontier points with this call's epoch; frontier
-// points that live in an overflow chain have no slot and go to the list kernel (list2).
-__global__ void __launch_bounds__(256)
-mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF, int N, int sweep_div,
-                     const int32_t *__restrict__ slot, int32_t *mark, int epoch, int32_t *list2,
-                     Counters *ctr)
-{
-    const int n = *nF;
-    if ((int64_t)n * sweep_div < N) return;
-    const int stride = gridDim.x * blockDim.x;
-    for (int f0 = blockIdx.x * blockDim.x; f0 < n; f0 += stride) {     // warp-uniform trip count
-        const int f = f0 + threadIdx.x;
-        int i = -1;
-        bool chain = false;
-        if (f < n) {
-            i = F[f];
-            const int sl = slot[i];
-            if (sl >= 0) mark[sl] = epoch;
-            else chain = true;
-        }
-        warp_append(chain, i, list2, &ctr->n_list2);
-    }
-}
-
-// ---- warp per query ---------------------------------------------------------------------------
-// One warp serves one query, one lane per cell of the 3^d block: every lane fetches its cell's
-// record range and chain head at once (one memory round trip for the whole block instead of one
-// per row), the own cell is scanned first by the whole warp, then every lane prunes its cell
-// against the second-best found so far; short surviving ranges are scanned by their lanes, long
-// ones (dense cells) by the whole warp, and two warp reductions extract the two smallest keys.
-// No lane ever waits for another query's insertions, and the order of the queries is irrelevant,
-// which is what a frontier list in id order needs (A7).  SLOTS = true runs the same search for
-// every sorted slot of a fresh grid (A3 variant, for comparison with the tiled sweep).
-template <int D>
-__device__ __forceinline__ void lane_offer(Top2 &tmp, float s, int j, float thr, int self)
-{
-    insert_bf(tmp, s, j, s <= thr && j >= 0 && j != self);
-}
-template <int D>
-__device__ int wpq_search(const View &v, bool chains, int lane, float qx, float qy, float qz, int self,
-                          Top2 &best)
-{
-    constexpr int NC = D == 3 ? 27 : 9, OWN = NC / 2;
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    const int ox = lane % 3 - 1, oy = (lane / 3) % 3 - 1, oz = D == 3 ? lane / 9 - 1 : 0;
-    const int x = cx + ox, y = cy + oy, z = cz + oz;
-    const bool valid = lane < NC && x >= 0 && x < v.G0 && y >= 0 && y < v.G1 && z >= 0 && z < v.G2;
-    const int cid = valid ? (z * v.G1 + y) * v.G0 + x : 0;
-    int b = 0, e = 0, hd = -1;
-    if (valid) {
-        b = v.cell_start[cid]; e = v.cell_start[cid + 1];
-        if (chains) hd = v.head[cid];
-    }
-    // own cell: the whole warp
-    Top2 tmp;
-    tmp.init();
-    const int ob = __shfl_sync(0xffffffffu, b, OWN), oe = __shfl_sync(0xffffffffu, e, OWN);
-    coop_range<D>(v, lane, ob, oe, qx, qy, qz, self, CUDART_INF_F, KC_NOIDX, KC_NOIDX, tmp);
-    if (lane == OWN)
-        for (int c = hd; c >= 0; c = v.next[c]) {
-            const float4 o = v.opos[c];
-            lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, o.x, o.y) : sqd3(qx, qy, qz, o.x, o.y, o.z), c, CUDART_INF_F, self);
-        }
-    float sa, sb;
-    int ja, jb;
-    coop_pop(tmp, sa, ja);
-    coop_pop(tmp, sb, jb);
-    best.s1 = sa; best.j1 = ja; best.s2 = sb; best.j2 = jb;         // ordered: sa <= sb (or none)
-    const float thr = best.s2;
-    // the other cells: prune, then short ranges by their lanes, long ones by the warp
-    const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
-    const float lb2 = __fadd_rn(__fadd_rn(ox < 0 ? g.xm : (ox > 0 ? g.xp : 0.f), oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f)),
-                                oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
-    const bool need = valid && lane != OWN && !(thr < lb2);
-    const int len = need ? e - b : 0;
-    tmp.init();
-    for (unsigned m = __ballot_sync(0xffffffffu, len > 16); m; m &= m - 1) {
-        const int L = __ffs(m) - 1;
-        coop_range<D>(v, lane, __shfl_sync(0xffffffffu, b, L), __shfl_sync(0xffffffffu, e, L), qx, qy, qz, self,
-                      thr, KC_NOIDX, KC_NOIDX, tmp);
-    }
-    if (len <= 16)
-        for (int t0 = b; t0 < b + len; t0 += 4) {        // 4 records per round trip, loads issued together
-            const float qnan = __int_as_float(0x7fc00000);
-            float4 c[4];
-            int j[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const bool ok = t0 + k < b + len;
-                if (D == 2) {
-                    const float2 r = ok ? v.spos2[t0 + k] : make_float2(qnan, qnan);
-                    c[k] = make_float4(r.x, r.y, 0.f, 0.f);
-                    j[k] = ok ? v.sidx[t0 + k] : -1;
-                } else {
-                    c[k] = ok ? v.spos4[t0 + k] : make_float4(qnan, qnan, qnan, __int_as_float(-1));
-                    j[k] = __float_as_int(c[k].w);
-                }
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k)
-                lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, c[k].x, c[k].y) : sqd3(qx, qy, qz, c[k].x, c[k].y, c[k].z),
-                              j[k], thr, self);
-        }
-    if (need)
-        for (int c = hd; c >= 0; c = v.next[c]) {
-            const float4 o = v.opos[c];
-            lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, o.x, o.y) : sqd3(qx, qy, qz, o.x, o.y, o.z), c, thr, self);
-        }
-    coop_pop(tmp, sa, ja);
-    coop_pop(tmp, sb, jb);
-    if (ja != KC_NOIDX) best.offer(sa, ja);
-    if (jb != KC_NOIDX) best.offer(sb, jb);
-    // every lane holds the same state: the rare ring continuation runs redundantly on all of them
-    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
-}
-
-template <int D, bool SLOTS>
-__global__ void __launch_bounds__(128)
-search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__restrict__ F,
-                  const int32_t *__restrict__ nF, const int32_t *__restrict__ list2, int sweep_div,
-                  Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
-{
-    const int lane = threadIdx.x & 31;
-    const int w0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
-    int n = N;
-    const int32_t *__restrict__ Q = nullptr;
-    bool chains = false;
-    if (!SLOTS) {
-        // a large frontier is served by the slot sweep; only its chain residents (list2) come here
-        const bool swept = sweep_div > 0 && (int64_t)*nF * sweep_div >= N;
-        n = swept ? ctr->n_list2 : *nF;
-        Q = swept ? list2 : F;
-        chains = ctr->n_misfiled > 0;
-    }
-    if (!SLOTS && n > v.wpq_max) {
-        // long list: one thread per query keeps more queries in flight
-        for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
-            const int i = Q[f];
-            const float qx = p_new[(int64_t)i * D], qy = p_new[(int64_t)i * D + 1];
-            const float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
-            Top2 best;
-            best.init();
-            const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-            const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-            const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-            const int r = block_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
-            if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-            store_cert(best, i, nn, nn2, d1, d2, c);
-        }
-        return;
-    }
-    for (int f = w0; f < n; f += nw) {
-        float qx, qy, qz = 0.f;
-        int i;
-        if (SLOTS) {
-            if (D == 2) { const float2 q = v.spos2[f]; qx = q.x; qy = q.y; i = v.sidx[f]; }
-            else { const float4 q = v.spos4[f]; qx = q.x; qy = q.y; qz = q.z; i = __float_as_int(q.w); }
-        } else {
-            i = Q[f];
-            qx = p_new[(int64_t)i * D]; qy = p_new[(int64_t)i * D + 1];
-            if (D == 3) qz = p_new[(int64_t)i * D + 2];
-        }
-        Top2 best;
-        const int r = wpq_search<D>(v, chains, lane, qx, qy, qz, i, best);
-        if (lane == 0) {
-            if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-            store_cert(best, i, nn, nn2, d1, d2, c);
-        }
-    }
-}
-
-// ---- NEXT #4: K-list certificates through the grid ---------------------------------------------
-// One thread per sorted slot of a freshly built grid: own cell, then Chebyshev rings, until the
-// bound of the scanned block exceeds the K-th best distance (the same strict test as A3, with
-// s_K in the place of s_2: every unscanned point is then strictly farther than the K-th key).
-template <int D, int K>
-__device__ __forceinline__ void topk_scan_cells(const View &v, int rowbase, int x0, int x1, float qx, float qy,
-                                                float qz, int self, TopK<K> &best)
-{
-    const int b = v.cell_start[rowbase + x0], e = v.cell_start[rowbase + x1 + 1];
-    for (int t = b; t < e; ++t) {
-        float s;
-        int j;
-        if (D == 2) {
-            const float2 c = v.spos2[t];
-            s = sqd2(qx, qy, c.x, c.y);
-            j = v.sidx[t];
-        } else {
-            const float4 c = v.spos4[t];
-            s = sqd3(qx, qy, qz, c.x, c.y, c.z);
-            j = __float_as_int(c.w);
-        }
-        if (s <= best.s[K - 1] && j >= 0 && j != self) best.offer(s, j);
-    }
-}
-template <int D, int K>
-__global__ void __launch_bounds__(128)
-search_topk_kernel(View v, int N, int32_t *__restrict__ nnk, float *__restrict__ dk, float *__restrict__ ck)
-{
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    float qx, qy, qz = 0.f;
-    int self;
-    if (D == 2) {
-        const float2 q = v.spos2[s];
-        qx = q.x; qy = q.y; self = v.sidx[s];
-    } else {
-        const float4 q = v.spos4[s];
-        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
-    }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    TopK<K> best;
-    best.init();
-    topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-    for (int r = 0;;) {
-        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
-        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
-        ++r;
-        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
-        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y) {
-                const int rowbase = (z * v.G1 + y) * v.G0;
-                const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
-                if (shell) {
-                    topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                } else {
-                    if (cx - r >= 0) topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                    if (cx + r <= v.G0 - 1) topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                }
-            }
-    }
-    best.store(self, nnk, dk, ck);
-}
-// K-list repair (A7 for K keys): one thread per id of the list, against the incrementally updated
-// grid: tombstones are inert records, the overflow chain of every visited cell is scanned too.
-template <int D, int K>
-__device__ __forceinline__ void topk_scan_chains(const View &v, int rowbase, int x0, int x1, float qx, float qy,
-                                                 float qz, int self, TopK<K> &best)
-{
-    for (int x = x0; x <= x1; ++x)
-        for (int e = v.head[rowbase + x]; e >= 0; e = v.next[e]) {
-            const float4 c = v.opos[e];
-            const float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
-            if (s <= best.s[K - 1] && e != self) best.offer(s, e);
-        }
-}
-template <int D, int K>
-__global__ void __launch_bounds__(128)
-search_topk_list_kernel(View v, const float *__restrict__ p_new, const int32_t *__restrict__ F,
-                        const int32_t *__restrict__ nF, const Counters *ctr, int32_t *__restrict__ nnk,
-                        float *__restrict__ dk, float *__restrict__ ck)
-{
-    const int n = *nF;
-    const bool chains = ctr->n_misfiled > 0;
-    for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
-        const int self = F[f];
-        const float qx = p_new[(int64_t)self * D], qy = p_new[(int64_t)self * D + 1];
-        const float qz = D == 3 ? p_new[(int64_t)self * D + 2] : 0.f;
-        const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-        const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-        const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-        TopK<K> best;
-        best.init();
-        topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-        if (chains) topk_scan_chains<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-        for (int r = 0;;) {
-            int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-            int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
-            int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-            if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
-            ++r;
-            z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-            y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
-            x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-            for (int z = z0; z <= z1; ++z)
-                for (int y = y0; y <= y1; ++y) {
-                    const int rowbase = (z * v.G1 + y) * v.G0;
-                    const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
-                    if (shell) {
-                        topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                        if (chains) topk_scan_chains<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                    } else {
-                        if (cx - r >= 0) {
-                            topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                        }
-                        if (cx + r <= v.G0 - 1) {
-                            topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                        }
-                    }
-                }
-        }
-        best.store(self, nnk, dk, ck);
-    }
-}
-template <int D>
-bool dispatch_list_topk(int K, const View &v, const float *p_new, const int32_t *F, const int32_t *nF, int64_t nF_max,
-                        const Counters *ctr, int32_t *nnk, float *dk, float *ck, cudaStream_t st)
-{
-    int64_t want = (nF_max + 127) / 128;
-    const int nb = (int)(want < 1 ? 1 : (want < 148 * 16 ? want : 148 * 16));
-    switch (K) {
-    case 2: search_topk_list_kernel<D, 2><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 3: search_topk_list_kernel<D, 3><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 4: search_topk_list_kernel<D, 4><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 5: search_topk_list_kernel<D, 5><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 6: search_topk_list_kernel<D, 6><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 7: search_topk_list_kernel<D, 7><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    case 8: search_topk_list_kernel<D, 8><<<nb, 128, 0, st>>>(v, p_new, F, nF, ctr, nnk, dk, ck); return true;
-    default: return false;
-    }
-}
-template <int D>
-bool dispatch_grid_topk(int K, const View &v, int n, int32_t *nnk, float *dk, float *ck, cudaStream_t st)
-{
-    const int nb = (n + 127) / 128;
-    switch (K) {
-    case 2: search_topk_kernel<D, 2><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 3: search_topk_kernel<D, 3><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 4: search_topk_kernel<D, 4><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 5: search_topk_kernel<D, 5><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 6: search_topk_kernel<D, 6><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 7: search_topk_kernel<D, 7><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    case 8: search_topk_kernel<D, 8><<<nb, 128, 0, st>>>(v, n, nnk, dk, ck); return true;
-    default: return false;
-    }
 }
 
 // ------------------------------------------------------------------ A6 incremental update
@@ -1475,22 +508,6 @@ classify_local_kernel(View v, float R, int N, const int32_t *__restrict__ cell,
     if (infr) F[bbase + wsum[warp] + __popc(m & ((1u << lane) - 1))] = i;
 }
 
-inline int blocks_for(int64_t n, int threads, int cap = 148 * 16)
-{
-    int64_t b = (n + threads - 1) / threads;
-    if (b < 1) b = 1;
-    return (int)(b < cap ? b : cap);
-}
-
-kc_status check_certs(const int32_t *nn, const float *d1, const float *d2, const float *c, const char *who)
-{
-    if (!nn || !d1 || !d2 || !c) {
-        set_error("%s: nn, d1, d2, c must be non-NULL", who);
-        return KC_EINVAL;
-    }
-    return KC_OK;
-}
-
 }  // namespace
 
 // ====================================================================== C-ABI
@@ -1603,86 +620,6 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     return KC_OK;
 }
 
-extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2,
-                                         float *c, void *stream)
-{
-    if (!g) { set_error("kc_cert_grid_search: NULL grid"); return KC_EINVAL; }
-    kc_status s = check_certs(nn, d1, d2, c, "kc_cert_grid_search");
-    if (s != KC_OK) return s;
-    if (!g->built || g->dirty) {
-        set_error("kc_cert_grid_search: grid is not freshly built");
-        return KC_EREBUILD;
-    }
-    cudaStream_t st = (cudaStream_t)stream;
-    View v = make_view(g);
-    const int n = (int)g->N;
-    static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 1;
-    const int tb = 32 * WT_WARPS;
-    if (variant == 1) {
-        if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-        else search_tiled_kernel<3, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-    } else if (variant == 2) {
-        const int blocks = blocks_for(n, 4, 148 * 16);
-        if (g->geom.d == 2) search_wpq_kernel<2, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
-        else search_wpq_kernel<3, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
-    } else {
-        if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-        else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-    }
-    count_launches(1);
-    KC_LAUNCH_CHECK("kc_cert_grid_search");
-    return KC_OK;
-}
-
-extern "C" kc_status kc_cert_grid_rebuild(kc_grid *g, const float *p, int64_t N, int32_t *nn,
-                                          int32_t *nn2, float *d1, float *d2, float *c, void *stream)
-{
-    kc_status s = check_certs(nn, d1, d2, c, "kc_cert_grid_rebuild");
-    if (s != KC_OK) return s;
-    s = kc_grid_build(g, p, N, stream);
-    if (s != KC_OK) return s;
-    return kc_cert_grid_search(g, nn, nn2, d1, d2, c, stream);
-}
-
-extern "C" kc_status kc_cert_grid_topk(kc_grid *g, int K, int32_t *nnk, float *dk, float *ck, void *stream)
-{
-    if (!g || !nnk || !dk || !ck || K < 2 || K > KC_TOPK_MAX) {
-        set_error("kc_cert_grid_topk: bad argument (need grid, nnk, dk, ck, 2 <= K <= %d)", KC_TOPK_MAX);
-        return KC_EINVAL;
-    }
-    if (!g->built || g->dirty) {
-        set_error("kc_cert_grid_topk: grid is not freshly built");
-        return KC_EREBUILD;
-    }
-    const View v = make_view(g);
-    if (g->geom.d == 2) dispatch_grid_topk<2>(K, v, (int)g->N, nnk, dk, ck, (cudaStream_t)stream);
-    else dispatch_grid_topk<3>(K, v, (int)g->N, nnk, dk, ck, (cudaStream_t)stream);
-    count_launches(1);
-    KC_LAUNCH_CHECK("kc_cert_grid_topk");
-    return KC_OK;
-}
-
-extern "C" kc_status kc_frontier_search_topk(kc_grid *g, const float *p_new, int64_t N, const int32_t *F,
-                                             const int32_t *nF, int64_t nF_max, int K, int32_t *nnk, float *dk,
-                                             float *ck, void *stream)
-{
-    if (!g || !p_new || !F || !nF || nF_max < 0 || !nnk || !dk || !ck || K < 2 || K > KC_TOPK_MAX) {
-        set_error("kc_frontier_search_topk: bad argument (2 <= K <= %d)", KC_TOPK_MAX);
-        return KC_EINVAL;
-    }
-    if (!g->built || N != g->N) {
-        set_error("kc_frontier_search_topk: grid not built for this N");
-        return KC_EREBUILD;
-    }
-    if (nF_max == 0) return KC_OK;
-    const View v = make_view(g);
-    if (g->geom.d == 2) dispatch_list_topk<2>(K, v, p_new, F, nF, nF_max, g->ctr, nnk, dk, ck, (cudaStream_t)stream);
-    else dispatch_list_topk<3>(K, v, p_new, F, nF, nF_max, g->ctr, nnk, dk, ck, (cudaStream_t)stream);
-    count_launches(1);
-    KC_LAUNCH_CHECK("kc_frontier_search_topk");
-    return KC_OK;
-}
-
 extern "C" kc_status kc_frontier_classify_local(kc_grid *g, const float *p, const float *p2, int64_t N,
                                                 const int32_t *nn, const float *d1, const float *c,
                                                 const float *eps, uint8_t *flags, int32_t *F, int32_t *nF,
@@ -1766,70 +703,6 @@ extern "C" kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, c
     g->dirty = 1;
     KC_LAUNCH_CHECK("kc_grid_update");
     return KC_OK;
-}
-
-// A7, Algorithm 1 lines 4-7: re-search the frontier only.  On a large grid a
-// frontier of at least N / sweep_div points (decided on the device from *nF) is served in slot
-// order by the tiled sweep, anything else straight from the id list (one warp per query while the
-// list is short: latency; one thread per query when it is long: throughput); both kernels are
-// launched when the host bound allows either.
-extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const int32_t *F,
-                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
-                                        float *d1, float *d2, float *c, void *stream)
-{
-    if (!g || !p_new || !F || !nF || nF_max < 0) {
-        set_error("kc_frontier_search: bad argument");
-        return KC_EINVAL;
-    }
-    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_search");
-    if (s != KC_OK) return s;
-    if (!g->built || N != g->N) {
-        set_error("kc_frontier_search: grid not built for this N");
-        return KC_EREBUILD;
-    }
-    if (nF_max == 0) return KC_OK;
-    cudaStream_t st = (cudaStream_t)stream;
-    View v = make_view(g);
-    const int n = (int)N;
-    static const int div_env = getenv("KC_SWEEP_DIV") ? atoi(getenv("KC_SWEEP_DIV")) : 8;
-    static const int min_env = getenv("KC_SWEEP_MIN_N") ? atoi(getenv("KC_SWEEP_MIN_N")) : 200000;
-    const int sweep_div = N >= min_env && nF_max * (int64_t)div_env >= N ? div_env : 0;
-    const int tb = 32 * WT_WARPS;
-    if (sweep_div > 0) {
-        ++g->epoch;
-        mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
-        if (g->geom.d == 2)
-            search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-        else
-            search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-        count_launches(2);
-    }
-    int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
-    if (nF_max > v.wpq_max) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
-    if (g->geom.d == 2)
-        search_wpq_kernel<2, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
-    else
-        search_wpq_kernel<3, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
-    count_launches(1);
-    KC_LAUNCH_CHECK("kc_frontier_search");
-    return KC_OK;
-}
-
-// A6 + A7 in one call.
-extern "C" kc_status kc_frontier_repair(kc_grid *g, const float *p_new, int64_t N, const int32_t *movers,
-                                        const int32_t *n_movers, int64_t n_movers_max, const int32_t *F,
-                                        const int32_t *nF, int64_t nF_max, int32_t *nn, int32_t *nn2,
-                                        float *d1, float *d2, float *c, void *stream)
-{
-    if (!F || !nF || nF_max < 0) {
-        set_error("kc_frontier_repair: bad argument");
-        return KC_EINVAL;
-    }
-    kc_status s = check_certs(nn, d1, d2, c, "kc_frontier_repair");
-    if (s != KC_OK) return s;
-    s = kc_grid_update(g, p_new, N, movers, n_movers, n_movers_max, stream);
-    if (s != KC_OK) return s;
-    return kc_frontier_search(g, p_new, N, F, nF, nF_max, nn, nn2, d1, d2, c, stream);
 }
 
 extern "C" kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream)

@@ -27,6 +27,43 @@ kc_status cuda_fail(cudaError_t e, const char *where)
     return KC_ECUDA;
 }
 
+static std::atomic<int *> g_errword_host{nullptr};
+static std::atomic<int *> g_errword_dev{nullptr};
+static std::atomic_flag g_errword_busy = ATOMIC_FLAG_INIT;
+
+void error_word_init()
+{
+    if (g_errword_dev.load(std::memory_order_acquire)) return;
+    if (g_errword_busy.test_and_set()) return;             // another thread is at it
+    // a host allocation is a "potentially unsafe" call while a stream capture is in progress in
+    // global mode: make it in relaxed mode (it touches no stream) and restore the thread's mode
+    cudaStreamCaptureMode m = cudaStreamCaptureModeRelaxed;
+    cudaThreadExchangeStreamCaptureMode(&m);
+    int *h = nullptr, *d = nullptr;
+    if (!g_errword_dev.load() && cudaHostAlloc((void **)&h, sizeof(int), cudaHostAllocMapped) == cudaSuccess) {
+        *h = 0;
+        if (cudaHostGetDevicePointer((void **)&d, h, 0) == cudaSuccess) {
+            g_errword_host.store(h, std::memory_order_release);
+            g_errword_dev.store(d, std::memory_order_release);
+        } else {
+            cudaFreeHost(h);
+        }
+    }
+    cudaGetLastError();
+    cudaThreadExchangeStreamCaptureMode(&m);
+    g_errword_busy.clear();
+}
+int *error_word_dev() { return g_errword_dev.load(std::memory_order_acquire); }
+int error_word_take()
+{
+    int *h = g_errword_host.load(std::memory_order_acquire);
+    if (!h) return 0;
+    volatile int *vh = h;
+    const int v = *vh;
+    if (v) *vh = 0;
+    return v;
+}
+
 }  // namespace kc
 
 using namespace kc;

@@ -595,3 +595,68 @@ def test_bbox_device():
     assert np.array_equal(b[:3], p.min(0)) and np.array_equal(b[3:], p.max(0))
     lo, hi = oracle.bbox(p)
     assert np.array_equal(b[:3], lo) and np.array_equal(b[3:], hi)
+
+
+def test_allpairs_dirty_workspace_is_reported_not_trapped():
+    """A workspace that was never zero-filled (kc.h, workspace contract) must not poison the CUDA
+    context: the kernel reports through the error word, the NEXT all-pairs call returns KC_EINVAL
+    after clearing the counters, and the call after that is exact again."""
+    p = wl.make_points("cfg2")
+    N, d = p.shape
+    want = ref_certs(p)
+    P = dev(p)
+    need = kc.lib().kc_cert_allpairs_workspace(N, d)
+    ws = torch.full((need + 64,), 0x7f, dtype=torch.uint8, device="cuda")      # counters hold 0x7f7f7f7f
+    kc.kc_cert_allpairs(P, workspace=ws, seed1=dev(want.nn), seed2=dev(want.nn2))   # j-split launch
+    torch.cuda.synchronize()                                     # the context is still alive
+    with pytest.raises(kc.KcError) as e:
+        kc.kc_cert_allpairs(P, workspace=ws)
+    assert e.value.status == kc.KC_EINVAL and "zero-filled" in str(e.value)
+    assert_same(kc.kc_cert_allpairs(P, workspace=ws), want, what="after the report")
+    assert_same(kc.kc_cert_allpairs(P, workspace=ws, seed1=dev(want.nn), seed2=dev(want.nn2)), want,
+                what="seeded after the report")
+
+
+def test_frontier_search_twice_on_one_update():
+    """Two sweep-sized kc_frontier_search calls after ONE kc_grid_update: the second must not
+    replay the chain residents of the first (entries outside its list stay untouched)."""
+    N = 230_000
+    p = wl.uniform_points(N, 2, 77)
+    rng = np.random.default_rng(78)
+    q = (p + rng.uniform(-2e-3, 2e-3, p.shape)).astype(np.float32)      # many points change cell
+    grid = kc.Grid(N, geoms(p)[1])
+    certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+    Q = dev(q)
+    kc.kc_grid_update(grid, Q)
+    assert grid.info().n_misfiled > N // 20
+    post = ref_certs(q)
+    perm = rng.permutation(N).astype(np.int32)
+    F1, F2 = np.sort(perm[: N // 2]), np.sort(perm[N // 2: N // 2 + N // 4])
+    sentinel = kc.Certs.empty(N)
+    for name in ("nn", "nn2"):
+        getattr(sentinel, name).fill_(-7)
+    for name in ("d1", "d2", "c"):
+        getattr(sentinel, name).fill_(-7.0)
+    for F in (F1, F2, F1):
+        out = sentinel.clone()
+        kc.kc_frontier_search(grid, Q, dev(F), dev(np.array([F.size], np.int32)), out)
+        got = host(out)
+        assert_same(got, post, idx=F, what="searched entries")
+        rest = np.setdiff1d(np.arange(N), F)
+        assert np.all(got.nn[rest] == -7) and np.all(got.c[rest] == -7.0), "entries outside F were written"
+
+
+@pytest.mark.parametrize("N", [1001, 1002, 1003])
+def test_maintainer_any_N(N):
+    """Certs.empty keeps every row 16-byte aligned for N that is not a multiple of 4."""
+    from paper_2606_18314_b200.driver import Maintainer
+    p, mot = wl.make_scene("cfg1", N=N)
+    q, _ = mot.step(p)
+    m = Maintainer(dev(p))
+    res = m.step(dev(q))
+    post = ref_certs(q)
+    assert_same(res.rebuilt, post, what="rebuilt")
+    assert_same(res.certified, post, what="certified")
+    F = oracle.frontier(ref_certs(p).c, oracle.max_displacement(p, q))[1]
+    assert int(res.nF.item()) == F.size
+    assert_same(res.repaired, post, idx=F, what="repaired")
