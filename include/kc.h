@@ -76,6 +76,9 @@ typedef struct {
     int32_t built;       /* 1 once kc_grid_build has run */
     int32_t dirty;       /* 1 once kc_frontier_repair has updated the grid since the build */
     int32_t n_stragglers;/* queries of the last search that needed more than the solo rings */
+    int32_t n_heavy;     /* level-0 cells the last build subdivided (two-level index) */
+    int32_t n_leaves;    /* leaves of the last build: undivided cells + sub-cells */
+    int32_t heavy_T;     /* build-time record count from which a cell is subdivided */
 } kc_grid_info_t;
 
 /* ---- host utilities -------------------------------------------------------------------- */
@@ -312,7 +315,12 @@ kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream);
  *         1: cell_start, int32[n_cells+1]      (exclusive scan of the last build's histogram)
  *         2: sorted_idx, int32[N]              (point id in each sorted slot; -1 = tombstone)
  *         3: slot, int32[N]                    (sorted slot of point i; -1 = in an overflow chain)
- *         4: counts, int32[n_cells]            (live occupancy per cell) */
+ *         4: counts, int32[n_cells]            (live occupancy per cell)
+ *         5: subinfo, int32[2*n_cells]         (two-level index: per cell {S, first leaf}; meaningful
+ *                                               only when kc_grid_info reports n_heavy > 0; S = 0: the
+ *                                               cell is one leaf, else it has S^d sub-cells, x fastest)
+ *         6: leaf_start, int32[n_cells+N+9]    (exclusive scan of the leaf sizes: the first
+ *                                               n_leaves + 1 entries are meaningful) */
 kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, int64_t capacity, int64_t *count,
                          void *stream);
 

@@ -1,26 +1,21 @@
-// kc_grid.cu — the resident uniform grid: A2 build, A3 whole-set ring search, A5 frontier
-// entropy, A6 incremental cell update, A7 frontier-only repair.  Contract: include/kc.h.
+// kc_grid.cu — the resident grid: A2 build (two-level counting sort), A5 frontier entropy, A6
+// incremental cell update, NEXT #2 local motion budget.  Searches: kc_search.cu.  Contract: include/kc.h.
 //
-// Layout in HBM (N points, C_tot cells):
+// Layout in HBM (N points, C_tot level-0 cells; shared declarations in kc_grid.cuh):
 //   cell[N]        int32   current filing cell of point i
 //   counts[C_tot]  int32   live occupancy per cell (histogram, kept current by A6)
-//   cell_start[C_tot+1] int32  exclusive scan of the build histogram (entry c+1 doubles as the
-//                           scatter cursor of cell c during the build)
-//   spos2[N] float2 (d=2) / spos4[N] float4 = (x,y,z,bits(idx)) (d=3)   cell-sorted positions
+//   cell_start[C_tot+1] int32  exclusive scan of the build histogram
+//   subinfo[C_tot] int2    two-level index: {S, first leaf} of every cell (S = 0: not subdivided)
+//   leaf_start[n_leaves+1] int32  exclusive scan of the leaf sizes (entry l+1 doubles as the scatter
+//                           cursor of leaf l during the build)
+//   spos2[N] float2 (d=2) / spos4[N] float4 = (x,y,z,bits(idx)) (d=3)   leaf-sorted positions
 //   sidx[N]        int32   point id per sorted slot (-1 = tombstone)
 //   slot[N]        int32   sorted slot of point i (-1 = lives in an overflow chain)
 //   head[C_tot], next[N], opos[N] float4, mlist[N]   overflow chains of re-filed points (A6)
 //   fcount[C_tot], mhist[]  scratch of A5 (always left zeroed)
 // Rows of cells along x are contiguous in the sorted arrays (linear id has x fastest), so a
-// (2r+1)-cell row segment is ONE contiguous candidate range: two cell_start reads per row.
-#include <math.h>
-#include <stdlib.h>
-
-#include <new>
-
-#include "kc_common.cuh"
-
-using namespace kc;
+// (2r+1)-cell row segment is ONE contiguous candidate range: two cell_start reads per row; the same
+// holds for the sub-cells of a subdivided cell and leaf_start.
 #include <new>
 
 #include "kc_grid.cuh"
@@ -30,9 +25,16 @@ using namespace kc;
 namespace {
 
 constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
-constexpr int SCAN_CHUNK = 2048;   // cells per scan block (256 threads x 8)
+constexpr int SCAN_CHUNK = 2048;   // entries per scan block (256 threads x 8)
+constexpr int SCAN_SMALL_MAX = 16384;   // up to this many entries a scan is one CTA (1024 threads x 16)
 
 // ------------------------------------------------------------------ A2 build
+// A counting sort in two levels.  (1) prep: drop the chains of the previous residency, zero the
+// histograms.  (2) cell id per point + level-0 histogram (one RED per point).  (3) scan over the
+// cells: cell_start, and per cell the sub-resolution S and the index of its first leaf.  (4) only
+// if some cell is subdivided: leaf of every point + leaf histogram.  (5) scan over the leaves.
+// (6) scatter by leaf (returning atomic on the leaf's cursor).  Without a subdivided cell the
+// leaves ARE the cells, steps 4-5 leave at once and the cell scan writes the cursors itself.
 __global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell,
                                     int32_t *head, const Counters *ctr)
 {
@@ -40,17 +42,21 @@ __global__ void clear_chains_kernel(const int32_t *__restrict__ mlist, const int
     for (int e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x)
         head[cell[mlist[e]]] = -1;
 }
-// start of a build: drop the overflow chains of the previous residency and empty the histogram
+__device__ __forceinline__ void zero_i32(int32_t *a, int64_t n, int64_t t0, int64_t nt)
+{
+    int4 *a4 = reinterpret_cast<int4 *>(a);                // cudaMalloc'ed: 256-byte aligned
+    for (int64_t k = t0; k < n / 4; k += nt) a4[k] = make_int4(0, 0, 0, 0);
+    for (int64_t k = (n & ~(int64_t)3) + t0; k < n; k += nt) a[k] = 0;
+}
 __global__ void __launch_bounds__(256)
 build_prep_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell, int32_t *head,
-                  const Counters *ctr, int32_t *counts, int n_cells)
+                  Counters *ctr, int32_t *counts, int n_cells, int32_t *leaf_cnt, int64_t n_leaves_max)
 {
     const int n = ctr->n_misfiled;
-    const int t0 = blockIdx.x * blockDim.x + threadIdx.x, nt = gridDim.x * blockDim.x;
-    for (int e = t0; e < n; e += nt) head[cell[mlist[e]]] = -1;
-    int4 *c4 = reinterpret_cast<int4 *>(counts);
-    for (int k = t0; k < n_cells / 4; k += nt) c4[k] = make_int4(0, 0, 0, 0);
-    for (int k = (n_cells & ~3) + t0; k < n_cells; k += nt) counts[k] = 0;
+    const int64_t t0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, nt = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t e = t0; e < n; e += nt) head[cell[mlist[e]]] = -1;
+    zero_i32(counts, n_cells, t0, nt);
+    zero_i32(leaf_cnt, n_leaves_max, t0, nt);
 }
 
 template <int D>
@@ -61,7 +67,7 @@ cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restri
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {          // the chains were dropped by the previous kernel; the scan recounts C
         ctr->n_misfiled = 0; ctr->c_occ = 0; ctr->max_occ = 0; ctr->n_stragglers = 0;
-        ctr->n_list2 = 0;
+        ctr->n_list2 = 0; ctr->n_heavy = 0; ctr->n_leaves = 0;
     }
     if (i >= N) return;
     float x, y, z = 0.f;
@@ -76,116 +82,153 @@ cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restri
     atomicAdd(&counts[cidx], 1);                  // result unused: compiles to a RED
 }
 
+__device__ __forceinline__ int ipow_d(int S, int d) { return d == 2 ? S * S : S * S * S; }
+
+// Exclusive scan over the block of one pair per thread; wsum: shared int2[32]; returns this
+// thread's exclusive offsets.  Every thread of the block must call it.
+__device__ __forceinline__ int2 block_excl_scan2(int a, int b, int2 *wsum)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    int ia = a, ib = b;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+        if (lane >= o) { ia += ta; ib += tb; }
+    }
+    __syncthreads();                               // wsum may still be read from a previous call
+    if (lane == 31) wsum[w] = make_int2(ia, ib);
+    __syncthreads();
+    if (w == 0) {
+        const int2 x = lane < nw ? wsum[lane] : make_int2(0, 0);
+        int xa = x.x, xb = x.y;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int ta = __shfl_up_sync(0xffffffffu, xa, o), tb = __shfl_up_sync(0xffffffffu, xb, o);
+            if (lane >= o) { xa += ta; xb += tb; }
+        }
+        wsum[lane] = make_int2(xa - x.x, xb - x.y);   // exclusive warp offsets
+    }
+    __syncthreads();
+    const int2 off = wsum[w];
+    return make_int2(off.x + ia - a, off.y + ib - b);
+}
+
+// ---- scan over the cells: {records, leaves} --------------------------------------------------
 __global__ void __launch_bounds__(256)
-scan_reduce_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *blocksums, Counters *ctr)
+scan_reduce_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ, int2 *blocksums,
+                   Counters *ctr)
 {
     int base = blockIdx.x * SCAN_CHUNK;
-    int sum = 0, occ = 0, mx = 0;
+    int sum = 0, lv = 0, occ = 0, mx = 0, hv = 0;
 #pragma unroll
     for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
         int idx = base + k * 256 + threadIdx.x;
-        int cnt = idx < n_cells ? counts[idx] : 0;
-        sum += cnt; occ += cnt > 0; mx = max(mx, cnt);
+        if (idx < n_cells) {
+            const int cnt = counts[idx];
+            const int S = sub_res(cnt, d, heavy_T, sub_occ);
+            sum += cnt; occ += cnt > 0; mx = max(mx, cnt);
+            lv += S ? ipow_d(S, d) : 1; hv += S > 0;
+        }
     }
     sum = __reduce_add_sync(0xffffffffu, sum);
+    lv = __reduce_add_sync(0xffffffffu, lv);
     occ = __reduce_add_sync(0xffffffffu, occ);
+    hv = __reduce_add_sync(0xffffffffu, hv);
     mx = __reduce_max_sync(0xffffffffu, mx);
-    __shared__ int s_sum[8], s_occ[8], s_mx[8];
+    __shared__ int s_sum[8], s_lv[8], s_occ[8], s_mx[8], s_hv[8];
     int w = threadIdx.x >> 5;
-    if ((threadIdx.x & 31) == 0) { s_sum[w] = sum; s_occ[w] = occ; s_mx[w] = mx; }
+    if ((threadIdx.x & 31) == 0) { s_sum[w] = sum; s_lv[w] = lv; s_occ[w] = occ; s_mx[w] = mx; s_hv[w] = hv; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int a = 0, b = 0, c = 0;
-        for (int k = 0; k < 8; ++k) { a += s_sum[k]; b += s_occ[k]; c = max(c, s_mx[k]); }
-        blocksums[blockIdx.x] = a;
+        int a = 0, l = 0, b = 0, c = 0, e = 0;
+        for (int k = 0; k < 8; ++k) { a += s_sum[k]; l += s_lv[k]; b += s_occ[k]; c = max(c, s_mx[k]); e += s_hv[k]; }
+        blocksums[blockIdx.x] = make_int2(a, l);
         if (b) atomicAdd(&ctr->c_occ, b);
+        if (e) atomicAdd(&ctr->n_heavy, e);
         atomicMax(&ctr->max_occ, c);
     }
 }
-// exclusive scan of blocksums[0..nb) in place, one CTA of 1024 threads, carry across segments
-__global__ void __launch_bounds__(1024) scan_blocksums_kernel(int32_t *blocksums, int nb)
+// exclusive scan of blocksums[0..nb) in place (both components), one CTA of 1024 threads, carry
+// across segments; the total of the second component goes to *total_y if given
+__global__ void __launch_bounds__(1024) scan_blocksums_kernel(int2 *blocksums, int nb, int *total_y)
 {
-    __shared__ int wsum[32];
-    __shared__ int carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
+    __shared__ int2 wsum[32];
+    __shared__ int2 carry_s;
+    if (threadIdx.x == 0) carry_s = make_int2(0, 0);
     __syncthreads();
     for (int base = 0; base < nb; base += 1024) {
-        int idx = base + threadIdx.x;
-        int v = idx < nb ? blocksums[idx] : 0;
-        int incl = v;
-        int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += t;
-        }
-        if (lane == 31) wsum[w] = incl;
+        const int idx = base + threadIdx.x;
+        const int2 v = idx < nb ? blocksums[idx] : make_int2(0, 0);
+        const int2 e = block_excl_scan2(v.x, v.y, wsum);
+        const int2 carry = carry_s;
+        if (idx < nb) blocksums[idx] = make_int2(carry.x + e.x, carry.y + e.y);
         __syncthreads();
-        if (w == 0) {
-            int x = wsum[lane], xi = x;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int t = __shfl_up_sync(0xffffffffu, xi, o);
-                if (lane >= o) xi += t;
-            }
-            wsum[lane] = xi - x;   // exclusive warp offsets
-        }
+        if (threadIdx.x == 1023) carry_s = make_int2(carry.x + e.x + v.x, carry.y + e.y + v.y);
         __syncthreads();
-        int carry = carry_s;
-        int excl = carry + wsum[w] + incl - v;
-        if (idx < nb) blocksums[idx] = excl;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = excl + v;
-        __syncthreads();
+    }
+    if (threadIdx.x == 0 && total_y) *total_y = carry_s.y;
+}
+// One cell of the scan's output.  With a subdivided cell anywhere in the grid: subinfo and, for an
+// undivided cell, the size of its single leaf (the leaf scan follows).  Without one: leaf = cell,
+// so the scatter cursor is written straight away (leaf_start[c + 1] = start of c).
+__device__ __forceinline__ void scan_emit(int c, int cnt, int S, int run, int lrun, bool any_heavy,
+                                          int32_t *cell_start, int2 *subinfo, int32_t *leaf_cnt,
+                                          int32_t *leaf_start)
+{
+    cell_start[c] = run;
+    if (any_heavy) {
+        subinfo[c] = make_int2(S, lrun);
+        if (!S) leaf_cnt[lrun] = cnt;
+    } else {
+        leaf_start[c + 1] = run;
     }
 }
 __global__ void __launch_bounds__(256)
-scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, const int32_t *__restrict__ blocksums,
-                  int32_t *__restrict__ cell_start, int N)
+scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ,
+                  const int2 *__restrict__ blocksums, int32_t *__restrict__ cell_start,
+                  int2 *__restrict__ subinfo, int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start,
+                  const Counters *ctr, int N)
 {
     // thread t owns 8 consecutive cells
-    int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
-    int v[8];
-    int tsum = 0;
+    __shared__ int2 wsum[32];
+    const bool any_heavy = ctr->n_heavy > 0;
+    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
+    int v[8], S[8];
+    int tsum = 0, tl = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         v[k] = base + k < n_cells ? counts[base + k] : 0;
+        S[k] = sub_res(v[k], d, heavy_T, sub_occ);
         tsum += v[k];
+        tl += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
     }
-    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    int incl = tsum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    __shared__ int wsum[8];
-    if (lane == 31) wsum[w] = incl;
-    __syncthreads();
-    int off = blocksums[blockIdx.x];
-    for (int k = 0; k < w; ++k) off += wsum[k];
-    int run = off + incl - tsum;
+    const int2 e = block_excl_scan2(tsum, tl, wsum);
+    const int2 off = blocksums[blockIdx.x];
+    int run = off.x + e.x, lrun = off.y + e.y;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        // stored one slot to the right: cell_start[c+1] is the scatter cursor of cell c and ends
-        // up as start[c] + count[c] = start[c+1], i.e. the array becomes the exclusive scan itself
-        if (base + k < n_cells) cell_start[base + k + 1] = run;
+        if (base + k < n_cells)
+            scan_emit(base + k, v[k], S[k], run, lrun, any_heavy, cell_start, subinfo, leaf_cnt, leaf_start);
         run += v[k];
+        lrun += S[k] ? ipow_d(S[k], d) : 1;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) cell_start[0] = 0;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        cell_start[n_cells] = N;
+        leaf_start[0] = 0;
+    }
 }
-
-// Small grids: the whole scan in one CTA (thread t owns PER consecutive cells).
-constexpr int SCAN_SMALL_MAX = 16384;
+// Small grids: the whole cell scan in one CTA (thread t owns 16 consecutive cells).
 __global__ void __launch_bounds__(1024)
-scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *__restrict__ cell_start,
-                  Counters *ctr)
+scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ,
+                  int32_t *__restrict__ cell_start, int2 *__restrict__ subinfo, int32_t *__restrict__ leaf_cnt,
+                  int32_t *__restrict__ leaf_start, Counters *ctr, int N)
 {
-    // thread t owns the 16 cells from 16 t; all its loads are issued before the first is used
+    __shared__ int2 wsum[32];
+    __shared__ int s_heavy;
     const int base = threadIdx.x * 16;
-    int v[16];
+    int v[16], S[16];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < 4; ++q) {                 // all loads issued before the first is used
         const int i = base + 4 * q;
         int4 x = make_int4(0, 0, 0, 0);
         if (i + 3 < n_cells) x = *reinterpret_cast<const int4 *>(counts + i);
@@ -196,49 +239,171 @@ scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int32_t *__re
         }
         v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
     }
-    int tsum = 0, occ = 0, mx = 0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) { tsum += v[k]; occ += v[k] > 0; mx = max(mx, v[k]); }
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    int incl = tsum;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    occ = __reduce_add_sync(0xffffffffu, occ);
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    __shared__ int wsum[32], wocc[32], wmx[32];
-    if (lane == 31) wsum[w] = incl;
-    if (lane == 0) { wocc[w] = occ; wmx[w] = mx; }
-    __syncthreads();
-    if (w == 0) {
-        int x = wsum[lane], xi = x;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            int t = __shfl_up_sync(0xffffffffu, xi, o);
-            if (lane >= o) xi += t;
-        }
-        wsum[lane] = xi - x;
-        const int a = __reduce_add_sync(0xffffffffu, wocc[lane]);
-        const int b = __reduce_max_sync(0xffffffffu, wmx[lane]);
-        if (lane == 0) { ctr->c_occ = a; ctr->max_occ = b; }
-    }
-    __syncthreads();
-    int run = wsum[w] + incl - tsum;
+    int tsum = 0, tl = 0, occ = 0, mx = 0, hv = 0;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-        // stored one slot to the right, as in scan_write_kernel (the scatter's cursors)
-        if (base + k < n_cells) cell_start[base + k + 1] = run;
+        S[k] = sub_res(v[k], d, heavy_T, sub_occ);
+        tsum += v[k]; occ += v[k] > 0; mx = max(mx, v[k]); hv += S[k] > 0;
+        tl += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
+    }
+    if (threadIdx.x == 0) s_heavy = 0;
+    const int2 e = block_excl_scan2(tsum, tl, wsum);      // (syncs: s_heavy is visible after it)
+    occ = __reduce_add_sync(0xffffffffu, occ);
+    hv = __reduce_add_sync(0xffffffffu, hv);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0) {
+        if (occ) atomicAdd(&ctr->c_occ, occ);
+        if (hv) { atomicAdd(&ctr->n_heavy, hv); atomicAdd(&s_heavy, hv); }
+        atomicMax(&ctr->max_occ, mx);
+    }
+    __syncthreads();
+    const bool any_heavy = s_heavy > 0;
+    int run = e.x, lrun = e.y;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        if (base + k < n_cells)
+            scan_emit(base + k, v[k], S[k], run, lrun, any_heavy, cell_start, subinfo, leaf_cnt, leaf_start);
+        run += v[k];
+        lrun += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
+    }
+    if (threadIdx.x == 1023) ctr->n_leaves = lrun;
+    if (threadIdx.x == 0) { cell_start[n_cells] = N; leaf_start[0] = 0; }
+}
+
+// ---- leaf of every point + leaf histogram (only with subdivided cells) ------------------------
+template <int D>
+__global__ void __launch_bounds__(256)
+leafid_hist_kernel(View v, const float *__restrict__ p, int N, const int32_t *__restrict__ cell,
+                   int32_t *leaf_cnt, int32_t *__restrict__ leafid, const Counters *ctr)
+{
+    if (ctr->n_heavy == 0) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int2 si = v.subinfo[cell[i]];
+    int leaf = si.y;
+    if (si.x) {
+        float x, y, z = 0.f;
+        if (D == 2) {
+            float2 t = reinterpret_cast<const float2 *>(p)[i];
+            x = t.x; y = t.y;
+        } else {
+            x = p[3 * (int64_t)i]; y = p[3 * (int64_t)i + 1]; z = p[3 * (int64_t)i + 2];
+        }
+        const int S = si.x;
+        const float fS = (float)S;
+        const int ux = sub_axis(x, v.lo0, v.inv_h, cell_axis(x, v.lo0, v.inv_h, v.G0), fS, S);
+        const int uy = sub_axis(y, v.lo1, v.inv_h, cell_axis(y, v.lo1, v.inv_h, v.G1), fS, S);
+        const int uz = D == 3 ? sub_axis(z, v.lo2, v.inv_h, cell_axis(z, v.lo2, v.inv_h, v.G2), fS, S) : 0;
+        leaf += (uz * S + uy) * S + ux;
+        atomicAdd(&leaf_cnt[leaf], 1);            // RED
+    }
+    leafid[i] = leaf;
+}
+
+// ---- scan over the leaves: leaf_start[l + 1] = start of leaf l (the scatter's cursor) ----------
+__global__ void __launch_bounds__(256)
+lscan_reduce_kernel(const int32_t *__restrict__ leaf_cnt, int2 *blocksums, const Counters *ctr)
+{
+    if (ctr->n_heavy == 0) return;
+    const int n = ctr->n_leaves;
+    const int base = blockIdx.x * SCAN_CHUNK;
+    if (base >= n) { if (threadIdx.x == 0) blocksums[blockIdx.x] = make_int2(0, 0); return; }
+    int sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        const int idx = base + k * 256 + threadIdx.x;
+        sum += idx < n ? leaf_cnt[idx] : 0;
+    }
+    sum = __reduce_add_sync(0xffffffffu, sum);
+    __shared__ int s_sum[8];
+    if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int a = 0;
+        for (int k = 0; k < 8; ++k) a += s_sum[k];
+        blocksums[blockIdx.x] = make_int2(a, 0);
+    }
+}
+__global__ void __launch_bounds__(1024) lscan_blocksums_kernel(int2 *blocksums, int nb, const Counters *ctr)
+{
+    if (ctr->n_heavy == 0) return;
+    __shared__ int2 wsum[32];
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < nb; base += 1024) {
+        const int idx = base + threadIdx.x;
+        const int v = idx < nb ? blocksums[idx].x : 0;
+        const int2 e = block_excl_scan2(v, 0, wsum);
+        const int carry = carry_s;
+        if (idx < nb) blocksums[idx].x = carry + e.x;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = carry + e.x + v;
+        __syncthreads();
+    }
+}
+__global__ void __launch_bounds__(256)
+lscan_write_kernel(const int32_t *__restrict__ leaf_cnt, const int2 *__restrict__ blocksums,
+                   int32_t *__restrict__ leaf_start, const Counters *ctr)
+{
+    if (ctr->n_heavy == 0) return;
+    __shared__ int2 wsum[32];
+    const int n = ctr->n_leaves;
+    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
+    if (blockIdx.x * SCAN_CHUNK >= n) return;
+    int v[8];
+    int tsum = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        v[k] = base + k < n ? leaf_cnt[base + k] : 0;
+        tsum += v[k];
+    }
+    const int2 e = block_excl_scan2(tsum, 0, wsum);
+    int run = blocksums[blockIdx.x].x + e.x;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        if (base + k < n) leaf_start[base + k + 1] = run;
         run += v[k];
     }
-    if (threadIdx.x == 0) cell_start[0] = 0;
+}
+// the same in one CTA, any length (small problems: one launch instead of three)
+__global__ void __launch_bounds__(1024)
+lscan_small_kernel(const int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start, const Counters *ctr)
+{
+    if (ctr->n_heavy == 0) return;
+    __shared__ int2 wsum[32];
+    __shared__ int carry_s;
+    const int n = ctr->n_leaves;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int c0 = 0; c0 < n; c0 += 1024 * 16) {
+        const int base = c0 + threadIdx.x * 16;
+        int v[16];
+        int tsum = 0;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            v[k] = base + k < n ? leaf_cnt[base + k] : 0;
+            tsum += v[k];
+        }
+        const int2 e = block_excl_scan2(tsum, 0, wsum);
+        const int carry = carry_s;
+        int run = carry + e.x;
+#pragma unroll
+        for (int k = 0; k < 16; ++k) {
+            if (base + k < n) leaf_start[base + k + 1] = run;
+            run += v[k];
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = run;
+        __syncthreads();
+    }
 }
 
 template <int D>
 __global__ void __launch_bounds__(256)
 scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ cell,
-               int32_t *cell_start, float2 *__restrict__ spos2, float4 *__restrict__ spos4, int32_t *__restrict__ sidx,
+               const int32_t *__restrict__ leafid, int32_t *leaf_start, const Counters *ctr,
+               float2 *__restrict__ spos2, float4 *__restrict__ spos4, int32_t *__restrict__ sidx,
                int32_t *__restrict__ slot)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -249,7 +414,8 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
         sidx[N + i] = -1;
     }
     if (i >= N) return;
-    int s = atomicAdd(&cell_start[cell[i] + 1], 1);
+    const int leaf = ctr->n_heavy ? leafid[i] : cell[i];
+    int s = atomicAdd(&leaf_start[leaf + 1], 1);
     if (D == 2) {
         spos2[s] = reinterpret_cast<const float2 *>(p)[i];
     } else {
@@ -288,7 +454,22 @@ refresh_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__
             int sl = slot[i];
             bool in_chain = sl < 0;
             if (sl >= 0) {
-                if (cnew == cold) {
+                bool stay = cnew == cold;
+                if (stay && v.cell_start[cold + 1] - v.cell_start[cold] >= v.heavy_T) {
+                    // subdivided cell: the record keeps its slot only if it also stays in its
+                    // sub-cell (the slot still holds the position it was filed under)
+                    const int S = v.subinfo[cold].x;
+                    const float fS = (float)S;
+                    float ox, oy, oz = 0.f;
+                    if (D == 2) { const float2 o = spos2[sl]; ox = o.x; oy = o.y; }
+                    else { const float4 o = spos4[sl]; ox = o.x; oy = o.y; oz = o.z; }
+                    const int kx = cell_axis(x, v.lo0, v.inv_h, v.G0), ky = cell_axis(y, v.lo1, v.inv_h, v.G1);
+                    const int kz = D == 3 ? cell_axis(z, v.lo2, v.inv_h, v.G2) : 0;
+                    stay = sub_axis(x, v.lo0, v.inv_h, kx, fS, S) == sub_axis(ox, v.lo0, v.inv_h, kx, fS, S) &&
+                           sub_axis(y, v.lo1, v.inv_h, ky, fS, S) == sub_axis(oy, v.lo1, v.inv_h, ky, fS, S) &&
+                           (D == 2 || sub_axis(z, v.lo2, v.inv_h, kz, fS, S) == sub_axis(oz, v.lo2, v.inv_h, kz, fS, S));
+                }
+                if (stay) {
                     if (D == 2) spos2[sl] = make_float2(x, y);
                     else spos4[sl] = make_float4(x, y, z, __int_as_float(i));
                 } else {
@@ -530,7 +711,19 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     if (!g) return KC_ENOMEM;
     g->geom = *geom;
     g->N_max = N_max; g->n_cells = n_cells; g->N = 0; g->built = 0; g->dirty = 0; g->bytes = 0;
-    g->n_scan_blocks = (int)((n_cells + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    // leaves: one per undivided cell, S^d <= max(count / sub_occ, 2^d) per subdivided one
+    g->n_leaves_max = n_cells + N_max + 8;
+    if (g->n_leaves_max > 0x7ffffff0) {
+        set_error("kc_grid_create: grid too large");
+        delete g;
+        return KC_EINVAL;
+    }
+    static const int thr_env = getenv("KC_HEAVY_T") ? atoi(getenv("KC_HEAVY_T")) : 0;
+    static const int occ_env = getenv("KC_SUB_OCC") ? atoi(getenv("KC_SUB_OCC")) : 0;
+    g->sub_occ = occ_env > 0 ? occ_env : 4;
+    const int thr_min = g->sub_occ << (geom->d + 1);   // keeps the leaf count within n_leaves_max
+    g->heavy_T = thr_env > 0 ? (thr_env < thr_min ? thr_min : thr_env) : (geom->d == 2 ? 128 : 256);
+    g->n_scan_blocks = (int)((g->n_leaves_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
     bool ok = true;
     auto alloc = [&](void **p, size_t bytes) {
         *p = nullptr;
@@ -545,7 +738,11 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     alloc((void **)&g->head, nc * 4); alloc((void **)&g->next, n * 4);
     alloc((void **)&g->mlist, n * 4); alloc((void **)&g->fcount, nc * 4);
     alloc((void **)&g->mhist, MHIST * 4);
-    alloc((void **)&g->blocksums, (size_t)g->n_scan_blocks * 4 + 4);
+    alloc((void **)&g->blocksums, ((size_t)g->n_scan_blocks + 1) * sizeof(int2));
+    alloc((void **)&g->subinfo, nc * sizeof(int2));
+    alloc((void **)&g->leaf_cnt, (size_t)g->n_leaves_max * 4);
+    alloc((void **)&g->leaf_start, ((size_t)g->n_leaves_max + 1) * 4);
+    alloc((void **)&g->leafid, n * 4);
     alloc((void **)&g->mark, (n + 8) * 4);
     alloc((void **)&g->list2, n * 4);
     alloc((void **)&g->delta, n * 4); alloc((void **)&g->cellmax, nc * 4);
@@ -579,7 +776,7 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
     void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
-                    g->mlist, g->fcount, g->mhist, g->blocksums, g->mark, g->list2, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
+                    g->mlist, g->fcount, g->mhist, g->blocksums, g->subinfo, g->leaf_cnt, g->leaf_start, g->leafid, g->mark, g->list2, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete g;
@@ -597,24 +794,44 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)N, nc = (int)g->n_cells;
-    // drop the overflow chains of the previous residency and empty the histogram, then cell ids +
-    // histogram, scan (one CTA for a small grid), scatter
-    build_prep_kernel<<<blocks_for(nc / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr, g->counts, nc);
-    if (g->geom.d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
+    const int d = g->geom.d, T = g->heavy_T, so = g->sub_occ;
+    // upper bound of the number of leaves of THIS build (the device knows the exact count)
+    const int64_t nl_max = (int64_t)nc + N + 8;
+    const int ncb = (nc + SCAN_CHUNK - 1) / SCAN_CHUNK, nlb = (int)((nl_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    build_prep_kernel<<<blocks_for(nl_max / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr,
+                                                                              g->counts, nc, g->leaf_cnt, nl_max);
+    if (d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     if (nc <= SCAN_SMALL_MAX) {
-        scan_small_kernel<<<1, 1024, 0, st>>>(g->counts, nc, g->cell_start, g->ctr);
-        count_launches(4);
+        scan_small_kernel<<<1, 1024, 0, st>>>(g->counts, nc, d, T, so, g->cell_start, g->subinfo, g->leaf_cnt,
+                                              g->leaf_start, g->ctr, n);
+        count_launches(1);
     } else {
-        scan_reduce_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->ctr);
-        scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, g->n_scan_blocks);
-        scan_write_kernel<<<g->n_scan_blocks, 256, 0, st>>>(g->counts, nc, g->blocksums, g->cell_start, n);
-        count_launches(6);
+        scan_reduce_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, g->blocksums, g->ctr);
+        scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, ncb, &g->ctr->n_leaves);
+        scan_write_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, g->blocksums, g->cell_start, g->subinfo,
+                                               g->leaf_cnt, g->leaf_start, g->ctr, n);
+        count_launches(3);
     }
-    if (g->geom.d == 2)
-        scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+    // second level (these kernels leave at once when no cell is subdivided)
+    if (d == 2) leafid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
+    else leafid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
+    if (nl_max <= 4 * SCAN_SMALL_MAX) {
+        lscan_small_kernel<<<1, 1024, 0, st>>>(g->leaf_cnt, g->leaf_start, g->ctr);
+        count_launches(1);
+    } else {
+        lscan_reduce_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, g->blocksums, g->ctr);
+        lscan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, nlb, g->ctr);
+        lscan_write_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, g->blocksums, g->leaf_start, g->ctr);
+        count_launches(3);
+    }
+    if (d == 2)
+        scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->leafid, g->leaf_start, g->ctr, g->spos2,
+                                                           g->spos4, g->sidx, g->slot);
     else
-        scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->cell_start, g->spos2, g->spos4, g->sidx, g->slot);
+        scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->leafid, g->leaf_start, g->ctr, g->spos2,
+                                                           g->spos4, g->sidx, g->slot);
+    count_launches(4);
     KC_LAUNCH_CHECK("kc_grid_build");
     g->N = N; g->built = 1; g->dirty = 0;
     return KC_OK;
@@ -714,6 +931,8 @@ extern "C" kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream)
     out->n_points = g->N; out->n_cells = g->n_cells;
     out->c_occ = h.c_occ; out->max_occ = h.max_occ; out->n_misfiled = h.n_misfiled;
     out->built = g->built; out->dirty = g->dirty; out->n_stragglers = h.n_stragglers;
+    out->n_heavy = h.n_heavy; out->n_leaves = h.n_heavy ? h.n_leaves : (int32_t)g->n_cells;
+    out->heavy_T = g->heavy_T;
     return KC_OK;
 }
 
@@ -729,6 +948,8 @@ extern "C" kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, in
     case 2: src = g->sidx; n = g->N; break;
     case 3: src = g->slot; n = g->N; break;
     case 4: src = g->counts; n = g->n_cells; break;
+    case 5: src = reinterpret_cast<const int32_t *>(g->subinfo); n = 2 * g->n_cells; break;
+    case 6: src = g->leaf_start; n = g->n_cells + g->N + 9; break;
     default: set_error("kc_grid_export: unknown array %d", what); return KC_EINVAL;
     }
     *count = n;

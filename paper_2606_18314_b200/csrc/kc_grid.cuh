@@ -19,8 +19,41 @@ struct Counters {
     int c_occ_acc;            // recount of the occupied cells in progress (A5 after an incremental update)
     int kmax;                 // largest per-cell frontier count seen by the current A5 call
     int ticket2;              // blocks of the A7 list kernel that are done (the last one empties list2)
+    int n_heavy;              // level-0 cells that the last build subdivided (two-level index)
+    int n_leaves;             // leaves of the last build: one per undivided cell + S^d per subdivided one
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
+
+// Two-level index ("a hierarchical GPU index ... could lower its constant further", in
+// its grid form).  A level-0 cell that holds at least heavy_T records at build time is subdivided
+// into S^d sub-cells, S = floor((count / sub_occ)^(1/d)) >= 2 (sub_occ = 2 records per sub-cell), and its records are sorted by sub-cell
+// (x fastest), so a sub-row segment is again ONE contiguous range.  Level-0 contiguity is untouched:
+// cell_start[c] .. cell_start[c+1] still holds exactly the records of cell c, and every kernel that
+// ignores the second level stays exact.  Leaves (undivided cells and sub-cells) are numbered in
+// storage order; leaf_start is the exclusive scan of their sizes, subinfo[c] = {S or 0, first leaf}.
+// Sub-cell of coordinate x in cell k of an axis: clamp(floorf(fl(fl(t - k) * S)), 0, S-1) with the
+// cell coordinate t = fl(fl(x - lo) * inv_h) of cell_axis(): monotone in x like cell_axis itself.
+__host__ __device__ inline int sub_res(int cnt, int d, int heavy_T, int sub_occ)
+{
+    if (cnt < heavy_T) return 0;
+    const long long q = cnt / sub_occ;
+    int S = d == 2 ? (int)sqrtf((float)q) : (int)cbrtf((float)q);
+    if (S < 2) S = 2;
+    if (d == 2) {
+        while ((long long)(S + 1) * (S + 1) <= q) ++S;
+        while (S > 2 && (long long)S * S > q) --S;
+    } else {
+        while ((long long)(S + 1) * (S + 1) * (S + 1) <= q) ++S;
+        while (S > 2 && (long long)S * S * S > q) --S;
+    }
+    return S;
+}
+__device__ __forceinline__ int sub_axis(float x, float lo, float inv_h, int k, float fS, int S)
+{
+    const float t = __fmul_rn(__fsub_rn(x, lo), inv_h);
+    const float f = floorf(__fmul_rn(__fsub_rn(t, (float)k), fS));
+    return f < 0.0f ? 0 : (f > (float)(S - 1) ? S - 1 : (int)f);
+}
 
 struct View {
     int G0, G1, G2;
@@ -35,6 +68,9 @@ struct View {
     const int32_t *head;
     const int32_t *next;
     const float4 *opos;
+    int heavy_T;              // build-time record count from which a level-0 cell is subdivided
+    const int2 *subinfo;      // per level-0 cell: {S (0 = not subdivided), index of its first leaf}
+    const int32_t *leaf_start;   // exclusive scan of the leaf sizes (n_leaves + 1 entries)
 };
 
 }  // namespace kc
@@ -45,7 +81,11 @@ struct kc_grid {
     int built, dirty;
     size_t bytes;
     int32_t *cell, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
-    int32_t *blocksums;
+    int2 *blocksums;          // per scan block: {records, leaves} (cell scan) / {records, -} (leaf scan)
+    int2 *subinfo;            // two-level index, see View
+    int32_t *leaf_cnt, *leaf_start, *leafid;   // leaf sizes, their scan (doubles as scatter cursors), leaf of point i
+    int64_t n_leaves_max;
+    int heavy_T, sub_occ;
     int32_t *mark;            // per sorted slot: epoch of the last sweep that queried it
     int32_t *list2;           // frontier points of the current sweep that live in chains
     float *delta;             // NEXT #2: displacement of every point in the current step
@@ -77,12 +117,14 @@ inline View make_view(const kc_grid *g)
     }
     v.slk0 = slk[0]; v.slk1 = slk[1]; v.slk2 = slk[2];
     static const int dense_env = getenv("KC_DENSE_THR") ? atoi(getenv("KC_DENSE_THR")) : 0;
-    v.dense_thr = dense_env > 0 ? dense_env : 128;
+    v.dense_thr = dense_env > 0 ? dense_env : 0x7fffffff;
+    if (v.dense_thr > g->heavy_T) v.dense_thr = g->heavy_T;   // a window with a subdivided cell is never taken whole
     static const int wpq_env = getenv("KC_WPQ_MAX") ? atoi(getenv("KC_WPQ_MAX")) : -1;
     v.wpq_max = wpq_env >= 0 ? wpq_env : 32768;
     v.cell_start = g->cell_start;
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;
+    v.heavy_T = g->heavy_T; v.subinfo = g->subinfo; v.leaf_start = g->leaf_start;
     return v;
 }
 

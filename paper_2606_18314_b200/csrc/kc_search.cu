@@ -167,6 +167,131 @@ __device__ __forceinline__ bool bound_ok(float bound, float s2)
     return bound > 0.0f && s2 < __fmul_rn(bound, bound);
 }
 
+// ---- second level: a subdivided cell ------------------------------------------------------------
+// Sub-cell boundary a (0..S) of cell k on an axis, in x-space: lo + (k S + a)(h / S).  The records
+// filed in sub-cells >= a have cell coordinate t >= k + (a/S)(1 - u) (one more rounding than the
+// level-0 filing: fl(fl(t - k) S), where t - k is exact), i.e. x >= lo + (k + a/S) h - 4.02 u G h;
+// the computed boundary is off by <= u(|lo| + 4 G h) (hs = h/S, the product and the sum are rounded,
+// k S + a < 2^27 is converted with relative error u).  Together <= u(|lo| + 8.1 G h), inside the
+// slack slk = 16 u (|lo| + G h) that gap_lb() already subtracts for the level-0 faces, so the same
+// gap_lb() gives a valid lower bound of the real axis distance behind a sub-cell boundary.
+struct SubAx {
+    float lo, q, slk;
+    int base;                                  // k * S
+    int u;                                     // sub-cell of the query's projection into the cell
+};
+__device__ __forceinline__ float sub_face(const SubAx &a, int idx, float hs)
+{
+    return __fadd_rn(a.lo, __fmul_rn((float)(a.base + idx), hs));
+}
+// squared lower bound of the axis distance from the query to every record in sub-cells < idx
+__device__ __forceinline__ float sub_low2(const View &v, const SubAx &a, int idx, float hs)
+{
+    const float t = gap_lb(v, __fsub_rn(a.q, sub_face(a, idx, hs)), a.slk);
+    return __fmul_rn(t, t);
+}
+// ... to every record in sub-cells >= idx
+__device__ __forceinline__ float sub_high2(const View &v, const SubAx &a, int idx, float hs)
+{
+    const float t = gap_lb(v, __fsub_rn(sub_face(a, idx, hs), a.q), a.slk);
+    return __fmul_rn(t, t);
+}
+__device__ __forceinline__ float sub_gap2(const View &v, const SubAx &a, int idx, float hs)
+{
+    return idx == a.u ? 0.0f : (idx < a.u ? sub_low2(v, a, idx + 1, hs) : sub_high2(v, a, idx, hs));
+}
+// Exact visit of a subdivided level-0 cell (cid = linear id, (kx, ky, kz) its coordinates, cend the
+// end of its record range).  The query may lie inside the cell or in a neighbour.  While nothing
+// bounds the search yet (s2 = +inf) the 3^d sub-block around the query's projection is scanned; if
+// that still leaves s2 = +inf the whole cell is.  Then every sub-row that the ball of radius
+// sqrt(s2) around the query can reach is scanned over the x-range it can reach, each test strict
+// and against the current s2 (which only shrinks), skipping what the first step covered.
+template <int D>
+__device__ __noinline__ Top2 visit_heavy(const View &v, int cid, int kx, int ky, int kz, int cend,
+                                         float qx, float qy, float qz, int self, Top2 best)
+{
+    const int2 si = v.subinfo[cid];
+    const int S = si.x;
+    const int32_t *__restrict__ ss = v.leaf_start + si.y;
+    const float fS = (float)S;
+    const float hs = __fdiv_rn(v.h, fS);
+    SubAx ax, ay, az;
+    ax.lo = v.lo0; ax.q = qx; ax.slk = v.slk0; ax.base = kx * S; ax.u = sub_axis(qx, v.lo0, v.inv_h, kx, fS, S);
+    ay.lo = v.lo1; ay.q = qy; ay.slk = v.slk1; ay.base = ky * S; ay.u = sub_axis(qy, v.lo1, v.inv_h, ky, fS, S);
+    az.lo = v.lo2; az.q = qz; az.slk = v.slk2; az.base = kz * S; az.u = D == 3 ? sub_axis(qz, v.lo2, v.inv_h, kz, fS, S) : 0;
+    int px0 = 0, px1 = -1, py0 = 0, py1 = -1, pz0 = 0, pz1 = -1;      // block already scanned (empty)
+    if (best.s2 == CUDART_INF_F) {
+        px0 = max(ax.u - 1, 0); px1 = min(ax.u + 1, S - 1);
+        py0 = max(ay.u - 1, 0); py1 = min(ay.u + 1, S - 1);
+        pz0 = D == 3 ? max(az.u - 1, 0) : 0; pz1 = D == 3 ? min(az.u + 1, S - 1) : 0;
+        for (int z = pz0; z <= pz1; ++z)
+            for (int y = py0; y <= py1; ++y) {
+                const int row = (z * S + y) * S;
+                scan_range<D>(v, ss[row + px0], ss[row + px1 + 1], qx, qy, qz, self, best);
+            }
+        if (best.s2 == CUDART_INF_F) {
+            scan_range<D>(v, ss[0], cend, qx, qy, qz, self, best);
+            return best;
+        }
+    }
+    int z0 = 0, z1 = 0;
+    if (D == 3) {
+        z0 = az.u; z1 = az.u;
+        while (z0 > 0 && !(best.s2 < sub_low2(v, az, z0, hs))) --z0;
+        while (z1 < S - 1 && !(best.s2 < sub_high2(v, az, z1 + 1, hs))) ++z1;
+    }
+    for (int z = z0; z <= z1; ++z) {
+        const float gz2 = D == 3 ? sub_gap2(v, az, z, hs) : 0.0f;
+        if (best.s2 < gz2) continue;
+        int y0 = ay.u, y1 = ay.u;
+        while (y0 > 0 && !(best.s2 < __fadd_rn(gz2, sub_low2(v, ay, y0, hs)))) --y0;
+        while (y1 < S - 1 && !(best.s2 < __fadd_rn(gz2, sub_high2(v, ay, y1 + 1, hs)))) ++y1;
+        for (int y = y0; y <= y1; ++y) {
+            const float rb2 = __fadd_rn(gz2, sub_gap2(v, ay, y, hs));
+            if (best.s2 < rb2) continue;
+            int x0 = ax.u, x1 = ax.u;
+            while (x0 > 0 && !(best.s2 < __fadd_rn(rb2, sub_low2(v, ax, x0, hs)))) --x0;
+            while (x1 < S - 1 && !(best.s2 < __fadd_rn(rb2, sub_high2(v, ax, x1 + 1, hs)))) ++x1;
+            const int row = (z * S + y) * S;
+            if (y >= py0 && y <= py1 && z >= pz0 && z <= pz1) {
+                if (x0 < px0) scan_range<D>(v, ss[row + x0], ss[row + px0], qx, qy, qz, self, best);
+                if (x1 > px1) scan_range<D>(v, ss[row + px1 + 1], ss[row + x1 + 1], qx, qy, qz, self, best);
+            } else {
+                scan_range<D>(v, ss[row + x0], ss[row + x1 + 1], qx, qy, qz, self, best);
+            }
+        }
+    }
+    return best;
+}
+// One level-0 cell: its whole record range [b, e), or its sub-cells when it is subdivided.
+template <int D>
+__device__ __forceinline__ void visit_cell(const View &v, int cid, int kx, int ky, int kz, int b, int e,
+                                           float qx, float qy, float qz, int self, Top2 &best)
+{
+    if (e - b < v.heavy_T) scan_range<D>(v, b, e, qx, qy, qz, self, best);
+    else best = visit_heavy<D>(v, cid, kx, ky, kz, e, qx, qy, qz, self, best);
+}
+// Cells x0..x1 of one grid row (rowbase = linear id of its first cell).
+template <int D>
+__device__ __forceinline__ void visit_row(const View &v, bool chains, int rowbase, int ky, int kz, int x0, int x1,
+                                          float qx, float qy, float qz, int self, Top2 &best)
+{
+    const int32_t *cs = v.cell_start + rowbase;
+    const int b = cs[x0], e = cs[x1 + 1];
+    if (e - b < v.heavy_T) {                        // no subdivided cell among them
+        scan_range<D>(v, b, e, qx, qy, qz, self, best);
+    } else {
+        int lo = b;
+        for (int x = x0; x <= x1; ++x) {
+            const int hi = x == x1 ? e : cs[x + 1];
+            if (hi > lo) visit_cell<D>(v, rowbase + x, x, ky, kz, lo, hi, qx, qy, qz, self, best);
+            lo = hi;
+        }
+    }
+    if (chains)
+        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
+}
+
 // Chebyshev rings r = 2, 3, ... around the query's own cell, entered with the radius-1 block
 // already done; leaves as soon as the bound of the scanned block allows it.  (Rare path: kept out
 // of line, state passed by value.)
@@ -227,14 +352,14 @@ __device__ int block_search(const View &v, bool chains, float qx, float qy, floa
     {
         const int32_t *cs = v.cell_start + rb0 + cx;
         const int s0 = cs[0], s1 = cs[1];
-        scan_range<D>(v, s0, s1, qx, qy, qz, self, best);
+        visit_cell<D>(v, rb0 + cx, cx, cy, cz, s0, s1, qx, qy, qz, self, best);
         if (chains) scan_chain<D>(v, rb0 + cx, qx, qy, qz, self, best);
         if (cx > 0 && !(best.s2 < g.xm)) {
-            scan_range<D>(v, cs[-1], s0, qx, qy, qz, self, best);
+            visit_cell<D>(v, rb0 + cx - 1, cx - 1, cy, cz, cs[-1], s0, qx, qy, qz, self, best);
             if (chains) scan_chain<D>(v, rb0 + cx - 1, qx, qy, qz, self, best);
         }
         if (cx < v.G0 - 1 && !(best.s2 < g.xp)) {
-            scan_range<D>(v, s1, cs[2], qx, qy, qz, self, best);
+            visit_cell<D>(v, rb0 + cx + 1, cx + 1, cy, cz, s1, cs[2], qx, qy, qz, self, best);
             if (chains) scan_chain<D>(v, rb0 + cx + 1, qx, qy, qz, self, best);
         }
     }
@@ -248,9 +373,271 @@ __device__ int block_search(const View &v, bool chains, float qx, float qy, floa
         int x0 = cx, x1 = cx;
         if (cx > 0 && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
         if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
-        scan_row<D>(v, chains, (z * v.G1 + y) * v.G0, x0, x1, qx, qy, qz, self, best);
+        visit_row<D>(v, chains, (z * v.G1 + y) * v.G0, y, z, x0, x1, qx, qy, qz, self, best);
     }
     return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+}
+
+// ---- A3 / A7, phased -------------------------------------------------------------------------
+// One thread per query.  The search of a query is a handful of short record ranges; what costs is
+// not the arithmetic but the control flow around them, which differs from lane to lane.  So every
+// lane first QUEUES the ranges it needs (own row or, in a subdivided cell, the 3^d sub-block; after
+// that, with a finite second-best, every cell / sub-row it cannot rule out) in a small
+// shared-memory list, and the warp then scans all lists in ONE loop, four records per lane and
+// step: the distance arithmetic and the loads, three quarters of the instructions, run with the
+// lanes in step, only the range bookkeeping diverges.  Pruning is decided when a range is queued,
+// against the second-best of the moment: an upper bound of the final one, so every test stays a
+// valid strict lower-bound test (see gap_lb above).
+constexpr int PS_THREADS = 128;
+constexpr int RL_CAP = 16;                       // ranges a lane can queue between two scans
+
+struct Qry { float x, y, z; int self; };
+struct Lane { int2 *rl; int cnt; };              // entry i of this thread's list: rl[i * PS_THREADS]
+
+template <int D>
+__device__ __forceinline__ void rl_push(const View &v, Lane &L, int b, int e, const Qry &q, Top2 &best)
+{
+    if (b >= e) return;
+    if (L.cnt == RL_CAP) {                       // full (rare): this lane scans its list on its own
+        for (int i = 0; i < RL_CAP; ++i) {
+            const int2 r = L.rl[i * PS_THREADS];
+            scan_range<D>(v, r.x, r.y, q.x, q.y, q.z, q.self, best);
+        }
+        L.cnt = 0;
+    }
+    L.rl[L.cnt * PS_THREADS] = make_int2(b, e);
+    ++L.cnt;
+}
+// All 32 lanes of the warp call this; a lane without ranges just waits for the others.  d = 3 records
+// are one float4 each, so a range is entered at its first record; d = 2 records are read two per
+// float4, so a range is entered at the even slot at or below its first record.  Records behind the
+// end of a range (up to 3) are other cells' records or the NaN padding: candidates or inert.
+template <int D>
+__device__ __forceinline__ void rl_scan(const View &v, Lane &L, const Qry &q, Top2 &best)
+{
+    int idx = 0, t = 0, e = 0;
+    for (;;) {
+        if (t >= e && idx < L.cnt) {
+            const int2 r = L.rl[idx * PS_THREADS];
+            ++idx;
+            t = D == 2 ? (r.x & ~1) : r.x;
+            e = r.y;
+        }
+        const bool work = t < e;
+        if (!__any_sync(0xffffffffu, work)) break;
+        if (work) {
+            float s0, s1, s2, s3;
+            if (D == 2) {
+                const float4 A = *reinterpret_cast<const float4 *>(v.spos2 + t);
+                const float4 B = *reinterpret_cast<const float4 *>(v.spos2 + t + 2);
+                s0 = sqd2(q.x, q.y, A.x, A.y); s1 = sqd2(q.x, q.y, A.z, A.w);
+                s2 = sqd2(q.x, q.y, B.x, B.y); s3 = sqd2(q.x, q.y, B.z, B.w);
+            } else {
+                const float4 c0 = v.spos4[t], c1 = v.spos4[t + 1], c2 = v.spos4[t + 2], c3 = v.spos4[t + 3];
+                s0 = sqd3(q.x, q.y, q.z, c0.x, c0.y, c0.z); s1 = sqd3(q.x, q.y, q.z, c1.x, c1.y, c1.z);
+                s2 = sqd3(q.x, q.y, q.z, c2.x, c2.y, c2.z); s3 = sqd3(q.x, q.y, q.z, c3.x, c3.y, c3.z);
+            }
+            const float m = fminf(fminf(s0, s1), fminf(s2, s3));
+            if (m <= best.s2) best = slow_offer4<D>(v, best, t, s0, s1, s2, s3, q.self);
+            t += 4;
+        }
+    }
+    L.cnt = 0;
+}
+
+// Ranges of a subdivided cell (see visit_heavy).  Without a bound (s2 = +inf) only the 3^d
+// sub-block around the query's projection is queued and true is returned: the caller comes back
+// after the scan.  With a bound: every sub-row the ball can reach, minus that block if it has been
+// scanned (block_done).
+template <int D>
+__device__ __noinline__ bool gen_heavy(const View &v, Lane &L, int cid, int kx, int ky, int kz, const Qry &q,
+                                       Top2 &best, bool block_done)
+{
+    const int2 si = v.subinfo[cid];
+    const int S = si.x;
+    const int32_t *__restrict__ ss = v.leaf_start + si.y;
+    const float fS = (float)S;
+    const float hs = __fdiv_rn(v.h, fS);
+    SubAx ax, ay, az;
+    ax.lo = v.lo0; ax.q = q.x; ax.slk = v.slk0; ax.base = kx * S; ax.u = sub_axis(q.x, v.lo0, v.inv_h, kx, fS, S);
+    ay.lo = v.lo1; ay.q = q.y; ay.slk = v.slk1; ay.base = ky * S; ay.u = sub_axis(q.y, v.lo1, v.inv_h, ky, fS, S);
+    az.lo = v.lo2; az.q = q.z; az.slk = v.slk2; az.base = kz * S; az.u = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, kz, fS, S) : 0;
+    const int px0 = max(ax.u - 1, 0), px1 = min(ax.u + 1, S - 1);
+    const int py0 = max(ay.u - 1, 0), py1 = min(ay.u + 1, S - 1);
+    const int pz0 = D == 3 ? max(az.u - 1, 0) : 0, pz1 = D == 3 ? min(az.u + 1, S - 1) : 0;
+    // no bound yet, or one so loose that the ball would cover a large part of the cell: the block
+    // first (it holds the cell's records nearest to the query), the rest after the next scan
+    if (!block_done && !(best.s2 < __fmul_rn(4.0f, __fmul_rn(hs, hs)))) {
+        for (int z = pz0; z <= pz1; ++z)
+            for (int y = py0; y <= py1; ++y) {
+                const int row = (z * S + y) * S;
+                rl_push<D>(v, L, ss[row + px0], ss[row + px1 + 1], q, best);
+            }
+        return true;
+    }
+    int z0 = 0, z1 = 0;
+    if (D == 3) {
+        z0 = az.u; z1 = az.u;
+        while (z0 > 0 && !(best.s2 < sub_low2(v, az, z0, hs))) --z0;
+        while (z1 < S - 1 && !(best.s2 < sub_high2(v, az, z1 + 1, hs))) ++z1;
+    }
+    for (int z = z0; z <= z1; ++z) {
+        const float gz2 = D == 3 ? sub_gap2(v, az, z, hs) : 0.0f;
+        int y0 = ay.u, y1 = ay.u;
+        while (y0 > 0 && !(best.s2 < __fadd_rn(gz2, sub_low2(v, ay, y0, hs)))) --y0;
+        while (y1 < S - 1 && !(best.s2 < __fadd_rn(gz2, sub_high2(v, ay, y1 + 1, hs)))) ++y1;
+        for (int y = y0; y <= y1; ++y) {
+            const float rb2 = __fadd_rn(gz2, sub_gap2(v, ay, y, hs));
+            int x0 = ax.u, x1 = ax.u;
+            while (x0 > 0 && !(best.s2 < __fadd_rn(rb2, sub_low2(v, ax, x0, hs)))) --x0;
+            while (x1 < S - 1 && !(best.s2 < __fadd_rn(rb2, sub_high2(v, ax, x1 + 1, hs)))) ++x1;
+            const int row = (z * S + y) * S;
+            if (block_done && y >= py0 && y <= py1 && z >= pz0 && z <= pz1) {
+                if (x0 < px0) rl_push<D>(v, L, ss[row + x0], ss[row + px0], q, best);
+                if (x1 > px1) rl_push<D>(v, L, ss[row + px1 + 1], ss[row + x1 + 1], q, best);
+            } else {
+                rl_push<D>(v, L, ss[row + x0], ss[row + x1 + 1], q, best);
+            }
+        }
+    }
+    return false;
+}
+
+// Ranges of the cells x0..x1 of one grid row other than the own cell's handled part.  heavy_only:
+// second visit, only subdivided cells whose first visit had no bound yet (their block is done).
+template <int D>
+__device__ __forceinline__ bool gen_row(const View &v, Lane &L, bool chains, bool heavy_only, int rowbase, int ky,
+                                        int kz, int x0, int x1, const Qry &q, Top2 &best)
+{
+    const int32_t *cs = v.cell_start + rowbase;
+    const int b = cs[x0], e = cs[x1 + 1];
+    bool pending = false;
+    if (e - b < v.heavy_T) {                        // no subdivided cell among them
+        if (!heavy_only) rl_push<D>(v, L, b, e, q, best);
+    } else {
+        int lo = b;
+        for (int x = x0; x <= x1; ++x) {
+            const int hi = x == x1 ? e : cs[x + 1];
+            if (hi - lo >= v.heavy_T) {
+                if (heavy_only && best.s2 == CUDART_INF_F) rl_push<D>(v, L, lo, hi, q, best);   // still no bound: all of it
+                else pending |= gen_heavy<D>(v, L, rowbase + x, x, ky, kz, q, best, heavy_only);
+            } else if (!heavy_only) {
+                rl_push<D>(v, L, lo, hi, q, best);
+            }
+            lo = hi;
+        }
+    }
+    if (chains && !heavy_only)
+        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, q.x, q.y, q.z, q.self, best);
+    return pending;
+}
+// Everything of the 3^d block except what phase 1 queued (the own cell, or the whole own row when
+// row_done), pruned cell by cell against the current second-best.
+template <int D>
+__device__ __forceinline__ bool gen_block(const View &v, Lane &L, bool chains, bool heavy_only, unsigned covered,
+                                          const Gaps &g, int cx, int cy, int cz, const Qry &q, Top2 &best)
+{
+    // covered: bit 0 = the row neighbours of the own cell are done, bit k + 1 = row k is done
+    bool pending = false;
+    const int rb0 = (cz * v.G1 + cy) * v.G0;
+    if (!(covered & 1u)) {
+        if (cx > 0 && !(best.s2 < g.xm)) pending |= gen_row<D>(v, L, chains, heavy_only, rb0, cy, cz, cx - 1, cx - 1, q, best);
+        if (cx < v.G0 - 1 && !(best.s2 < g.xp)) pending |= gen_row<D>(v, L, chains, heavy_only, rb0, cy, cz, cx + 1, cx + 1, q, best);
+    }
+#pragma unroll 1
+    for (int k = 0; k < (D == 3 ? 8 : 2); ++k) {
+        if ((covered >> (k + 1)) & 1u) continue;
+        const int oy = row_oy(k), oz = row_oz(k);
+        const int y = cy + oy, z = cz + oz;
+        if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
+        const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
+        if (best.s2 < rb2) continue;
+        int x0 = cx, x1 = cx;
+        if (cx > 0 && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
+        if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
+        pending |= gen_row<D>(v, L, chains, heavy_only, (z * v.G1 + y) * v.G0, y, z, x0, x1, q, best);
+    }
+    return pending;
+}
+
+// MODE 0: A3, every sorted slot of a freshly built grid is a query.
+// MODE 1: A7 for a large frontier: the slots marked with this call's epoch are the queries, on the
+//   incrementally updated grid (tombstones are inert records, the chains of every visited cell are
+//   scanned too); runs only when *nF * sweep_div >= N.
+template <int D, int MODE>
+__global__ void __launch_bounds__(PS_THREADS)
+search_phased_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
+                     const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
+                     float *d2, float *c)
+{
+    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
+    if (MODE == 1 && (int64_t)*nF * sweep_div < N) return;
+    const bool chains = MODE == 1 && ctr->n_misfiled > 0;
+    Lane L;
+    L.rl = s_rl + threadIdx.x;
+    L.cnt = 0;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const int sc = min(s, N - 1);
+    bool query = s < N;
+    if (MODE == 1) query = query && mark[sc] == epoch;
+    if (!__any_sync(0xffffffffu, query)) return;
+    Qry q;
+    q.z = 0.f;
+    if (D == 2) {
+        const float2 t = v.spos2[sc];
+        q.x = t.x; q.y = t.y; q.self = v.sidx[sc];
+    } else {
+        const float4 t = v.spos4[sc];
+        q.x = t.x; q.y = t.y; q.z = t.z; q.self = __float_as_int(t.w);
+    }
+    const int cx = cell_axis(q.x, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(q.y, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(q.z, v.lo2, v.inv_h, v.G2) : 0;
+    const int rb0 = (cz * v.G1 + cy) * v.G0;
+    Top2 best;
+    best.init();
+    bool own_heavy = false, row_done = false, pending = false;
+    int cs0 = 0, cs1 = 0;
+    // phase 1: the own cell (its sub-block when subdivided), with the row neighbours when cheap
+    if (query) {
+        const int32_t *cs = v.cell_start + rb0 + cx;
+        cs0 = cs[0]; cs1 = cs[1];
+        own_heavy = cs1 - cs0 >= v.heavy_T;
+        if (own_heavy) {
+            gen_heavy<D>(v, L, rb0 + cx, cx, cy, cz, q, best, false);
+        } else {
+            const int bl = cx > 0 ? cs[-1] : cs0, er = cx < v.G0 - 1 ? cs[2] : cs1;
+            row_done = er - bl < v.heavy_T;
+            if (row_done) rl_push<D>(v, L, bl, er, q, best);
+            else rl_push<D>(v, L, cs0, cs1, q, best);
+        }
+        if (chains) {
+            scan_chain<D>(v, rb0 + cx, q.x, q.y, q.z, q.self, best);
+            if (row_done && cx > 0) scan_chain<D>(v, rb0 + cx - 1, q.x, q.y, q.z, q.self, best);
+            if (row_done && cx < v.G0 - 1) scan_chain<D>(v, rb0 + cx + 1, q.x, q.y, q.z, q.self, best);
+        }
+    }
+    rl_scan<D>(v, L, q, best);
+    // phase 2: the rest of the 3^d block, pruned against what phase 1 found
+    Gaps g;
+    if (query) {
+        g = make_gaps<D>(v, q.x, q.y, q.z, cx, cy, cz);
+        if (own_heavy) {
+            if (best.s2 == CUDART_INF_F) rl_push<D>(v, L, cs0, cs1, q, best);
+            else gen_heavy<D>(v, L, rb0 + cx, cx, cy, cz, q, best, true);
+        }
+        pending = gen_block<D>(v, L, chains, false, row_done ? 1u : 0u, g, cx, cy, cz, q, best);
+    }
+    rl_scan<D>(v, L, q, best);
+    // phase 3 (rare): subdivided neighbours met while there was no bound yet
+    if (__any_sync(0xffffffffu, pending)) {
+        if (query && pending) gen_block<D>(v, L, chains, true, row_done ? 1u : 0u, g, cx, cy, cz, q, best);
+        rl_scan<D>(v, L, q, best);
+    }
+    if (!query) return;
+    const int r = finish_block<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
+    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    store_cert(best, q.self, nn, nn2, d1, d2, c);
 }
 
 template <int D>
@@ -435,6 +822,29 @@ __device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float
     tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
 }
 
+// Distance (lower bound) from the query to the nearest face of the sub-block u-1..u+1 (clipped to
+// the cell) that lies INSIDE the subdivided cell (k = cell coordinates); +inf if there is none.
+template <int D>
+__device__ __forceinline__ float sub_block_inner_bound(const View &v, float qx, float qy, float qz, int kx, int ky,
+                                                       int kz, int S, float hs, int ux, int uy, int uz)
+{
+    float bound = CUDART_INF_F;
+    SubAx a;
+    a.u = 0;
+    a.lo = v.lo0; a.q = qx; a.slk = v.slk0; a.base = kx * S;
+    if (ux - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qx, sub_face(a, ux - 1, hs)), v.slk0));
+    if (ux + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, ux + 2, hs), qx), v.slk0));
+    a.lo = v.lo1; a.q = qy; a.slk = v.slk1; a.base = ky * S;
+    if (uy - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qy, sub_face(a, uy - 1, hs)), v.slk1));
+    if (uy + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, uy + 2, hs), qy), v.slk1));
+    if (D == 3) {
+        a.lo = v.lo2; a.q = qz; a.slk = v.slk2; a.base = kz * S;
+        if (uz - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qz, sub_face(a, uz - 1, hs)), v.slk2));
+        if (uz + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, uz + 2, hs), qz), v.slk2));
+    }
+    return bound;
+}
+
 // SWEEP = false: A3, every slot of a freshly built grid is a query.
 // SWEEP = true:  A7 for a large frontier: the same slot-ordered sweep over the incrementally
 //   updated grid, but only the slots marked with this call's epoch are queries (their lanes stay
@@ -514,7 +924,50 @@ search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ ma
             if (k < 0) {
                 int s0 = 0, s1 = 0;
                 if (mine) { s0 = crow[cx]; s1 = crow[cx + 1]; }
-                tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
+                const bool hv = mine && s1 - s0 >= v.heavy_T;
+                if (!__any_sync(0xffffffffu, hv)) {
+                    tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
+                } else {
+                    // Second level: a lane in a subdivided cell scans the 3^d sub-block around its own
+                    // sub-cell (clipped to the cell) instead of the whole cell, row by row through the
+                    // tile; the other lanes of the segment scan their own cell in the first pass.
+                    int S = 0, ux = 0, uy = 0, uz = 0;
+                    const int32_t *ss = v.leaf_start;
+                    if (hv) {
+                        const int2 si = v.subinfo[rowid * v.G0 + cx];
+                        S = si.x; ss += si.y;
+                        const float fS = (float)S;
+                        ux = sub_axis(qx, v.lo0, v.inv_h, cx, fS, S);
+                        uy = sub_axis(qy, v.lo1, v.inv_h, cy, fS, S);
+                        uz = D == 3 ? sub_axis(qz, v.lo2, v.inv_h, cz, fS, S) : 0;
+                    }
+#pragma unroll 1
+                    for (int j = -1; j < (D == 3 ? 8 : 2); ++j) {
+                        int b = 0, e = 0;
+                        if (hv) {
+                            const int y = uy + (j < 0 ? 0 : row_oy(j)), z = uz + (j < 0 ? 0 : row_oz(j));
+                            if (y >= 0 && y < S && z >= 0 && z < (D == 3 ? S : 1)) {
+                                const int32_t *srow = ss + (z * S + y) * S;
+                                b = srow[max(ux - 1, 0)]; e = srow[min(ux + 1, S - 1) + 1];
+                            }
+                        } else if (j < 0) {
+                            b = s0; e = s1;
+                        }
+                        const int Bj = __reduce_min_sync(0xffffffffu, b < e ? b : 0x7fffffff);
+                        const int Ej = __reduce_max_sync(0xffffffffu, b < e ? e : 0);
+                        if (Bj < Ej) tile_pass<D>(v, N, lane, tp2, tp4, tix, Bj, Ej, b, e, 0, 0, qx, qy, qz, self, best);
+                    }
+                    // the rest of the own cell, for a lane whose ball leaves the sub-block through a
+                    // face inside the cell (the faces on the cell's boundary are the neighbours' business)
+                    int rb = 0, re = 0;
+                    if (hv) {
+                        const float hs = __fdiv_rn(v.h, (float)S);
+                        if (!bound_ok(sub_block_inner_bound<D>(v, qx, qy, qz, cx, cy, cz, S, hs, ux, uy, uz), best.s2)) {
+                            rb = s0; re = s1;
+                        }
+                    }
+                    dense_pass<D>(v, N, lane, tp2, tp4, tix, rb, re, 0, 0, qx, qy, qz, self, best);
+                }
                 int bl = 0, el = 0, br = 0, er = 0;
                 if (mine && has_l && !(best.s2 < g.xm)) { bl = crow[cx - 1]; el = s0; }
                 if (mine && has_r && !(best.s2 < g.xp)) { br = s1; er = crow[cx + 2]; }
@@ -540,6 +993,330 @@ search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ ma
     if (s >= N) return;
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
     store_cert(best, self, nn, nn2, d1, d2, c);
+}
+
+// ---- A3 / A7, leaf-tiled: the kernel behind kc_cert_grid_search and the slot sweep of A7 ---------
+// A warp owns 32 consecutive sorted slots.  Slots are sorted by leaf, so the windows the lanes need
+// from one row of their 3^d blocks (3 cells of a grid row for a lane in an undivided cell, 3
+// sub-cells of a sub-row of its own cell for a lane in a subdivided cell) lie close together in
+// the sorted arrays.  Phase 1, warp-uniform control flow: every lane computes its window for each of
+// the 3^(d-1) rows (all start indices are fetched in one round trip), and row by row the hull of the
+// lanes' windows goes through the warp's shared-memory tile (coalesced loads) and every lane scans
+// its own window of it.  Phase 2, per lane and only where needed: a lane whose block bound already
+// exceeds its second-best is done; the others queue what phase 1 did not serve -- windows that
+// hold a subdivided cell, everything outside the 3^d sub-block of a lane in a subdivided cell --
+// range by range with every pruning test applied, and the queues are scanned by the warp in step.
+constexpr int LT_WARPS = 4;
+#ifndef LT_MIN_BLOCKS
+#define LT_MIN_BLOCKS 7
+#endif
+constexpr int LT_HULL_MAX = 4096;                 // a longer hull (lanes far apart in memory) is left to phase 2
+static_assert(32 * LT_WARPS == PS_THREADS, "the range queues are strided by PS_THREADS");
+
+// bound of the scanned sub-block [x0,x1]x[y0,y1]x[z0,z1] of a subdivided cell: distance (lower
+// bound) from the query to its nearest face that is interior to the grid.  A face of the block on
+// the cell's boundary is a face of the cell; everything outside the block lies behind one of them.
+template <int D>
+__device__ __forceinline__ float sub_block_bound(const View &v, const Qry &q, int cx, int cy, int cz, int S,
+                                                 float hs, int x0, int x1, int y0, int y1, int z0, int z1)
+{
+    float bound = CUDART_INF_F;
+    SubAx a;
+    a.lo = v.lo0; a.q = q.x; a.slk = v.slk0; a.base = cx * S; a.u = 0;
+    if (x0 > 0 || cx > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.x, sub_face(a, x0, hs)), v.slk0));
+    if (x1 < S - 1 || cx < v.G0 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, x1 + 1, hs), q.x), v.slk0));
+    a.lo = v.lo1; a.base = cy * S;
+    if (y0 > 0 || cy > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.y, sub_face(a, y0, hs)), v.slk1));
+    if (y1 < S - 1 || cy < v.G1 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, y1 + 1, hs), q.y), v.slk1));
+    if (D == 3) {
+        a.lo = v.lo2; a.base = cz * S;
+        if (z0 > 0 || cz > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.z, sub_face(a, z0, hs)), v.slk2));
+        if (z1 < S - 1 || cz < v.G2 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, z1 + 1, hs), q.z), v.slk2));
+    }
+    return bound;
+}
+
+// index (k of phase 1) of the block row at offset (oy, oz): k = 0 own row, k >= 1: row_oy/row_oz(k-1)
+__device__ __forceinline__ int block_row_index(int oy, int oz)
+{
+    // (oz+1)*3 + (oy+1) -> k, 4 bits each: {5,3,6, 1,0,2, 7,4,8}
+    const unsigned long long tab = 0x5ull | (0x3ull << 4) | (0x6ull << 8) | (0x1ull << 12) | (0x0ull << 16) |
+                                   (0x2ull << 20) | (0x7ull << 24) | (0x4ull << 28) | (0x8ull << 32);
+    return (int)((tab >> (4 * ((oz + 1) * 3 + oy + 1))) & 15ull);
+}
+// Sub-rows of the subdivided cell cid = (kx, ky, kz) inside the index box of the ball, minus the
+// sub-block [bx0,bx1]x[by0,by1]x[bz0,bz1] if has_block (served by phase 1).
+template <int D>
+__device__ __forceinline__ void ball_sub(const View &v, Lane &L, int cid, int kx, int ky, int kz, const float (&lo)[3],
+                                         const float (&hi)[3], bool has_block, int bx0, int bx1, int by0, int by1,
+                                         int bz0, int bz1, const Qry &q, Top2 &best)
+{
+    const int2 si = v.subinfo[cid];
+    const int S = si.x;
+    const int32_t *__restrict__ ss = v.leaf_start + si.y;
+    const float fS = (float)S;
+    const int x0 = sub_axis(lo[0], v.lo0, v.inv_h, kx, fS, S), x1 = sub_axis(hi[0], v.lo0, v.inv_h, kx, fS, S);
+    const int y0 = sub_axis(lo[1], v.lo1, v.inv_h, ky, fS, S), y1 = sub_axis(hi[1], v.lo1, v.inv_h, ky, fS, S);
+    const int z0 = D == 3 ? sub_axis(lo[2], v.lo2, v.inv_h, kz, fS, S) : 0;
+    const int z1 = D == 3 ? sub_axis(hi[2], v.lo2, v.inv_h, kz, fS, S) : 0;
+    for (int z = z0; z <= z1; ++z)
+        for (int y = y0; y <= y1; ++y) {
+            const int row = (z * S + y) * S;
+            if (has_block && y >= by0 && y <= by1 && z >= bz0 && z <= bz1) {
+                if (x0 < bx0) rl_push<D>(v, L, ss[row + x0], ss[row + min(x1, bx0 - 1) + 1], q, best);
+                if (x1 > bx1) rl_push<D>(v, L, ss[row + max(x0, bx1 + 1)], ss[row + x1 + 1], q, best);
+            } else {
+                rl_push<D>(v, L, ss[row + x0], ss[row + x1 + 1], q, best);
+            }
+        }
+}
+// Cells xa..xb of grid row (y, z) inside the ball's index box.
+template <int D>
+__device__ __forceinline__ void ball_cells(const View &v, Lane &L, bool chains, int y, int z, int xa, int xb,
+                                           const float (&lo)[3], const float (&hi)[3], const Qry &q, Top2 &best)
+{
+    if (xa > xb) return;
+    const int rowbase = (z * v.G1 + y) * v.G0;
+    const int32_t *cs = v.cell_start + rowbase;
+    const int b = cs[xa], e = cs[xb + 1];
+    if (e - b < v.heavy_T) {
+        rl_push<D>(v, L, b, e, q, best);
+    } else {
+        int lo_s = b;
+        for (int x = xa; x <= xb; ++x) {
+            const int hi_s = x == xb ? e : cs[x + 1];
+            if (hi_s - lo_s >= v.heavy_T) ball_sub<D>(v, L, rowbase + x, x, y, z, lo, hi, false, 0, 0, 0, 0, 0, 0, q, best);
+            else rl_push<D>(v, L, lo_s, hi_s, q, best);
+            lo_s = hi_s;
+        }
+    }
+    if (chains)
+        for (int x = xa; x <= xb; ++x) scan_chain<D>(v, rowbase + x, q.x, q.y, q.z, q.self, best);
+}
+// Queues what the ball needs beyond phase 1.  Returns true when the lane has to fall back to the
+// ring search (no bound yet, or the box holds too many cells to queue).
+template <int D>
+__device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, const Qry &q, Top2 &best, int cx, int cy,
+                                         int cz, bool heavy, unsigned covered, int cs0, int cs1, int S,
+                                         const int32_t *ss, int ux, int uy, int uz)
+{
+    if (best.s2 == CUDART_INF_F) return true;
+    // r >= the real distance of anything whose computed squared distance is <= s2 (fp32 rounding
+    // of s: relative 3u, or absolute 2^-149 per operation in the denormal range)
+    const float r = __fadd_ru(__fmul_ru(__fsqrt_ru(best.s2), 1.0009765625f), 8.470329e-22f);
+    float lo[3], hi[3];
+    lo[0] = __fsub_rd(q.x, r); hi[0] = __fadd_ru(q.x, r);
+    lo[1] = __fsub_rd(q.y, r); hi[1] = __fadd_ru(q.y, r);
+    lo[2] = D == 3 ? __fsub_rd(q.z, r) : 0.f; hi[2] = D == 3 ? __fadd_ru(q.z, r) : 0.f;
+    const int X0 = cell_axis(lo[0], v.lo0, v.inv_h, v.G0), X1 = cell_axis(hi[0], v.lo0, v.inv_h, v.G0);
+    const int Y0 = cell_axis(lo[1], v.lo1, v.inv_h, v.G1), Y1 = cell_axis(hi[1], v.lo1, v.inv_h, v.G1);
+    const int Z0 = D == 3 ? cell_axis(lo[2], v.lo2, v.inv_h, v.G2) : 0, Z1 = D == 3 ? cell_axis(hi[2], v.lo2, v.inv_h, v.G2) : 0;
+    if ((int64_t)(X1 - X0 + 1) * (Y1 - Y0 + 1) * (Z1 - Z0 + 1) > 64) return true;
+    // the common case: the box lies inside what phase 1 served
+    const bool in_block = X0 >= cx - 1 && X1 <= cx + 1 && Y0 >= cy - 1 && Y1 <= cy + 1 && Z0 >= cz - 1 && Z1 <= cz + 1;
+    if (!heavy && in_block && covered == (D == 3 ? 0x7ffffffu : 0x1ffu)) return false;
+    if (heavy && X0 == cx && X1 == cx && Y0 == cy && Y1 == cy && Z0 == cz && Z1 == cz) {
+        const float fS = (float)S;
+        if (sub_axis(lo[0], v.lo0, v.inv_h, cx, fS, S) >= ux - 1 && sub_axis(hi[0], v.lo0, v.inv_h, cx, fS, S) <= ux + 1 &&
+            sub_axis(lo[1], v.lo1, v.inv_h, cy, fS, S) >= uy - 1 && sub_axis(hi[1], v.lo1, v.inv_h, cy, fS, S) <= uy + 1 &&
+            (D == 2 || (sub_axis(lo[2], v.lo2, v.inv_h, cz, fS, S) >= uz - 1 &&
+                        sub_axis(hi[2], v.lo2, v.inv_h, cz, fS, S) <= uz + 1))) {
+            if (chains) scan_chain<D>(v, (cz * v.G1 + cy) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
+            return false;
+        }
+    }
+    for (int z = Z0; z <= Z1; ++z)
+        for (int y = Y0; y <= Y1; ++y) {
+            const int oy = y - cy, oz = z - cz;
+            const bool near = oy >= -1 && oy <= 1 && oz >= -1 && oz <= 1;
+            if (heavy) {
+                if (oy == 0 && oz == 0) {
+                    // own row: the own cell through its sub-cells (minus the sub-block), the others whole
+                    ball_cells<D>(v, L, chains, y, z, X0, cx - 1, lo, hi, q, best);
+                    if (chains) scan_chain<D>(v, (z * v.G1 + y) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
+                    ball_sub<D>(v, L, (z * v.G1 + y) * v.G0 + cx, cx, cy, cz, lo, hi, true, max(ux - 1, 0),
+                                min(ux + 1, S - 1), max(uy - 1, 0), min(uy + 1, S - 1), D == 3 ? max(uz - 1, 0) : 0,
+                                D == 3 ? min(uz + 1, S - 1) : 0, q, best);
+                    ball_cells<D>(v, L, chains, y, z, cx + 1, X1, lo, hi, q, best);
+                } else {
+                    ball_cells<D>(v, L, chains, y, z, X0, X1, lo, hi, q, best);
+                }
+            } else if (near && ((covered >> (3 * block_row_index(oy, oz))) & 7u)) {
+                // phase 1 served some of the cells cx-1..cx+1 of this row (and their chains)
+                const unsigned cv = (covered >> (3 * block_row_index(oy, oz))) & 7u;
+                ball_cells<D>(v, L, chains, y, z, X0, cx - 2, lo, hi, q, best);
+                for (int x = max(X0, cx - 1); x <= min(X1, cx + 1); ++x)
+                    if (!((cv >> (x - cx + 1)) & 1u)) ball_cells<D>(v, L, chains, y, z, x, x, lo, hi, q, best);
+                ball_cells<D>(v, L, chains, y, z, cx + 2, X1, lo, hi, q, best);
+            } else {
+                ball_cells<D>(v, L, chains, y, z, X0, X1, lo, hi, q, best);
+            }
+        }
+    return false;
+}
+
+template <int D, int MODE>
+__global__ void __launch_bounds__(32 * LT_WARPS, LT_MIN_BLOCKS)
+search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
+                   const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
+                   float *d2, float *c)
+{
+    constexpr int NR = D == 3 ? 9 : 3;             // rows of a 3^d block
+    __shared__ __align__(16) float4 s_p4[D == 3 ? LT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
+    __shared__ __align__(16) float2 s_p2[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int s_ix[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
+    if (MODE == 1 && (int64_t)*nF * sweep_div < N) return;
+    const bool chains = MODE == 1 && ctr->n_misfiled > 0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float qnan = __int_as_float(0x7fc00000);
+    float4 *tp4 = s_p4[D == 3 ? warp : 0];
+    float2 *tp2 = s_p2[D == 2 ? warp : 0];
+    int *tix = s_ix[D == 2 ? warp : 0];
+    for (int k = lane; k < WT_TILE + 4; k += 32) {          // the tile starts inert
+        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
+    }
+    Lane L;
+    L.rl = s_rl + threadIdx.x;
+    L.cnt = 0;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s - lane >= N) return;                     // whole warp past the end
+    const int sc = min(s, N - 1);
+    bool query = s < N;
+    if (MODE == 1) query = query && mark[sc] == epoch;
+    if (!__any_sync(0xffffffffu, query)) return;
+    Qry q;
+    q.z = 0.f;
+    if (D == 2) {
+        const float2 t = v.spos2[sc];
+        q.x = t.x; q.y = t.y; q.self = v.sidx[sc];
+    } else {
+        const float4 t = v.spos4[sc];
+        q.x = t.x; q.y = t.y; q.z = t.z; q.self = __float_as_int(t.w);
+    }
+    const int cx = cell_axis(q.x, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(q.y, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(q.z, v.lo2, v.inv_h, v.G2) : 0;
+    const int cellid = (cz * v.G1 + cy) * v.G0 + cx;
+    const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
+    int cs0 = 0, cs1 = 0;
+    if (query) { cs0 = v.cell_start[cellid]; cs1 = v.cell_start[cellid + 1]; }
+    const bool heavy = query && cs1 - cs0 >= v.heavy_T;
+    int S = 0, ux = 0, uy = 0, uz = 0;
+    const int32_t *ss = v.leaf_start;
+    if (heavy) {
+        const int2 si = v.subinfo[cellid];
+        S = si.x; ss += si.y;
+        const float fS = (float)S;
+        ux = sub_axis(q.x, v.lo0, v.inv_h, cx, fS, S);
+        uy = sub_axis(q.y, v.lo1, v.inv_h, cy, fS, S);
+        uz = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, cz, fS, S) : 0;
+    }
+    Top2 best;
+    best.init();
+    // phase 1a: this lane's window in every row of its block (k = 0: its own row); covered = rows
+    // that need nothing more (light lanes: served by the tile or outside the grid)
+    unsigned covered = 0;
+    if (query) {
+#pragma unroll
+        for (int k = 0; k < NR; ++k) {
+            const int oy = k == 0 ? 0 : row_oy(k - 1), oz = k == 0 ? 0 : row_oz(k - 1);
+            int b = 0, e = 0;
+            if (heavy) {
+                const int y = uy + oy, z = uz + oz;
+                if (y >= 0 && y < S && z >= 0 && z < (D == 3 ? S : 1)) {
+                    const int32_t *srow = ss + (z * S + y) * S;
+                    b = srow[max(ux - 1, 0)]; e = srow[min(ux + 1, S - 1) + 1];
+                }
+            } else {
+                const int y = cy + oy, z = cz + oz;
+                if (y >= 0 && y < v.G1 && z >= 0 && z < v.G2) {
+                    const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
+                    b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1];
+                    if (e - b < v.dense_thr) {
+                        covered |= 7u << (3 * k);
+                    } else if (k == 0) {
+                        // a long window (dense cells, or a subdivided one): the ball of phase 2 prunes
+                        // it; here only the own cell, which gives that ball its radius
+                        b = crow[cx]; e = crow[cx + 1];
+                        covered |= 2u << (3 * k);            // (the own cell of a light lane is undivided)
+                    } else {
+                        b = 0; e = 0;
+                    }
+                } else {
+                    covered |= 7u << (3 * k);
+                }
+            }
+            L.rl[(RL_CAP - 1 - k) * PS_THREADS] = make_int2(b, e);    // top of the queue's storage: the
+        }                                                              // queue itself holds < RL_CAP - NR here
+    }
+    // phase 1b: row by row through the tile
+    float gym = 0.f, gyp = 0.f, gzm = 0.f, gzp = 0.f;
+#pragma unroll 1
+    for (int k = 0; k < NR; ++k) {
+        int2 w = make_int2(0, 0);
+        if (query) w = L.rl[(RL_CAP - 1 - k) * PS_THREADS];
+        if (k == 1 && query && !heavy) {
+            // squared lower bounds of the distance to the neighbouring rows (see gap_lb), from the
+            // second-best the own row has given: a row that lies provably farther is skipped
+            float t;
+            t = gap_lb(v, __fsub_rn(q.y, face_at(v.lo1, cy, v.h)), v.slk1); gym = __fmul_rn(t, t);
+            t = gap_lb(v, __fsub_rn(face_at(v.lo1, cy + 1, v.h), q.y), v.slk1); gyp = __fmul_rn(t, t);
+            if (D == 3) {
+                t = gap_lb(v, __fsub_rn(q.z, face_at(v.lo2, cz, v.h)), v.slk2); gzm = __fmul_rn(t, t);
+                t = gap_lb(v, __fsub_rn(face_at(v.lo2, cz + 1, v.h), q.z), v.slk2); gzp = __fmul_rn(t, t);
+            }
+        }
+        if (k >= 1 && !heavy && w.x < w.y) {
+            const int oy = row_oy(k - 1), oz = row_oz(k - 1);
+            const float rb2 = __fadd_rn(oy < 0 ? gym : (oy > 0 ? gyp : 0.f), oz < 0 ? gzm : (oz > 0 ? gzp : 0.f));
+            if (best.s2 < rb2) w.y = w.x;                       // (its cells stay marked as served)
+        }
+        const bool has = w.x < w.y;
+        if (chains && query && !heavy && ((covered >> (3 * k)) & 7u)) {
+            // the overflow chains of the served cells (a cell without sorted records may still hold
+            // re-filed points)
+            const int oy = k == 0 ? 0 : row_oy(k - 1), oz = k == 0 ? 0 : row_oz(k - 1);
+            const int y = cy + oy, z = cz + oz;
+            if (y >= 0 && y < v.G1 && z >= 0 && z < v.G2)
+                for (int x = has_l ? cx - 1 : cx; x <= (has_r ? cx + 1 : cx); ++x)
+                    if ((covered >> (3 * k + x - cx + 1)) & 1u)
+                        scan_chain<D>(v, (z * v.G1 + y) * v.G0 + x, q.x, q.y, q.z, q.self, best);
+        }
+        // the lanes in undivided cells and those in subdivided cells look at different places: one
+        // hull each (a hull that is still long -- lanes in two grid rows -- goes to the queues)
+#pragma unroll 1
+        for (int grp = 0; grp < 2; ++grp) {
+            const bool in = has && heavy == (grp == 1);
+            const int B = __reduce_min_sync(0xffffffffu, in ? w.x : 0x7fffffff);
+            const int E = __reduce_max_sync(0xffffffffu, in ? w.y : 0);
+            if (B >= E) continue;
+            if (E - B > LT_HULL_MAX) {                          // (rare; the queue's storage holds the windows)
+                if (in) scan_range<D>(v, w.x, w.y, q.x, q.y, q.z, q.self, best);
+                continue;
+            }
+            tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, in ? w.x : 0, in ? w.y : 0, 0, 0, q.x, q.y, q.z, q.self, best);
+        }
+    }
+    // phase 2: the ball.  Every record that can still enter the list lies within r = d2 (as of now)
+    // of the query, so on every axis its coordinate lies in [q - r, q + r], and because the filing
+    // functions cell_axis / sub_axis are monotone, its cell (sub-cell) index lies between the
+    // indices of those two end points: the candidates are the cells of an index box.  Whatever of
+    // that box phase 1 has not served is queued (usually nothing) and scanned by the warp in step.
+    // No face arithmetic and no slack are involved: the end points are rounded outwards.
+    bool fallback = false;
+    if (query) {
+        fallback = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+    }
+    if (__any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
+    if (!query) return;
+    if (fallback) {
+        // no bound yet, or a ball of many cells (an isolated point): the classic ring search
+        const int r = block_search<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
+        if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    }
+    store_cert(best, q.self, nn, nn2, d1, d2, c);
 }
 
 // A7, large frontier: stamp the slots of the frontier points with this call's epoch; frontier
@@ -911,9 +1688,17 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)g->N;
-    static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 1;
+    static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 4;
     const int tb = 32 * WT_WARPS;
-    if (variant == 1) {
+    if (variant == 4) {
+        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+        if (g->geom.d == 2) search_leaf_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+        else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+    } else if (variant == 3) {
+        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+        if (g->geom.d == 2) search_phased_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+        else search_phased_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
+    } else if (variant == 1) {
         if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
         else search_tiled_kernel<3, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
     } else if (variant == 2) {
@@ -1008,7 +1793,20 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     if (sweep_div > 0) {
         ++g->epoch;
         mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
-        if (g->geom.d == 2)
+        static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 4;
+        if (variant == 4) {
+            const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+            if (g->geom.d == 2)
+                search_leaf_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+            else
+                search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+        } else if (variant == 3) {
+            const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+            if (g->geom.d == 2)
+                search_phased_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+            else
+                search_phased_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+        } else if (g->geom.d == 2)
             search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
         else
             search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
