@@ -4,10 +4,14 @@
     python bench.py --gpus 1 --steps K --warmup W            # this repo's CUDA path
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands
 
-A "step" is one maintenance transition p -> p' through every row of the hot path (max
-displacement, Lemma-1 classify, incremental repair, frontier entropy, O(N) grid rebuild, all-pairs
-certification) on BASELINE.json configs[1] (N=16,000, d=2, five motion families, eps=1e-3).
-Prints ONE JSON line (rank 0).  Details of every field: DESIGN.md §measurement.
+Default workload: BASELINE.json config 5 ("Scale"), N = 4,194,304 points in d = 3 (``--workload
+cfg5_d2`` for d = 2): 50 % uniform background + 50 % from 256 Gaussian clusters, random-walk steps
+with eps = 2e-4.  A "step" is one maintenance transition p -> p' through every row of the hot path:
+max displacement (A0), Lemma-1 classify (A4), incremental repair (A6+A7), frontier entropy (A5),
+O(N) grid rebuild (A2+A3) at all 4,194,304 points, and the all-pairs oracle pass (A1) at the
+first 1,048,576 points of p' (1.1e12 pair evaluations).  ``--workload cfg2 / cfg3`` runs the small
+launch-bound configurations (N = 16,000, five motion families) as CUDA graphs.
+Prints ONE JSON line (rank 0).  Details of every field: DESIGN.md §6.
 """
 from __future__ import annotations
 
@@ -28,9 +32,16 @@ METRIC = "certified_points_per_s"
 UNIT = "points/s"
 L2_FLUSH_BYTES = int(os.environ.get("KC_FLUSH_MB", "256")) << 20
 FP32_LANES = 148 * 128          # B200: 148 SMs x 128 FP32 lanes, one non-fused op / lane / clk
-# dram__bytes_read.sum + dram__bytes_write.sum of one allpairs_kernel launch, from the committed ncu
-# --set full capture of this command (profiles/r1e_allpairs_cfg2_full.txt); null for other workloads
-AP_TRAFFIC_BYTES = {("cfg2", 16000): 279552}   # profiles/r1f_allpairs_cfg2_full.txt: dram read + write per launch
+N_ALLPAIRS = 1 << 20            # config 5: the all-pairs oracle pass runs on the first 2^20 points
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the named kernel, from the committed
+# ncu --set full captures (profiles/, file named beside each figure); None where no capture exists
+NCU_TRAFFIC_BYTES = {
+    ("cfg2", "allpairs_kernel"): 279552,            # profiles/r1f_allpairs_cfg2_full.txt
+}
+# algorithmic bytes per point of the O(N) rebuild (A2 + A3) with this layout
+REBUILD_BYTES_PER_POINT = {2: 76.0, 3: 90.0}
+BUILD_BYTES_PER_POINT = {2: 46.0, 3: 56.0}          # A2 alone
+SEARCH_BYTES_PER_POINT = {2: 36.0, 3: 40.0}         # A3 alone (compulsory traffic)
 
 
 def log(*a):
@@ -108,6 +119,52 @@ def run_oracle_arm(cfg, K, W, time_budget_s=None, pair_budget=1.5e11):
     # points certified per step by the O(N^2) definition, as in the GPU arm's all-pairs row
     value = (N * frac) * done / t_total
     return dict(value=value, steps=done, seconds=t_total, cores=oracle.num_procs(), sample=sample,
+                ms_per_step=1e3 * t_total / max(done, 1))
+
+
+def oracle_scale_step(oracle, p, q, pre_c, geom, n_ap, n_bf):
+    """Config 5, the oracle's restatement of one step at full size: O3, O4, O5+O6, the exact k-d
+    tree relabel of all N points (all cores), and for the all-pairs row the k-d tree on the first
+    n_ap points plus the brute-force definition for n_bf sampled queries (1.1e12 pairs on the CPU
+    are not run)."""
+    eps = oracle.max_displacement(p, q)
+    flags, F = oracle.frontier(pre_c, eps)
+    cid = oracle.cell_ids(q, geom)
+    H, m, C = oracle.entropy(cid, F, geom.n_cells)
+    post = oracle.kdtree_top2(q)
+    qa = np.ascontiguousarray(q[:n_ap])
+    ap = oracle.kdtree_top2(qa)
+    qs = np.sort(np.random.default_rng(11).choice(n_ap, n_bf, replace=False)).astype(np.int32)
+    bf = oracle.bruteforce_top2(qa, queries=qs)
+    return dict(eps=eps, flags=flags, F=F, cid=cid, H=H, m=m, C=C, post=post, ap=ap, bf=bf, qs=qs)
+
+
+def run_oracle_scale(cfg, K, W, time_budget_s=150.0):
+    """--impl reference on config 5: K steps of oracle_scale_step (W capped at one untimed step),
+    stopped early when the time budget is spent (the number of steps done is reported)."""
+    import oracle
+    oracle.build()
+    c = wl.CONFIGS[cfg]
+    N = c["N"]
+    p, mot = wl.make_scene(cfg)
+    geom = oracle.geom_for(p)
+    pre = oracle.kdtree_top2(p)
+    done, t_total = 0, 0.0
+    for t in range(min(W, 1) + K):
+        q, _ = mot.step(p)
+        t0 = time.perf_counter()
+        r = oracle_scale_step(oracle, p, q, pre.c, geom, N_ALLPAIRS, 64)
+        dt = time.perf_counter() - t0
+        p, pre = q, r["post"]
+        if t >= min(W, 1):
+            t_total += dt
+            done += 1
+            if t_total > time_budget_s:
+                break
+    sample = (f"{done} full steps of {cfg}: per step max displacement, Lemma-1 frontier, cell ids + entropy, exact "
+              f"k-d tree relabel of all {N} points, k-d tree on the first {N_ALLPAIRS} points and the brute-force "
+              f"definition for 64 of them")
+    return dict(value=N * done / t_total, steps=done, seconds=t_total, cores=oracle.num_procs(), sample=sample,
                 ms_per_step=1e3 * t_total / max(done, 1))
 
 
@@ -356,7 +413,7 @@ def run_gpu_arm(args):
         peak = FP32_LANES * sm_max * 1e6 / 1e12
         probe = kc.kc_fp32_probe() / 1e12
         roofline = dict(bound="alu", kernel="allpairs_kernel", achieved=achieved, peak=peak, unit="TFLOP/s",
-                        frac=achieved / peak, traffic=AP_TRAFFIC_BYTES.get((cfg, N)),
+                        frac=achieved / peak, traffic=NCU_TRAFFIC_BYTES.get((cfg, "allpairs_kernel")),
                         note=(f"{ops_per_pair} separately rounded FP32 ops per ordered pair (no FMA by contract); peak = "
                               f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md); measured non-fused "
                               f"FADD/FMUL chain rate {probe:.2f} Top/s; kernel share of step = "
@@ -370,7 +427,7 @@ def run_gpu_arm(args):
                             ms_per_step=cpu["ms_per_step"])
         extras = {}
         if not args.no_extras:
-            extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks)
+            extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=cfg)
         families = {f: dict(steps=s["steps"], frontier_frac=s["frontier"] / max(1, s["steps"]) / N,
                             H=s["H"] / max(1, s["steps"]),
                             repair_path_ms=s["repair_ms"] / max(1, s.get("ph_steps", 0)),
@@ -414,6 +471,234 @@ def run_gpu_arm(args):
         dist.destroy_process_group()
     return out
 
+
+def run_gpu_arm_scale(args):
+    """Config 5 (the headline): N = 4,194,304 points, random-walk steps, every row of the hot path
+    per step; the all-pairs row on the first 2^20 points of p'.  Grids of this size are not
+    launch-bound: the calls are issued eagerly through the public API."""
+    import torch
+    import torch.distributed as dist
+
+    from paper_2606_18314_b200 import binding as kc
+    from paper_2606_18314_b200.driver import Maintainer, crossover_fraction
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    kc.lib()
+    dev = torch.device("cuda", local)
+    cfg, K, W = args.workload, args.steps, args.warmup
+    c = wl.CONFIGS[cfg]
+    N, d = c["N"], c["d"]
+    n_ap = min(N_ALLPAIRS, N)
+    # replicas only (DESIGN.md §7): every rank runs its own seeded copy of the workload
+    p0, mot = wl.make_scene(cfg, seed=c["seed"] + 7919 * rank)
+    host = [p0]
+    for _ in range(W + K):
+        host.append(mot.step(host[-1])[0])
+    flush = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dev_traj = [torch.from_numpy(p).to(dev) for p in host]         # resident before the timed region
+    m = Maintainer(dev_traj[0], allpairs=False)
+    ap = kc.Certs.empty(n_ap, dev)
+    ws = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
+
+    def step(mm, p_next, timed):
+        res = mm.step(p_next, time_phases=timed, do_allpairs=False)
+        ev = None
+        if timed:
+            ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            ev[0].record()
+        kc.kc_cert_allpairs(p_next[:n_ap], ap, ws)                  # A1: the oracle pass, 2^20 points of p'
+        if timed:
+            ev[1].record()
+        return res, ev
+
+    for t in range(W):
+        step(m, dev_traj[t + 1], False)
+    barrier()
+    sampler = ClockSampler(local, period_s=0.02)
+    launches0 = kc.kc_launch_count()
+    t_wall0 = time.perf_counter()
+    step_events, infos = [], []
+    for t in range(K):
+        flush.zero_()                                                # L2 flush between timed steps
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        res, ev = step(m, dev_traj[W + t + 1], True)
+        e1.record()
+        step_events.append((e0, e1))
+        infos.append((res.phase_ms, ev, res.nF.clone(), res.H.clone()))
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    launches = kc.kc_launch_count() - launches0
+    clocks = sampler.stop()
+    dev_ms = sum(a.elapsed_time(b) for a, b in step_events)
+    phase_sum = {ph: 0.0 for ph in ("maxdisp", "classify", "repair", "entropy", "rebuild", "allpairs")}
+    nF_sum, H_sum = 0, 0.0
+    for ph_ev, ev, nF, H in infos:
+        pt = Maintainer.phase_times(ph_ev)
+        for ph in ("maxdisp", "classify", "repair", "entropy", "rebuild"):
+            phase_sum[ph] += pt[ph]
+        phase_sum["allpairs"] += ev[0].elapsed_time(ev[1])
+        nF_sum += int(nF.item()); H_sum += float(H.item())
+    dev_ms_max, units = aggregate_over_ranks(dev_ms, N * K, dev)
+    value = units / (dev_ms_max * 1e-3)
+    info = m.grid.info()
+    del m
+
+    # ---- end to end through the public API: pinned host inputs, H2D + step + D2H per step ----
+    pinned = [torch.from_numpy(p).pin_memory() for p in host[: K + 1]]
+    m2 = Maintainer(dev_traj[0], allpairs=False)
+    n_pad = m2.certs.buf.shape[1]
+    host_certs = torch.empty((5, n_pad), dtype=torch.int32).pin_memory()     # nn, d1, d2, c, nn2 of all N points
+    host_scal = torch.empty(24, dtype=torch.uint8).pin_memory()
+    bufs = [torch.empty(N, d, device=dev), torch.empty(N, d, device=dev)]
+    h2d, d2h = N * d * 4, 5 * N * 4 + 24
+    e2e_events = []
+    barrier()
+    for t in range(K):
+        flush.zero_()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record()
+        buf = bufs[t & 1]
+        buf.copy_(pinned[t + 1], non_blocking=True)
+        res, _ = step(m2, buf, False)
+        host_certs.copy_(res.rebuilt.buf, non_blocking=True)
+        host_scal.copy_(m2.scalars, non_blocking=True)
+        e1.record()
+        e1.synchronize()                                             # the user reads the result here
+        e2e_events.append((e0, e1))
+    barrier()
+    e2e_ms = sum(a.elapsed_time(b) for a, b in e2e_events)
+    e2e_ms_max, units = aggregate_over_ranks(e2e_ms, N * K, dev)
+    e2e_value = units / (e2e_ms_max * 1e-3)
+    del m2, pinned, bufs
+
+    out = None
+    if rank == 0:
+        import oracle
+        oracle.build()
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except OSError:
+            pass
+        hbm = float(peaks.get("hbm_gbs", 6650.0))
+        hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback (B200_PROFILING.md)"
+        # ---- certified: the first transition recomputed by the CPU oracle (k-d tree at this size,
+        # itself validated bitwise against brute force; brute-force definition on sampled queries);
+        # the oracle's wall time for that step is the cpu_baseline (the oracle as it stands)
+        g_or = oracle.geom_for(host[0])
+        pre = oracle.kdtree_top2(host[0])
+        t0 = time.perf_counter()
+        w = oracle_scale_step(oracle, host[0], host[1], pre.c, g_or, n_ap, 64)
+        t_cpu = time.perf_counter() - t0
+        m3 = Maintainer(dev_traj[0], allpairs=False)
+        u32 = lambda a: np.ascontiguousarray(a).view(np.uint32)
+        ok = all(np.array_equal(u32(getattr(m3.certs, f).cpu().numpy()), u32(getattr(pre, f)))
+                 for f in ("nn", "nn2", "d1", "d2", "c"))
+        res, _ = step(m3, dev_traj[1], False)
+        torch.cuda.synchronize()
+        ok &= u32(res.eps.cpu().numpy())[0] == u32(np.array([w["eps"]], np.float32))[0]
+        ok &= int(res.nF.item()) == w["F"].size
+        F = w["F"]
+        for f in ("nn", "nn2", "d1", "d2", "c"):
+            want = u32(getattr(w["post"], f))
+            ok &= bool(np.array_equal(u32(getattr(res.rebuilt, f).cpu().numpy()), want))
+            ok &= bool(np.array_equal(u32(getattr(res.repaired, f).cpu().numpy())[F], want[F]))
+            gap = u32(getattr(ap, f).cpu().numpy())
+            ok &= bool(np.array_equal(gap, u32(getattr(w["ap"], f))))
+            ok &= bool(np.array_equal(gap[w["qs"]], u32(getattr(w["bf"], f))))
+        rest = np.flatnonzero(w["flags"] == 0)
+        ok &= bool(np.array_equal(res.repaired.nn.cpu().numpy()[rest], w["post"].nn[rest]))      # Lemma 1
+        ok &= abs(float(res.H.item()) - w["H"]) <= 1e-6 and int(res.m_cells.item()) == w["m"] and \
+            int(res.C_occ.item()) == w["C"]
+        if not ok:
+            raise RuntimeError(f"parity failure against the CPU oracle: {cfg} step 0")
+        certified = (f"1 transition at N={N}: rebuild (all points), repair (at F), all-pairs ({n_ap} points), eps, |F|, "
+                     f"Lemma-1 nn bit-exact vs the CPU k-d tree oracle (+ 64 brute-force queries), H within 1e-6")
+        del m3
+        cpu_baseline = dict(value=N / t_cpu, unit=UNIT, cores=oracle.num_procs(), kind="oracle (exact k-d tree, all cores)",
+                            sample=(f"1 full step at N={N}: max displacement, Lemma-1 frontier, cell ids + entropy, k-d tree "
+                                    f"relabel of all points, k-d tree on the first {n_ap} points + 64 brute-force queries"),
+                            ms_per_step=1e3 * t_cpu)
+        # ---- rooflines
+        ms = {ph: v / K for ph, v in phase_sum.items()}
+        sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
+        ops_per_pair = 5 if d == 2 else 8
+        alu_peak = FP32_LANES * sm_max * 1e6 / 1e12
+        probe = kc.kc_fp32_probe() / 1e12
+        ap_achieved = n_ap * (n_ap - 1) * ops_per_pair / (ms["allpairs"] * 1e-3) / 1e12
+        step_ms = dev_ms_max / K
+        roofline = dict(bound="alu", kernel="allpairs_kernel", achieved=ap_achieved, peak=alu_peak, unit="TFLOP/s",
+                        frac=ap_achieved / alu_peak, traffic=NCU_TRAFFIC_BYTES.get((cfg, "allpairs_kernel")),
+                        note=(f"dominant kernel of the step by time (share {ms['allpairs'] / step_ms:.3f}): {ops_per_pair} separately "
+                              f"rounded FP32 ops per ordered pair (no FMA by contract) x {n_ap}*({n_ap}-1) pairs per launch; peak = "
+                              f"148 SM x 128 lanes x {sm_max:.0f} MHz (derived, DESIGN.md §5); measured non-fused FADD/FMUL "
+                              f"chain rate {probe:.2f} Top/s"),
+                        pairs_per_s=n_ap * (n_ap - 1) / (ms["allpairs"] * 1e-3), ms_per_launch=ms["allpairs"],
+                        fp32_probe_tops=probe)
+        reb_bytes = REBUILD_BYTES_PER_POINT[d] * N
+        reb_gbs = reb_bytes / (ms["rebuild"] * 1e-3) / 1e9
+        roofline_rebuild = dict(bound="hbm", kernel="kc_cert_grid_rebuild (A2 + A3: build kernels + search_leaf_kernel)",
+                                achieved=reb_gbs, peak=hbm, unit="GB/s", frac=reb_gbs / hbm,
+                                traffic=NCU_TRAFFIC_BYTES.get((cfg, "rebuild")),
+                                note=(f"{REBUILD_BYTES_PER_POINT[d]:.0f} algorithmic B/point (SURVEY.md §8(d)) x {N} points / "
+                                      f"{ms['rebuild']:.4f} ms (CUDA events around the call inside the timed steps); peak {hbm_src}; "
+                                      f"the search is issue/latency-bound, not HBM-bound (DESIGN.md §5)"),
+                                ms_per_call=ms["rebuild"])
+        frontier_frac = nF_sum / K / N
+        paths = {"allpairs": n_ap / (ms["allpairs"] * 1e-3), "grid_rebuild": N / (ms["rebuild"] * 1e-3),
+                 "frontier_repair": N / ((ms["repair"] + ms["classify"] + ms["maxdisp"]) * 1e-3)}
+        extras = {}
+        if not args.no_extras:
+            extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=cfg)
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": (f"{cfg} (BASELINE.json config 5, Scale): N={N}, d={d}, 50% uniform + 50% from 256 Gaussian "
+                                    f"clusters (sigma=0.005), random-walk steps eps={c['eps']}, grid occupancy 2; every step = A0, A4, "
+                                    f"A6+A7 (Lemma-1 frontier, {frontier_frac:.3f} of the points), A5, A2+A3 at all {N} points, and the "
+                                    f"all-pairs oracle pass A1 on the first {n_ap} points of p' ({n_ap * (n_ap - 1):.3e} pairs)"),
+                       "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
+                       "launch": "eager stream launches through the C-ABI (a grid of this size is not launch-bound)",
+                       "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
+                       "certified": certified},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_ms_max / K},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "roofline_rebuild": roofline_rebuild,
+            "cpu_baseline": cpu_baseline,
+            "phases_ms_per_step": ms,
+            "paths_points_per_s": paths,
+            "repair_over_rebuild": (ms["repair"] + ms["classify"] + ms["maxdisp"]) / ms["rebuild"],
+            "lemma1_frontier_frac": frontier_frac, "H_mean": H_sum / K,
+            "grid": {"max_cell_occupancy": int(info.max_occ), "occupied_cells": int(info.c_occ),
+                     "subdivided_cells": int(info.n_heavy), "leaves": int(info.n_leaves)},
+            "wall_s_timed_region": t_wall,
+            "extras": extras,
+        }
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return out
 
 def verify_against_oracle(kc, Maintainer, torch, dev, cfg, traj, fams, steps_per_family=2, graph_cls=None):
     """'Certified' = the outputs of the timed configuration equal the CPU oracle's bit for bit
@@ -483,12 +768,76 @@ def _median_ms(torch, fn, reps, setup=None, flush=None):
     return float(np.median(ts))
 
 
-def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
-    """Other configs, reported beside the headline (not part of `value`):
-    config 4 repair-vs-rebuild sweep (crossover per entropy class) and config 5 at scale."""
+def family_table(kc, Maintainer, torch, dev, cfg, flush, steps=8):
+    """Configs 2 / 3 (N = 16,000, five motion families each): per family the Lemma-1 frontier
+    fraction, H(F), and the repair-path and rebuild-path time of a step (eager calls, medians).
+    Config 3's diffuse5 / ball5 pair is the equal-size, different-entropy control of the paper's
+    Fig. 2: the same number of movers, scattered or from one ball; the mover
+    list is the controlled frontier there (reading R12)."""
+    c = wl.CONFIGS[cfg]
+    N = c["N"]
+    rows = {}
+    for fam in c["families"]:
+        p, mot = wl.make_scene(cfg, fam)
+        m = Maintainer(torch.from_numpy(p).to(dev), allpairs=False)
+        rep_ms, reb_ms, fr, Hs, mvH, mv_ms = [], [], [], [], [], []
+        for t in range(steps + 2):
+            q, movers = mot.step(p)
+            Q = torch.from_numpy(q).to(dev)
+            mv = None if movers is None else torch.from_numpy(movers).to(dev)
+            if t >= 2:
+                flush.zero_()
+            r = m.step(Q, movers=mv, time_phases=True, do_allpairs=False)
+            torch.cuda.synchronize()
+            if t >= 2:
+                pt = Maintainer.phase_times(r.phase_ms)
+                rep_ms.append(pt["maxdisp"] + pt["classify"] + pt["repair"]); reb_ms.append(pt["rebuild"])
+                fr.append(int(r.nF.item()) / N); Hs.append(float(r.H.item()))
+            p = q
+        row = dict(lemma1_frontier_frac=float(np.mean(fr)), H=float(np.mean(Hs)), repair_path_ms=float(np.median(rep_ms)),
+                   rebuild_path_ms=float(np.median(reb_ms)),
+                   repair_over_rebuild=float(np.median(rep_ms) / np.median(reb_ms)))
+        if fam in ("diffuse5", "ball5", "local"):
+            # the mover list as the frontier: A0 + A6 + A7 at the movers only, and H of that list
+            p, mot = wl.make_scene(cfg, fam)
+            m = Maintainer(torch.from_numpy(p).to(dev), allpairs=False)
+            H = torch.zeros(1, dtype=torch.float64, device=dev)
+            for t in range(steps + 2):
+                q, movers = mot.step(p)
+                Q = torch.from_numpy(q).to(dev)
+                mv = torch.from_numpy(movers).to(dev)
+                nmv = torch.tensor([movers.size], dtype=torch.int32, device=dev)
+                if t >= 2:
+                    flush.zero_()
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                kc.kc_max_displacement(m.p, Q, m.eps)
+                kc.kc_frontier_repair(m.grid, Q, mv, nmv, m.certs, movers=mv, n_movers=nmv)
+                e1.record()
+                kc.kc_frontier_entropy(m.grid, mv, nmv, out=(H, m.m, m.C))
+                kc.kc_cert_grid_rebuild(m.grid, Q, m.certs)
+                m.p = Q
+                torch.cuda.synchronize()
+                if t >= 2:
+                    mv_ms.append(e0.elapsed_time(e1)); mvH.append(float(H.item()))
+                p = q
+            row.update(movers=int(movers.size), mover_frontier_H=float(np.mean(mvH)), mover_repair_ms=float(np.median(mv_ms)),
+                       mover_repair_over_rebuild=float(np.median(mv_ms) / np.median(reb_ms)))
+        rows[fam] = row
+        del m
+    return rows
+
+
+def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=None):
+    """Other configs, reported beside the headline (not part of `value`): configs 2 / 3 per
+    family, config 4 repair-vs-rebuild sweep (crossover per entropy class), the other dimension of
+    config 5."""
     hbm = float(peaks.get("hbm_gbs", 6650.0))
     flush = torch.empty(L2_FLUSH_BYTES // 4, dtype=torch.float32, device=dev)
     ex = {"hbm_peak_gbs": hbm, "hbm_peak_source": "measured" if "hbm_gbs" in peaks else "fallback"}
+    if skip_cfg not in ("cfg2", "cfg3"):
+        ex["cfg2_families"] = family_table(kc, Maintainer, torch, dev, "cfg2", flush)
+        ex["cfg3_families"] = family_table(kc, Maintainer, torch, dev, "cfg3", flush)
     # ---------------- config 4: N=262,144, d=3, mover fraction sweep, scattered vs one ball
     c4 = wl.CONFIGS["cfg4"]
     N = c4["N"]
@@ -625,6 +974,8 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
     ex["table2_sizes"] = t2
     # ---------------- config 5: 4,194,304 points, rebuild + Lemma-1 repair; all-pairs at 2^20
     for cfg in ("cfg5_d2", "cfg5_d3"):
+        if cfg == skip_cfg:
+            continue
         c5 = wl.CONFIGS[cfg]
         N, d = c5["N"], c5["d"]
         p, mot = wl.make_scene(cfg)
@@ -657,19 +1008,15 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
 
         t_loc = _median_ms(torch, repair_local, 3, setup=lambda: kc.kc_grid_build(m.grid, P), flush=flush)
         local_frac = int(m.nF.item()) / N
-        # algorithmic bytes per point of the rebuild: positions read twice,
-        # cell+rank written and read, histogram + scan, sorted records, idx, slot, certificates
-        pos = 4 * d
-        rec = 8 if d == 2 else 16
-        cells_per_pt = m.grid.geom.n_cells / N
-        bpp = (pos + 8) + cells_per_pt * (4 + 4 + 4 + 4) + (pos + 8 + 4 + rec + 4 + 4) + (rec + (4 if d == 2 else 0) + 8 + 20)
+        bpp = REBUILD_BYTES_PER_POINT[d]
         n_ap = 1 << 20
         PA = P[:n_ap].contiguous()
         ap = kc.Certs.empty(n_ap, dev)
         ws = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
         t_ap = _median_ms(torch, lambda: kc.kc_cert_allpairs(PA, ap, ws), 2, flush=flush)
         ops = 5 if d == 2 else 8
-        ex[cfg] = dict(N=N, grid_build_ms=t_build, rebuild_ms=t_reb, rebuild_points_per_s=N / (t_reb * 1e-3),
+        ex[cfg] = dict(N=N, grid_build_ms=t_build, grid_build_frac_of_hbm=N * BUILD_BYTES_PER_POINT[d] / (t_build * 1e-3) / 1e9 / hbm,
+                       rebuild_ms=t_reb, rebuild_points_per_s=N / (t_reb * 1e-3),
                        rebuild_alg_bytes_per_point=bpp, rebuild_gbs=N * bpp / (t_reb * 1e-3) / 1e9,
                        rebuild_frac_of_hbm=N * bpp / (t_reb * 1e-3) / 1e9 / hbm,
                        max_cell_occupancy=int(info.max_occ), occupied_cells=int(info.c_occ),
@@ -686,10 +1033,10 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg5_d3", choices=["cfg5_d3", "cfg5_d2", "cfg2", "cfg3"])
     ap.add_argument("--no-extras", action="store_true", help="skip the config 4 / config 5 side measurements")
     ap.add_argument("--no-graph", action="store_true", help="issue the step eagerly instead of replaying CUDA graphs")
     args = ap.parse_args()
@@ -699,7 +1046,9 @@ def main():
     if args.impl == "reference":
         if rank != 0:
             return
-        r = run_oracle_arm(args.workload, args.steps, args.warmup)
+        scale = args.workload.startswith("cfg5")
+        r = run_oracle_scale(args.workload, args.steps, args.warmup) if scale else \
+            run_oracle_arm(args.workload, args.steps, args.warmup)
         c = wl.CONFIGS[args.workload]
         line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT,
                 "n_gpus": args.gpus, "steps": r["steps"], "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
@@ -711,7 +1060,7 @@ def main():
                 "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
         print(json.dumps(line), flush=True)
         return
-    out = run_gpu_arm(args)
+    out = run_gpu_arm_scale(args) if args.workload.startswith("cfg5") else run_gpu_arm(args)
     if out is not None:
         print(json.dumps(out), flush=True)
 
