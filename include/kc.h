@@ -169,8 +169,16 @@ kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom *geom);
 kc_status kc_grid_destroy(kc_grid *g);
 /* Bytes of device memory the grid holds (host). */
 size_t kc_grid_bytes(const kc_grid *g);
+/* host.  Parameters of the two-level index ("a hierarchical GPU index ... could lower its constant
+ * further"): a cell that holds at least heavy_T records at build time is subdivided
+ * into S^d sub-cells, S = floor((count / sub_occ)^(1/d)) >= 2, and its records are sorted by
+ * sub-cell, so the searches prune inside it.  Defaults: sub_occ = 4, heavy_T = 128 (d = 2) / 256
+ * (d = 3); heavy_T is raised to sub_occ * 2^(d+1) if smaller.  Results never depend on these
+ * values.  Takes effect with the next kc_grid_build (the grid counts as not built until then). */
+kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ);
 
-/* A2: cell id per point, per-cell histogram, exclusive scan, scatter into cell-sorted arrays.
+/* A2: cell id per point, per-cell histogram, exclusive scan, scatter into cell-sorted arrays (a
+ * counting sort in two levels: the records of a subdivided cell are sorted by sub-cell).
  * After it the grid is resident at positions p (copied; p may be freed afterwards). */
 kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream);
 /* A3: certificates of all N points of a freshly built grid by the ring-expanding search
@@ -248,8 +256,12 @@ kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF, i
  * frontier only.
  *  movers: device int32 list of DISTINCT ids whose position differs from what the grid holds
  *          (*n_movers on the device, at most n_movers_max), or NULL = every point may have
- *          moved.  Movers keep their slot if their cell is unchanged; otherwise they are
- *          tombstoned and re-filed into their new cell's overflow chain (line 3).
+ *          moved.  Movers keep their slot if their cell (and, in a subdivided cell, their
+ *          sub-cell) is unchanged; otherwise they are tombstoned and re-filed into their new
+ *          cell's overflow chain (line 3).  On a grid of >= 100,000 points an update whose
+ *          host-side bound allows at least N/8 movers (n_movers_max, or N for NULL) re-bins the
+ *          whole grid at p_new instead (A2, O(N)): cheaper than re-filing that many points one by
+ *          one, and the search that follows runs on a fresh grid.
  *  F, nF, nF_max: as for kc_frontier_entropy; the queries to recompute (lines 4-7).
  *  nn, nn2, d1, d2, c: certificates, updated IN PLACE at the ids in F, untouched elsewhere.
  * The search is the same unbounded ring search as A3, over sorted ranges and chains. */
@@ -267,6 +279,15 @@ kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, const int32_
 kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const int32_t *F, const int32_t *nF,
                              int64_t nF_max, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
                              void *stream);
+
+/* CUDA graphs.  Every call only enqueues kernels and memsets on `stream` (kc_grid_create,
+ * kc_grid_info and kc_fp32_probe excepted), takes every device-side count from device memory and
+ * keeps no per-call counter on the host, so a sequence of calls can be captured once and replayed
+ * with other DATA in the same buffers.  What is decided on the HOST at call (= capture) time, and
+ * therefore frozen in a captured graph: the kernel variant chosen from N, nF_max and n_movers_max
+ * (host-side bounds), whether kc_grid_update re-bins, and the grid's built / updated state, which
+ * must be the same at every replay as at capture (capture a whole step, including the build or the
+ * update that precedes a search, as paper_2606_18314_b200/driver.py does). */
 
 /* ---- NEXT #4: K-list certificates ---------------------------------------------------------- */
 /* "Richer geometric certificates (Delaunay edges, k-nearest-neighbour graphs, ...) are left open"

@@ -23,7 +23,7 @@ EXPORTS = (
     "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_max_displacement",
     "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded", "kc_cert_allpairs_seeded",
     "kc_frontier_oracle_workspace",
-    "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_build",
+    "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_set_index", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
     "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
     "kc_cert_allpairs_topk_workspace", "kc_cert_allpairs_topk", "kc_cert_grid_topk", "kc_frontier_search_topk",
@@ -88,6 +88,7 @@ def lib():
     L.kc_grid_destroy.argtypes = [vp]
     L.kc_grid_bytes.restype = sz
     L.kc_grid_bytes.argtypes = [vp]
+    L.kc_grid_set_index.argtypes = [vp, ci, ci]
     L.kc_grid_build.argtypes = [vp, vp, i64, vp]
     L.kc_cert_grid_search.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     L.kc_cert_grid_rebuild.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
@@ -303,6 +304,11 @@ class Grid:
     @property
     def bytes(self) -> int:
         return int(lib().kc_grid_bytes(self._h))
+
+    def set_index(self, heavy_T: int, sub_occ: int = 4):
+        """Parameters of the two-level index (kc_grid_set_index); effective from the next build."""
+        _check(lib().kc_grid_set_index(self._h, int(heavy_T), int(sub_occ)), "kc_grid_set_index")
+        self.N = 0
 
     def info(self) -> kc_grid_info_t:
         out = kc_grid_info_t()

@@ -27,6 +27,7 @@ namespace {
 constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
 constexpr int SCAN_CHUNK = 2048;   // entries per scan block (256 threads x 8)
 constexpr int SCAN_SMALL_MAX = 16384;   // up to this many entries a scan is one CTA (1024 threads x 16)
+constexpr int64_t REBIN_MIN_N = 100000, REBIN_DIV = 8;   // A6: when an update re-bins instead of re-filing
 
 // ------------------------------------------------------------------ A2 build
 // A counting sort in two levels.  (1) prep: drop the chains of the previous residency, zero the
@@ -718,11 +719,10 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
         delete g;
         return KC_EINVAL;
     }
-    static const int thr_env = getenv("KC_HEAVY_T") ? atoi(getenv("KC_HEAVY_T")) : 0;
-    static const int occ_env = getenv("KC_SUB_OCC") ? atoi(getenv("KC_SUB_OCC")) : 0;
-    g->sub_occ = occ_env > 0 ? occ_env : 4;
-    const int thr_min = g->sub_occ << (geom->d + 1);   // keeps the leaf count within n_leaves_max
-    g->heavy_T = thr_env > 0 ? (thr_env < thr_min ? thr_min : thr_env) : (geom->d == 2 ? 128 : 256);
+    // two-level index defaults (measured on config 5): cells of >= 128 (d=2) / 256
+    // (d=3) records are subdivided at ~4 records per sub-cell; kc_grid_set_index changes them
+    g->sub_occ = 4;
+    g->heavy_T = geom->d == 2 ? 128 : 256;
     g->n_scan_blocks = (int)((g->n_leaves_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
     bool ok = true;
     auto alloc = [&](void **p, size_t bytes) {
@@ -760,7 +760,7 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     bool e = cudaMemset(g->head, 0xff, nc * 4) != cudaSuccess ||
              cudaMemset(g->fcount, 0, nc * 4) != cudaSuccess ||
              cudaMemset(g->mhist, 0, MHIST * 4) != cudaSuccess ||
-             (g->epoch = 0, cudaMemset(g->mark, 0, (n + 8) * 4)) != cudaSuccess ||
+             cudaMemset(g->mark, 0, (n + 8) * 4) != cudaSuccess ||
              cudaMemset(g->ctr, 0, sizeof(Counters)) != cudaSuccess ||
              cudaDeviceSynchronize() != cudaSuccess;
     if (e) {
@@ -784,6 +784,19 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 }
 
 extern "C" size_t kc_grid_bytes(const kc_grid *g) { return g ? g->bytes : 0; }
+
+extern "C" kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ)
+{
+    if (!g || sub_occ < 1 || sub_occ > 64 || heavy_T < 1) {
+        set_error("kc_grid_set_index: bad argument (1 <= sub_occ <= 64, heavy_T >= 1)");
+        return KC_EINVAL;
+    }
+    const int thr_min = sub_occ << (g->geom.d + 1);      // keeps the leaf count within n_leaves_max
+    g->sub_occ = sub_occ;
+    g->heavy_T = heavy_T < thr_min ? thr_min : heavy_T;
+    g->built = 0;                                         // takes effect with the next build
+    return KC_OK;
+}
 
 extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream)
 {
@@ -900,10 +913,14 @@ extern "C" kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, c
         set_error("kc_grid_update: grid not built for this N");
         return KC_EREBUILD;
     }
+    // Most points may have moved on a large grid: re-bin (A2, O(N), ~0.3 ms at 4 M points) instead of
+    // re-filing them one by one -- cheaper than the refresh pass itself, no tombstones, no chains,
+    // and the frontier search that follows runs on a fresh grid.  (Decided from the host-side bounds.)
+    const int64_t nm = movers ? n_movers_max : N;
+    if (N >= REBIN_MIN_N && nm * REBIN_DIV >= N) return kc_grid_build(g, p_new, N, stream);
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)N;
-    const int64_t nm = movers ? n_movers_max : N;
     const int chain_blocks = blocks_for(g->dirty ? N : 1, 256, 148 * 4);
     if (g->dirty) clear_chains_kernel<<<chain_blocks, 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr);
     count_launches((g->dirty ? 1 : 0) + (nm > 0 ? 1 : 0) + 1);

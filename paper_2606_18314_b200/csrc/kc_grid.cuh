@@ -59,8 +59,6 @@ struct View {
     int G0, G1, G2;
     float lo0, lo1, lo2, h, inv_h, shrink;
     float slk0, slk1, slk2;   // absolute rounding slack of a computed face / cell boundary per axis
-    int dense_thr;            // a row range of at least this many records is handled as dense (A3)
-    int wpq_max;              // id lists up to this long are served one warp per query (A7)
     const int32_t *cell_start;
     const float2 *spos2;
     const float4 *spos4;
@@ -86,11 +84,10 @@ struct kc_grid {
     int32_t *leaf_cnt, *leaf_start, *leafid;   // leaf sizes, their scan (doubles as scatter cursors), leaf of point i
     int64_t n_leaves_max;
     int heavy_T, sub_occ;
-    int32_t *mark;            // per sorted slot: epoch of the last sweep that queried it
+    int32_t *mark;            // per sorted slot: 1 while a sweep has it as a query (zero between calls)
     int32_t *list2;           // frontier points of the current sweep that live in chains
     float *delta;             // NEXT #2: displacement of every point in the current step
     unsigned *cellmax;        // NEXT #2: largest displacement (float bits) per cell
-    int epoch;
     float2 *spos2;
     float4 *spos4, *opos;
     kc::Counters *ctr;
@@ -116,11 +113,6 @@ inline View make_view(const kc_grid *g)
         slk[a] = nextafterf((float)t, INFINITY);
     }
     v.slk0 = slk[0]; v.slk1 = slk[1]; v.slk2 = slk[2];
-    static const int dense_env = getenv("KC_DENSE_THR") ? atoi(getenv("KC_DENSE_THR")) : 0;
-    v.dense_thr = dense_env > 0 ? dense_env : 0x7fffffff;
-    if (v.dense_thr > g->heavy_T) v.dense_thr = g->heavy_T;   // a window with a subdivided cell is never taken whole
-    static const int wpq_env = getenv("KC_WPQ_MAX") ? atoi(getenv("KC_WPQ_MAX")) : -1;
-    v.wpq_max = wpq_env >= 0 ? wpq_env : 32768;
     v.cell_start = g->cell_start;
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;

@@ -445,226 +445,6 @@ __device__ __forceinline__ void rl_scan(const View &v, Lane &L, const Qry &q, To
     L.cnt = 0;
 }
 
-// Ranges of a subdivided cell (see visit_heavy).  Without a bound (s2 = +inf) only the 3^d
-// sub-block around the query's projection is queued and true is returned: the caller comes back
-// after the scan.  With a bound: every sub-row the ball can reach, minus that block if it has been
-// scanned (block_done).
-template <int D>
-__device__ __noinline__ bool gen_heavy(const View &v, Lane &L, int cid, int kx, int ky, int kz, const Qry &q,
-                                       Top2 &best, bool block_done)
-{
-    const int2 si = v.subinfo[cid];
-    const int S = si.x;
-    const int32_t *__restrict__ ss = v.leaf_start + si.y;
-    const float fS = (float)S;
-    const float hs = __fdiv_rn(v.h, fS);
-    SubAx ax, ay, az;
-    ax.lo = v.lo0; ax.q = q.x; ax.slk = v.slk0; ax.base = kx * S; ax.u = sub_axis(q.x, v.lo0, v.inv_h, kx, fS, S);
-    ay.lo = v.lo1; ay.q = q.y; ay.slk = v.slk1; ay.base = ky * S; ay.u = sub_axis(q.y, v.lo1, v.inv_h, ky, fS, S);
-    az.lo = v.lo2; az.q = q.z; az.slk = v.slk2; az.base = kz * S; az.u = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, kz, fS, S) : 0;
-    const int px0 = max(ax.u - 1, 0), px1 = min(ax.u + 1, S - 1);
-    const int py0 = max(ay.u - 1, 0), py1 = min(ay.u + 1, S - 1);
-    const int pz0 = D == 3 ? max(az.u - 1, 0) : 0, pz1 = D == 3 ? min(az.u + 1, S - 1) : 0;
-    // no bound yet, or one so loose that the ball would cover a large part of the cell: the block
-    // first (it holds the cell's records nearest to the query), the rest after the next scan
-    if (!block_done && !(best.s2 < __fmul_rn(4.0f, __fmul_rn(hs, hs)))) {
-        for (int z = pz0; z <= pz1; ++z)
-            for (int y = py0; y <= py1; ++y) {
-                const int row = (z * S + y) * S;
-                rl_push<D>(v, L, ss[row + px0], ss[row + px1 + 1], q, best);
-            }
-        return true;
-    }
-    int z0 = 0, z1 = 0;
-    if (D == 3) {
-        z0 = az.u; z1 = az.u;
-        while (z0 > 0 && !(best.s2 < sub_low2(v, az, z0, hs))) --z0;
-        while (z1 < S - 1 && !(best.s2 < sub_high2(v, az, z1 + 1, hs))) ++z1;
-    }
-    for (int z = z0; z <= z1; ++z) {
-        const float gz2 = D == 3 ? sub_gap2(v, az, z, hs) : 0.0f;
-        int y0 = ay.u, y1 = ay.u;
-        while (y0 > 0 && !(best.s2 < __fadd_rn(gz2, sub_low2(v, ay, y0, hs)))) --y0;
-        while (y1 < S - 1 && !(best.s2 < __fadd_rn(gz2, sub_high2(v, ay, y1 + 1, hs)))) ++y1;
-        for (int y = y0; y <= y1; ++y) {
-            const float rb2 = __fadd_rn(gz2, sub_gap2(v, ay, y, hs));
-            int x0 = ax.u, x1 = ax.u;
-            while (x0 > 0 && !(best.s2 < __fadd_rn(rb2, sub_low2(v, ax, x0, hs)))) --x0;
-            while (x1 < S - 1 && !(best.s2 < __fadd_rn(rb2, sub_high2(v, ax, x1 + 1, hs)))) ++x1;
-            const int row = (z * S + y) * S;
-            if (block_done && y >= py0 && y <= py1 && z >= pz0 && z <= pz1) {
-                if (x0 < px0) rl_push<D>(v, L, ss[row + x0], ss[row + px0], q, best);
-                if (x1 > px1) rl_push<D>(v, L, ss[row + px1 + 1], ss[row + x1 + 1], q, best);
-            } else {
-                rl_push<D>(v, L, ss[row + x0], ss[row + x1 + 1], q, best);
-            }
-        }
-    }
-    return false;
-}
-
-// Ranges of the cells x0..x1 of one grid row other than the own cell's handled part.  heavy_only:
-// second visit, only subdivided cells whose first visit had no bound yet (their block is done).
-template <int D>
-__device__ __forceinline__ bool gen_row(const View &v, Lane &L, bool chains, bool heavy_only, int rowbase, int ky,
-                                        int kz, int x0, int x1, const Qry &q, Top2 &best)
-{
-    const int32_t *cs = v.cell_start + rowbase;
-    const int b = cs[x0], e = cs[x1 + 1];
-    bool pending = false;
-    if (e - b < v.heavy_T) {                        // no subdivided cell among them
-        if (!heavy_only) rl_push<D>(v, L, b, e, q, best);
-    } else {
-        int lo = b;
-        for (int x = x0; x <= x1; ++x) {
-            const int hi = x == x1 ? e : cs[x + 1];
-            if (hi - lo >= v.heavy_T) {
-                if (heavy_only && best.s2 == CUDART_INF_F) rl_push<D>(v, L, lo, hi, q, best);   // still no bound: all of it
-                else pending |= gen_heavy<D>(v, L, rowbase + x, x, ky, kz, q, best, heavy_only);
-            } else if (!heavy_only) {
-                rl_push<D>(v, L, lo, hi, q, best);
-            }
-            lo = hi;
-        }
-    }
-    if (chains && !heavy_only)
-        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, q.x, q.y, q.z, q.self, best);
-    return pending;
-}
-// Everything of the 3^d block except what phase 1 queued (the own cell, or the whole own row when
-// row_done), pruned cell by cell against the current second-best.
-template <int D>
-__device__ __forceinline__ bool gen_block(const View &v, Lane &L, bool chains, bool heavy_only, unsigned covered,
-                                          const Gaps &g, int cx, int cy, int cz, const Qry &q, Top2 &best)
-{
-    // covered: bit 0 = the row neighbours of the own cell are done, bit k + 1 = row k is done
-    bool pending = false;
-    const int rb0 = (cz * v.G1 + cy) * v.G0;
-    if (!(covered & 1u)) {
-        if (cx > 0 && !(best.s2 < g.xm)) pending |= gen_row<D>(v, L, chains, heavy_only, rb0, cy, cz, cx - 1, cx - 1, q, best);
-        if (cx < v.G0 - 1 && !(best.s2 < g.xp)) pending |= gen_row<D>(v, L, chains, heavy_only, rb0, cy, cz, cx + 1, cx + 1, q, best);
-    }
-#pragma unroll 1
-    for (int k = 0; k < (D == 3 ? 8 : 2); ++k) {
-        if ((covered >> (k + 1)) & 1u) continue;
-        const int oy = row_oy(k), oz = row_oz(k);
-        const int y = cy + oy, z = cz + oz;
-        if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
-        const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
-        if (best.s2 < rb2) continue;
-        int x0 = cx, x1 = cx;
-        if (cx > 0 && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
-        if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
-        pending |= gen_row<D>(v, L, chains, heavy_only, (z * v.G1 + y) * v.G0, y, z, x0, x1, q, best);
-    }
-    return pending;
-}
-
-// MODE 0: A3, every sorted slot of a freshly built grid is a query.
-// MODE 1: A7 for a large frontier: the slots marked with this call's epoch are the queries, on the
-//   incrementally updated grid (tombstones are inert records, the chains of every visited cell are
-//   scanned too); runs only when *nF * sweep_div >= N.
-template <int D, int MODE>
-__global__ void __launch_bounds__(PS_THREADS)
-search_phased_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
-                     const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
-                     float *d2, float *c)
-{
-    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
-    if (MODE == 1 && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = MODE == 1 && ctr->n_misfiled > 0;
-    Lane L;
-    L.rl = s_rl + threadIdx.x;
-    L.cnt = 0;
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    const int sc = min(s, N - 1);
-    bool query = s < N;
-    if (MODE == 1) query = query && mark[sc] == epoch;
-    if (!__any_sync(0xffffffffu, query)) return;
-    Qry q;
-    q.z = 0.f;
-    if (D == 2) {
-        const float2 t = v.spos2[sc];
-        q.x = t.x; q.y = t.y; q.self = v.sidx[sc];
-    } else {
-        const float4 t = v.spos4[sc];
-        q.x = t.x; q.y = t.y; q.z = t.z; q.self = __float_as_int(t.w);
-    }
-    const int cx = cell_axis(q.x, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(q.y, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(q.z, v.lo2, v.inv_h, v.G2) : 0;
-    const int rb0 = (cz * v.G1 + cy) * v.G0;
-    Top2 best;
-    best.init();
-    bool own_heavy = false, row_done = false, pending = false;
-    int cs0 = 0, cs1 = 0;
-    // phase 1: the own cell (its sub-block when subdivided), with the row neighbours when cheap
-    if (query) {
-        const int32_t *cs = v.cell_start + rb0 + cx;
-        cs0 = cs[0]; cs1 = cs[1];
-        own_heavy = cs1 - cs0 >= v.heavy_T;
-        if (own_heavy) {
-            gen_heavy<D>(v, L, rb0 + cx, cx, cy, cz, q, best, false);
-        } else {
-            const int bl = cx > 0 ? cs[-1] : cs0, er = cx < v.G0 - 1 ? cs[2] : cs1;
-            row_done = er - bl < v.heavy_T;
-            if (row_done) rl_push<D>(v, L, bl, er, q, best);
-            else rl_push<D>(v, L, cs0, cs1, q, best);
-        }
-        if (chains) {
-            scan_chain<D>(v, rb0 + cx, q.x, q.y, q.z, q.self, best);
-            if (row_done && cx > 0) scan_chain<D>(v, rb0 + cx - 1, q.x, q.y, q.z, q.self, best);
-            if (row_done && cx < v.G0 - 1) scan_chain<D>(v, rb0 + cx + 1, q.x, q.y, q.z, q.self, best);
-        }
-    }
-    rl_scan<D>(v, L, q, best);
-    // phase 2: the rest of the 3^d block, pruned against what phase 1 found
-    Gaps g;
-    if (query) {
-        g = make_gaps<D>(v, q.x, q.y, q.z, cx, cy, cz);
-        if (own_heavy) {
-            if (best.s2 == CUDART_INF_F) rl_push<D>(v, L, cs0, cs1, q, best);
-            else gen_heavy<D>(v, L, rb0 + cx, cx, cy, cz, q, best, true);
-        }
-        pending = gen_block<D>(v, L, chains, false, row_done ? 1u : 0u, g, cx, cy, cz, q, best);
-    }
-    rl_scan<D>(v, L, q, best);
-    // phase 3 (rare): subdivided neighbours met while there was no bound yet
-    if (__any_sync(0xffffffffu, pending)) {
-        if (query && pending) gen_block<D>(v, L, chains, true, row_done ? 1u : 0u, g, cx, cy, cz, q, best);
-        rl_scan<D>(v, L, q, best);
-    }
-    if (!query) return;
-    const int r = finish_block<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
-    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, q.self, nn, nn2, d1, d2, c);
-}
-
-template <int D>
-__global__ void __launch_bounds__(128)
-search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
-{
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= N) return;
-    float qx, qy, qz = 0.f;
-    int self;
-    if (D == 2) {
-        float2 q = v.spos2[s];
-        qx = q.x; qy = q.y; self = v.sidx[s];
-    } else {
-        float4 q = v.spos4[s];
-        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
-    }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    Top2 best;
-    best.init();
-    int r = block_search<D>(v, false, qx, qy, qz, self, cx, cy, cz, best);
-    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, self, nn, nn2, d1, d2, c);
-}
-
 // ---- A3, warp-tiled: the whole-set search of a freshly built grid --------------------------
 // A warp owns 32 consecutive sorted slots.  Slots are cell-sorted, so the lanes of one grid row
 // form a contiguous lane segment, and what they need from any row of the 3^d block is ONE
@@ -681,7 +461,6 @@ search_all_kernel(View v, int N, Counters *ctr, int32_t *nn, int32_t *nn2, float
 //    two best are extracted with warp reductions.
 // Lanes whose radius-1 block does not satisfy the bound continue with the ring loop (rare).
 constexpr int WT_TILE = 128;   // records per warp tile
-constexpr int WT_WARPS = 4;
 
 template <int D>
 __device__ __forceinline__ void tile_scan(const float2 *tp2, const float4 *tp4, const int *tidx, int lb,
@@ -777,224 +556,6 @@ __device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
         tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
     }
 }
-// Dense pass: every lane brings up to two ranges left after pruning.  Served lane by lane by the
-// whole warp when that is cheaper than a tile pass over the hull [B, E) (issue-slot estimates:
-// tile pass ~11 per record of the longest lane, cooperative ~45 per served lane + 12 per 32
-// records).  Called by all 32 lanes.
-template <int D>
-__device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
-                                           int b1, int e1, int b2, int e2, float qx, float qy, float qz,
-                                           int self, Top2 &best)
-{
-    const bool h1 = b1 < e1, h2 = b2 < e2;
-    const int len = (h1 ? e1 - b1 : 0) + (h2 ? e2 - b2 : 0);
-    const unsigned active = __ballot_sync(0xffffffffu, len > 0);
-    if (!active) return;
-    const int maxlen = __reduce_max_sync(0xffffffffu, len);
-    const int sumlen = __reduce_add_sync(0xffffffffu, len);
-    if (__popc(active) * 360 + sumlen * 3 < maxlen * 88) {
-        for (unsigned a = active; a; a &= a - 1) {
-            const int L = __ffs(a) - 1;
-            const float Lx = __shfl_sync(0xffffffffu, qx, L), Ly = __shfl_sync(0xffffffffu, qy, L);
-            const float Lz = D == 3 ? __shfl_sync(0xffffffffu, qz, L) : 0.f;
-            const int Lself = __shfl_sync(0xffffffffu, self, L);
-            const float thr = __shfl_sync(0xffffffffu, best.s2, L);
-            const int Lj1 = __shfl_sync(0xffffffffu, best.j1, L), Lj2 = __shfl_sync(0xffffffffu, best.j2, L);
-            const int Lb1 = __shfl_sync(0xffffffffu, b1, L), Le1 = __shfl_sync(0xffffffffu, e1, L);
-            const int Lb2 = __shfl_sync(0xffffffffu, b2, L), Le2 = __shfl_sync(0xffffffffu, e2, L);
-            Top2 tmp;
-            tmp.init();
-            coop_range<D>(v, lane, Lb1, Le1, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
-            coop_range<D>(v, lane, Lb2, Le2, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
-            float sa, sb;
-            int ja, jb;
-            coop_pop(tmp, sa, ja);
-            coop_pop(tmp, sb, jb);
-            if (lane == L) {
-                if (ja != KC_NOIDX) best.offer(sa, ja);
-                if (jb != KC_NOIDX) best.offer(sb, jb);
-            }
-        }
-        return;
-    }
-    const int B = __reduce_min_sync(0xffffffffu, min(h1 ? b1 : 0x7fffffff, h2 ? b2 : 0x7fffffff));
-    const int E = __reduce_max_sync(0xffffffffu, max(h1 ? e1 : 0, h2 ? e2 : 0));
-    tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
-}
-
-// Distance (lower bound) from the query to the nearest face of the sub-block u-1..u+1 (clipped to
-// the cell) that lies INSIDE the subdivided cell (k = cell coordinates); +inf if there is none.
-template <int D>
-__device__ __forceinline__ float sub_block_inner_bound(const View &v, float qx, float qy, float qz, int kx, int ky,
-                                                       int kz, int S, float hs, int ux, int uy, int uz)
-{
-    float bound = CUDART_INF_F;
-    SubAx a;
-    a.u = 0;
-    a.lo = v.lo0; a.q = qx; a.slk = v.slk0; a.base = kx * S;
-    if (ux - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qx, sub_face(a, ux - 1, hs)), v.slk0));
-    if (ux + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, ux + 2, hs), qx), v.slk0));
-    a.lo = v.lo1; a.q = qy; a.slk = v.slk1; a.base = ky * S;
-    if (uy - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qy, sub_face(a, uy - 1, hs)), v.slk1));
-    if (uy + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, uy + 2, hs), qy), v.slk1));
-    if (D == 3) {
-        a.lo = v.lo2; a.q = qz; a.slk = v.slk2; a.base = kz * S;
-        if (uz - 1 > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(qz, sub_face(a, uz - 1, hs)), v.slk2));
-        if (uz + 1 < S - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, uz + 2, hs), qz), v.slk2));
-    }
-    return bound;
-}
-
-// SWEEP = false: A3, every slot of a freshly built grid is a query.
-// SWEEP = true:  A7 for a large frontier: the same slot-ordered sweep over the incrementally
-//   updated grid, but only the slots marked with this call's epoch are queries (their lanes stay
-//   idle otherwise; warps without a marked slot leave at once), tombstones are inert records and
-//   the overflow chains of every visited cell are scanned too.  Runs only when *nF * sweep_div >= N
-//   (the list kernel serves smaller frontiers and the frontier points that live in chains).
-template <int D, bool SWEEP>
-__global__ void __launch_bounds__(32 * WT_WARPS)
-search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
-                    const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
-                    float *d2, float *c)
-{
-    __shared__ __align__(16) float4 s_p4[D == 3 ? WT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
-    __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    if (SWEEP && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = SWEEP && ctr->n_misfiled > 0;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const float qnan = __int_as_float(0x7fc00000);
-    float4 *tp4 = s_p4[D == 3 ? warp : 0];
-    float2 *tp2 = s_p2[D == 2 ? warp : 0];
-    int *tix = s_ix[D == 2 ? warp : 0];
-    // the whole tile starts inert: a short range leaves records behind it untouched
-    for (int k = lane; k < WT_TILE + 4; k += 32) {
-        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
-    }
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s - lane >= N) return;                     // whole warp past the end
-    const int sc = min(s, N - 1);                  // tail lanes mirror the last slot (no store)
-    float qx, qy, qz = 0.f;
-    int self;
-    if (D == 2) {
-        float2 q = v.spos2[sc];
-        qx = q.x; qy = q.y; self = v.sidx[sc];
-    } else {
-        float4 q = v.spos4[sc];
-        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
-    }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-    const int rowid = cz * v.G1 + cy;
-    const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
-    Top2 best;
-    best.init();
-    // queries of this warp (marked slots are never tombstones, so their cells are in slot order)
-    const bool query = SWEEP ? (s < N && mark[sc] == epoch) : true;
-    unsigned todo = __ballot_sync(0xffffffffu, query);
-    while (todo) {
-        const int leader = __ffs(todo) - 1;
-        const int R = __shfl_sync(0xffffffffu, rowid, leader);
-        const unsigned seg = __ballot_sync(0xffffffffu, rowid == R) & todo;
-        const int first = __ffs(seg) - 1, last = 31 - __clz(seg);
-        const int xf = __shfl_sync(0xffffffffu, cx, first), xl = __shfl_sync(0xffffffffu, cx, last);
-        const int ry = __shfl_sync(0xffffffffu, cy, first), rz = __shfl_sync(0xffffffffu, cz, first);
-        const bool mine = (seg >> lane) & 1u;
-        const int ux0 = max(xf - 1, 0), ux1 = min(xl + 1, v.G0 - 1);
-#pragma unroll 1
-        for (int k = -1; k < (D == 3 ? 8 : 2); ++k) {          // k = -1: the lanes' own row
-            const int oy = k < 0 ? 0 : row_oy(k), oz = k < 0 ? 0 : row_oz(k);
-            const int y = ry + oy, z = rz + oz;
-            if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
-            const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
-            if (chains && mine)
-                for (int x = has_l ? cx - 1 : cx; x <= (has_r ? cx + 1 : cx); ++x)
-                    scan_chain<D>(v, (z * v.G1 + y) * v.G0 + x, qx, qy, qz, self, best);
-            const int B = crow[ux0], E = crow[ux1 + 1];
-            if (B == E) continue;
-            if (E - B < v.dense_thr) {
-                int b = 0, e = 0;
-                if (mine) { b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1]; }
-                tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b, e, 0, 0, qx, qy, qz, self, best);
-                continue;
-            }
-            const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
-            if (k < 0) {
-                int s0 = 0, s1 = 0;
-                if (mine) { s0 = crow[cx]; s1 = crow[cx + 1]; }
-                const bool hv = mine && s1 - s0 >= v.heavy_T;
-                if (!__any_sync(0xffffffffu, hv)) {
-                    tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
-                } else {
-                    // Second level: a lane in a subdivided cell scans the 3^d sub-block around its own
-                    // sub-cell (clipped to the cell) instead of the whole cell, row by row through the
-                    // tile; the other lanes of the segment scan their own cell in the first pass.
-                    int S = 0, ux = 0, uy = 0, uz = 0;
-                    const int32_t *ss = v.leaf_start;
-                    if (hv) {
-                        const int2 si = v.subinfo[rowid * v.G0 + cx];
-                        S = si.x; ss += si.y;
-                        const float fS = (float)S;
-                        ux = sub_axis(qx, v.lo0, v.inv_h, cx, fS, S);
-                        uy = sub_axis(qy, v.lo1, v.inv_h, cy, fS, S);
-                        uz = D == 3 ? sub_axis(qz, v.lo2, v.inv_h, cz, fS, S) : 0;
-                    }
-#pragma unroll 1
-                    for (int j = -1; j < (D == 3 ? 8 : 2); ++j) {
-                        int b = 0, e = 0;
-                        if (hv) {
-                            const int y = uy + (j < 0 ? 0 : row_oy(j)), z = uz + (j < 0 ? 0 : row_oz(j));
-                            if (y >= 0 && y < S && z >= 0 && z < (D == 3 ? S : 1)) {
-                                const int32_t *srow = ss + (z * S + y) * S;
-                                b = srow[max(ux - 1, 0)]; e = srow[min(ux + 1, S - 1) + 1];
-                            }
-                        } else if (j < 0) {
-                            b = s0; e = s1;
-                        }
-                        const int Bj = __reduce_min_sync(0xffffffffu, b < e ? b : 0x7fffffff);
-                        const int Ej = __reduce_max_sync(0xffffffffu, b < e ? e : 0);
-                        if (Bj < Ej) tile_pass<D>(v, N, lane, tp2, tp4, tix, Bj, Ej, b, e, 0, 0, qx, qy, qz, self, best);
-                    }
-                    // the rest of the own cell, for a lane whose ball leaves the sub-block through a
-                    // face inside the cell (the faces on the cell's boundary are the neighbours' business)
-                    int rb = 0, re = 0;
-                    if (hv) {
-                        const float hs = __fdiv_rn(v.h, (float)S);
-                        if (!bound_ok(sub_block_inner_bound<D>(v, qx, qy, qz, cx, cy, cz, S, hs, ux, uy, uz), best.s2)) {
-                            rb = s0; re = s1;
-                        }
-                    }
-                    dense_pass<D>(v, N, lane, tp2, tp4, tix, rb, re, 0, 0, qx, qy, qz, self, best);
-                }
-                int bl = 0, el = 0, br = 0, er = 0;
-                if (mine && has_l && !(best.s2 < g.xm)) { bl = crow[cx - 1]; el = s0; }
-                if (mine && has_r && !(best.s2 < g.xp)) { br = s1; er = crow[cx + 2]; }
-                dense_pass<D>(v, N, lane, tp2, tp4, tix, bl, el, br, er, qx, qy, qz, self, best);
-            } else {
-                int b = 0, e = 0;
-                if (mine) {
-                    const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
-                    if (!(best.s2 < rb2)) {
-                        int x0 = cx, x1 = cx + 1;
-                        if (has_l && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
-                        if (has_r && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 2;
-                        b = crow[x0]; e = crow[x1];
-                    }
-                }
-                dense_pass<D>(v, N, lane, tp2, tp4, tix, b, e, 0, 0, qx, qy, qz, self, best);
-            }
-        }
-        todo &= ~seg;
-    }
-    if (!query) return;
-    const int r = finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
-    if (s >= N) return;
-    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, self, nn, nn2, d1, d2, c);
-}
-
 // ---- A3 / A7, leaf-tiled: the kernel behind kc_cert_grid_search and the slot sweep of A7 ---------
 // A warp owns 32 consecutive sorted slots.  Slots are sorted by leaf, so the windows the lanes need
 // from one row of their 3^d blocks (3 cells of a grid row for a lane in an undivided cell, 3
@@ -1007,34 +568,13 @@ search_tiled_kernel(View v, int N, Counters *ctr, const int32_t *__restrict__ ma
 // hold a subdivided cell, everything outside the 3^d sub-block of a lane in a subdivided cell --
 // range by range with every pruning test applied, and the queues are scanned by the warp in step.
 constexpr int LT_WARPS = 4;
+constexpr int SWEEP_MIN_N = 200000, SWEEP_DIV = 8;   // A7: when the slot sweep serves a frontier
+constexpr int WPQ_MAX = 32768;                       // A7: id lists up to this long get one warp per query
 #ifndef LT_MIN_BLOCKS
 #define LT_MIN_BLOCKS 7
 #endif
 constexpr int LT_HULL_MAX = 4096;                 // a longer hull (lanes far apart in memory) is left to phase 2
 static_assert(32 * LT_WARPS == PS_THREADS, "the range queues are strided by PS_THREADS");
-
-// bound of the scanned sub-block [x0,x1]x[y0,y1]x[z0,z1] of a subdivided cell: distance (lower
-// bound) from the query to its nearest face that is interior to the grid.  A face of the block on
-// the cell's boundary is a face of the cell; everything outside the block lies behind one of them.
-template <int D>
-__device__ __forceinline__ float sub_block_bound(const View &v, const Qry &q, int cx, int cy, int cz, int S,
-                                                 float hs, int x0, int x1, int y0, int y1, int z0, int z1)
-{
-    float bound = CUDART_INF_F;
-    SubAx a;
-    a.lo = v.lo0; a.q = q.x; a.slk = v.slk0; a.base = cx * S; a.u = 0;
-    if (x0 > 0 || cx > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.x, sub_face(a, x0, hs)), v.slk0));
-    if (x1 < S - 1 || cx < v.G0 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, x1 + 1, hs), q.x), v.slk0));
-    a.lo = v.lo1; a.base = cy * S;
-    if (y0 > 0 || cy > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.y, sub_face(a, y0, hs)), v.slk1));
-    if (y1 < S - 1 || cy < v.G1 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, y1 + 1, hs), q.y), v.slk1));
-    if (D == 3) {
-        a.lo = v.lo2; a.base = cz * S;
-        if (z0 > 0 || cz > 0) bound = fminf(bound, gap_lb(v, __fsub_rn(q.z, sub_face(a, z0, hs)), v.slk2));
-        if (z1 < S - 1 || cz < v.G2 - 1) bound = fminf(bound, gap_lb(v, __fsub_rn(sub_face(a, z1 + 1, hs), q.z), v.slk2));
-    }
-    return bound;
-}
 
 // index (k of phase 1) of the block row at offset (oy, oz): k = 0 own row, k >= 1: row_oy/row_oz(k-1)
 __device__ __forceinline__ int block_row_index(int oy, int oz)
@@ -1157,7 +697,7 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
 
 template <int D, int MODE>
 __global__ void __launch_bounds__(32 * LT_WARPS, LT_MIN_BLOCKS)
-search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, const int32_t *__restrict__ mark, int epoch,
+search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t *mark,
                    const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
                    float *d2, float *c)
 {
@@ -1184,7 +724,10 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, const i
     if (s - lane >= N) return;                     // whole warp past the end
     const int sc = min(s, N - 1);
     bool query = s < N;
-    if (MODE == 1) query = query && mark[sc] == epoch;
+    if (MODE == 1) {
+        query = query && mark[sc] != 0;
+        if (query) mark[sc] = 0;                   // the marks are all zero again when the sweep ends
+    }
     if (!__any_sync(0xffffffffu, query)) return;
     Qry q;
     q.z = 0.f;
@@ -1234,7 +777,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, const i
                 if (y >= 0 && y < v.G1 && z >= 0 && z < v.G2) {
                     const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
                     b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1];
-                    if (e - b < v.dense_thr) {
+                    if (e - b < v.heavy_T) {
                         covered |= 7u << (3 * k);
                     } else if (k == 0) {
                         // a long window (dense cells, or a subdivided one): the ball of phase 2 prunes
@@ -1323,7 +866,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, const i
 // points that live in an overflow chain have no slot and go to the list kernel (list2).
 __global__ void __launch_bounds__(256)
 mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ nF, int N, int sweep_div,
-                     const int32_t *__restrict__ slot, int32_t *mark, int epoch, int32_t *list2,
+                     const int32_t *__restrict__ slot, int32_t *mark, int32_t *list2,
                      Counters *ctr)
 {
     const int n = *nF;
@@ -1336,7 +879,7 @@ mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ 
         if (f < n) {
             i = F[f];
             const int sl = slot[i];
-            if (sl >= 0) mark[sl] = epoch;
+            if (sl >= 0) mark[sl] = 1;
             else chain = true;
         }
         warp_append(chain, i, list2, &ctr->n_list2);
@@ -1350,8 +893,7 @@ mark_frontier_kernel(const int32_t *__restrict__ F, const int32_t *__restrict__ 
 // against the second-best found so far; short surviving ranges are scanned by their lanes, long
 // ones (dense cells) by the whole warp, and two warp reductions extract the two smallest keys.
 // No lane ever waits for another query's insertions, and the order of the queries is irrelevant,
-// which is what a frontier list in id order needs (A7).  SLOTS = true runs the same search for
-// every sorted slot of a fresh grid (A3 variant, for comparison with the tiled sweep).
+// which is what a frontier list in id order needs (A7).
 template <int D>
 __device__ __forceinline__ void lane_offer(Top2 &tmp, float s, int j, float thr, int self)
 {
@@ -1451,7 +993,7 @@ __device__ __forceinline__ void list2_done(Counters *ctr)
         }
     }
 }
-template <int D, bool SLOTS>
+template <int D>
 __global__ void __launch_bounds__(128)
 search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__restrict__ F,
                   const int32_t *__restrict__ nF, const int32_t *__restrict__ list2, int sweep_div,
@@ -1459,17 +1001,12 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
 {
     const int lane = threadIdx.x & 31;
     const int w0 = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = (gridDim.x * blockDim.x) >> 5;
-    int n = N;
-    const int32_t *__restrict__ Q = nullptr;
-    bool chains = false;
-    if (!SLOTS) {
-        // a large frontier is served by the slot sweep; only its chain residents (list2) come here
-        const bool swept = sweep_div > 0 && (int64_t)*nF * sweep_div >= N;
-        n = swept ? ctr->n_list2 : *nF;
-        Q = swept ? list2 : F;
-        chains = ctr->n_misfiled > 0;
-    }
-    if (!SLOTS && n > v.wpq_max) {
+    // a large frontier is served by the slot sweep; only its chain residents (list2) come here
+    const bool swept = sweep_div > 0 && (int64_t)*nF * sweep_div >= N;
+    const int n = swept ? ctr->n_list2 : *nF;
+    const int32_t *__restrict__ Q = swept ? list2 : F;
+    const bool chains = ctr->n_misfiled > 0;
+    if (n > WPQ_MAX) {
         // long list: one thread per query keeps more queries in flight
         for (int f = blockIdx.x * blockDim.x + threadIdx.x; f < n; f += gridDim.x * blockDim.x) {
             const int i = Q[f];
@@ -1488,16 +1025,9 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
         return;
     }
     for (int f = w0; f < n; f += nw) {
-        float qx, qy, qz = 0.f;
-        int i;
-        if (SLOTS) {
-            if (D == 2) { const float2 q = v.spos2[f]; qx = q.x; qy = q.y; i = v.sidx[f]; }
-            else { const float4 q = v.spos4[f]; qx = q.x; qy = q.y; qz = q.z; i = __float_as_int(q.w); }
-        } else {
-            i = Q[f];
-            qx = p_new[(int64_t)i * D]; qy = p_new[(int64_t)i * D + 1];
-            if (D == 3) qz = p_new[(int64_t)i * D + 2];
-        }
+        const int i = Q[f];
+        const float qx = p_new[(int64_t)i * D], qy = p_new[(int64_t)i * D + 1];
+        const float qz = D == 3 ? p_new[(int64_t)i * D + 2] : 0.f;
         Top2 best;
         const int r = wpq_search<D>(v, chains, lane, qx, qy, qz, i, best);
         if (lane == 0) {
@@ -1505,7 +1035,7 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
             store_cert(best, i, nn, nn2, d1, d2, c);
         }
     }
-    if (!SLOTS) list2_done(ctr);
+    list2_done(ctr);
 }
 
 // ---- NEXT #4: K-list certificates through the grid ---------------------------------------------
@@ -1688,27 +1218,9 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)g->N;
-    static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 4;
-    const int tb = 32 * WT_WARPS;
-    if (variant == 4) {
-        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
-        if (g->geom.d == 2) search_leaf_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-        else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-    } else if (variant == 3) {
-        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
-        if (g->geom.d == 2) search_phased_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-        else search_phased_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-    } else if (variant == 1) {
-        if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-        else search_tiled_kernel<3, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, 0, nullptr, 0, nn, nn2, d1, d2, c);
-    } else if (variant == 2) {
-        const int blocks = blocks_for(n, 4, 148 * 16);
-        if (g->geom.d == 2) search_wpq_kernel<2, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
-        else search_wpq_kernel<3, true><<<blocks, 128, 0, st>>>(v, nullptr, n, nullptr, nullptr, nullptr, 0, g->ctr, nn, nn2, d1, d2, c);
-    } else {
-        if (g->geom.d == 2) search_all_kernel<2><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-        else search_all_kernel<3><<<(n + 127) / 128, 128, 0, st>>>(v, n, g->ctr, nn, nn2, d1, d2, c);
-    }
+    const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+    if (g->geom.d == 2) search_leaf_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
+    else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
     return KC_OK;
@@ -1786,38 +1298,24 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)N;
-    static const int div_env = getenv("KC_SWEEP_DIV") ? atoi(getenv("KC_SWEEP_DIV")) : 8;
-    static const int min_env = getenv("KC_SWEEP_MIN_N") ? atoi(getenv("KC_SWEEP_MIN_N")) : 200000;
-    const int sweep_div = N >= min_env && nF_max * (int64_t)div_env >= N ? div_env : 0;
-    const int tb = 32 * WT_WARPS;
+    // slot sweep: grids of at least SWEEP_MIN_N points, frontier of at least N / SWEEP_DIV points
+    // (the host bound decides whether the sweep kernels are launched, the device count whether they run)
+    const int sweep_div = N >= SWEEP_MIN_N && nF_max * (int64_t)SWEEP_DIV >= N ? SWEEP_DIV : 0;
     if (sweep_div > 0) {
-        ++g->epoch;
-        mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->epoch, g->list2, g->ctr);
-        static const int variant = getenv("KC_SEARCH_VARIANT") ? atoi(getenv("KC_SEARCH_VARIANT")) : 4;
-        if (variant == 4) {
-            const int nb = (n + PS_THREADS - 1) / PS_THREADS;
-            if (g->geom.d == 2)
-                search_leaf_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-            else
-                search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-        } else if (variant == 3) {
-            const int nb = (n + PS_THREADS - 1) / PS_THREADS;
-            if (g->geom.d == 2)
-                search_phased_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-            else
-                search_phased_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
-        } else if (g->geom.d == 2)
-            search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+        mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->list2, g->ctr);
+        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+        if (g->geom.d == 2)
+            search_leaf_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         else
-            search_tiled_kernel<3, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, g->epoch, nF, sweep_div, nn, nn2, d1, d2, c);
+            search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         count_launches(2);
     }
     int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
-    if (nF_max > v.wpq_max) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
+    if (nF_max > WPQ_MAX) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
     if (g->geom.d == 2)
-        search_wpq_kernel<2, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
+        search_wpq_kernel<2><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
     else
-        search_wpq_kernel<3, false><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
+        search_wpq_kernel<3><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
     count_launches(1);
     KC_LAUNCH_CHECK("kc_frontier_search");
     return KC_OK;

@@ -624,11 +624,14 @@ def test_frontier_search_twice_on_one_update():
     p = wl.uniform_points(N, 2, 77)
     rng = np.random.default_rng(78)
     q = (p + rng.uniform(-2e-3, 2e-3, p.shape)).astype(np.float32)      # many points change cell
+    movers = np.sort(rng.choice(N, N // 10, replace=False)).astype(np.int32)   # below the re-bin bound N/8
+    still = np.setdiff1d(np.arange(N), movers)
+    q[still] = p[still]
     grid = kc.Grid(N, geoms(p)[1])
     certs = kc.kc_cert_grid_rebuild(grid, dev(p))
     Q = dev(q)
-    kc.kc_grid_update(grid, Q)
-    assert grid.info().n_misfiled > N // 20
+    kc.kc_grid_update(grid, Q, movers=dev(movers))
+    assert grid.info().n_misfiled > N // 200 and grid.info().dirty == 1
     post = ref_certs(q)
     perm = rng.permutation(N).astype(np.int32)
     F1, F2 = np.sort(perm[: N // 2]), np.sort(perm[N // 2: N // 2 + N // 4])
@@ -660,3 +663,69 @@ def test_maintainer_any_N(N):
     F = oracle.frontier(ref_certs(p).c, oracle.max_displacement(p, q))[1]
     assert int(res.nF.item()) == F.size
     assert_same(res.repaired, post, idx=F, what="repaired")
+
+
+def test_update_rebins_when_most_points_move():
+    """kc_grid_update on a large grid with every point a potential mover re-bins (A2) instead of
+    re-filing: no chains, the grid counts as fresh, the frontier search that follows is exact."""
+    N = 150_000
+    p = wl.mixture_points(N, 3, 91, 16, 0.01)
+    rng = np.random.default_rng(92)
+    q = (p + rng.uniform(-1e-3, 1e-3, p.shape)).astype(np.float32)
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+    kc.kc_grid_update(grid, dev(q))
+    info = grid.info()
+    assert info.n_misfiled == 0 and info.dirty == 0
+    assert np.array_equal(grid.export(0).cpu().numpy(), oracle.cell_ids(q, g_or))
+    F = np.sort(rng.choice(N, N // 3, replace=False)).astype(np.int32)
+    kc.kc_frontier_search(grid, dev(q), dev(F), dev(np.array([F.size], np.int32)), certs)
+    post = ref_certs(q)
+    assert_same(certs, post, idx=F, what="after a re-binning update")
+    rest = np.setdiff1d(np.arange(N), F)
+    assert_same(certs, ref_certs(p), idx=rest, what="untouched")
+
+
+def test_sweep_path_replays_from_a_cuda_graph():
+    """The slot sweep keeps no host-side counter: update + classify + sweep captured once at
+    N = 262,144 and replayed on new positions is exact every time."""
+    N = 262_144
+    p = wl.uniform_points(N, 3, 93)
+    rng = np.random.default_rng(94)
+    g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
+    P, Q = dev(p), dev(p)
+    certs = kc.kc_cert_grid_rebuild(grid, P)
+    eps = torch.zeros(1, device="cuda")
+    flags = torch.empty(N, dtype=torch.uint8, device="cuda")
+    F = torch.empty(N, dtype=torch.int32, device="cuda")
+    nF = torch.zeros(1, dtype=torch.int32, device="cuda")
+    work = kc.Certs.empty(N)
+
+    def body():
+        work.buf.copy_(certs.buf)
+        kc.kc_max_displacement(P, Q, eps)
+        kc.kc_frontier_classify(work.c, eps, flags, F, nF)
+        kc.kc_grid_build(grid, P)                              # the grid resident at p ...
+        kc.kc_frontier_repair(grid, Q, F, nF, work)            # ... updated to q, F re-searched
+
+    q0 = (p + rng.uniform(-5e-4, 5e-4, p.shape)).astype(np.float32)
+    Q.copy_(dev(q0))
+    body()
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        body()
+    pre = ref_certs(p)
+    for rnd in range(3):
+        q = (p + rng.uniform(-5e-4, 5e-4, p.shape)).astype(np.float32)
+        Q.copy_(dev(q))
+        g.replay()
+        torch.cuda.synchronize()
+        wf, wF = oracle.frontier(pre.c, oracle.max_displacement(p, q))
+        assert int(nF.item()) == wF.size and wF.size * 8 >= N          # sweep-sized
+        post = ref_certs(q)
+        assert_same(work, post, idx=wF, what=f"replay {rnd}")
+        rest = np.flatnonzero(wf == 0)
+        assert np.array_equal(host(work).nn[rest], post.nn[rest])

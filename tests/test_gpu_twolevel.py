@@ -50,7 +50,7 @@ def check_structure(grid, p, g_or):
     nleaf = np.where(S > 0, S.astype(np.int64) ** d, 1)
     assert np.array_equal(sub[:, 1], np.concatenate([[0], np.cumsum(nleaf)[:-1]]))
     assert info.n_leaves == nleaf.sum()
-    assert np.all(S[heavy].astype(np.int64) ** d * 2 <= np.maximum(counts[heavy], 2 ** (d + 1)))
+    assert np.all(S[heavy].astype(np.int64) ** d <= np.maximum(counts[heavy], 2 ** d))
     G = np.array(g_or.G[:d])
     lo = np.array(g_or.lo[:d], np.float64)
     h = float(g_or.h)
@@ -72,12 +72,15 @@ def check_structure(grid, p, g_or):
     return info
 
 
+@pytest.mark.parametrize("index", [None, (1, 1), (1, 2), (64, 8)])
 @pytest.mark.parametrize("d,N,n_blobs,sigma", [(2, 40000, 3, 2e-3), (3, 40000, 2, 4e-3), (3, 9000, 1, 1e-4),
                                               (2, 9000, 1, 1e-5)])
-def test_two_level_build_and_search_dense_cells(d, N, n_blobs, sigma):
+def test_two_level_build_and_search_dense_cells(d, N, n_blobs, sigma, index):
     p = blob_scene(N, d, 100 + d + N, n_blobs, sigma)
     g_or, g_kc = geoms(p)
     grid = kc.Grid(N, g_kc)
+    if index is not None:                                   # (heavy_T, sub_occ): many small sub-grids ... few large ones
+        grid.set_index(*index)
     certs = kc.kc_cert_grid_rebuild(grid, dev(p))
     info = check_structure(grid, p, g_or)
     assert info.max_occ >= 2000 and info.n_heavy >= 1
@@ -110,6 +113,7 @@ def test_repair_on_subdivided_cells(d):
     p = blob_scene(N, d, 55 + d, 4, 3e-3)
     g_or, g_kc = geoms(p)
     grid = kc.Grid(N, g_kc)
+    grid.set_index(16, 2)
     certs = kc.kc_cert_grid_rebuild(grid, dev(p))
     rng = np.random.default_rng(9)
     for step in range(3):
@@ -125,3 +129,24 @@ def test_repair_on_subdivided_cells(d):
         certs = kc.Certs(*(dev(x) for x in (post.nn, post.nn2, post.d1, post.d2, post.c)))
         p = q
     assert grid.info().n_misfiled > 0
+
+
+@pytest.mark.parametrize("cfg", ["cfg3", "cfg5_d2", "cfg5_d3"])
+def test_index_parameters_never_change_a_result(cfg):
+    """Config scenes with the second level forced on everywhere it can apply (small thresholds)
+    and switched off: rebuild and a sweep-sized repair are bit-exact either way."""
+    N = 250_000 if cfg != "cfg3" else 16000
+    p, mot = wl.make_scene(cfg, "cluster_drift" if cfg == "cfg3" else None, N=N)
+    q, _ = mot.step(p)
+    want, post = ref_certs(p), ref_certs(q)
+    F = np.sort(np.random.default_rng(3).choice(N, N // 2, replace=False)).astype(np.int32)
+    movers = np.sort(np.random.default_rng(4).choice(N, N // 12, replace=False)).astype(np.int32)
+    q2 = p.copy(); q2[movers] = q[movers]
+    post2 = ref_certs(q2)
+    for index in [(1, 1), (1, 4), (32, 2), (10 ** 9, 4)]:
+        grid = kc.Grid(N, geoms(p)[1])
+        grid.set_index(*index)
+        certs = kc.kc_cert_grid_rebuild(grid, dev(p))
+        assert_same(certs, want, what=f"{cfg} index={index}")
+        kc.kc_frontier_repair(grid, dev(q2), dev(F), dev(np.array([F.size], np.int32)), certs, movers=dev(movers))
+        assert_same(certs, post2, idx=F, what=f"{cfg} index={index} repair")
