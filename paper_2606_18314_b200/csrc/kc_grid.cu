@@ -9,7 +9,7 @@
 //   leaf_start[n_leaves+1] int32  exclusive scan of the leaf sizes (entry l+1 doubles as the scatter
 //                           cursor of leaf l during the build)
 //   spos2[N] float2 (d=2) / spos4[N] float4 = (x,y,z,bits(idx)) (d=3)   leaf-sorted positions
-//   sidx[N]        int32   point id per sorted slot (-1 = tombstone)
+//   sidx[N]        int32   point id per sorted slot (-1 = tombstone); d = 2 only: a d = 3 record carries its id
 //   slot[N]        int32   sorted slot of point i (-1 = lives in an overflow chain)
 //   head[C_tot], next[N], opos[N] float4, mlist[N]   overflow chains of re-filed points (A6)
 //   fcount[C_tot], mhist[]  scratch of A5 (always left zeroed)
@@ -423,7 +423,7 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
         spos4[s] = make_float4(p[3 * (int64_t)i], p[3 * (int64_t)i + 1], p[3 * (int64_t)i + 2],
                                __int_as_float(i));
     }
-    sidx[s] = i;
+    if (D == 2) sidx[s] = i;              // d = 3: the id travels in the record's fourth word
     slot[i] = s;
 }
 
@@ -477,7 +477,7 @@ refresh_kernel(View v, const float *__restrict__ p_new, int N, const int32_t *__
                     const float qnan = __int_as_float(0x7fc00000);
                     if (D == 2) spos2[sl] = make_float2(qnan, qnan);
                     else spos4[sl] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-                    sidx[sl] = -1;
+                    if (D == 2) sidx[sl] = -1;
                     slot[i] = -1;
                     misfile = true;
                     in_chain = true;
@@ -688,6 +688,12 @@ classify_local_kernel(View v, float R, int N, const int32_t *__restrict__ cell,
     }
     __syncthreads();
     if (infr) F[bbase + wsum[warp] + __popc(m & ((1u << lane) - 1))] = i;
+}
+
+__global__ void record_ids_kernel(const float4 *__restrict__ spos4, int n, int32_t *__restrict__ out)
+{
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x)
+        out[t] = __float_as_int(spos4[t].w);
 }
 
 }  // namespace
@@ -962,7 +968,16 @@ extern "C" kc_status kc_grid_export(const kc_grid *g, int what, int32_t *dst, in
     switch (what) {
     case 0: src = g->cell; n = g->N; break;
     case 1: src = g->cell_start; n = g->n_cells + 1; break;
-    case 2: src = g->sidx; n = g->N; break;
+    case 2:
+        n = g->N;
+        if (g->geom.d == 3 && dst && capacity >= n) {     // d = 3 keeps the ids inside the records
+            record_ids_kernel<<<blocks_for(n, 256, 148 * 8), 256, 0, (cudaStream_t)stream>>>(g->spos4, (int)n, dst);
+            *count = n;
+            KC_LAUNCH_CHECK("kc_grid_export");
+            return KC_OK;
+        }
+        src = g->sidx;
+        break;
     case 3: src = g->slot; n = g->N; break;
     case 4: src = g->counts; n = g->n_cells; break;
     case 5: src = reinterpret_cast<const int32_t *>(g->subinfo); n = 2 * g->n_cells; break;
