@@ -172,9 +172,10 @@ size_t kc_grid_bytes(const kc_grid *g);
 /* host.  Parameters of the two-level index ("a hierarchical GPU index ... could lower its constant
  * further"): a cell that holds at least heavy_T records at build time is subdivided
  * into S^d sub-cells, S = floor((count / sub_occ)^(1/d)) >= 2, and its records are sorted by
- * sub-cell, so the searches prune inside it.  Defaults: sub_occ = 4, heavy_T = 128 (d = 2) / 256
- * (d = 3); heavy_T is raised to sub_occ * 2^(d+1) if smaller.  Results never depend on these
- * values.  Takes effect with the next kc_grid_build (the grid counts as not built until then). */
+ * sub-cell, so the searches prune inside it.  Defaults: sub_occ = 4; heavy_T = 256 for d = 3 and
+ * INT_MAX (no second level) for d = 2, where the whole-set search prunes cell by cell instead;
+ * heavy_T is raised to sub_occ * 2^(d+1) if smaller.  Results never depend on these values.
+ * Takes effect with the next kc_grid_build (the grid counts as not built until then). */
 kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ);
 
 /* A2: cell id per point, per-cell histogram, exclusive scan, scatter into cell-sorted arrays (a

@@ -725,10 +725,11 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
         delete g;
         return KC_EINVAL;
     }
-    // two-level index defaults (measured on config 5): cells of >= 128 (d=2) / 256
-    // (d=3) records are subdivided at ~4 records per sub-cell; kc_grid_set_index changes them
+    // two-level index defaults (measured on config 5): d = 3: cells of >= 256 records
+    // are subdivided at ~4 records per sub-cell; d = 2: off (the plane's whole-set kernel prunes
+    // cell by cell instead); kc_grid_set_index changes them
     g->sub_occ = 4;
-    g->heavy_T = geom->d == 2 ? 128 : 256;
+    g->heavy_T = geom->d == 2 ? KC_INDEX_OFF : 256;
     g->n_scan_blocks = (int)((g->n_leaves_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
     bool ok = true;
     auto alloc = [&](void **p, size_t bytes) {
@@ -799,7 +800,7 @@ extern "C" kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ)
     }
     const int thr_min = sub_occ << (g->geom.d + 1);      // keeps the leaf count within n_leaves_max
     g->sub_occ = sub_occ;
-    g->heavy_T = heavy_T < thr_min ? thr_min : heavy_T;
+    g->heavy_T = heavy_T < thr_min ? thr_min : heavy_T;   // (KC_INDEX_OFF = INT_MAX: no second level)
     g->built = 0;                                         // takes effect with the next build
     return KC_OK;
 }
@@ -815,9 +816,10 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     const int n = (int)N, nc = (int)g->n_cells;
     const int d = g->geom.d, T = g->heavy_T, so = g->sub_occ;
     // upper bound of the number of leaves of THIS build (the device knows the exact count)
-    const int64_t nl_max = (int64_t)nc + N + 8;
+    const bool two_level = T != KC_INDEX_OFF;             // off: the leaves are the cells, no second pass
+    const int64_t nl_max = two_level ? (int64_t)nc + N + 8 : 0;
     const int ncb = (nc + SCAN_CHUNK - 1) / SCAN_CHUNK, nlb = (int)((nl_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
-    build_prep_kernel<<<blocks_for(nl_max / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr,
+    build_prep_kernel<<<blocks_for((nl_max > nc ? nl_max : nc) / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr,
                                                                               g->counts, nc, g->leaf_cnt, nl_max);
     if (d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
@@ -833,9 +835,12 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
         count_launches(3);
     }
     // second level (these kernels leave at once when no cell is subdivided)
-    if (d == 2) leafid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
+    if (!two_level) {
+    } else if (d == 2) leafid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
     else leafid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
-    if (nl_max <= 4 * SCAN_SMALL_MAX) {
+    if (!two_level) {
+        count_launches(-1);
+    } else if (nl_max <= 4 * SCAN_SMALL_MAX) {
         lscan_small_kernel<<<1, 1024, 0, st>>>(g->leaf_cnt, g->leaf_start, g->ctr);
         count_launches(1);
     } else {

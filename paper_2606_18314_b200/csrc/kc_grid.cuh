@@ -33,6 +33,8 @@ struct Counters {
 // storage order; leaf_start is the exclusive scan of their sizes, subinfo[c] = {S or 0, first leaf}.
 // Sub-cell of coordinate x in cell k of an axis: clamp(floorf(fl(fl(t - k) * S)), 0, S-1) with the
 // cell coordinate t = fl(fl(x - lo) * inv_h) of cell_axis(): monotone in x like cell_axis itself.
+constexpr int KC_INDEX_OFF = 0x7fffffff;          // heavy_T value that switches the second level off
+
 __host__ __device__ inline int sub_res(int cnt, int d, int heavy_T, int sub_occ)
 {
     if (cnt < heavy_T) return 0;

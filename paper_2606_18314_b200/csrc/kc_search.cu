@@ -556,6 +556,170 @@ __device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
         tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
     }
 }
+// ---- d = 2: the row-segment kernel with cell-wise pruning of dense rows -------------------------
+// In the plane the leaf-tiled kernel below loses to this older one on clustered data (config 5,
+// d = 2: 0.75 vs 0.68 ms): cells of 10-70 records are too small for a second level, and what pays
+// there is pruning cell by cell plus the warp-cooperative scan of the few long ranges that survive
+// it.  A warp owns 32 consecutive sorted slots; the lanes of one grid row form a segment whose 3-cell
+// windows are one contiguous range per row: sparse rows go through the tile whole, dense rows
+// (>= WT_DENSE records) own cell first, then only the cells a lane cannot rule out.  The second level
+// of the index is ignored (level-0 ranges are contiguous whatever the order inside a cell).
+constexpr int WT_WARPS = 4;
+constexpr int WT_DENSE = 128;
+
+// Dense pass: every lane brings up to two ranges left after pruning.  Served lane by lane by the
+// whole warp when that is cheaper than a tile pass over the hull [B, E) (issue-slot estimates:
+// tile pass ~11 per record of the longest lane, cooperative ~45 per served lane + 12 per 32
+// records).  Called by all 32 lanes.
+template <int D>
+__device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float2 *tp2, float4 *tp4, int *tix,
+                                           int b1, int e1, int b2, int e2, float qx, float qy, float qz,
+                                           int self, Top2 &best)
+{
+    const bool h1 = b1 < e1, h2 = b2 < e2;
+    const int len = (h1 ? e1 - b1 : 0) + (h2 ? e2 - b2 : 0);
+    const unsigned active = __ballot_sync(0xffffffffu, len > 0);
+    if (!active) return;
+    const int maxlen = __reduce_max_sync(0xffffffffu, len);
+    const int sumlen = __reduce_add_sync(0xffffffffu, len);
+    if (__popc(active) * 360 + sumlen * 3 < maxlen * 88) {
+        for (unsigned a = active; a; a &= a - 1) {
+            const int L = __ffs(a) - 1;
+            const float Lx = __shfl_sync(0xffffffffu, qx, L), Ly = __shfl_sync(0xffffffffu, qy, L);
+            const float Lz = D == 3 ? __shfl_sync(0xffffffffu, qz, L) : 0.f;
+            const int Lself = __shfl_sync(0xffffffffu, self, L);
+            const float thr = __shfl_sync(0xffffffffu, best.s2, L);
+            const int Lj1 = __shfl_sync(0xffffffffu, best.j1, L), Lj2 = __shfl_sync(0xffffffffu, best.j2, L);
+            const int Lb1 = __shfl_sync(0xffffffffu, b1, L), Le1 = __shfl_sync(0xffffffffu, e1, L);
+            const int Lb2 = __shfl_sync(0xffffffffu, b2, L), Le2 = __shfl_sync(0xffffffffu, e2, L);
+            Top2 tmp;
+            tmp.init();
+            coop_range<D>(v, lane, Lb1, Le1, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
+            coop_range<D>(v, lane, Lb2, Le2, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
+            float sa, sb;
+            int ja, jb;
+            coop_pop(tmp, sa, ja);
+            coop_pop(tmp, sb, jb);
+            if (lane == L) {
+                if (ja != KC_NOIDX) best.offer(sa, ja);
+                if (jb != KC_NOIDX) best.offer(sb, jb);
+            }
+        }
+        return;
+    }
+    const int B = __reduce_min_sync(0xffffffffu, min(h1 ? b1 : 0x7fffffff, h2 ? b2 : 0x7fffffff));
+    const int E = __reduce_max_sync(0xffffffffu, max(h1 ? e1 : 0, h2 ? e2 : 0));
+    tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b1, e1, b2, e2, qx, qy, qz, self, best);
+}
+
+// SWEEP = false: A3, every slot of a freshly built grid is a query.
+// SWEEP = true:  A7 for a large frontier: the same slot-ordered sweep over the incrementally
+//   updated grid, but only the slots marked with this call's epoch are queries (their lanes stay
+//   idle otherwise; warps without a marked slot leave at once), tombstones are inert records and
+//   the overflow chains of every visited cell are scanned too.  Runs only when *nF * sweep_div >= N
+//   (the list kernel serves smaller frontiers and the frontier points that live in chains).
+template <int D, bool SWEEP>
+__global__ void __launch_bounds__(32 * WT_WARPS)
+search_tiled_kernel(View v, int N, Counters *ctr, int32_t *mark,
+                    const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
+                    float *d2, float *c)
+{
+    __shared__ __align__(16) float4 s_p4[D == 3 ? WT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
+    __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    if (SWEEP && (int64_t)*nF * sweep_div < N) return;
+    const bool chains = SWEEP && ctr->n_misfiled > 0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float qnan = __int_as_float(0x7fc00000);
+    float4 *tp4 = s_p4[D == 3 ? warp : 0];
+    float2 *tp2 = s_p2[D == 2 ? warp : 0];
+    int *tix = s_ix[D == 2 ? warp : 0];
+    // the whole tile starts inert: a short range leaves records behind it untouched
+    for (int k = lane; k < WT_TILE + 4; k += 32) {
+        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
+    }
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s - lane >= N) return;                     // whole warp past the end
+    const int sc = min(s, N - 1);                  // tail lanes mirror the last slot (no store)
+    float qx, qy, qz = 0.f;
+    int self;
+    if (D == 2) {
+        float2 q = v.spos2[sc];
+        qx = q.x; qy = q.y; self = v.sidx[sc];
+    } else {
+        float4 q = v.spos4[sc];
+        qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
+    }
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    const int rowid = cz * v.G1 + cy;
+    const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
+    Top2 best;
+    best.init();
+    // queries of this warp (marked slots are never tombstones, so their cells are in slot order)
+    const bool query = SWEEP ? (s < N && mark[sc] != 0) : true;
+    if (SWEEP && query) mark[sc] = 0;              // the marks are all zero again when the sweep ends
+    unsigned todo = __ballot_sync(0xffffffffu, query);
+    while (todo) {
+        const int leader = __ffs(todo) - 1;
+        const int R = __shfl_sync(0xffffffffu, rowid, leader);
+        const unsigned seg = __ballot_sync(0xffffffffu, rowid == R) & todo;
+        const int first = __ffs(seg) - 1, last = 31 - __clz(seg);
+        const int xf = __shfl_sync(0xffffffffu, cx, first), xl = __shfl_sync(0xffffffffu, cx, last);
+        const int ry = __shfl_sync(0xffffffffu, cy, first), rz = __shfl_sync(0xffffffffu, cz, first);
+        const bool mine = (seg >> lane) & 1u;
+        const int ux0 = max(xf - 1, 0), ux1 = min(xl + 1, v.G0 - 1);
+#pragma unroll 1
+        for (int k = -1; k < (D == 3 ? 8 : 2); ++k) {          // k = -1: the lanes' own row
+            const int oy = k < 0 ? 0 : row_oy(k), oz = k < 0 ? 0 : row_oz(k);
+            const int y = ry + oy, z = rz + oz;
+            if (y < 0 || y >= v.G1 || z < 0 || z >= v.G2) continue;
+            const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
+            if (chains && mine)
+                for (int x = has_l ? cx - 1 : cx; x <= (has_r ? cx + 1 : cx); ++x)
+                    scan_chain<D>(v, (z * v.G1 + y) * v.G0 + x, qx, qy, qz, self, best);
+            const int B = crow[ux0], E = crow[ux1 + 1];
+            if (B == E) continue;
+            if (E - B < WT_DENSE) {
+                int b = 0, e = 0;
+                if (mine) { b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1]; }
+                tile_pass<D>(v, N, lane, tp2, tp4, tix, B, E, b, e, 0, 0, qx, qy, qz, self, best);
+                continue;
+            }
+            const Gaps g = make_gaps<D>(v, qx, qy, qz, cx, cy, cz);
+            if (k < 0) {
+                int s0 = 0, s1 = 0;
+                if (mine) { s0 = crow[cx]; s1 = crow[cx + 1]; }
+                tile_pass<D>(v, N, lane, tp2, tp4, tix, crow[xf], crow[xl + 1], s0, s1, 0, 0, qx, qy, qz, self, best);
+                int bl = 0, el = 0, br = 0, er = 0;
+                if (mine && has_l && !(best.s2 < g.xm)) { bl = crow[cx - 1]; el = s0; }
+                if (mine && has_r && !(best.s2 < g.xp)) { br = s1; er = crow[cx + 2]; }
+                dense_pass<D>(v, N, lane, tp2, tp4, tix, bl, el, br, er, qx, qy, qz, self, best);
+            } else {
+                int b = 0, e = 0;
+                if (mine) {
+                    const float rb2 = __fadd_rn(oy < 0 ? g.ym : (oy > 0 ? g.yp : 0.f), oz < 0 ? g.zm : (oz > 0 ? g.zp : 0.f));
+                    if (!(best.s2 < rb2)) {
+                        int x0 = cx, x1 = cx + 1;
+                        if (has_l && !(best.s2 < __fadd_rn(rb2, g.xm))) x0 = cx - 1;
+                        if (has_r && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 2;
+                        b = crow[x0]; e = crow[x1];
+                    }
+                }
+                dense_pass<D>(v, N, lane, tp2, tp4, tix, b, e, 0, 0, qx, qy, qz, self, best);
+            }
+        }
+        todo &= ~seg;
+    }
+    if (!query) return;
+    const int r = finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    if (s >= N) return;
+    if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    store_cert(best, self, nn, nn2, d1, d2, c);
+}
+
 // ---- A3 / A7, leaf-tiled: the kernel behind kc_cert_grid_search and the slot sweep of A7 ---------
 // A warp owns 32 consecutive sorted slots.  Slots are sorted by leaf, so the windows the lanes need
 // from one row of their 3^d blocks (3 cells of a grid row for a lane in an undivided cell, 3
@@ -1240,8 +1404,8 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)g->N;
-    const int nb = (n + PS_THREADS - 1) / PS_THREADS;
-    if (g->geom.d == 2) search_leaf_kernel<2, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
+    const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
+    if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
@@ -1325,9 +1489,9 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     const int sweep_div = N >= SWEEP_MIN_N && nF_max * (int64_t)SWEEP_DIV >= N ? SWEEP_DIV : 0;
     if (sweep_div > 0) {
         mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->list2, g->ctr);
-        const int nb = (n + PS_THREADS - 1) / PS_THREADS;
+        const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
         if (g->geom.d == 2)
-            search_leaf_kernel<2, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         else
             search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         count_launches(2);
