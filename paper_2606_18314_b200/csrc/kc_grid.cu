@@ -417,13 +417,20 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
     if (i >= N) return;
     const int leaf = ctr->n_heavy ? leafid[i] : cell[i];
     int s = atomicAdd(&leaf_start[leaf + 1], 1);
+    // The sorted arrays are written at random slots, a fraction of a 32-byte sector at a time: the
+    // stores ask L2 to keep their sectors (evict_last) so that a sector is completed in L2 and
+    // written back once instead of being evicted half-written and filled again.
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     if (D == 2) {
-        spos2[s] = reinterpret_cast<const float2 *>(p)[i];
+        const float2 r = reinterpret_cast<const float2 *>(p)[i];
+        asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(spos2 + s), "f"(r.x), "f"(r.y), "l"(pol) : "memory");
+        asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(sidx + s), "r"(i), "l"(pol) : "memory");
     } else {
-        spos4[s] = make_float4(p[3 * (int64_t)i], p[3 * (int64_t)i + 1], p[3 * (int64_t)i + 2],
-                               __int_as_float(i));
+        const float x = p[3 * (int64_t)i], y = p[3 * (int64_t)i + 1], z = p[3 * (int64_t)i + 2];
+        asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(spos4 + s), "f"(x), "f"(y), "f"(z),
+                     "f"(__int_as_float(i)), "l"(pol) : "memory");   // d = 3: the id travels in the record's fourth word
     }
-    if (D == 2) sidx[s] = i;              // d = 3: the id travels in the record's fourth word
     slot[i] = s;
 }
 
