@@ -556,6 +556,28 @@ __device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
         tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
     }
 }
+// store_cert with the L2 evict_last policy.  The certificates of a slot-ordered sweep go to ids
+// all over the five output arrays, four bytes at a time: a 32-byte sector of an output array is
+// completed by eight writes spread over the whole kernel, and a sector that L2 evicts half-written
+// costs a fill and a second write-back (ncu, 4,194,304 points: 723 MB written for 84 MB of output).
+// The outputs (84 MB) fit the 126 MB L2 if the streamed grid data does not push them out.
+__device__ __forceinline__ void st_keep(void *p, unsigned v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void store_cert_keep(const Top2 &t, int i, int32_t *nn, int32_t *nn2, float *d1,
+                                                float *d2, float *c)
+{
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    const float a = __fsqrt_rn(t.s1), b = __fsqrt_rn(t.s2);
+    st_keep(nn + i, (unsigned)(t.j1 == KC_NOIDX ? -1 : t.j1), pol);
+    if (nn2) st_keep(nn2 + i, (unsigned)(t.j2 == KC_NOIDX ? -1 : t.j2), pol);
+    st_keep(d1 + i, __float_as_uint(a), pol);
+    st_keep(d2 + i, __float_as_uint(b), pol);
+    st_keep(c + i, __float_as_uint(__fsub_rn(b, a)), pol);
+}
+
 // ---- d = 2: the row-segment kernel with cell-wise pruning of dense rows -------------------------
 // In the plane the leaf-tiled kernel below loses to this older one on clustered data (config 5,
 // d = 2: 0.75 vs 0.68 ms): cells of 10-70 records are too small for a second level, and what pays
@@ -717,7 +739,7 @@ search_tiled_kernel(View v, int N, Counters *ctr, int32_t *mark,
     const int r = finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
     if (s >= N) return;
     if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-    store_cert(best, self, nn, nn2, d1, d2, c);
+    store_cert_keep(best, self, nn, nn2, d1, d2, c);
 }
 
 // ---- A3 / A7, leaf-tiled: the kernel behind kc_cert_grid_search and the slot sweep of A7 ---------
@@ -739,28 +761,6 @@ constexpr int WPQ_MAX = 32768;                       // A7: id lists up to this 
 #endif
 constexpr int LT_HULL_MAX = 4096;                 // a longer hull (lanes far apart in memory) is left to phase 2
 static_assert(32 * LT_WARPS == PS_THREADS, "the range queues are strided by PS_THREADS");
-
-// store_cert with the L2 evict_last policy.  The certificates of a slot-ordered sweep go to ids
-// all over the five output arrays, four bytes at a time: a 32-byte sector of an output array is
-// completed by eight writes spread over the whole kernel, and a sector that L2 evicts half-written
-// costs a fill and a second write-back (ncu, 4,194,304 points: 723 MB written for 84 MB of output).
-// The outputs (84 MB) fit the 126 MB L2 if the streamed grid data does not push them out.
-__device__ __forceinline__ void st_keep(void *p, unsigned v, unsigned long long pol)
-{
-    asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(p), "r"(v), "l"(pol) : "memory");
-}
-__device__ __forceinline__ void store_cert_keep(const Top2 &t, int i, int32_t *nn, int32_t *nn2, float *d1,
-                                                float *d2, float *c)
-{
-    unsigned long long pol;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
-    const float a = __fsqrt_rn(t.s1), b = __fsqrt_rn(t.s2);
-    st_keep(nn + i, (unsigned)(t.j1 == KC_NOIDX ? -1 : t.j1), pol);
-    if (nn2) st_keep(nn2 + i, (unsigned)(t.j2 == KC_NOIDX ? -1 : t.j2), pol);
-    st_keep(d1 + i, __float_as_uint(a), pol);
-    st_keep(d2 + i, __float_as_uint(b), pol);
-    st_keep(c + i, __float_as_uint(__fsub_rn(b, a)), pol);
-}
 
 // index (k of phase 1) of the block row at offset (oy, oz): k = 0 own row, k >= 1: row_oy/row_oz(k-1)
 __device__ __forceinline__ int block_row_index(int oy, int oz)

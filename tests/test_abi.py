@@ -110,3 +110,74 @@ def test_product_never_imports_oracle():
     otxt = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "kc_oracle.c")).read()
     assert not re.search(r"^\s*(import|from)\s+paper_2606_18314_b200", otxt, flags=re.M)
     assert '#include "kc' not in otxt and "include/kc.h" not in otxt
+
+
+@pytest.mark.gpu
+def test_full_step_through_raw_ctypes():
+    """One maintenance step (A0, A4, A6+A7, A5, A2+A3, A1) driven through ctypes.CDLL alone --
+    no binding.py, torch only as the owner of device memory -- and checked against the oracle."""
+    import ctypes as C
+
+    import torch
+
+    import oracle
+    from paper_2606_18314_b200 import workloads as wl
+    from paper_2606_18314_b200.binding import LIB_PATH, kc_geom
+
+    lib = C.CDLL(LIB_PATH)
+    lib.kc_cert_allpairs_workspace.restype = C.c_size_t
+    lib.kc_cert_allpairs_workspace.argtypes = [C.c_int64, C.c_int]
+    vp = C.c_void_p
+    p, mot = wl.make_scene("cfg1")
+    q, _ = mot.step(p)
+    N, d = p.shape
+    P, Q = torch.from_numpy(p).cuda(), torch.from_numpy(q).cuda()
+    lo = (C.c_float * 3)(*p.min(0), 0.0)
+    hi = (C.c_float * 3)(*p.max(0), 0.0)
+    geom = kc_geom()
+    lib.kc_geom_from_bbox.argtypes = [C.c_int64, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_double, C.POINTER(kc_geom)]
+    assert lib.kc_geom_from_bbox(N, d, lo, hi, 2.0, C.byref(geom)) == 0
+    grid = vp()
+    lib.kc_grid_create.argtypes = [C.POINTER(vp), C.c_int64, C.POINTER(kc_geom)]
+    assert lib.kc_grid_create(C.byref(grid), N, C.byref(geom)) == 0
+    i32 = lambda n: torch.empty(n, dtype=torch.int32, device="cuda")
+    f32 = lambda n: torch.empty(n, dtype=torch.float32, device="cuda")
+    pre = [i32(N), i32(N), f32(N), f32(N), f32(N)]          # nn, nn2, d1, d2, c
+    post = [i32(N), i32(N), f32(N), f32(N), f32(N)]
+    ap = [i32(N), i32(N), f32(N), f32(N), f32(N)]
+    ptr = lambda t: vp(t.data_ptr())
+    st = vp(torch.cuda.current_stream().cuda_stream)
+    lib.kc_cert_grid_rebuild.argtypes = [vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
+    assert lib.kc_cert_grid_rebuild(grid, ptr(P), N, *map(ptr, pre), st) == 0
+    eps, flags, F, nF = f32(1), torch.empty(N, dtype=torch.uint8, device="cuda"), i32(N), i32(1)
+    lib.kc_max_displacement.argtypes = [vp, vp, C.c_int64, C.c_int, vp, vp]
+    assert lib.kc_max_displacement(ptr(P), ptr(Q), N, d, ptr(eps), st) == 0
+    lib.kc_frontier_classify.argtypes = [vp, C.c_int64, vp, vp, vp, vp, vp]
+    assert lib.kc_frontier_classify(ptr(pre[4]), N, ptr(eps), ptr(flags), ptr(F), ptr(nF), st) == 0
+    lib.kc_frontier_repair.argtypes = [vp, vp, C.c_int64, vp, vp, C.c_int64, vp, vp, C.c_int64, vp, vp, vp, vp, vp, vp]
+    assert lib.kc_frontier_repair(grid, ptr(Q), N, None, None, 0, ptr(F), ptr(nF), N, *map(ptr, pre), st) == 0
+    H = torch.empty(1, dtype=torch.float64, device="cuda")
+    m, Cc = i32(1), i32(1)
+    lib.kc_frontier_entropy.argtypes = [vp, vp, vp, C.c_int64, vp, vp, vp, vp]
+    assert lib.kc_frontier_entropy(grid, ptr(F), ptr(nF), N, ptr(H), ptr(m), ptr(Cc), st) == 0
+    assert lib.kc_cert_grid_rebuild(grid, ptr(Q), N, *map(ptr, post), st) == 0
+    need = lib.kc_cert_allpairs_workspace(N, d)
+    ws = torch.zeros(max(need, 16), dtype=torch.uint8, device="cuda")
+    lib.kc_cert_allpairs.argtypes = [vp, C.c_int64, C.c_int, vp, vp, vp, vp, vp, vp, C.c_size_t, vp]
+    assert lib.kc_cert_allpairs(ptr(Q), N, d, *map(ptr, ap), ptr(ws), ws.numel(), st) == 0
+    torch.cuda.synchronize()
+    want = oracle.bruteforce_top2(q)
+    w_eps = oracle.max_displacement(p, q)
+    wf, wF = oracle.frontier(oracle.bruteforce_top2(p).c, w_eps)
+    assert eps.cpu().numpy().view(np.uint32)[0] == np.array([w_eps], np.float32).view(np.uint32)[0]
+    assert int(nF.item()) == wF.size and np.array_equal(flags.cpu().numpy(), wf)
+    for k, name in enumerate(("nn", "nn2", "d1", "d2", "c")):
+        ref = getattr(want, name).view(np.uint32)
+        assert np.array_equal(post[k].cpu().numpy().view(np.uint32), ref), name
+        assert np.array_equal(ap[k].cpu().numpy().view(np.uint32), ref), name
+        assert np.array_equal(pre[k].cpu().numpy().view(np.uint32)[wF], ref[wF]), name
+    g_or = oracle.geom_for(p)
+    wH, wm, wC = oracle.entropy(oracle.cell_ids(q, g_or), wF, g_or.n_cells)
+    assert abs(float(H.item()) - wH) <= 1e-6 and int(m.item()) == wm and int(Cc.item()) == wC
+    lib.kc_grid_destroy.argtypes = [vp]
+    assert lib.kc_grid_destroy(grid) == 0
