@@ -37,6 +37,12 @@ N_ALLPAIRS = 1 << 20            # config 5: the all-pairs oracle pass runs on th
 # ncu --set full captures (profiles/, file named beside each figure); None where no capture exists
 NCU_TRAFFIC_BYTES = {
     ("cfg2", "allpairs_kernel"): 279552,            # profiles/r1f_allpairs_cfg2_full.txt
+    ("cfg5_d3", "allpairs_kernel"): 164913152,      # profiles/r2_allpairs_1m_cfg5_d3_full.txt (86.5 MB read + 78.4 MB written)
+    ("cfg5_d2", "allpairs_kernel"): 148216832,      # profiles/r2_allpairs_1m_cfg5_d2_full.txt
+    # A2 + A3, summed over the kernels of one kc_cert_grid_rebuild call (cellid_hist, scan_write, leafid_hist,
+    # lscan_write, scatter, search): profiles/r2_grid_cfg5_d3_full.txt / r2_grid_cfg5_d2_full.txt
+    ("cfg5_d3", "rebuild"): 844600000,
+    ("cfg5_d2", "rebuild"): 984300000,
 }
 # algorithmic bytes per point of the O(N) rebuild (A2 + A3) with this layout
 REBUILD_BYTES_PER_POINT = {2: 76.0, 3: 90.0}
@@ -120,6 +126,16 @@ def run_oracle_arm(cfg, K, W, time_budget_s=None, pair_budget=1.5e11):
     value = (N * frac) * done / t_total
     return dict(value=value, steps=done, seconds=t_total, cores=oracle.num_procs(), sample=sample,
                 ms_per_step=1e3 * t_total / max(done, 1))
+
+
+def scale_workload_text(cfg):
+    """config.workload of the headline (the same string in both arms)."""
+    c = wl.CONFIGS[cfg]
+    N, d, n_ap = c["N"], c["d"], min(N_ALLPAIRS, c["N"])
+    return (f"{cfg} (BASELINE.json config 5, Scale): N={N}, d={d}, 50% uniform + 50% from 256 Gaussian clusters "
+            f"(sigma=0.005), random-walk steps eps={c['eps']}, grid occupancy 2; every step = A0, A4, A6+A7 (Lemma-1 "
+            f"frontier), A5, A2+A3 at all {N} points, and the all-pairs oracle pass A1 on the first {n_ap} points of p' "
+            f"({n_ap * (n_ap - 1):.3e} pairs)")
 
 
 def oracle_scale_step(oracle, p, q, pre_c, geom, n_ap, n_bf):
@@ -632,7 +648,8 @@ def run_gpu_arm_scale(args):
         certified = (f"1 transition at N={N}: rebuild (all points), repair (at F), all-pairs ({n_ap} points), eps, |F|, "
                      f"Lemma-1 nn bit-exact vs the CPU k-d tree oracle (+ 64 brute-force queries), H within 1e-6")
         del m3
-        cpu_baseline = dict(value=N / t_cpu, unit=UNIT, cores=oracle.num_procs(), kind="oracle (exact k-d tree, all cores)",
+        cpu_baseline = dict(value=N / t_cpu, unit=UNIT, cores=oracle.num_procs(), kind="oracle",
+                            algorithm="exact k-d tree over all points, all cores (PAPER.md:106, Table 2's 149 ms row)",
                             sample=(f"1 full step at N={N}: max displacement, Lemma-1 frontier, cell ids + entropy, k-d tree "
                                     f"relabel of all points, k-d tree on the first {n_ap} points + 64 brute-force queries"),
                             ms_per_step=1e3 * t_cpu)
@@ -654,7 +671,7 @@ def run_gpu_arm_scale(args):
                         fp32_probe_tops=probe)
         reb_bytes = REBUILD_BYTES_PER_POINT[d] * N
         reb_gbs = reb_bytes / (ms["rebuild"] * 1e-3) / 1e9
-        roofline_rebuild = dict(bound="hbm", kernel="kc_cert_grid_rebuild (A2 + A3: build kernels + search_leaf_kernel)",
+        roofline_rebuild = dict(bound="hbm", kernel=f"kc_cert_grid_rebuild (A2 + A3: build kernels + {'search_leaf_kernel' if d == 3 else 'search_tiled_kernel'})",
                                 achieved=reb_gbs, peak=hbm, unit="GB/s", frac=reb_gbs / hbm,
                                 traffic=NCU_TRAFFIC_BYTES.get((cfg, "rebuild")),
                                 note=(f"{REBUILD_BYTES_PER_POINT[d]:.0f} algorithmic B/point (SURVEY.md §8(d)) x {N} points / "
@@ -671,10 +688,7 @@ def run_gpu_arm_scale(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": (f"{cfg} (BASELINE.json config 5, Scale): N={N}, d={d}, 50% uniform + 50% from 256 Gaussian "
-                                    f"clusters (sigma=0.005), random-walk steps eps={c['eps']}, grid occupancy 2; every step = A0, A4, "
-                                    f"A6+A7 (Lemma-1 frontier, {frontier_frac:.3f} of the points), A5, A2+A3 at all {N} points, and the "
-                                    f"all-pairs oracle pass A1 on the first {n_ap} points of p' ({n_ap * (n_ap - 1):.3e} pairs)"),
+            "config": {"workload": scale_workload_text(cfg),
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
                        "launch": "eager stream launches through the C-ABI (a grid of this size is not launch-bound)",
                        "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
@@ -1054,7 +1068,8 @@ def main():
                 "n_gpus": args.gpus, "steps": r["steps"], "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
                 "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
                 "data": "synthetic",
-                "config": {"workload": f"{args.workload}: N={c['N']}, d={c['d']}, eps={c['eps']} (CPU oracle arm)"},
+                "config": {"workload": scale_workload_text(args.workload) if scale else
+                           f"{args.workload}: N={c['N']}, d={c['d']}, eps={c['eps']} (CPU oracle arm)"},
                 "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                                  "sample": r["sample"]},
                 "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
