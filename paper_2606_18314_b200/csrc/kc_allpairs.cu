@@ -416,27 +416,15 @@ allpairs_redo_kernel(const ApArgs a)
     }
 }
 
-// Launch shape.  Tuning overrides for experiments: KC_AP_QPT, KC_AP_C4, KC_AP_THREADS, KC_AP_JS
-// (read once per process).
+// Launch shape (a function of the sizes only).
 struct Shape { int qpt, c4, threads, js; };
-
-int env_int(const char *name, int dflt)
-{
-    const char *v = getenv(name);
-    return v && *v ? atoi(v) : dflt;
-}
 
 Shape choose_shape(int64_t nq, int64_t N)
 {
-    static const int e_qpt = env_int("KC_AP_QPT", 0), e_thr = env_int("KC_AP_THREADS", 0),
-                     e_js = env_int("KC_AP_JS", 0), e_c4 = env_int("KC_AP_C4", 0);
     Shape s;
     s.qpt = nq >= 148 * 8 * 128 * 2 ? 4 : (nq >= 148 * 4 * 128 ? 2 : 1);
     s.threads = 128;
-    if (e_qpt == 1 || e_qpt == 2 || e_qpt == 4) s.qpt = e_qpt;
     s.c4 = s.qpt == 4 ? 2 : (s.qpt == 2 ? 2 : 4);
-    if (e_c4 == 1 || e_c4 == 2 || e_c4 == 4) s.c4 = e_c4;
-    if (e_thr == 32 || e_thr == 64 || e_thr == 128) s.threads = e_thr;
     // j-split (chunks start from the seed pass or from the caller's bound, so short chunks are
     // fine; granularity AP_GRAN candidates, at least 4 units per chunk).  Few query blocks: as many
     // chunks as make ONE full wave of resident CTAs (a second, partly filled wave of this
@@ -447,7 +435,6 @@ Shape choose_shape(int64_t nq, int64_t N)
     int64_t want = itiles * 2 <= resident ? resident / itiles : (148 * 8 * 8 + itiles - 1) / itiles;
     int64_t cap = (N - AP_SEED) / (4 * AP_GRAN);
     int64_t js = want < cap ? want : cap;
-    if (e_js > 0) js = e_js;
     if (js < 1) js = 1;
     if (js > 65535) js = 65535;
     if (itiles > AP_TICKETS) js = 1;             // the ticket area holds AP_TICKETS query blocks
@@ -470,9 +457,8 @@ size_t workspace_bytes_for(int64_t nq, const Shape &sh)
 template <int D, int QPT, int C4>
 void launch_t(int threads, dim3 grid, cudaStream_t st, const ApArgs &a)
 {
-    if (threads == 32) allpairs_kernel<D, QPT, C4, 32><<<grid, 32, 0, st>>>(a);
-    else if (threads == 64) allpairs_kernel<D, QPT, C4, 64><<<grid, 64, 0, st>>>(a);
-    else allpairs_kernel<D, QPT, C4, 128><<<grid, 128, 0, st>>>(a);
+    (void)threads;
+    allpairs_kernel<D, QPT, C4, 128><<<grid, 128, 0, st>>>(a);
 }
 
 template <int D>
@@ -519,8 +505,7 @@ kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
     if (sh.qpt == Q && sh.c4 == C) {                               \
         launch_t<D, Q, C>(sh.threads, grid, st, a);                \
     } else
-    KC_AP_CASE(4, 1) KC_AP_CASE(4, 2) KC_AP_CASE(2, 1) KC_AP_CASE(2, 2) KC_AP_CASE(2, 4)
-    KC_AP_CASE(1, 1) KC_AP_CASE(1, 2) KC_AP_CASE(1, 4)
+    KC_AP_CASE(4, 2) KC_AP_CASE(2, 2) KC_AP_CASE(1, 4)
     {
         set_error("kc_cert_allpairs: unsupported launch shape");
         return KC_EINVAL;
