@@ -640,7 +640,7 @@ __device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float
 //   idle otherwise; warps without a marked slot leave at once), tombstones are inert records and
 //   the overflow chains of every visited cell are scanned too.  Runs only when *nF * sweep_div >= N
 //   (the list kernel serves smaller frontiers and the frontier points that live in chains).
-template <int D, bool SWEEP>
+template <int D, bool SWEEP, bool FRESH>
 __global__ void __launch_bounds__(32 * WT_WARPS)
 search_tiled_kernel(View v, int N, Counters *ctr, int32_t *mark,
                     const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
@@ -650,7 +650,7 @@ search_tiled_kernel(View v, int N, Counters *ctr, int32_t *mark,
     __shared__ __align__(16) float2 s_p2[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
     __shared__ int s_ix[D == 2 ? WT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
     if (SWEEP && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = SWEEP && ctr->n_misfiled > 0;
+    const bool chains = SWEEP && !FRESH && ctr->n_misfiled > 0;   // FRESH: no incremental update since the build
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float qnan = __int_as_float(0x7fc00000);
     float4 *tp4 = s_p4[D == 3 ? warp : 0];
@@ -892,8 +892,8 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
     __shared__ __align__(16) float2 s_p2[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
     __shared__ int s_ix[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
     __shared__ int2 s_rl[RL_CAP * PS_THREADS];
-    if (MODE == 1 && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = MODE == 1 && ctr->n_misfiled > 0;
+    if (MODE != 0 && (int64_t)*nF * sweep_div < N) return;
+    const bool chains = MODE == 1 && ctr->n_misfiled > 0;     // MODE 2: a fresh grid has no chains (compile-time)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float qnan = __int_as_float(0x7fc00000);
     float4 *tp4 = s_p4[D == 3 ? warp : 0];
@@ -910,7 +910,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
     if (s - lane >= N) return;                     // whole warp past the end
     const int sc = min(s, N - 1);
     bool query = s < N;
-    if (MODE == 1) {
+    if (MODE != 0) {
         query = query && mark[sc] != 0;
         if (query) mark[sc] = 0;                   // the marks are all zero again when the sweep ends
     }
@@ -1405,7 +1405,7 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     View v = make_view(g);
     const int n = (int)g->N;
     const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
-    if (g->geom.d == 2) search_tiled_kernel<2, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
+    if (g->geom.d == 2) search_tiled_kernel<2, false, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     count_launches(1);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
@@ -1490,10 +1490,15 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     if (sweep_div > 0) {
         mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->list2, g->ctr);
         const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
-        if (g->geom.d == 2)
-            search_tiled_kernel<2, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
-        else
-            search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+        // a grid that is fresh (built or re-binned, not updated incrementally) has no tombstones and
+        // no chains: the sweep then is the whole-set kernel with a query mask
+        if (g->geom.d == 2) {
+            if (g->dirty) search_tiled_kernel<2, true, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            else search_tiled_kernel<2, true, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+        } else {
+            if (g->dirty) search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            else search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+        }
         count_launches(2);
     }
     int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
