@@ -319,27 +319,6 @@ allpairs_kernel(const ApArgs a)
     }
 }
 
-__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
-{
-    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
-    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
-    const float ns2 = lt1 ? b.s1 : s;
-    const int nj2 = lt1 ? b.j1 : j;
-    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
-    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
-}
-// smallest key (s, j) over the warp's private lists, removed from the list that held it
-__device__ __forceinline__ void warp_pop(Top2 &tmp, float &s, int &j)
-{
-    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
-    const unsigned m = __reduce_min_sync(0xffffffffu, key);
-    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
-    s = __uint_as_float(m);
-    if (key == m && tmp.j1 == j) {
-        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
-        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
-    }
-}
 // Seed pass: one warp per query at a time, the 32 lanes take different candidates of [0, S) and
 // keep a private top-2 with branch-free selects; two warp reductions pick the two smallest keys.
 template <int D>

@@ -73,6 +73,30 @@ struct Top2 {
     }
 };
 
+// Branch-free (s, j)-ordered insertion (converged code for loops whose lanes all insert).
+__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
+{
+    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
+    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
+    const float ns2 = lt1 ? b.s1 : s;
+    const int nj2 = lt1 ? b.j1 : j;
+    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
+    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
+}
+// Smallest key (s, j) over the warp's private lists, removed from the list that held it (all 32
+// lanes call it; two calls give the two smallest keys of the union).
+__device__ __forceinline__ void warp_pop(Top2 &tmp, float &s, int &j)
+{
+    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
+    const unsigned m = __reduce_min_sync(0xffffffffu, key);
+    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
+    s = __uint_as_float(m);
+    if (key == m && tmp.j1 == j) {
+        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
+        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
+    }
+}
+
 // Definition 1: d1 = sqrtf(s1), d2 = sqrtf(s2), c = d2 - d1.
 __device__ __forceinline__ void store_cert(const Top2 &t, int i, int32_t *nn, int32_t *nn2,
                                            float *d1, float *d2, float *c)
@@ -83,6 +107,37 @@ __device__ __forceinline__ void store_cert(const Top2 &t, int i, int32_t *nn, in
     d1[i] = a;
     d2[i] = b;
     c[i] = __fsub_rn(b, a);
+}
+
+// Block-wide stream compaction shared by the classify kernels (A4 and its clock / local-budget
+// forms): every thread of a 256-thread block brings up to 4 consecutive candidate ids as the bits of
+// `bits` (id = base + k for bit k); the block reserves one range of list[] with a single atomicAdd
+// on *cursor and writes its ids ascending inside it.  Every thread of the block must call it.
+__device__ __forceinline__ void block_append_ids(unsigned bits, int64_t base, int32_t *__restrict__ list, int32_t *cursor)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int cnt = __popc(bits);
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    __shared__ int wsum[8];
+    __shared__ int bbase;
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) { const int t = wsum[w]; wsum[w] = tot; tot += t; }
+        bbase = tot ? atomicAdd(cursor, tot) : 0;
+    }
+    __syncthreads();
+    int pos = bbase + wsum[warp] + incl - cnt;
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+        if (bits & (1u << k)) list[pos++] = (int32_t)(base + k);
 }
 
 // Cell coordinate on one axis (kc_geom comment): clamp(floorf(fl(fl(x - lo) * inv_h)), 0, G-1).

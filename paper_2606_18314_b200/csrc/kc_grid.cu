@@ -680,21 +680,7 @@ classify_local_kernel(View v, float R, int N, const int32_t *__restrict__ cell,
         }
         if (flags) flags[i] = (uint8_t)infr;
     }
-    // compaction: ids ascending inside the block, one atomicAdd per block
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned m = __ballot_sync(0xffffffffu, infr);
-    __shared__ int wsum[8];
-    __shared__ int bbase;
-    if (lane == 0) wsum[warp] = __popc(m);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int tot = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
-        bbase = tot ? atomicAdd(nF, tot) : 0;
-    }
-    __syncthreads();
-    if (infr) F[bbase + wsum[warp] + __popc(m & ((1u << lane) - 1))] = i;
+    block_append_ids(infr ? 1u : 0u, i, F, nF);      // ids ascending inside the block, one atomicAdd per block
 }
 
 __global__ void record_ids_kernel(const float4 *__restrict__ spos4, int n, int32_t *__restrict__ out)

@@ -299,29 +299,7 @@ __global__ void __launch_bounds__(256) classify_kernel(const float *__restrict__
                 if (flags) flags[base + k] = (uint8_t)f;
             }
     }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int cnt = __popc(bits);
-    int incl = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    __shared__ int wsum[8];
-    __shared__ int bbase;
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int tot = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
-        bbase = tot ? atomicAdd(nF, tot) : 0;
-    }
-    __syncthreads();
-    int pos = bbase + wsum[warp] + incl - cnt;
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-        if (bits & (1u << k)) F[pos++] = (int32_t)(base + k);
+    block_append_ids(bits, base, F, nF);
 }
 
 extern "C" kc_status kc_frontier_classify(const float *c, int64_t N, const float *eps,
@@ -367,29 +345,7 @@ __global__ void __launch_bounds__(256) classify_clock_kernel(const float *__rest
             bits |= f << k;
             if (flags) flags[base + k] = (uint8_t)f;
         }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    int cnt = __popc(bits);
-    int incl = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    __shared__ int wsum[8];
-    __shared__ int bbase;
-    if (lane == 31) wsum[warp] = incl;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int tot = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { int t = wsum[w]; wsum[w] = tot; tot += t; }
-        bbase = tot ? atomicAdd(nF, tot) : 0;
-    }
-    __syncthreads();
-    int pos = bbase + wsum[warp] + incl - cnt;
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-        if (bits & (1u << k)) F[pos++] = (int32_t)(base + k);
+    block_append_ids(bits, base, F, nF);
 }
 // stamp[i] = S rounded down, for the ids in F (NULL: all N points)
 __global__ void __launch_bounds__(256) clock_stamp_kernel(const int32_t *__restrict__ F,

@@ -40,16 +40,6 @@ __device__ __forceinline__ void offer_once(Top2 &best, float s, int j, int self)
 {
     if (s <= best.s2 && j >= 0 && j != self && j != best.j1 && j != best.j2) best.offer(s, j);
 }
-// branch-free (s, j)-ordered insertion (converged code for loops whose lanes all insert)
-__device__ __forceinline__ void insert_bf(Top2 &b, float s, int j, bool valid)
-{
-    const bool lt1 = valid && (s < b.s1 || (s == b.s1 && j < b.j1));
-    const bool lt2 = valid && (s < b.s2 || (s == b.s2 && j < b.j2));   // lt1 implies lt2
-    const float ns2 = lt1 ? b.s1 : s;
-    const int nj2 = lt1 ? b.j1 : j;
-    b.s2 = lt2 ? ns2 : b.s2; b.j2 = lt2 ? nj2 : b.j2;
-    b.s1 = lt1 ? s : b.s1; b.j1 = lt1 ? j : b.j1;
-}
 template <int D>
 __device__ __noinline__ Top2 slow_offer4(const View &v, Top2 best, int t, float s0, float s1,
                                          float s2, float s3, int self)
@@ -544,18 +534,6 @@ __device__ __forceinline__ void coop_range(const View &v, int lane, int b, int e
         if (s <= thr && j >= 0 && j != self && j != h1 && j != h2) tmp.offer(s, j);
     }
 }
-// smallest key (s, j) over the warp's partial lists, removed from the list that held it
-__device__ __forceinline__ void coop_pop(Top2 &tmp, float &s, int &j)
-{
-    const unsigned key = __float_as_uint(tmp.s1);              // s >= 0 or +inf: ordered as unsigned
-    const unsigned m = __reduce_min_sync(0xffffffffu, key);
-    j = __reduce_min_sync(0xffffffffu, key == m ? tmp.j1 : KC_NOIDX);
-    s = __uint_as_float(m);
-    if (key == m && tmp.j1 == j) {
-        tmp.s1 = tmp.s2; tmp.j1 = tmp.j2;
-        tmp.s2 = CUDART_INF_F; tmp.j2 = KC_NOIDX;
-    }
-}
 // store_cert with the L2 evict_last policy.  The certificates of a slot-ordered sweep go to ids
 // all over the five output arrays, four bytes at a time: a 32-byte sector of an output array is
 // completed by eight writes spread over the whole kernel, and a sector that L2 evicts half-written
@@ -620,8 +598,8 @@ __device__ __forceinline__ void dense_pass(const View &v, int N, int lane, float
             coop_range<D>(v, lane, Lb2, Le2, Lx, Ly, Lz, Lself, thr, Lj1, Lj2, tmp);
             float sa, sb;
             int ja, jb;
-            coop_pop(tmp, sa, ja);
-            coop_pop(tmp, sb, jb);
+            warp_pop(tmp, sa, ja);
+            warp_pop(tmp, sb, jb);
             if (lane == L) {
                 if (ja != KC_NOIDX) best.offer(sa, ja);
                 if (jb != KC_NOIDX) best.offer(sb, jb);
@@ -1114,8 +1092,8 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
         }
     float sa, sb;
     int ja, jb;
-    coop_pop(tmp, sa, ja);
-    coop_pop(tmp, sb, jb);
+    warp_pop(tmp, sa, ja);
+    warp_pop(tmp, sb, jb);
     best.s1 = sa; best.j1 = ja; best.s2 = sb; best.j2 = jb;         // ordered: sa <= sb (or none)
     const float thr = best.s2;
     // the other cells: prune, then short ranges by their lanes, long ones by the warp
@@ -1157,8 +1135,8 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
             const float4 o = v.opos[c];
             lane_offer<D>(tmp, D == 2 ? sqd2(qx, qy, o.x, o.y) : sqd3(qx, qy, qz, o.x, o.y, o.z), c, thr, self);
         }
-    coop_pop(tmp, sa, ja);
-    coop_pop(tmp, sb, jb);
+    warp_pop(tmp, sa, ja);
+    warp_pop(tmp, sb, jb);
     if (ja != KC_NOIDX) best.offer(sa, ja);
     if (jb != KC_NOIDX) best.offer(sb, jb);
     // every lane holds the same state: the rare ring continuation runs redundantly on all of them
@@ -1249,6 +1227,60 @@ __device__ __forceinline__ void topk_scan_cells(const View &v, int rowbase, int 
     }
 }
 template <int D, int K>
+__device__ __forceinline__ void topk_scan_chains(const View &v, int rowbase, int x0, int x1, float qx, float qy,
+                                                 float qz, int self, TopK<K> &best)
+{
+    for (int x = x0; x <= x1; ++x)
+        for (int e = v.head[rowbase + x]; e >= 0; e = v.next[e]) {
+            const float4 c = v.opos[e];
+            const float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
+            if (s <= best.s[K - 1] && e != self) best.offer(s, e);
+        }
+}
+// K-list ring search of one query: own cell, then Chebyshev rings until the bound of the scanned block
+// exceeds the K-th best squared distance (the same strict test as A3, with s_K in the place of s_2:
+// every unscanned point is then strictly farther than the K-th key); with `chains` the overflow chains
+// of every visited cell are scanned too (incrementally updated grid, tombstones are inert records).
+template <int D, int K>
+__device__ __forceinline__ void topk_visit(const View &v, bool chains, int rowbase, int x0, int x1, float qx, float qy,
+                                           float qz, int self, TopK<K> &best)
+{
+    topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
+    if (chains) topk_scan_chains<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
+}
+template <int D, int K>
+__device__ __forceinline__ void topk_ring_search(const View &v, bool chains, float qx, float qy, float qz, int self,
+                                                 TopK<K> &best)
+{
+    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
+    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
+    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
+    topk_visit<D, K>(v, chains, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
+    for (int r = 0;;) {
+        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
+        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
+        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
+        ++r;
+        // ring r: shell rows get the full segment, inner rows only the two end cells
+        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
+        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
+        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
+        for (int z = z0; z <= z1; ++z)
+            for (int y = y0; y <= y1; ++y) {
+                const int rowbase = (z * v.G1 + y) * v.G0;
+                const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
+                if (shell) {
+                    topk_visit<D, K>(v, chains, rowbase, x0, x1, qx, qy, qz, self, best);
+                } else {
+                    if (cx - r >= 0) topk_visit<D, K>(v, chains, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
+                    if (cx + r <= v.G0 - 1) topk_visit<D, K>(v, chains, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                }
+            }
+    }
+}
+// One thread per sorted slot of a freshly built grid.
+template <int D, int K>
 __global__ void __launch_bounds__(128)
 search_topk_kernel(View v, int N, int32_t *__restrict__ nnk, float *__restrict__ dk, float *__restrict__ ck)
 {
@@ -1263,48 +1295,12 @@ search_topk_kernel(View v, int N, int32_t *__restrict__ nnk, float *__restrict__
         const float4 q = v.spos4[s];
         qx = q.x; qy = q.y; qz = q.z; self = __float_as_int(q.w);
     }
-    const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-    const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-    const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
     TopK<K> best;
     best.init();
-    topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-    for (int r = 0;;) {
-        int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
-        int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-        if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
-        ++r;
-        z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-        y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
-        x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-        for (int z = z0; z <= z1; ++z)
-            for (int y = y0; y <= y1; ++y) {
-                const int rowbase = (z * v.G1 + y) * v.G0;
-                const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
-                if (shell) {
-                    topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                } else {
-                    if (cx - r >= 0) topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                    if (cx + r <= v.G0 - 1) topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                }
-            }
-    }
+    topk_ring_search<D, K>(v, false, qx, qy, qz, self, best);
     best.store(self, nnk, dk, ck);
 }
-// K-list repair (A7 for K keys): one thread per id of the list, against the incrementally updated
-// grid: tombstones are inert records, the overflow chain of every visited cell is scanned too.
-template <int D, int K>
-__device__ __forceinline__ void topk_scan_chains(const View &v, int rowbase, int x0, int x1, float qx, float qy,
-                                                 float qz, int self, TopK<K> &best)
-{
-    for (int x = x0; x <= x1; ++x)
-        for (int e = v.head[rowbase + x]; e >= 0; e = v.next[e]) {
-            const float4 c = v.opos[e];
-            const float s = D == 2 ? sqd2(qx, qy, c.x, c.y) : sqd3(qx, qy, qz, c.x, c.y, c.z);
-            if (s <= best.s[K - 1] && e != self) best.offer(s, e);
-        }
-}
+// K-list repair (A7 for K keys): one thread per id of the list, against the incrementally updated grid.
 template <int D, int K>
 __global__ void __launch_bounds__(128)
 search_topk_list_kernel(View v, const float *__restrict__ p_new, const int32_t *__restrict__ F,
@@ -1317,41 +1313,9 @@ search_topk_list_kernel(View v, const float *__restrict__ p_new, const int32_t *
         const int self = F[f];
         const float qx = p_new[(int64_t)self * D], qy = p_new[(int64_t)self * D + 1];
         const float qz = D == 3 ? p_new[(int64_t)self * D + 2] : 0.f;
-        const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
-        const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
-        const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
         TopK<K> best;
         best.init();
-        topk_scan_cells<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-        if (chains) topk_scan_chains<D, K>(v, (cz * v.G1 + cy) * v.G0, cx, cx, qx, qy, qz, self, best);
-        for (int r = 0;;) {
-            int z0 = D == 3 ? max(cz - r, 0) : 0, z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-            int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
-            int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
-            if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s[K - 1])) break;
-            ++r;
-            z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
-            y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
-            x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-            for (int z = z0; z <= z1; ++z)
-                for (int y = y0; y <= y1; ++y) {
-                    const int rowbase = (z * v.G1 + y) * v.G0;
-                    const bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
-                    if (shell) {
-                        topk_scan_cells<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                        if (chains) topk_scan_chains<D, K>(v, rowbase, x0, x1, qx, qy, qz, self, best);
-                    } else {
-                        if (cx - r >= 0) {
-                            topk_scan_cells<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                        }
-                        if (cx + r <= v.G0 - 1) {
-                            topk_scan_cells<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                            if (chains) topk_scan_chains<D, K>(v, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
-                        }
-                    }
-                }
-        }
+        topk_ring_search<D, K>(v, chains, qx, qy, qz, self, best);
         best.store(self, nnk, dk, ck);
     }
 }
