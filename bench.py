@@ -684,6 +684,7 @@ def run_gpu_arm_scale(args):
         extras = {}
         if not args.no_extras:
             extras = run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=cfg)
+            extras["mover_sweep_" + cfg] = mover_sweep_scale(kc, Maintainer, crossover_fraction, torch, dev, cfg, flush)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -840,6 +841,40 @@ def family_table(kc, Maintainer, torch, dev, cfg, flush, steps=8):
         rows[fam] = row
         del m
     return rows
+
+
+def mover_sweep_scale(kc, Maintainer, crossover_fraction, torch, dev, cfg, flush,
+                      fractions=(0.001, 0.01, 0.03, 0.1, 0.3, 1.0)):
+    """Config 5's points with config 4's protocol: a fraction f of the 4,194,304 points (scattered)
+    moves by exactly eps; the mover list is the controlled frontier (reading R12).  Repair = A0 + A4 +
+    A6 + A7 at the movers against the rebuild A2 + A3, and the crossover f* (Prop. 1)."""
+    c = wl.CONFIGS[cfg]
+    N, d = c["N"], c["d"]
+    p = wl.make_points(cfg)
+    P = torch.from_numpy(p).to(dev)
+    m = Maintainer(P, allpairs=False)
+    certs = m.certs.clone()
+    eps = torch.zeros(1, device=dev)
+    H = torch.zeros(1, dtype=torch.float64, device=dev)
+    rows = []
+    for f in fractions:
+        mot = wl.Motion("fraction", d, c["eps"], c["seed"] * 1000 + int(f * 1e6), fraction=f, ball=False)
+        q, movers = mot.step(p)
+        Q, MV = torch.from_numpy(q).to(dev), torch.from_numpy(movers).to(dev)
+        nMV = torch.tensor([movers.size], dtype=torch.int32, device=dev)
+
+        def repair():
+            kc.kc_max_displacement(P, Q, eps)
+            kc.kc_frontier_classify(certs.c, eps, m.flags, m.F, m.nF)
+            kc.kc_frontier_repair(m.grid, Q, MV, nMV, certs, movers=MV, n_movers=nMV)
+
+        t_rep = _median_ms(torch, repair, 3, setup=lambda: kc.kc_grid_build(m.grid, P), flush=flush)
+        kc.kc_frontier_entropy(m.grid, MV, nMV, out=(H, m.m, m.C))
+        t_reb = _median_ms(torch, lambda: kc.kc_cert_grid_rebuild(m.grid, Q, m.other), 3, flush=flush)
+        rows.append(dict(f=f, movers=int(movers.size), repair_ms=t_rep, rebuild_ms=t_reb, H=float(H.item())))
+        del Q, MV
+    fs = [r["f"] for r in rows]
+    return dict(rows=rows, crossover_f=crossover_fraction(fs, [r["repair_ms"] for r in rows], [r["rebuild_ms"] for r in rows]))
 
 
 def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=None):
