@@ -182,10 +182,14 @@ kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ);
  * counting sort in two levels: the records of a subdivided cell are sorted by sub-cell).
  * After it the grid is resident at positions p (copied; p may be freed afterwards). */
 kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream);
-/* A3: certificates of all N points of a freshly built grid by the ring-expanding search
- * (3^d block first, then wider Chebyshev rings; a query stops only when the distance to the
- * nearest unscanned cell face, shrunk by a rounding slack, exceeds d2 — Corollary 1,
- * PAPER.md:171-173; never a search cap).  KC_EREBUILD if the grid is not freshly built. */
+/* A3: certificates of all N points of a freshly built grid by an exact, unbounded search of the
+ * grid (Corollary 1: the block is widened until the second neighbour is
+ * provably enclosed; never a search cap).  The 3^d block of the query's leaf first (its sub-cell's
+ * block inside a subdivided cell); then d = 3: every cell of the index box
+ * [cell(q - r), cell(q + r)] per axis, r >= d2 rounded outwards (the filing function is monotone,
+ * so nothing within r can lie outside that box); d = 2 and the fallback of d = 3: wider Chebyshev
+ * rings until the distance to the nearest unscanned cell face, shrunk by a rounding slack,
+ * exceeds d2, strictly.  KC_EREBUILD if the grid is not freshly built. */
 kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
                               void *stream);
 /* A2 + A3 in one call: the O(N) rebuild strategy. */

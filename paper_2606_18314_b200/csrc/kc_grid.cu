@@ -190,28 +190,51 @@ scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int he
                   int2 *__restrict__ subinfo, int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start,
                   const Counters *ctr, int N)
 {
-    // thread t owns 8 consecutive cells
+    // thread t owns 8 consecutive cells of the block's chunk; the chunk goes through shared memory both
+    // ways so that the global loads and stores are coalesced
     __shared__ int2 wsum[32];
+    __shared__ int s_cnt[SCAN_CHUNK];              // counts in, starts out
+    __shared__ int2 s_sub[SCAN_CHUNK];
     const bool any_heavy = ctr->n_heavy > 0;
-    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
+    const int cbase = blockIdx.x * SCAN_CHUNK;
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        const int c = cbase + k * 256 + threadIdx.x;
+        s_cnt[k * 256 + threadIdx.x] = c < n_cells ? counts[c] : 0;
+    }
+    __syncthreads();
+    const int lbase = threadIdx.x * 8, base = cbase + lbase;
     int v[8], S[8];
     int tsum = 0, tl = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        v[k] = base + k < n_cells ? counts[base + k] : 0;
+        v[k] = s_cnt[lbase + k];
         S[k] = sub_res(v[k], d, heavy_T, sub_occ);
         tsum += v[k];
         tl += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
     }
-    const int2 e = block_excl_scan2(tsum, tl, wsum);
+    const int2 e = block_excl_scan2(tsum, tl, wsum);      // (syncs: every thread has read its counts)
     const int2 off = blocksums[blockIdx.x];
     int run = off.x + e.x, lrun = off.y + e.y;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        if (base + k < n_cells)
-            scan_emit(base + k, v[k], S[k], run, lrun, any_heavy, cell_start, subinfo, leaf_cnt, leaf_start);
+        s_cnt[lbase + k] = run;
+        s_sub[lbase + k] = make_int2(S[k], lrun);
+        // an undivided cell of a grid with subdivided cells is one leaf of that size
+        if (any_heavy && !S[k] && base + k < n_cells) leaf_cnt[lrun] = v[k];
         run += v[k];
         lrun += S[k] ? ipow_d(S[k], d) : 1;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        const int c = cbase + k * 256 + threadIdx.x;
+        if (c < n_cells) {
+            const int st = s_cnt[k * 256 + threadIdx.x];
+            cell_start[c] = st;
+            if (any_heavy) subinfo[c] = s_sub[k * 256 + threadIdx.x];
+            else leaf_start[c + 1] = st;           // leaf = cell: the scatter's cursor straight away
+        }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         cell_start[n_cells] = N;
