@@ -372,22 +372,36 @@ lscan_write_kernel(const int32_t *__restrict__ leaf_cnt, const int2 *__restrict_
 {
     if (ctr->n_heavy == 0) return;
     __shared__ int2 wsum[32];
+    __shared__ int s_cnt[SCAN_CHUNK];              // sizes in, starts out (coalesced both ways)
     const int n = ctr->n_leaves;
-    const int base = blockIdx.x * SCAN_CHUNK + threadIdx.x * 8;
-    if (blockIdx.x * SCAN_CHUNK >= n) return;
+    const int cbase = blockIdx.x * SCAN_CHUNK;
+    if (cbase >= n) return;
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        const int l = cbase + k * 256 + threadIdx.x;
+        s_cnt[k * 256 + threadIdx.x] = l < n ? leaf_cnt[l] : 0;
+    }
+    __syncthreads();
+    const int lbase = threadIdx.x * 8;
     int v[8];
     int tsum = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        v[k] = base + k < n ? leaf_cnt[base + k] : 0;
+        v[k] = s_cnt[lbase + k];
         tsum += v[k];
     }
     const int2 e = block_excl_scan2(tsum, 0, wsum);
     int run = blocksums[blockIdx.x].x + e.x;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-        if (base + k < n) leaf_start[base + k + 1] = run;
+        s_cnt[lbase + k] = run;
         run += v[k];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
+        const int l = cbase + k * 256 + threadIdx.x;
+        if (l < n) leaf_start[l + 1] = s_cnt[k * 256 + threadIdx.x];
     }
 }
 // the same in one CTA, any length (small problems: one launch instead of three)
