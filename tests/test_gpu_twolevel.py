@@ -154,3 +154,53 @@ def test_index_parameters_never_change_a_result(cfg):
         assert_same(certs, want, what=f"{cfg} index={index}")
         kc.kc_frontier_repair(grid, dev(q2), dev(F), dev(np.array([F.size], np.int32)), certs, movers=dev(movers))
         assert_same(certs, post2, idx=F, what=f"{cfg} index={index} repair")
+
+
+def test_set_index_arguments():
+    p = wl.uniform_points(1000, 3, 1)
+    grid = kc.Grid(1000, geoms(p)[1])
+    for bad in [(0, 4), (16, 0), (16, 65), (-3, 2)]:
+        with pytest.raises(kc.KcError) as e:
+            grid.set_index(*bad)
+        assert e.value.status == kc.KC_EINVAL
+    grid.set_index(1, 1)                       # raised to sub_occ * 2^(d+1)
+    kc.kc_grid_build(grid, dev(p))
+    assert grid.info().heavy_T == 16
+    grid.set_index(5, 4)
+    with pytest.raises(kc.RebuildRequired):    # takes effect with the next build: not built until then
+        kc.kc_cert_grid_search(grid, kc.Certs.empty(1000))
+
+
+@pytest.mark.parametrize("d", [2, 3])
+@pytest.mark.parametrize("N", [2, 3, 5, 17, 33, 64, 129])
+def test_tiny_sets_in_one_subdivided_cell(d, N):
+    """Few points, one level-0 cell, second level forced on: short lists (N = 2: d2 = +inf), duplicates,
+    empty sub-cells, windows clipped on every side."""
+    rng = np.random.default_rng(100 * d + N)
+    p = (0.25 + 0.01 * rng.random((N, d))).astype(np.float32)
+    if N >= 5:
+        p[3] = p[1]                                         # a coincident pair
+    g_or, g_kc = geoms(p, lo=np.zeros(d, np.float32), hi=np.ones(d, np.float32), occ=float(N))
+    assert g_kc.n_cells == 1
+    grid = kc.Grid(N, g_kc)
+    grid.set_index(1, 1)
+    assert_same(kc.kc_cert_grid_rebuild(grid, dev(p)), oracle.bruteforce_top2(p), what=f"tiny d={d} N={N}")
+
+
+@pytest.mark.parametrize("offset", [0.0, 4096.5, -3.0e5])
+def test_dense_cells_far_from_origin_and_outside_the_box(offset):
+    """The ball's index box (R22) rests on the monotonicity of the filing functions only:
+    dense blobs far from the origin (coarse float spacing, many exact ties and duplicates after the
+    cast) and a geometry fitted to the central part of the points (the rest is clamped into boundary
+    cells and boundary sub-cells)."""
+    p = blob_scene(30000, 3, 71, 3, 2e-3).astype(np.float64) + offset
+    p = p.astype(np.float32)
+    want = ref_certs(p)
+    lo, hi = p.min(0), p.max(0)
+    for shrink in (0.0, 0.3):
+        g_or, g_kc = geoms(p, lo=lo + shrink * (hi - lo), hi=hi - shrink * (hi - lo))
+        for index in [None, (16, 1), (64, 4)]:
+            grid = kc.Grid(p.shape[0], g_kc)
+            if index is not None:
+                grid.set_index(*index)
+            assert_same(kc.kc_cert_grid_rebuild(grid, dev(p)), want, what=f"offset {offset} shrink {shrink} index {index}")
