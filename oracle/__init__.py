@@ -243,6 +243,40 @@ def geom_for(p, occ=2.0) -> Geom:
     return geom_from_bbox(p.shape[0], p.shape[1], lo, hi, occ)
 
 
+def geom_by_median_density(p, occ=2.0) -> Geom:
+    """Reading R24 of PAPER.md:27 ("the resolution is set so that the mean cell occupancy is a small
+    constant") for point sets whose density is far from uniform: the occupancy is measured against
+    the MEDIAN density of the occupied volume instead of the mean one, so that points packed into
+    clusters of negligible volume do not shrink the cells of everything else.  Step by step:
+      1. R = the largest integer with R^d * 64 <= N, at most 32 (d = 3) / 256 (d = 2); R < 2: no
+         estimate, the result is geom_for(p, occ);
+      2. a coarse grid of R cells per axis over the bounding box (geom_from_bbox(R^d, ..., occ = 1))
+         and the number of points in each of its cells (the cell ids of O5);
+      3. med = the lower median of the counts of the occupied coarse cells; n_eff = med * R^d is
+         the size a uniform set of that density would have;
+      4. k = log2(N / n_eff) rounded to the nearest integer and clamped to 0 .. 2 (decided in
+         integers: k grows while 2 * (n_eff * 2^k)^2 < N^2);
+      5. the result is geom_from_bbox(ceil(N / 2^k), d, lo, hi, occ): the cells of a set 2^k times
+         smaller.  A uniform set gives k = 0, i.e. exactly geom_for(p, occ)."""
+    p = _f32(p)
+    N, d = p.shape
+    lo, hi = bbox(p)
+    r_max = 32 if d == 3 else 256
+    R = 1
+    while R + 1 <= r_max and (R + 1) ** d * 64 <= N:
+        R += 1
+    k = 0
+    if R >= 2:
+        gc = geom_from_bbox(R ** d, d, lo, hi, 1.0)
+        counts = np.bincount(cell_ids(p, gc), minlength=gc.n_cells)
+        occupied = np.sort(counts[counts > 0])
+        med = int(occupied[(occupied.size - 1) // 2])
+        n_eff = med * R ** d
+        while k < 2 and 2 * (n_eff * 2 ** k) ** 2 < N * N:
+            k += 1
+    return geom_from_bbox(-(-N // 2 ** k), d, lo, hi, occ)
+
+
 def cell_ids(p, g: Geom) -> np.ndarray:
     """O5: index cell of every point."""
     p = _f32(p, g.d)

@@ -243,6 +243,51 @@ def test_geometry_rule():
         assert float(g.inv_h) == float(np.float32(1.0 / float(g.h)))
 
 
+def _heap_scene(d, R, m, N, seed=0):
+    """N points in [0,1]^d whose coarse R^d histogram is known: m points inside every coarse cell (well
+    away from its faces), the remaining N - m R^d in one cell; the two box corners are among them."""
+    rng = np.random.default_rng(seed)
+    cells = np.stack(np.meshgrid(*[np.arange(R)] * d, indexing="ij"), -1).reshape(-1, d)
+    base = (np.repeat(cells, m, axis=0) + rng.uniform(0.2, 0.8, (cells.shape[0] * m, d))) / R
+    heap = (np.full((N - base.shape[0], d), R // 2) + rng.uniform(0.2, 0.8, (N - base.shape[0], d))) / R
+    p = np.concatenate([base, heap]).astype(np.float32)
+    p[0] = 0.0                                                    # cell (0,..,0) keeps its m points
+    p[base.shape[0] - 1] = 1.0                                    # so does cell (R-1,..,R-1)
+    return p[rng.permutation(N)]
+
+
+@pytest.mark.parametrize("d,R,G_of_k", [(2, 8, {0: 46, 1: 32, 2: 23}), (3, 4, {0: 13, 1: 11, 2: 8})])
+def test_geometry_by_median_density_hand_worked(d, R, G_of_k):
+    # Reading R24.  N = 4096 = 64 R^d, so the coarse grid has R cells per axis; with m points in every
+    # coarse cell and the rest heaped into one, the lower median of the occupied counts is m and
+    # N / n_eff = 64 / m.  k = that ratio's log2 rounded to the nearest integer, clamped to 0..2 (the
+    # boundaries are sqrt(2) = 1.414 and 2 sqrt(2) = 2.828), and the grid is the occupancy-2 grid of
+    # ceil(N / 2^k) points: G = smallest integer with G^d >= 2048 / 1024 / 512, written out by hand.
+    N = 4096
+    for m, k in [(64, 0), (49, 0), (46, 0), (45, 1), (32, 1), (23, 1), (22, 2), (16, 2), (4, 2)]:
+        g = oracle.geom_by_median_density(_heap_scene(d, R, m, N), 2.0)
+        G = G_of_k[k]
+        assert g.G == (G, G, G if d == 3 else 1), (m, k, g.G)
+        assert float(g.h) == float(np.float32(1.0 / G * (1 + 2.0 ** -20)))
+        assert g.lo[:d] == (np.float32(0),) * d
+
+
+def test_geometry_by_median_density_limits():
+    # a uniform set: exactly the mean-occupancy geometry (k = 0)
+    for N, d in [(1000, 2), (16000, 2), (16000, 3), (262144, 3)]:
+        p = wl.uniform_points(N, d, 3)
+        assert oracle.geom_by_median_density(p) == oracle.geom_for(p)
+    # too few points for an estimate (R < 2): the mean-occupancy geometry, whatever the set looks like
+    p = _heap_scene(2, 2, 1, 255)
+    assert oracle.geom_by_median_density(p) == oracle.geom_for(p)
+    # config 5's mixture (half of the points in 256 clusters of negligible volume): the background has
+    # half the mean density, the cells are those of a set half the size
+    for d in (2, 3):
+        p = wl.mixture_points(262144, d, 5)
+        lo, hi = oracle.bbox(p)
+        assert oracle.geom_by_median_density(p) == oracle.geom_from_bbox(131072, d, lo, hi, 2.0)
+
+
 def test_cell_ids_closed_form():
     # dyadic geometry: lo = 0, h = 1/8 exactly, G = 8 -> cell of x is floor(8x), faces go up
     g = oracle.Geom(2, (8, 8, 1), (np.float32(0), np.float32(0), np.float32(0)), np.float32(0.125), np.float32(8))
