@@ -133,7 +133,7 @@ def scale_workload_text(cfg):
     c = wl.CONFIGS[cfg]
     N, d, n_ap = c["N"], c["d"], min(N_ALLPAIRS, c["N"])
     return (f"{cfg} (BASELINE.json config 5, Scale): N={N}, d={d}, 50% uniform + 50% from 256 Gaussian clusters "
-            f"(sigma=0.005), random-walk steps eps={c['eps']}, grid occupancy 2; every step = A0, A4, A6+A7 (Lemma-1 "
+            f"(sigma=0.005), random-walk steps eps={c['eps']}, grid occupancy 2 against the median density (DESIGN.md R24); every step = A0, A4, A6+A7 (Lemma-1 "
             f"frontier), A5, A2+A3 at all {N} points, and the all-pairs oracle pass A1 on the first {n_ap} points of p' "
             f"({n_ap * (n_ap - 1):.3e} pairs)")
 
@@ -163,7 +163,7 @@ def run_oracle_scale(cfg, K, W, time_budget_s=150.0):
     c = wl.CONFIGS[cfg]
     N = c["N"]
     p, mot = wl.make_scene(cfg)
-    geom = oracle.geom_for(p)
+    geom = oracle.geom_by_median_density(p)
     pre = oracle.kdtree_top2(p)
     done, t_total = 0, 0.0
     for t in range(min(W, 1) + K):
@@ -526,7 +526,8 @@ def run_gpu_arm_scale(args):
         torch.cuda.synchronize()
 
     dev_traj = [torch.from_numpy(p).to(dev) for p in host]         # resident before the timed region
-    m = Maintainer(dev_traj[0], allpairs=False)
+    geom = kc.kc_geom_by_median_density(dev_traj[0])               # reading R24 (both arms)
+    m = Maintainer(dev_traj[0], geom=geom, allpairs=False)
     ap = kc.Certs.empty(n_ap, dev)
     ws = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
 
@@ -577,7 +578,7 @@ def run_gpu_arm_scale(args):
 
     # ---- end to end through the public API: pinned host inputs, H2D + step + D2H per step ----
     pinned = [torch.from_numpy(p).pin_memory() for p in host[: K + 1]]
-    m2 = Maintainer(dev_traj[0], allpairs=False)
+    m2 = Maintainer(dev_traj[0], geom=geom, allpairs=False)
     n_pad = m2.certs.buf.shape[1]
     host_certs = torch.empty((5, n_pad), dtype=torch.int32).pin_memory()     # nn, d1, d2, c, nn2 of all N points
     host_scal = torch.empty(24, dtype=torch.uint8).pin_memory()
@@ -618,12 +619,12 @@ def run_gpu_arm_scale(args):
         # ---- certified: the first transition recomputed by the CPU oracle (k-d tree at this size,
         # itself validated bitwise against brute force; brute-force definition on sampled queries);
         # the oracle's wall time for that step is the cpu_baseline (the oracle as it stands)
-        g_or = oracle.geom_for(host[0])
+        g_or = oracle.geom_by_median_density(host[0])
         pre = oracle.kdtree_top2(host[0])
         t0 = time.perf_counter()
         w = oracle_scale_step(oracle, host[0], host[1], pre.c, g_or, n_ap, 64)
         t_cpu = time.perf_counter() - t0
-        m3 = Maintainer(dev_traj[0], allpairs=False)
+        m3 = Maintainer(dev_traj[0], geom=geom, allpairs=False)
         u32 = lambda a: np.ascontiguousarray(a).view(np.uint32)
         ok = all(np.array_equal(u32(getattr(m3.certs, f).cpu().numpy()), u32(getattr(pre, f)))
                  for f in ("nn", "nn2", "d1", "d2", "c"))
@@ -852,7 +853,7 @@ def mover_sweep_scale(kc, Maintainer, crossover_fraction, torch, dev, cfg, flush
     N, d = c["N"], c["d"]
     p = wl.make_points(cfg)
     P = torch.from_numpy(p).to(dev)
-    m = Maintainer(P, allpairs=False)
+    m = Maintainer(P, geom=kc.kc_geom_by_median_density(P), allpairs=False)
     certs = m.certs.clone()
     eps = torch.zeros(1, device=dev)
     H = torch.zeros(1, dtype=torch.float64, device=dev)
@@ -1030,7 +1031,7 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=N
         p, mot = wl.make_scene(cfg)
         q, _ = mot.step(p)
         P, Q = torch.from_numpy(p).to(dev), torch.from_numpy(q).to(dev)
-        m = Maintainer(P, allpairs=False)
+        m = Maintainer(P, geom=kc.kc_geom_by_median_density(P), allpairs=False)
         t_build = _median_ms(torch, lambda: kc.kc_grid_build(m.grid, Q), 5, flush=flush)
         t_reb = _median_ms(torch, lambda: kc.kc_cert_grid_rebuild(m.grid, Q, m.other), 5, flush=flush)
         info = m.grid.info()

@@ -99,6 +99,20 @@ kc_status kc_geom_from_bbox(int64_t N, int d, const float *lo, const float *hi, 
  * unused axes 0).  For callers that refit the geometry to moved points. */
 kc_status kc_bbox(const float *p, int64_t N, int d, float *lo_hi, void *stream);
 
+/* p: device.  Geometry for point sets whose density is far from uniform (reading R24 of
+ * PAPER.md:27, "the resolution is set so that the mean cell occupancy is a small constant"): the
+ * occupancy is measured against the MEDIAN density of the occupied volume, so that points packed into
+ * clusters of negligible volume do not shrink the cells of everything else.  R = the largest integer
+ * with R^d * 64 <= N (at most 32 for d = 3, 256 for d = 2); the points are counted in the R^d cells of
+ * kc_geom_from_bbox(R^d, d, lo, hi, 1.0) over their bounding box (kc_bbox); med = the lower median of
+ * the non-zero counts, n_eff = med * R^d; k = log2(N / n_eff) rounded to the nearest integer and
+ * clamped to 0..2 (k grows while 2 (n_eff 2^k)^2 < N^2, in integers); *out = kc_geom_from_bbox(
+ * ceil(N / 2^k), d, lo, hi, occ).  A uniform set, or R < 2, gives k = 0: exactly the geometry of
+ * kc_geom_from_bbox on the bounding box.  A setup call: it allocates and frees its own scratch
+ * (R^d ints), launches 4 kernels on `stream` and SYNCHRONISES it twice; not capturable. */
+kc_status kc_geom_by_median_density(const float *p, int64_t N, int d, double occ, void *stream,
+                                    kc_geom *out);
+
 /* ---- A0: Algorithm 1 line 1, eps_t = max_i ||p'_i - p_i|| ----------------- */
 /* eps_out: device float[1].  Each norm is sqrtf of the squared distance defined above. */
 kc_status kc_max_displacement(const float *p, const float *p2, int64_t N, int d, float *eps_out,

@@ -20,7 +20,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libkc.so")
 
 EXPORTS = (
-    "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_max_displacement",
+    "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_geom_by_median_density",
+    "kc_max_displacement",
     "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded", "kc_cert_allpairs_seeded",
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_set_index", "kc_grid_build",
@@ -75,6 +76,7 @@ def lib():
     L.kc_geom_from_bbox.argtypes = [i64, ci, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_double,
                                     C.POINTER(kc_geom)]
     L.kc_bbox.argtypes = [vp, i64, ci, vp, vp]
+    L.kc_geom_by_median_density.argtypes = [vp, i64, ci, C.c_double, vp, C.POINTER(kc_geom)]
     L.kc_max_displacement.argtypes = [vp, vp, i64, ci, vp, vp]
     L.kc_cert_allpairs_workspace.restype = sz
     L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
@@ -206,6 +208,16 @@ def kc_geom_for(p, occ=2.0) -> kc_geom:
     """Convenience: device bbox (one sync) then kc_geom_from_bbox."""
     b = kc_bbox(p).cpu().numpy()
     return kc_geom_from_bbox(p.shape[0], p.shape[1], b[:3], b[3:], occ)
+
+
+def kc_geom_by_median_density(p, occ=2.0) -> kc_geom:
+    """Geometry of reading R24: the occupancy is measured against the median density of
+    the occupied volume (a uniform set gives the geometry of kc_geom_for).  A setup call: it syncs."""
+    pp, N, d = _pos(p)
+    g = kc_geom()
+    _check(lib().kc_geom_by_median_density(pp, N, d, float(occ), _stream(), C.byref(g)),
+           "kc_geom_by_median_density")
+    return g
 
 
 def kc_max_displacement(p, p2, eps_out=None):

@@ -1,9 +1,11 @@
 // kc_misc.cu — host utilities, A0 max displacement, A4 frontier classify + compaction, bbox,
 // FP32 probe.  See include/kc.h for the contract of each entry point.
+#include <algorithm>
 #include <atomic>
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 
 #include "kc_common.cuh"
 
@@ -175,6 +177,79 @@ extern "C" kc_status kc_bbox(const float *p, int64_t N, int d, float *lo_hi, voi
     count_launches(3);
     KC_LAUNCH_CHECK("kc_bbox");
     return KC_OK;
+}
+
+// ------------------------------------------------------------------ geometry from the median density (R24)
+template <int D>
+__global__ void __launch_bounds__(256) coarse_hist_kernel(const float *__restrict__ p, int64_t N, kc_geom g,
+                                                          int *counts)
+{
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < N;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int kx = cell_axis(p[i * D], g.lo[0], g.inv_h, g.G[0]);
+        const int ky = cell_axis(p[i * D + 1], g.lo[1], g.inv_h, g.G[1]);
+        const int kz = D == 3 ? cell_axis(p[i * D + 2], g.lo[2], g.inv_h, g.G[2]) : 0;
+        atomicAdd(counts + (kz * g.G[1] + ky) * g.G[0] + kx, 1);
+    }
+}
+
+extern "C" kc_status kc_geom_by_median_density(const float *p, int64_t N, int d, double occ, void *stream,
+                                               kc_geom *out)
+{
+    if (!p || !out || N < 1 || (d != 2 && d != 3) || !(occ > 0.0)) {
+        set_error("kc_geom_by_median_density: bad argument");
+        return KC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int r_max = d == 3 ? 32 : 256;
+    int64_t R = 1;
+    while (R + 1 <= r_max && (R + 1) * (R + 1) * (d == 3 ? R + 1 : 1) * 64 <= N) ++R;
+    const int64_t Cc = R * R * (d == 3 ? R : 1);
+    // scratch of this call: 6 floats (bounding box) + the coarse histogram
+    char *scratch = nullptr;
+    cudaError_t e = cudaMalloc((void **)&scratch, 32 + (size_t)Cc * sizeof(int));
+    if (e != cudaSuccess) return cuda_fail(e, "kc_geom_by_median_density: scratch");
+    float *lo_hi = reinterpret_cast<float *>(scratch);
+    int *counts = reinterpret_cast<int *>(scratch + 32);
+    float box[6];
+    kc_status rc = kc_bbox(p, N, d, lo_hi, stream);
+    if (rc == KC_OK) {
+        e = cudaMemcpyAsync(box, lo_hi, sizeof(box), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = cuda_fail(e, "kc_geom_by_median_density: bounding box");
+    }
+    int k = 0;
+    if (rc == KC_OK && R >= 2) {
+        kc_geom gc;
+        rc = kc_geom_from_bbox(Cc, d, box, box + 3, 1.0, &gc);
+        int *h_counts = rc == KC_OK ? (int *)malloc((size_t)Cc * sizeof(int)) : nullptr;
+        if (rc == KC_OK && !h_counts) { set_error("kc_geom_by_median_density: out of host memory"); rc = KC_EINVAL; }
+        if (rc == KC_OK) {
+            e = cudaMemsetAsync(counts, 0, (size_t)Cc * sizeof(int), st);
+            const int blocks = (int)((N + 255) / 256 < 148 * 8 ? (N + 255) / 256 : 148 * 8);
+            if (d == 2) coarse_hist_kernel<2><<<blocks, 256, 0, st>>>(p, N, gc, counts);
+            else coarse_hist_kernel<3><<<blocks, 256, 0, st>>>(p, N, gc, counts);
+            count_launches(1);
+            if (e == cudaSuccess) e = cudaGetLastError();
+            if (e == cudaSuccess) e = cudaMemcpyAsync(h_counts, counts, (size_t)Cc * sizeof(int), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) rc = cuda_fail(e, "kc_geom_by_median_density: coarse histogram");
+        }
+        if (rc == KC_OK) {
+            // lower median of the occupied coarse cells' counts
+            int64_t m = 0;
+            for (int64_t c = 0; c < Cc; ++c)
+                if (h_counts[c] > 0) h_counts[m++] = h_counts[c];
+            std::nth_element(h_counts, h_counts + (m - 1) / 2, h_counts + m);
+            const unsigned __int128 n_eff = (unsigned __int128)h_counts[(m - 1) / 2] * (unsigned __int128)Cc;
+            const unsigned __int128 NN = (unsigned __int128)N * (unsigned __int128)N;
+            while (k < 2 && 2 * ((n_eff << k) * (n_eff << k)) < NN) ++k;   // log2(N / n_eff) to the nearest integer
+        }
+        free(h_counts);
+    }
+    cudaFree(scratch);
+    if (rc != KC_OK) return rc;
+    return kc_geom_from_bbox((N + ((int64_t)1 << k) - 1) >> k, d, box, box + 3, occ, out);
 }
 
 // ------------------------------------------------------------------ A0 max displacement

@@ -21,14 +21,23 @@ def sampled_bruteforce_check(p, got, n_samples, seed, what):
     assert_same(got, want, idx=q, what=what + " (sampled brute force)")
 
 
+@pytest.mark.parametrize("density", ["median", "mean"])
 @pytest.mark.parametrize("cfg", ["cfg5_d2", "cfg5_d3"])
-def test_config5_rebuild_and_repair_4m(cfg):
+def test_config5_rebuild_and_repair_4m(cfg, density):
+    """density = "median": the geometry bench.py times (reading R24), computed by each side on its own;
+    "mean": the plain occupancy-2 grid of the bounding box."""
     c = wl.CONFIGS[cfg]
     p, mot = wl.make_scene(cfg)
     N = c["N"]
-    g_or, g_kc = geoms(p)
-    grid = kc.Grid(N, g_kc)
     P = dev(p)
+    if density == "median":
+        g_or, g_kc = oracle.geom_by_median_density(p), kc.kc_geom_by_median_density(P)
+        assert tuple(g_or.G) == tuple(g_kc.G) and g_or.h == np.float32(g_kc.h) and g_or.inv_h == np.float32(g_kc.inv_h)
+        assert list(g_or.lo) == [np.float32(g_kc.lo[k]) for k in range(3)]
+        assert g_kc.G[0] < geoms(p)[1].G[0]
+    else:
+        g_or, g_kc = geoms(p)
+    grid = kc.Grid(N, g_kc)
     certs = kc.kc_cert_grid_rebuild(grid, P)
     got = host(certs)
     want = oracle.kdtree_top2(p)

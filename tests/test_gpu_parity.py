@@ -729,3 +729,40 @@ def test_sweep_path_replays_from_a_cuda_graph():
         assert_same(work, post, idx=wF, what=f"replay {rnd}")
         rest = np.flatnonzero(wf == 0)
         assert np.array_equal(host(work).nn[rest], post.nn[rest])
+
+
+def _same_geom(g_or, g_kc):
+    assert g_or.d == g_kc.d and tuple(g_or.G) == (g_kc.G[0], g_kc.G[1], g_kc.G[2])
+    assert g_or.h == np.float32(g_kc.h) and g_or.inv_h == np.float32(g_kc.inv_h)
+    assert list(g_or.lo) == [np.float32(g_kc.lo[k]) for k in range(3)]
+
+
+@pytest.mark.parametrize("d", [2, 3])
+def test_geometry_by_median_density_matches_the_oracle(d):
+    """Reading R24: the library's coarse histogram + median and the oracle's give the same geometry,
+    field by field, on uniform sets (k = 0), config 5's mixture (k = 1), sets heaped into one coarse
+    cell around the rounding boundaries of k, sets too small for an estimate and a box far from the
+    origin; the certificates on the coarser grid are the oracle's."""
+    rng = np.random.default_rng(7 + d)
+    scenes = [wl.uniform_points(20000, d, 4), wl.mixture_points(262144, d, 5), wl.uniform_points(100, d, 6),
+              (wl.mixture_points(65536, d, 8, 16, 0.002).astype(np.float64) * 3.0 + 250.0).astype(np.float32)]
+    R = 8 if d == 2 else 4
+    cells = np.stack(np.meshgrid(*[np.arange(R)] * d, indexing="ij"), -1).reshape(-1, d)
+    for m in (64, 46, 45, 32, 23, 22, 4):
+        base = (np.repeat(cells, m, axis=0) + rng.uniform(0.2, 0.8, (cells.shape[0] * m, d))) / R
+        heap = (np.full((4096 - base.shape[0], d), R // 2) + rng.uniform(0.2, 0.8, (4096 - base.shape[0], d))) / R
+        p = np.concatenate([base, heap]).astype(np.float32)
+        p[0] = 0.0
+        p[base.shape[0] - 1] = 1.0
+        scenes.append(p)
+    for p in scenes:
+        g_or = oracle.geom_by_median_density(p)
+        g_kc = kc.kc_geom_by_median_density(dev(p))
+        _same_geom(g_or, g_kc)
+    with pytest.raises(kc.KcError):
+        kc.kc_geom_by_median_density(dev(scenes[0]), occ=0.0)
+    p = scenes[1]
+    g_kc = kc.kc_geom_by_median_density(dev(p))
+    assert g_kc.G[0] < geoms(p)[1].G[0]                            # coarser than the mean-occupancy grid
+    grid = kc.Grid(p.shape[0], g_kc)
+    assert_same(kc.kc_cert_grid_rebuild(grid, dev(p)), oracle.kdtree_top2(p), what=f"median-density grid d{d}")
