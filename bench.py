@@ -512,8 +512,10 @@ def run_gpu_arm_scale(args):
     c = wl.CONFIGS[cfg]
     N, d = c["N"], c["d"]
     n_ap = min(N_ALLPAIRS, N)
-    # replicas only: every rank runs its own seeded copy of the workload
-    p0, mot = wl.make_scene(cfg, seed=c["seed"] + 7919 * rank)
+    # default: replicas only, every rank runs its own seeded copy of the workload;
+    # --shard queries: ONE copy, the N x N pass split by query over the ranks
+    sharded = args.shard == "queries"
+    p0, mot = wl.make_scene(cfg, seed=c["seed"] + (0 if sharded else 7919 * rank))
     host = [p0]
     for _ in range(W + K):
         host.append(mot.step(host[-1])[0])
@@ -530,6 +532,12 @@ def run_gpu_arm_scale(args):
     m = Maintainer(dev_traj[0], geom=geom, allpairs=False)
     ap = kc.Certs.empty(n_ap, dev)
     ws = torch.zeros(max(16, kc.lib().kc_cert_allpairs_workspace(n_ap, d)), dtype=torch.uint8, device=dev)
+    if sharded:
+        from paper_2606_18314_b200.sharding import gather_columns, query_slice
+        q_lo, q_hi = query_slice(n_ap, rank, world)
+        q_ids = torch.arange(q_lo, q_hi, dtype=torch.int32, device=dev)
+        q_n = torch.tensor([q_hi - q_lo], dtype=torch.int32, device=dev)
+        ws_q = torch.zeros(max(16, kc.lib().kc_frontier_oracle_workspace(n_ap, d, q_hi - q_lo)), dtype=torch.uint8, device=dev)
 
     def step(mm, p_next, timed):
         res = mm.step(p_next, time_phases=timed, do_allpairs=False)
@@ -537,7 +545,13 @@ def run_gpu_arm_scale(args):
         if timed:
             ev = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
             ev[0].record()
-        kc.kc_cert_allpairs(p_next[:n_ap], ap, ws)                  # A1: the oracle pass, 2^20 points of p'
+        if sharded:
+            # A1 by query: this rank's ids against all 2^20 points, then the certificate columns of the
+            # other ranks (20 B per point, one all-gather)
+            kc.kc_frontier_oracle(p_next[:n_ap], q_ids, q_n, ap, workspace=ws_q)
+            gather_columns(ap.buf, n_ap)
+        else:
+            kc.kc_cert_allpairs(p_next[:n_ap], ap, ws)              # A1: the oracle pass, 2^20 points of p'
         if timed:
             ev[1].record()
         return res, ev
@@ -572,6 +586,8 @@ def run_gpu_arm_scale(args):
         phase_sum["allpairs"] += ev[0].elapsed_time(ev[1])
         nF_sum += int(nF.item()); H_sum += float(H.item())
     dev_ms_max, units = aggregate_over_ranks(dev_ms, N * K, dev)
+    if sharded:
+        units = N * K                                                # one job: every rank certified the same points
     value = units / (dev_ms_max * 1e-3)
     info = m.grid.info()
     del m
@@ -602,6 +618,8 @@ def run_gpu_arm_scale(args):
     barrier()
     e2e_ms = sum(a.elapsed_time(b) for a, b in e2e_events)
     e2e_ms_max, units = aggregate_over_ranks(e2e_ms, N * K, dev)
+    if sharded:
+        units = N * K
     e2e_value = units / (e2e_ms_max * 1e-3)
     del m2, pinned, bufs
 
@@ -688,12 +706,15 @@ def run_gpu_arm_scale(args):
             extras["mover_sweep_" + cfg] = mover_sweep_scale(kc, Maintainer, crossover_fraction, torch, dev, cfg, flush)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": scale_workload_text(cfg),
                        "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event times summed",
                        "launch": "eager stream launches through the C-ABI (a grid of this size is not launch-bound)",
-                       "multi_gpu": "replicas only: each rank runs its own seeded copy, no collective on the data path",
+                       "multi_gpu": ("query-partitioned all-pairs pass (SURVEY.md §8(e)): one copy of the workload, rank r "
+                                     "runs kc_frontier_oracle on its contiguous share of the 2^20 queries, one all-gather of the "
+                                     "certificate columns (20 B/point); the O(N) rows run replicated" if sharded else
+                                     "replicas only: each rank runs its own seeded copy, no collective on the data path"),
                        "certified": certified},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -1087,6 +1108,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--workload", default="cfg5_d3", choices=["cfg5_d3", "cfg5_d2", "cfg2", "cfg3"])
+    ap.add_argument("--shard", choices=["none", "queries"], default="none",
+                    help="multi-GPU mode of the config 5 workloads: replicas (default) or the all-pairs pass split by query")
     ap.add_argument("--no-extras", action="store_true", help="skip the config 4 / config 5 side measurements")
     ap.add_argument("--no-graph", action="store_true", help="issue the step eagerly instead of replaying CUDA graphs")
     args = ap.parse_args()

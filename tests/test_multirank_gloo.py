@@ -59,3 +59,56 @@ def test_reference_arm_other_ranks_exit_silently():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--steps", "1", "--warmup", "3"], env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+# ---- the all-pairs pass sharded by query ----------------------------------------
+def test_query_slices_partition_the_ids():
+    from paper_2606_18314_b200.sharding import query_slice, slice_width
+    for n, world in [(1048576, 1), (1048576, 2), (1048576, 8), (1001, 2), (10, 3), (2, 4), (0, 2), (7, 7)]:
+        cuts = [query_slice(n, r, world) for r in range(world)]
+        assert cuts[0][0] == 0 and cuts[-1][1] == n
+        assert all(cuts[r][1] == cuts[r + 1][0] for r in range(world - 1))          # contiguous, in rank order
+        sizes = [b - a for a, b in cuts]
+        assert max(sizes) - min(sizes) <= 1 and max(sizes) == slice_width(n, world) and sizes == sorted(sizes, reverse=True)
+    import pytest
+    with pytest.raises(ValueError):
+        query_slice(10, 2, 2)
+
+
+def _shard_worker(rank, world, port, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    from paper_2606_18314_b200.sharding import gather_columns, query_slice
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        ok = True
+        for n in (1001, 4096, 5):
+            # the "certificates" of id i are a known function of i; a rank fills only its own slice
+            # (the rest of its buffer holds garbage), then the ranks exchange the columns
+            want = torch.stack([torch.arange(n, dtype=torch.int32) * (k + 3) + k for k in range(5)])
+            buf = torch.full((5, (n + 3) // 4 * 4), -777, dtype=torch.int32)
+            lo, hi = query_slice(n, rank, world)
+            buf[:, lo:hi] = want[:, lo:hi]
+            gather_columns(buf, n)
+            ok &= bool(torch.equal(buf[:, :n], want))
+            ok &= bool((buf[:, n:] == -777).all())                        # the padding is not touched
+        flags = [torch.zeros(1, dtype=torch.int32) for _ in range(world)]
+        dist.all_gather(flags, torch.tensor([int(ok)], dtype=torch.int32))
+        if rank == 0:
+            json.dump(dict(ok=[int(f) for f in flags]), open(out, "w"))
+    finally:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def test_sharded_certificates_are_gathered_on_every_rank(tmp_path):
+    for world in (2, 3):
+        out = str(tmp_path / f"s{world}.json")
+        port = 31500 + (os.getpid() + world) % 2000
+        mp.spawn(_shard_worker, args=(world, port, out), nprocs=world, join=True)
+        assert json.load(open(out))["ok"] == [1] * world
+
+
+def test_gather_without_a_process_group_is_the_identity():
+    from paper_2606_18314_b200.sharding import gather_columns
+    buf = torch.arange(20, dtype=torch.int32).reshape(5, 4)
+    assert gather_columns(buf, 4) is buf and torch.equal(buf, torch.arange(20, dtype=torch.int32).reshape(5, 4))
