@@ -139,6 +139,27 @@ kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t *nn, int32_
                            float *d2, float *c, void *workspace, size_t workspace_bytes,
                            void *stream);
 
+/* A1 for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same pass as kc_cert_allpairs (Table 2;
+ * same kernels, bit-identical certificates) with its workspace in a file-scope device array of the
+ * library instead of a caller-allocated one.  The call makes no cudaMalloc / cudaFree / cudaHostAlloc
+ * and calls no allocating routine: one cudaMemsetAsync of the workspace's counters (75,792 B; the array
+ * keeps the last call's contents and the counters must start at zero) and the kernels of
+ * kc_cert_allpairs, all on `stream`.
+ *   p: device float[N*d] (8-byte aligned); nn, d1, d2, c: device [N]; nn2: device [N] or NULL: the
+ *   caller's, as in kc_cert_allpairs.
+ *   LIMIT: 2 <= N <= kc_cert_allpairs_static_max_n() = 65,536 (the array is 5 MiB; every GPU that loads
+ *   the library holds it until exit).  A larger N returns KC_EINVAL with a message naming the limit
+ *   and nothing is launched.
+ *   SHARED STATE: every call on a device uses the same array.  Calls on one stream (or otherwise
+ *   ordered) are fine, back to back; calls that OVERLAP on the GPU (two streams, two host threads,
+ *   two replays of a captured graph in flight) race on it and their results are unspecified.
+ *   The device address of the array is looked up once per device (cudaGetSymbolAddress, on the first
+ *   call with that device current). */
+int64_t kc_cert_allpairs_static_max_n(void);
+kc_status kc_cert_allpairs_static(const float *p, int64_t N, int d, int32_t *nn, int32_t *nn2, float *d1,
+                                  float *d2, float *c, void *stream);
+
 /* A1 started from a kinetic bound.  The certificate logic of Lemma 1: a step in
  * which no point moves by more than eps changes every pairwise distance by at most 2 eps, so the
  * new second-neighbour distance of point i is at most d2_prev[i] + 2 eps.  Given such a bound per

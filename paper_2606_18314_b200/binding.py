@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libkc.so")
 EXPORTS = (
     "kc_version", "kc_last_error", "kc_geom_from_bbox", "kc_bbox", "kc_geom_by_median_density",
     "kc_max_displacement",
-    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_bounded", "kc_cert_allpairs_seeded",
+    "kc_cert_allpairs_workspace", "kc_cert_allpairs", "kc_cert_allpairs_static_max_n", "kc_cert_allpairs_static", "kc_cert_allpairs_bounded", "kc_cert_allpairs_seeded",
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_set_index", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
@@ -78,6 +78,8 @@ def lib():
     L.kc_bbox.argtypes = [vp, i64, ci, vp, vp]
     L.kc_geom_by_median_density.argtypes = [vp, i64, ci, C.c_double, vp, C.POINTER(kc_geom)]
     L.kc_max_displacement.argtypes = [vp, vp, i64, ci, vp, vp]
+    L.kc_cert_allpairs_static_max_n.restype = i64
+    L.kc_cert_allpairs_static.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp]
     L.kc_cert_allpairs_workspace.restype = sz
     L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
     L.kc_cert_allpairs.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp, sz, vp]
@@ -246,6 +248,14 @@ def _workspace(nbytes, device, kind="allpairs"):
         w = torch.zeros(nbytes, dtype=torch.uint8, device=device)
         _ws_cache[key] = w
     return w
+
+
+def kc_cert_allpairs_static(p, out: Certs) -> Certs:
+    """A1 with the library's static scratch (no allocation anywhere in the call, kc.h): N up to
+    ``lib().kc_cert_allpairs_static_max_n()``; ``out`` is the caller's, allocated beforehand."""
+    pp, N, d = _pos(p)
+    _check(lib().kc_cert_allpairs_static(pp, N, d, *out._ptrs(), _stream()), "kc_cert_allpairs_static")
+    return out
 
 
 def kc_cert_allpairs(p, out: Certs | None = None, workspace=None, d2_prev=None, eps=None,

@@ -18,6 +18,8 @@
 //     lanes that puts some lane on the insertion path in almost every step of a short chunk.
 #include <stdlib.h>
 
+#include <atomic>
+
 #include "kc_common.cuh"
 
 using namespace kc;
@@ -441,14 +443,14 @@ void launch_t(int threads, dim3 grid, cudaStream_t st, const ApArgs &a)
 }
 
 template <int D>
-kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st)
+kc_status launch(ApArgs a, char *ws, Shape sh, cudaStream_t st, int *errword = nullptr)
 {
     const int64_t nq = a.nq_host;
     const bool split = sh.js > 1, bounded = a.bound_d2 != nullptr;
     a.one2 = 0x3f8000003f800000ull;
     a.n_redo = reinterpret_cast<int32_t *>(ws);
     a.tickets = reinterpret_cast<int32_t *>(ws + 16);
-    a.errword = error_word_dev();
+    a.errword = errword ? errword : error_word_dev();
     a.redo = reinterpret_cast<int32_t *>(ws + head_bytes(nq, sh));
     Partial *seed = reinterpret_cast<Partial *>(ws + head_bytes(nq, sh) + pad16((size_t)nq * 4));
     const bool idseed = a.seed1 != nullptr;
@@ -551,6 +553,77 @@ extern "C" kc_status kc_cert_allpairs(const float *p, int64_t N, int d, int32_t 
 {
     return run("kc_cert_allpairs", p, N, d, nullptr, nullptr, N, nullptr, nullptr, nullptr, nullptr, nn, nn2, d1, d2, c,
                workspace, workspace_bytes, stream);
+}
+
+// ---- A1 without any allocation: the workspace is a file-scope device array ---------------------
+// For callers that cannot allocate (kc.h).  Every GPU that loads the library holds these 5 MiB until
+// exit.  KC_ALLPAIRS_STATIC_MAX_N = 65,536: the largest workspace_bytes_for(N, choose_shape(N, N)) over
+// N <= 65,536 is 4,811,792 B (at N = 56,832).
+constexpr int64_t AP_STATIC_MAX_N = 65536;
+constexpr size_t AP_STATIC_BYTES = 5u << 20;
+static __device__ __align__(256) unsigned char g_ap_static_scratch[AP_STATIC_BYTES];
+
+namespace {
+// In host code the array's name is a host-side stand-in: its device address is looked up once per
+// device, with that device current.
+constexpr int AP_MAX_DEVICES = 64;
+std::atomic<void *> g_ap_static_ptr[AP_MAX_DEVICES];
+
+kc_status ap_static_address(char **out)
+{
+    int dev = -1;
+    KC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= AP_MAX_DEVICES) {
+        set_error("kc_cert_allpairs_static: device ordinal %d not supported (< %d)", dev, AP_MAX_DEVICES);
+        return KC_EINVAL;
+    }
+    void *ptr = g_ap_static_ptr[dev].load(std::memory_order_acquire);
+    if (!ptr) {
+        KC_CUDA(cudaGetSymbolAddress(&ptr, g_ap_static_scratch));
+        g_ap_static_ptr[dev].store(ptr, std::memory_order_release);
+    }
+    *out = static_cast<char *>(ptr);
+    return KC_OK;
+}
+}  // namespace
+
+extern "C" int64_t kc_cert_allpairs_static_max_n(void) { return AP_STATIC_MAX_N; }
+
+extern "C" kc_status kc_cert_allpairs_static(const float *p, int64_t N, int d, int32_t *nn, int32_t *nn2,
+                                             float *d1, float *d2, float *c, void *stream)
+{
+    const char *who = "kc_cert_allpairs_static";
+    if (!p || !nn || !d1 || !d2 || !c || N < 2 || (d != 2 && d != 3) || (reinterpret_cast<uintptr_t>(p) & 7)) {
+        set_error("%s: bad argument", who);
+        return KC_EINVAL;
+    }
+    if (N > AP_STATIC_MAX_N) {
+        set_error("%s: N = %lld exceeds the static scratch's maximum of %lld points; use kc_cert_allpairs "
+                  "with a caller-allocated workspace", who, (long long)N, (long long)AP_STATIC_MAX_N);
+        return KC_EINVAL;
+    }
+    const Shape sh = choose_shape(N, N);
+    const size_t need = workspace_bytes_for(N, sh);
+    if (need > AP_STATIC_BYTES) {
+        set_error("%s: N = %lld needs %zu bytes of scratch, the static array holds %zu", who, (long long)N, need,
+                  (size_t)AP_STATIC_BYTES);
+        return KC_EINVAL;
+    }
+    char *ws = nullptr;
+    const kc_status rc = ap_static_address(&ws);
+    if (rc != KC_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps the last call's contents: the counters at its head (n_redo, this variant's error
+    // word, the tickets) must start at zero; everything behind them is written before it is read
+    KC_CUDA(cudaMemsetAsync(ws, 0, head_bytes(N, sh), st));
+    ApArgs a = {};
+    a.p = p; a.N = N; a.nq_host = N;
+    a.nn = nn; a.nn2 = nn2; a.d1 = d1; a.d2 = d2; a.c = c;
+    // the error word of this variant lives in the head's padding (device memory: the pinned host word
+    // of the other entry points would be an allocation)
+    int *errword = reinterpret_cast<int *>(ws + 8);
+    if (d == 2) return launch<2>(a, ws, sh, st, errword);
+    return launch<3>(a, ws, sh, st, errword);
 }
 
 extern "C" kc_status kc_cert_allpairs_bounded(const float *p, int64_t N, int d, const float *d2_prev,
