@@ -79,6 +79,7 @@ typedef struct {
     int32_t n_heavy;     /* level-0 cells the last build subdivided (two-level index) */
     int32_t n_leaves;    /* leaves of the last build: undivided cells + sub-cells */
     int32_t heavy_T;     /* build-time record count from which a cell is subdivided */
+    int32_t n_handed;    /* queries the ring search handed to the brute-force pass since the last build */
 } kc_grid_info_t;
 
 /* ---- host utilities -------------------------------------------------------------------- */
@@ -224,7 +225,13 @@ kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *stream);
  * [cell(q - r), cell(q + r)] per axis, r >= d2 rounded outwards (the filing function is monotone,
  * so nothing within r can lie outside that box); d = 2 and the fallback of d = 3: wider Chebyshev
  * rings until the distance to the nearest unscanned cell face, shrunk by a rounding slack,
- * exceeds d2, strictly.  KC_EREBUILD if the grid is not freshly built. */
+ * exceeds d2, strictly.  Straggler hand-off (this call, kc_frontier_search and
+ * kc_frontier_repair): on a grid of >= 200,000 points a query whose rings have reached radius 24
+ * (d = 2) / 8 (d = 3) without meeting that bound -- an isolated point, for which ring r costs one
+ * thread O(r^(d-1)) dependent row visits -- is put on a list of up to 1,024 queries and finished by a
+ * brute-force pass of the whole GPU over all records (the definition of the certificate, so the same
+ * bits), launched behind the search kernel; a query that finds the list full goes on with its rings.
+ * kc_grid_info_t::n_handed counts them.  KC_EREBUILD if the grid is not freshly built. */
 kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
                               void *stream);
 /* A2 + A3 in one call: the O(N) rebuild strategy. */

@@ -21,6 +21,9 @@ struct Counters {
     int ticket2;              // blocks of the A7 list kernel that are done (the last one empties list2)
     int n_heavy;              // level-0 cells that the last build subdivided (two-level index)
     int n_leaves;             // leaves of the last build: one per undivided cell + S^d per subdivided one
+    int n_handoff;            // queries in the hand-off list of the search in progress (zero between calls)
+    int ticket3;              // blocks of the hand-off kernel that are done (the last one empties the list)
+    int n_handed;             // queries handed to the brute-force pass since the last build
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -71,7 +74,22 @@ struct View {
     int heavy_T;              // build-time record count from which a level-0 cell is subdivided
     const int2 *subinfo;      // per level-0 cell: {S (0 = not subdivided), index of its first leaf}
     const int32_t *leaf_start;   // exclusive scan of the leaf sizes (n_leaves + 1 entries)
+    float4 *handoff;          // hand-off list (x, y, z, bits(id)) of ring_continue, or null: rings without limit
+    int *n_handoff;           // its length (Counters::n_handoff)
 };
+
+// Straggler hand-off: a query whose ring search has scanned radius
+// HANDOFF_R without meeting its bound (an isolated point: ring r costs O(r^(d-1)) dependent row
+// visits of ONE thread, about a thousand by that radius) is appended to a list and finished by a
+// brute-force pass of the whole GPU over all records, after the search kernel.  Only on grids of at
+// least HANDOFF_MIN_N points (below that the whole grid is a few thousand rows); a list that is full
+// leaves the query to the rings.
+constexpr int HANDOFF_CAP = 1024;
+constexpr int HANDOFF_BLOCKS = 148;              // CTAs of the pass: one record chunk and one partial list each
+constexpr int HANDOFF_MIN_N = 200000;
+constexpr int HANDOFF_R2 = 24, HANDOFF_R3 = 8;
+struct HandoffPart { float s1, s2; int j1, j2; };
+
 
 }  // namespace kc
 
@@ -88,6 +106,8 @@ struct kc_grid {
     int heavy_T, sub_occ;
     int32_t *mark;            // per sorted slot: 1 while a sweep has it as a query (zero between calls)
     int32_t *list2;           // frontier points of the current sweep that live in chains
+    float4 *handoff;          // hand-off list of the search in progress (HANDOFF_CAP entries; grids of
+    kc::HandoffPart *handoff_part;   //   >= HANDOFF_MIN_N points only) and the pass's partial lists [CAP][BLOCKS]
     float *delta;             // NEXT #2: displacement of every point in the current step
     unsigned *cellmax;        // NEXT #2: largest displacement (float bits) per cell
     float2 *spos2;
@@ -119,6 +139,7 @@ inline View make_view(const kc_grid *g)
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;
     v.heavy_T = g->heavy_T; v.subinfo = g->subinfo; v.leaf_start = g->leaf_start;
+    v.handoff = nullptr; v.n_handoff = nullptr;       // (the callers that launch the hand-off pass set them)
     return v;
 }
 

@@ -288,7 +288,7 @@ __device__ __forceinline__ void visit_row(const View &v, bool chains, int rowbas
 struct RingOut { Top2 best; int r; };
 template <int D>
 __device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float qx, float qy, float qz,
-                                              int self, int cx, int cy, int cz, Top2 best)
+                                              int self, int cx, int cy, int cz, Top2 best, bool warp_wide)
 {
     int r = 1;
     for (;;) {
@@ -296,6 +296,20 @@ __device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float 
         int y0 = max(cy - r, 0), y1 = min(cy + r, v.G1 - 1);
         int x0 = max(cx - r, 0), x1 = min(cx + r, v.G0 - 1);
         if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) break;
+        if (v.handoff && r == (D == 3 ? HANDOFF_R3 : HANDOFF_R2)) {
+            // an isolated query: the brute-force pass behind this kernel finishes it (the certificate
+            // the caller stores now is overwritten there).  warp_wide: all 32 lanes are here with the
+            // same query (the list kernel), lane 0 speaks for them.
+            const bool speaker = !warp_wide || (threadIdx.x & 31) == 0;
+            int idx = HANDOFF_CAP;
+            if (speaker) idx = atomicAdd(v.n_handoff, 1);
+            if (warp_wide) idx = __shfl_sync(0xffffffffu, idx, 0);
+            if (idx < HANDOFF_CAP) {                   // (a full list leaves the query to the rings)
+                if (speaker) v.handoff[idx] = make_float4(qx, qy, qz, __int_as_float(self));
+                ++r;
+                break;
+            }
+        }
         ++r;
         // ring r: shell rows get the full segment, inner rows only the two end cells
         z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
@@ -320,13 +334,13 @@ __device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float 
 // final check of the radius-1 block, then wider rings if the bound requires them
 template <int D>
 __device__ __forceinline__ int finish_block(const View &v, bool chains, float qx, float qy, float qz, int self,
-                                            int cx, int cy, int cz, Top2 &best)
+                                            int cx, int cy, int cz, Top2 &best, bool warp_wide = false)
 {
     const int z0 = D == 3 ? max(cz - 1, 0) : 0, z1 = D == 3 ? min(cz + 1, v.G2 - 1) : 0;
     const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
     const int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
     if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) return 1;
-    const RingOut o = ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    const RingOut o = ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best, warp_wide);
     best = o.best;
     return o.r;
 }
@@ -1140,7 +1154,7 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
     if (ja != KC_NOIDX) best.offer(sa, ja);
     if (jb != KC_NOIDX) best.offer(sb, jb);
     // every lane holds the same state: the rare ring continuation runs redundantly on all of them
-    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best, true);
 }
 
 // The list kernel is the last reader of list2 (the chain residents of a swept frontier): the block
@@ -1355,6 +1369,124 @@ bool dispatch_grid_topk(int K, const View &v, int n, int32_t *nnk, float *dk, fl
 }  // namespace
 
 // ====================================================================== C-ABI
+// ---- straggler hand-off: brute force for the queries ring_continue gave up on ---------------------
+// The whole GPU scans every record of the grid once per batch of HO_BATCH listed queries: CTA b owns
+// one chunk of the records -- the sorted array (tombstones are inert) followed by the chain residents
+// (mlist) -- keeps the two smallest keys (s, j) of every query of the batch over its chunk and writes
+// them to part[query][b]; the CTA that finishes last merges the HANDOFF_BLOCKS partial lists of
+// every query and stores its certificate: the definition itself, so the result is the one the rings
+// would have reached.  That CTA also empties the list: every search call starts from an empty one.
+// (One batch reads the records from HBM, later ones find them in L2.)
+namespace {
+constexpr int HO_THREADS = 512, HO_BATCH = 8;
+template <int D>
+__global__ void __launch_bounds__(HO_THREADS)
+handoff_kernel(const View v, int N, const int32_t *__restrict__ mlist, Counters *ctr, HandoffPart *part,
+               int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
+{
+    __shared__ float s_s[HO_BATCH][2 * HO_THREADS / 32];
+    __shared__ int s_j[HO_BATCH][2 * HO_THREADS / 32];
+    __shared__ bool s_last;
+    const int n = min(ctr->n_handoff, HANDOFF_CAP);
+    if (n == 0) return;                            // (every CTA sees the same count: it changes below only)
+    const int nm = ctr->n_misfiled, total = N + nm;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nb = gridDim.x;
+    const int chunk = (total + nb - 1) / nb;
+    const int r0 = blockIdx.x * chunk, r1 = min(r0 + chunk, total);
+    for (int f0 = 0; f0 < n; f0 += HO_BATCH) {
+        float qx[HO_BATCH], qy[HO_BATCH], qz[HO_BATCH];
+        int self[HO_BATCH];
+        Top2 t[HO_BATCH];
+#pragma unroll
+        for (int k = 0; k < HO_BATCH; ++k) {
+            const float4 q = v.handoff[min(f0 + k, n - 1)];
+            qx[k] = q.x; qy[k] = q.y; qz[k] = q.z; self[k] = __float_as_int(q.w);
+            t[k].init();
+        }
+        for (int r = r0 + threadIdx.x; r < r1; r += HO_THREADS) {
+            float x, y, z = 0.f;
+            int j;
+            if (r >= N) {
+                j = mlist[r - N];
+                const float4 o = v.opos[j];
+                x = o.x; y = o.y; z = o.z;
+            } else if (D == 2) {
+                const float2 o = v.spos2[r];
+                x = o.x; y = o.y; j = v.sidx[r];
+            } else {
+                const float4 o = v.spos4[r];
+                x = o.x; y = o.y; z = o.z; j = __float_as_int(o.w);
+            }
+#pragma unroll
+            for (int k = 0; k < HO_BATCH; ++k) {
+                const float s = D == 2 ? sqd2(qx[k], qy[k], x, y) : sqd3(qx[k], qy[k], qz[k], x, y, z);
+                insert_bf(t[k], s, j, j >= 0 && j != self[k]);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < HO_BATCH; ++k) {
+            float sa, sb;
+            int ja, jb;
+            warp_pop(t[k], sa, ja);
+            warp_pop(t[k], sb, jb);
+            if (lane == 0) { s_s[k][2 * w] = sa; s_j[k][2 * w] = ja; s_s[k][2 * w + 1] = sb; s_j[k][2 * w + 1] = jb; }
+        }
+        __syncthreads();
+        if (threadIdx.x < HO_BATCH && f0 + threadIdx.x < n) {
+            const int k = threadIdx.x;
+            Top2 best;
+            best.init();
+            for (int e = 0; e < 2 * HO_THREADS / 32; ++e)
+                if (s_j[k][e] != KC_NOIDX) best.offer(s_s[k][e], s_j[k][e]);
+            HandoffPart o;
+            o.s1 = best.s1; o.s2 = best.s2; o.j1 = best.j1; o.j2 = best.j2;
+            part[(size_t)(f0 + k) * nb + blockIdx.x] = o;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        s_last = atomicAdd(&ctr->ticket3, 1) == nb - 1;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int f = threadIdx.x; f < n; f += HO_THREADS) {
+        Top2 best;
+        best.init();
+        for (int b = 0; b < nb; ++b) {
+            const HandoffPart o = part[(size_t)f * nb + b];
+            if (o.j1 != KC_NOIDX) best.offer(o.s1, o.j1);
+            if (o.j2 != KC_NOIDX) best.offer(o.s2, o.j2);
+        }
+        store_cert(best, __float_as_int(v.handoff[f].w), nn, nn2, d1, d2, c);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        ctr->n_handed += n;
+        ctr->n_handoff = 0;
+        ctr->ticket3 = 0;
+    }
+}
+// Grids that hand off (kc_grid.cuh): the view carries the list, and the pass runs behind the search
+// kernels of the call (it returns at once when the list is empty).
+inline bool hands_off(const kc_grid *g) { return g->N >= HANDOFF_MIN_N && g->handoff != nullptr; }
+inline void view_handoff(const kc_grid *g, View &v)
+{
+    if (hands_off(g)) { v.handoff = g->handoff; v.n_handoff = &g->ctr->n_handoff; }
+}
+inline void launch_handoff(const kc_grid *g, const View &v, int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c,
+                           cudaStream_t st)
+{
+    if (!hands_off(g)) return;
+    if (g->geom.d == 2)
+        handoff_kernel<2><<<HANDOFF_BLOCKS, HO_THREADS, 0, st>>>(v, (int)g->N, g->mlist, g->ctr, g->handoff_part, nn, nn2, d1, d2, c);
+    else
+        handoff_kernel<3><<<HANDOFF_BLOCKS, HO_THREADS, 0, st>>>(v, (int)g->N, g->mlist, g->ctr, g->handoff_part, nn, nn2, d1, d2, c);
+    count_launches(1);
+}
+}  // namespace
+
 extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, float *d1, float *d2,
                                          float *c, void *stream)
 {
@@ -1367,11 +1499,13 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     }
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
+    view_handoff(g, v);
     const int n = (int)g->N;
     const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
     if (g->geom.d == 2) search_tiled_kernel<2, false, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
     count_launches(1);
+    launch_handoff(g, v, nn, nn2, d1, d2, c, st);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
     return KC_OK;
 }
@@ -1447,6 +1581,7 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     if (nF_max == 0) return KC_OK;
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
+    view_handoff(g, v);
     const int n = (int)N;
     // slot sweep: grids of at least SWEEP_MIN_N points, frontier of at least N / SWEEP_DIV points
     // (the host bound decides whether the sweep kernels are launched, the device count whether they run)
@@ -1472,6 +1607,7 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     else
         search_wpq_kernel<3><<<blocks, 128, 0, st>>>(v, p_new, n, F, nF, g->list2, sweep_div, g->ctr, nn, nn2, d1, d2, c);
     count_launches(1);
+    launch_handoff(g, v, nn, nn2, d1, d2, c, st);
     KC_LAUNCH_CHECK("kc_frontier_search");
     return KC_OK;
 }
