@@ -998,6 +998,52 @@ def run_extras(kc, Maintainer, crossover_fraction, torch, dev, peaks, skip_cfg=N
                                      points_per_s=Ncl / (t_clock * 1e-3))
         del cm
     ex["clock_loop"] = clock
+    # the same loop at 4,194,304 points (config 5's d = 3 set, random walk) for three step sizes: the
+    # expired set through the expiry tree (Theorem 2, kc_frontier_classify_clock_tree) and through the
+    # flat test; the step follows the revisited fraction, the tree's classify the number of opened nodes
+    if skip_cfg != "clock4m":
+        c5 = wl.CONFIGS["cfg5_d3"]
+        p0 = wl.make_points("cfg5_d3")
+        P0 = torch.from_numpy(p0).to(dev)
+        geom5 = kc.kc_geom_by_median_density(P0)
+        rows = []
+        for eps_w in (2e-8, 2e-7, 2e-6, 2e-4):
+            mot = wl.Motion("walk", c5["d"], eps_w, 4242)
+            hp = [p0]
+            for _ in range(7):
+                hp.append(mot.step(hp[-1])[0])
+            dp = [torch.from_numpy(x).to(dev) for x in hp]
+            row = dict(eps=eps_w, N=c5["N"])
+            for tree in (True, False):
+                cm = ClockMaintainer(dp[0], tree=tree, geom=geom5)
+                fsum = torch.zeros(1, dtype=torch.int64, device=dev)
+                for t in (1, 2):
+                    cm.step(dp[t])
+                torch.cuda.synchronize()
+                flush.zero_()
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for t in range(3, 8):
+                    _, nF = cm.step(dp[t])
+                    fsum += nF
+                e1.record(); e1.synchronize()
+                key = "tree" if tree else "flat"
+                row[f"clock_step_ms_{key}"] = e0.elapsed_time(e1) / 5
+                row["mean_revisited_frac"] = float(fsum.item()) / 5 / c5["N"]
+                # the classify alone, on the state the loop has reached (it changes neither c nor the stamps)
+                Sx = torch.zeros(1, dtype=torch.float64, device=dev)
+                if tree:
+                    fn = lambda: kc.kc_frontier_classify_clock_tree(cm.certs.c, cm.stamp, cm.tree, cm.S[0], cm.eps, Sx, cm.F, cm.nF)
+                else:
+                    fn = lambda: kc.kc_frontier_classify_clock(cm.certs.c, cm.stamp, cm.S[0], cm.eps, Sx, cm.flags, cm.F, cm.nF)
+                row[f"classify_ms_{key}"] = _median_ms(torch, fn, 7, flush=flush)
+                del cm
+            other = kc.Certs.empty(c5["N"], dev)
+            g5 = kc.Grid(c5["N"], geom5)
+            row["rebuild_step_ms"] = _median_ms(torch, lambda: kc.kc_cert_grid_rebuild(g5, dp[7], other), 5, flush=flush)
+            del g5, other, dp
+            rows.append(row)
+        ex["clock_loop_cfg5_d3"] = rows
     # ---------------- NEXT #4: K-list certificates (K = 4): all-pairs pass and grid search
     topk = {}
     for cfg, n_sub in (("cfg2", None), ("cfg4", 131072)):

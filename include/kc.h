@@ -278,6 +278,29 @@ kc_status kc_frontier_classify_clock(const float *c, const float *stamp, int64_t
 kc_status kc_clock_stamp(const int32_t *F, const int32_t *nF, int64_t nF_max, int64_t N, const double *S,
                          float *stamp, void *stream);
 
+/* The expiry structure of the clock (Theorem 2: "an expiry heap ... O(|F_t| log N)
+ * per step") in data-parallel form: a tournament tree over the point ids with fanout 32.  Level-1
+ * node j holds a lower bound of min over points 32j .. 32j+31 of the expiry clock stamp_i + c_i / 4
+ * (double, rounded down to float, lowered by a relative 2^-22 and 1e-37: more than every rounding of
+ * the flat test), level-2 node k the minimum of level-1 nodes 32k .. 32k+31.
+ *   tree: device float[kc_clock_tree_floats(N)] = ceil(N/32) + ceil(N/1024) floats, the caller's.
+ *   kc_clock_tree_build: all nodes from c and stamp (O(N)).
+ *   kc_frontier_classify_clock_tree: the SAME set F as kc_frontier_classify_clock for the same c, stamp,
+ *     S_in, eps (and the same S_out), found by reading the ceil(N/1024) level-2 nodes, the children of
+ *     those whose bound is <= S (rounded up to float), and the 32 points of those whose bound is <= S,
+ *     to which the flat test is applied as written above.  No flags array (that would be O(N) writes);
+ *     F in arbitrary order.  c, stamp and tree must be consistent (built, or updated after every change).
+ *   kc_clock_tree_update: after the certificates of the ids in F (*nF on the device, at most nF_max)
+ *     have been recomputed and re-stamped: their level-1 and level-2 nodes are recomputed (from all
+ *     N points when *nF > N / 16, decided on the device; F = NULL: same as build). */
+size_t kc_clock_tree_floats(int64_t N);
+kc_status kc_clock_tree_build(const float *c, const float *stamp, int64_t N, float *tree, void *stream);
+kc_status kc_frontier_classify_clock_tree(const float *c, const float *stamp, int64_t N, const float *tree,
+                                          const double *S_in, const float *eps, double *S_out, int32_t *F,
+                                          int32_t *nF, void *stream);
+kc_status kc_clock_tree_update(const int32_t *F, const int32_t *nF, int64_t nF_max, const float *c,
+                               const float *stamp, int64_t N, float *tree, void *stream);
+
 /* ---- NEXT #2: certificate-failure audit (Definition 2; Table 1) -- */
 /* The true repair frontier F_t = { i : nn_post[i] != nn_pre[i] } of a step and the audit of the
  * Lemma-1 rule against it.  nn_pre / nn_post: device int32[N], exact certificates before / after

@@ -18,7 +18,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libkc.so")
-SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_topk.cu", "kc_grid.cu", "kc_search.cu"]
+SOURCES = ["kc_misc.cu", "kc_allpairs.cu", "kc_topk.cu", "kc_grid.cu", "kc_search.cu", "kc_clock.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",

@@ -26,7 +26,8 @@ EXPORTS = (
     "kc_frontier_oracle_workspace",
     "kc_frontier_oracle", "kc_grid_create", "kc_grid_destroy", "kc_grid_bytes", "kc_grid_set_index", "kc_grid_build",
     "kc_cert_grid_search", "kc_cert_grid_rebuild", "kc_frontier_classify", "kc_frontier_entropy",
-    "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_frontier_classify_local",
+    "kc_frontier_repair", "kc_grid_update", "kc_frontier_search", "kc_failure_audit", "kc_frontier_classify_clock", "kc_clock_stamp", "kc_clock_tree_floats", "kc_clock_tree_build",
+    "kc_frontier_classify_clock_tree", "kc_clock_tree_update", "kc_frontier_classify_local",
     "kc_cert_allpairs_topk_workspace", "kc_cert_allpairs_topk", "kc_cert_grid_topk", "kc_frontier_search_topk",
     "kc_grid_info", "kc_grid_export", "kc_fp32_probe", "kc_launch_count",
 )
@@ -79,6 +80,11 @@ def lib():
     L.kc_geom_by_median_density.argtypes = [vp, i64, ci, C.c_double, vp, C.POINTER(kc_geom)]
     L.kc_max_displacement.argtypes = [vp, vp, i64, ci, vp, vp]
     L.kc_cert_allpairs_static_max_n.restype = i64
+    L.kc_clock_tree_floats.restype = sz
+    L.kc_clock_tree_floats.argtypes = [i64]
+    L.kc_clock_tree_build.argtypes = [vp, vp, i64, vp, vp]
+    L.kc_frontier_classify_clock_tree.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp, vp]
+    L.kc_clock_tree_update.argtypes = [vp, vp, i64, vp, vp, i64, vp, vp]
     L.kc_cert_allpairs_static.argtypes = [vp, i64, ci, vp, vp, vp, vp, vp, vp]
     L.kc_cert_allpairs_workspace.restype = sz
     L.kc_cert_allpairs_workspace.argtypes = [i64, ci]
@@ -519,6 +525,39 @@ def kc_clock_stamp(stamp, S, F=None, nF=None, nF_max=None):
                                 _ptr(S, torch.float64, "S"), _ptr(stamp, torch.float32, "stamp"), _stream()),
            "kc_clock_stamp")
     return stamp
+
+
+def kc_clock_tree_build(c, stamp, tree=None):
+    """Expiry tournament tree of the clock (Theorem 2; kc.h) from c and stamp."""
+    N = c.numel()
+    if tree is None:
+        tree = torch.empty(int(lib().kc_clock_tree_floats(N)), dtype=torch.float32, device=c.device)
+    _check(lib().kc_clock_tree_build(_ptr(c, torch.float32, "c"), _ptr(stamp, torch.float32, "stamp"), N,
+                                     _ptr(tree, torch.float32, "tree"), _stream()), "kc_clock_tree_build")
+    return tree
+
+
+def kc_frontier_classify_clock_tree(c, stamp, tree, S_in, eps, S_out, F=None, nF=None):
+    """kc_frontier_classify_clock's F (as a set) through the expiry tree: reads N/1024 nodes + the opened ones."""
+    N = c.numel()
+    F = F if F is not None else torch.empty(N, dtype=torch.int32, device=c.device)
+    nF = nF if nF is not None else torch.empty(1, dtype=torch.int32, device=c.device)
+    _check(lib().kc_frontier_classify_clock_tree(_ptr(c, torch.float32, "c"), _ptr(stamp, torch.float32, "stamp"), N,
+                                                 _ptr(tree, torch.float32, "tree"), _ptr(S_in, torch.float64, "S_in"),
+                                                 _ptr(eps, torch.float32, "eps"), _ptr(S_out, torch.float64, "S_out"),
+                                                 _ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), _stream()),
+           "kc_frontier_classify_clock_tree")
+    return F, nF
+
+
+def kc_clock_tree_update(tree, c, stamp, F, nF, nF_max=None):
+    """Recompute the tree nodes above the ids in F (after their certificates were re-stamped)."""
+    N = c.numel()
+    nF_max = int(F.numel() if nF_max is None else nF_max)
+    _check(lib().kc_clock_tree_update(_ptr(F, torch.int32, "F"), _ptr(nF, torch.int32, "nF"), nF_max,
+                                      _ptr(c, torch.float32, "c"), _ptr(stamp, torch.float32, "stamp"), N,
+                                      _ptr(tree, torch.float32, "tree"), _stream()), "kc_clock_tree_update")
+    return tree
 
 
 def kc_failure_audit(nn_pre, nn_post, flags, Ft=None, counts=None, want_list=True):

@@ -169,17 +169,21 @@ class ClockMaintainer:
     point (Theorem 1 on cumulative displacement); d1, d2, c are exact for the points revisited in
     the current step and stale for the rest, by design."""
 
-    def __init__(self, p0: torch.Tensor, occ: float = 2.0, rebin_every: int = 4):
+    def __init__(self, p0: torch.Tensor, occ: float = 2.0, rebin_every: int = 4, tree: bool = False,
+                 geom: kc.kc_geom | None = None):
         assert p0.is_cuda and p0.dtype == torch.float32 and p0.dim() == 2
         self.N = int(p0.shape[0])
         dev = p0.device
+        # tree: the expired set comes from the expiry tournament tree (Theorem 2's heap, kc.h) instead
+        # of the flat test of all N certificates: same set, no flags array
+        self.tree = torch.empty(int(kc.lib().kc_clock_tree_floats(self.N)), dtype=torch.float32, device=dev) if tree else None
         # every `rebin_every` steps the grid is re-binned at the new positions (A2 only: O(N), no
         # certificate is recomputed) instead of updated incrementally, so the overflow chains of
         # re-filed points never grow long; 0 = never
         self.rebin_every = int(rebin_every)
         self.k = 0
         self.none = torch.zeros(1, dtype=torch.int32, device=dev)
-        self.geom = kc.kc_geom_for(p0, occ)
+        self.geom = geom if geom is not None else kc.kc_geom_for(p0, occ)
         self.grid = kc.Grid(self.N, self.geom)
         self.certs = kc.Certs.empty(self.N, dev)
         self.stamp = torch.zeros(self.N, dtype=torch.float32, device=dev)
@@ -194,14 +198,20 @@ class ClockMaintainer:
         """Fresh grid and exact certificates at p; every stamp is set to the current clock."""
         kc.kc_cert_grid_rebuild(self.grid, p, self.certs)
         kc.kc_clock_stamp(self.stamp, self.S[0])
+        if self.tree is not None:
+            kc.kc_clock_tree_build(self.certs.c, self.stamp, self.tree)
         self.p = p
 
     def step(self, p_next: torch.Tensor, movers: torch.Tensor | None = None):
         """p -> p_next: A0, clock classify, A6 + A7 on the expired certificates, re-stamp.  No host
         sync.  Returns (F, nF) of this step (device tensors)."""
         kc.kc_max_displacement(self.p, p_next, self.eps)
-        kc.kc_frontier_classify_clock(self.certs.c, self.stamp, self.S[0], self.eps, self.S[1],
-                                      self.flags, self.F, self.nF)
+        if self.tree is not None:
+            kc.kc_frontier_classify_clock_tree(self.certs.c, self.stamp, self.tree, self.S[0], self.eps, self.S[1],
+                                               self.F, self.nF)
+        else:
+            kc.kc_frontier_classify_clock(self.certs.c, self.stamp, self.S[0], self.eps, self.S[1],
+                                          self.flags, self.F, self.nF)
         self.S.reverse()
         self.k += 1
         if self.rebin_every and self.k % self.rebin_every == 0:
@@ -212,6 +222,8 @@ class ClockMaintainer:
         kc.kc_frontier_repair(self.grid, p_next, self.F, self.nF, self.certs, movers=movers,
                               n_movers=n_movers, nF_max=self.N)
         kc.kc_clock_stamp(self.stamp, self.S[0], self.F, self.nF, self.N)
+        if self.tree is not None:
+            kc.kc_clock_tree_update(self.tree, self.certs.c, self.stamp, self.F, self.nF, self.N)
         self.p = p_next
         return self.F, self.nF
 
