@@ -579,6 +579,13 @@ __device__ __forceinline__ void store_cert_keep(const Top2 &t, int i, int32_t *n
 // (>= WT_DENSE records) own cell first, then only the cells a lane cannot rule out.  The second level
 // of the index is ignored (level-0 ranges are contiguous whatever the order inside a cell).
 constexpr int WT_WARPS = 4;
+constexpr int SW_WORDS = 8;                        // sweep: a warp owns up to 32 * SW_WORDS consecutive slots
+// Slots per sweep warp, in units of 32: as many as hold about one warp of marked slots (measured on
+// config 5: a second round per warp costs more than idle lanes, so the count aims below 32).
+__device__ __forceinline__ int sweep_words(int N, int nF)
+{
+    return (int)min((int64_t)SW_WORDS, max((int64_t)1, (int64_t)N * 9 / ((int64_t)max(nF, 1) * 10)));
+}
 constexpr int WT_DENSE = 128;
 
 // Dense pass: every lane brings up to two ranges left after pruning.  Served lane by lane by the
@@ -873,39 +880,14 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
     return false;
 }
 
+// The search of one round: lane `lane` serves the query at sorted slot sc (query = false: the lane only
+// takes part in the warp-wide steps).  Called by all 32 lanes.
 template <int D, int MODE>
-__global__ void __launch_bounds__(32 * LT_WARPS, LT_MIN_BLOCKS)
-search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t *mark,
-                   const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
-                   float *d2, float *c)
+__device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters *ctr, bool chains, int lane,
+                                                  float2 *tp2, float4 *tp4, int *tix, Lane &L, int sc, bool query,
+                                                  int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
 {
     constexpr int NR = D == 3 ? 9 : 3;             // rows of a 3^d block
-    __shared__ __align__(16) float4 s_p4[D == 3 ? LT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
-    __shared__ __align__(16) float2 s_p2[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    __shared__ int s_ix[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
-    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
-    if (MODE != 0 && (int64_t)*nF * sweep_div < N) return;
-    const bool chains = MODE == 1 && ctr->n_misfiled > 0;     // MODE 2: a fresh grid has no chains (compile-time)
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const float qnan = __int_as_float(0x7fc00000);
-    float4 *tp4 = s_p4[D == 3 ? warp : 0];
-    float2 *tp2 = s_p2[D == 2 ? warp : 0];
-    int *tix = s_ix[D == 2 ? warp : 0];
-    for (int k = lane; k < WT_TILE + 4; k += 32) {          // the tile starts inert
-        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
-        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
-    }
-    Lane L;
-    L.rl = s_rl + threadIdx.x;
-    L.cnt = 0;
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s - lane >= N) return;                     // whole warp past the end
-    const int sc = min(s, N - 1);
-    bool query = s < N;
-    if (MODE != 0) {
-        query = query && mark[sc] != 0;
-        if (query) mark[sc] = 0;                   // the marks are all zero again when the sweep ends
-    }
     if (!__any_sync(0xffffffffu, query)) return;
     Qry q;
     q.z = 0.f;
@@ -1040,6 +1022,89 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
     store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
 }
 
+// MODE 0: A3, thread t serves slot t.  MODE 1 / 2: the slot sweep of A7 on an updated / a fresh grid.  A
+// warp of the sweep owns 32 * SW_WORDS consecutive slots and serves the marked ones among them 32 at a
+// time, in slot order (the k-th marked slot goes to lane k mod 32 of round k / 32): every round runs
+// with full lanes whatever the frontier's density, and its queries are still neighbours in the sorted
+// arrays, which is all the tile passes need.  The marks are cleared on the way (all zero between calls).
+template <int D, int MODE>
+__global__ void __launch_bounds__(32 * LT_WARPS, LT_MIN_BLOCKS)
+search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t *mark,
+                   const int32_t *__restrict__ nF, int sweep_div, int32_t *nn, int32_t *nn2, float *d1,
+                   float *d2, float *c)
+{
+    __shared__ __align__(16) float4 s_p4[D == 3 ? LT_WARPS : 1][D == 3 ? WT_TILE + 4 : 1];
+    __shared__ __align__(16) float2 s_p2[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int s_ix[D == 2 ? LT_WARPS : 1][D == 2 ? WT_TILE + 4 : 1];
+    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
+    if (MODE != 0 && (int64_t)*nF * sweep_div < N) return;
+    // the sweep has two instantiations, both launched; the frontier's density decides which one runs
+    if (MODE != 0 && (sweep_words(N, *nF) == 1) != (MODE <= 2)) return;
+    const bool chains = (MODE == 1 || MODE == 3) && ctr->n_misfiled > 0;     // MODE 2, 4: a fresh grid has no chains (compile-time)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float qnan = __int_as_float(0x7fc00000);
+    float4 *tp4 = s_p4[D == 3 ? warp : 0];
+    float2 *tp2 = s_p2[D == 2 ? warp : 0];
+    int *tix = s_ix[D == 2 ? warp : 0];
+    for (int k = lane; k < WT_TILE + 4; k += 32) {          // the tile starts inert
+        if (D == 3) tp4[k] = make_float4(qnan, qnan, qnan, __int_as_float(-1));
+        else { tp2[k] = make_float2(qnan, qnan); tix[k] = -1; }
+    }
+    Lane L;
+    L.rl = s_rl + threadIdx.x;
+    L.cnt = 0;
+    if (MODE <= 2) {
+        const int s = blockIdx.x * blockDim.x + threadIdx.x;
+        if (s - lane >= N) return;                 // whole warp past the end
+        const int sc = min(s, N - 1);
+        bool query = s < N;
+        if (MODE != 0) {
+            query = query && mark[sc] != 0;
+            if (query) mark[sc] = 0;               // the marks are all zero again when the sweep ends
+        }
+        leaf_search_round<D, MODE>(v, N, ctr, chains, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
+        return;
+    }
+    // (the sweep's bookkeeping lives in shared memory: nothing of it stays in registers across a round)
+    __shared__ unsigned s_mask[LT_WARPS][SW_WORDS];
+    __shared__ int s_tot[LT_WARPS], s_r0[LT_WARPS], s_sw[LT_WARPS];
+    {
+        const int sw = sweep_words(N, *nF);
+        const int wbase = (blockIdx.x * LT_WARPS + warp) * (32 * sw);
+        if (wbase >= N) return;
+        int total = 0;
+        for (int k = 0; k < sw; ++k) {
+            const int s = wbase + 32 * k + lane;
+            const bool mk = s < N && mark[s] != 0;
+            if (mk) mark[s] = 0;                   // the marks are all zero again when the sweep ends
+            const unsigned b = __ballot_sync(0xffffffffu, mk);
+            if (lane == 0) s_mask[warp][k] = b;
+            total += __popc(b);
+        }
+        if (lane == 0) { s_tot[warp] = total; s_r0[warp] = 0; s_sw[warp] = sw; }
+        __syncwarp();
+    }
+#pragma unroll 1
+    for (;;) {
+        const int r0 = s_r0[warp], total = s_tot[warp], sw = s_sw[warp];
+        if (r0 >= total) break;
+        const int wbase = (blockIdx.x * LT_WARPS + warp) * (32 * sw);
+        int t = r0 + lane, sc = wbase;
+        const bool query = t < total;
+        for (int k = 0; k < sw; ++k) {
+            const unsigned b = s_mask[warp][k];
+            const int cnt = __popc(b);
+            if (query && t >= 0 && t < cnt) sc = wbase + 32 * k + (int)__fns(b, 0, t + 1);
+            t -= cnt;
+        }
+        __syncwarp();
+        if (lane == 0) s_r0[warp] = r0 + 32;
+        __syncwarp();
+        leaf_search_round<D, MODE>(v, N, ctr, chains, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
+        __syncwarp();
+    }
+}
+
 // A7, large frontier: stamp the slots of the frontier points with this call's epoch; frontier
 // points that live in an overflow chain have no slot and go to the list kernel (list2).
 __global__ void __launch_bounds__(256)
@@ -1159,7 +1224,9 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
 
 // The list kernel is the last reader of list2 (the chain residents of a swept frontier): the block
 // that finishes last empties the list, so that every kc_frontier_search call starts from an empty
-// one whatever preceded it (every block has read the count before it takes its ticket).
+// one whatever preceded it (every block has read the count before it takes its ticket).  Only a
+// call whose frontier was swept can have filled the list, so only such a call takes tickets (one
+// atomic per block on one address: 17 us for 4,736 blocks).
 __device__ __forceinline__ void list2_done(Counters *ctr)
 {
     __syncthreads();
@@ -1199,7 +1266,7 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
             if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
             store_cert(best, i, nn, nn2, d1, d2, c);
         }
-        list2_done(ctr);
+        if (swept) list2_done(ctr);
         return;
     }
     for (int f = w0; f < n; f += nw) {
@@ -1213,7 +1280,7 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
             store_cert(best, i, nn, nn2, d1, d2, c);
         }
     }
-    list2_done(ctr);
+    if (swept) list2_done(ctr);
 }
 
 // ---- NEXT #4: K-list certificates through the grid ---------------------------------------------
@@ -1588,17 +1655,26 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     const int sweep_div = N >= SWEEP_MIN_N && nF_max * (int64_t)SWEEP_DIV >= N ? SWEEP_DIV : 0;
     if (sweep_div > 0) {
         mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->list2, g->ctr);
-        const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
         // a grid that is fresh (built or re-binned, not updated incrementally) has no tombstones and
-        // no chains: the sweep then is the whole-set kernel with a query mask
+        // no chains: the sweep then is the whole-set kernel with a query mask.  d = 3: two launches, of
+        // which the device runs one: a frontier of more than 45 % of the points is served slot by slot,
+        // a thinner one by the compacting instantiation (a warp owns >= 64 slots there: a smaller grid).
+        // (d = 2: compaction measured no gain on the row-segment kernel, 0.43 vs 0.45 ms at 12.5 %.)
+        const int tb = 32 * WT_WARPS, nbt = (n + tb - 1) / tb;
+        const int nb = (n + PS_THREADS - 1) / PS_THREADS, nb2 = (n + 2 * PS_THREADS - 1) / (2 * PS_THREADS);
         if (g->geom.d == 2) {
-            if (g->dirty) search_tiled_kernel<2, true, false><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
-            else search_tiled_kernel<2, true, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            if (g->dirty) search_tiled_kernel<2, true, false><<<nbt, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            else search_tiled_kernel<2, true, true><<<nbt, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         } else {
-            if (g->dirty) search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
-            else search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            if (g->dirty) {
+                search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+                search_leaf_kernel<3, 3><<<nb2, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            } else {
+                search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+                search_leaf_kernel<3, 4><<<nb2, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+            }
         }
-        count_launches(2);
+        count_launches(g->geom.d == 2 ? 2 : 3);
     }
     int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
     if (nF_max > WPQ_MAX) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
