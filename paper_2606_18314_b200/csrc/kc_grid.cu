@@ -452,7 +452,8 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
         sidx[N + i] = -1;
     }
     if (i >= N) return;
-    const int leaf = ctr->n_heavy ? leafid[i] : cell[i];
+    // (inputs are read once: streaming loads, so that they do not push the sorted arrays out of L2)
+    const int leaf = ctr->n_heavy ? __ldcs(leafid + i) : __ldcs(cell + i);
     int s = atomicAdd(&leaf_start[leaf + 1], 1);
     // The sorted arrays are written at random slots, a fraction of a 32-byte sector at a time: the
     // stores ask L2 to keep their sectors (evict_last) so that a sector is completed in L2 and
@@ -460,15 +461,15 @@ scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ c
     unsigned long long pol;
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
     if (D == 2) {
-        const float2 r = reinterpret_cast<const float2 *>(p)[i];
+        const float2 r = __ldcs(reinterpret_cast<const float2 *>(p) + i);
         asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(spos2 + s), "f"(r.x), "f"(r.y), "l"(pol) : "memory");
         asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(sidx + s), "r"(i), "l"(pol) : "memory");
     } else {
-        const float x = p[3 * (int64_t)i], y = p[3 * (int64_t)i + 1], z = p[3 * (int64_t)i + 2];
+        const float x = __ldcs(p + 3 * (int64_t)i), y = __ldcs(p + 3 * (int64_t)i + 1), z = __ldcs(p + 3 * (int64_t)i + 2);
         asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(spos4 + s), "f"(x), "f"(y), "f"(z),
                      "f"(__int_as_float(i)), "l"(pol) : "memory");   // d = 3: the id travels in the record's fourth word
     }
-    slot[i] = s;
+    __stcs(slot + i, s);
 }
 
 // ------------------------------------------------------------------ A6 incremental update

@@ -1666,15 +1666,18 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
             if (g->dirty) search_tiled_kernel<2, true, false><<<nbt, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
             else search_tiled_kernel<2, true, true><<<nbt, tb, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
         } else {
+            // (a list buffer too short for the direct kernel's density does not launch it)
+            const bool direct = 20 * nF_max > 9 * N;
             if (g->dirty) {
-                search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+                if (direct) search_leaf_kernel<3, 1><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
                 search_leaf_kernel<3, 3><<<nb2, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
             } else {
-                search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
+                if (direct) search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
                 search_leaf_kernel<3, 4><<<nb2, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
             }
+            count_launches(direct ? 1 : 0);
         }
-        count_launches(g->geom.d == 2 ? 2 : 3);
+        count_launches(2);
     }
     int blocks = blocks_for(nF_max, 4, 148 * 16);          // short list: one warp per query
     if (nF_max > WPQ_MAX) blocks = max(blocks, blocks_for(nF_max, 128, 148 * 32));
