@@ -44,16 +44,17 @@ template <int D>
 __device__ __noinline__ Top2 slow_offer4(const View &v, Top2 best, int t, float s0, float s1,
                                          float s2, float s3, int self)
 {
-    if (D == 2) {
-        if (s0 <= best.s2) offer_once(best, s0, v.sidx[t + 0], self);
-        if (s1 <= best.s2) offer_once(best, s1, v.sidx[t + 1], self);
-        if (s2 <= best.s2) offer_once(best, s2, v.sidx[t + 2], self);
-        if (s3 <= best.s2) offer_once(best, s3, v.sidx[t + 3], self);
-    } else {
-        if (s0 <= best.s2) offer_once(best, s0, __float_as_int(v.spos4[t + 0].w), self);
-        if (s1 <= best.s2) offer_once(best, s1, __float_as_int(v.spos4[t + 1].w), self);
-        if (s2 <= best.s2) offer_once(best, s2, __float_as_int(v.spos4[t + 2].w), self);
-        if (s3 <= best.s2) offer_once(best, s3, __float_as_int(v.spos4[t + 3].w), self);
+    // the smallest of the four first, retired with NaN (fminf skips it), until none qualifies: the
+    // lanes on this path stay in step whichever of their four candidates it is about
+    float m = fminf(fminf(s0, s1), fminf(s2, s3));
+    while (m <= best.s2) {
+        const bool p0 = s0 == m, p1 = !p0 && s1 == m, p2 = !p0 && !p1 && s2 == m;
+        const int k = p0 ? 0 : (p1 ? 1 : (p2 ? 2 : 3));
+        const float qn = __int_as_float(0x7fc00000);
+        s0 = p0 ? qn : s0; s1 = p1 ? qn : s1; s2 = p2 ? qn : s2; s3 = (p0 || p1 || p2) ? s3 : qn;
+        const int j = D == 2 ? v.sidx[t + k] : __float_as_int(v.spos4[t + k].w);
+        offer_once(best, m, j, self);
+        m = fminf(fminf(s0, s1), fminf(s2, s3));
     }
     return best;
 }
@@ -487,10 +488,17 @@ __device__ __forceinline__ void tile_scan(const float2 *tp2, const float4 *tp4, 
         float m = fminf(fminf(s0, s1), fminf(s2, s3));
         if (m <= best.s2) {
             if (D == 2) { j0 = tidx[t]; j1 = tidx[t + 1]; j2 = tidx[t + 2]; j3 = tidx[t + 3]; }
-            offer_once(best, s0, j0, self);
-            offer_once(best, s1, j1, self);
-            offer_once(best, s2, j2, self);
-            offer_once(best, s3, j3, self);
+            // Usually one of the four qualifies: offer the smallest, retire it (NaN: fminf skips it),
+            // and look again.  Every lane on this path runs the same instructions whichever of its four
+            // candidates it is about; the top-2 does not depend on the order of the offers.
+            do {
+                const bool p0 = s0 == m, p1 = !p0 && s1 == m, p2 = !p0 && !p1 && s2 == m;
+                const int jm = p0 ? j0 : (p1 ? j1 : (p2 ? j2 : j3));
+                const float qn = __int_as_float(0x7fc00000);
+                s0 = p0 ? qn : s0; s1 = p1 ? qn : s1; s2 = p2 ? qn : s2; s3 = (p0 || p1 || p2) ? s3 : qn;
+                offer_once(best, m, jm, self);
+                m = fminf(fminf(s0, s1), fminf(s2, s3));
+            } while (m <= best.s2);
         }
     }
 }
