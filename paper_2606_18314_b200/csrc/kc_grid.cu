@@ -51,11 +51,14 @@ __device__ __forceinline__ void zero_i32(int32_t *a, int64_t n, int64_t t0, int6
 }
 __global__ void __launch_bounds__(256)
 build_prep_kernel(const int32_t *__restrict__ mlist, const int32_t *__restrict__ cell, int32_t *head,
-                  Counters *ctr, int32_t *counts, int n_cells, int32_t *leaf_cnt, int64_t n_leaves_max)
+                  Counters *ctr, int32_t *counts, int n_cells, int32_t *leaf_cnt, int64_t n_leaves_max,
+                  unsigned long long *desc, int n_desc)
 {
     const int n = ctr->n_misfiled;
     const int64_t t0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x, nt = (int64_t)gridDim.x * blockDim.x;
     for (int64_t e = t0; e < n; e += nt) head[cell[mlist[e]]] = -1;
+    for (int64_t k = t0; k < n_desc; k += nt) desc[k] = 0ull;       // the scans' descriptors and tickets
+    if (t0 == 0) { ctr->scan_ticket = 0; ctr->lscan_ticket = 0; }
     zero_i32(counts, n_cells, t0, nt);
     zero_i32(leaf_cnt, n_leaves_max, t0, nt);
 }
@@ -114,61 +117,44 @@ __device__ __forceinline__ int2 block_excl_scan2(int a, int b, int2 *wsum)
     return make_int2(off.x + ia - a, off.y + ib - b);
 }
 
+// ---- scans in one pass (decoupled look-back) ----------------------------------------------------
+// A scan block takes a ticket (blocks with smaller tickets are running or done, so waiting for them
+// cannot deadlock), publishes the sums of its chunk, and adds up its predecessors' descriptors until
+// it meets one that already carries an inclusive prefix.  A descriptor is one 64-bit word -- state
+// (0 nothing yet, 1 the block's own sums, 2 inclusive prefix) in the top two bits, two 31-bit sums
+// below -- so a single volatile load or store moves state and values together (no fence needed).
+// build_prep_kernel zeroes the descriptors and the tickets.
+__device__ __forceinline__ unsigned long long desc_pack(int st, int a, int b)
+{
+    return ((unsigned long long)st << 62) | ((unsigned long long)(unsigned)a << 31) | (unsigned long long)(unsigned)b;
+}
+// Called by all 32 lanes of ONE warp of the block: exclusive prefix of block `bid` whose own sums are (a, b).
+__device__ __forceinline__ int2 scan_lookback(volatile unsigned long long *desc, int bid, int a, int b)
+{
+    const int lane = threadIdx.x & 31;
+    if (bid == 0) {
+        if (lane == 0) desc[0] = desc_pack(2, a, b);
+        return make_int2(0, 0);
+    }
+    if (lane == 0) desc[bid] = desc_pack(1, a, b);
+    int ra = 0, rb = 0;
+    for (int look = bid - 1;; look -= 32) {
+        const int idx = look - lane;               // lane 0 reads the nearest predecessor
+        unsigned long long dsc;
+        do {
+            dsc = idx >= 0 ? desc[idx] : desc_pack(2, 0, 0);
+        } while (__any_sync(0xffffffffu, (dsc >> 62) == 0));
+        const unsigned full = __ballot_sync(0xffffffffu, (dsc >> 62) == 2);
+        const bool take = !full || lane <= __ffs(full) - 1;
+        ra += __reduce_add_sync(0xffffffffu, take ? (int)((dsc >> 31) & 0x7fffffffu) : 0);
+        rb += __reduce_add_sync(0xffffffffu, take ? (int)(dsc & 0x7fffffffu) : 0);
+        if (full) break;
+    }
+    if (lane == 0) desc[bid] = desc_pack(2, ra + a, rb + b);
+    return make_int2(ra, rb);
+}
+
 // ---- scan over the cells: {records, leaves} --------------------------------------------------
-__global__ void __launch_bounds__(256)
-scan_reduce_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ, int2 *blocksums,
-                   Counters *ctr)
-{
-    int base = blockIdx.x * SCAN_CHUNK;
-    int sum = 0, lv = 0, occ = 0, mx = 0, hv = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
-        int idx = base + k * 256 + threadIdx.x;
-        if (idx < n_cells) {
-            const int cnt = counts[idx];
-            const int S = sub_res(cnt, d, heavy_T, sub_occ);
-            sum += cnt; occ += cnt > 0; mx = max(mx, cnt);
-            lv += S ? ipow_d(S, d) : 1; hv += S > 0;
-        }
-    }
-    sum = __reduce_add_sync(0xffffffffu, sum);
-    lv = __reduce_add_sync(0xffffffffu, lv);
-    occ = __reduce_add_sync(0xffffffffu, occ);
-    hv = __reduce_add_sync(0xffffffffu, hv);
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    __shared__ int s_sum[8], s_lv[8], s_occ[8], s_mx[8], s_hv[8];
-    int w = threadIdx.x >> 5;
-    if ((threadIdx.x & 31) == 0) { s_sum[w] = sum; s_lv[w] = lv; s_occ[w] = occ; s_mx[w] = mx; s_hv[w] = hv; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int a = 0, l = 0, b = 0, c = 0, e = 0;
-        for (int k = 0; k < 8; ++k) { a += s_sum[k]; l += s_lv[k]; b += s_occ[k]; c = max(c, s_mx[k]); e += s_hv[k]; }
-        blocksums[blockIdx.x] = make_int2(a, l);
-        if (b) atomicAdd(&ctr->c_occ, b);
-        if (e) atomicAdd(&ctr->n_heavy, e);
-        atomicMax(&ctr->max_occ, c);
-    }
-}
-// exclusive scan of blocksums[0..nb) in place (both components), one CTA of 1024 threads, carry
-// across segments; the total of the second component goes to *total_y if given
-__global__ void __launch_bounds__(1024) scan_blocksums_kernel(int2 *blocksums, int nb, int *total_y)
-{
-    __shared__ int2 wsum[32];
-    __shared__ int2 carry_s;
-    if (threadIdx.x == 0) carry_s = make_int2(0, 0);
-    __syncthreads();
-    for (int base = 0; base < nb; base += 1024) {
-        const int idx = base + threadIdx.x;
-        const int2 v = idx < nb ? blocksums[idx] : make_int2(0, 0);
-        const int2 e = block_excl_scan2(v.x, v.y, wsum);
-        const int2 carry = carry_s;
-        if (idx < nb) blocksums[idx] = make_int2(carry.x + e.x, carry.y + e.y);
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = make_int2(carry.x + e.x + v.x, carry.y + e.y + v.y);
-        __syncthreads();
-    }
-    if (threadIdx.x == 0 && total_y) *total_y = carry_s.y;
-}
 // One cell of the scan's output.  With a subdivided cell anywhere in the grid: subinfo and, for an
 // undivided cell, the size of its single leaf (the leaf scan follows).  Without one: leaf = cell,
 // so the scatter cursor is written straight away (leaf_start[c + 1] = start of c).
@@ -184,19 +170,25 @@ __device__ __forceinline__ void scan_emit(int c, int cnt, int S, int run, int lr
         leaf_start[c + 1] = run;
     }
 }
+// Thread t owns 8 consecutive cells of the block's chunk; the chunk goes through shared memory both
+// ways so that the global loads and stores are coalesced.  Whether any cell of the grid is
+// subdivided is not known before the last block is done, so with the second level enabled a cell
+// gets both forms of its output: {cell_start, scatter cursor} for a grid without subdivided cells
+// (leaf = cell) and {subinfo, size of the single leaf of an undivided cell} for one with; the leaf
+// scan, which runs only in the second case, overwrites every cursor (n_leaves >= n_cells).
 __global__ void __launch_bounds__(256)
-scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ,
-                  const int2 *__restrict__ blocksums, int32_t *__restrict__ cell_start,
-                  int2 *__restrict__ subinfo, int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start,
-                  const Counters *ctr, int N)
+scan_cells_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ, bool two_level,
+                  unsigned long long *desc, int32_t *__restrict__ cell_start, int2 *__restrict__ subinfo,
+                  int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start, Counters *ctr, int N)
 {
-    // thread t owns 8 consecutive cells of the block's chunk; the chunk goes through shared memory both
-    // ways so that the global loads and stores are coalesced
     __shared__ int2 wsum[32];
     __shared__ int s_cnt[SCAN_CHUNK];              // counts in, starts out
     __shared__ int2 s_sub[SCAN_CHUNK];
-    const bool any_heavy = ctr->n_heavy > 0;
-    const int cbase = blockIdx.x * SCAN_CHUNK;
+    __shared__ int s_bid;
+    __shared__ int2 s_agg, s_pre;
+    if (threadIdx.x == 0) s_bid = atomicAdd(&ctr->scan_ticket, 1);
+    __syncthreads();
+    const int bid = s_bid, cbase = bid * SCAN_CHUNK;
 #pragma unroll
     for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
         const int c = cbase + k * 256 + threadIdx.x;
@@ -205,25 +197,40 @@ scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int he
     __syncthreads();
     const int lbase = threadIdx.x * 8, base = cbase + lbase;
     int v[8], S[8];
-    int tsum = 0, tl = 0;
+    int tsum = 0, tl = 0, occ = 0, mx = 0, hv = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         v[k] = s_cnt[lbase + k];
         S[k] = sub_res(v[k], d, heavy_T, sub_occ);
-        tsum += v[k];
+        tsum += v[k]; occ += v[k] > 0; mx = max(mx, v[k]); hv += S[k] > 0;
         tl += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
     }
     const int2 e = block_excl_scan2(tsum, tl, wsum);      // (syncs: every thread has read its counts)
-    const int2 off = blocksums[blockIdx.x];
+    if (threadIdx.x == 255) s_agg = make_int2(e.x + tsum, e.y + tl);
+    occ = __reduce_add_sync(0xffffffffu, occ);
+    hv = __reduce_add_sync(0xffffffffu, hv);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0) {
+        if (occ) atomicAdd(&ctr->c_occ, occ);
+        if (hv) atomicAdd(&ctr->n_heavy, hv);
+        if (mx) atomicMax(&ctr->max_occ, mx);
+    }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int2 pre = scan_lookback(desc, bid, s_agg.x, s_agg.y);
+        if (threadIdx.x == 0) s_pre = pre;
+    }
+    __syncthreads();
+    const int2 off = s_pre;
     int run = off.x + e.x, lrun = off.y + e.y;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         s_cnt[lbase + k] = run;
         s_sub[lbase + k] = make_int2(S[k], lrun);
         // an undivided cell of a grid with subdivided cells is one leaf of that size
-        if (any_heavy && !S[k] && base + k < n_cells) leaf_cnt[lrun] = v[k];
+        if (two_level && !S[k] && base + k < n_cells) leaf_cnt[lrun] = v[k];
         run += v[k];
-        lrun += S[k] ? ipow_d(S[k], d) : 1;
+        lrun += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
     }
     __syncthreads();
 #pragma unroll
@@ -232,11 +239,12 @@ scan_write_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int he
         if (c < n_cells) {
             const int st = s_cnt[k * 256 + threadIdx.x];
             cell_start[c] = st;
-            if (any_heavy) subinfo[c] = s_sub[k * 256 + threadIdx.x];
-            else leaf_start[c + 1] = st;           // leaf = cell: the scatter's cursor straight away
+            leaf_start[c + 1] = st;                // leaf = cell: the scatter's cursor straight away
+            if (two_level) subinfo[c] = s_sub[k * 256 + threadIdx.x];
         }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (threadIdx.x == 255 && cbase + SCAN_CHUNK >= n_cells && cbase < n_cells) {   // the last chunk
+        ctr->n_leaves = lrun;
         cell_start[n_cells] = N;
         leaf_start[0] = 0;
     }
@@ -325,56 +333,19 @@ leafid_hist_kernel(View v, const float *__restrict__ p, int N, const int32_t *__
 }
 
 // ---- scan over the leaves: leaf_start[l + 1] = start of leaf l (the scatter's cursor) ----------
+// One pass, as above (second component unused); blocks behind the last leaf leave at once.
 __global__ void __launch_bounds__(256)
-lscan_reduce_kernel(const int32_t *__restrict__ leaf_cnt, int2 *blocksums, const Counters *ctr)
-{
-    if (ctr->n_heavy == 0) return;
-    const int n = ctr->n_leaves;
-    const int base = blockIdx.x * SCAN_CHUNK;
-    if (base >= n) { if (threadIdx.x == 0) blocksums[blockIdx.x] = make_int2(0, 0); return; }
-    int sum = 0;
-#pragma unroll
-    for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
-        const int idx = base + k * 256 + threadIdx.x;
-        sum += idx < n ? leaf_cnt[idx] : 0;
-    }
-    sum = __reduce_add_sync(0xffffffffu, sum);
-    __shared__ int s_sum[8];
-    if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = sum;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int a = 0;
-        for (int k = 0; k < 8; ++k) a += s_sum[k];
-        blocksums[blockIdx.x] = make_int2(a, 0);
-    }
-}
-__global__ void __launch_bounds__(1024) lscan_blocksums_kernel(int2 *blocksums, int nb, const Counters *ctr)
-{
-    if (ctr->n_heavy == 0) return;
-    __shared__ int2 wsum[32];
-    __shared__ int carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int base = 0; base < nb; base += 1024) {
-        const int idx = base + threadIdx.x;
-        const int v = idx < nb ? blocksums[idx].x : 0;
-        const int2 e = block_excl_scan2(v, 0, wsum);
-        const int carry = carry_s;
-        if (idx < nb) blocksums[idx].x = carry + e.x;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + e.x + v;
-        __syncthreads();
-    }
-}
-__global__ void __launch_bounds__(256)
-lscan_write_kernel(const int32_t *__restrict__ leaf_cnt, const int2 *__restrict__ blocksums,
-                   int32_t *__restrict__ leaf_start, const Counters *ctr)
+lscan_kernel(const int32_t *__restrict__ leaf_cnt, unsigned long long *desc, int32_t *__restrict__ leaf_start,
+             Counters *ctr)
 {
     if (ctr->n_heavy == 0) return;
     __shared__ int2 wsum[32];
     __shared__ int s_cnt[SCAN_CHUNK];              // sizes in, starts out (coalesced both ways)
+    __shared__ int s_bid, s_agg, s_pre;
+    if (threadIdx.x == 0) s_bid = atomicAdd(&ctr->lscan_ticket, 1);
+    __syncthreads();
     const int n = ctr->n_leaves;
-    const int cbase = blockIdx.x * SCAN_CHUNK;
+    const int bid = s_bid, cbase = bid * SCAN_CHUNK;
     if (cbase >= n) return;
 #pragma unroll
     for (int k = 0; k < SCAN_CHUNK / 256; ++k) {
@@ -391,7 +362,14 @@ lscan_write_kernel(const int32_t *__restrict__ leaf_cnt, const int2 *__restrict_
         tsum += v[k];
     }
     const int2 e = block_excl_scan2(tsum, 0, wsum);
-    int run = blocksums[blockIdx.x].x + e.x;
+    if (threadIdx.x == 255) s_agg = e.x + tsum;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        const int2 pre = scan_lookback(desc, bid, s_agg, 0);
+        if (threadIdx.x == 0) s_pre = pre.x;
+    }
+    __syncthreads();
+    int run = s_pre + e.x;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         s_cnt[lbase + k] = run;
@@ -776,7 +754,7 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     alloc((void **)&g->head, nc * 4); alloc((void **)&g->next, n * 4);
     alloc((void **)&g->mlist, n * 4); alloc((void **)&g->fcount, nc * 4);
     alloc((void **)&g->mhist, MHIST * 4);
-    alloc((void **)&g->blocksums, ((size_t)g->n_scan_blocks + 1) * sizeof(int2));
+    alloc((void **)&g->scan_desc, (2 * (size_t)g->n_scan_blocks + 2) * sizeof(unsigned long long));
     alloc((void **)&g->subinfo, nc * sizeof(int2));
     alloc((void **)&g->leaf_cnt, (size_t)g->n_leaves_max * 4);
     alloc((void **)&g->leaf_start, ((size_t)g->n_leaves_max + 1) * 4);
@@ -818,7 +796,7 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
     void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
-                    g->mlist, g->fcount, g->mhist, g->blocksums, g->subinfo, g->leaf_cnt, g->leaf_start, g->leafid, g->mark, g->list2, g->handoff, g->handoff_part, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
+                    g->mlist, g->fcount, g->mhist, g->scan_desc, g->subinfo, g->leaf_cnt, g->leaf_start, g->leafid, g->mark, g->list2, g->handoff, g->handoff_part, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete g;
@@ -854,8 +832,10 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     const bool two_level = T != KC_INDEX_OFF;             // off: the leaves are the cells, no second pass
     const int64_t nl_max = two_level ? (int64_t)nc + N + 8 : 0;
     const int ncb = (nc + SCAN_CHUNK - 1) / SCAN_CHUNK, nlb = (int)((nl_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
+    unsigned long long *desc_c = g->scan_desc, *desc_l = g->scan_desc + ncb;
     build_prep_kernel<<<blocks_for((nl_max > nc ? nl_max : nc) / 4 + 1, 256, 148 * 8), 256, 0, st>>>(g->mlist, g->cell, g->head, g->ctr,
-                                                                              g->counts, nc, g->leaf_cnt, nl_max);
+                                                                              g->counts, nc, g->leaf_cnt, nl_max,
+                                                                              g->scan_desc, ncb + nlb);
     if (d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     if (nc <= SCAN_SMALL_MAX) {
@@ -863,11 +843,9 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
                                               g->leaf_start, g->ctr, n);
         count_launches(1);
     } else {
-        scan_reduce_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, g->blocksums, g->ctr);
-        scan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, ncb, &g->ctr->n_leaves);
-        scan_write_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, g->blocksums, g->cell_start, g->subinfo,
+        scan_cells_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, two_level, desc_c, g->cell_start, g->subinfo,
                                                g->leaf_cnt, g->leaf_start, g->ctr, n);
-        count_launches(3);
+        count_launches(1);
     }
     // second level (these kernels leave at once when no cell is subdivided)
     if (!two_level) {
@@ -879,10 +857,8 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
         lscan_small_kernel<<<1, 1024, 0, st>>>(g->leaf_cnt, g->leaf_start, g->ctr);
         count_launches(1);
     } else {
-        lscan_reduce_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, g->blocksums, g->ctr);
-        lscan_blocksums_kernel<<<1, 1024, 0, st>>>(g->blocksums, nlb, g->ctr);
-        lscan_write_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, g->blocksums, g->leaf_start, g->ctr);
-        count_launches(3);
+        lscan_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, desc_l, g->leaf_start, g->ctr);
+        count_launches(1);
     }
     if (d == 2)
         scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->leafid, g->leaf_start, g->ctr, g->spos2,

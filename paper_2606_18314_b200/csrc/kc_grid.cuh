@@ -24,6 +24,8 @@ struct Counters {
     int n_handoff;            // queries in the hand-off list of the search in progress (zero between calls)
     int ticket3;              // blocks of the hand-off kernel that are done (the last one empties the list)
     int n_handed;             // queries handed to the brute-force pass since the last build
+    int scan_ticket;          // block order of the cell scan / the leaf scan of the build in progress
+    int lscan_ticket;
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -99,7 +101,7 @@ struct kc_grid {
     int built, dirty;
     size_t bytes;
     int32_t *cell, *counts, *cell_start, *sidx, *slot, *head, *next, *mlist, *fcount, *mhist;
-    int2 *blocksums;          // per scan block: {records, leaves} (cell scan) / {records, -} (leaf scan)
+    unsigned long long *scan_desc;   // look-back descriptors of the build's two scans (cells, then leaves)
     int2 *subinfo;            // two-level index, see View
     int32_t *leaf_cnt, *leaf_start, *leafid;   // leaf sizes, their scan (doubles as scatter cursors), leaf of point i
     int64_t n_leaves_max;
