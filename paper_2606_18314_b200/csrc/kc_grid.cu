@@ -26,7 +26,6 @@ namespace {
 
 constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
 constexpr int SCAN_CHUNK = 2048;   // entries per scan block (256 threads x 8)
-constexpr int SCAN_SMALL_MAX = 16384;   // up to this many entries a scan is one CTA (1024 threads x 16)
 constexpr int64_t REBIN_MIN_N = 100000, REBIN_DIV = 8;   // A6: when an update re-bins instead of re-filing
 
 // ------------------------------------------------------------------ A2 build
@@ -155,21 +154,6 @@ __device__ __forceinline__ int2 scan_lookback(volatile unsigned long long *desc,
 }
 
 // ---- scan over the cells: {records, leaves} --------------------------------------------------
-// One cell of the scan's output.  With a subdivided cell anywhere in the grid: subinfo and, for an
-// undivided cell, the size of its single leaf (the leaf scan follows).  Without one: leaf = cell,
-// so the scatter cursor is written straight away (leaf_start[c + 1] = start of c).
-__device__ __forceinline__ void scan_emit(int c, int cnt, int S, int run, int lrun, bool any_heavy,
-                                          int32_t *cell_start, int2 *subinfo, int32_t *leaf_cnt,
-                                          int32_t *leaf_start)
-{
-    cell_start[c] = run;
-    if (any_heavy) {
-        subinfo[c] = make_int2(S, lrun);
-        if (!S) leaf_cnt[lrun] = cnt;
-    } else {
-        leaf_start[c + 1] = run;
-    }
-}
 // Thread t owns 8 consecutive cells of the block's chunk; the chunk goes through shared memory both
 // ways so that the global loads and stores are coalesced.  Whether any cell of the grid is
 // subdivided is not known before the last block is done, so with the second level enabled a cell
@@ -249,59 +233,6 @@ scan_cells_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int he
         leaf_start[0] = 0;
     }
 }
-// Small grids: the whole cell scan in one CTA (thread t owns 16 consecutive cells).
-__global__ void __launch_bounds__(1024)
-scan_small_kernel(const int32_t *__restrict__ counts, int n_cells, int d, int heavy_T, int sub_occ,
-                  int32_t *__restrict__ cell_start, int2 *__restrict__ subinfo, int32_t *__restrict__ leaf_cnt,
-                  int32_t *__restrict__ leaf_start, Counters *ctr, int N)
-{
-    __shared__ int2 wsum[32];
-    __shared__ int s_heavy;
-    const int base = threadIdx.x * 16;
-    int v[16], S[16];
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {                 // all loads issued before the first is used
-        const int i = base + 4 * q;
-        int4 x = make_int4(0, 0, 0, 0);
-        if (i + 3 < n_cells) x = *reinterpret_cast<const int4 *>(counts + i);
-        else if (i < n_cells) {
-            x.x = counts[i];
-            if (i + 1 < n_cells) x.y = counts[i + 1];
-            if (i + 2 < n_cells) x.z = counts[i + 2];
-        }
-        v[4 * q] = x.x; v[4 * q + 1] = x.y; v[4 * q + 2] = x.z; v[4 * q + 3] = x.w;
-    }
-    int tsum = 0, tl = 0, occ = 0, mx = 0, hv = 0;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        S[k] = sub_res(v[k], d, heavy_T, sub_occ);
-        tsum += v[k]; occ += v[k] > 0; mx = max(mx, v[k]); hv += S[k] > 0;
-        tl += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
-    }
-    if (threadIdx.x == 0) s_heavy = 0;
-    const int2 e = block_excl_scan2(tsum, tl, wsum);      // (syncs: s_heavy is visible after it)
-    occ = __reduce_add_sync(0xffffffffu, occ);
-    hv = __reduce_add_sync(0xffffffffu, hv);
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    if ((threadIdx.x & 31) == 0) {
-        if (occ) atomicAdd(&ctr->c_occ, occ);
-        if (hv) { atomicAdd(&ctr->n_heavy, hv); atomicAdd(&s_heavy, hv); }
-        atomicMax(&ctr->max_occ, mx);
-    }
-    __syncthreads();
-    const bool any_heavy = s_heavy > 0;
-    int run = e.x, lrun = e.y;
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-        if (base + k < n_cells)
-            scan_emit(base + k, v[k], S[k], run, lrun, any_heavy, cell_start, subinfo, leaf_cnt, leaf_start);
-        run += v[k];
-        lrun += base + k < n_cells ? (S[k] ? ipow_d(S[k], d) : 1) : 0;
-    }
-    if (threadIdx.x == 1023) ctr->n_leaves = lrun;
-    if (threadIdx.x == 0) { cell_start[n_cells] = N; leaf_start[0] = 0; }
-}
-
 // ---- leaf of every point + leaf histogram (only with subdivided cells) ------------------------
 template <int D>
 __global__ void __launch_bounds__(256)
@@ -382,39 +313,6 @@ lscan_kernel(const int32_t *__restrict__ leaf_cnt, unsigned long long *desc, int
         if (l < n) leaf_start[l + 1] = s_cnt[k * 256 + threadIdx.x];
     }
 }
-// the same in one CTA, any length (small problems: one launch instead of three)
-__global__ void __launch_bounds__(1024)
-lscan_small_kernel(const int32_t *__restrict__ leaf_cnt, int32_t *__restrict__ leaf_start, const Counters *ctr)
-{
-    if (ctr->n_heavy == 0) return;
-    __shared__ int2 wsum[32];
-    __shared__ int carry_s;
-    const int n = ctr->n_leaves;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    for (int c0 = 0; c0 < n; c0 += 1024 * 16) {
-        const int base = c0 + threadIdx.x * 16;
-        int v[16];
-        int tsum = 0;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            v[k] = base + k < n ? leaf_cnt[base + k] : 0;
-            tsum += v[k];
-        }
-        const int2 e = block_excl_scan2(tsum, 0, wsum);
-        const int carry = carry_s;
-        int run = carry + e.x;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) {
-            if (base + k < n) leaf_start[base + k + 1] = run;
-            run += v[k];
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = run;
-        __syncthreads();
-    }
-}
-
 template <int D>
 __global__ void __launch_bounds__(256)
 scatter_kernel(const float *__restrict__ p, int N, const int32_t *__restrict__ cell,
@@ -838,27 +736,13 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
                                                                               g->scan_desc, ncb + nlb);
     if (d == 2) cellid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
     else cellid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->counts, g->ctr);
-    if (nc <= SCAN_SMALL_MAX) {
-        scan_small_kernel<<<1, 1024, 0, st>>>(g->counts, nc, d, T, so, g->cell_start, g->subinfo, g->leaf_cnt,
-                                              g->leaf_start, g->ctr, n);
-        count_launches(1);
-    } else {
-        scan_cells_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, two_level, desc_c, g->cell_start, g->subinfo,
-                                               g->leaf_cnt, g->leaf_start, g->ctr, n);
-        count_launches(1);
-    }
+    scan_cells_kernel<<<ncb, 256, 0, st>>>(g->counts, nc, d, T, so, two_level, desc_c, g->cell_start, g->subinfo,
+                                           g->leaf_cnt, g->leaf_start, g->ctr, n);
     // second level (these kernels leave at once when no cell is subdivided)
-    if (!two_level) {
-    } else if (d == 2) leafid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
-    else leafid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
-    if (!two_level) {
-        count_launches(-1);
-    } else if (nl_max <= 4 * SCAN_SMALL_MAX) {
-        lscan_small_kernel<<<1, 1024, 0, st>>>(g->leaf_cnt, g->leaf_start, g->ctr);
-        count_launches(1);
-    } else {
+    if (two_level) {
+        if (d == 2) leafid_hist_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
+        else leafid_hist_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(v, p, n, g->cell, g->leaf_cnt, g->leafid, g->ctr);
         lscan_kernel<<<nlb, 256, 0, st>>>(g->leaf_cnt, desc_l, g->leaf_start, g->ctr);
-        count_launches(1);
     }
     if (d == 2)
         scatter_kernel<2><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->leafid, g->leaf_start, g->ctr, g->spos2,
@@ -866,7 +750,7 @@ extern "C" kc_status kc_grid_build(kc_grid *g, const float *p, int64_t N, void *
     else
         scatter_kernel<3><<<(n + 255) / 256, 256, 0, st>>>(p, n, g->cell, g->leafid, g->leaf_start, g->ctr, g->spos2,
                                                            g->spos4, g->sidx, g->slot);
-    count_launches(4);
+    count_launches(two_level ? 6 : 4);
     KC_LAUNCH_CHECK("kc_grid_build");
     g->N = N; g->built = 1; g->dirty = 0;
     return KC_OK;
