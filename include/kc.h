@@ -80,6 +80,8 @@ typedef struct {
     int32_t n_leaves;    /* leaves of the last build: undivided cells + sub-cells */
     int32_t heavy_T;     /* build-time record count from which a cell is subdivided */
     int32_t n_handed;    /* queries the ring search handed to the brute-force pass since the last build */
+    int32_t n_deferred;  /* d = 3, grids of >= 100,000 points with subdivided cells: queries that the whole-set
+                          * search / the slot sweep left to their second kernel since the last build */
 } kc_grid_info_t;
 
 /* ---- host utilities -------------------------------------------------------------------- */

@@ -56,7 +56,8 @@ class kc_grid_info_t(C.Structure):
     _fields_ = [("n_points", C.c_int64), ("n_cells", C.c_int64), ("c_occ", C.c_int32),
                 ("max_occ", C.c_int32), ("n_misfiled", C.c_int32), ("built", C.c_int32),
                 ("dirty", C.c_int32), ("n_stragglers", C.c_int32), ("n_heavy", C.c_int32),
-                ("n_leaves", C.c_int32), ("heavy_T", C.c_int32), ("n_handed", C.c_int32)]
+                ("n_leaves", C.c_int32), ("heavy_T", C.c_int32), ("n_handed", C.c_int32),
+                ("n_deferred", C.c_int32)]
 
 
 _lib = None

@@ -70,7 +70,7 @@ cellid_hist_kernel(View v, const float *__restrict__ p, int N, int32_t *__restri
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {          // the chains were dropped by the previous kernel; the scan recounts C
         ctr->n_misfiled = 0; ctr->c_occ = 0; ctr->max_occ = 0; ctr->n_stragglers = 0;
-        ctr->n_list2 = 0; ctr->n_heavy = 0; ctr->n_leaves = 0; ctr->n_handed = 0;
+        ctr->n_list2 = 0; ctr->n_heavy = 0; ctr->n_leaves = 0; ctr->n_handed = 0; ctr->n_deferred = 0;
     }
     if (i >= N) return;
     float x, y, z = 0.f;
@@ -668,6 +668,8 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
     if (geom->d == 2) alloc((void **)&g->spos2, (n + 8) * sizeof(float2));
     else alloc((void **)&g->spos4, (n + 8) * sizeof(float4));
     alloc((void **)&g->opos, n * sizeof(float4));
+    g->defer = nullptr;
+    if (geom->d == 3) alloc((void **)&g->defer, 2 * n * sizeof(float4));
     alloc((void **)&g->ctr, sizeof(Counters));
     if (!ok) {
         kc_grid_destroy(g);
@@ -694,7 +696,7 @@ extern "C" kc_status kc_grid_destroy(kc_grid *g)
 {
     if (!g) return KC_OK;
     void *ptrs[] = {g->cell, g->counts, g->cell_start, g->sidx, g->slot, g->head, g->next,
-                    g->mlist, g->fcount, g->mhist, g->scan_desc, g->subinfo, g->leaf_cnt, g->leaf_start, g->leafid, g->mark, g->list2, g->handoff, g->handoff_part, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->ctr};
+                    g->mlist, g->fcount, g->mhist, g->scan_desc, g->subinfo, g->leaf_cnt, g->leaf_start, g->leafid, g->mark, g->list2, g->handoff, g->handoff_part, g->delta, g->cellmax, g->spos2, g->spos4, g->opos, g->defer, g->ctr};
     for (void *p : ptrs)
         if (p) cudaFree(p);
     delete g;
@@ -855,7 +857,7 @@ extern "C" kc_status kc_grid_info(kc_grid *g, kc_grid_info_t *out, void *stream)
     out->c_occ = h.c_occ; out->max_occ = h.max_occ; out->n_misfiled = h.n_misfiled;
     out->built = g->built; out->dirty = g->dirty; out->n_stragglers = h.n_stragglers; out->n_handed = h.n_handed;
     out->n_heavy = h.n_heavy; out->n_leaves = h.n_heavy ? h.n_leaves : (int32_t)g->n_cells;
-    out->heavy_T = g->heavy_T;
+    out->heavy_T = g->heavy_T; out->n_deferred = h.n_deferred;
     return KC_OK;
 }
 

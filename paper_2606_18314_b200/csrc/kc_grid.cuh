@@ -26,6 +26,10 @@ struct Counters {
     int n_handed;             // queries handed to the brute-force pass since the last build
     int scan_ticket;          // block order of the cell scan / the leaf scan of the build in progress
     int lscan_ticket;
+    int n_defer;              // queries the leaf search has left to its second kernel (zero between calls)
+    int ticket4;              // blocks of that kernel that are done (the last one empties the list)
+    int n_deferred;           // queries served by that kernel since the last build
+    int defer_next;           // next unserved entry of the list (warps of the second kernel take 32 at a time)
     double big;               // sum k ln k over cells with k >= MHIST (rare)
 };
 
@@ -78,6 +82,8 @@ struct View {
     const int32_t *leaf_start;   // exclusive scan of the leaf sizes (n_leaves + 1 entries)
     float4 *handoff;          // hand-off list (x, y, z, bits(id)) of ring_continue, or null: rings without limit
     int *n_handoff;           // its length (Counters::n_handoff)
+    float4 *defer;            // d = 3: queries whose ball reaches beyond what phase 1 of the leaf search served:
+    int *n_defer;             //   two float4 per entry {slot, covered, -, -}, {s1, s2, j1, j2}; length (Counters::n_defer)
 };
 
 // Straggler hand-off: a query whose ring search has scanned radius
@@ -114,6 +120,7 @@ struct kc_grid {
     unsigned *cellmax;        // NEXT #2: largest displacement (float bits) per cell
     float2 *spos2;
     float4 *spos4, *opos;
+    float4 *defer;            // d = 3: list of the leaf search's second kernel (2 float4 per point)
     kc::Counters *ctr;
     int n_scan_blocks;
 };
@@ -142,6 +149,7 @@ inline View make_view(const kc_grid *g)
     v.head = g->head; v.next = g->next; v.opos = g->opos;
     v.heavy_T = g->heavy_T; v.subinfo = g->subinfo; v.leaf_start = g->leaf_start;
     v.handoff = nullptr; v.n_handoff = nullptr;       // (the callers that launch the hand-off pass set them)
+    v.defer = g->defer; v.n_defer = &g->ctr->n_defer;
     return v;
 }
 

@@ -826,38 +826,57 @@ __device__ __forceinline__ void ball_cells(const View &v, Lane &L, bool chains, 
     if (chains)
         for (int x = xa; x <= xb; ++x) scan_chain<D>(v, rowbase + x, q.x, q.y, q.z, q.self, best);
 }
+// What the ball of a query still needs beyond phase 1: nothing, ranges to queue (ball_box), or the
+// ring search (no bound yet, or an index box of too many cells: an isolated point).
+enum { BALL_DONE = 0, BALL_MORE = 1, BALL_RINGS = 2 };
+struct BallBox {
+    float lo[3], hi[3];
+    int X0, X1, Y0, Y1, Z0, Z1;
+};
+template <int D>
+__device__ __forceinline__ int ball_state(const View &v, const Qry &q, const Top2 &best, int cx, int cy, int cz,
+                                          bool heavy, unsigned covered, int S, int ux, int uy, int uz, BallBox &B)
+{
+    if (best.s2 == CUDART_INF_F) return BALL_RINGS;
+    // r >= the real distance of anything whose computed squared distance is <= s2 (fp32 rounding
+    // of s: relative 3u, or absolute 2^-149 per operation in the denormal range)
+    const float r = __fadd_ru(__fmul_ru(__fsqrt_ru(best.s2), 1.0009765625f), 8.470329e-22f);
+    B.lo[0] = __fsub_rd(q.x, r); B.hi[0] = __fadd_ru(q.x, r);
+    B.lo[1] = __fsub_rd(q.y, r); B.hi[1] = __fadd_ru(q.y, r);
+    B.lo[2] = D == 3 ? __fsub_rd(q.z, r) : 0.f; B.hi[2] = D == 3 ? __fadd_ru(q.z, r) : 0.f;
+    B.X0 = cell_axis(B.lo[0], v.lo0, v.inv_h, v.G0); B.X1 = cell_axis(B.hi[0], v.lo0, v.inv_h, v.G0);
+    B.Y0 = cell_axis(B.lo[1], v.lo1, v.inv_h, v.G1); B.Y1 = cell_axis(B.hi[1], v.lo1, v.inv_h, v.G1);
+    B.Z0 = D == 3 ? cell_axis(B.lo[2], v.lo2, v.inv_h, v.G2) : 0; B.Z1 = D == 3 ? cell_axis(B.hi[2], v.lo2, v.inv_h, v.G2) : 0;
+    if ((int64_t)(B.X1 - B.X0 + 1) * (B.Y1 - B.Y0 + 1) * (B.Z1 - B.Z0 + 1) > 64) return BALL_RINGS;
+    // the common case: the box lies inside what phase 1 served
+    const bool in_block = B.X0 >= cx - 1 && B.X1 <= cx + 1 && B.Y0 >= cy - 1 && B.Y1 <= cy + 1 && B.Z0 >= cz - 1 && B.Z1 <= cz + 1;
+    if (!heavy && in_block && covered == (D == 3 ? 0x7ffffffu : 0x1ffu)) return BALL_DONE;
+    if (heavy && B.X0 == cx && B.X1 == cx && B.Y0 == cy && B.Y1 == cy && B.Z0 == cz && B.Z1 == cz) {
+        const float fS = (float)S;
+        if (sub_axis(B.lo[0], v.lo0, v.inv_h, cx, fS, S) >= ux - 1 && sub_axis(B.hi[0], v.lo0, v.inv_h, cx, fS, S) <= ux + 1 &&
+            sub_axis(B.lo[1], v.lo1, v.inv_h, cy, fS, S) >= uy - 1 && sub_axis(B.hi[1], v.lo1, v.inv_h, cy, fS, S) <= uy + 1 &&
+            (D == 2 || (sub_axis(B.lo[2], v.lo2, v.inv_h, cz, fS, S) >= uz - 1 &&
+                        sub_axis(B.hi[2], v.lo2, v.inv_h, cz, fS, S) <= uz + 1)))
+            return BALL_DONE;      // (on an updated grid the caller still scans the own cell's chain)
+    }
+    return BALL_MORE;
+}
 // Queues what the ball needs beyond phase 1.  Returns true when the lane has to fall back to the
-// ring search (no bound yet, or the box holds too many cells to queue).
+// ring search.
 template <int D>
 __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, const Qry &q, Top2 &best, int cx, int cy,
                                          int cz, bool heavy, unsigned covered, int cs0, int cs1, int S,
                                          const int32_t *ss, int ux, int uy, int uz)
 {
-    if (best.s2 == CUDART_INF_F) return true;
-    // r >= the real distance of anything whose computed squared distance is <= s2 (fp32 rounding
-    // of s: relative 3u, or absolute 2^-149 per operation in the denormal range)
-    const float r = __fadd_ru(__fmul_ru(__fsqrt_ru(best.s2), 1.0009765625f), 8.470329e-22f);
-    float lo[3], hi[3];
-    lo[0] = __fsub_rd(q.x, r); hi[0] = __fadd_ru(q.x, r);
-    lo[1] = __fsub_rd(q.y, r); hi[1] = __fadd_ru(q.y, r);
-    lo[2] = D == 3 ? __fsub_rd(q.z, r) : 0.f; hi[2] = D == 3 ? __fadd_ru(q.z, r) : 0.f;
-    const int X0 = cell_axis(lo[0], v.lo0, v.inv_h, v.G0), X1 = cell_axis(hi[0], v.lo0, v.inv_h, v.G0);
-    const int Y0 = cell_axis(lo[1], v.lo1, v.inv_h, v.G1), Y1 = cell_axis(hi[1], v.lo1, v.inv_h, v.G1);
-    const int Z0 = D == 3 ? cell_axis(lo[2], v.lo2, v.inv_h, v.G2) : 0, Z1 = D == 3 ? cell_axis(hi[2], v.lo2, v.inv_h, v.G2) : 0;
-    if ((int64_t)(X1 - X0 + 1) * (Y1 - Y0 + 1) * (Z1 - Z0 + 1) > 64) return true;
-    // the common case: the box lies inside what phase 1 served
-    const bool in_block = X0 >= cx - 1 && X1 <= cx + 1 && Y0 >= cy - 1 && Y1 <= cy + 1 && Z0 >= cz - 1 && Z1 <= cz + 1;
-    if (!heavy && in_block && covered == (D == 3 ? 0x7ffffffu : 0x1ffu)) return false;
-    if (heavy && X0 == cx && X1 == cx && Y0 == cy && Y1 == cy && Z0 == cz && Z1 == cz) {
-        const float fS = (float)S;
-        if (sub_axis(lo[0], v.lo0, v.inv_h, cx, fS, S) >= ux - 1 && sub_axis(hi[0], v.lo0, v.inv_h, cx, fS, S) <= ux + 1 &&
-            sub_axis(lo[1], v.lo1, v.inv_h, cy, fS, S) >= uy - 1 && sub_axis(hi[1], v.lo1, v.inv_h, cy, fS, S) <= uy + 1 &&
-            (D == 2 || (sub_axis(lo[2], v.lo2, v.inv_h, cz, fS, S) >= uz - 1 &&
-                        sub_axis(hi[2], v.lo2, v.inv_h, cz, fS, S) <= uz + 1))) {
-            if (chains) scan_chain<D>(v, (cz * v.G1 + cy) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
-            return false;
-        }
+    BallBox B;
+    const int st = ball_state<D>(v, q, best, cx, cy, cz, heavy, covered, S, ux, uy, uz, B);
+    if (st == BALL_RINGS) return true;
+    if (st == BALL_DONE) {
+        if (heavy && chains) scan_chain<D>(v, (cz * v.G1 + cy) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
+        return false;
     }
+    const float (&lo)[3] = B.lo, (&hi)[3] = B.hi;
+    const int X0 = B.X0, X1 = B.X1, Y0 = B.Y0, Y1 = B.Y1, Z0 = B.Z0, Z1 = B.Z1;
     for (int z = Z0; z <= Z1; ++z)
         for (int y = Y0; y <= Y1; ++y) {
             const int oy = y - cy, oz = z - cz;
@@ -891,7 +910,7 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
 // The search of one round: lane `lane` serves the query at sorted slot sc (query = false: the lane only
 // takes part in the warp-wide steps).  Called by all 32 lanes.
 template <int D, int MODE>
-__device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters *ctr, bool chains, int lane,
+__device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters *ctr, bool chains, bool defer_mode, int lane,
                                                   float2 *tp2, float4 *tp4, int *tix, Lane &L, int sc, bool query,
                                                   int32_t *nn, int32_t *nn2, float *d1, float *d2, float *c)
 {
@@ -1013,21 +1032,129 @@ __device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters
     // phase 2: the ball.  Every record that can still enter the list lies within r = d2 (as of now)
     // of the query, so on every axis its coordinate lies in [q - r, q + r], and because the filing
     // functions cell_axis / sub_axis are monotone, its cell (sub-cell) index lies between the
-    // indices of those two end points: the candidates are the cells of an index box.  Whatever of
-    // that box phase 1 has not served is queued (usually nothing) and scanned by the warp in step.
-    // No face arithmetic and no slack are involved: the end points are rounded outwards.
-    bool fallback = false;
+    // indices of those two end points: the candidates are the cells of an index box.  No face
+    // arithmetic and no slack are involved: the end points are rounded outwards.  A query whose box
+    // lies inside what phase 1 served (the common case) is done; the others -- a fifth of the
+    // queries of config 5, a few lanes of every warp -- go to a list with what they have found, and
+    // ball_finish_kernel serves that list with full warps.
+    // On a grid without (many) subdivided cells few queries get here and the list would only expose
+    // their latency: there every lane queues and scans its own ranges on the spot (defer_mode false).
+    bool defer = false, rings = false;
     if (query) {
-        fallback = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+        if (defer_mode) {
+            BallBox B;
+            const int st = ball_state<D>(v, q, best, cx, cy, cz, heavy, covered, S, ux, uy, uz, B);
+            defer = st == BALL_MORE;
+            rings = st == BALL_RINGS;
+            if (st == BALL_DONE && heavy && chains) scan_chain<D>(v, cellid, q.x, q.y, q.z, q.self, best);
+        } else {
+            rings = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+        }
     }
-    if (__any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
-    if (!query) return;
-    if (fallback) {
-        // no bound yet, or a ball of many cells (an isolated point): the classic ring search
-        const int r = block_search<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
-        if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+    if (!defer_mode && __any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
+    if (query && !defer) {
+        if (rings) {
+            // no bound yet, or a ball of many cells (an isolated point): the classic ring search (here
+            // and not in the second kernel, where its serial rings would be the tail of a short kernel)
+            const int r = block_search<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
+            if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+        }
+        store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
     }
-    store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
+    const unsigned dm = __ballot_sync(0xffffffffu, defer);
+    if (dm) {
+        const int leader = __ffs(dm) - 1;
+        int base = 0;
+        if (lane == leader) base = atomicAdd(v.n_defer, __popc(dm));
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (defer) {
+            float4 *e = v.defer + 2 * (size_t)(base + __popc(dm & ((1u << lane) - 1)));
+            e[0] = make_float4(__int_as_float(sc), __uint_as_float(covered), 0.f, 0.f);
+            e[1] = make_float4(best.s1, best.s2, __int_as_float(best.j1), __int_as_float(best.j2));
+        }
+    }
+}
+
+// The second kernel of the leaf search: the queries phase 1 could not finish, 32 list entries per warp.
+// Every lane queues what its ball needs beyond phase 1 (ball_box), the warp scans the queues in step,
+// the few queries without a bound or with a wide box run the ring search.  The block that finishes
+// last empties the list.
+// Resident blocks only; a warp takes the next 32 entries from a shared counter, so that the expensive
+// tail of the list (the queries of the densest cells) spreads over all SMs.
+constexpr int BF_PER_SM = 14;
+constexpr int DEFER_MIN_N = 100000;              // smaller grids are launch-bound: no second kernel
+inline int bf_blocks(int n) { return min(148 * BF_PER_SM, (n + PS_THREADS - 1) / PS_THREADS); }
+template <int D>
+__global__ void __launch_bounds__(PS_THREADS)
+ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may_chain, int32_t *nn, int32_t *nn2,
+                   float *d1, float *d2, float *c)
+{
+    __shared__ int2 s_rl[RL_CAP * PS_THREADS];
+    const int n = ctr->n_defer;
+    if (n == 0) return;                            // (every CTA sees the same count: it changes below only)
+    const bool chains = may_chain && ctr->n_misfiled > 0;
+    const int lane = threadIdx.x & 31;
+    Lane L;
+    L.rl = s_rl + threadIdx.x;
+    L.cnt = 0;
+#pragma unroll 1
+    for (;;) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(&ctr->defer_next, 32);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= n) break;
+        const bool query = base + lane < n;
+        const int ent = min(base + lane, n - 1);
+        const float4 e0 = v.defer[2 * (size_t)ent], e1 = v.defer[2 * (size_t)ent + 1];
+        const int sc = __float_as_int(e0.x);
+        const unsigned covered = __float_as_uint(e0.y);
+        Top2 best;
+        best.s1 = e1.x; best.s2 = e1.y; best.j1 = __float_as_int(e1.z); best.j2 = __float_as_int(e1.w);
+        Qry q;
+        q.z = 0.f;
+        if (D == 2) {
+            const float2 t = v.spos2[sc];
+            q.x = t.x; q.y = t.y; q.self = v.sidx[sc];
+        } else {
+            const float4 t = v.spos4[sc];
+            q.x = t.x; q.y = t.y; q.z = t.z; q.self = __float_as_int(t.w);
+        }
+        const int cx = cell_axis(q.x, v.lo0, v.inv_h, v.G0);
+        const int cy = cell_axis(q.y, v.lo1, v.inv_h, v.G1);
+        const int cz = D == 3 ? cell_axis(q.z, v.lo2, v.inv_h, v.G2) : 0;
+        const int cellid = (cz * v.G1 + cy) * v.G0 + cx;
+        const int cs0 = v.cell_start[cellid], cs1 = v.cell_start[cellid + 1];
+        const bool heavy = cs1 - cs0 >= v.heavy_T;
+        int S = 0, ux = 0, uy = 0, uz = 0;
+        const int32_t *ss = v.leaf_start;
+        if (heavy) {
+            const int2 si = v.subinfo[cellid];
+            S = si.x; ss += si.y;
+            const float fS = (float)S;
+            ux = sub_axis(q.x, v.lo0, v.inv_h, cx, fS, S);
+            uy = sub_axis(q.y, v.lo1, v.inv_h, cy, fS, S);
+            uz = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, cz, fS, S) : 0;
+        }
+        bool fallback = false;
+        if (query) fallback = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+        if (__any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
+        if (query) {
+            if (fallback) {
+                // no bound yet, or a ball of many cells (an isolated point): the classic ring search
+                const int r = block_search<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
+                if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
+            }
+            store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
+        }
+        __syncwarp();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && atomicAdd(&ctr->ticket4, 1) == (int)gridDim.x - 1) {
+        ctr->n_deferred += n;
+        ctr->n_defer = 0;
+        ctr->defer_next = 0;
+        ctr->ticket4 = 0;
+    }
 }
 
 // MODE 0: A3, thread t serves slot t.  MODE 1 / 2: the slot sweep of A7 on an updated / a fresh grid.  A
@@ -1049,6 +1176,8 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
     // the sweep has two instantiations, both launched; the frontier's density decides which one runs
     if (MODE != 0 && (sweep_words(N, *nF) == 1) != (MODE <= 2)) return;
     const bool chains = (MODE == 1 || MODE == 3) && ctr->n_misfiled > 0;     // MODE 2, 4: a fresh grid has no chains (compile-time)
+    // with subdivided cells that hold at least N / 32 points, the queries phase 1 cannot finish go to the second kernel
+    const bool defer_mode = N >= DEFER_MIN_N && (int64_t)ctr->n_heavy * v.heavy_T * 32 >= N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float qnan = __int_as_float(0x7fc00000);
     float4 *tp4 = s_p4[D == 3 ? warp : 0];
@@ -1070,7 +1199,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
             query = query && mark[sc] != 0;
             if (query) mark[sc] = 0;               // the marks are all zero again when the sweep ends
         }
-        leaf_search_round<D, MODE>(v, N, ctr, chains, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
+        leaf_search_round<D, MODE>(v, N, ctr, chains, defer_mode, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
         return;
     }
     // (the sweep's bookkeeping lives in shared memory: nothing of it stays in registers across a round)
@@ -1108,7 +1237,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
         __syncwarp();
         if (lane == 0) s_r0[warp] = r0 + 32;
         __syncwarp();
-        leaf_search_round<D, MODE>(v, N, ctr, chains, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
+        leaf_search_round<D, MODE>(v, N, ctr, chains, defer_mode, lane, tp2, tp4, tix, L, sc, query, nn, nn2, d1, d2, c);
         __syncwarp();
     }
 }
@@ -1578,7 +1707,13 @@ extern "C" kc_status kc_cert_grid_search(kc_grid *g, int32_t *nn, int32_t *nn2, 
     const int n = (int)g->N;
     const int nb = (n + PS_THREADS - 1) / PS_THREADS, tb = 32 * WT_WARPS;
     if (g->geom.d == 2) search_tiled_kernel<2, false, true><<<(n + tb - 1) / tb, tb, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
-    else search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
+    else {
+        search_leaf_kernel<3, 0><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, nullptr, nullptr, 0, nn, nn2, d1, d2, c);
+        if (n >= DEFER_MIN_N) {
+            ball_finish_kernel<3><<<bf_blocks(n), PS_THREADS, 0, st>>>(v, n, g->ctr, 0, nn, nn2, d1, d2, c);
+            count_launches(1);
+        }
+    }
     count_launches(1);
     launch_handoff(g, v, nn, nn2, d1, d2, c, st);
     KC_LAUNCH_CHECK("kc_cert_grid_search");
@@ -1683,7 +1818,8 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
                 if (direct) search_leaf_kernel<3, 2><<<nb, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
                 search_leaf_kernel<3, 4><<<nb2, PS_THREADS, 0, st>>>(v, n, g->ctr, g->mark, nF, sweep_div, nn, nn2, d1, d2, c);
             }
-            count_launches(direct ? 1 : 0);
+            ball_finish_kernel<3><<<bf_blocks(n), PS_THREADS, 0, st>>>(v, n, g->ctr, g->dirty ? 1 : 0, nn, nn2, d1, d2, c);   // (n >= SWEEP_MIN_N >= DEFER_MIN_N)
+            count_launches(direct ? 2 : 1);
         }
         count_launches(2);
     }
