@@ -764,7 +764,7 @@ constexpr int LT_WARPS = 4;
 constexpr int SWEEP_MIN_N = 200000, SWEEP_DIV = 8;   // A7: when the slot sweep serves a frontier
 constexpr int WPQ_MAX = 32768;                       // A7: id lists up to this long get one warp per query
 #ifndef LT_MIN_BLOCKS
-#define LT_MIN_BLOCKS 7
+#define LT_MIN_BLOCKS 8
 #endif
 constexpr int LT_HULL_MAX = 4096;                 // a longer hull (lanes far apart in memory) is left to phase 2
 static_assert(32 * LT_WARPS == PS_THREADS, "the range queues are strided by PS_THREADS");
@@ -877,31 +877,29 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
     }
     const float (&lo)[3] = B.lo, (&hi)[3] = B.hi;
     const int X0 = B.X0, X1 = B.X1, Y0 = B.Y0, Y1 = B.Y1, Z0 = B.Z0, Z1 = B.Z1;
+    // Row by row, the cells X0..X1 in maximal runs of cells phase 1 has NOT served (one call site of
+    // ball_cells: the kernel's code stays small).  Served: for a light lane the cells cx-1..cx+1 of a
+    // block row whose `covered` bit is set (their chains too); for a lane in a subdivided cell the
+    // 3^d sub-block of its own cell, so that cell goes through its sub-cells minus the sub-block.
     for (int z = Z0; z <= Z1; ++z)
         for (int y = Y0; y <= Y1; ++y) {
             const int oy = y - cy, oz = z - cz;
             const bool near = oy >= -1 && oy <= 1 && oz >= -1 && oz <= 1;
-            if (heavy) {
-                if (oy == 0 && oz == 0) {
-                    // own row: the own cell through its sub-cells (minus the sub-block), the others whole
-                    ball_cells<D>(v, L, chains, y, z, X0, cx - 1, lo, hi, q, best);
+            const unsigned cv = (!heavy && near) ? (covered >> (3 * block_row_index(oy, oz))) & 7u : 0u;
+            const bool own_row = heavy && oy == 0 && oz == 0;
+            int xa = X0;
+            for (int x = X0; x <= X1 + 1; ++x) {
+                const bool own = own_row && x == cx;
+                const bool served = x >= cx - 1 && x <= cx + 1 && ((cv >> (x - cx + 1)) & 1u);
+                if (x <= X1 && !own && !served) continue;
+                if (xa < x) ball_cells<D>(v, L, chains, y, z, xa, x - 1, lo, hi, q, best);
+                xa = x + 1;
+                if (own && x <= X1) {
                     if (chains) scan_chain<D>(v, (z * v.G1 + y) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
                     ball_sub<D>(v, L, (z * v.G1 + y) * v.G0 + cx, cx, cy, cz, lo, hi, true, max(ux - 1, 0),
                                 min(ux + 1, S - 1), max(uy - 1, 0), min(uy + 1, S - 1), D == 3 ? max(uz - 1, 0) : 0,
                                 D == 3 ? min(uz + 1, S - 1) : 0, q, best);
-                    ball_cells<D>(v, L, chains, y, z, cx + 1, X1, lo, hi, q, best);
-                } else {
-                    ball_cells<D>(v, L, chains, y, z, X0, X1, lo, hi, q, best);
                 }
-            } else if (near && ((covered >> (3 * block_row_index(oy, oz))) & 7u)) {
-                // phase 1 served some of the cells cx-1..cx+1 of this row (and their chains)
-                const unsigned cv = (covered >> (3 * block_row_index(oy, oz))) & 7u;
-                ball_cells<D>(v, L, chains, y, z, X0, cx - 2, lo, hi, q, best);
-                for (int x = max(X0, cx - 1); x <= min(X1, cx + 1); ++x)
-                    if (!((cv >> (x - cx + 1)) & 1u)) ball_cells<D>(v, L, chains, y, z, x, x, lo, hi, q, best);
-                ball_cells<D>(v, L, chains, y, z, cx + 2, X1, lo, hi, q, best);
-            } else {
-                ball_cells<D>(v, L, chains, y, z, X0, X1, lo, hi, q, best);
             }
         }
     return false;
@@ -1084,8 +1082,11 @@ __device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters
 constexpr int BF_PER_SM = 14;
 constexpr int DEFER_MIN_N = 100000;              // smaller grids are launch-bound: no second kernel
 inline int bf_blocks(int n) { return min(148 * BF_PER_SM, (n + PS_THREADS - 1) / PS_THREADS); }
+#ifndef BF_MIN_BLOCKS
+#define BF_MIN_BLOCKS 8
+#endif
 template <int D>
-__global__ void __launch_bounds__(PS_THREADS)
+__global__ void __launch_bounds__(PS_THREADS, BF_MIN_BLOCKS)
 ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may_chain, int32_t *nn, int32_t *nn2,
                    float *d1, float *d2, float *c)
 {
@@ -1135,17 +1136,11 @@ ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may
             uy = sub_axis(q.y, v.lo1, v.inv_h, cy, fS, S);
             uz = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, cz, fS, S) : 0;
         }
-        bool fallback = false;
-        if (query) fallback = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+        // (an entry is here because ball_state said BALL_MORE in the first kernel; state and inputs are
+        // the same, so ball_box never asks for the ring search -- those queries ran it there)
+        if (query) ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
         if (__any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
-        if (query) {
-            if (fallback) {
-                // no bound yet, or a ball of many cells (an isolated point): the classic ring search
-                const int r = block_search<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, best);
-                if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
-            }
-            store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
-        }
+        if (query) store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
         __syncwarp();
     }
     __syncthreads();
