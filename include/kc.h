@@ -210,9 +210,12 @@ size_t kc_grid_bytes(const kc_grid *g);
 /* host.  Parameters of the two-level index ("a hierarchical GPU index ... could lower its constant
  * further"): a cell that holds at least heavy_T records at build time is subdivided
  * into S^d sub-cells, S = floor((count / sub_occ)^(1/d)) >= 2, and its records are sorted by
- * sub-cell, so the searches prune inside it.  Defaults: sub_occ = 4; heavy_T = 256 for d = 3 and
+ * sub-cell, so the searches prune inside it.  Defaults: sub_occ = 4; heavy_T = 128 for d = 3 and
  * INT_MAX (no second level) for d = 2, where the whole-set search prunes cell by cell instead;
- * heavy_T is raised to sub_occ * 2^(d+1) if smaller.  Results never depend on these values.
+ * heavy_T is raised to sub_occ * 2^(d+1) if smaller.  (Every search that enters a subdivided cell
+ * from outside prunes by sub-cell; the d = 3 whole-set search and slot sweep serve a cell's OWN
+ * queries through its sub-cells from max(heavy_T, 256) records on, through the 3^d block of whole
+ * cells below that.)  Results never depend on these values.
  * Takes effect with the next kc_grid_build (the grid counts as not built until then). */
 kc_status kc_grid_set_index(kc_grid *g, int heavy_T, int sub_occ);
 

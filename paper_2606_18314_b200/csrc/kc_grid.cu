@@ -632,11 +632,12 @@ extern "C" kc_status kc_grid_create(kc_grid **out, int64_t N_max, const kc_geom 
         delete g;
         return KC_EINVAL;
     }
-    // two-level index defaults (measured on config 5): d = 3: cells of >= 256 records
-    // are subdivided at ~4 records per sub-cell; d = 2: off (the plane's whole-set kernel prunes
+    // two-level index defaults (measured on config 5): d = 3: cells of >= 128 records
+    // are subdivided at ~4 records per sub-cell (LANE_T_MIN in kc_grid.cuh: from where a cell's own
+    // queries use the sub-cells); d = 2: off (the plane's whole-set kernel prunes
     // cell by cell instead); kc_grid_set_index changes them
     g->sub_occ = 4;
-    g->heavy_T = geom->d == 2 ? KC_INDEX_OFF : 256;
+    g->heavy_T = geom->d == 2 ? KC_INDEX_OFF : 128;
     g->n_scan_blocks = (int)((g->n_leaves_max + SCAN_CHUNK - 1) / SCAN_CHUNK);
     bool ok = true;
     auto alloc = [&](void **p, size_t bytes) {

@@ -42,6 +42,11 @@ struct Counters {
 // storage order; leaf_start is the exclusive scan of their sizes, subinfo[c] = {S or 0, first leaf}.
 // Sub-cell of coordinate x in cell k of an axis: clamp(floorf(fl(fl(t - k) * S)), 0, S-1) with the
 // cell coordinate t = fl(fl(x - lo) * inv_h) of cell_axis(): monotone in x like cell_axis itself.
+// Two thresholds (measured on config 5): a cell is SUBDIVIDED from heavy_T records on
+// (default 128: whoever visits it from outside prunes by sub-cell), but the leaf search serves the cell's OWN
+// queries through its sub-cells only from max(heavy_T, LANE_T_MIN) records on -- below that the 3^d block
+// of whole cells is cheaper than the many sub-cells that touch the cell's faces.
+constexpr int LANE_T_MIN = 256;
 constexpr int KC_INDEX_OFF = 0x7fffffff;          // heavy_T value that switches the second level off
 
 __host__ __device__ inline int sub_res(int cnt, int d, int heavy_T, int sub_occ)
@@ -78,6 +83,7 @@ struct View {
     const int32_t *next;
     const float4 *opos;
     int heavy_T;              // build-time record count from which a level-0 cell is subdivided
+    int lane_T;               // >= heavy_T: count from which the leaf search serves a cell's OWN queries through its sub-cells
     const int2 *subinfo;      // per level-0 cell: {S (0 = not subdivided), index of its first leaf}
     const int32_t *leaf_start;   // exclusive scan of the leaf sizes (n_leaves + 1 entries)
     float4 *handoff;          // hand-off list (x, y, z, bits(id)) of ring_continue, or null: rings without limit
@@ -147,7 +153,8 @@ inline View make_view(const kc_grid *g)
     v.cell_start = g->cell_start;
     v.spos2 = g->spos2; v.spos4 = g->spos4; v.sidx = g->sidx;
     v.head = g->head; v.next = g->next; v.opos = g->opos;
-    v.heavy_T = g->heavy_T; v.subinfo = g->subinfo; v.leaf_start = g->leaf_start;
+    v.heavy_T = g->heavy_T; v.lane_T = g->heavy_T > LANE_T_MIN ? g->heavy_T : LANE_T_MIN;
+    v.subinfo = g->subinfo; v.leaf_start = g->leaf_start;
     v.handoff = nullptr; v.n_handoff = nullptr;       // (the callers that launch the hand-off pass set them)
     v.defer = g->defer; v.n_defer = &g->ctr->n_defer;
     return v;

@@ -394,6 +394,9 @@ __device__ int block_search(const View &v, bool chains, float qx, float qy, floa
 // against the second-best of the moment: an upper bound of the final one, so every test stays a
 // valid strict lower-bound test (see gap_lb above).
 constexpr int PS_THREADS = 128;
+#ifndef RL_STEP8
+#define RL_STEP8 1
+#endif
 constexpr int RL_CAP = 16;                       // ranges a lane can queue between two scans
 
 struct Qry { float x, y, z; int self; };
@@ -437,6 +440,17 @@ __device__ __forceinline__ void rl_scan(const View &v, Lane &L, const Qry &q, To
                 const float4 B = *reinterpret_cast<const float4 *>(v.spos2 + t + 2);
                 s0 = sqd2(q.x, q.y, A.x, A.y); s1 = sqd2(q.x, q.y, A.z, A.w);
                 s2 = sqd2(q.x, q.y, B.x, B.y); s3 = sqd2(q.x, q.y, B.z, B.w);
+            } else if (RL_STEP8 && t + 4 < e) {
+                // eight records per round trip (a queue is scanned at the latency of its loads)
+                const float4 c0 = v.spos4[t], c1 = v.spos4[t + 1], c2 = v.spos4[t + 2], c3 = v.spos4[t + 3];
+                const float4 c4 = v.spos4[t + 4], c5 = v.spos4[t + 5], c6 = v.spos4[t + 6], c7 = v.spos4[t + 7];
+                s0 = sqd3(q.x, q.y, q.z, c0.x, c0.y, c0.z); s1 = sqd3(q.x, q.y, q.z, c1.x, c1.y, c1.z);
+                s2 = sqd3(q.x, q.y, q.z, c2.x, c2.y, c2.z); s3 = sqd3(q.x, q.y, q.z, c3.x, c3.y, c3.z);
+                const float m0 = fminf(fminf(s0, s1), fminf(s2, s3));
+                if (m0 <= best.s2) best = slow_offer4<D>(v, best, t, s0, s1, s2, s3, q.self);
+                t += 4;
+                s0 = sqd3(q.x, q.y, q.z, c4.x, c4.y, c4.z); s1 = sqd3(q.x, q.y, q.z, c5.x, c5.y, c5.z);
+                s2 = sqd3(q.x, q.y, q.z, c6.x, c6.y, c6.z); s3 = sqd3(q.x, q.y, q.z, c7.x, c7.y, c7.z);
             } else {
                 const float4 c0 = v.spos4[t], c1 = v.spos4[t + 1], c2 = v.spos4[t + 2], c3 = v.spos4[t + 3];
                 s0 = sqd3(q.x, q.y, q.z, c0.x, c0.y, c0.z); s1 = sqd3(q.x, q.y, q.z, c1.x, c1.y, c1.z);
@@ -930,7 +944,7 @@ __device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters
     const bool has_l = cx > 0, has_r = cx < v.G0 - 1;
     int cs0 = 0, cs1 = 0;
     if (query) { cs0 = v.cell_start[cellid]; cs1 = v.cell_start[cellid + 1]; }
-    const bool heavy = query && cs1 - cs0 >= v.heavy_T;
+    const bool heavy = query && cs1 - cs0 >= v.lane_T;
     int S = 0, ux = 0, uy = 0, uz = 0;
     const int32_t *ss = v.leaf_start;
     if (heavy) {
@@ -962,7 +976,7 @@ __device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters
                 if (y >= 0 && y < v.G1 && z >= 0 && z < v.G2) {
                     const int32_t *crow = v.cell_start + (z * v.G1 + y) * v.G0;
                     b = crow[has_l ? cx - 1 : cx]; e = crow[has_r ? cx + 2 : cx + 1];
-                    if (e - b < v.heavy_T) {
+                    if (e - b < v.lane_T) {
                         covered |= 7u << (3 * k);
                     } else if (k == 0) {
                         // a long window (dense cells, or a subdivided one): the ball of phase 2 prunes
@@ -1125,7 +1139,7 @@ ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may
         const int cz = D == 3 ? cell_axis(q.z, v.lo2, v.inv_h, v.G2) : 0;
         const int cellid = (cz * v.G1 + cy) * v.G0 + cx;
         const int cs0 = v.cell_start[cellid], cs1 = v.cell_start[cellid + 1];
-        const bool heavy = cs1 - cs0 >= v.heavy_T;
+        const bool heavy = cs1 - cs0 >= v.lane_T;
         int S = 0, ux = 0, uy = 0, uz = 0;
         const int32_t *ss = v.leaf_start;
         if (heavy) {
