@@ -211,7 +211,10 @@ __device__ __noinline__ Top2 visit_heavy(const View &v, int cid, int kx, int ky,
     ay.lo = v.lo1; ay.q = qy; ay.slk = v.slk1; ay.base = ky * S; ay.u = sub_axis(qy, v.lo1, v.inv_h, ky, fS, S);
     az.lo = v.lo2; az.q = qz; az.slk = v.slk2; az.base = kz * S; az.u = D == 3 ? sub_axis(qz, v.lo2, v.inv_h, kz, fS, S) : 0;
     int px0 = 0, px1 = -1, py0 = 0, py1 = -1, pz0 = 0, pz1 = -1;      // block already scanned (empty)
-    if (best.s2 == CUDART_INF_F) {
+    // No bound yet, or a poor one (worse than two sub-cell widths: a sparse point beside a dense cell):
+    // the sub-cells nearest to the query first, so that the sweep below prunes against a bound of the
+    // cell's own scale instead of scanning a third of it at the latency of one thread.
+    if (!(best.s2 < __fmul_rn(4.0f, __fmul_rn(hs, hs)))) {
         px0 = max(ax.u - 1, 0); px1 = min(ax.u + 1, S - 1);
         py0 = max(ay.u - 1, 0); py1 = min(ay.u + 1, S - 1);
         pz0 = D == 3 ? max(az.u - 1, 0) : 0; pz1 = D == 3 ? min(az.u + 1, S - 1) : 0;
@@ -400,20 +403,33 @@ constexpr int PS_THREADS = 128;
 constexpr int RL_CAP = 16;                       // ranges a lane can queue between two scans
 
 struct Qry { float x, y, z; int self; };
-struct Lane { int2 *rl; int cnt; };              // entry i of this thread's list: rl[i * PS_THREADS]
+// A lane's queue is bounded in entries (RL_CAP) and in records (RL_BUDGET): a query whose ball holds more
+// than that -- a sparse point next to a dense cluster, with the poor bound its own cell gave it -- would scan
+// it all at the latency of one thread, against a bound that no longer shrinks what was queued.  Such a lane
+// drops its queue (big) and runs the ring search instead, which prunes cell by cell and sub-row by sub-row
+// against the current bound.
+constexpr int RL_BUDGET = 768;
+struct Lane { int2 *rl; int cnt; int tot; int last_e; bool big; };   // entry i of this thread's list: rl[i * PS_THREADS]
+__device__ __forceinline__ void lane_reset(Lane &L) { L.cnt = 0; L.tot = 0; L.last_e = -1; L.big = false; }
 
 template <int D>
 __device__ __forceinline__ void rl_push(const View &v, Lane &L, int b, int e, const Qry &q, Top2 &best)
 {
-    if (b >= e) return;
-    if (L.cnt == RL_CAP) {                       // full (rare): this lane scans its list on its own
-        for (int i = 0; i < RL_CAP; ++i) {
-            const int2 r = L.rl[i * PS_THREADS];
-            scan_range<D>(v, r.x, r.y, q.x, q.y, q.z, q.self, best);
-        }
+    if (b >= e || L.big) return;
+    L.tot += e - b;
+    if (L.cnt > 0 && b == L.last_e) {            // continues the previous range (full sub-rows of one cell)
+        L.rl[(L.cnt - 1) * PS_THREADS].y = e;
+        L.last_e = e;
+        if (L.tot > RL_BUDGET) { L.big = true; L.cnt = 0; }
+        return;
+    }
+    if (L.cnt == RL_CAP || L.tot > RL_BUDGET) {
+        L.big = true;
         L.cnt = 0;
+        return;
     }
     L.rl[L.cnt * PS_THREADS] = make_int2(b, e);
+    L.last_e = e;
     ++L.cnt;
 }
 // All 32 lanes of the warp call this; a lane without ranges just waits for the others.  d = 3 records
@@ -461,7 +477,7 @@ __device__ __forceinline__ void rl_scan(const View &v, Lane &L, const Qry &q, To
             t += 4;
         }
     }
-    L.cnt = 0;
+    L.cnt = 0; L.tot = 0; L.last_e = -1;
 }
 
 // ---- A3, warp-tiled: the whole-set search of a freshly built grid --------------------------
@@ -808,6 +824,7 @@ __device__ __forceinline__ void ball_sub(const View &v, Lane &L, int cid, int kx
     const int z1 = D == 3 ? sub_axis(hi[2], v.lo2, v.inv_h, kz, fS, S) : 0;
     for (int z = z0; z <= z1; ++z)
         for (int y = y0; y <= y1; ++y) {
+            if (L.big) return;                   // (queue dropped: nothing more to collect)
             const int row = (z * S + y) * S;
             if (has_block && y >= by0 && y <= by1 && z >= bz0 && z <= bz1) {
                 if (x0 < bx0) rl_push<D>(v, L, ss[row + x0], ss[row + min(x1, bx0 - 1) + 1], q, best);
@@ -830,7 +847,7 @@ __device__ __forceinline__ void ball_cells(const View &v, Lane &L, bool chains, 
         rl_push<D>(v, L, b, e, q, best);
     } else {
         int lo_s = b;
-        for (int x = xa; x <= xb; ++x) {
+        for (int x = xa; x <= xb && !L.big; ++x) {
             const int hi_s = x == xb ? e : cs[x + 1];
             if (hi_s - lo_s >= v.heavy_T) ball_sub<D>(v, L, rowbase + x, x, y, z, lo, hi, false, 0, 0, 0, 0, 0, 0, q, best);
             else rl_push<D>(v, L, lo_s, hi_s, q, best);
@@ -842,7 +859,7 @@ __device__ __forceinline__ void ball_cells(const View &v, Lane &L, bool chains, 
 }
 // What the ball of a query still needs beyond phase 1: nothing, ranges to queue (ball_box), or the
 // ring search (no bound yet, or an index box of too many cells: an isolated point).
-enum { BALL_DONE = 0, BALL_MORE = 1, BALL_RINGS = 2 };
+enum { BALL_DONE = 0, BALL_MORE = 1, BALL_RINGS = 2, BALL_BIG = 3 };
 struct BallBox {
     float lo[3], hi[3];
     int X0, X1, Y0, Y1, Z0, Z1;
@@ -875,19 +892,54 @@ __device__ __forceinline__ int ball_state(const View &v, const Qry &q, const Top
     }
     return BALL_MORE;
 }
-// Queues what the ball needs beyond phase 1.  Returns true when the lane has to fall back to the
-// ring search.
-template <int D>
-__device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, const Qry &q, Top2 &best, int cx, int cy,
-                                         int cz, bool heavy, unsigned covered, int cs0, int cs1, int S,
-                                         const int32_t *ss, int ux, int uy, int uz)
+// Squared lower bound (R7's face bound: slack, shrink) of the axis distance from the query coordinate q in
+// cell c to anything filed in cell k of that axis.
+__device__ __forceinline__ float axis_gap2(const View &v, float q, float lo, float slk, int k, int c)
 {
-    BallBox B;
+    if (k == c) return 0.0f;
+    const float g = k > c ? __fsub_rn(face_at(lo, k, v.h), q) : __fsub_rn(q, face_at(lo, k + 1, v.h));
+    const float t = gap_lb(v, g, slk);
+    return __fmul_rn(t, t);
+}
+// A query whose ball box holds more than a lane's queue may hold (a sparse point beside a dense cluster:
+// most of the box lies outside the ball): the cells of the box one by one, each row and cell tested
+// against the CURRENT bound (strict), subdivided cells through visit_heavy, which prunes sub-row by
+// sub-row.  Whatever phase 1 has offered already is skipped by id.  (Rare path: out of line.)
+template <int D>
+__device__ __noinline__ Top2 box_visit(const View &v, bool chains, float qx, float qy, float qz, int self, int cx,
+                                       int cy, int cz, int X0, int X1, int Y0, int Y1, int Z0, int Z1, Top2 best)
+{
+    for (int z = Z0; z <= Z1; ++z) {
+        const float gz = D == 3 ? axis_gap2(v, qz, v.lo2, v.slk2, z, cz) : 0.0f;
+        if (best.s2 < gz) continue;
+        for (int y = Y0; y <= Y1; ++y) {
+            const float gy = __fadd_rn(gz, axis_gap2(v, qy, v.lo1, v.slk1, y, cy));
+            if (best.s2 < gy) continue;
+            const int rowbase = (z * v.G1 + y) * v.G0;
+            const int32_t *cs = v.cell_start + rowbase;
+            for (int x = X0; x <= X1; ++x) {
+                if (best.s2 < __fadd_rn(gy, axis_gap2(v, qx, v.lo0, v.slk0, x, cx))) continue;
+                const int b = cs[x], e = cs[x + 1];
+                if (e > b) visit_cell<D>(v, rowbase + x, x, y, z, b, e, qx, qy, qz, self, best);
+                if (chains) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
+            }
+        }
+    }
+    return best;
+}
+// Queues what the ball needs beyond phase 1.  Returns BALL_DONE (everything the ball needs is served or
+// queued), BALL_RINGS (no bound yet / a box of too many cells: the ring search) or BALL_BIG (the box B
+// holds more than a lane's queue may hold: box_visit).
+template <int D>
+__device__ __forceinline__ int ball_box(const View &v, Lane &L, bool chains, const Qry &q, Top2 &best, int cx, int cy,
+                                        int cz, bool heavy, unsigned covered, int cs0, int cs1, int S,
+                                        const int32_t *ss, int ux, int uy, int uz, BallBox &B)
+{
     const int st = ball_state<D>(v, q, best, cx, cy, cz, heavy, covered, S, ux, uy, uz, B);
-    if (st == BALL_RINGS) return true;
+    if (st == BALL_RINGS) return BALL_RINGS;
     if (st == BALL_DONE) {
         if (heavy && chains) scan_chain<D>(v, (cz * v.G1 + cy) * v.G0 + cx, q.x, q.y, q.z, q.self, best);
-        return false;
+        return BALL_DONE;
     }
     const float (&lo)[3] = B.lo, (&hi)[3] = B.hi;
     const int X0 = B.X0, X1 = B.X1, Y0 = B.Y0, Y1 = B.Y1, Z0 = B.Z0, Z1 = B.Z1;
@@ -901,6 +953,7 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
             const bool near = oy >= -1 && oy <= 1 && oz >= -1 && oz <= 1;
             const unsigned cv = (!heavy && near) ? (covered >> (3 * block_row_index(oy, oz))) & 7u : 0u;
             const bool own_row = heavy && oy == 0 && oz == 0;
+            if (L.big) return BALL_BIG;          // queue dropped: the caller walks the box (box_visit)
             int xa = X0;
             for (int x = X0; x <= X1 + 1; ++x) {
                 const bool own = own_row && x == cx;
@@ -916,7 +969,7 @@ __device__ __forceinline__ bool ball_box(const View &v, Lane &L, bool chains, co
                 }
             }
         }
-    return false;
+    return L.big ? BALL_BIG : BALL_DONE;
 }
 
 // The search of one round: lane `lane` serves the query at sorted slot sc (query = false: the lane only
@@ -1052,15 +1105,17 @@ __device__ __forceinline__ void leaf_search_round(const View &v, int N, Counters
     // On a grid without (many) subdivided cells few queries get here and the list would only expose
     // their latency: there every lane queues and scans its own ranges on the spot (defer_mode false).
     bool defer = false, rings = false;
+    BallBox B;
+    lane_reset(L);
     if (query) {
         if (defer_mode) {
-            BallBox B;
             const int st = ball_state<D>(v, q, best, cx, cy, cz, heavy, covered, S, ux, uy, uz, B);
             defer = st == BALL_MORE;
             rings = st == BALL_RINGS;
             if (st == BALL_DONE && heavy && chains) scan_chain<D>(v, cellid, q.x, q.y, q.z, q.self, best);
         } else {
-            rings = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+            const int st = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz, B);
+            rings = st != BALL_DONE;             // (a queue that overflows, on these small or uniform grids: the rings too)
         }
     }
     if (!defer_mode && __any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
@@ -1111,7 +1166,7 @@ ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may
     const int lane = threadIdx.x & 31;
     Lane L;
     L.rl = s_rl + threadIdx.x;
-    L.cnt = 0;
+    lane_reset(L);
 #pragma unroll 1
     for (;;) {
         int base = 0;
@@ -1150,11 +1205,18 @@ ball_finish_kernel(const __grid_constant__ View v, int N, Counters *ctr, int may
             uy = sub_axis(q.y, v.lo1, v.inv_h, cy, fS, S);
             uz = D == 3 ? sub_axis(q.z, v.lo2, v.inv_h, cz, fS, S) : 0;
         }
-        // (an entry is here because ball_state said BALL_MORE in the first kernel; state and inputs are
-        // the same, so ball_box never asks for the ring search -- those queries ran it there)
-        if (query) ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz);
+        // (an entry is here because ball_state said BALL_MORE in the first kernel; state and inputs are the
+        // same, so ball_box never asks for the ring search -- those queries ran it there; a lane whose
+        // queue overflows walks its box instead, see Lane)
+        lane_reset(L);
+        BallBox B;
+        int st = BALL_DONE;
+        if (query) st = ball_box<D>(v, L, chains, q, best, cx, cy, cz, heavy, covered, cs0, cs1, S, ss, ux, uy, uz, B);
         if (__any_sync(0xffffffffu, L.cnt > 0)) rl_scan<D>(v, L, q, best);
-        if (query) store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
+        if (query) {
+            if (st == BALL_BIG) best = box_visit<D>(v, chains, q.x, q.y, q.z, q.self, cx, cy, cz, B.X0, B.X1, B.Y0, B.Y1, B.Z0, B.Z1, best);
+            store_cert_keep(best, q.self, nn, nn2, d1, d2, c);
+        }
         __syncwarp();
     }
     __syncthreads();
@@ -1198,7 +1260,7 @@ search_leaf_kernel(const __grid_constant__ View v, int N, Counters *ctr, int32_t
     }
     Lane L;
     L.rl = s_rl + threadIdx.x;
-    L.cnt = 0;
+    lane_reset(L);
     if (MODE <= 2) {
         const int s = blockIdx.x * blockDim.x + threadIdx.x;
         if (s - lane >= N) return;                 // whole warp past the end
