@@ -37,12 +37,13 @@ N_ALLPAIRS = 1 << 20            # config 5: the all-pairs oracle pass runs on th
 # ncu --set full captures (profiles/, file named beside each figure); None where no capture exists
 NCU_TRAFFIC_BYTES = {
     ("cfg2", "allpairs_kernel"): 279552,            # profiles/r1f_allpairs_cfg2_full.txt
-    ("cfg5_d3", "allpairs_kernel"): 164913152,      # profiles/r2_allpairs_1m_cfg5_d3_full.txt (86.5 MB read + 78.4 MB written)
-    ("cfg5_d2", "allpairs_kernel"): 148216832,      # profiles/r2_allpairs_1m_cfg5_d2_full.txt
-    # A2 + A3, summed over the kernels of one kc_cert_grid_rebuild call (cellid_hist, scan_write, leafid_hist,
-    # lscan_write, scatter, search): profiles/r2_grid_cfg5_d3_full.txt / r2_grid_cfg5_d2_full.txt
-    ("cfg5_d3", "rebuild"): 834500000,
-    ("cfg5_d2", "rebuild"): 984300000,
+    ("cfg5_d3", "allpairs_kernel"): 164840704,      # profiles/r2_allpairs_1m_cfg5_d3_full.txt (87.3 MB read + 77.6 MB written)
+    ("cfg5_d2", "allpairs_kernel"): 143417856,      # profiles/r2_allpairs_1m_cfg5_d2_full.txt (71.3 + 72.2 MB)
+    # A2 + A3, summed over the kernels of one kc_cert_grid_rebuild call (build_prep, cellid_hist, scan_cells,
+    # leafid_hist, lscan, scatter, search_leaf + ball_finish / search_tiled): profiles/r2_grid_cfg5_d3_full.txt
+    # (591 MB read + 387 MB written) / r2_grid_cfg5_d2_full.txt (413 + 647 MB)
+    ("cfg5_d3", "rebuild"): 978100000,
+    ("cfg5_d2", "rebuild"): 1060200000,
 }
 # algorithmic bytes per point of the O(N) rebuild (A2 + A3) with this layout
 REBUILD_BYTES_PER_POINT = {2: 76.0, 3: 90.0}
@@ -690,7 +691,7 @@ def run_gpu_arm_scale(args):
                         fp32_probe_tops=probe)
         reb_bytes = REBUILD_BYTES_PER_POINT[d] * N
         reb_gbs = reb_bytes / (ms["rebuild"] * 1e-3) / 1e9
-        roofline_rebuild = dict(bound="hbm", kernel=f"kc_cert_grid_rebuild (A2 + A3: build kernels + {'search_leaf_kernel' if d == 3 else 'search_tiled_kernel'})",
+        roofline_rebuild = dict(bound="hbm", kernel=f"kc_cert_grid_rebuild (A2 + A3: build kernels + {'search_leaf_kernel + ball_finish_kernel' if d == 3 else 'search_tiled_kernel'})",
                                 achieved=reb_gbs, peak=hbm, unit="GB/s", frac=reb_gbs / hbm,
                                 traffic=NCU_TRAFFIC_BYTES.get((cfg, "rebuild")),
                                 note=(f"{REBUILD_BYTES_PER_POINT[d]:.0f} algorithmic B/point (SURVEY.md §8(d)) x {N} points / "
