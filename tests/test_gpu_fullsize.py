@@ -60,6 +60,17 @@ def test_config5_rebuild_and_repair_4m(cfg, density):
     H, m, C = kc.kc_frontier_entropy(grid, F, nF)
     wH, wm, wC = oracle.entropy(oracle.cell_ids(q, g_or), wF, g_or.n_cells)
     assert abs(float(H.item()) - wH) <= 1e-6 and int(m.item()) == wm and int(C.item()) == wC
+    # thin frontiers on the grid resident at q (4 M points: d = 3 sweeps from N/32 on, d = 2 from N/4 on, so
+    # these two sizes take the list kernels in the plane and the compacting sweep in space)
+    rng = np.random.default_rng(17)
+    for f in (0.04, 0.15):
+        ids = np.sort(rng.choice(N, int(N * f), replace=False)).astype(np.int32)
+        out = kc.Certs.empty(N, "cuda")
+        out.nn.fill_(-7)
+        kc.kc_frontier_search(grid, Q, dev(ids), dev(np.array([ids.size], np.int32)), out)
+        assert_same(out, post, idx=ids, what=f"{cfg} frontier of {f:.0%}")
+        torch.cuda.synchronize()
+        assert np.array_equal(np.flatnonzero(out.nn.cpu().numpy() != -7), ids)
 
 
 @pytest.mark.parametrize("d", [2, 3])
