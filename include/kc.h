@@ -334,9 +334,9 @@ kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF, i
  *          moved.  Movers keep their slot if their cell (and, in a subdivided cell, their
  *          sub-cell) is unchanged; otherwise they are tombstoned and re-filed into their new
  *          cell's overflow chain (line 3).  On a grid of >= 100,000 points an update whose
- *          host-side bound allows at least N/8 movers (n_movers_max, or N for NULL) re-bins the
- *          whole grid at p_new instead (A2, O(N)): cheaper than re-filing that many points one by
- *          one, and the search that follows runs on a fresh grid.
+ *          host-side bound allows at least N/8 (d = 2) or N/32 (d = 3) movers (n_movers_max, or N
+ *          for NULL) re-bins the whole grid at p_new instead (A2, O(N)): cheaper than re-filing that
+ *          many points one by one, and the search that follows runs on a fresh grid.
  *  F, nF, nF_max: as for kc_frontier_entropy; the queries to recompute (lines 4-7).
  *  nn, nn2, d1, d2, c: certificates, updated IN PLACE at the ids in F, untouched elsewhere.
  * The search is the same unbounded ring search as A3, over sorted ranges and chains. */
