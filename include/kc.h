@@ -334,7 +334,7 @@ kc_status kc_frontier_entropy(kc_grid *g, const int32_t *F, const int32_t *nF, i
  *          moved.  Movers keep their slot if their cell (and, in a subdivided cell, their
  *          sub-cell) is unchanged; otherwise they are tombstoned and re-filed into their new
  *          cell's overflow chain (line 3).  On a grid of >= 100,000 points an update whose
- *          host-side bound allows at least N/8 (d = 2) or N/32 (d = 3) movers (n_movers_max, or N
+ *          host-side bound allows at least N/8 movers (d = 3, N >= 2^20: N/32) (n_movers_max, or N
  *          for NULL) re-bins the whole grid at p_new instead (A2, O(N)): cheaper than re-filing that
  *          many points one by one, and the search that follows runs on a fresh grid.
  *  F, nF, nF_max: as for kc_frontier_entropy; the queries to recompute (lines 4-7).
@@ -362,7 +362,9 @@ kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t N, const in
  * therefore frozen in a captured graph: the kernel variant chosen from N, nF_max and n_movers_max
  * (host-side bounds), whether kc_grid_update re-bins, and the grid's built / updated state, which
  * must be the same at every replay as at capture (capture a whole step, including the build or the
- * update that precedes a search, as paper_2606_18314_b200/driver.py does). */
+ * update that precedes a search, as paper_2606_18314_b200/driver.py does).  Work lists that a call
+ * fills on the device (the sweep marks, the hand-off list, the list of the d = 3 search's second
+ * kernel, the scans' descriptors) are emptied or reset by that call's own kernels. */
 
 /* ---- NEXT #4: K-list certificates ---------------------------------------------------------- */
 /* "Richer geometric certificates (Delaunay edges, k-nearest-neighbour graphs, ...) are left open"

@@ -27,9 +27,10 @@ namespace {
 constexpr int MHIST = 4096;   // frontier-count histogram bins held exactly; larger counts go to `big`
 constexpr int SCAN_CHUNK = 2048;   // entries per scan block (256 threads x 8)
 // A6: when an update re-bins instead of re-filing: grids of >= REBIN_MIN_N points, host-side bound of at least
-// N / 8 movers (d = 2) or N / 32 (d = 3, where chain residents are served one thread per query and a fresh
-// grid lets the slot sweep take them: 10 % movers of 4,194,304 clustered points 1.15 -> 0.7 ms).
-constexpr int64_t REBIN_MIN_N = 100000, REBIN_DIV2 = 8, REBIN_DIV3 = 32;
+// N / 8 movers (d = 2) or N / list_div3(N) (d = 3: N / 8 on small grids, N / 32 from a million points on, where
+// chain residents would be served one thread per query and a fresh grid lets the slot sweep take them:
+// 10 % movers of 4,194,304 clustered points 1.15 -> 0.68 ms).
+constexpr int64_t REBIN_MIN_N = 100000, REBIN_DIV2 = 8;
 
 // ------------------------------------------------------------------ A2 build
 // A counting sort in two levels.  (1) prep: drop the chains of the previous residency, zero the
@@ -829,7 +830,7 @@ extern "C" kc_status kc_grid_update(kc_grid *g, const float *p_new, int64_t N, c
     // re-filing them one by one -- cheaper than the refresh pass itself, no tombstones, no chains,
     // and the frontier search that follows runs on a fresh grid.  (Decided from the host-side bounds.)
     const int64_t nm = movers ? n_movers_max : N;
-    if (N >= REBIN_MIN_N && nm * (g->geom.d == 2 ? REBIN_DIV2 : REBIN_DIV3) >= N) return kc_grid_build(g, p_new, N, stream);
+    if (N >= REBIN_MIN_N && nm * (g->geom.d == 2 ? REBIN_DIV2 : (int64_t)list_div3(N)) >= N) return kc_grid_build(g, p_new, N, stream);
     cudaStream_t st = (cudaStream_t)stream;
     View v = make_view(g);
     const int n = (int)N;

@@ -182,6 +182,17 @@ __device__ __forceinline__ int cell_of(const View &v, float x, float y, float z)
     return (kz * v.G1 + ky) * v.G0 + kx;
 }
 
+// d = 3: the fraction 1 / div of the points from which a frontier list goes to the slot sweep (kc_search.cu)
+// and an update re-bins the grid (kc_grid.cu): lists of up to WPQ_MAX ids get one WARP per query, which wins
+// on small grids; beyond that one THREAD per query is slow on clustered cells and the sweep on a fresh grid
+// wins down to N / 32 (measured on config 5 and config 4, DESIGN.md section 5 A7).
+constexpr int WPQ_MAX = 32768;                       // A7: id lists up to this long get one warp per query
+inline int list_div3(int64_t N)
+{
+    const int64_t d = N / WPQ_MAX;
+    return (int)(d < 8 ? 8 : (d > 32 ? 32 : d));
+}
+
 inline int blocks_for(int64_t n, int threads, int cap = 148 * 16)
 {
     int64_t b = (n + threads - 1) / threads;

@@ -796,8 +796,7 @@ constexpr int LT_WARPS = 4;
 // d = 2: the list kernels win up to a quarter of the points (12.5 %: 0.26 vs 0.43 ms; 30 %: 0.53 vs 0.48);
 // d = 3: one thread per query on clustered cells is slow (10 %: 0.96 ms, the sweep 0.44), so the sweep takes
 // over as soon as the list is too long for one WARP per query (WPQ_MAX), down to N / 32 (3 %: 0.37 vs 0.37).
-constexpr int SWEEP_MIN_N = 200000, SWEEP_DIV2 = 4, SWEEP_DIV3_MIN = 8, SWEEP_DIV3_MAX = 32;
-constexpr int WPQ_MAX = 32768;                       // A7: id lists up to this long get one warp per query
+constexpr int SWEEP_MIN_N = 200000, SWEEP_DIV2 = 4;   // (d = 3: list_div3, kc_grid.cuh)
 #ifndef LT_MIN_BLOCKS
 #define LT_MIN_BLOCKS 8
 #endif
@@ -1871,8 +1870,7 @@ extern "C" kc_status kc_frontier_search(kc_grid *g, const float *p_new, int64_t 
     const int n = (int)N;
     // slot sweep: grids of at least SWEEP_MIN_N points, frontier of at least N / div points
     // (the host bound decides whether the sweep kernels are launched, the device count whether they run)
-    const int div = g->geom.d == 2 ? SWEEP_DIV2
-                                   : (int)std::min<int64_t>(SWEEP_DIV3_MAX, std::max<int64_t>(SWEEP_DIV3_MIN, N / WPQ_MAX));
+    const int div = g->geom.d == 2 ? SWEEP_DIV2 : list_div3(N);
     const int sweep_div = N >= SWEEP_MIN_N && nF_max * (int64_t)div >= N ? div : 0;
     if (sweep_div > 0) {
         mark_frontier_kernel<<<blocks_for(nF_max, 256, 148 * 8), 256, 0, st>>>(F, nF, n, sweep_div, g->slot, g->mark, g->list2, g->ctr);

@@ -87,7 +87,7 @@ def test_sweep_through_the_second_kernel(frac, updated):
     rng = np.random.default_rng(int(frac * 10) + updated)
     q = p.copy()
     if updated:
-        movers = np.sort(rng.choice(N, N // 40, replace=False)).astype(np.int32)     # < N/32: re-filed one by one
+        movers = np.sort(rng.choice(N, N // 40, replace=False)).astype(np.int32)     # below the re-bin bound: re-filed one by one
         q[movers] += rng.uniform(-3e-4, 3e-4, (movers.size, 3)).astype(np.float32)
     else:
         movers = np.zeros(0, np.int32)
