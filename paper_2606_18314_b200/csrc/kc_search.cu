@@ -88,15 +88,6 @@ __device__ __forceinline__ void scan_chain(const View &v, int cidx, float qx, fl
         offer_once(best, s, e, self);
     }
 }
-template <int D>
-__device__ __forceinline__ void scan_row(const View &v, bool chains, int rowbase, int x0, int x1,
-                                         float qx, float qy, float qz, int self, Top2 &best)
-{
-    int b = v.cell_start[rowbase + x0], e = v.cell_start[rowbase + x1 + 1];
-    scan_range<D>(v, b, e, qx, qy, qz, self, best);
-    if (chains)
-        for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
-}
 
 __device__ __forceinline__ float face_at(float lo, int k, float h)
 {
@@ -286,11 +277,44 @@ __device__ __forceinline__ void visit_row(const View &v, bool chains, int rowbas
         for (int x = x0; x <= x1; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
 }
 
+// Squared lower bound (R7's face bound: slack, shrink) of the axis distance from the query coordinate q in
+// cell c to anything filed in cell k of that axis.
+__device__ __forceinline__ float axis_gap2(const View &v, float q, float lo, float slk, int k, int c)
+{
+    if (k == c) return 0.0f;
+    const float g = k > c ? __fsub_rn(face_at(lo, k, v.h), q) : __fsub_rn(q, face_at(lo, k + 1, v.h));
+    const float t = gap_lb(v, g, slk);
+    return __fmul_rn(t, t);
+}
+// Cells xa..xb of one row of a ring.  A sparse row (the usual case: rings are for isolated queries) is one
+// range; a row that holds many records -- the ring of a sparse point beside a dense cluster contains the
+// cluster's core -- goes cell by cell, each tested against the current bound (rowgap2 = squared lower bound
+// of the row's distance in y and z), subdivided cells through visit_heavy.
+constexpr int RING_ROW_DENSE = 64;
+template <int D, bool PRUNE>
+__device__ __forceinline__ void ring_cells(const View &v, bool chains, int rowbase, int y, int z, int xa, int xb,
+                                           float rowgap2, float qx, float qy, float qz, int self, int cx, Top2 &best)
+{
+    const int32_t *cs = v.cell_start + rowbase;
+    const int b = cs[xa], e = cs[xb + 1];
+    if (!PRUNE || e - b <= RING_ROW_DENSE) {
+        scan_range<D>(v, b, e, qx, qy, qz, self, best);
+    } else {
+        for (int x = xa; x <= xb; ++x) {
+            if (best.s2 < __fadd_rn(rowgap2, axis_gap2(v, qx, v.lo0, v.slk0, x, cx))) continue;
+            const int cb = cs[x], ce = cs[x + 1];
+            if (ce > cb) visit_cell<D>(v, rowbase + x, x, y, z, cb, ce, qx, qy, qz, self, best);
+        }
+    }
+    if (chains)
+        for (int x = xa; x <= xb; ++x) scan_chain<D>(v, rowbase + x, qx, qy, qz, self, best);
+}
+
 // Chebyshev rings r = 2, 3, ... around the query's own cell, entered with the radius-1 block
 // already done; leaves as soon as the bound of the scanned block allows it.  (Rare path: kept out
 // of line, state passed by value.)
 struct RingOut { Top2 best; int r; };
-template <int D>
+template <int D, bool PRUNE>
 __device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float qx, float qy, float qz,
                                               int self, int cx, int cy, int cz, Top2 best, bool warp_wide)
 {
@@ -319,24 +343,33 @@ __device__ __noinline__ RingOut ring_continue(const View &v, bool chains, float 
         z0 = D == 3 ? max(cz - r, 0) : 0; z1 = D == 3 ? min(cz + r, v.G2 - 1) : 0;
         y0 = max(cy - r, 0); y1 = min(cy + r, v.G1 - 1);
         x0 = max(cx - r, 0); x1 = min(cx + r, v.G0 - 1);
-        for (int z = z0; z <= z1; ++z)
+        // PRUNE (the list kernels of A7): rows and, in rows that hold many records, cells are tested against
+        // the current bound -- the ring of a sparse query beside a dense cluster contains the cluster's core.
+        // The whole-set kernels keep the plain form: their ring queries hide behind the other warps, and the
+        // longer code measured 13 % on the whole kernel (register allocation of the caller).
+        for (int z = z0; z <= z1; ++z) {
+            const float gz = PRUNE && D == 3 ? axis_gap2(v, qz, v.lo2, v.slk2, z, cz) : 0.0f;
+            if (PRUNE && best.s2 < gz) continue;                 // (strict: nothing behind that face can enter)
             for (int y = y0; y <= y1; ++y) {
+                const float gy = PRUNE ? __fadd_rn(gz, axis_gap2(v, qy, v.lo1, v.slk1, y, cy)) : 0.0f;
+                if (PRUNE && best.s2 < gy) continue;
                 int rowbase = (z * v.G1 + y) * v.G0;
                 bool shell = (D == 3 && (z == cz - r || z == cz + r)) || y == cy - r || y == cy + r;
                 if (shell) {
-                    scan_row<D>(v, chains, rowbase, x0, x1, qx, qy, qz, self, best);
+                    ring_cells<D, PRUNE>(v, chains, rowbase, y, z, x0, x1, gy, qx, qy, qz, self, cx, best);
                 } else {
-                    if (cx - r >= 0) scan_row<D>(v, chains, rowbase, cx - r, cx - r, qx, qy, qz, self, best);
-                    if (cx + r <= v.G0 - 1) scan_row<D>(v, chains, rowbase, cx + r, cx + r, qx, qy, qz, self, best);
+                    if (cx - r >= 0) ring_cells<D, PRUNE>(v, chains, rowbase, y, z, cx - r, cx - r, gy, qx, qy, qz, self, cx, best);
+                    if (cx + r <= v.G0 - 1) ring_cells<D, PRUNE>(v, chains, rowbase, y, z, cx + r, cx + r, gy, qx, qy, qz, self, cx, best);
                 }
             }
+        }
     }
     RingOut o;
     o.best = best; o.r = r;
     return o;
 }
 // final check of the radius-1 block, then wider rings if the bound requires them
-template <int D>
+template <int D, bool PRUNE = false>
 __device__ __forceinline__ int finish_block(const View &v, bool chains, float qx, float qy, float qz, int self,
                                             int cx, int cy, int cz, Top2 &best, bool warp_wide = false)
 {
@@ -344,14 +377,14 @@ __device__ __forceinline__ int finish_block(const View &v, bool chains, float qx
     const int y0 = max(cy - 1, 0), y1 = min(cy + 1, v.G1 - 1);
     const int x0 = max(cx - 1, 0), x1 = min(cx + 1, v.G0 - 1);
     if (bound_ok(box_bound<D>(v, qx, qy, qz, x0, x1, y0, y1, z0, z1), best.s2)) return 1;
-    const RingOut o = ring_continue<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best, warp_wide);
+    const RingOut o = ring_continue<D, PRUNE>(v, chains, qx, qy, qz, self, cx, cy, cz, best, warp_wide);
     best = o.best;
     return o.r;
 }
 
 // One thread per query, straight from global memory (A7, and A3's comparison variant): own
 // cell, row neighbours, other rows nearest first, every cell subject to pruning; then rings.
-template <int D>
+template <int D, bool PRUNE = false>
 __device__ int block_search(const View &v, bool chains, float qx, float qy, float qz, int self,
                             int cx, int cy, int cz, Top2 &best)
 {
@@ -383,7 +416,7 @@ __device__ int block_search(const View &v, bool chains, float qx, float qy, floa
         if (cx < v.G0 - 1 && !(best.s2 < __fadd_rn(rb2, g.xp))) x1 = cx + 1;
         visit_row<D>(v, chains, (z * v.G1 + y) * v.G0, y, z, x0, x1, qx, qy, qz, self, best);
     }
-    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
+    return finish_block<D, PRUNE>(v, chains, qx, qy, qz, self, cx, cy, cz, best);
 }
 
 // ---- A3 / A7, phased -------------------------------------------------------------------------
@@ -895,15 +928,6 @@ __device__ __forceinline__ int ball_state(const View &v, const Qry &q, const Top
             return BALL_DONE;      // (on an updated grid the caller still scans the own cell's chain)
     }
     return BALL_MORE;
-}
-// Squared lower bound (R7's face bound: slack, shrink) of the axis distance from the query coordinate q in
-// cell c to anything filed in cell k of that axis.
-__device__ __forceinline__ float axis_gap2(const View &v, float q, float lo, float slk, int k, int c)
-{
-    if (k == c) return 0.0f;
-    const float g = k > c ? __fsub_rn(face_at(lo, k, v.h), q) : __fsub_rn(q, face_at(lo, k + 1, v.h));
-    const float t = gap_lb(v, g, slk);
-    return __fmul_rn(t, t);
 }
 // A query whose ball box holds more than a lane's queue may hold (a sparse point beside a dense cluster:
 // most of the box lies outside the ball): the cells of the box one by one, each row and cell tested
@@ -1431,7 +1455,7 @@ __device__ int wpq_search(const View &v, bool chains, int lane, float qx, float 
     if (ja != KC_NOIDX) best.offer(sa, ja);
     if (jb != KC_NOIDX) best.offer(sb, jb);
     // every lane holds the same state: the rare ring continuation runs redundantly on all of them
-    return finish_block<D>(v, chains, qx, qy, qz, self, cx, cy, cz, best, true);
+    return finish_block<D, true>(v, chains, qx, qy, qz, self, cx, cy, cz, best, true);
 }
 
 // The list kernel is the last reader of list2 (the chain residents of a swept frontier): the block
@@ -1474,7 +1498,7 @@ search_wpq_kernel(View v, const float *__restrict__ p_new, int N, const int32_t 
             const int cx = cell_axis(qx, v.lo0, v.inv_h, v.G0);
             const int cy = cell_axis(qy, v.lo1, v.inv_h, v.G1);
             const int cz = D == 3 ? cell_axis(qz, v.lo2, v.inv_h, v.G2) : 0;
-            const int r = block_search<D>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
+            const int r = block_search<D, true>(v, chains, qx, qy, qz, i, cx, cy, cz, best);
             if (r > 2) atomicAdd(&ctr->n_stragglers, 1);
             store_cert(best, i, nn, nn2, d1, d2, c);
         }
