@@ -37,13 +37,13 @@ N_ALLPAIRS = 1 << 20            # config 5: the all-pairs oracle pass runs on th
 # ncu --set full captures (profiles/, file named beside each figure); None where no capture exists
 NCU_TRAFFIC_BYTES = {
     ("cfg2", "allpairs_kernel"): 279552,            # profiles/r1f_allpairs_cfg2_full.txt
-    ("cfg5_d3", "allpairs_kernel"): 164840704,      # profiles/r2_allpairs_1m_cfg5_d3_full.txt (87.3 MB read + 77.6 MB written)
-    ("cfg5_d2", "allpairs_kernel"): 143417856,      # profiles/r2_allpairs_1m_cfg5_d2_full.txt (71.3 + 72.2 MB)
+    ("cfg5_d3", "allpairs_kernel"): 165806848,      # profiles/r2_allpairs_1m_cfg5_d3_full.txt (read + written)
+    ("cfg5_d2", "allpairs_kernel"): 145646592,      # profiles/r2_allpairs_1m_cfg5_d2_full.txt
     # A2 + A3, summed over the kernels of one kc_cert_grid_rebuild call (build_prep, cellid_hist, scan_cells,
     # leafid_hist, lscan, scatter, search_leaf + ball_finish / search_tiled): profiles/r2_grid_cfg5_d3_full.txt
-    # (591 MB read + 387 MB written) / r2_grid_cfg5_d2_full.txt (413 + 647 MB)
+    # (591 MB read + 387 MB written) / r2_grid_cfg5_d2_full.txt (420 + 663 MB)
     ("cfg5_d3", "rebuild"): 978100000,
-    ("cfg5_d2", "rebuild"): 1060200000,
+    ("cfg5_d2", "rebuild"): 1082500000,
 }
 # algorithmic bytes per point of the O(N) rebuild (A2 + A3) with this layout
 REBUILD_BYTES_PER_POINT = {2: 76.0, 3: 90.0}
